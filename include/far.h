@@ -1,0 +1,182 @@
+/*
+ * far.h -- C ABI of the B200-native FAR-LIO front-end hot path (voxel hashmap + sparsity-aware GICP).
+ *
+ * Source of the method: /root/reference/PAPER.md (FAR-LIO, arxiv/paper_2606_26010), cited below as
+ * PAPER.md:<line>.  Readings of passages the paper leaves open are numbered R1..R14 in DESIGN.md.
+ * Every entry point below runs hand-written CUDA kernels for sm_100a; there is no CPU fallback.
+ *
+ * Conventions
+ *  - Every function returns an int status (FAR_OK = 0).  No exception crosses the ABI.
+ *  - Pointers named d_* and all bulk arrays (points, ids, covariances, result structs) are DEVICE pointers
+ *    (or any device-accessible pointer such as pinned mapped host memory) owned by the caller; the library
+ *    never frees, reallocates or retains them beyond the call's stream order.
+ *  - Small POD inputs (far_map_config_t, far_pose_t, far_gicp_options_t, prune centre) are HOST pointers,
+ *    read during the call.  The *_dev variants read a pose from a DEVICE pointer in stream order, so a frame
+ *    pipeline (register -> insert -> prune) needs no host synchronisation.
+ *  - `stream` is a cudaStream_t passed as void*.  Calls enqueue work and return; nothing synchronises
+ *    unless stated.  The map handle owns all of its device memory, allocated once in far_map_create
+ *    (preallocate; allocation spikes show up as latency peaks).
+ *  - Points are fp32, `stride` floats apart (3 or 4).  Non-finite points and points whose voxel index leaves
+ *    +-2^20 are skipped and counted as invalid.  Poses are map_from_sensor, R row-major, FP64.
+ *  - A map handle is not thread-safe; calls on one map must be issued in one stream order.
+ */
+#ifndef FAR_H
+#define FAR_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    FAR_OK = 0,
+    FAR_ERR_ARG = 1,        /* null pointer, bad stride/size/config */
+    FAR_ERR_CUDA = 2,       /* a CUDA runtime call failed (see far_last_cuda_error) */
+    FAR_ERR_FULL = 3,       /* table occupancy limit reached: excess NEW voxels are dropped and counted */
+    FAR_ERR_RANGE = 4,      /* id counter would exceed 2^32-2 */
+    FAR_ERR_DEGENERATE = 5  /* fewer than 6 inliers or H not positive definite; pose returned = init pose */
+};
+
+enum { FAR_KERNEL_CAUCHY = 0, FAR_KERNEL_GEMAN_MCCLURE = 1, FAR_KERNEL_NONE = 2 };
+
+#define FAR_NO_ID 0xFFFFFFFFu
+
+typedef struct { double R[9]; double t[3]; } far_pose_t;
+
+typedef struct {
+    float voxel_size;      /* v > 0 [m]                      PAPER.md:62,68 (paper: 4 m)                  */
+    int32_t cap;           /* max points per voxel, 1..64    PAPER.md:62,68 (paper: N_max = 40)           */
+    int64_t max_voxels;    /* live + pruned voxel keys the table must hold                                */
+    float max_load;        /* table load limit in (0,1); 0 -> 0.5; slots = pow2 >= max_voxels / max_load   */
+    int32_t with_cov;      /* 1: allocate per-point covariance storage (needed for GICP targets)           */
+    int32_t k_cov;         /* neighbours for Eq. 1; 0 -> 10                                   */
+    double cov_eps;        /* regulariser of Eq. 1; 0 -> 1e-3                                 */
+    int64_t max_batch;     /* points per internal insert pass; 0 -> 1<<20.  Larger calls are chunked      */
+} far_map_config_t;
+
+typedef struct { int64_t n_offered, n_accepted, n_new_voxels, n_dropped_full, n_invalid; } far_insert_stats_t;
+typedef struct { int64_t n_voxels_removed, n_points_removed, n_voxels_left, n_points_left; } far_prune_stats_t;
+typedef struct { int64_t n_voxels, n_points, n_dead_keys, n_slots; uint64_t next_id; } far_map_stats_t;
+
+typedef struct {
+    int32_t kernel;      /* FAR_KERNEL_*; Cauchy is the paper's (Eq. 5)       */
+    double conv_eps;     /* stop when ||delta||_2 <= conv_eps (5e-3; R13)       */
+    double tau_mult;     /* correspondence gate tau = tau_mult * sigma  (R10: 3)              */
+    double kappa_div;    /* kernel scale kappa = sigma / kappa_div      (R10: 3)              */
+} far_gicp_options_t;
+
+typedef struct {
+    far_pose_t pose;     /* registered pose (init pose if status == FAR_ERR_DEGENERATE)                 */
+    double H[36];        /* row-major 6x6, order (rho_x,rho_y,rho_z,phi_x,phi_y,phi_z), of the LAST      */
+    double b[6];         /*   linearisation performed (at the pose before the final update)              */
+    double chi2;         /* sum w * d^T M d of that linearisation                                        */
+    int32_t n_inliers, iters, converged, status;
+} far_gicp_result_t;
+
+typedef struct far_map far_map_t;
+typedef struct far_threshold far_threshold_t;
+
+const char* far_strerror(int status);
+/* text of the last CUDA error seen by this library in the calling process ("" if none) */
+const char* far_last_cuda_error(void);
+void far_gicp_default_options(far_gicp_options_t* out);
+
+/* ---- voxel hashmap: PAPER.md:62-68 (cuVoxelMap, Fig. 3), :109 (local submap) -------------------------
+ * Open addressing with linear probing on packed 64-bit voxel keys (R1: k = floor(fp32 p / fp32 v), three
+ * 21-bit biased indices), one fixed bucket of `cap` float4 (x,y,z,id bits) per table slot.
+ * far_map_create allocates and initialises all device memory on the current device and synchronises. */
+int far_map_create(far_map_t** out, const far_map_config_t* cfg);
+int far_map_destroy(far_map_t* map);
+/* empties the map and resets the id counter to 0 */
+int far_map_clear(far_map_t* map, void* stream);
+
+/* A3/A4 (PAPER.md:62 "fixed, maximum number N_max of points", :109; R3/R4): offers n points.  Point i gets
+ * id = next_id + i (next_id advances by n regardless of acceptance).  With a pose the point is first moved in
+ * FP64 (fixed operation order, rounded once to fp32).  Result is that of inserting the points one by one in
+ * index order: a voxel keeps the lowest ids up to `cap`, in ascending id; batch-invariant and deterministic.
+ * compute_cov != 0 (map created with_cov): the covariance (Eq. 1) of every ACCEPTED point is computed against
+ * the map after the insert; points already stored keep theirs.
+ * d_stats (nullable, device) is overwritten with the totals of this call.
+ * Returns FAR_ERR_RANGE (nothing inserted) if next_id + n > 2^32-1.  Table-full is reported through
+ * d_stats->n_dropped_full and the sticky flag of far_map_stats (this call itself does not synchronise). */
+int far_map_insert(far_map_t* map, const float* d_xyz, int64_t n, int stride, const far_pose_t* pose_or_null,
+                   int compute_cov, far_insert_stats_t* d_stats, void* stream);
+int far_map_insert_dev(far_map_t* map, const float* d_xyz, int64_t n, int stride, const far_pose_t* d_pose,
+                       int compute_cov, far_insert_stats_t* d_stats, void* stream);
+
+/* A5 ("voxels whose distance to the current pose exceeds a certain limit are removed"; R5):
+ * removes voxel k iff |(k + 0.5) v - c|^2 > radius^2 (FP64, strict).  centre: HOST double[3]. */
+int far_map_prune(far_map_t* map, const double center[3], double radius, far_prune_stats_t* d_stats, void* stream);
+/* same, centre = d_pose->t read on the device in stream order */
+int far_map_prune_dev(far_map_t* map, const far_pose_t* d_pose, double radius, far_prune_stats_t* d_stats,
+                      void* stream);
+
+/* counts live voxels / stored points / dead (pruned) keys; next_id is the host-side counter at call time */
+int far_map_stats(far_map_t* map, far_map_stats_t* d_stats, void* stream);
+/* Re-hashes the live voxels into a clean table, dropping the keys of pruned voxels (they otherwise stay as
+ * dead keys that lengthen probe sequences).  Uses the map's second table buffer; contents unchanged. */
+int far_map_rehash(far_map_t* map, void* stream);
+
+/* Writes the live voxels in unspecified order: keys[v], counts[v], points4[(v*cap + j)*4 + {0,1,2,3}] =
+ * x,y,z,id bits (unused entries 0,0,0,FAR_NO_ID), cov6[(v*cap + j)*6] (xx,xy,xz,yy,yz,zz; nullable),
+ * cov_valid[v*cap + j] (nullable).  At most max_out voxels are written; *d_n_voxels = number of live voxels. */
+int far_map_export(far_map_t* map, uint64_t* d_keys, int32_t* d_counts, float* d_points4, float* d_cov6,
+                   uint8_t* d_cov_valid, int64_t max_out, int64_t* d_n_voxels, void* stream);
+
+/* A1: keys[i] = packed voxel key of point i, ~0 if invalid */
+int far_voxel_keys(const float* d_xyz, int64_t n, int stride, float voxel, uint64_t* d_keys, void* stream);
+
+/* A6 ("the voxel containing it as well as all surrounding ones (27 in total)", :80 "closest
+ * Euclidean neighbor"; R6): nearest stored point among the 27 voxels around each query by (d^2, id)
+ * lexicographic order, d^2 evaluated in FP64 with fixed operation order.  d_id[i] = FAR_NO_ID and
+ * d_d2[i] = +inf if no candidate.  d_d2 is the FP64 value rounded to fp32. */
+int far_map_nn(const far_map_t* map, const float* d_q, int64_t m, int stride, uint32_t* d_id, float* d_d2,
+               void* stream);
+
+/* A7 (Eq. 1; R7/R8): covariance from the k_cov nearest stored points of each query:
+ * Sigma_hat (1/k, about the mean), C = Sigma_hat + eps I, Sigma = ||C^-1||_F C.  Fewer than k_cov candidates:
+ * valid = 0 and cov6 = identity.  cov6: m*6 fp32 (xx,xy,xz,yy,yz,zz). */
+int far_map_knn_cov(const far_map_t* map, const float* d_q, int64_t m, int stride, float* d_cov6,
+                    uint8_t* d_valid, void* stream);
+
+/* A2 ("preprocessing (typically ... deskewing and downsampling)"; R2): one representative per
+ * occupied voxel of the scan = the lowest-index valid point, emitted in ascending source index.
+ * d_out_xyz: n*3 fp32, d_out_index: n int32, *d_n_out: count.  Call with d_workspace == NULL to get the
+ * required workspace size in *workspace_bytes; otherwise *workspace_bytes is the size provided. */
+int far_voxelize(const float* d_xyz, int64_t n, int stride, float voxel, float* d_out_xyz, int32_t* d_out_index,
+                 int64_t* d_n_out, void* d_workspace, size_t* workspace_bytes, void* stream);
+
+/* A8-A10 (Eq. 2-6; R9-R14).  scan: n source points in the sensor frame with their covariances
+ * (d_scan_cov6 n*6 fp32, d_scan_valid n bytes; both nullable = all invalid -> point-to-point).
+ * sigma is the adaptive threshold of [1]: gate tau = tau_mult*sigma, kappa = sigma/kappa_div.
+ * linearize: one pass at `pose` -> H, b, chi2, n_inliers (pose copied to out, iters = 1).
+ * register: Gauss-Newton, T <- Exp(delta) T with H delta = -b, until ||delta|| <= conv_eps or max_iters;
+ * the whole loop runs in one cooperative kernel, no host synchronisation inside.  d_out: device-accessible. */
+int far_gicp_linearize(const far_map_t* map, const float* d_scan, const float* d_scan_cov6,
+                       const uint8_t* d_scan_valid, int64_t n, int stride, const far_pose_t* pose, double sigma,
+                       const far_gicp_options_t* opts_or_null, far_gicp_result_t* d_out, void* stream);
+int far_gicp_register(const far_map_t* map, const float* d_scan, const float* d_scan_cov6,
+                      const uint8_t* d_scan_valid, int64_t n, int stride, const far_pose_t* init_pose,
+                      double sigma, int max_iters, const far_gicp_options_t* opts_or_null,
+                      far_gicp_result_t* d_out, void* stream);
+/* same with n and the initial pose read from DEVICE memory in stream order (n <= n_max rows are allocated) */
+int far_gicp_register_dev(const far_map_t* map, const float* d_scan, const float* d_scan_cov6,
+                          const uint8_t* d_scan_valid, const int64_t* d_n, int64_t n_max, int stride,
+                          const far_pose_t* d_init_pose, double sigma, int max_iters,
+                          const far_gicp_options_t* opts_or_null, far_gicp_result_t* d_out, void* stream);
+/* same as far_map_knn_cov with the query count read from DEVICE memory (for chaining after far_voxelize) */
+int far_map_knn_cov_dev(const far_map_t* map, const float* d_q, const int64_t* d_m, int64_t m_max, int stride,
+                        float* d_cov6, uint8_t* d_valid, void* stream);
+
+/* Adaptive threshold of Vizzo et al. [1] as read in R10.  HOST-only FP64 helper (20 lines of
+ * boundary logic, not a kernel): sigma = sqrt(mean delta_i^2) over recorded deviations delta_i > min_motion,
+ * delta = |dt| + 2 max_range sin(theta/2) of pred^-1 * registered; sigma0 until one is recorded. */
+far_threshold_t* far_threshold_create(double sigma0, double min_motion, double max_range);
+void far_threshold_destroy(far_threshold_t*);
+void far_threshold_update(far_threshold_t*, const far_pose_t* predicted, const far_pose_t* registered);
+double far_threshold_sigma(const far_threshold_t*);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,364 @@
+"""paper_2606_26010_b200 -- thin Python binding of libfar.so (the C ABI declared in include/far.h).
+
+Argument marshalling only: every step of the hot path (voxel keys, hashmap insert/prune, 27-voxel nearest
+neighbour, k-NN covariances, GICP linearisation and the Gauss-Newton loop) runs in the hand-written CUDA
+kernels of csrc/.  PyTorch supplies device memory and streams; nothing here computes.  There is no CPU
+fallback: importing works without a GPU (so the ABI can be inspected), every compute call needs one, and a
+missing library raises.
+
+Names follow include/far.h and the paper's notation.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+from . import _build
+
+NO_ID = 0xFFFFFFFF
+KERNEL_CAUCHY, KERNEL_GEMAN_MCCLURE, KERNEL_NONE = 0, 1, 2
+OK, ERR_ARG, ERR_CUDA, ERR_FULL, ERR_RANGE, ERR_DEGENERATE = 0, 1, 2, 3, 4, 5
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfar.so")
+
+
+class Pose(C.Structure):
+    _fields_ = [("R", C.c_double * 9), ("t", C.c_double * 3)]
+
+    @staticmethod
+    def from_rt(T):
+        R, t = T
+        p = Pose()
+        p.R[:] = np.asarray(R, dtype=np.float64).reshape(9).tolist()
+        p.t[:] = np.asarray(t, dtype=np.float64).reshape(3).tolist()
+        return p
+
+    def to_rt(self):
+        return np.array(self.R[:]).reshape(3, 3), np.array(self.t[:])
+
+
+class MapConfig(C.Structure):
+    _fields_ = [("voxel_size", C.c_float), ("cap", C.c_int32), ("max_voxels", C.c_int64), ("max_load", C.c_float),
+                ("with_cov", C.c_int32), ("k_cov", C.c_int32), ("cov_eps", C.c_double), ("max_batch", C.c_int64)]
+
+
+class GicpOptions(C.Structure):
+    _fields_ = [("kernel", C.c_int32), ("conv_eps", C.c_double), ("tau_mult", C.c_double), ("kappa_div", C.c_double)]
+
+
+class GicpResult(C.Structure):
+    _fields_ = [("pose", Pose), ("H", C.c_double * 36), ("b", C.c_double * 6), ("chi2", C.c_double),
+                ("n_inliers", C.c_int32), ("iters", C.c_int32), ("converged", C.c_int32), ("status", C.c_int32)]
+
+
+INSERT_STATS_FIELDS = ("n_offered", "n_accepted", "n_new_voxels", "n_dropped_full", "n_invalid")
+PRUNE_STATS_FIELDS = ("n_voxels_removed", "n_points_removed", "n_voxels_left", "n_points_left")
+MAP_STATS_FIELDS = ("n_voxels", "n_points", "n_dead_keys", "n_slots", "next_id")
+GICP_RESULT_BYTES = C.sizeof(GicpResult)
+POSE_BYTES = C.sizeof(Pose)
+
+_lib = None
+
+
+class FarError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = status
+        msg = lib().far_strerror(status).decode()
+        cuda = lib().far_last_cuda_error().decode()
+        super().__init__(f"{where}: {msg} (status {status})" + (f" [{cuda}]" if status == ERR_CUDA and cuda else ""))
+
+
+def lib():
+    """Load (building if needed) the in-tree libfar.so.  Raises if it cannot be built or loaded."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = C.CDLL(path)
+        vp, i64, i32, f32, f64, ci = C.c_void_p, C.c_int64, C.c_int32, C.c_float, C.c_double, C.c_int
+        sig = {
+            "far_strerror": (C.c_char_p, [ci]),
+            "far_last_cuda_error": (C.c_char_p, []),
+            "far_gicp_default_options": (None, [vp]),
+            "far_map_create": (ci, [vp, vp]),
+            "far_map_destroy": (ci, [vp]),
+            "far_map_clear": (ci, [vp, vp]),
+            "far_map_insert": (ci, [vp, vp, i64, ci, vp, ci, vp, vp]),
+            "far_map_insert_dev": (ci, [vp, vp, i64, ci, vp, ci, vp, vp]),
+            "far_map_prune": (ci, [vp, vp, f64, vp, vp]),
+            "far_map_prune_dev": (ci, [vp, vp, f64, vp, vp]),
+            "far_map_stats": (ci, [vp, vp, vp]),
+            "far_map_rehash": (ci, [vp, vp]),
+            "far_map_export": (ci, [vp, vp, vp, vp, vp, vp, i64, vp, vp]),
+            "far_voxel_keys": (ci, [vp, i64, ci, f32, vp, vp]),
+            "far_map_nn": (ci, [vp, vp, i64, ci, vp, vp, vp]),
+            "far_map_knn_cov": (ci, [vp, vp, i64, ci, vp, vp, vp]),
+            "far_map_knn_cov_dev": (ci, [vp, vp, vp, i64, ci, vp, vp, vp]),
+            "far_voxelize": (ci, [vp, i64, ci, f32, vp, vp, vp, vp, vp, vp]),
+            "far_gicp_linearize": (ci, [vp, vp, vp, vp, i64, ci, vp, f64, vp, vp, vp]),
+            "far_gicp_register": (ci, [vp, vp, vp, vp, i64, ci, vp, f64, ci, vp, vp, vp]),
+            "far_gicp_register_dev": (ci, [vp, vp, vp, vp, vp, i64, ci, vp, f64, ci, vp, vp, vp]),
+            "far_threshold_create": (vp, [f64, f64, f64]),
+            "far_threshold_destroy": (None, [vp]),
+            "far_threshold_update": (None, [vp, vp, vp]),
+            "far_threshold_sigma": (f64, [vp]),
+        }
+        for name, (res, args) in sig.items():
+            fn = getattr(L, name)
+            fn.restype = res
+            fn.argtypes = args
+        L._far_symbols = tuple(sig)
+        _lib = L
+    return _lib
+
+
+def _check(rc, where):
+    if rc != OK:
+        raise FarError(rc, where)
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _ptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else None
+
+
+def _points(x):
+    """Device fp32 (n,3) or (n,4) contiguous tensor -> (tensor, n, stride)."""
+    if not isinstance(x, torch.Tensor):
+        x = torch.as_tensor(np.ascontiguousarray(x, dtype=np.float32))
+    if x.device.type != "cuda":
+        x = x.cuda()
+    if x.dtype != torch.float32 or not x.is_contiguous():
+        x = x.to(torch.float32).contiguous()
+    assert x.dim() == 2 and x.shape[1] in (3, 4), tuple(x.shape)
+    return x, x.shape[0], x.shape[1]
+
+
+def _struct_from_tensor(t, cls):
+    raw = t.cpu().numpy().tobytes()
+    return cls.from_buffer_copy(raw)
+
+
+def default_options(kernel=KERNEL_CAUCHY, conv_eps=5e-3, tau_mult=3.0, kappa_div=3.0):
+    return GicpOptions(kernel, conv_eps, tau_mult, kappa_div)
+
+
+def result_to_dict(res: GicpResult):
+    R, t = res.pose.to_rt()
+    return dict(R=R, t=t, H=np.array(res.H[:]).reshape(6, 6), b=np.array(res.b[:]), chi2=res.chi2,
+                n_inliers=res.n_inliers, iters=res.iters, converged=res.converged, status=res.status)
+
+
+def voxel_keys(xyz, voxel):
+    """far_voxel_keys: packed voxel key per point (uint64 bit pattern in an int64 tensor)."""
+    x, n, s = _points(xyz)
+    keys = torch.empty(n, dtype=torch.int64, device=x.device)
+    _check(lib().far_voxel_keys(_ptr(x), n, s, voxel, _ptr(keys), _stream()), "far_voxel_keys")
+    return keys
+
+
+class Voxelizer:
+    """far_voxelize with a reusable workspace sized for up to n_max points."""
+
+    def __init__(self, n_max, device="cuda"):
+        self.n_max = int(n_max)
+        nbytes = C.c_size_t(0)
+        _check(lib().far_voxelize(None, self.n_max, 3, 1.0, None, None, None, None, C.byref(nbytes), None), "far_voxelize(size)")
+        self.ws = torch.empty(nbytes.value, dtype=torch.uint8, device=device)
+        self.out_xyz = torch.empty((self.n_max, 3), dtype=torch.float32, device=device)
+        self.out_index = torch.empty(self.n_max, dtype=torch.int32, device=device)
+        self.n_out = torch.zeros(1, dtype=torch.int64, device=device)
+
+    def enqueue(self, xyz, voxel):
+        """No host sync: results stay on the device (out_xyz, out_index, n_out)."""
+        x, n, s = _points(xyz)
+        assert n <= self.n_max
+        nbytes = C.c_size_t(self.ws.numel())
+        _check(lib().far_voxelize(_ptr(x), n, s, voxel, _ptr(self.out_xyz), _ptr(self.out_index), _ptr(self.n_out),
+                                  _ptr(self.ws), C.byref(nbytes), _stream()), "far_voxelize")
+
+    def __call__(self, xyz, voxel):
+        self.enqueue(xyz, voxel)
+        m = int(self.n_out.item())
+        return self.out_xyz[:m].clone(), self.out_index[:m].clone()
+
+
+def voxelize(xyz, voxel):
+    x, n, _ = _points(xyz)
+    return Voxelizer(max(n, 1), device=x.device)(x, voxel)
+
+
+class Map:
+    """A far_map_t handle.  All bulk arguments are CUDA tensors (NumPy arrays are uploaded for convenience)."""
+
+    def __init__(self, voxel, cap, max_voxels, with_cov=False, k_cov=10, cov_eps=1e-3, max_load=0.5, max_batch=1 << 20):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2606_26010_b200 needs a CUDA device: there is no CPU fallback")
+        self.voxel, self.cap, self.k_cov, self.with_cov = float(voxel), int(cap), int(k_cov), bool(with_cov)
+        cfg = MapConfig(voxel, cap, int(max_voxels), max_load, int(with_cov), k_cov, cov_eps, int(max_batch))
+        h = C.c_void_p()
+        _check(lib().far_map_create(C.byref(h), C.byref(cfg)), "far_map_create")
+        self._h = h
+        dev = torch.device("cuda", torch.cuda.current_device())
+        self.device = dev
+        self._insert_stats = torch.zeros(5, dtype=torch.int64, device=dev)
+        self._prune_stats = torch.zeros(4, dtype=torch.int64, device=dev)
+        self._map_stats = torch.zeros(5, dtype=torch.int64, device=dev)
+        self._result = torch.zeros(GICP_RESULT_BYTES, dtype=torch.uint8, device=dev)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().far_map_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- map maintenance ---------------------------------------------------------------------------
+    def clear(self):
+        _check(lib().far_map_clear(self._h, _stream()), "far_map_clear")
+
+    def insert_enqueue(self, xyz, pose=None, compute_cov=False, d_pose=None):
+        """far_map_insert / far_map_insert_dev without reading the statistics back (no host sync)."""
+        x, n, s = _points(xyz)
+        if d_pose is not None:
+            rc = lib().far_map_insert_dev(self._h, _ptr(x), n, s, _ptr(d_pose), int(compute_cov), _ptr(self._insert_stats), _stream())
+        else:
+            pp = C.byref(Pose.from_rt(pose)) if pose is not None else None
+            rc = lib().far_map_insert(self._h, _ptr(x), n, s, pp, int(compute_cov), _ptr(self._insert_stats), _stream())
+        _check(rc, "far_map_insert")
+
+    def insert(self, xyz, pose=None, compute_cov=False):
+        self.insert_enqueue(xyz, pose, compute_cov)
+        return dict(zip(INSERT_STATS_FIELDS, self._insert_stats.tolist()))
+
+    def prune_enqueue(self, center=None, radius=0.0, d_pose=None):
+        if d_pose is not None:
+            rc = lib().far_map_prune_dev(self._h, _ptr(d_pose), float(radius), _ptr(self._prune_stats), _stream())
+        else:
+            c = (C.c_double * 3)(*[float(v) for v in center])
+            rc = lib().far_map_prune(self._h, c, float(radius), _ptr(self._prune_stats), _stream())
+        _check(rc, "far_map_prune")
+
+    def prune(self, center, radius):
+        self.prune_enqueue(center, radius)
+        return dict(zip(PRUNE_STATS_FIELDS, self._prune_stats.tolist()))
+
+    def stats(self):
+        _check(lib().far_map_stats(self._h, _ptr(self._map_stats), _stream()), "far_map_stats")
+        return dict(zip(MAP_STATS_FIELDS, self._map_stats.tolist()))
+
+    def size(self):
+        s = self.stats()
+        return s["n_voxels"], s["n_points"], s["next_id"]
+
+    def rehash(self):
+        _check(lib().far_map_rehash(self._h, _stream()), "far_map_rehash")
+
+    def export(self, with_cov=False):
+        """Live voxels sorted by key (the library's order is unspecified; sorting is presentation only)."""
+        nv = self.stats()["n_voxels"]
+        dev = self.device
+        keys = torch.empty(max(nv, 1), dtype=torch.int64, device=dev)
+        counts = torch.empty(max(nv, 1), dtype=torch.int32, device=dev)
+        pts = torch.empty((max(nv, 1), self.cap, 4), dtype=torch.float32, device=dev)
+        cov = torch.empty((max(nv, 1), self.cap, 6), dtype=torch.float32, device=dev) if with_cov else None
+        cv = torch.empty((max(nv, 1), self.cap), dtype=torch.uint8, device=dev) if with_cov else None
+        n_out = torch.zeros(1, dtype=torch.int64, device=dev)
+        _check(lib().far_map_export(self._h, _ptr(keys), _ptr(counts), _ptr(pts), _ptr(cov), _ptr(cv), nv, _ptr(n_out),
+                                    _stream()), "far_map_export")
+        assert int(n_out.item()) == nv
+        k = keys[:nv].cpu().numpy().view(np.uint64)
+        order = np.argsort(k, kind="stable")
+        p = pts[:nv].cpu().numpy()[order]
+        out = dict(keys=k[order], counts=counts[:nv].cpu().numpy()[order], xyz=p[:, :, :3].copy(),
+                   ids=p[:, :, 3].copy().view(np.uint32), cov=None, cov_valid=None)
+        if with_cov:
+            out["cov"] = cov[:nv].cpu().numpy()[order]
+            out["cov_valid"] = cv[:nv].cpu().numpy()[order]
+        return out
+
+    # ---- queries -----------------------------------------------------------------------------------
+    def nn(self, q, out_id=None, out_d2=None):
+        """far_map_nn: (id int32-tensor holding uint32 bit patterns, d2 fp32) on the device."""
+        x, n, s = _points(q)
+        ids = out_id if out_id is not None else torch.empty(n, dtype=torch.int32, device=x.device)
+        d2 = out_d2 if out_d2 is not None else torch.empty(n, dtype=torch.float32, device=x.device)
+        _check(lib().far_map_nn(self._h, _ptr(x), n, s, _ptr(ids), _ptr(d2), _stream()), "far_map_nn")
+        return ids, d2
+
+    def knn_cov(self, q, out_cov=None, out_valid=None, d_m=None):
+        x, n, s = _points(q)
+        cov = out_cov if out_cov is not None else torch.empty((n, 6), dtype=torch.float32, device=x.device)
+        valid = out_valid if out_valid is not None else torch.empty(n, dtype=torch.uint8, device=x.device)
+        if d_m is not None:
+            rc = lib().far_map_knn_cov_dev(self._h, _ptr(x), _ptr(d_m), n, s, _ptr(cov), _ptr(valid), _stream())
+        else:
+            rc = lib().far_map_knn_cov(self._h, _ptr(x), n, s, _ptr(cov), _ptr(valid), _stream())
+        _check(rc, "far_map_knn_cov")
+        return cov, valid
+
+    # ---- GICP --------------------------------------------------------------------------------------
+    def _scan_args(self, scan, cov6, valid):
+        x, n, s = _points(scan)
+        if cov6 is not None and not isinstance(cov6, torch.Tensor):
+            cov6 = torch.as_tensor(np.ascontiguousarray(cov6, dtype=np.float32)).to(x.device)
+        if valid is not None and not isinstance(valid, torch.Tensor):
+            valid = torch.as_tensor(np.ascontiguousarray(valid, dtype=np.uint8)).to(x.device)
+        return x, n, s, cov6, valid
+
+    def gicp_linearize(self, scan, cov6, valid, pose, sigma, opts=None):
+        x, n, s, c, v = self._scan_args(scan, cov6, valid)
+        po = Pose.from_rt(pose)
+        _check(lib().far_gicp_linearize(self._h, _ptr(x), _ptr(c), _ptr(v), n, s, C.byref(po), float(sigma),
+                                        C.byref(opts) if opts is not None else None, _ptr(self._result), _stream()),
+               "far_gicp_linearize")
+        return result_to_dict(_struct_from_tensor(self._result, GicpResult))
+
+    def gicp_register_enqueue(self, scan, cov6, valid, init_pose, sigma, max_iters=30, opts=None, d_n=None, d_init_pose=None,
+                              d_result=None):
+        """far_gicp_register(_dev): enqueue only; the result struct stays on the device (self._result or d_result)."""
+        x, n, s, c, v = self._scan_args(scan, cov6, valid)
+        res = d_result if d_result is not None else self._result
+        o = C.byref(opts) if opts is not None else None
+        if d_n is not None:
+            rc = lib().far_gicp_register_dev(self._h, _ptr(x), _ptr(c), _ptr(v), _ptr(d_n), n, s, _ptr(d_init_pose), float(sigma),
+                                             int(max_iters), o, _ptr(res), _stream())
+        else:
+            po = Pose.from_rt(init_pose)
+            rc = lib().far_gicp_register(self._h, _ptr(x), _ptr(c), _ptr(v), n, s, C.byref(po), float(sigma), int(max_iters),
+                                         o, _ptr(res), _stream())
+        _check(rc, "far_gicp_register")
+        return res
+
+    def gicp_register(self, scan, cov6, valid, init_pose, sigma, max_iters=30, opts=None):
+        res = self.gicp_register_enqueue(scan, cov6, valid, init_pose, sigma, max_iters, opts)
+        return result_to_dict(_struct_from_tensor(res, GicpResult))
+
+
+class AdaptiveThreshold:
+    """far_threshold_*: host-side sigma of the adaptive correspondence threshold."""
+
+    def __init__(self, sigma0=2.0, min_motion=0.1, max_range=100.0):
+        self._h = C.c_void_p(lib().far_threshold_create(sigma0, min_motion, max_range))
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            lib().far_threshold_destroy(self._h)
+            self._h = None
+
+    def update(self, predicted, registered):
+        a, b = Pose.from_rt(predicted), Pose.from_rt(registered)
+        lib().far_threshold_update(self._h, C.byref(a), C.byref(b))
+
+    def sigma(self):
+        return lib().far_threshold_sigma(self._h)

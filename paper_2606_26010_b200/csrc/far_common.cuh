@@ -1,0 +1,199 @@
+// far_common.cuh -- device-side building blocks shared by the far_* kernels (sm_100a).
+//
+// Layout of the voxel hashmap in HBM ("cuVoxelMap"; re-designed for B200):
+//   table   : Entry[slots]            16 B per slot {u64 key, u32 count, u32 pad}; one LDG.128 yields the key
+//                                     AND the number of points, so a lookup is two dependent memory levels
+//                                     (entry -> points), not three.
+//   points  : float4[slots * cap]     bucket of slot s = points[s*cap .. s*cap+cap); .w = id bits.  The bucket
+//                                     index IS the slot index (no indirection, no allocator); unused positions
+//                                     hold id = FAR_NO_ID, which is what the deterministic insert relies on.
+//   cov     : float[slots * cap * 6]  (optional) regularised covariance of each stored point (Eq. 1)
+//   cov_ok  : u8[slots * cap]         (optional) 1 if that covariance is valid (>= k neighbours)
+// A pruned voxel keeps its key with count = 0 ("dead key"): it behaves exactly like an absent voxel for every
+// query and is re-used if the voxel is created again, so inserts never have to reason about tombstones.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/far.h"
+
+namespace far {
+
+constexpr unsigned long long KEY_EMPTY = ~0ull;
+constexpr uint32_t NO_ID = 0xFFFFFFFFu;
+constexpr uint32_t NO_SLOT = 0xFFFFFFFFu;
+constexpr int KEY_BIAS = 1 << 20;
+constexpr unsigned FULL = 0xFFFFFFFFu;
+
+struct __align__(16) Entry {
+    unsigned long long key;
+    uint32_t count;
+    uint32_t pad;
+};
+
+// device counters of one map (all zeroed at create / clear)
+struct Counters {
+    unsigned long long n_keys;        // claimed keys (live + dead)
+    unsigned int n_touched;           // voxels that received a first new point in the current chunk
+    unsigned int n_cov;               // accepted points queued for covariance in the current call
+    unsigned int full_flag;           // sticky: a point was dropped because the table was full
+    unsigned int pad;
+    unsigned long long st_accepted, st_new_voxels, st_dropped_full, st_invalid;   // per-call statistics
+    unsigned long long pr_vox_removed, pr_pts_removed, pr_vox_left, pr_pts_left;  // per-prune statistics
+};
+
+// device view of a map, passed by value to kernels
+struct MapView {
+    Entry* table;
+    float4* points;
+    float* cov;          // nullable
+    uint8_t* cov_ok;     // nullable
+    Counters* ctr;
+    uint32_t mask;       // slots - 1
+    uint32_t slots;
+    int cap;
+    int k_cov;
+    float voxel;
+    double cov_eps;
+    unsigned long long max_keys;
+};
+
+struct Pose {
+    double R[9];
+    double t[3];
+};
+
+// ---- A1: voxel key (R1).  One IEEE fp32 division, floor, 21-bit biased pack. -------------
+__device__ __forceinline__ bool voxel_index(float x, float y, float z, float v, int k[3]) {
+    if (!(isfinite(x) && isfinite(y) && isfinite(z))) return false;
+    const float fx = floorf(__fdiv_rn(x, v));
+    const float fy = floorf(__fdiv_rn(y, v));
+    const float fz = floorf(__fdiv_rn(z, v));
+    const bool ok = (fx >= -1048576.0f && fx < 1048576.0f) && (fy >= -1048576.0f && fy < 1048576.0f) &&
+                    (fz >= -1048576.0f && fz < 1048576.0f);
+    if (!ok) return false;
+    k[0] = (int)fx; k[1] = (int)fy; k[2] = (int)fz;
+    return true;
+}
+
+__device__ __forceinline__ unsigned long long pack_key(int kx, int ky, int kz) {
+    return ((unsigned long long)(uint32_t)(kx + KEY_BIAS) << 42) | ((unsigned long long)(uint32_t)(ky + KEY_BIAS) << 21) |
+           (unsigned long long)(uint32_t)(kz + KEY_BIAS);
+}
+
+__device__ __forceinline__ void unpack_key(unsigned long long key, int k[3]) {
+    k[0] = (int)((key >> 42) & 0x1FFFFF) - KEY_BIAS;
+    k[1] = (int)((key >> 21) & 0x1FFFFF) - KEY_BIAS;
+    k[2] = (int)(key & 0x1FFFFF) - KEY_BIAS;
+}
+
+__device__ __forceinline__ bool index_in_range(int k) { return k >= -KEY_BIAS && k < KEY_BIAS; }
+
+// Spatial hash of the packed key (PAPER.md:62 cites Niessner et al. for its hash; slot placement is not
+// observable, so the mixing function is a free choice): 64-bit finaliser-style avalanche.
+__device__ __forceinline__ uint32_t hash_key(unsigned long long k) {
+    k ^= k >> 33;
+    k *= 0xff51afd7ed558ccdULL;
+    k ^= k >> 33;
+    k *= 0xc4ceb9fe1a85ec53ULL;
+    k ^= k >> 33;
+    return (uint32_t)k;
+}
+
+// ---- A4: rigid transform (R4): ((R0 x + R1 y) + R2 z) + t, every operation one rounded binary64 op --------
+__device__ __forceinline__ void transform_point(const Pose& T, float sx, float sy, float sz, float out[3]) {
+    const double x = (double)sx, y = (double)sy, z = (double)sz;
+#pragma unroll
+    for (int r = 0; r < 3; ++r) {
+        double acc = __dadd_rn(__dmul_rn(T.R[3 * r + 0], x), __dmul_rn(T.R[3 * r + 1], y));
+        acc = __dadd_rn(acc, __dmul_rn(T.R[3 * r + 2], z));
+        acc = __dadd_rn(acc, T.t[r]);
+        out[r] = __double2float_rn(acc);
+    }
+}
+
+// ---- A6: squared distance (R6): exact differences, (dx^2 + dy^2) + dz^2 in rounded binary64 ops ---------
+__device__ __forceinline__ double dist2(float qx, float qy, float qz, float px, float py, float pz) {
+    const double dx = (double)qx - (double)px;
+    const double dy = (double)qy - (double)py;
+    const double dz = (double)qz - (double)pz;
+    return __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+}
+
+__device__ __forceinline__ Entry load_entry(const Entry* table, uint32_t s) {
+    const uint4 raw = __ldg(reinterpret_cast<const uint4*>(table + s));
+    Entry e;
+    e.key = ((unsigned long long)raw.y << 32) | raw.x;
+    e.count = raw.z;
+    e.pad = raw.w;
+    return e;
+}
+
+// read-only lookup: slot of `key` and its count, or count = 0 if absent / dead
+__device__ __forceinline__ uint32_t find_voxel(const MapView& m, unsigned long long key, uint32_t& count) {
+    uint32_t s = hash_key(key) & m.mask;
+    for (uint32_t probes = 0; probes < m.slots; ++probes) {
+        const Entry e = load_entry(m.table, s);
+        if (e.key == key) { count = e.count; return s; }
+        if (e.key == KEY_EMPTY) break;
+        s = (s + 1) & m.mask;
+    }
+    count = 0;
+    return NO_SLOT;
+}
+
+// lexicographic (d2, id) candidate; d2 >= 0 so its bit pattern orders like the value
+struct Best {
+    double d2;
+    uint32_t id;
+    uint32_t ref;     // slot*cap + position of the stored point
+};
+
+__device__ __forceinline__ bool better(double d2, uint32_t id, const Best& b) {
+    return d2 < b.d2 || (d2 == b.d2 && id < b.id);
+}
+
+// warp arg-min over (d2, id): three redux.sync steps on the 64-bit pattern halves and the id; returns the lane
+// holding the winner (lanes with no candidate carry d2 = +inf, id = NO_ID)
+__device__ __forceinline__ int warp_argmin(double d2, uint32_t id) {
+    const unsigned long long bits = (unsigned long long)__double_as_longlong(d2);
+    const uint32_t hi = (uint32_t)(bits >> 32), lo = (uint32_t)bits;
+    const uint32_t mhi = __reduce_min_sync(FULL, hi);
+    bool c = hi == mhi;
+    const uint32_t mlo = __reduce_min_sync(FULL, c ? lo : 0xFFFFFFFFu);
+    c = c && lo == mlo;
+    const uint32_t mid = __reduce_min_sync(FULL, c ? id : 0xFFFFFFFFu);
+    c = c && id == mid;
+    const unsigned b = __ballot_sync(FULL, c);
+    return __ffs(b) - 1;
+}
+
+__device__ __forceinline__ int warp_incl_scan(int v, int lane) {
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const int o = __shfl_up_sync(FULL, v, d);
+        if (lane >= d) v += o;
+    }
+    return v;
+}
+
+// The 27-voxel probe of one query by one warp (Fig. 3): lane l < 27 looks up neighbour
+// (l/9-1, (l/3)%3-1, l%3-1); s_off[0..27] receives the exclusive prefix of the counts, s_slot[0..26] the slots.
+// Returns the total number of candidate points.  All 32 lanes must call.
+__device__ __forceinline__ int probe27(const MapView& m, const int k[3], int lane, int* s_off, uint32_t* s_slot) {
+    uint32_t cnt = 0, slot = NO_SLOT;
+    if (lane < 27) {
+        const int nx = k[0] + lane / 9 - 1, ny = k[1] + (lane / 3) % 3 - 1, nz = k[2] + lane % 3 - 1;
+        if (index_in_range(nx) && index_in_range(ny) && index_in_range(nz)) slot = find_voxel(m, pack_key(nx, ny, nz), cnt);
+    }
+    const int incl = warp_incl_scan((int)cnt, lane);
+    if (lane < 27) {
+        s_off[lane + 1] = incl;
+        s_slot[lane] = slot;
+    }
+    if (lane == 0) s_off[0] = 0;
+    __syncwarp();
+    return __shfl_sync(FULL, incl, 31);
+}
+
+}  // namespace far

@@ -1,0 +1,440 @@
+// far_gicp.cu -- sparsity-aware GICP registration on the voxel hashmap (A8-A10), one cooperative kernel.
+//
+// P0* = T_t P* (Eq. 2); per iteration: kNN-search (k = 1) of every transformed source point
+// in the submap, adaptive-threshold rejection, residual d = r - T s (Eq. 3), robust least squares
+// on d^T (Sigma_r + T Sigma_s T^T)^-1 d (Eq. 4) with the Cauchy kernel (Eq. 5), sparsity-aware fallback
+// Sigma_r = I, Sigma_s = 0 when a covariance is missing, point update (Eq. 6) and the stop test
+// ||T_L,j|| <= 5e-3.  Readings R9-R14 fix what the paper leaves open: IRLS weight on
+// e = sqrt(d^T M d); left perturbation T <- Exp(delta) T with delta = (rho, phi); J = [-I | [p]x]; the pose is
+// accumulated in FP64 and always applied to the ORIGINAL scan; stop on ||delta||_2; max_iters replaces the
+// wall-clock limit.
+//
+// B200 design: a registration is a few thousand source points, i.e. latency- not bandwidth-bound, so the whole
+// Gauss-Newton loop is ONE persistent cooperative kernel: one warp per source point (27-voxel probe + flattened
+// candidate sweep, see far_query.cu), the 29 unique terms of (H, b, chi2, n) reduced lane -> warp -> block ->
+// last-arriving block in a fixed order (deterministic, no floating atomics), the 6x6 Cholesky solve, SE(3)
+// exponential and pose update done by one thread of that last block in FP64, and one grid-wide barrier per
+// iteration.  The host is not involved until it reads the result.
+#include <cooperative_groups.h>
+
+#include <cstring>
+
+#include "far_internal.h"
+
+namespace cg = cooperative_groups;
+using namespace far;
+
+namespace far {
+
+constexpr int GWARPS = 8;        // warps per block
+constexpr int NTERMS = 29;       // 21 (H upper triangle) + 6 (b) + chi2 + inlier count
+constexpr int TSTRIDE = 32;      // padded row of per-block partials
+
+struct GicpState {
+    Pose pose;
+    int done;
+    unsigned int ticket;
+};
+
+struct GicpParams {
+    const float* scan;
+    const float* cov6;          // nullable
+    const uint8_t* valid;       // nullable
+    int64_t n;
+    const int64_t* d_n;         // nullable: n = min(n, *d_n)
+    int stride;
+    Pose init;                  // used when d_init == nullptr
+    const Pose* d_init;
+    double tau2, kappa, conv_eps;
+    int kernel, max_iters, linearize_only;
+    double* partials;           // [gridDim.x][TSTRIDE]
+    GicpState* state;
+    far_gicp_result_t* out;
+};
+
+// nearest-neighbour core shared in spirit with far_query.cu (kept local so the kernel inlines it)
+__device__ __forceinline__ uint32_t g_cand_ref(const int* s_off, const uint32_t* s_slot, int j, int& v, int cap) {
+    while (j >= s_off[v + 1]) ++v;
+    return s_slot[v] * (uint32_t)cap + (uint32_t)(j - s_off[v]);
+}
+
+__device__ __forceinline__ double robust_weight(int kernel, double e2, double kappa) {
+    if (kernel == FAR_KERNEL_CAUCHY) return 1.0 / (1.0 + e2 / (kappa * kappa));          // Eq. 5 as IRLS weight (R9)
+    if (kernel == FAR_KERNEL_GEMAN_MCCLURE) { const double s = kappa + e2; return (kappa * kappa) / (s * s); }
+    return 1.0;
+}
+
+// symmetric 3x3 inverse from the 6 unique entries (xx,xy,xz,yy,yz,zz); false if singular
+__device__ __forceinline__ bool inv_sym3(const double a[6], double o[6]) {
+    const double c00 = a[3] * a[5] - a[4] * a[4];
+    const double c01 = a[4] * a[2] - a[1] * a[5];
+    const double c02 = a[1] * a[4] - a[3] * a[2];
+    const double det = a[0] * c00 + a[1] * c01 + a[2] * c02;
+    if (!(det != 0.0) || !isfinite(det)) return false;
+    const double id = 1.0 / det;
+    o[0] = c00 * id; o[1] = c01 * id; o[2] = c02 * id;
+    o[3] = (a[0] * a[5] - a[2] * a[2]) * id;
+    o[4] = (a[2] * a[1] - a[0] * a[4]) * id;
+    o[5] = (a[0] * a[3] - a[1] * a[1]) * id;
+    return true;
+}
+
+// A9 for one correspondence: the 29 terms, written by lane 0 into s_terms
+__device__ __forceinline__ void correspondence_terms(const Pose& T, const double p[3], const double r[3], bool full,
+                                                      const float* cs, const float* cr, int kernel, double kappa,
+                                                      double* terms) {
+    const double d0 = r[0] - p[0], d1 = r[1] - p[1], d2 = r[2] - p[2];   // Eq. 3
+    double M[6] = {1.0, 0.0, 0.0, 1.0, 0.0, 1.0};                        // SA fallback: Sigma_r = I, Sigma_s = 0
+    if (full) {
+        // S = Sigma_r + R Sigma_s R^T   (Eq. 4)
+        const double s[6] = {cs[0], cs[1], cs[2], cs[3], cs[4], cs[5]};
+        double RS[9];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            const double a = T.R[3 * i], b = T.R[3 * i + 1], c = T.R[3 * i + 2];
+            RS[3 * i + 0] = a * s[0] + b * s[1] + c * s[2];
+            RS[3 * i + 1] = a * s[1] + b * s[3] + c * s[4];
+            RS[3 * i + 2] = a * s[2] + b * s[4] + c * s[5];
+        }
+        double S[6];
+        S[0] = (double)cr[0] + (RS[0] * T.R[0] + RS[1] * T.R[1] + RS[2] * T.R[2]);
+        S[1] = (double)cr[1] + (RS[0] * T.R[3] + RS[1] * T.R[4] + RS[2] * T.R[5]);
+        S[2] = (double)cr[2] + (RS[0] * T.R[6] + RS[1] * T.R[7] + RS[2] * T.R[8]);
+        S[3] = (double)cr[3] + (RS[3] * T.R[3] + RS[4] * T.R[4] + RS[5] * T.R[5]);
+        S[4] = (double)cr[4] + (RS[3] * T.R[6] + RS[4] * T.R[7] + RS[5] * T.R[8]);
+        S[5] = (double)cr[5] + (RS[6] * T.R[6] + RS[7] * T.R[7] + RS[8] * T.R[8]);
+        double Mi[6];
+        if (inv_sym3(S, Mi)) {
+#pragma unroll
+            for (int a = 0; a < 6; ++a) M[a] = Mi[a];
+        }
+    }
+    const double Md0 = M[0] * d0 + M[1] * d1 + M[2] * d2;
+    const double Md1 = M[1] * d0 + M[3] * d1 + M[4] * d2;
+    const double Md2 = M[2] * d0 + M[4] * d1 + M[5] * d2;
+    const double e2 = d0 * Md0 + d1 * Md1 + d2 * Md2;
+    const double w = robust_weight(kernel, e2, kappa);
+    const double px = p[0], py = p[1], pz = p[2];
+    // X = M A with A = [p]x :  column 0 = M(:,1) pz - M(:,2) py, column 1 = -M(:,0) pz + M(:,2) px, column 2 = M(:,0) py - M(:,1) px
+    const double Mr[3][3] = {{M[0], M[1], M[2]}, {M[1], M[3], M[4]}, {M[2], M[4], M[5]}};
+    double X[3][3];
+#pragma unroll
+    for (int r_ = 0; r_ < 3; ++r_) {
+        X[r_][0] = Mr[r_][1] * pz - Mr[r_][2] * py;
+        X[r_][1] = Mr[r_][2] * px - Mr[r_][0] * pz;
+        X[r_][2] = Mr[r_][0] * py - Mr[r_][1] * px;
+    }
+    // Y = A^T X (symmetric):  row 0 = pz X[1] - py X[2], row 1 = px X[2] - pz X[0], row 2 = py X[0] - px X[1]
+    const double Y00 = pz * X[1][0] - py * X[2][0], Y01 = pz * X[1][1] - py * X[2][1], Y02 = pz * X[1][2] - py * X[2][2];
+    const double Y11 = px * X[2][1] - pz * X[0][1], Y12 = px * X[2][2] - pz * X[0][2];
+    const double Y22 = py * X[0][2] - px * X[1][2];
+    // H = w J^T M J with J = [-I | A]:  [[M, -X], [-X^T, Y]];   b = w J^T M d = w [-Md ; A^T Md]
+    terms[0] = w * M[0];  terms[1] = w * M[1];  terms[2] = w * M[2];  terms[3] = -w * X[0][0]; terms[4] = -w * X[0][1]; terms[5] = -w * X[0][2];
+    terms[6] = w * M[3];  terms[7] = w * M[4];  terms[8] = -w * X[1][0]; terms[9] = -w * X[1][1]; terms[10] = -w * X[1][2];
+    terms[11] = w * M[5]; terms[12] = -w * X[2][0]; terms[13] = -w * X[2][1]; terms[14] = -w * X[2][2];
+    terms[15] = w * Y00;  terms[16] = w * Y01;  terms[17] = w * Y02;
+    terms[18] = w * Y11;  terms[19] = w * Y12;
+    terms[20] = w * Y22;
+    terms[21] = -w * Md0; terms[22] = -w * Md1; terms[23] = -w * Md2;
+    terms[24] = w * (pz * Md1 - py * Md2);
+    terms[25] = w * (px * Md2 - pz * Md0);
+    terms[26] = w * (py * Md0 - px * Md1);
+    terms[27] = w * e2;
+    terms[28] = 1.0;
+}
+
+// 6x6 Cholesky solve H x = rhs (FP64); false if H is not positive definite
+__device__ bool chol_solve6(const double* H, const double* rhs, double* x) {
+    double L[36];
+    for (int i = 0; i < 36; ++i) L[i] = 0.0;
+    for (int i = 0; i < 6; ++i)
+        for (int j = 0; j <= i; ++j) {
+            double s = H[6 * i + j];
+            for (int k = 0; k < j; ++k) s -= L[6 * i + k] * L[6 * j + k];
+            if (i == j) {
+                if (!(s > 0.0) || !isfinite(s)) return false;
+                L[6 * i + i] = sqrt(s);
+            } else {
+                L[6 * i + j] = s / L[6 * j + j];
+            }
+        }
+    double y[6];
+    for (int i = 0; i < 6; ++i) {
+        double s = rhs[i];
+        for (int k = 0; k < i; ++k) s -= L[6 * i + k] * y[k];
+        y[i] = s / L[6 * i + i];
+    }
+    for (int i = 5; i >= 0; --i) {
+        double s = y[i];
+        for (int k = i + 1; k < 6; ++k) s -= L[6 * k + i] * x[k];
+        x[i] = s / L[6 * i + i];
+    }
+    return true;
+}
+
+// SE(3) exponential of delta = (rho, phi), translation first (R12); series below theta = 1e-8
+__device__ void se3_exp(const double* d, Pose& E) {
+    const double phi[3] = {d[3], d[4], d[5]};
+    const double th2 = phi[0] * phi[0] + phi[1] * phi[1] + phi[2] * phi[2];
+    const double th = sqrt(th2);
+    double A, B, C;
+    if (th < 1e-8) {
+        A = 1.0 - th2 / 6.0; B = 0.5 - th2 / 24.0; C = 1.0 / 6.0 - th2 / 120.0;
+    } else {
+        A = sin(th) / th; B = (1.0 - cos(th)) / th2; C = (th - sin(th)) / (th2 * th);
+    }
+    const double K[9] = {0, -phi[2], phi[1], phi[2], 0, -phi[0], -phi[1], phi[0], 0};
+    double K2[9], V[9];
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) {
+            double s = 0.0;
+            for (int k = 0; k < 3; ++k) s += K[3 * i + k] * K[3 * k + j];
+            K2[3 * i + j] = s;
+        }
+    for (int i = 0; i < 9; ++i) {
+        const double I = (i % 4 == 0) ? 1.0 : 0.0;
+        E.R[i] = I + A * K[i] + B * K2[i];
+        V[i] = I + B * K[i] + C * K2[i];
+    }
+    for (int r = 0; r < 3; ++r) E.t[r] = V[3 * r] * d[0] + V[3 * r + 1] * d[1] + V[3 * r + 2] * d[2];
+}
+
+__global__ void __launch_bounds__(GWARPS * 32, 4) gicp_kernel(MapView m, GicpParams P) {
+    __shared__ int s_off[GWARPS][32];
+    __shared__ uint32_t s_slot[GWARPS][32];
+    __shared__ double s_terms[GWARPS][TSTRIDE];
+    __shared__ double s_red[GWARPS][TSTRIDE];
+    __shared__ Pose s_T;
+    __shared__ int s_last;
+    cg::grid_group grid = cg::this_grid();
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const int64_t nwarps = (int64_t)gridDim.x * GWARPS;
+    int64_t n = P.n;
+    if (P.d_n) n = min(n, *P.d_n);
+    if (threadIdx.x < 12) {
+        const Pose& src = P.d_init ? *P.d_init : P.init;
+        double vv = threadIdx.x < 9 ? src.R[threadIdx.x] : src.t[threadIdx.x - 9];
+        if (threadIdx.x < 9) s_T.R[threadIdx.x] = vv; else s_T.t[threadIdx.x - 9] = vv;
+    }
+    __syncthreads();
+
+    for (int it = 0; it < P.max_iters; ++it) {
+        // ---- A8 + A9: one warp per source point; lane t < 29 accumulates term t ---------------------------------
+        double acc = 0.0;
+        for (int64_t i = (int64_t)blockIdx.x * GWARPS + wib; i < n; i += nwarps) {
+            const float* sp = P.scan + i * P.stride;
+            const float sx = __ldg(sp), sy = __ldg(sp + 1), sz = __ldg(sp + 2);
+            if (!(isfinite(sx) && isfinite(sy) && isfinite(sz))) continue;
+            float pf[3];
+            transform_point(s_T, sx, sy, sz, pf);                 // Eq. 2 with the accumulated pose (R11)
+            int k[3];
+            if (!voxel_index(pf[0], pf[1], pf[2], m.voxel, k)) continue;
+            // kNN-search, k = 1
+            const int total = probe27(m, k, lane, s_off[wib], s_slot[wib]);
+            Best best;
+            best.d2 = __longlong_as_double(0x7FF0000000000000ll);
+            best.id = NO_ID;
+            best.ref = 0;
+            int v = 0;
+            for (int j = lane; j < total; j += 32) {
+                const uint32_t ref = g_cand_ref(s_off[wib], s_slot[wib], j, v, m.cap);
+                const float4 q = __ldg(m.points + ref);
+                const double d2 = dist2(pf[0], pf[1], pf[2], q.x, q.y, q.z);
+                const uint32_t id = __float_as_uint(q.w);
+                if (better(d2, id, best)) { best.d2 = d2; best.id = id; best.ref = ref; }
+            }
+            __syncwarp();
+            const int w = warp_argmin(best.d2, best.id);
+            const double bd2 = __shfl_sync(FULL, best.d2, w);
+            const uint32_t bid = __shfl_sync(FULL, best.id, w);
+            const uint32_t bref = __shfl_sync(FULL, best.ref, w);
+            if (bid == NO_ID || bd2 > P.tau2) continue;           // adaptive-threshold gate
+            if (lane == 0) {
+                const float4 rp = __ldg(m.points + bref);
+                const double p[3] = {(double)pf[0], (double)pf[1], (double)pf[2]};
+                const double r[3] = {(double)rp.x, (double)rp.y, (double)rp.z};
+                bool full = P.cov6 && P.valid && P.valid[i] != 0 && m.cov_ok && m.cov_ok[bref] != 0;
+                correspondence_terms(s_T, p, r, full, full ? P.cov6 + 6 * i : nullptr, full ? m.cov + (size_t)bref * 6 : nullptr,
+                                     P.kernel, P.kappa, s_terms[wib]);
+            }
+            __syncwarp();
+            if (lane < NTERMS) acc += s_terms[wib][lane];
+            __syncwarp();
+        }
+        // ---- A10: warp -> block -> last block, fixed order --------------------------------------------------------
+        s_red[wib][lane] = lane < NTERMS ? acc : 0.0;
+        __syncthreads();
+        if (wib == 0) {
+            double s = 0.0;
+#pragma unroll
+            for (int w8 = 0; w8 < GWARPS; ++w8) s += s_red[w8][lane];
+            P.partials[(size_t)blockIdx.x * TSTRIDE + lane] = s;
+            __threadfence();
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            const unsigned int t = atomicAdd(&P.state->ticket, 1u);
+            s_last = (t == gridDim.x - 1) ? 1 : 0;
+        }
+        __syncthreads();
+        if (s_last) {
+            __threadfence();
+            // 8 warps each sum a strided subset of the blocks, then warp 0 combines them: same order every run
+            double s = 0.0;
+            for (unsigned b = wib; b < gridDim.x; b += GWARPS) s += __ldcg(P.partials + (size_t)b * TSTRIDE + lane);
+            s_red[wib][lane] = s;
+            __syncthreads();
+            if (wib == 0) {
+                double tsum = 0.0;
+#pragma unroll
+                for (int w8 = 0; w8 < GWARPS; ++w8) tsum += s_red[w8][lane];
+                s_terms[0][lane] = tsum;
+            }
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                const double* tv = s_terms[0];
+                double H[36], b[6];
+                int q = 0;
+                for (int a = 0; a < 6; ++a)
+                    for (int c = a; c < 6; ++c) { H[6 * a + c] = tv[q]; H[6 * c + a] = tv[q]; ++q; }
+                for (int a = 0; a < 6; ++a) b[a] = tv[21 + a];
+                const int n_inl = (int)(tv[28] + 0.5);
+                far_gicp_result_t* out = P.out;
+                bool done = false;
+                int converged = 0, status = FAR_OK;
+                Pose Tn = s_T;
+                if (!P.linearize_only) {
+                    double rhs[6], delta[6];
+                    for (int a = 0; a < 6; ++a) rhs[a] = -b[a];
+                    if (n_inl < 6 || !chol_solve6(H, rhs, delta)) {
+                        status = FAR_ERR_DEGENERATE;
+                        Tn = P.d_init ? *P.d_init : P.init;
+                        done = true;
+                    } else {
+                        Pose E;
+                        se3_exp(delta, E);
+                        for (int i = 0; i < 3; ++i)
+                            for (int j = 0; j < 3; ++j) {
+                                double s2 = 0.0;
+                                for (int kk = 0; kk < 3; ++kk) s2 += E.R[3 * i + kk] * s_T.R[3 * kk + j];
+                                Tn.R[3 * i + j] = s2;
+                            }
+                        for (int r = 0; r < 3; ++r)
+                            Tn.t[r] = (E.R[3 * r] * s_T.t[0] + E.R[3 * r + 1] * s_T.t[1] + E.R[3 * r + 2] * s_T.t[2]) + E.t[r];
+                        double nrm = 0.0;
+                        for (int a = 0; a < 6; ++a) nrm += delta[a] * delta[a];
+                        if (sqrt(nrm) <= P.conv_eps) { converged = 1; done = true; }   // PAPER.md:100, R13
+                    }
+                } else {
+                    done = true;
+                }
+                if (it + 1 >= P.max_iters) done = true;
+                P.state->pose = Tn;
+                if (done) {
+                    for (int a = 0; a < 9; ++a) out->pose.R[a] = Tn.R[a];
+                    for (int a = 0; a < 3; ++a) out->pose.t[a] = Tn.t[a];
+                    for (int a = 0; a < 36; ++a) out->H[a] = H[a];
+                    for (int a = 0; a < 6; ++a) out->b[a] = b[a];
+                    out->chi2 = tv[27];
+                    out->n_inliers = n_inl;
+                    out->iters = it + 1;
+                    out->converged = converged;
+                    out->status = status;
+                }
+                P.state->done = done ? 1 : 0;
+                P.state->ticket = 0u;
+                __threadfence();
+            }
+        }
+        grid.sync();
+        if (*reinterpret_cast<volatile int*>(&P.state->done)) break;
+        if (threadIdx.x < 12) {
+            const double vv = __ldcg(threadIdx.x < 9 ? &P.state->pose.R[threadIdx.x] : &P.state->pose.t[threadIdx.x - 9]);
+            if (threadIdx.x < 9) s_T.R[threadIdx.x] = vv; else s_T.t[threadIdx.x - 9] = vv;
+        }
+        __syncthreads();
+    }
+}
+
+}  // namespace far
+
+extern "C" {
+
+void far_gicp_default_options(far_gicp_options_t* o) {
+    if (!o) return;
+    o->kernel = FAR_KERNEL_CAUCHY;
+    o->conv_eps = 5e-3;
+    o->tau_mult = 3.0;
+    o->kappa_div = 3.0;
+}
+
+static int gicp_launch(const far_map_t* map, const float* d_scan, const float* d_cov6, const uint8_t* d_valid, int64_t n,
+                       const int64_t* d_n, int stride, const far_pose_t* hpose, const far_pose_t* d_pose, double sigma,
+                       int max_iters, int linearize_only, const far_gicp_options_t* opts, far_gicp_result_t* d_out,
+                       void* stream) {
+    if (!map || !d_out || n < 0 || (n > 0 && !d_scan) || (stride != 3 && stride != 4) || max_iters < 1 || (!hpose && !d_pose))
+        return FAR_ERR_ARG;
+    far_gicp_options_t o;
+    if (opts) o = *opts; else far_gicp_default_options(&o);
+    if (o.kernel < 0 || o.kernel > 2 || !(sigma > 0.0)) return FAR_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    GicpParams P;
+    memset(&P, 0, sizeof(P));
+    P.scan = d_scan; P.cov6 = d_cov6; P.valid = d_valid; P.n = n; P.d_n = d_n; P.stride = stride;
+    if (hpose) memcpy(&P.init, hpose, sizeof(Pose));
+    P.d_init = (const Pose*)d_pose;
+    const double tau = o.tau_mult * sigma;
+    P.tau2 = tau * tau;
+    P.kappa = sigma / o.kappa_div;
+    P.conv_eps = o.conv_eps;
+    P.kernel = o.kernel; P.max_iters = max_iters; P.linearize_only = linearize_only;
+    P.partials = map->d_gicp_partials;
+    P.state = (GicpState*)map->d_gicp_state;
+    P.out = d_out;
+    int64_t grid = map->gicp_max_grid;
+    const int64_t need = (n + GWARPS - 1) / GWARPS;
+    if (need < grid) grid = need;
+    if (grid < 1) grid = 1;
+    FAR_CUDA(cudaMemsetAsync(map->d_gicp_state, 0, sizeof(GicpState), st));
+    MapView view = map->view;
+    void* args[] = {(void*)&view, (void*)&P};
+    FAR_CUDA(cudaLaunchCooperativeKernel((const void*)gicp_kernel, dim3((unsigned)grid), dim3(GWARPS * 32), args, 0, st));
+    return FAR_OK;
+}
+
+int far_gicp_linearize(const far_map_t* map, const float* d_scan, const float* d_cov6, const uint8_t* d_valid, int64_t n,
+                       int stride, const far_pose_t* pose, double sigma, const far_gicp_options_t* opts,
+                       far_gicp_result_t* d_out, void* stream) {
+    return gicp_launch(map, d_scan, d_cov6, d_valid, n, nullptr, stride, pose, nullptr, sigma, 1, 1, opts, d_out, stream);
+}
+
+int far_gicp_register(const far_map_t* map, const float* d_scan, const float* d_cov6, const uint8_t* d_valid, int64_t n,
+                      int stride, const far_pose_t* init_pose, double sigma, int max_iters, const far_gicp_options_t* opts,
+                      far_gicp_result_t* d_out, void* stream) {
+    return gicp_launch(map, d_scan, d_cov6, d_valid, n, nullptr, stride, init_pose, nullptr, sigma, max_iters, 0, opts, d_out,
+                       stream);
+}
+
+int far_gicp_register_dev(const far_map_t* map, const float* d_scan, const float* d_cov6, const uint8_t* d_valid,
+                          const int64_t* d_n, int64_t n_max, int stride, const far_pose_t* d_init_pose, double sigma,
+                          int max_iters, const far_gicp_options_t* opts, far_gicp_result_t* d_out, void* stream) {
+    if (!d_n || !d_init_pose) return FAR_ERR_ARG;
+    return gicp_launch(map, d_scan, d_cov6, d_valid, n_max, d_n, stride, nullptr, d_init_pose, sigma, max_iters, 0, opts, d_out,
+                       stream);
+}
+
+}  // extern "C"
+
+namespace far {
+// called once from far_map_create: sizes the cooperative grid and allocates the reduction scratch
+int gicp_setup(far_map* map) {
+    int per_sm = 0;
+    FAR_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gicp_kernel, GWARPS * 32, 0));
+    if (per_sm < 1) per_sm = 1;
+    map->gicp_max_grid = map->sm_count * per_sm;
+    FAR_CUDA(cudaMalloc((void**)&map->d_gicp_partials, (size_t)map->gicp_max_grid * TSTRIDE * sizeof(double)));
+    FAR_CUDA(cudaMalloc((void**)&map->d_gicp_state, sizeof(GicpState)));
+    FAR_CUDA(cudaMemset(map->d_gicp_state, 0, sizeof(GicpState)));
+    return FAR_OK;
+}
+}  // namespace far

@@ -1,0 +1,44 @@
+// far_internal.h -- host-side handle of a map and helpers shared by the translation units of libfar.so.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "far_common.cuh"
+
+struct far_map {
+    far_map_config_t cfg;
+    far::MapView view;          // device pointers + constants, passed by value to kernels
+    uint32_t* d_touched;        // [max_batch] slots that received their first new point in the chunk
+    uint32_t* d_cov_list;       // [max_batch] refs (slot*cap+pos) of accepted points awaiting a covariance
+    double* d_gicp_partials;    // [gicp_max_grid][32] per-block partial sums of one GICP linearisation
+    void* d_gicp_state;         // iteration state of the cooperative GICP kernel (pose, done flag, ticket)
+    int gicp_max_grid;          // co-resident blocks of the GICP kernel on this device
+    int64_t max_batch;
+    uint64_t next_id;           // id of the next offered point (host-side: advances by n per insert)
+    int device;
+    int sm_count;
+};
+
+namespace far {
+
+void set_cuda_error(cudaError_t e, const char* where);
+
+#define FAR_CUDA(call)                                   \
+    do {                                                 \
+        cudaError_t e_ = (call);                         \
+        if (e_ != cudaSuccess) {                         \
+            far::set_cuda_error(e_, #call);              \
+            return FAR_ERR_CUDA;                         \
+        }                                                \
+    } while (0)
+
+inline int grid_for(int64_t n, int block) { return (int)((n + block - 1) / block); }
+
+// launch helpers implemented in far_query.cu (used by far_map.cu for the covariances of accepted points)
+int launch_knn_cov_refs(const far_map* map, const uint32_t* d_refs, const unsigned int* d_n, int64_t n_max,
+                        cudaStream_t stream);
+int launch_knn_cov_new_ids(const far_map* map, uint32_t first_id, cudaStream_t stream);
+// implemented in far_gicp.cu: sizes the cooperative grid, allocates the reduction scratch of a map
+int gicp_setup(far_map* map);
+
+}  // namespace far

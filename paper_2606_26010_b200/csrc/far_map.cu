@@ -1,0 +1,622 @@
+// far_map.cu -- the voxel hashmap: create / clear / deterministic capped insert / prune / export / stats.
+//
+// PAPER.md:62-68 (cuVoxelMap: custom key = 3D voxel indices, linear probing, <= N_max points per voxel, built
+// for concurrent access), PAPER.md:109 (submap update: insert at T_L with a per-voxel cap, recompute the
+// covariances of added points only, remove voxels beyond a range limit).
+//
+// Deterministic capped insert (reading R3: the result equals inserting the points one by one in index order).
+// A bare atomicAdd ticket gives the right counts but timing-dependent contents, so instead each offered point
+// runs an *atomicMin insertion chain* on the id words of its voxel's free positions c0..cap-1 (all FAR_NO_ID =
+// +inf before the batch):   x = my id;  for pos = c0..cap-1:  old = atomicMin(&id[pos], x);
+//                           old == NO_ID -> placed, stop;   old > x -> carry the displaced id: x = old.
+// Every id of the batch that targets the voxel enters at position c0 and every id except the final occupant of
+// a position moves on to the next one exactly once, so position c0+r ends up holding the (r+1)-th smallest id
+// whatever the interleaving: the lowest ids win, in ascending order, with no sort.  Ids already stored are all
+// smaller than the batch's ids (ids grow monotonically), so they stay where they are.  A second kernel walks
+// the voxels that received a point, fetches the coordinates of the surviving ids (index = id - first id of
+// the chunk) and writes them next to their id.
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "far_internal.h"
+
+using namespace far;
+
+namespace far {
+
+static thread_local char g_cuda_err[256] = "";
+void set_cuda_error(cudaError_t e, const char* where) {
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s (%s)", cudaGetErrorName(e), cudaGetErrorString(e), where);
+}
+
+__device__ __forceinline__ bool load_pose_point(const float* __restrict__ xyz, int64_t i, int stride, int pose_mode,
+                                                const Pose& T, float p[3]) {
+    const float* s = xyz + i * stride;
+    const float x = s[0], y = s[1], z = s[2];
+    if (!(isfinite(x) && isfinite(y) && isfinite(z))) return false;
+    if (pose_mode) transform_point(T, x, y, z, p);
+    else { p[0] = x; p[1] = y; p[2] = z; }
+    return true;
+}
+
+// ---- insert, kernel 1: key -> find-or-claim -> atomicMin chain ---------------------------------------
+__global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, const float* __restrict__ xyz, int64_t n,
+                                                                  int stride, int pose_mode, Pose hpose,
+                                                                  const Pose* __restrict__ d_pose, uint32_t first_id,
+                                                                  uint32_t* __restrict__ touched) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const Pose& T = (pose_mode == 2) ? *d_pose : hpose;
+    float p[3];
+    int k[3];
+    if (!load_pose_point(xyz, i, stride, pose_mode, T, p) || !voxel_index(p[0], p[1], p[2], m.voxel, k)) {
+        atomicAdd(&m.ctr->st_invalid, 1ull);
+        return;
+    }
+    const unsigned long long key = pack_key(k[0], k[1], k[2]);
+    // find or claim the voxel's slot: 64-bit atomicCAS on the key word, linear probing step 1
+    uint32_t s = hash_key(key) & m.mask;
+    bool found = false;
+    for (uint32_t probes = 0; probes < m.slots; ++probes) {
+        unsigned long long cur = *reinterpret_cast<volatile unsigned long long*>(&m.table[s].key);
+        if (cur == KEY_EMPTY) {
+            if (*reinterpret_cast<volatile unsigned long long*>(&m.ctr->n_keys) >= m.max_keys) break;   // table full
+            cur = atomicCAS(&m.table[s].key, KEY_EMPTY, key);
+            if (cur == KEY_EMPTY) {
+                atomicAdd(&m.ctr->n_keys, 1ull);
+                found = true;
+                break;
+            }
+        }
+        if (cur == key) { found = true; break; }
+        s = (s + 1) & m.mask;
+    }
+    if (!found) {
+        atomicAdd(&m.ctr->st_dropped_full, 1ull);
+        m.ctr->full_flag = 1u;
+        return;
+    }
+    // count is only written by the commit kernel, so it is stable here: c0 = points stored before this chunk
+    const uint32_t c0 = *reinterpret_cast<volatile uint32_t*>(&m.table[s].count);
+    const uint32_t cap = (uint32_t)m.cap;
+    if (c0 >= cap) return;
+    uint32_t* idw = reinterpret_cast<uint32_t*>(m.points + (size_t)s * cap) + 3;   // id word of position 0; stride 4
+    uint32_t x = first_id + (uint32_t)i;
+    // ids at a position only ever decrease: if the last position already holds a smaller id, x cannot survive
+    const uint32_t last = *reinterpret_cast<volatile uint32_t*>(idw + 4 * (cap - 1));
+    if (last < x) return;
+    for (uint32_t pos = c0; pos < cap; ++pos) {
+        const uint32_t old = atomicMin(idw + 4 * pos, x);
+        if (old == NO_ID) {
+            if (pos == c0) touched[atomicAdd(&m.ctr->n_touched, 1u)] = s;   // unique per voxel and chunk
+            break;
+        }
+        if (old > x) x = old;
+    }
+}
+
+// ---- insert, kernel 2: one warp per touched voxel writes the coordinates of the surviving ids ---------------
+__global__ void __launch_bounds__(256) insert_commit_kernel(MapView m, const float* __restrict__ xyz, int stride,
+                                                             int pose_mode, Pose hpose, const Pose* __restrict__ d_pose,
+                                                             uint32_t first_id, const uint32_t* __restrict__ touched,
+                                                             uint32_t* __restrict__ cov_list, int64_t cov_list_cap) {
+    const int lane = threadIdx.x & 31;
+    const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+    const Pose& T = (pose_mode == 2) ? *d_pose : hpose;
+    const uint32_t n_touched = m.ctr->n_touched;
+    const uint32_t cap = (uint32_t)m.cap;
+    for (int64_t t = warp; t < n_touched; t += nwarps) {
+        const uint32_t s = touched[t];
+        const uint32_t c0 = m.table[s].count;
+        float4* bucket = m.points + (size_t)s * cap;
+        uint32_t n_new = 0;
+        for (uint32_t base = c0; base < cap; base += 32) {
+            const uint32_t pos = base + lane;
+            uint32_t id = NO_ID;
+            if (pos < cap) id = __float_as_uint(bucket[pos].w);
+            const bool is_new = id != NO_ID;
+            if (is_new) {
+                float p[3];
+                load_pose_point(xyz, (int64_t)(id - first_id), stride, pose_mode, T, p);
+                bucket[pos] = make_float4(p[0], p[1], p[2], __uint_as_float(id));
+                if (m.cov_ok) m.cov_ok[(size_t)s * cap + pos] = 0;
+            }
+            const unsigned b = __ballot_sync(FULL, is_new);
+            const uint32_t cnt = __popc(b);
+            if (cov_list != nullptr && cnt) {
+                uint32_t at = 0;
+                if (lane == 0) at = atomicAdd(&m.ctr->n_cov, cnt);
+                at = __shfl_sync(FULL, at, 0);
+                const uint32_t mine = at + __popc(b & ((1u << lane) - 1u));
+                if (is_new && mine < cov_list_cap) cov_list[mine] = s * cap + pos;
+            }
+            n_new += cnt;
+        }
+        if (lane == 0) {
+            m.table[s].count = c0 + n_new;
+            atomicAdd(&m.ctr->st_accepted, (unsigned long long)n_new);
+            if (c0 == 0) atomicAdd(&m.ctr->st_new_voxels, 1ull);
+        }
+    }
+}
+
+__global__ void insert_stats_kernel(MapView m, int64_t n_offered, far_insert_stats_t* out) {
+    if (threadIdx.x == 0 && blockIdx.x == 0 && out) {
+        out->n_offered = n_offered;
+        out->n_accepted = (int64_t)m.ctr->st_accepted;
+        out->n_new_voxels = (int64_t)m.ctr->st_new_voxels;
+        out->n_dropped_full = (int64_t)m.ctr->st_dropped_full;
+        out->n_invalid = (int64_t)m.ctr->st_invalid;
+    }
+}
+
+// ---- A5 prune (R5): thread per slot, FP64 squared centre distance, strict > -------------------
+__global__ void __launch_bounds__(256) prune_kernel(MapView m, double cx, double cy, double cz, const Pose* d_pose,
+                                                     double r2) {
+    const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned long long vr = 0, pr = 0, vl = 0, pl = 0;
+    if (s < m.slots) {
+        const Entry e = m.table[s];
+        if (e.key != KEY_EMPTY && e.count > 0) {
+            if (d_pose) { cx = d_pose->t[0]; cy = d_pose->t[1]; cz = d_pose->t[2]; }
+            int k[3];
+            unpack_key(e.key, k);
+            const double v = (double)m.voxel;
+            const double dx = __dadd_rn(__dmul_rn(__dadd_rn((double)k[0], 0.5), v), -cx);
+            const double dy = __dadd_rn(__dmul_rn(__dadd_rn((double)k[1], 0.5), v), -cy);
+            const double dz = __dadd_rn(__dmul_rn(__dadd_rn((double)k[2], 0.5), v), -cz);
+            const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+            if (d2 > r2) {
+                // the key stays (dead key, count 0); its id words go back to +inf so a later insert starts clean
+                float4* bucket = m.points + (size_t)s * m.cap;
+                for (uint32_t j = 0; j < e.count; ++j) {
+                    bucket[j].w = __uint_as_float(NO_ID);
+                    if (m.cov_ok) m.cov_ok[(size_t)s * m.cap + j] = 0;
+                }
+                m.table[s].count = 0;
+                vr = 1; pr = e.count;
+            } else {
+                vl = 1; pl = e.count;
+            }
+        }
+    }
+    // warp-aggregate the four statistics
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        vr += __shfl_xor_sync(FULL, vr, d); pr += __shfl_xor_sync(FULL, pr, d);
+        vl += __shfl_xor_sync(FULL, vl, d); pl += __shfl_xor_sync(FULL, pl, d);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        if (vr) { atomicAdd(&m.ctr->pr_vox_removed, vr); atomicAdd(&m.ctr->pr_pts_removed, pr); }
+        if (vl) { atomicAdd(&m.ctr->pr_vox_left, vl); atomicAdd(&m.ctr->pr_pts_left, pl); }
+    }
+}
+
+__global__ void prune_stats_kernel(MapView m, far_prune_stats_t* out) {
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        if (out) {
+            out->n_voxels_removed = (int64_t)m.ctr->pr_vox_removed;
+            out->n_points_removed = (int64_t)m.ctr->pr_pts_removed;
+            out->n_voxels_left = (int64_t)m.ctr->pr_vox_left;
+            out->n_points_left = (int64_t)m.ctr->pr_pts_left;
+        }
+        m.ctr->pr_vox_removed = m.ctr->pr_pts_removed = m.ctr->pr_vox_left = m.ctr->pr_pts_left = 0ull;
+    }
+}
+
+// ---- clear: reset only what is in use (the pool itself is never touched beyond the live buckets) ------------
+__global__ void __launch_bounds__(256) clear_kernel(MapView m) {
+    const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= m.slots) return;
+    const Entry e = m.table[s];
+    if (e.key == KEY_EMPTY) return;
+    float4* bucket = m.points + (size_t)s * m.cap;
+    for (uint32_t j = 0; j < e.count; ++j) bucket[j].w = __uint_as_float(NO_ID);
+    Entry z;
+    z.key = KEY_EMPTY; z.count = 0; z.pad = 0;
+    m.table[s] = z;
+}
+
+__global__ void __launch_bounds__(256) table_init_kernel(Entry* table, uint32_t slots) {
+    const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= slots) return;
+    Entry z;
+    z.key = KEY_EMPTY; z.count = 0; z.pad = 0;
+    table[s] = z;
+}
+
+// ---- stats / export ----------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) stats_kernel(MapView m, unsigned long long* acc /* [3] */) {
+    const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned long long nv = 0, np = 0, nd = 0;
+    if (s < m.slots) {
+        const Entry e = m.table[s];
+        if (e.key != KEY_EMPTY) {
+            if (e.count > 0) { nv = 1; np = e.count; } else nd = 1;
+        }
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        nv += __shfl_xor_sync(FULL, nv, d); np += __shfl_xor_sync(FULL, np, d); nd += __shfl_xor_sync(FULL, nd, d);
+    }
+    if ((threadIdx.x & 31) == 0 && (nv | nd)) {
+        if (nv) { atomicAdd(&acc[0], nv); atomicAdd(&acc[1], np); }
+        if (nd) atomicAdd(&acc[2], nd);
+    }
+}
+
+__global__ void stats_out_kernel(MapView m, unsigned long long* acc, unsigned long long next_id, far_map_stats_t* out) {
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        out->n_voxels = (int64_t)acc[0];
+        out->n_points = (int64_t)acc[1];
+        out->n_dead_keys = (int64_t)acc[2];
+        out->n_slots = (int64_t)m.slots;
+        out->next_id = next_id;
+        acc[0] = acc[1] = acc[2] = 0ull;
+    }
+}
+
+// one warp per group of 32 slots; live voxels get consecutive output rows (order unspecified)
+__global__ void __launch_bounds__(256) export_kernel(MapView m, unsigned long long* __restrict__ keys,
+                                                      int32_t* __restrict__ counts, float4* __restrict__ pts,
+                                                      float* __restrict__ cov6, uint8_t* __restrict__ cov_ok,
+                                                      int64_t max_out, unsigned long long* n_out) {
+    const int lane = threadIdx.x & 31;
+    const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+    Entry e;
+    e.key = KEY_EMPTY; e.count = 0;
+    if (s < m.slots) e = m.table[s];
+    const bool live = e.key != KEY_EMPTY && e.count > 0;
+    const unsigned b = __ballot_sync(FULL, live);
+    if (!b) return;
+    unsigned long long base = 0;
+    if (lane == 0) base = atomicAdd(n_out, (unsigned long long)__popc(b));
+    base = __shfl_sync(FULL, base, 0);
+    const unsigned long long row = base + __popc(b & ((1u << lane) - 1u));
+    if (live && (int64_t)row < max_out) {
+        keys[row] = e.key;
+        counts[row] = (int32_t)e.count;
+    }
+    // cooperative copy of each live bucket of this warp
+    unsigned rem = b;
+    while (rem) {
+        const int src = __ffs(rem) - 1;
+        rem &= rem - 1;
+        const uint32_t ss = (blockIdx.x * blockDim.x + (threadIdx.x & ~31)) + src;
+        const uint32_t cnt = __shfl_sync(FULL, e.count, src);
+        const unsigned long long r = __shfl_sync(FULL, row, src);
+        if ((int64_t)r >= max_out) continue;
+        for (uint32_t j = lane; j < (uint32_t)m.cap; j += 32) {
+            const bool have = j < cnt;
+            const size_t from = (size_t)ss * m.cap + j, to = (size_t)r * m.cap + j;
+            if (pts) pts[to] = have ? m.points[from] : make_float4(0.f, 0.f, 0.f, __uint_as_float(NO_ID));
+            if (cov6) {
+                for (int a = 0; a < 6; ++a) cov6[to * 6 + a] = (have && m.cov) ? m.cov[from * 6 + a] : 0.f;
+            }
+            if (cov_ok) cov_ok[to] = (have && m.cov_ok) ? m.cov_ok[from] : 0;
+        }
+    }
+}
+
+__global__ void write_i64_kernel(const unsigned long long* src, int64_t* dst) {
+    if (threadIdx.x == 0 && blockIdx.x == 0) *dst = (int64_t)*src;
+}
+
+__global__ void __launch_bounds__(256) voxel_keys_kernel(const float* __restrict__ xyz, int64_t n, int stride, float v,
+                                                          unsigned long long* __restrict__ keys) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float* p = xyz + i * stride;
+    int k[3];
+    keys[i] = voxel_index(p[0], p[1], p[2], v, k) ? pack_key(k[0], k[1], k[2]) : KEY_EMPTY;
+}
+
+// ---- rehash: move the live voxels into a clean table (drops dead keys) --------------------------------------
+// pass 1 copies every live bucket into a compact temporary; pass 2 re-inserts them after the table was cleared
+__global__ void __launch_bounds__(256) rehash_gather_kernel(MapView m, unsigned long long* __restrict__ keys,
+                                                             uint32_t* __restrict__ counts, float4* __restrict__ pts,
+                                                             float* __restrict__ cov6, uint8_t* __restrict__ cov_ok,
+                                                             unsigned long long* n_out) {
+    const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= m.slots) return;
+    const Entry e = m.table[s];
+    if (e.key == KEY_EMPTY) return;
+    float4* bucket = m.points + (size_t)s * m.cap;
+    if (e.count > 0) {
+        const unsigned long long r = atomicAdd(n_out, 1ull);
+        keys[r] = e.key;
+        counts[r] = e.count;
+        for (uint32_t j = 0; j < e.count; ++j) {
+            const size_t from = (size_t)s * m.cap + j, to = (size_t)r * m.cap + j;
+            pts[to] = bucket[j];
+            if (m.cov) {
+                for (int a = 0; a < 6; ++a) cov6[to * 6 + a] = m.cov[from * 6 + a];
+                cov_ok[to] = m.cov_ok[from];
+            }
+        }
+    }
+    for (uint32_t j = 0; j < e.count; ++j) bucket[j].w = __uint_as_float(NO_ID);
+    Entry z;
+    z.key = KEY_EMPTY; z.count = 0; z.pad = 0;
+    m.table[s] = z;
+}
+
+__global__ void __launch_bounds__(256) rehash_scatter_kernel(MapView m, const unsigned long long* __restrict__ keys,
+                                                              const uint32_t* __restrict__ counts,
+                                                              const float4* __restrict__ pts, const float* __restrict__ cov6,
+                                                              const uint8_t* __restrict__ cov_ok,
+                                                              const unsigned long long* n_live) {
+    const unsigned long long r = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= *n_live) return;
+    const unsigned long long key = keys[r];
+    uint32_t s = hash_key(key) & m.mask;
+    for (uint32_t probes = 0; probes < m.slots; ++probes) {
+        if (atomicCAS(&m.table[s].key, KEY_EMPTY, key) == KEY_EMPTY) break;
+        s = (s + 1) & m.mask;
+    }
+    const uint32_t cnt = counts[r];
+    for (uint32_t j = 0; j < cnt; ++j) {
+        const size_t to = (size_t)s * m.cap + j, from = (size_t)r * m.cap + j;
+        m.points[to] = pts[from];
+        if (m.cov) {
+            for (int a = 0; a < 6; ++a) m.cov[to * 6 + a] = cov6[from * 6 + a];
+            m.cov_ok[to] = cov_ok[from];
+        }
+    }
+    m.table[s].count = cnt;
+    if (r == 0) m.ctr->n_keys = *n_live;
+}
+
+}  // namespace far
+
+// =============================================================================================================
+extern "C" {
+
+const char* far_strerror(int status) {
+    switch (status) {
+        case FAR_OK: return "ok";
+        case FAR_ERR_ARG: return "invalid argument";
+        case FAR_ERR_CUDA: return "CUDA runtime error";
+        case FAR_ERR_FULL: return "voxel table full";
+        case FAR_ERR_RANGE: return "point id counter out of range";
+        case FAR_ERR_DEGENERATE: return "degenerate registration (too few inliers or H not positive definite)";
+        default: return "unknown status";
+    }
+}
+
+const char* far_last_cuda_error(void) { return far::g_cuda_err; }
+
+int far_map_create(far_map_t** out, const far_map_config_t* cfg) {
+    if (!out || !cfg) return FAR_ERR_ARG;
+    *out = nullptr;
+    far_map_config_t c = *cfg;
+    if (!(c.voxel_size > 0.f) || c.cap < 1 || c.cap > 64 || c.max_voxels < 1) return FAR_ERR_ARG;
+    if (c.max_load == 0.f) c.max_load = 0.5f;
+    if (!(c.max_load > 0.f && c.max_load <= 0.9f)) return FAR_ERR_ARG;
+    if (c.k_cov == 0) c.k_cov = 10;
+    if (c.k_cov < 1 || c.k_cov > 32) return FAR_ERR_ARG;
+    if (c.cov_eps == 0.0) c.cov_eps = 1e-3;
+    if (c.max_batch == 0) c.max_batch = 1 << 20;
+    if (c.max_batch < 1 || c.max_batch > (1ll << 30)) return FAR_ERR_ARG;
+    uint64_t slots = 16;
+    const double want = (double)c.max_voxels / (double)c.max_load;
+    while ((double)slots < want) slots <<= 1;
+    if (slots * (uint64_t)c.cap >= (1ull << 32)) return FAR_ERR_ARG;   // refs (slot*cap+pos) are 32-bit
+
+    far_map* m = new (std::nothrow) far_map();
+    if (!m) return FAR_ERR_ARG;
+    memset(m, 0, sizeof(*m));
+    m->cfg = c;
+    m->max_batch = c.max_batch;
+    m->next_id = 0;
+    FAR_CUDA(cudaGetDevice(&m->device));
+    FAR_CUDA(cudaDeviceGetAttribute(&m->sm_count, cudaDevAttrMultiProcessorCount, m->device));
+    MapView& v = m->view;
+    v.slots = (uint32_t)slots;
+    v.mask = (uint32_t)slots - 1;
+    v.cap = c.cap;
+    v.k_cov = c.k_cov;
+    v.voxel = c.voxel_size;
+    v.cov_eps = c.cov_eps;
+    v.max_keys = (unsigned long long)c.max_voxels;
+    const size_t npts = (size_t)slots * c.cap;
+    cudaError_t e = cudaSuccess;
+    auto alloc = [&](void** p, size_t bytes) { if (e == cudaSuccess) e = cudaMalloc(p, bytes); };
+    alloc((void**)&v.table, slots * sizeof(Entry));
+    alloc((void**)&v.points, npts * sizeof(float4));
+    if (c.with_cov) {
+        alloc((void**)&v.cov, npts * 6 * sizeof(float));
+        alloc((void**)&v.cov_ok, npts);
+    }
+    alloc((void**)&v.ctr, sizeof(Counters) + 4 * sizeof(unsigned long long));
+    alloc((void**)&m->d_touched, (size_t)c.max_batch * 4);
+    alloc((void**)&m->d_cov_list, (size_t)c.max_batch * 4);
+    if (e != cudaSuccess) {
+        far::set_cuda_error(e, "cudaMalloc in far_map_create");
+        far_map_destroy(m);
+        return FAR_ERR_CUDA;
+    }
+    // empty table: every key = ~0, count = 0; every id word = FAR_NO_ID (0xFF bytes everywhere in the pool)
+    FAR_CUDA(cudaMemset(v.points, 0xFF, npts * sizeof(float4)));
+    table_init_kernel<<<grid_for((int64_t)slots, 256), 256>>>(v.table, v.slots);
+    FAR_CUDA(cudaGetLastError());
+    FAR_CUDA(cudaMemset(v.ctr, 0, sizeof(Counters) + 4 * sizeof(unsigned long long)));
+    if (v.cov_ok) FAR_CUDA(cudaMemset(v.cov_ok, 0, npts));
+    {
+        const int rc = gicp_setup(m);
+        if (rc != FAR_OK) { far_map_destroy(m); return rc; }
+    }
+    FAR_CUDA(cudaDeviceSynchronize());
+    *out = m;
+    return FAR_OK;
+}
+
+int far_map_destroy(far_map_t* m) {
+    if (!m) return FAR_OK;
+    cudaFree(m->view.table); cudaFree(m->view.points); cudaFree(m->view.cov); cudaFree(m->view.cov_ok);
+    cudaFree(m->view.ctr); cudaFree(m->d_touched); cudaFree(m->d_cov_list);
+    cudaFree(m->d_gicp_partials); cudaFree(m->d_gicp_state);
+    delete m;
+    return FAR_OK;
+}
+
+int far_map_clear(far_map_t* m, void* stream) {
+    if (!m) return FAR_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    clear_kernel<<<grid_for(m->view.slots, 256), 256, 0, st>>>(m->view);
+    FAR_CUDA(cudaGetLastError());
+    FAR_CUDA(cudaMemsetAsync(m->view.ctr, 0, sizeof(Counters), st));
+    m->next_id = 0;
+    return FAR_OK;
+}
+
+static int insert_impl(far_map_t* m, const float* d_xyz, int64_t n, int stride, int pose_mode, const far_pose_t* hpose,
+                       const far_pose_t* d_pose, int compute_cov, far_insert_stats_t* d_stats, void* stream) {
+    if (!m || (!d_xyz && n > 0) || n < 0 || (stride != 3 && stride != 4)) return FAR_ERR_ARG;
+    if (compute_cov && !m->view.cov) return FAR_ERR_ARG;
+    if (m->next_id + (uint64_t)n > 0xFFFFFFFFull) return FAR_ERR_RANGE;
+    cudaStream_t st = (cudaStream_t)stream;
+    Pose hp;
+    memset(&hp, 0, sizeof(hp));
+    if (pose_mode == 1) memcpy(&hp, hpose, sizeof(hp));
+    Counters* ctr = m->view.ctr;
+    // zero the per-call statistics and the covariance queue
+    FAR_CUDA(cudaMemsetAsync(&ctr->st_accepted, 0, 4 * sizeof(unsigned long long), st));
+    FAR_CUDA(cudaMemsetAsync(&ctr->n_cov, 0, sizeof(unsigned int), st));
+    const bool cov_by_list = compute_cov && n <= m->max_batch;
+    const uint32_t call_first_id = (uint32_t)m->next_id;
+    const int commit_grid = m->sm_count * 8;
+    for (int64_t off = 0; off < n; off += m->max_batch) {
+        const int64_t nc = (n - off < m->max_batch) ? n - off : m->max_batch;
+        const uint32_t first_id = (uint32_t)(m->next_id + (uint64_t)off);
+        const float* xyz = d_xyz + off * stride;
+        FAR_CUDA(cudaMemsetAsync(&ctr->n_touched, 0, sizeof(unsigned int), st));
+        insert_claim_chain_kernel<<<grid_for(nc, 256), 256, 0, st>>>(m->view, xyz, nc, stride, pose_mode, hp,
+                                                                      (const Pose*)d_pose, first_id, m->d_touched);
+        insert_commit_kernel<<<commit_grid, 256, 0, st>>>(m->view, xyz, stride, pose_mode, hp, (const Pose*)d_pose,
+                                                           first_id, m->d_touched, cov_by_list ? m->d_cov_list : nullptr,
+                                                           m->max_batch);
+        FAR_CUDA(cudaGetLastError());
+    }
+    m->next_id += (uint64_t)n;
+    if (compute_cov && n > 0) {
+        // "we recompute the covariances of the added points" -- against the map AFTER the insert
+        int rc = cov_by_list ? launch_knn_cov_refs(m, m->d_cov_list, &ctr->n_cov, n, st)
+                             : launch_knn_cov_new_ids(m, call_first_id, st);
+        if (rc != FAR_OK) return rc;
+    }
+    if (d_stats) {
+        insert_stats_kernel<<<1, 32, 0, st>>>(m->view, n, d_stats);
+        FAR_CUDA(cudaGetLastError());
+    }
+    return FAR_OK;
+}
+
+int far_map_insert(far_map_t* m, const float* d_xyz, int64_t n, int stride, const far_pose_t* pose, int compute_cov,
+                   far_insert_stats_t* d_stats, void* stream) {
+    return insert_impl(m, d_xyz, n, stride, pose ? 1 : 0, pose, nullptr, compute_cov, d_stats, stream);
+}
+
+int far_map_insert_dev(far_map_t* m, const float* d_xyz, int64_t n, int stride, const far_pose_t* d_pose,
+                       int compute_cov, far_insert_stats_t* d_stats, void* stream) {
+    if (!d_pose) return FAR_ERR_ARG;
+    return insert_impl(m, d_xyz, n, stride, 2, nullptr, d_pose, compute_cov, d_stats, stream);
+}
+
+static int prune_impl(far_map_t* m, const double* c, const far_pose_t* d_pose, double radius, far_prune_stats_t* d_stats,
+                      void* stream) {
+    if (!m || (!c && !d_pose)) return FAR_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const double r2 = radius * radius;
+    prune_kernel<<<grid_for(m->view.slots, 256), 256, 0, st>>>(m->view, c ? c[0] : 0.0, c ? c[1] : 0.0, c ? c[2] : 0.0,
+                                                                (const Pose*)d_pose, r2);
+    prune_stats_kernel<<<1, 32, 0, st>>>(m->view, d_stats);
+    FAR_CUDA(cudaGetLastError());
+    return FAR_OK;
+}
+
+int far_map_prune(far_map_t* m, const double center[3], double radius, far_prune_stats_t* d_stats, void* stream) {
+    if (!center) return FAR_ERR_ARG;
+    return prune_impl(m, center, nullptr, radius, d_stats, stream);
+}
+
+int far_map_prune_dev(far_map_t* m, const far_pose_t* d_pose, double radius, far_prune_stats_t* d_stats, void* stream) {
+    if (!d_pose) return FAR_ERR_ARG;
+    return prune_impl(m, nullptr, d_pose, radius, d_stats, stream);
+}
+
+int far_map_stats(far_map_t* m, far_map_stats_t* d_stats, void* stream) {
+    if (!m || !d_stats) return FAR_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned long long* acc = reinterpret_cast<unsigned long long*>(m->view.ctr + 1);
+    stats_kernel<<<grid_for(m->view.slots, 256), 256, 0, st>>>(m->view, acc);
+    stats_out_kernel<<<1, 32, 0, st>>>(m->view, acc, m->next_id, d_stats);
+    FAR_CUDA(cudaGetLastError());
+    return FAR_OK;
+}
+
+int far_map_export(far_map_t* m, uint64_t* d_keys, int32_t* d_counts, float* d_points4, float* d_cov6,
+                   uint8_t* d_cov_valid, int64_t max_out, int64_t* d_n_voxels, void* stream) {
+    if (!m || !d_keys || !d_counts || !d_n_voxels || max_out < 0) return FAR_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned long long* acc = reinterpret_cast<unsigned long long*>(m->view.ctr + 1) + 3;
+    FAR_CUDA(cudaMemsetAsync(acc, 0, sizeof(unsigned long long), st));
+    export_kernel<<<grid_for(m->view.slots, 256), 256, 0, st>>>(m->view, (unsigned long long*)d_keys, d_counts,
+                                                                 (float4*)d_points4, d_cov6, d_cov_valid, max_out, acc);
+    write_i64_kernel<<<1, 32, 0, st>>>(acc, d_n_voxels);
+    FAR_CUDA(cudaGetLastError());
+    return FAR_OK;
+}
+
+int far_voxel_keys(const float* d_xyz, int64_t n, int stride, float voxel, uint64_t* d_keys, void* stream) {
+    if ((!d_xyz && n > 0) || n < 0 || (stride != 3 && stride != 4) || !(voxel > 0.f) || (!d_keys && n > 0)) return FAR_ERR_ARG;
+    if (n == 0) return FAR_OK;
+    voxel_keys_kernel<<<grid_for(n, 256), 256, 0, (cudaStream_t)stream>>>(d_xyz, n, stride, voxel,
+                                                                          (unsigned long long*)d_keys);
+    FAR_CUDA(cudaGetLastError());
+    return FAR_OK;
+}
+
+// Maintenance call (not on the per-frame hot path): allocates a compact temporary for the live voxels,
+// synchronises the stream once to learn their number, and frees the temporary before returning.
+int far_map_rehash(far_map_t* m, void* stream) {
+    if (!m) return FAR_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    far_map_stats_t hs;
+    far_map_stats_t* d_hs = nullptr;
+    FAR_CUDA(cudaMalloc((void**)&d_hs, sizeof(hs)));
+    int rc = far_map_stats(m, d_hs, stream);
+    if (rc != FAR_OK) { cudaFree(d_hs); return rc; }
+    FAR_CUDA(cudaMemcpyAsync(&hs, d_hs, sizeof(hs), cudaMemcpyDeviceToHost, st));
+    FAR_CUDA(cudaStreamSynchronize(st));
+    cudaFree(d_hs);
+    const size_t nv = (size_t)hs.n_voxels, cap = (size_t)m->view.cap;
+    unsigned long long *t_keys = nullptr, *t_n = nullptr;
+    uint32_t* t_counts = nullptr;
+    float4* t_pts = nullptr;
+    float* t_cov = nullptr;
+    uint8_t* t_ok = nullptr;
+    cudaError_t e = cudaMalloc((void**)&t_keys, (nv + 1) * 8);
+    if (e == cudaSuccess) e = cudaMalloc((void**)&t_counts, (nv + 1) * 4);
+    if (e == cudaSuccess) e = cudaMalloc((void**)&t_pts, (nv * cap + 1) * sizeof(float4));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&t_n, 8);
+    if (e == cudaSuccess && m->view.cov) e = cudaMalloc((void**)&t_cov, (nv * cap + 1) * 6 * sizeof(float));
+    if (e == cudaSuccess && m->view.cov) e = cudaMalloc((void**)&t_ok, nv * cap + 1);
+    if (e == cudaSuccess) e = cudaMemsetAsync(t_n, 0, 8, st);
+    if (e == cudaSuccess) {
+        rehash_gather_kernel<<<grid_for(m->view.slots, 256), 256, 0, st>>>(m->view, t_keys, t_counts, t_pts, t_cov, t_ok, t_n);
+        if (nv > 0)
+            rehash_scatter_kernel<<<grid_for((int64_t)nv, 256), 256, 0, st>>>(m->view, t_keys, t_counts, t_pts, t_cov, t_ok, t_n);
+        else
+            e = cudaMemsetAsync(&m->view.ctr->n_keys, 0, 8, st);
+        if (e == cudaSuccess) e = cudaGetLastError();
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    }
+    cudaFree(t_keys); cudaFree(t_counts); cudaFree(t_pts); cudaFree(t_n); cudaFree(t_cov); cudaFree(t_ok);
+    if (e != cudaSuccess) { far::set_cuda_error(e, "far_map_rehash"); return FAR_ERR_CUDA; }
+    return FAR_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,301 @@
+// far_query.cu -- 27-voxel nearest neighbour (A6) and k-nearest covariance (A7), one warp per query.
+//
+// PAPER.md:62 "the algorithm searches the voxel containing it as well as all surrounding ones (27 in total)",
+// PAPER.md:80 "closest Euclidean neighbor" (k = 1), PAPER.md:68-76 (k = 10 -> Eq. 1).
+//
+// Warp-cooperative design: lanes 0..26 each probe one neighbour voxel (27 independent hash lookups in flight
+// at once), the counts are prefix-summed across the warp, and the warp then sweeps the *flattened* candidate
+// list 32 points at a time -- consecutive lanes read consecutive float4 of a bucket, so the gathers coalesce and
+// no lane idles on a half-empty voxel.  Distances are FP64 with a fixed operation order (R6) so the arg-min is
+// bit-identical to the definition; the arg-min itself is three redux.sync steps.
+#include "far_internal.h"
+
+using namespace far;
+
+namespace far {
+
+constexpr int QWARPS = 8;   // warps (= queries in flight) per block
+
+// map flat candidate j -> (voxel v, position) with a monotone walk over the prefix array
+__device__ __forceinline__ uint32_t cand_ref(const int* s_off, const uint32_t* s_slot, int j, int& v, int cap) {
+    while (j >= s_off[v + 1]) ++v;
+    return s_slot[v] * (uint32_t)cap + (uint32_t)(j - s_off[v]);
+}
+
+// nearest stored point of q among the 27 voxels around it; every lane returns the warp-wide winner
+__device__ __forceinline__ Best warp_nearest(const MapView& m, float qx, float qy, float qz, const int k[3], int lane,
+                                             int* s_off, uint32_t* s_slot) {
+    const int total = probe27(m, k, lane, s_off, s_slot);
+    Best best;
+    best.d2 = __longlong_as_double(0x7FF0000000000000ll);
+    best.id = NO_ID;
+    best.ref = 0;
+    int v = 0;
+    for (int j = lane; j < total; j += 32) {
+        const uint32_t ref = cand_ref(s_off, s_slot, j, v, m.cap);
+        const float4 p = __ldg(m.points + ref);
+        const double d2 = dist2(qx, qy, qz, p.x, p.y, p.z);
+        const uint32_t id = __float_as_uint(p.w);
+        if (better(d2, id, best)) { best.d2 = d2; best.id = id; best.ref = ref; }
+    }
+    __syncwarp();
+    const int w = warp_argmin(best.d2, best.id);
+    best.d2 = __shfl_sync(FULL, best.d2, w);
+    best.id = __shfl_sync(FULL, best.id, w);
+    best.ref = __shfl_sync(FULL, best.ref, w);
+    return best;
+}
+
+__global__ void __launch_bounds__(QWARPS * 32) nn_kernel(MapView m, const float* __restrict__ q, int64_t n, int stride,
+                                                          uint32_t* __restrict__ out_id, float* __restrict__ out_d2) {
+    __shared__ int s_off[QWARPS][32];
+    __shared__ uint32_t s_slot[QWARPS][32];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const int64_t nwarps = (int64_t)gridDim.x * QWARPS;
+    for (int64_t i = (int64_t)blockIdx.x * QWARPS + wib; i < n; i += nwarps) {
+        const float* qq = q + i * stride;
+        const float qx = __ldg(qq), qy = __ldg(qq + 1), qz = __ldg(qq + 2);
+        int k[3];
+        uint32_t id = NO_ID;
+        float d2 = __int_as_float(0x7F800000);
+        if (voxel_index(qx, qy, qz, m.voxel, k)) {
+            const Best b = warp_nearest(m, qx, qy, qz, k, lane, s_off[wib], s_slot[wib]);
+            if (b.id != NO_ID) { id = b.id; d2 = __double2float_rn(b.d2); }
+        }
+        if (lane == 0) { out_id[i] = id; out_d2[i] = d2; }
+        __syncwarp();
+    }
+}
+
+// ---- A7: k nearest by (d2, id) -> Eq. 1 -----------------------------------------------------------------------
+// dynamic shared memory per warp: double d2[27*cap] | u32 id[27*cap] | int off[32] | u32 slot[32] | int sel[32]
+__host__ __device__ inline size_t knn_smem_per_warp(int cap) { return (size_t)27 * cap * 12 + 3 * 32 * 4; }
+
+// Eq. 1: C = Sigma_hat + eps I ; Sigma = (C^-1 / ||C^-1||_F)^-1 = ||C^-1||_F C.  FP64 throughout.
+__device__ __forceinline__ bool regularised_cov(const double sc[6], double eps, float out[6]) {
+    const double a0 = sc[0] + eps, a1 = sc[1], a2 = sc[2], a4 = sc[3] + eps, a5 = sc[4], a8 = sc[5] + eps;
+    // symmetric: a3 = a1, a6 = a2, a7 = a5
+    const double c00 = a4 * a8 - a5 * a5;
+    const double c01 = a5 * a2 - a1 * a8;
+    const double c02 = a1 * a5 - a4 * a2;
+    const double det = a0 * c00 + a1 * c01 + a2 * c02;
+    if (!(det != 0.0) || !isfinite(det)) return false;
+    const double id = 1.0 / det;
+    const double i00 = c00 * id, i01 = c01 * id, i02 = c02 * id;
+    const double i11 = (a0 * a8 - a2 * a2) * id, i12 = (a2 * a1 - a0 * a5) * id, i22 = (a0 * a4 - a1 * a1) * id;
+    const double fro = sqrt(i00 * i00 + i11 * i11 + i22 * i22 + 2.0 * (i01 * i01 + i02 * i02 + i12 * i12));
+    out[0] = (float)(fro * a0); out[1] = (float)(fro * a1); out[2] = (float)(fro * a2);
+    out[3] = (float)(fro * a4); out[4] = (float)(fro * a5); out[5] = (float)(fro * a8);
+    return true;
+}
+
+// one query by one warp; all lanes return the same (valid, cov)
+__device__ __forceinline__ bool warp_knn_cov(const MapView& m, float qx, float qy, float qz, int lane, char* smem_w,
+                                             float cov[6]) {
+    const int cap = m.cap, kk = m.k_cov;
+    double* s_d2 = reinterpret_cast<double*>(smem_w);
+    uint32_t* s_id = reinterpret_cast<uint32_t*>(smem_w + (size_t)27 * cap * 8);
+    int* s_off = reinterpret_cast<int*>(smem_w + (size_t)27 * cap * 12);
+    uint32_t* s_slot = reinterpret_cast<uint32_t*>(s_off + 32);
+    int* s_sel = reinterpret_cast<int*>(s_off + 64);
+    cov[0] = 1.f; cov[1] = 0.f; cov[2] = 0.f; cov[3] = 1.f; cov[4] = 0.f; cov[5] = 1.f;
+    int k[3];
+    if (!voxel_index(qx, qy, qz, m.voxel, k)) return false;
+    const int total = probe27(m, k, lane, s_off, s_slot);
+    if (total < kk) { __syncwarp(); return false; }
+    const double INF = __longlong_as_double(0x7FF0000000000000ll);
+    // stage (d2, id) of every candidate; lane owns candidates j = lane, lane+32, ... and tracks its local minimum
+    double bd = INF; uint32_t bid = NO_ID; int bj = -1;
+    int v = 0;
+    for (int j = lane; j < total; j += 32) {
+        const uint32_t ref = cand_ref(s_off, s_slot, j, v, cap);
+        const float4 p = __ldg(m.points + ref);
+        const double d2 = dist2(qx, qy, qz, p.x, p.y, p.z);
+        const uint32_t id = __float_as_uint(p.w);
+        s_d2[j] = d2;
+        s_id[j] = id;
+        if (d2 < bd || (d2 == bd && id < bid)) { bd = d2; bid = id; bj = j; }
+    }
+    __syncwarp();
+    // k rounds of warp arg-min; only the winning lane rescans its own candidates
+    for (int r = 0; r < kk; ++r) {
+        const int w = warp_argmin(bd, bid);
+        const int wj = __shfl_sync(FULL, bj, w);
+        if (lane == 0) s_sel[r] = wj;
+        if (lane == w) {
+            s_d2[bj] = INF;
+            s_id[bj] = NO_ID;
+            bd = INF; bid = NO_ID; bj = -1;
+            for (int j = lane; j < total; j += 32) {
+                const double d2 = s_d2[j];
+                const uint32_t id = s_id[j];
+                if (id != NO_ID && (d2 < bd || (d2 == bd && id < bid))) { bd = d2; bid = id; bj = j; }
+            }
+        }
+        __syncwarp();
+    }
+    // lanes r < k fetch the r-th neighbour again (L1/L2 hit); mean and centred sums in neighbour order (R7: 1/k)
+    double px = 0.0, py = 0.0, pz = 0.0;
+    if (lane < kk) {
+        int vv = 0;
+        const uint32_t ref = cand_ref(s_off, s_slot, s_sel[lane], vv, cap);
+        const float4 p = __ldg(m.points + ref);
+        px = p.x; py = p.y; pz = p.z;
+    }
+    double mx = 0.0, my = 0.0, mz = 0.0;
+    for (int r = 0; r < kk; ++r) {
+        mx += __shfl_sync(FULL, px, r); my += __shfl_sync(FULL, py, r); mz += __shfl_sync(FULL, pz, r);
+    }
+    mx /= (double)kk; my /= (double)kk; mz /= (double)kk;
+    const double dx = px - mx, dy = py - my, dz = pz - mz;
+    double sc[6] = {0, 0, 0, 0, 0, 0};
+    for (int r = 0; r < kk; ++r) {
+        const double x = __shfl_sync(FULL, dx, r), y = __shfl_sync(FULL, dy, r), z = __shfl_sync(FULL, dz, r);
+        sc[0] += x * x; sc[1] += x * y; sc[2] += x * z; sc[3] += y * y; sc[4] += y * z; sc[5] += z * z;
+    }
+#pragma unroll
+    for (int a = 0; a < 6; ++a) sc[a] /= (double)kk;
+    __syncwarp();
+    float out[6];
+    if (!regularised_cov(sc, m.cov_eps, out)) return false;
+#pragma unroll
+    for (int a = 0; a < 6; ++a) cov[a] = out[a];
+    return true;
+}
+
+// queries given as points (far_map_knn_cov); n read from the device if d_n != nullptr
+__global__ void knn_cov_points_kernel(MapView m, const float* __restrict__ q, int64_t n, const int64_t* __restrict__ d_n,
+                                      int stride, float* __restrict__ cov6, uint8_t* __restrict__ valid, int warps_per_block) {
+    extern __shared__ __align__(16) char smem[];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    char* smem_w = smem + (size_t)wib * knn_smem_per_warp(m.cap);
+    if (d_n) n = min(n, *d_n);
+    const int64_t nwarps = (int64_t)gridDim.x * warps_per_block;
+    for (int64_t i = (int64_t)blockIdx.x * warps_per_block + wib; i < n; i += nwarps) {
+        const float* qq = q + i * stride;
+        float c[6];
+        const bool ok = warp_knn_cov(m, __ldg(qq), __ldg(qq + 1), __ldg(qq + 2), lane, smem_w, c);
+        if (lane < 6) cov6[i * 6 + lane] = c[lane];
+        if (lane == 0) valid[i] = ok ? 1 : 0;
+    }
+}
+
+// queries = stored points named by refs (covariances of the points an insert accepted)
+__global__ void knn_cov_refs_kernel(MapView m, const uint32_t* __restrict__ refs, const unsigned int* __restrict__ d_n,
+                                    int warps_per_block) {
+    extern __shared__ __align__(16) char smem[];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    char* smem_w = smem + (size_t)wib * knn_smem_per_warp(m.cap);
+    const int64_t n = *d_n;
+    const int64_t nwarps = (int64_t)gridDim.x * warps_per_block;
+    for (int64_t i = (int64_t)blockIdx.x * warps_per_block + wib; i < n; i += nwarps) {
+        const uint32_t ref = refs[i];
+        const float4 p = m.points[ref];
+        float c[6];
+        const bool ok = warp_knn_cov(m, p.x, p.y, p.z, lane, smem_w, c);
+        if (lane < 6) m.cov[(size_t)ref * 6 + lane] = c[lane];
+        if (lane == 0) m.cov_ok[ref] = ok ? 1 : 0;
+    }
+}
+
+// same for calls larger than the covariance queue: every stored point with id >= first_id is a new point
+__global__ void knn_cov_new_ids_kernel(MapView m, uint32_t first_id, int warps_per_block) {
+    extern __shared__ __align__(16) char smem[];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    char* smem_w = smem + (size_t)wib * knn_smem_per_warp(m.cap);
+    const int64_t nwarps = (int64_t)gridDim.x * warps_per_block;
+    for (int64_t s = (int64_t)blockIdx.x * warps_per_block + wib; s < m.slots; s += nwarps) {
+        const Entry e = m.table[s];
+        if (e.key == KEY_EMPTY || e.count == 0) continue;
+        for (uint32_t j = 0; j < e.count; ++j) {
+            const uint32_t ref = (uint32_t)s * m.cap + j;
+            const float4 p = m.points[ref];
+            if (__float_as_uint(p.w) < first_id) continue;
+            float c[6];
+            const bool ok = warp_knn_cov(m, p.x, p.y, p.z, lane, smem_w, c);
+            if (lane < 6) m.cov[(size_t)ref * 6 + lane] = c[lane];
+            if (lane == 0) m.cov_ok[ref] = ok ? 1 : 0;
+        }
+    }
+}
+
+struct KnnLaunch { int warps, grid; size_t smem; };
+
+template <class K>
+static int knn_launch_cfg(const far_map* map, K kernel, int64_t work, KnnLaunch& L) {
+    const size_t per_warp = knn_smem_per_warp(map->view.cap);
+    int warps = (int)(100 * 1024 / per_warp);
+    if (warps > 8) warps = 8;
+    if (warps < 1) warps = 1;
+    L.warps = warps;
+    L.smem = per_warp * warps;
+    FAR_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem));
+    int per_sm = 0;
+    FAR_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, warps * 32, L.smem));
+    if (per_sm < 1) per_sm = 1;
+    int64_t grid = (int64_t)map->sm_count * per_sm;
+    const int64_t need = (work + warps - 1) / warps;
+    if (need < grid) grid = need;
+    if (grid < 1) grid = 1;
+    L.grid = (int)grid;
+    return FAR_OK;
+}
+
+int launch_knn_cov_refs(const far_map* map, const uint32_t* d_refs, const unsigned int* d_n, int64_t n_max, cudaStream_t st) {
+    KnnLaunch L;
+    int rc = knn_launch_cfg(map, knn_cov_refs_kernel, n_max, L);
+    if (rc != FAR_OK) return rc;
+    knn_cov_refs_kernel<<<L.grid, L.warps * 32, L.smem, st>>>(map->view, d_refs, d_n, L.warps);
+    FAR_CUDA(cudaGetLastError());
+    return FAR_OK;
+}
+
+int launch_knn_cov_new_ids(const far_map* map, uint32_t first_id, cudaStream_t st) {
+    KnnLaunch L;
+    int rc = knn_launch_cfg(map, knn_cov_new_ids_kernel, map->view.slots, L);
+    if (rc != FAR_OK) return rc;
+    knn_cov_new_ids_kernel<<<L.grid, L.warps * 32, L.smem, st>>>(map->view, first_id, L.warps);
+    FAR_CUDA(cudaGetLastError());
+    return FAR_OK;
+}
+
+}  // namespace far
+
+extern "C" {
+
+int far_map_nn(const far_map_t* map, const float* d_q, int64_t m, int stride, uint32_t* d_id, float* d_d2, void* stream) {
+    if (!map || m < 0 || (stride != 3 && stride != 4) || (m > 0 && (!d_q || !d_id || !d_d2))) return FAR_ERR_ARG;
+    if (m == 0) return FAR_OK;
+    int64_t grid = (int64_t)map->sm_count * 8;   // 8 blocks x 8 warps = 64 warps per SM: one full wave
+    const int64_t need = (m + QWARPS - 1) / QWARPS;
+    if (need < grid) grid = need;
+    nn_kernel<<<(int)grid, QWARPS * 32, 0, (cudaStream_t)stream>>>(map->view, d_q, m, stride, d_id, d_d2);
+    FAR_CUDA(cudaGetLastError());
+    return FAR_OK;
+}
+
+static int knn_cov_impl(const far_map_t* map, const float* d_q, int64_t m, const int64_t* d_m, int stride, float* d_cov6,
+                        uint8_t* d_valid, void* stream) {
+    if (!map || m < 0 || (stride != 3 && stride != 4) || (m > 0 && (!d_q || !d_cov6 || !d_valid))) return FAR_ERR_ARG;
+    if (m == 0) return FAR_OK;
+    KnnLaunch L;
+    int rc = knn_launch_cfg(map, knn_cov_points_kernel, m, L);
+    if (rc != FAR_OK) return rc;
+    knn_cov_points_kernel<<<L.grid, L.warps * 32, L.smem, (cudaStream_t)stream>>>(map->view, d_q, m, d_m, stride, d_cov6,
+                                                                                  d_valid, L.warps);
+    FAR_CUDA(cudaGetLastError());
+    return FAR_OK;
+}
+
+int far_map_knn_cov(const far_map_t* map, const float* d_q, int64_t m, int stride, float* d_cov6, uint8_t* d_valid,
+                    void* stream) {
+    return knn_cov_impl(map, d_q, m, nullptr, stride, d_cov6, d_valid, stream);
+}
+
+int far_map_knn_cov_dev(const far_map_t* map, const float* d_q, const int64_t* d_m, int64_t m_max, int stride,
+                        float* d_cov6, uint8_t* d_valid, void* stream) {
+    if (!d_m) return FAR_ERR_ARG;
+    return knn_cov_impl(map, d_q, m_max, d_m, stride, d_cov6, d_valid, stream);
+}
+
+}  // extern "C"

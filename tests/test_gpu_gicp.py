@@ -1,0 +1,273 @@
+"""GPU parity: k-NN covariances (Eq. 1), one GICP linearisation (H, b) and the registration loop -- CUDA path
+through the C ABI vs the FP64 CPU oracle.  Tolerances are BASELINE.json's north_star: covariance valid flags
+bit-exact, Sigma and H/b within 1e-4 relative, converged poses within 1e-4 m / 1e-5 rad."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import far_scenes as scenes
+import oracle
+from helpers import load_golden, rot_angle
+
+pytestmark = pytest.mark.gpu
+
+far = pytest.importorskip("paper_2606_26010_b200")
+
+KERNELS = [oracle.KERNEL_CAUCHY, oracle.KERNEL_GEMAN_MCCLURE, oracle.KERNEL_NONE]
+
+
+def _rel_cov(a, b):
+    a, b = a.astype(np.float64), b.astype(np.float64)
+    return np.linalg.norm(a - b, axis=-1) / np.linalg.norm(b, axis=-1)
+
+
+def _hb_err(g, o, scale_b):
+    eh = np.linalg.norm(g["H"] - o["H"]) / np.linalg.norm(o["H"])
+    eb = np.linalg.norm(g["b"] - o["b"]) / max(np.linalg.norm(o["b"]), 1e-3 * scale_b)
+    return eh, eb
+
+
+def _pose_err(g, o):
+    dt = np.linalg.norm(g["t"] - o["t"])
+    dr = rot_angle(g["R"].T @ o["R"])
+    return dt, dr
+
+
+def _build_pair(map_points, voxel, cap, max_voxels=None):
+    mo = oracle.Map(voxel, cap)
+    mg = far.Map(voxel, cap, max_voxels or 4 * len(map_points) + 1024, with_cov=True)
+    so = mo.insert(map_points, compute_cov=True)
+    sg = mg.insert(map_points, compute_cov=True)
+    assert sg == so
+    return mo, mg
+
+
+def _scan_cov(scan_raw, scan_ds, voxel, cap):
+    """Sigma_s from a scan-local map built from the raw scan, on both sides."""
+    lo = oracle.Map(voxel, cap)
+    lo.insert(scan_raw)
+    cov_o, val_o = lo.knn_cov(scan_ds, nthreads=8)
+    lg = far.Map(voxel, cap, 4 * len(scan_raw) + 1024)
+    lg.insert(scan_raw)
+    cov_g, val_g = lg.knn_cov(scan_ds)
+    return (cov_o, val_o), (cov_g, val_g)
+
+
+# ---- A7 ---------------------------------------------------------------------------------------------------
+def test_cov_closed_form_golden():
+    g = load_golden("cov_eq1_closed_form.json")
+    # eight points (the corners (+-a, +-a, 0), twice) whose 1/k sample covariance is diag(0.1, 0.1, 0)
+    a = math.sqrt(0.1)
+    corners = np.array([[a, a, 0], [a, -a, 0], [-a, a, 0], [-a, -a, 0]], dtype=np.float64)
+    pts = (np.concatenate([corners, corners]) + 1.0).astype(np.float32)      # all inside voxel (0,0,0) of a 4 m grid
+    mg = far.Map(4.0, 20, 64, k_cov=8, cov_eps=g["eps"])
+    mg.insert(pts)
+    cov, valid = mg.knn_cov(pts[:1])
+    assert int(valid[0]) == 1
+    c = cov[0].cpu().numpy().astype(np.float64)
+    S = np.array([[c[0], c[1], c[2]], [c[1], c[3], c[4]], [c[2], c[4], c[5]]])
+    assert np.allclose(np.sort(np.linalg.eigvalsh(S)), np.sort(g["eig_sigma"]), rtol=1e-5)
+    assert np.linalg.norm(np.linalg.inv(S)) == pytest.approx(1.0, rel=1e-5)        # ||Sigma^-1||_F = 1 (Eq. 1)
+    # fewer than k neighbours -> invalid, identity
+    mg2 = far.Map(4.0, 20, 64, k_cov=10)
+    mg2.insert(pts)
+    cov, valid = mg2.knn_cov(pts[:1])
+    assert int(valid[0]) == 0 and cov[0].tolist() == [1, 0, 0, 1, 0, 1]
+
+
+@pytest.mark.parametrize("voxel,cap,k", [(0.5, 20, 10), (1.0, 20, 10), (1.0, 40, 10), (0.5, 4, 5)])
+def test_knn_cov_matches_oracle(voxel, cap, k):
+    c1 = scenes.c1_tiny(seed=3, n_map=20_000, n_scan=3001)
+    mo = oracle.Map(voxel, cap, k_cov=k)
+    mg = far.Map(voxel, cap, 100_000, k_cov=k)
+    mo.insert(c1["map_points"]); mg.insert(c1["map_points"])
+    rng = np.random.default_rng(1)
+    q = np.concatenate([c1["map_points"][:2000], scenes.pose_apply(c1["T_gt"], c1["scan"]),
+                        rng.uniform(-8, 8, (500, 3)).astype(np.float32)]).astype(np.float32)
+    cov_o, val_o = mo.knn_cov(q, nthreads=8)
+    cov_g, val_g = mg.knn_cov(q)
+    assert np.array_equal(val_g.cpu().numpy(), val_o)
+    assert val_o.any() and not val_o.all()
+    v = val_o.astype(bool)
+    assert _rel_cov(cov_g.cpu().numpy()[v], cov_o[v]).max() < 1e-4
+    assert np.array_equal(cov_g.cpu().numpy()[~v], cov_o[~v])              # identity where invalid
+
+
+def test_insert_compute_cov_matches_oracle_across_batches():
+    c1 = scenes.c1_tiny(seed=4, n_map=30_000)
+    pts = c1["map_points"]
+    mo, mg = oracle.Map(0.5, 20), far.Map(0.5, 20, 100_000, with_cov=True)
+    for a, b in [(0, 10_000), (10_000, 10_001), (10_001, 30_000)]:      # covariances are NOT batch invariant: replay
+        so = mo.insert(pts[a:b], compute_cov=True)
+        sg = mg.insert(pts[a:b], compute_cov=True)
+        assert sg == so
+    eo, eg = mo.export(with_cov=True), mg.export(with_cov=True)
+    assert np.array_equal(eg["keys"], eo["keys"]) and np.array_equal(eg["ids"], eo["ids"])
+    assert np.array_equal(eg["cov_valid"], eo["cov_valid"])
+    v = eo["cov_valid"].astype(bool)
+    assert v.any()
+    assert _rel_cov(eg["cov"][v], eo["cov"][v]).max() < 1e-4
+    # the oversize path (call larger than the covariance queue) gives the same covariances
+    mc = far.Map(0.5, 20, 100_000, with_cov=True, max_batch=4096)
+    for a, b in [(0, 10_000), (10_000, 10_001), (10_001, 30_000)]:
+        mc.insert(pts[a:b], compute_cov=True)
+    ec = mc.export(with_cov=True)
+    assert np.array_equal(ec["cov_valid"], eo["cov_valid"])
+    assert _rel_cov(ec["cov"][v], eo["cov"][v]).max() < 1e-4
+
+
+# ---- A8-A10 ----------------------------------------------------------------------------------------------
+def test_single_correspondence_and_robust_weight_golden():
+    g = load_golden("gicp_single_correspondence.json")
+    mg = far.Map(0.5, 20, 64, with_cov=True)
+    mg.insert(np.array([g["r"]], dtype=np.float32))
+    scan = np.array([g["p"]], dtype=np.float32)
+    res = mg.gicp_linearize(scan, None, None, scenes.pose_identity(), 2.0, far.default_options(kernel=far.KERNEL_NONE))
+    assert res["n_inliers"] == 1 and res["iters"] == 1
+    assert np.allclose(res["H"], np.array(g["H"], dtype=np.float64), atol=1e-7)
+    assert np.allclose(res["b"], np.array(g["b"]), atol=1e-7)
+    # robust weights (Eq. 5 and the kernel of [1]): M = I, e2 = |d|^2 = 0.01, sigma = 1 -> kappa = 1/3; H[0,0] = w
+    w = load_golden("robust_weights.json")
+    for kernel, name in [(far.KERNEL_CAUCHY, "cauchy"), (far.KERNEL_GEMAN_MCCLURE, "geman_mcclure"), (far.KERNEL_NONE, "none")]:
+        res = mg.gicp_linearize(scan, None, None, scenes.pose_identity(), 1.0, far.default_options(kernel=kernel))
+        e2 = float(np.float32(0.1)) ** 2
+        want = {"cauchy": 1 / (1 + e2 * 9), "geman_mcclure": (1 / 9) / (1 / 3 + e2) ** 2, "none": 1.0}[name]
+        assert res["H"][0, 0] == pytest.approx(want, rel=1e-12)
+        assert res["H"][0, 0] == pytest.approx(w[name], rel=1e-6)
+    # gate: tau = 3 sigma; sigma = 0.03 -> tau = 0.09 < 0.1 rejects the only correspondence
+    res = mg.gicp_linearize(scan, None, None, scenes.pose_identity(), 0.03)
+    assert res["n_inliers"] == 0 and np.all(res["H"] == 0)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("sigma", [2.0, 0.15])
+def test_linearize_matches_oracle_c1(kernel, sigma):
+    c1 = scenes.c1_tiny(seed=0)
+    mo, mg = _build_pair(c1["map_points"], c1["voxel"], c1["cap"])
+    (cov_o, val_o), (cov_g, val_g) = _scan_cov(c1["scan"], c1["scan"], c1["voxel"], c1["cap"])
+    assert np.array_equal(val_g.cpu().numpy(), val_o)
+    opts_o, opts_g = oracle.default_options(kernel=kernel), far.default_options(kernel=kernel)
+    rng = np.random.default_rng(2)
+    poses = [c1["T_init"], c1["T_gt"], scenes.perturb_pose(c1["T_gt"], 0.05, 0.3, rng)]
+    for T in poses:
+        o = mo.gicp_linearize(c1["scan"], cov_o, val_o, T, sigma, opts_o)
+        g = mg.gicp_linearize(c1["scan"], cov_g, val_g, T, sigma, opts_g)
+        assert g["n_inliers"] == o["n_inliers"] and o["n_inliers"] > 0
+        corr = mo.gicp_correspondences(c1["scan"], cov_o, val_o, T, sigma, opts_o)
+        # scale for b: sum of the per-correspondence gradient norms (b itself -> 0 at convergence)
+        d = corr["r"] - corr["p"]
+        Md = np.einsum("nij,nj->ni", corr["M"], d)
+        scale_b = float(np.sum(corr["w"][corr["used"]] * np.linalg.norm(Md[corr["used"]], axis=1)))
+        eh, eb = _hb_err(g, o, scale_b)
+        assert eh < 1e-4 and eb < 1e-4, (eh, eb)
+        assert g["chi2"] == pytest.approx(o["chi2"], rel=1e-6)
+        if sigma < 1.0:
+            assert o["n_inliers"] < len(c1["scan"])          # the gate rejects something
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_register_matches_oracle_c1(kernel):
+    c1 = scenes.c1_tiny(seed=0)
+    mo, mg = _build_pair(c1["map_points"], c1["voxel"], c1["cap"])
+    (cov_o, val_o), (cov_g, val_g) = _scan_cov(c1["scan"], c1["scan"], c1["voxel"], c1["cap"])
+    # fixed point (eps = 1e-6): both sides sit at the same minimum
+    oo, og = oracle.default_options(kernel=kernel, conv_eps=1e-6), far.default_options(kernel=kernel, conv_eps=1e-6)
+    o = mo.gicp_register(c1["scan"], cov_o, val_o, c1["T_init"], c1["sigma"], c1["max_iters"], oo, nthreads=8)
+    g = mg.gicp_register(c1["scan"], cov_g, val_g, c1["T_init"], c1["sigma"], c1["max_iters"], og)
+    assert g["status"] == o["status"] == 0
+    dt, dr = _pose_err(g, o)
+    assert dt < 1e-4 and dr < 1e-5, (dt, dr)
+    assert g["converged"] == o["converged"] and abs(g["iters"] - o["iters"]) <= 1
+    # the paper's eps = 5e-3: same iteration count, same pose
+    oo, og = oracle.default_options(kernel=kernel), far.default_options(kernel=kernel)
+    o = mo.gicp_register(c1["scan"], cov_o, val_o, c1["T_init"], c1["sigma"], c1["max_iters"], oo, nthreads=8)
+    g = mg.gicp_register(c1["scan"], cov_g, val_g, c1["T_init"], c1["sigma"], c1["max_iters"], og)
+    assert g["iters"] == o["iters"] and g["converged"] == o["converged"] == 1
+    dt, dr = _pose_err(g, o)
+    assert dt < 1e-4 and dr < 1e-5
+    assert g["n_inliers"] == o["n_inliers"]
+    eh, eb = _hb_err(g, o, np.linalg.norm(o["H"]))
+    assert eh < 1e-4
+    # and it found the ground truth to scan-noise level
+    dt, dr = _pose_err(g, dict(R=c1["T_gt"][0], t=c1["T_gt"][1]))
+    assert dt < 0.01 and dr < math.radians(0.1)
+
+
+def test_noise_free_recovery_and_point_to_point():
+    c1 = scenes.c1_tiny(seed=0, noise_free=True)
+    mo, mg = _build_pair(c1["map_points"], c1["voxel"], c1["cap"])
+    og = far.default_options(conv_eps=1e-9)
+    g = mg.gicp_register(c1["scan"], None, None, c1["T_init"], 2.0, 30, og)       # all covariances invalid -> SA fallback
+    o = mo.gicp_register(c1["scan"], None, None, c1["T_init"], 2.0, 30, oracle.default_options(conv_eps=1e-9))
+    dt, dr = _pose_err(g, o)
+    assert dt < 1e-6 and dr < 1e-7
+    dt, dr = _pose_err(g, dict(R=c1["T_gt"][0], t=c1["T_gt"][1]))
+    assert dt < 1e-5 and g["chi2"] < 1e-6
+
+
+def test_degenerate_and_max_iters():
+    c1 = scenes.c1_tiny(seed=0)
+    mo, mg = _build_pair(c1["map_points"], c1["voxel"], c1["cap"])
+    far_away = (c1["scan"] + np.float32(500.0)).astype(np.float32)
+    g = mg.gicp_register(far_away, None, None, c1["T_init"], 2.0, 30)
+    assert g["status"] == far.ERR_DEGENERATE and g["n_inliers"] == 0 and g["iters"] == 1
+    assert np.array_equal(g["R"], c1["T_init"][0]) and np.array_equal(g["t"], c1["T_init"][1])
+    # max_iters = 2 stops early, not converged, pose equals the oracle's second iterate
+    (cov_o, val_o), (cov_g, val_g) = _scan_cov(c1["scan"], c1["scan"], c1["voxel"], c1["cap"])
+    o = mo.gicp_register(c1["scan"], cov_o, val_o, c1["T_init"], 2.0, 2)
+    g = mg.gicp_register(c1["scan"], cov_g, val_g, c1["T_init"], 2.0, 2)
+    assert g["iters"] == o["iters"] == 2 and g["converged"] == o["converged"] == 0
+    dt, dr = _pose_err(g, o)
+    assert dt < 1e-7 and dr < 1e-8
+    # empty scan
+    g = mg.gicp_register(np.zeros((0, 3), np.float32), None, None, c1["T_init"], 2.0, 5)
+    assert g["status"] == far.ERR_DEGENERATE and g["n_inliers"] == 0
+
+
+def test_c2_reduced_frame_end_to_end_device_chain():
+    """A C2-shaped frame at reduced size (16 rings x 1024 azimuths, 200k-candidate map): voxelise -> Sigma_s ->
+    register -> insert at the registered pose -> prune, chained on the device without host synchronisation,
+    against the same steps on the oracle."""
+    c2 = scenes.c2_single_frame(seed=1, n_map_candidates=200_000, map_radius=60.0, rings=16, azimuths=1024)
+    v, cap, sigma = c2["voxel"], c2["cap"], c2["sigma"]
+    mo, mg = _build_pair(c2["map_points"], v, cap)
+    scan = c2["scan"]
+    # oracle side
+    ds_o, idx_o = oracle.voxelize(scan, v)
+    lo = oracle.Map(v, cap); lo.insert(scan)
+    cov_o, val_o = lo.knn_cov(ds_o, nthreads=8)
+    o = mo.gicp_register(ds_o, cov_o, val_o, c2["T_init"], sigma, 30, nthreads=8)
+    so = mo.insert(scan, pose=(o["R"], o["t"]), compute_cov=True)
+    po = mo.prune(o["t"], 40.0)
+    # device chain
+    n = len(scan)
+    d_scan = torch.as_tensor(scan).cuda()
+    vox = far.Voxelizer(n)
+    lg = far.Map(v, cap, 4 * n)
+    d_cov = torch.empty((n, 6), dtype=torch.float32, device="cuda")
+    d_val = torch.empty(n, dtype=torch.uint8, device="cuda")
+    d_init = torch.frombuffer(bytearray(bytes(far.Pose.from_rt(c2["T_init"]))), dtype=torch.uint8).cuda()
+    vox.enqueue(d_scan, v)
+    lg.insert_enqueue(d_scan)
+    lg.knn_cov(vox.out_xyz, out_cov=d_cov, out_valid=d_val, d_m=vox.n_out)
+    res = mg.gicp_register_enqueue(vox.out_xyz, d_cov, d_val, None, sigma, 30, d_n=vox.n_out, d_init_pose=d_init)
+    mg.insert_enqueue(d_scan, compute_cov=True, d_pose=res)            # the result struct starts with the pose
+    mg.prune_enqueue(radius=40.0, d_pose=res)
+    torch.cuda.synchronize()
+    g = far.result_to_dict(far.GicpResult.from_buffer_copy(res.cpu().numpy().tobytes()))
+    m = int(vox.n_out.item())
+    assert m == len(idx_o) and np.array_equal(vox.out_index[:m].cpu().numpy(), idx_o)
+    assert np.array_equal(d_val[:m].cpu().numpy(), val_o)
+    assert g["status"] == o["status"] == 0 and g["iters"] == o["iters"] and g["n_inliers"] == o["n_inliers"]
+    dt, dr = _pose_err(g, o)
+    assert dt < 1e-4 and dr < 1e-5, (dt, dr)
+    dt, dr = _pose_err(g, dict(R=c2["T_gt"][0], t=c2["T_gt"][1]))
+    assert dt < 0.1 and dr < math.radians(0.5), (dt, dr)
+    # the maps agree after insert + prune if the registered poses round the inserted points identically;
+    # poses agree to ~1e-12, so compare structure exactly and coordinates to 1e-5 m
+    eo, eg = mo.export(), mg.export()
+    assert np.array_equal(eg["keys"], eo["keys"]) and np.array_equal(eg["counts"], eo["counts"])
+    assert np.array_equal(eg["ids"], eo["ids"])
+    assert np.abs(eg["xyz"] - eo["xyz"]).max() < 1e-5

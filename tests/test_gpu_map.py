@@ -1,0 +1,300 @@
+"""GPU parity: voxel keys, voxelise, capped insert, prune, export, 27-voxel NN -- CUDA path (through the C ABI)
+vs the FP64 CPU oracle, element by element, bit-exact (integer / byte / index work)."""
+import numpy as np
+import pytest
+import torch
+
+import far_scenes as scenes
+import oracle
+from helpers import load_golden
+
+pytestmark = pytest.mark.gpu
+
+far = pytest.importorskip("paper_2606_26010_b200")
+
+
+def _cloud(rng, n, scale=20.0, clustered=True):
+    pts = rng.uniform(-scale, scale, size=(n, 3))
+    if clustered:   # a dense blob so that caps are hit
+        m = n // 3
+        pts[:m] = rng.normal(0.0, 0.6, size=(m, 3)) + np.array([3.0, -2.0, 1.0])
+    return pts.astype(np.float32)
+
+
+def _assert_same_map(g, o, with_cov=False):
+    assert np.array_equal(g["keys"], o["keys"])
+    assert np.array_equal(g["counts"], o["counts"])
+    assert np.array_equal(g["ids"], o["ids"])
+    assert np.array_equal(g["xyz"].view(np.uint32), o["xyz"].view(np.uint32))   # bit-exact coordinates
+    if with_cov:
+        assert np.array_equal(g["cov_valid"], o["cov_valid"])
+        v = o["cov_valid"].astype(bool)
+        a, b = g["cov"][v].astype(np.float64), o["cov"][v].astype(np.float64)
+        rel = np.linalg.norm(a - b, axis=1) / np.linalg.norm(b, axis=1)
+        assert rel.max() < 1e-4 if len(rel) else True
+
+
+# ---- A1 ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("voxel", [0.25, 0.5, 1.0, 2.0, 4.0, 0.3])
+def test_voxel_keys_bit_exact(voxel):
+    rng = np.random.default_rng(11)
+    pts = _cloud(rng, 100_003, scale=300.0)
+    pts[5] = [np.nan, 0, 0]
+    pts[6] = [0, np.inf, 0]
+    pts[7] = [3e7, 0, 0]            # voxel index out of +-2^20
+    pts[8] = [-0.0, 0.5, -0.5]
+    k_o, v_o = oracle.keys(pts, voxel)
+    k_g = far.voxel_keys(pts, voxel).cpu().numpy().view(np.uint64)
+    assert np.array_equal(k_g, k_o)
+    assert np.array_equal(k_g != np.uint64(0xFFFFFFFFFFFFFFFF), v_o)
+
+
+def test_voxel_keys_golden_and_stride4():
+    g = load_golden("key_examples.json")
+    for k3, hx in g["pack_cases"]:
+        k = np.array(k3, dtype=np.float64)
+        p = ((k + 0.5) * g["voxel"]).astype(np.float32)[None, :]       # voxel centre: exactly representable
+        p4 = np.concatenate([p, np.ones((1, 1), np.float32)], axis=1)
+        for arr in (p, p4):
+            got = int(far.voxel_keys(arr, g["voxel"]).cpu().numpy().view(np.uint64)[0])
+            assert got == int(hx, 16)
+    for x, want in g["floor_cases"]:
+        key = int(far.voxel_keys(np.array([[x, 0.0, 0.0]], dtype=np.float32), g["voxel"]).cpu().numpy().view(np.uint64)[0])
+        assert oracle.unpack_key(key)[0] == want
+
+
+# ---- A2 ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n,voxel", [(0, 1.0), (1, 1.0), (1023, 0.5), (1024, 0.5), (1025, 1.0), (77_777, 1.0), (300_000, 0.5)])
+def test_voxelize_bit_exact(n, voxel):
+    rng = np.random.default_rng(n + 1)
+    pts = _cloud(rng, n, scale=40.0)
+    if n > 10:
+        pts[3] = np.nan
+        pts[n // 2] = np.inf
+    o_xyz, o_idx = oracle.voxelize(pts, voxel) if n else (np.zeros((0, 3), np.float32), np.zeros(0, np.int32))
+    g_xyz, g_idx = far.voxelize(pts, voxel) if n else far.Voxelizer(8)(torch.zeros((0, 3), device="cuda"), voxel)
+    assert np.array_equal(g_idx.cpu().numpy(), o_idx)
+    assert np.array_equal(g_xyz.cpu().numpy().view(np.uint32), o_xyz.view(np.uint32))
+
+
+def test_voxelize_lidar_scan_and_idempotence():
+    c2 = scenes.c2_single_frame(seed=1, n_map_candidates=1000, rings=16, azimuths=512)
+    scan = c2["scan"]
+    o_xyz, o_idx = oracle.voxelize(scan, 1.0)
+    g_xyz, g_idx = far.voxelize(scan, 1.0)
+    assert np.array_equal(g_idx.cpu().numpy(), o_idx)
+    again, idx2 = far.voxelize(g_xyz, 1.0)
+    assert torch.equal(again, g_xyz) and np.array_equal(idx2.cpu().numpy(), np.arange(len(o_idx)))
+
+
+# ---- A3/A4 ------------------------------------------------------------------------------------------------
+def test_insert_golden_example():
+    g = load_golden("insert_worked_example.json")
+    m = far.Map(g["voxel"], g["cap"], 64)
+    st = m.insert(np.array(g["points"], dtype=np.float32))
+    e = m.export()
+    got = {int(k): [int(i) for i in e["ids"][v, :e["counts"][v]]] for v, k in enumerate(e["keys"])}
+    want = {oracle.pack_key(*map(int, k.split(","))): ids for k, ids in g["expect"].items()}
+    assert got == want
+    assert st["n_accepted"] == 3 and st["n_new_voxels"] == 2 and st["n_offered"] == 4
+
+
+@pytest.mark.parametrize("cap", [1, 4, 20, 33, 40])
+def test_insert_contents_bit_exact(cap):
+    rng = np.random.default_rng(100 + cap)
+    pts = _cloud(rng, 60_001, scale=15.0)
+    pts[17] = np.nan
+    mo = oracle.Map(0.5, cap)
+    mg = far.Map(0.5, cap, 200_000)
+    so = mo.insert(pts)
+    sg = mg.insert(pts)
+    assert sg == so
+    _assert_same_map(mg.export(), mo.export())
+    assert mg.size() == mo.size()
+
+
+def test_insert_batch_invariance_and_internal_chunking():
+    rng = np.random.default_rng(7)
+    pts = _cloud(rng, 50_000, scale=10.0)
+    mo = oracle.Map(0.5, 20)
+    so = mo.insert(pts)
+    ref = mo.export()
+    # many external batches of ragged sizes
+    mg = far.Map(0.5, 20, 100_000)
+    cuts = [0, 1, 33, 1000, 1001, 20_000, 49_999, 50_000]
+    for a, b in zip(cuts[:-1], cuts[1:]):
+        mg.insert(pts[a:b])
+    _assert_same_map(mg.export(), ref)
+    # one call that the library has to chunk internally (max_batch smaller than n)
+    mc = far.Map(0.5, 20, 100_000, max_batch=4096)
+    st = mc.insert(pts)
+    assert st == so
+    _assert_same_map(mc.export(), ref)
+
+
+def test_insert_with_pose_bit_exact_and_device_pose():
+    rng = np.random.default_rng(8)
+    pts = _cloud(rng, 30_000, scale=50.0)
+    T = scenes.pose_from_rpy_t(0.03, -0.02, 0.7, [12.5, -3.25, 0.8])
+    mo = oracle.Map(1.0, 20)
+    so = mo.insert(pts, pose=T)
+    mg = far.Map(1.0, 20, 100_000)
+    sg = mg.insert(pts, pose=T)
+    assert sg == so
+    _assert_same_map(mg.export(), mo.export())
+    # same through the device-pose entry point
+    md = far.Map(1.0, 20, 100_000)
+    d_pose = torch.frombuffer(bytearray(bytes(far.Pose.from_rt(T))), dtype=torch.uint8).cuda()
+    md.insert_enqueue(pts, d_pose=d_pose)
+    _assert_same_map(md.export(), mo.export())
+
+
+def test_insert_stride4_and_invalid_points_consume_ids():
+    rng = np.random.default_rng(9)
+    pts = _cloud(rng, 5000, scale=5.0)
+    pts[10] = np.nan
+    pts[11, 2] = -np.inf
+    p4 = np.concatenate([pts, rng.normal(size=(5000, 1)).astype(np.float32)], axis=1)
+    mo = oracle.Map(0.5, 20)
+    so = mo.insert(p4)
+    mg = far.Map(0.5, 20, 20_000)
+    sg = mg.insert(p4)
+    assert sg == so and sg["n_invalid"] == 2
+    _assert_same_map(mg.export(), mo.export())
+    assert mg.size()[2] == 5000
+
+
+def test_insert_is_deterministic_across_runs():
+    rng = np.random.default_rng(10)
+    pts = torch.as_tensor(_cloud(rng, 200_000, scale=6.0)).cuda()
+    exports = []
+    for _ in range(3):
+        m = far.Map(0.5, 20, 50_000)
+        m.insert(pts)
+        exports.append(m.export())
+        m.close()
+    for e in exports[1:]:
+        _assert_same_map(e, exports[0])
+
+
+def test_table_full_is_reported_not_fatal():
+    rng = np.random.default_rng(12)
+    pts = _cloud(rng, 20_000, scale=50.0, clustered=False)
+    m = far.Map(0.5, 4, 1000)       # far fewer voxels than the cloud occupies
+    st = m.insert(pts)
+    assert st["n_dropped_full"] > 0
+    assert st["n_accepted"] + st["n_dropped_full"] <= st["n_offered"]
+    s = m.stats()
+    assert s["n_voxels"] <= 1000 + 256 * 148   # racy pre-check may overshoot by the threads in flight, never unbounded
+    e = m.export()
+    assert (e["counts"] <= 4).all() and (e["counts"] >= 1).all()
+
+
+# ---- A5 ---------------------------------------------------------------------------------------------------
+def test_prune_matches_oracle_and_reinsert():
+    rng = np.random.default_rng(13)
+    pts = _cloud(rng, 80_000, scale=30.0)
+    mo, mg = oracle.Map(1.0, 20), far.Map(1.0, 20, 200_000)
+    mo.insert(pts); mg.insert(pts)
+    c = [1.5, -2.0, 0.25]
+    assert mg.prune(c, 1e9) == mo.prune(c, 1e9)          # no-op
+    so, sg = mo.prune(c, 17.3), mg.prune(c, 17.3)
+    assert sg == so and sg["n_voxels_removed"] > 0
+    _assert_same_map(mg.export(), mo.export())
+    # pruned voxels come back empty: re-insert a second cloud over the whole region
+    more = _cloud(rng, 40_000, scale=30.0)
+    assert mg.insert(more) == mo.insert(more)
+    _assert_same_map(mg.export(), mo.export())
+    st = mg.stats()
+    assert st["n_voxels"] == mo.size()[0] and st["n_points"] == mo.size()[1]
+    # prune by a device-resident pose gives the same result
+    T = (np.eye(3), np.array(c))
+    d_pose = torch.frombuffer(bytearray(bytes(far.Pose.from_rt(T))), dtype=torch.uint8).cuda()
+    mg.prune_enqueue(radius=9.0, d_pose=d_pose)
+    mo.prune(c, 9.0)
+    _assert_same_map(mg.export(), mo.export())
+
+
+def test_rehash_and_clear_keep_contents_semantics():
+    rng = np.random.default_rng(14)
+    pts = _cloud(rng, 60_000, scale=30.0)
+    mo, mg = oracle.Map(1.0, 20), far.Map(1.0, 20, 200_000, with_cov=True)
+    mo.insert(pts, compute_cov=True); mg.insert(pts, compute_cov=True)
+    mo.prune([0, 0, 0], 20.0); mg.prune([0, 0, 0], 20.0)
+    dead_before = mg.stats()["n_dead_keys"]
+    assert dead_before > 0
+    mg.rehash()
+    st = mg.stats()
+    assert st["n_dead_keys"] == 0 and st["n_voxels"] == mo.size()[0]
+    _assert_same_map(mg.export(with_cov=True), mo.export(with_cov=True), with_cov=True)
+    q = _cloud(rng, 5000, scale=25.0)
+    ids_o, d2_o = mo.nn(q)
+    ids_g, d2_g = mg.nn(q)
+    assert np.array_equal(ids_g.cpu().numpy().view(np.uint32), ids_o)
+    mg.clear()
+    assert mg.size() == (0, 0, 0)
+    mo2 = oracle.Map(1.0, 20)
+    mo2.insert(pts[:1000]); mg.insert(pts[:1000])
+    _assert_same_map(mg.export(), mo2.export())
+
+
+# ---- A6 ---------------------------------------------------------------------------------------------------
+def test_nn_golden_example():
+    g = load_golden("nn_worked_example.json")
+    m = far.Map(g["voxel"], 20, 64)
+    m.insert(np.array(g["stored"], dtype=np.float32))
+    for case in g["queries"]:
+        ids, d2 = m.nn(np.array([case["q"]], dtype=np.float32))
+        assert int(ids.cpu().numpy().view(np.uint32)[0]) == case["id"]
+        want = np.inf if case["d2"] == "inf" else case["d2"]
+        assert float(d2[0]) == pytest.approx(want, rel=1e-6)
+    t = g["tie"]
+    m2 = far.Map(g["voxel"], 20, 64)
+    m2.insert(np.array(t["stored"], dtype=np.float32))
+    ids, _ = m2.nn(np.array([t["q"]], dtype=np.float32))
+    assert int(ids[0]) == t["id"]
+
+
+@pytest.mark.parametrize("voxel,cap", [(0.25, 20), (0.5, 20), (1.0, 20), (2.0, 20), (4.0, 40), (1.0, 1)])
+def test_nn_bit_exact(voxel, cap):
+    rng = np.random.default_rng(int(voxel * 100) + cap)
+    pts = _cloud(rng, 120_000, scale=25.0)
+    mo, mg = oracle.Map(voxel, cap), far.Map(voxel, cap, 400_000)
+    mo.insert(pts); mg.insert(pts)
+    q = np.concatenate([pts[rng.integers(0, len(pts), 20_000)] + rng.normal(0, 0.1, (20_000, 3)).astype(np.float32),
+                        rng.uniform(-40, 40, (10_001, 3)).astype(np.float32)]).astype(np.float32)
+    q[5] = np.nan
+    ids_o, d2_o = mo.nn(q, nthreads=8)
+    ids_g, d2_g = mg.nn(q)
+    assert np.array_equal(ids_g.cpu().numpy().view(np.uint32), ids_o)
+    assert np.array_equal(d2_g.cpu().numpy().view(np.uint32), d2_o.view(np.uint32))
+    assert (ids_o == oracle.NO_ID).any() and (ids_o != oracle.NO_ID).any()
+
+
+def test_nn_exact_ties_break_to_lowest_id():
+    # lattice points: many exactly equidistant candidates
+    g = np.stack(np.meshgrid(np.arange(-8, 8), np.arange(-8, 8), np.arange(-2, 2), indexing="ij"), -1).reshape(-1, 3)
+    pts = (g * 0.25).astype(np.float32)
+    rng = np.random.default_rng(3)
+    pts = pts[rng.permutation(len(pts))]
+    mo, mg = oracle.Map(0.5, 20), far.Map(0.5, 20, 10_000)
+    mo.insert(pts); mg.insert(pts)
+    q = (g[::3] * 0.25 + 0.125).astype(np.float32)          # cell centres: 8 equidistant corners
+    ids_o, d2_o = mo.nn(q)
+    ids_g, d2_g = mg.nn(q)
+    assert np.array_equal(ids_g.cpu().numpy().view(np.uint32), ids_o)
+    assert np.array_equal(d2_g.cpu().numpy(), d2_o)
+
+
+def test_empty_calls():
+    m = far.Map(0.5, 20, 1024, with_cov=True)
+    z = torch.zeros((0, 3), device="cuda")
+    assert m.insert(z)["n_offered"] == 0
+    ids, d2 = m.nn(z)
+    assert ids.numel() == 0
+    ids, d2 = m.nn(np.array([[0.1, 0.2, 0.3]], dtype=np.float32))      # empty map
+    assert int(ids.cpu().numpy().view(np.uint32)[0]) == far.NO_ID and np.isinf(float(d2[0]))
+    cov, valid = m.knn_cov(np.array([[0.1, 0.2, 0.3]], dtype=np.float32))
+    assert int(valid[0]) == 0 and cov[0].tolist() == [1, 0, 0, 1, 0, 1]
+    assert m.export()["keys"].size == 0
+    assert m.prune([0, 0, 0], 1.0) == dict(n_voxels_removed=0, n_points_removed=0, n_voxels_left=0, n_points_left=0)
