@@ -142,7 +142,7 @@ def test_single_correspondence_and_robust_weight_golden():
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
-@pytest.mark.parametrize("sigma", [2.0, 0.15])
+@pytest.mark.parametrize("sigma", [2.0, 0.05])
 def test_linearize_matches_oracle_c1(kernel, sigma):
     c1 = scenes.c1_tiny(seed=0)
     mo, mg = _build_pair(c1["map_points"], c1["voxel"], c1["cap"])
@@ -151,7 +151,7 @@ def test_linearize_matches_oracle_c1(kernel, sigma):
     opts_o, opts_g = oracle.default_options(kernel=kernel), far.default_options(kernel=kernel)
     rng = np.random.default_rng(2)
     poses = [c1["T_init"], c1["T_gt"], scenes.perturb_pose(c1["T_gt"], 0.05, 0.3, rng)]
-    for T in poses:
+    for ip, T in enumerate(poses):
         o = mo.gicp_linearize(c1["scan"], cov_o, val_o, T, sigma, opts_o)
         g = mg.gicp_linearize(c1["scan"], cov_g, val_g, T, sigma, opts_g)
         assert g["n_inliers"] == o["n_inliers"] and o["n_inliers"] > 0
@@ -163,8 +163,8 @@ def test_linearize_matches_oracle_c1(kernel, sigma):
         eh, eb = _hb_err(g, o, scale_b)
         assert eh < 1e-4 and eb < 1e-4, (eh, eb)
         assert g["chi2"] == pytest.approx(o["chi2"], rel=1e-6)
-        if sigma < 1.0:
-            assert o["n_inliers"] < len(c1["scan"])          # the gate rejects something
+        if sigma < 1.0 and ip == 0:
+            assert o["n_inliers"] < len(c1["scan"])          # the gate (tau = 0.15 m) rejects something at T_init
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
