@@ -1,0 +1,412 @@
+#!/usr/bin/env python
+"""bench.py -- FAR-LIO front-end hot path on B200: scan registrations/s on BASELINE.json configs[1] (C2).
+
+One "step" = one LiDAR frame through the WHOLE hot path:
+  far_voxelize (1.0 m)  ->  scan-local map + k-NN covariances (Sigma_s)  ->  far_gicp_register against the
+  1.5 M-point local map from a 0.5 m / 3 deg perturbed pose  ->  far_map_insert of the raw scan at the registered
+  pose with covariances of the added points  ->  far_map_prune (150 m),
+issued as one stream-ordered chain (far_frontend_process) with no host synchronisation inside.
+
+Timing: CUDA events on the launching stream around each step; before every step the map is restored from a
+device snapshot (untimed; an 876 MB device copy, which also evicts the 126 MB L2), so every step does identical
+work on a cold cache.  `value` = K / sum of step times (max over ranks); `e2e` = the same frame through
+far_frontend_process_host: pinned HOST scan in, HOST result out, copies and the sync inside the timed region.
+
+`python bench.py --impl reference` times the FP64 CPU oracle (oracle/, as it stands) on the same workload.
+Multi-GPU (torchrun): replicas only -- the path does not shard (north_star: one GPU, no collectives); every rank
+runs the same workload on its own GPU and `value` is the aggregate.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "scan registrations/s (whole frame: voxelise + Sigma_s + GICP register + map insert + prune)"
+UNIT = "registrations/s"
+PRUNE_RADIUS = 150.0
+MAX_ITERS = 30
+
+
+def workload_c2():
+    import far_scenes as scenes
+    c2 = scenes.c2_single_frame(seed=1)
+    return c2
+
+
+def workload_name(c2, n_ds=None, n_vox=None, n_stored=None):
+    s = (f"C2 single-frame spinning-LiDAR registration (BASELINE.json configs[1], seed 1): 64x2048 rays -> "
+         f"{len(c2['scan'])} returns, voxelised at 1.0 m")
+    if n_ds is not None:
+        s += f" -> {n_ds} source points"
+    s += f"; local map v=1.0 m cap 20 from {len(c2['map_points'])} surface samples"
+    if n_stored is not None:
+        s += f" ({n_stored} stored, {n_vox} voxels)"
+    s += "; init pose 0.5 m / 3 deg off; sigma 2.0; max 30 iterations"
+    return s
+
+
+# ---------------------------------------------------------------------------------------------------------
+class ClockSampler(threading.Thread):
+    """Samples SM clock / throttle reasons through NVML every ~5 ms while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.sm, self.reasons, self.sm_max, self.ok = index, False, [], set(), None, False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.sm_max = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {getattr(nv, n): n.replace("nvmlClocksThrottleReason", "").replace("nvmlClocksEventReason", "")
+                 for n in dir(nv) if n.startswith("nvmlClocksThrottleReason") or n.startswith("nvmlClocksEventReason")}
+        while not self.stop_flag:
+            try:
+                self.sm.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if isinstance(bit, int) and bit and (r & bit) and name not in ("None", "All", "GpuIdle"):
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.005)
+
+    def summary(self):
+        if not self.ok or not self.sm:
+            return {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": ["nvml unavailable"]}
+        return {"sm_mhz": float(np.median(self.sm)), "sm_max_mhz": self.sm_max, "reasons": sorted(self.reasons),
+                "samples": len(self.sm)}
+
+
+def visible_index(local_rank):
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local_rank])
+        except Exception:
+            return local_rank
+    return local_rank
+
+
+# ---------------------------------------------------------------------------------------------------------
+def oracle_frame(oracle, mo, c2, n_threads, register_reps):
+    """The oracle's frame (same stages as far_frontend_process).  Returns (seconds per frame, result, detail)."""
+    scan, v, cap, sigma = c2["scan"], c2["voxel"], c2["cap"], c2["sigma"]
+    t_reg = []
+    for _ in range(register_reps):
+        t0 = time.perf_counter()
+        ds, _ = oracle.voxelize(scan, v)
+        lo = oracle.Map(v, cap)
+        lo.insert(scan)
+        cov, val = lo.knn_cov(ds, nthreads=n_threads)
+        res = mo.gicp_register(ds, cov, val, c2["T_init"], sigma, MAX_ITERS, nthreads=n_threads)
+        t_reg.append(time.perf_counter() - t0)
+    t0 = time.perf_counter()
+    st = mo.insert(scan, pose=(res["R"], res["t"]), compute_cov=True)
+    mo.prune(res["t"], PRUNE_RADIUS)
+    t_upd = time.perf_counter() - t0
+    return float(np.mean(t_reg)) + t_upd, res, dict(register_s=float(np.mean(t_reg)), update_s=t_upd, accepted=st["n_accepted"])
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    cores = os.cpu_count() or 1
+    c2 = workload_c2()
+    mo = oracle.Map(c2["voxel"], c2["cap"])
+    mo.insert(c2["map_points"], compute_cov=True)
+    times = []
+    res = None
+    for i in range(args.warmup + args.steps):
+        t, res, _ = oracle_frame(oracle, mo, c2, cores, 1)
+        if i >= args.warmup:
+            times.append(t)
+    total = float(np.sum(times))
+    value = len(times) / total
+    sample = (f"{args.steps} whole frames of the C2 workload on one oracle map (the map keeps the inserted scans between "
+              f"frames, so later frames insert less: this favours the reference)")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(c2), "iters": int(res["iters"])},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+# ---------------------------------------------------------------------------------------------------------
+def algorithmic_bytes(kernel, units, cand, n_slots=0, n_scan=0):
+    """Algorithmic bytes of one launch: what the method must move, per unit."""
+    probe = 27 * 16                                     # 27 table entries (key + count in one 16 B entry)
+    if kernel == "gicp_kernel":                         # unit = source point x iteration
+        return units * (12 + probe + cand * 16 + 16 + 25 + 25)
+    if kernel in ("knn_cov_refs_kernel", "knn_cov_points_kernel"):   # unit = query
+        return units * (16 + probe + cand * 16 + 25)
+    if kernel == "nn_kernel":
+        return units * (12 + probe + cand * 16 + 8)
+    if kernel == "insert_claim_chain_kernel":           # unit = offered point: read 12, key CAS 8, count 4, id word 4
+        return units * 28
+    if kernel == "insert_commit_kernel":                # unit = accepted point: id 4 + point 12 + float4 store 16
+        return units * 32
+    if kernel in ("prune_kernel", "clear_kernel"):
+        return n_slots * 16
+    return None
+
+
+def run_far(args):
+    import torch
+
+    import far_scenes as scenes
+    import paper_2606_26010_b200 as far
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the far_* path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl")
+    far.lib()
+    K, W = args.steps, args.warmup
+
+    c2 = workload_c2()
+    scan, v, cap, sigma = c2["scan"], c2["voxel"], c2["cap"], c2["sigma"]
+    fe = far.Frontend(v, cap, 262144, len(scan), ds_voxel=v, prune_radius=PRUNE_RADIUS, max_iters=MAX_ITERS)
+    d_map_pts = torch.as_tensor(c2["map_points"]).cuda()
+    build_stats = fe.map.insert(d_map_pts, compute_cov=True)
+    map_stats = fe.map.stats()
+    snap = fe.map.snapshot()
+    d_scan = torch.as_tensor(scan).cuda()
+    h_scan = torch.as_tensor(scan).pin_memory()
+    d_res = torch.zeros((max(K, 1), far.GICP_RESULT_BYTES), dtype=torch.uint8, device="cuda")
+    T_init = far.Pose.from_rt(c2["T_init"])
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    # ---- device-timed region ------------------------------------------------------------------------------
+    for _ in range(W):
+        fe.map.restore(snap)
+        fe.process_enqueue(d_scan, T_init, sigma, d_result=d_res[0])
+    barrier()
+    sampler = ClockSampler(visible_index(local_rank))
+    sampler.start()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    l0 = far.launch_count()
+    t0 = time.perf_counter()
+    for i in range(K):
+        fe.map.restore(snap)
+        evs[i][0].record()
+        fe.process_enqueue(d_scan, T_init, sigma, d_result=d_res[i])
+        evs[i][1].record()
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - t0
+    launches = far.launch_count() - l0
+    step_ms = np.array([a.elapsed_time(b) for a, b in evs])
+    total_ms = float(step_ms.sum())
+    barrier()
+    sampler.stop_flag = True
+    sampler.join()
+    if dist is not None:
+        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    value = world * K / (total_ms * 1e-3)
+    res = far.result_to_dict(far.GicpResult.from_buffer_copy(d_res[K - 1].cpu().numpy().tobytes()))
+    post_stats = fe.map.stats()
+    dt_gt = float(np.linalg.norm(res["t"] - c2["T_gt"][1]))
+    dr_gt = float(np.degrees(np.arccos(np.clip(0.5 * (np.trace(res["R"].T @ c2["T_gt"][0]) - 1), -1, 1))))
+
+    # ---- end to end: pinned host scan in, host result out, per-step sync -----------------------------------
+    Ke = max(3, min(K, 50))
+    for _ in range(3):
+        fe.map.restore(snap)
+        fe.process_host(h_scan, T_init, sigma)
+    e2e_t = []
+    for _ in range(Ke):
+        fe.map.restore(snap)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        r_e2e = fe.process_host(h_scan, T_init, sigma)
+        e2e_t.append(time.perf_counter() - t0)
+    e2e_total = float(np.sum(e2e_t))
+    if dist is not None:
+        t = torch.tensor([e2e_total], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_total = float(t.item())
+    e2e_value = world * Ke / e2e_total
+    assert r_e2e["iters"] == res["iters"] and r_e2e["n_inliers"] == res["n_inliers"]
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic"}
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- rank 0: per-kernel durations (tracing facility), roofline of the dominant kernel -----------------
+    P = 10
+    far.profile_enable(True)
+    for _ in range(P):
+        fe.map.restore(snap)
+        fe.process_enqueue(d_scan, T_init, sigma, d_result=d_res[0])
+    far.profile_enable(False)
+    prof = far.profile_collect()
+    kern = {k: {"ms_per_step": ms / P, "launches_per_step": n / P} for k, (ms, n) in prof.items()}
+    kern_total = sum(x["ms_per_step"] for x in kern.values())
+    for x in kern.values():
+        x["share"] = x["ms_per_step"] / kern_total
+    top = max(kern, key=lambda k: kern[k]["ms_per_step"])
+    # units: source points / iterations from the result, accepted points from the map statistics
+    n_ds = int(far.voxelize(d_scan, v)[0].shape[0])
+    fe.map.restore(snap)
+    fe.process_enqueue(d_scan, T_init, sigma, d_result=d_res[0])
+    torch.cuda.synchronize()
+    after = fe.map.stats()
+    world_scan = torch.as_tensor(scenes.pose_apply((res["R"], res["t"]), scan)).cuda()
+    cand_map = float(fe.map.count27(world_scan).float().mean())                      # candidates per query, updated map
+    ds_world = torch.as_tensor(scenes.pose_apply((res["R"], res["t"]), far.voxelize(d_scan, v)[0].cpu().numpy())).cuda()
+    cand_ds = float(fe.map.count27(ds_world).float().mean())
+    # prune removes nothing at 150 m on this map, so the point-count difference is the accepted count
+    accepted = int(after["n_points"] - map_stats["n_points"])
+    units = {"gicp_kernel": n_ds * res["iters"], "knn_cov_refs_kernel": accepted, "knn_cov_points_kernel": n_ds,
+             "insert_claim_chain_kernel": 2 * len(scan), "insert_commit_kernel": accepted + len(scan)}
+    cand = {"gicp_kernel": cand_ds, "knn_cov_refs_kernel": cand_map, "knn_cov_points_kernel": cand_ds}
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    peak = float(peaks.get("hbm_gbs", 6650.0))
+    peak_kind = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
+    nbytes = algorithmic_bytes(top, units.get(top, 0), cand.get(top, 0.0), n_slots=after["n_slots"])
+    dur_s = kern[top]["ms_per_step"] * 1e-3
+    roof = {"bound": "hbm", "kernel": top, "achieved": (nbytes / dur_s / 1e9) if nbytes else None, "peak": peak,
+            "unit": "GB/s", "frac": (nbytes / dur_s / 1e9 / peak) if nbytes else None, "traffic": None,
+            "peak_kind": peak_kind, "algorithmic_bytes_per_launch": nbytes, "kernel_ms": kern[top]["ms_per_step"],
+            "kernel_share_of_step": kern[top]["share"], "units_per_launch": units.get(top), "candidates_per_query": cand.get(top),
+            "note": "latency-bound at this size: a 5k-point registration cannot approach the HBM roofline (SURVEY 8d)"}
+
+    # ---- extras: NN-query and insert throughput on the same map (BASELINE.json metric's secondary numbers) -
+    extras = {}
+    if not args.no_extras:
+        fe.map.restore(snap)
+        rng = np.random.default_rng(0)
+        nq = 1_000_000
+        sel = rng.integers(0, len(c2["map_points"]), nq)
+        q = torch.as_tensor((c2["map_points"][sel] + rng.normal(0, 0.1, (nq, 3))).astype(np.float32)).cuda()
+        ids = torch.empty(nq, dtype=torch.int32, device="cuda")
+        d2 = torch.empty(nq, dtype=torch.float32, device="cuda")
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+        ts = []
+        for i in range(8):
+            flush.fill_(i)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); fe.map.nn(q, ids, d2); b.record(); torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        t_nn = float(np.median(ts[3:])) * 1e-3
+        cq = float(fe.map.count27(q).float().mean())
+        nn_bytes = algorithmic_bytes("nn_kernel", nq, cq)
+        extras["nn"] = {"queries": nq, "queries_per_s": nq / t_nn, "ms": t_nn * 1e3, "candidates_per_query": cq,
+                        "algorithmic_GBps": nn_bytes / t_nn / 1e9, "frac_of_hbm_peak": nn_bytes / t_nn / 1e9 / peak,
+                        "l2": "256 MB flush buffer written between repetitions"}
+        mp = far.Map(v, cap, 262144, with_cov=False, max_batch=1 << 21)
+        ts = []
+        for i in range(6):
+            mp.clear()
+            flush.fill_(i)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); mp.insert_enqueue(d_map_pts); b.record(); torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        t_ins = float(np.median(ts[2:])) * 1e-3
+        extras["insert"] = {"points": len(c2["map_points"]), "points_per_s": len(c2["map_points"]) / t_ins, "ms": t_ins * 1e3,
+                            "algorithmic_GBps": len(c2["map_points"]) * 40 / t_ins / 1e9,
+                            "note": "1.52 M points in one call into an empty v=1.0 cap-20 map, no covariances"}
+        mp.close()
+
+    # ---- CPU baseline: the oracle, as it stands, on this box's host cores ---------------------------------
+    cpu = None
+    if not args.no_cpu_baseline:
+        import oracle
+        cores = os.cpu_count() or 1
+        mo = oracle.Map(v, cap)
+        t0 = time.perf_counter()
+        mo.insert(c2["map_points"], compute_cov=True)
+        t_build = time.perf_counter() - t0
+        t_frame, o_res, detail = oracle_frame(oracle, mo, c2, cores, 5)
+        cpu = {"value": 1.0 / t_frame, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": (f"one whole C2 frame: 5 x (voxelise + Sigma_s + GICP, {cores} OpenMP threads over source points) "
+                          f"averaged + 1 x (insert with covariances + prune, single thread); map build ({t_build:.1f} s) untimed"),
+               "ms_per_frame": 1e3 * t_frame, "detail": detail,
+               "parity": {"iters_equal": bool(o_res["iters"] == res["iters"]), "inliers_equal": bool(o_res["n_inliers"] == res["n_inliers"]),
+                          "dt_m": float(np.linalg.norm(o_res["t"] - res["t"])),
+                          "drot_rad": float(np.arccos(np.clip(0.5 * (np.trace(o_res["R"].T @ res["R"]) - 1), -1, 1)))}}
+
+    line.update({
+        "config": {"workload": workload_name(c2, n_ds, map_stats["n_voxels"], map_stats["n_points"]),
+                   "timing": "CUDA events per step on the launching stream, summed over K steps; max over ranks",
+                   "l2": "map restored from a device snapshot before every step (untimed 876 MB copy > 126 MB L2): cold cache, identical work",
+                   "parallelism": "replicas only" if world > 1 else "1 GPU",
+                   "scan_points": len(scan), "source_points": n_ds, "map_points": map_stats["n_points"], "map_voxels": map_stats["n_voxels"],
+                   "table_slots": map_stats["n_slots"], "gicp_iters": res["iters"], "accepted_per_frame": accepted},
+        "clocks": sampler.summary(),
+        "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": 1e3 * e2e_total / Ke, "steps": Ke,
+                "h2d_bytes_per_step": int(scan.nbytes + 96), "d2h_bytes_per_step": int(far.GICP_RESULT_BYTES)},
+        "gpu_launches": int(launches),
+        "roofline": roof,
+        "cpu_baseline": cpu,
+        "result": {"status": res["status"], "iters": res["iters"], "converged": res["converged"], "n_inliers": res["n_inliers"],
+                   "err_vs_truth_m": dt_gt, "err_vs_truth_deg": dr_gt},
+        "step_ms": {"median": float(np.median(step_ms)), "p99": float(np.percentile(step_ms, 99)), "max": float(step_ms.max()),
+                    "enqueue_wall_ms_per_step": 1e3 * wall / K},
+        "kernels": {k: {a: round(b, 5) for a, b in x.items()} for k, x in sorted(kern.items(), key=lambda kv: -kv[1]["ms_per_step"])},
+        "extras": extras,
+        "map_build": {"points_offered": build_stats["n_offered"], "accepted": build_stats["n_accepted"]},
+    })
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="far", choices=["far", "reference"])
+    ap.add_argument("--no-extras", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_far(args)
+
+
+if __name__ == "__main__":
+    main()

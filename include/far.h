@@ -79,6 +79,12 @@ typedef struct far_threshold far_threshold_t;
 const char* far_strerror(int status);
 /* text of the last CUDA error seen by this library in the calling process ("" if none) */
 const char* far_last_cuda_error(void);
+/* Tracing: number of kernels this library has launched in the process; optional per-kernel timing with CUDA
+ * events on the launching stream.  far_profile_collect synchronises the device, writes one row per kernel name
+ * (names are static strings) and clears the records; returns the number of rows. */
+long long far_launch_count(void);
+void far_profile_enable(int on);
+int far_profile_collect(const char** names, double* total_ms, long long* launches, int max_entries);
 void far_gicp_default_options(far_gicp_options_t* out);
 
 /* ---- voxel hashmap: PAPER.md:62-68 (cuVoxelMap, Fig. 3), :109 (local submap) -------------------------
@@ -113,9 +119,17 @@ int far_map_prune_dev(far_map_t* map, const far_pose_t* d_pose, double radius, f
 
 /* counts live voxels / stored points / dead (pruned) keys; next_id is the host-side counter at call time */
 int far_map_stats(far_map_t* map, far_map_stats_t* d_stats, void* stream);
-/* Re-hashes the live voxels into a clean table, dropping the keys of pruned voxels (they otherwise stay as
- * dead keys that lengthen probe sequences).  Uses the map's second table buffer; contents unchanged. */
+/* Maintenance call, not on the per-frame path: re-hashes the live voxels into a clean table, dropping the keys
+ * of pruned voxels (they otherwise stay as dead keys that lengthen probe sequences).  Allocates a temporary for
+ * the live buckets, synchronises the stream, frees the temporary; map contents are unchanged. */
 int far_map_rehash(far_map_t* map, void* stream);
+
+/* Checkpoint / restore of a map's whole device state (table, buckets, covariances, counters, id counter).
+ * create allocates the copy (a maintenance call); restore is five stream-ordered device copies, no sync. */
+typedef struct far_snapshot far_snapshot_t;
+int far_map_snapshot_create(far_map_t* map, far_snapshot_t** out, void* stream);
+int far_map_snapshot_restore(far_map_t* map, const far_snapshot_t* snap, void* stream);
+int far_map_snapshot_destroy(far_snapshot_t* snap);
 
 /* Writes the live voxels in unspecified order: keys[v], counts[v], points4[(v*cap + j)*4 + {0,1,2,3}] =
  * x,y,z,id bits (unused entries 0,0,0,FAR_NO_ID), cov6[(v*cap + j)*6] (xx,xy,xz,yy,yz,zz; nullable),
@@ -138,6 +152,10 @@ int far_map_nn(const far_map_t* map, const float* d_q, int64_t m, int stride, ui
  * valid = 0 and cov6 = identity.  cov6: m*6 fp32 (xx,xy,xz,yy,yz,zz). */
 int far_map_knn_cov(const far_map_t* map, const float* d_q, int64_t m, int stride, float* d_cov6,
                     uint8_t* d_valid, void* stream);
+
+/* number of candidate points in the 27 voxels around each query (what A6/A7 scan): density probe, used by
+ * bench.py for the algorithmic-byte count and the quantity the ASMD rule averages */
+int far_map_count27(const far_map_t* map, const float* d_q, int64_t m, int stride, int32_t* d_count, void* stream);
 
 /* A2 ("preprocessing (typically ... deskewing and downsampling)"; R2): one representative per
  * occupied voxel of the scan = the lowest-index valid point, emitted in ascending source index.
@@ -167,6 +185,32 @@ int far_gicp_register_dev(const far_map_t* map, const float* d_scan, const float
 /* same as far_map_knn_cov with the query count read from DEVICE memory (for chaining after far_voxelize) */
 int far_map_knn_cov_dev(const far_map_t* map, const float* d_q, const int64_t* d_m, int64_t m_max, int stride,
                         float* d_cov6, uint8_t* d_valid, void* stream);
+
+/* ---- one frame through the whole path (the LiDAR scan callback) -----------------------------
+ * far_frontend_process chains, in stream order and with NO host synchronisation: far_voxelize (ds_voxel) ->
+ * scan-local map of the raw scan + far_map_knn_cov of the downsampled points (Sigma_s) ->
+ * far_gicp_register against the frontend's map from init_pose -> (update_map) far_map_insert of the raw scan at
+ * the registered pose with covariances + far_map_prune about it.  Sizes and the registered pose
+ * flow between the stages through device memory.  d_out (device, nullable = internal buffer) receives the
+ * registration result.  The _host variant takes a HOST scan (pinned for a truly asynchronous copy) and a HOST
+ * result struct: it uploads, runs the chain, downloads the result and synchronises the stream. */
+typedef struct {
+    far_map_config_t map;       /* the local submap (with_cov is forced to 1)                          */
+    float ds_voxel;             /* downsampling voxel of far_voxelize; 0 -> map.voxel_size             */
+    int64_t max_scan_points;    /* capacity of the per-frame buffers                                   */
+    double prune_radius;        /* <= 0: no pruning                                                    */
+    int32_t max_iters;          /* GICP iteration limit (R14)                                          */
+    int32_t update_map;         /* 0: register only                                                    */
+    far_gicp_options_t gicp;
+} far_frontend_config_t;
+typedef struct far_frontend far_frontend_t;
+int far_frontend_create(far_frontend_t** out, const far_frontend_config_t* cfg);
+int far_frontend_destroy(far_frontend_t* f);
+far_map_t* far_frontend_map(far_frontend_t* f);   /* borrowed handle, e.g. to preload the map with far_map_insert */
+int far_frontend_process(far_frontend_t* f, const float* d_scan, int64_t n, int stride, const far_pose_t* init_pose,
+                         double sigma, far_gicp_result_t* d_out, void* stream);
+int far_frontend_process_host(far_frontend_t* f, const float* h_scan, int64_t n, int stride,
+                              const far_pose_t* init_pose, double sigma, far_gicp_result_t* h_out, void* stream);
 
 /* Adaptive threshold of Vizzo et al. [1] as read in R10.  HOST-only FP64 helper (20 lines of
  * boundary logic, not a kernel): sigma = sqrt(mean delta_i^2) over recorded deviations delta_i > min_motion,

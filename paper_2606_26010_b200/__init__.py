@@ -55,6 +55,11 @@ class GicpResult(C.Structure):
                 ("n_inliers", C.c_int32), ("iters", C.c_int32), ("converged", C.c_int32), ("status", C.c_int32)]
 
 
+class FrontendConfig(C.Structure):
+    _fields_ = [("map", MapConfig), ("ds_voxel", C.c_float), ("max_scan_points", C.c_int64), ("prune_radius", C.c_double),
+                ("max_iters", C.c_int32), ("update_map", C.c_int32), ("gicp", GicpOptions)]
+
+
 INSERT_STATS_FIELDS = ("n_offered", "n_accepted", "n_new_voxels", "n_dropped_full", "n_invalid")
 PRUNE_STATS_FIELDS = ("n_voxels_removed", "n_points_removed", "n_voxels_left", "n_points_left")
 MAP_STATS_FIELDS = ("n_voxels", "n_points", "n_dead_keys", "n_slots", "next_id")
@@ -82,6 +87,9 @@ def lib():
         sig = {
             "far_strerror": (C.c_char_p, [ci]),
             "far_last_cuda_error": (C.c_char_p, []),
+            "far_launch_count": (C.c_longlong, []),
+            "far_profile_enable": (None, [ci]),
+            "far_profile_collect": (ci, [vp, vp, vp, ci]),
             "far_gicp_default_options": (None, [vp]),
             "far_map_create": (ci, [vp, vp]),
             "far_map_destroy": (ci, [vp]),
@@ -92,6 +100,10 @@ def lib():
             "far_map_prune_dev": (ci, [vp, vp, f64, vp, vp]),
             "far_map_stats": (ci, [vp, vp, vp]),
             "far_map_rehash": (ci, [vp, vp]),
+            "far_map_snapshot_create": (ci, [vp, vp, vp]),
+            "far_map_snapshot_restore": (ci, [vp, vp, vp]),
+            "far_map_snapshot_destroy": (ci, [vp]),
+            "far_map_count27": (ci, [vp, vp, i64, ci, vp, vp]),
             "far_map_export": (ci, [vp, vp, vp, vp, vp, vp, i64, vp, vp]),
             "far_voxel_keys": (ci, [vp, i64, ci, f32, vp, vp]),
             "far_map_nn": (ci, [vp, vp, i64, ci, vp, vp, vp]),
@@ -101,6 +113,11 @@ def lib():
             "far_gicp_linearize": (ci, [vp, vp, vp, vp, i64, ci, vp, f64, vp, vp, vp]),
             "far_gicp_register": (ci, [vp, vp, vp, vp, i64, ci, vp, f64, ci, vp, vp, vp]),
             "far_gicp_register_dev": (ci, [vp, vp, vp, vp, vp, i64, ci, vp, f64, ci, vp, vp, vp]),
+            "far_frontend_create": (ci, [vp, vp]),
+            "far_frontend_destroy": (ci, [vp]),
+            "far_frontend_map": (vp, [vp]),
+            "far_frontend_process": (ci, [vp, vp, i64, ci, vp, f64, vp, vp]),
+            "far_frontend_process_host": (ci, [vp, vp, i64, ci, vp, f64, vp, vp]),
             "far_threshold_create": (vp, [f64, f64, f64]),
             "far_threshold_destroy": (None, [vp]),
             "far_threshold_update": (None, [vp, vp, vp]),
@@ -155,6 +172,24 @@ def result_to_dict(res: GicpResult):
                 n_inliers=res.n_inliers, iters=res.iters, converged=res.converged, status=res.status)
 
 
+def launch_count():
+    """far_launch_count: kernels launched by libfar.so in this process so far."""
+    return int(lib().far_launch_count())
+
+
+def profile_enable(on=True):
+    lib().far_profile_enable(int(bool(on)))
+
+
+def profile_collect(max_entries=64):
+    """far_profile_collect -> {kernel name: (total_ms, launches)}; synchronises the device."""
+    names = (C.c_char_p * max_entries)()
+    ms = (C.c_double * max_entries)()
+    cnt = (C.c_longlong * max_entries)()
+    n = lib().far_profile_collect(names, ms, cnt, max_entries)
+    return {names[i].decode(): (ms[i], int(cnt[i])) for i in range(n)}
+
+
 def voxel_keys(xyz, voxel):
     """far_voxel_keys: packed voxel key per point (uint64 bit pattern in an int64 tensor)."""
     x, n, s = _points(xyz)
@@ -197,14 +232,19 @@ def voxelize(xyz, voxel):
 class Map:
     """A far_map_t handle.  All bulk arguments are CUDA tensors (NumPy arrays are uploaded for convenience)."""
 
-    def __init__(self, voxel, cap, max_voxels, with_cov=False, k_cov=10, cov_eps=1e-3, max_load=0.5, max_batch=1 << 20):
+    def __init__(self, voxel, cap, max_voxels, with_cov=False, k_cov=10, cov_eps=1e-3, max_load=0.5, max_batch=1 << 20,
+                 _borrowed=None):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2606_26010_b200 needs a CUDA device: there is no CPU fallback")
         self.voxel, self.cap, self.k_cov, self.with_cov = float(voxel), int(cap), int(k_cov), bool(with_cov)
-        cfg = MapConfig(voxel, cap, int(max_voxels), max_load, int(with_cov), k_cov, cov_eps, int(max_batch))
-        h = C.c_void_p()
-        _check(lib().far_map_create(C.byref(h), C.byref(cfg)), "far_map_create")
-        self._h = h
+        self._owned = _borrowed is None
+        if _borrowed is None:
+            cfg = MapConfig(voxel, cap, int(max_voxels), max_load, int(with_cov), k_cov, cov_eps, int(max_batch))
+            h = C.c_void_p()
+            _check(lib().far_map_create(C.byref(h), C.byref(cfg)), "far_map_create")
+            self._h = h
+        else:
+            self._h = _borrowed
         dev = torch.device("cuda", torch.cuda.current_device())
         self.device = dev
         self._insert_stats = torch.zeros(5, dtype=torch.int64, device=dev)
@@ -214,7 +254,8 @@ class Map:
 
     def close(self):
         if getattr(self, "_h", None):
-            lib().far_map_destroy(self._h)
+            if self._owned:
+                lib().far_map_destroy(self._h)
             self._h = None
 
     def __del__(self):
@@ -260,6 +301,25 @@ class Map:
     def size(self):
         s = self.stats()
         return s["n_voxels"], s["n_points"], s["next_id"]
+
+    def snapshot(self):
+        """far_map_snapshot_create: returns an opaque handle for restore()."""
+        h = C.c_void_p()
+        _check(lib().far_map_snapshot_create(self._h, C.byref(h), _stream()), "far_map_snapshot_create")
+        return h
+
+    def restore(self, snap):
+        _check(lib().far_map_snapshot_restore(self._h, snap, _stream()), "far_map_snapshot_restore")
+
+    @staticmethod
+    def snapshot_destroy(snap):
+        lib().far_map_snapshot_destroy(snap)
+
+    def count27(self, q):
+        x, n, s = _points(q)
+        out = torch.empty(n, dtype=torch.int32, device=x.device)
+        _check(lib().far_map_count27(self._h, _ptr(x), n, s, _ptr(out), _stream()), "far_map_count27")
+        return out
 
     def rehash(self):
         _check(lib().far_map_rehash(self._h, _stream()), "far_map_rehash")
@@ -343,6 +403,56 @@ class Map:
     def gicp_register(self, scan, cov6, valid, init_pose, sigma, max_iters=30, opts=None):
         res = self.gicp_register_enqueue(scan, cov6, valid, init_pose, sigma, max_iters, opts)
         return result_to_dict(_struct_from_tensor(res, GicpResult))
+
+
+class Frontend:
+    """far_frontend_*: one frame through the whole hot path as a single stream-ordered chain."""
+
+    def __init__(self, voxel, cap, max_voxels, max_scan_points, ds_voxel=0.0, prune_radius=0.0, max_iters=30,
+                 update_map=True, opts=None, k_cov=10, cov_eps=1e-3, max_load=0.5):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2606_26010_b200 needs a CUDA device: there is no CPU fallback")
+        o = opts if opts is not None else default_options()
+        cfg = FrontendConfig(MapConfig(voxel, cap, int(max_voxels), max_load, 1, k_cov, cov_eps, 0), ds_voxel,
+                             int(max_scan_points), float(prune_radius), int(max_iters), int(update_map), o)
+        h = C.c_void_p()
+        _check(lib().far_frontend_create(C.byref(h), C.byref(cfg)), "far_frontend_create")
+        self._h = h
+        self.map = Map(voxel, cap, max_voxels, with_cov=True, k_cov=k_cov, _borrowed=C.c_void_p(lib().far_frontend_map(h)))
+        self.max_scan_points = int(max_scan_points)
+        self.h_result = GicpResult()
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self.map.close()
+            lib().far_frontend_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def process_enqueue(self, d_scan, init_pose, sigma, d_result=None):
+        """Device scan in, result struct stays on the device; no host synchronisation."""
+        x, n, s = _points(d_scan)
+        po = Pose.from_rt(init_pose) if not isinstance(init_pose, Pose) else init_pose
+        _check(lib().far_frontend_process(self._h, _ptr(x), n, s, C.byref(po), float(sigma), _ptr(d_result), _stream()),
+               "far_frontend_process")
+
+    def process_host(self, h_scan, init_pose, sigma):
+        """HOST scan (a pinned torch CPU tensor or a NumPy array) in, result dict out; uploads, runs, downloads, syncs."""
+        if isinstance(h_scan, torch.Tensor):
+            assert h_scan.device.type == "cpu" and h_scan.dtype == torch.float32 and h_scan.is_contiguous()
+            ptr, n, s = C.c_void_p(h_scan.data_ptr()), h_scan.shape[0], h_scan.shape[1]
+        else:
+            h_scan = np.ascontiguousarray(h_scan, dtype=np.float32)
+            ptr, n, s = C.c_void_p(h_scan.ctypes.data), h_scan.shape[0], h_scan.shape[1]
+        po = Pose.from_rt(init_pose) if not isinstance(init_pose, Pose) else init_pose
+        _check(lib().far_frontend_process_host(self._h, ptr, n, s, C.byref(po), float(sigma), C.byref(self.h_result), _stream()),
+               "far_frontend_process_host")
+        return result_to_dict(self.h_result)
 
 
 class AdaptiveThreshold:

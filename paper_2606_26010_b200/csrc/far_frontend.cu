@@ -1,0 +1,124 @@
+// far_frontend.cu -- one LiDAR frame through the whole hot path as a single stream-ordered chain (host code
+// only: it strings the kernels of the other translation units together, nothing is computed here).
+//
+// PAPER.md:54-109 (LiDAR scan callback): [downsample, :171] -> Cov-Calc on a scan-local cuVoxelMap (:76) ->
+// GICP against the local submap from the predicted pose (:76-100) -> submap update at the registered pose:
+// capped insert, covariances of the added points, range pruning (:109).  Every stage reads its sizes and the
+// registered pose from device memory, so the chain needs no host synchronisation between stages.
+#include <cstring>
+#include <new>
+
+#include "far_internal.h"
+
+struct far_frontend {
+    far_frontend_config_t cfg;
+    far_map_t* map;          // the local submap Q
+    far_map_t* local;        // scan-local map used for Sigma_s
+    void* d_ws;              // far_voxelize workspace
+    size_t ws_bytes;
+    float* d_scan;           // staging for host scans [max_scan_points * 4]
+    float* d_ds_xyz;         // downsampled scan
+    int32_t* d_ds_index;
+    int64_t* d_n_ds;
+    float* d_cov6;
+    uint8_t* d_valid;
+    far_pose_t* d_init;
+    far_gicp_result_t* d_result;
+};
+
+extern "C" {
+
+int far_frontend_destroy(far_frontend_t* f) {
+    if (!f) return FAR_OK;
+    far_map_destroy(f->map);
+    far_map_destroy(f->local);
+    cudaFree(f->d_ws); cudaFree(f->d_scan); cudaFree(f->d_ds_xyz); cudaFree(f->d_ds_index); cudaFree(f->d_n_ds);
+    cudaFree(f->d_cov6); cudaFree(f->d_valid); cudaFree(f->d_init); cudaFree(f->d_result);
+    delete f;
+    return FAR_OK;
+}
+
+int far_frontend_create(far_frontend_t** out, const far_frontend_config_t* cfg) {
+    if (!out || !cfg || cfg->max_scan_points < 1 || cfg->max_iters < 1) return FAR_ERR_ARG;
+    *out = nullptr;
+    far_frontend* f = new (std::nothrow) far_frontend();
+    if (!f) return FAR_ERR_ARG;
+    memset(f, 0, sizeof(*f));
+    f->cfg = *cfg;
+    if (!(f->cfg.ds_voxel > 0.f)) f->cfg.ds_voxel = cfg->map.voxel_size;
+    far_map_config_t mc = cfg->map;
+    mc.with_cov = 1;
+    if (mc.max_batch < cfg->max_scan_points) mc.max_batch = cfg->max_scan_points;
+    int rc = far_map_create(&f->map, &mc);
+    if (rc == FAR_OK) {
+        far_map_config_t lc = cfg->map;
+        lc.with_cov = 0;
+        lc.max_voxels = cfg->max_scan_points;
+        lc.max_load = 0.5f;
+        lc.max_batch = cfg->max_scan_points;
+        rc = far_map_create(&f->local, &lc);
+    }
+    if (rc != FAR_OK) { far_frontend_destroy(f); return rc; }
+    const int64_t n = cfg->max_scan_points;
+    rc = far_voxelize(nullptr, n, 3, f->cfg.ds_voxel, nullptr, nullptr, nullptr, nullptr, &f->ws_bytes, nullptr);
+    cudaError_t e = cudaSuccess;
+    auto alloc = [&](void** p, size_t bytes) { if (e == cudaSuccess) e = cudaMalloc(p, bytes); };
+    alloc(&f->d_ws, f->ws_bytes);
+    alloc((void**)&f->d_scan, (size_t)n * 4 * sizeof(float));
+    alloc((void**)&f->d_ds_xyz, (size_t)n * 3 * sizeof(float));
+    alloc((void**)&f->d_ds_index, (size_t)n * sizeof(int32_t));
+    alloc((void**)&f->d_n_ds, sizeof(int64_t));
+    alloc((void**)&f->d_cov6, (size_t)n * 6 * sizeof(float));
+    alloc((void**)&f->d_valid, (size_t)n);
+    alloc((void**)&f->d_init, sizeof(far_pose_t));
+    alloc((void**)&f->d_result, sizeof(far_gicp_result_t));
+    if (rc != FAR_OK || e != cudaSuccess) {
+        if (e != cudaSuccess) far::set_cuda_error(e, "cudaMalloc in far_frontend_create");
+        far_frontend_destroy(f);
+        return rc != FAR_OK ? rc : FAR_ERR_CUDA;
+    }
+    *out = f;
+    return FAR_OK;
+}
+
+far_map_t* far_frontend_map(far_frontend_t* f) { return f ? f->map : nullptr; }
+
+int far_frontend_process(far_frontend_t* f, const float* d_scan, int64_t n, int stride, const far_pose_t* init_pose,
+                         double sigma, far_gicp_result_t* d_out, void* stream) {
+    if (!f || !init_pose || n < 0 || n > f->cfg.max_scan_points || (n > 0 && !d_scan) || (stride != 3 && stride != 4))
+        return FAR_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    far_gicp_result_t* res = d_out ? d_out : f->d_result;
+    int rc;
+    // A1/A2: downsample
+    size_t ws = f->ws_bytes;
+    if ((rc = far_voxelize(d_scan, n, stride, f->cfg.ds_voxel, f->d_ds_xyz, f->d_ds_index, f->d_n_ds, f->d_ws, &ws, stream))) return rc;
+    // A7: Sigma_s from a scan-local map of the raw scan
+    if ((rc = far_map_clear(f->local, stream))) return rc;
+    if ((rc = far_map_insert(f->local, d_scan, n, stride, nullptr, 0, nullptr, stream))) return rc;
+    if (n > 0 && (rc = far_map_knn_cov_dev(f->local, f->d_ds_xyz, f->d_n_ds, n, 3, f->d_cov6, f->d_valid, stream))) return rc;
+    // A6, A8-A10: registration from the predicted pose
+    FAR_CUDA(cudaMemcpyAsync(f->d_init, init_pose, sizeof(far_pose_t), cudaMemcpyHostToDevice, st));
+    if ((rc = far_gicp_register_dev(f->map, f->d_ds_xyz, f->d_cov6, f->d_valid, f->d_n_ds, n, 3, f->d_init, sigma,
+                                    f->cfg.max_iters, &f->cfg.gicp, res, stream))) return rc;
+    // A3-A5, A7: submap update at the registered pose
+    if (f->cfg.update_map) {
+        if ((rc = far_map_insert_dev(f->map, d_scan, n, stride, &res->pose, 1, nullptr, stream))) return rc;
+        if (f->cfg.prune_radius > 0.0 && (rc = far_map_prune_dev(f->map, &res->pose, f->cfg.prune_radius, nullptr, stream))) return rc;
+    }
+    return FAR_OK;
+}
+
+int far_frontend_process_host(far_frontend_t* f, const float* h_scan, int64_t n, int stride, const far_pose_t* init_pose,
+                              double sigma, far_gicp_result_t* h_out, void* stream) {
+    if (!f || !h_out || n < 0 || n > f->cfg.max_scan_points || (n > 0 && !h_scan) || (stride != 3 && stride != 4)) return FAR_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (n > 0) FAR_CUDA(cudaMemcpyAsync(f->d_scan, h_scan, (size_t)n * stride * sizeof(float), cudaMemcpyHostToDevice, st));
+    const int rc = far_frontend_process(f, f->d_scan, n, stride, init_pose, sigma, f->d_result, stream);
+    if (rc != FAR_OK) return rc;
+    FAR_CUDA(cudaMemcpyAsync(h_out, f->d_result, sizeof(far_gicp_result_t), cudaMemcpyDeviceToHost, st));
+    FAR_CUDA(cudaStreamSynchronize(st));
+    return FAR_OK;
+}
+
+}  // extern "C"

@@ -398,7 +398,10 @@ static int gicp_launch(const far_map_t* map, const float* d_scan, const float* d
     FAR_CUDA(cudaMemsetAsync(map->d_gicp_state, 0, sizeof(GicpState), st));
     MapView view = map->view;
     void* args[] = {(void*)&view, (void*)&P};
-    FAR_CUDA(cudaLaunchCooperativeKernel((const void*)gicp_kernel, dim3((unsigned)grid), dim3(GWARPS * 32), args, 0, st));
+    {
+        far::LaunchScope ls_("gicp_kernel", st);
+        FAR_CUDA(cudaLaunchCooperativeKernel((const void*)gicp_kernel, dim3((unsigned)grid), dim3(GWARPS * 32), args, 0, st));
+    }
     return FAR_OK;
 }
 

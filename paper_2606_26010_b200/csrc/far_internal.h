@@ -32,6 +32,22 @@ void set_cuda_error(cudaError_t e, const char* where);
         }                                                \
     } while (0)
 
+// Launch accounting (always on: one relaxed counter) and optional per-kernel timing with CUDA events recorded on
+// the launching stream (far_profile_enable / far_profile_collect): the tracing facility bench.py reads the
+// per-kernel durations from.  Disabled, a LaunchScope costs one atomic increment.
+struct LaunchScope {
+    LaunchScope(const char* name, cudaStream_t st);
+    ~LaunchScope();
+    int rec_;
+    cudaStream_t st_;
+};
+
+#define FAR_LAUNCH(kernel, grid, block, smem, st, ...)        \
+    do {                                                      \
+        far::LaunchScope ls_(#kernel, st);                    \
+        kernel<<<grid, block, smem, st>>>(__VA_ARGS__);       \
+    } while (0)
+
 inline int grid_for(int64_t n, int block) { return (int)((n + block - 1) / block); }
 
 // launch helpers implemented in far_query.cu (used by far_map.cu for the covariances of accepted points)

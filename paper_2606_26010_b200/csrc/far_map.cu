@@ -440,7 +440,7 @@ int far_map_create(far_map_t** out, const far_map_config_t* cfg) {
     }
     // empty table: every key = ~0, count = 0; every id word = FAR_NO_ID (0xFF bytes everywhere in the pool)
     FAR_CUDA(cudaMemset(v.points, 0xFF, npts * sizeof(float4)));
-    table_init_kernel<<<grid_for((int64_t)slots, 256), 256>>>(v.table, v.slots);
+    FAR_LAUNCH(table_init_kernel, grid_for((int64_t)slots, 256), 256, 0, 0, v.table, v.slots);
     FAR_CUDA(cudaGetLastError());
     FAR_CUDA(cudaMemset(v.ctr, 0, sizeof(Counters) + 4 * sizeof(unsigned long long)));
     if (v.cov_ok) FAR_CUDA(cudaMemset(v.cov_ok, 0, npts));
@@ -465,7 +465,7 @@ int far_map_destroy(far_map_t* m) {
 int far_map_clear(far_map_t* m, void* stream) {
     if (!m) return FAR_ERR_ARG;
     cudaStream_t st = (cudaStream_t)stream;
-    clear_kernel<<<grid_for(m->view.slots, 256), 256, 0, st>>>(m->view);
+    FAR_LAUNCH(clear_kernel, grid_for(m->view.slots, 256), 256, 0, st, m->view);
     FAR_CUDA(cudaGetLastError());
     FAR_CUDA(cudaMemsetAsync(m->view.ctr, 0, sizeof(Counters), st));
     m->next_id = 0;
@@ -493,9 +493,9 @@ static int insert_impl(far_map_t* m, const float* d_xyz, int64_t n, int stride, 
         const uint32_t first_id = (uint32_t)(m->next_id + (uint64_t)off);
         const float* xyz = d_xyz + off * stride;
         FAR_CUDA(cudaMemsetAsync(&ctr->n_touched, 0, sizeof(unsigned int), st));
-        insert_claim_chain_kernel<<<grid_for(nc, 256), 256, 0, st>>>(m->view, xyz, nc, stride, pose_mode, hp,
+        FAR_LAUNCH(insert_claim_chain_kernel, grid_for(nc, 256), 256, 0, st, m->view, xyz, nc, stride, pose_mode, hp,
                                                                       (const Pose*)d_pose, first_id, m->d_touched);
-        insert_commit_kernel<<<commit_grid, 256, 0, st>>>(m->view, xyz, stride, pose_mode, hp, (const Pose*)d_pose,
+        FAR_LAUNCH(insert_commit_kernel, commit_grid, 256, 0, st, m->view, xyz, stride, pose_mode, hp, (const Pose*)d_pose,
                                                            first_id, m->d_touched, cov_by_list ? m->d_cov_list : nullptr,
                                                            m->max_batch);
         FAR_CUDA(cudaGetLastError());
@@ -508,7 +508,7 @@ static int insert_impl(far_map_t* m, const float* d_xyz, int64_t n, int stride, 
         if (rc != FAR_OK) return rc;
     }
     if (d_stats) {
-        insert_stats_kernel<<<1, 32, 0, st>>>(m->view, n, d_stats);
+        FAR_LAUNCH(insert_stats_kernel, 1, 32, 0, st, m->view, n, d_stats);
         FAR_CUDA(cudaGetLastError());
     }
     return FAR_OK;
@@ -530,9 +530,9 @@ static int prune_impl(far_map_t* m, const double* c, const far_pose_t* d_pose, d
     if (!m || (!c && !d_pose)) return FAR_ERR_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     const double r2 = radius * radius;
-    prune_kernel<<<grid_for(m->view.slots, 256), 256, 0, st>>>(m->view, c ? c[0] : 0.0, c ? c[1] : 0.0, c ? c[2] : 0.0,
+    FAR_LAUNCH(prune_kernel, grid_for(m->view.slots, 256), 256, 0, st, m->view, c ? c[0] : 0.0, c ? c[1] : 0.0, c ? c[2] : 0.0,
                                                                 (const Pose*)d_pose, r2);
-    prune_stats_kernel<<<1, 32, 0, st>>>(m->view, d_stats);
+    FAR_LAUNCH(prune_stats_kernel, 1, 32, 0, st, m->view, d_stats);
     FAR_CUDA(cudaGetLastError());
     return FAR_OK;
 }
@@ -551,8 +551,8 @@ int far_map_stats(far_map_t* m, far_map_stats_t* d_stats, void* stream) {
     if (!m || !d_stats) return FAR_ERR_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     unsigned long long* acc = reinterpret_cast<unsigned long long*>(m->view.ctr + 1);
-    stats_kernel<<<grid_for(m->view.slots, 256), 256, 0, st>>>(m->view, acc);
-    stats_out_kernel<<<1, 32, 0, st>>>(m->view, acc, m->next_id, d_stats);
+    FAR_LAUNCH(stats_kernel, grid_for(m->view.slots, 256), 256, 0, st, m->view, acc);
+    FAR_LAUNCH(stats_out_kernel, 1, 32, 0, st, m->view, acc, m->next_id, d_stats);
     FAR_CUDA(cudaGetLastError());
     return FAR_OK;
 }
@@ -563,9 +563,9 @@ int far_map_export(far_map_t* m, uint64_t* d_keys, int32_t* d_counts, float* d_p
     cudaStream_t st = (cudaStream_t)stream;
     unsigned long long* acc = reinterpret_cast<unsigned long long*>(m->view.ctr + 1) + 3;
     FAR_CUDA(cudaMemsetAsync(acc, 0, sizeof(unsigned long long), st));
-    export_kernel<<<grid_for(m->view.slots, 256), 256, 0, st>>>(m->view, (unsigned long long*)d_keys, d_counts,
+    FAR_LAUNCH(export_kernel, grid_for(m->view.slots, 256), 256, 0, st, m->view, (unsigned long long*)d_keys, d_counts,
                                                                  (float4*)d_points4, d_cov6, d_cov_valid, max_out, acc);
-    write_i64_kernel<<<1, 32, 0, st>>>(acc, d_n_voxels);
+    FAR_LAUNCH(write_i64_kernel, 1, 32, 0, st, acc, d_n_voxels);
     FAR_CUDA(cudaGetLastError());
     return FAR_OK;
 }
@@ -573,7 +573,7 @@ int far_map_export(far_map_t* m, uint64_t* d_keys, int32_t* d_counts, float* d_p
 int far_voxel_keys(const float* d_xyz, int64_t n, int stride, float voxel, uint64_t* d_keys, void* stream) {
     if ((!d_xyz && n > 0) || n < 0 || (stride != 3 && stride != 4) || !(voxel > 0.f) || (!d_keys && n > 0)) return FAR_ERR_ARG;
     if (n == 0) return FAR_OK;
-    voxel_keys_kernel<<<grid_for(n, 256), 256, 0, (cudaStream_t)stream>>>(d_xyz, n, stride, voxel,
+    FAR_LAUNCH(voxel_keys_kernel, grid_for(n, 256), 256, 0, (cudaStream_t)stream, d_xyz, n, stride, voxel,
                                                                           (unsigned long long*)d_keys);
     FAR_CUDA(cudaGetLastError());
     return FAR_OK;
@@ -606,9 +606,9 @@ int far_map_rehash(far_map_t* m, void* stream) {
     if (e == cudaSuccess && m->view.cov) e = cudaMalloc((void**)&t_ok, nv * cap + 1);
     if (e == cudaSuccess) e = cudaMemsetAsync(t_n, 0, 8, st);
     if (e == cudaSuccess) {
-        rehash_gather_kernel<<<grid_for(m->view.slots, 256), 256, 0, st>>>(m->view, t_keys, t_counts, t_pts, t_cov, t_ok, t_n);
+        FAR_LAUNCH(rehash_gather_kernel, grid_for(m->view.slots, 256), 256, 0, st, m->view, t_keys, t_counts, t_pts, t_cov, t_ok, t_n);
         if (nv > 0)
-            rehash_scatter_kernel<<<grid_for((int64_t)nv, 256), 256, 0, st>>>(m->view, t_keys, t_counts, t_pts, t_cov, t_ok, t_n);
+            FAR_LAUNCH(rehash_scatter_kernel, grid_for((int64_t)nv, 256), 256, 0, st, m->view, t_keys, t_counts, t_pts, t_cov, t_ok, t_n);
         else
             e = cudaMemsetAsync(&m->view.ctr->n_keys, 0, 8, st);
         if (e == cudaSuccess) e = cudaGetLastError();
@@ -616,6 +616,142 @@ int far_map_rehash(far_map_t* m, void* stream) {
     }
     cudaFree(t_keys); cudaFree(t_counts); cudaFree(t_pts); cudaFree(t_n); cudaFree(t_cov); cudaFree(t_ok);
     if (e != cudaSuccess) { far::set_cuda_error(e, "far_map_rehash"); return FAR_ERR_CUDA; }
+    return FAR_OK;
+}
+
+}  // extern "C"
+
+// =============================================================================================================
+// launch accounting / per-kernel timing (tracing facility) and map snapshots (checkpoint / restore)
+#include <atomic>
+#include <map>
+#include <mutex>
+#include <string>
+#include <vector>
+
+namespace far {
+
+static std::atomic<long long> g_launches{0};
+static std::atomic<int> g_prof{0};
+static std::mutex g_prof_mu;
+struct ProfRec { const char* name; cudaEvent_t a, b; };
+static std::vector<ProfRec> g_recs;
+
+LaunchScope::LaunchScope(const char* name, cudaStream_t st) : rec_(-1), st_(st) {
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    if (g_prof.load(std::memory_order_relaxed)) {
+        ProfRec r;
+        r.name = name;
+        if (cudaEventCreate(&r.a) == cudaSuccess && cudaEventCreate(&r.b) == cudaSuccess) {
+            cudaEventRecord(r.a, st);
+            std::lock_guard<std::mutex> lk(g_prof_mu);
+            g_recs.push_back(r);
+            rec_ = (int)g_recs.size() - 1;
+        }
+    }
+}
+
+LaunchScope::~LaunchScope() {
+    if (rec_ >= 0) {
+        std::lock_guard<std::mutex> lk(g_prof_mu);
+        cudaEventRecord(g_recs[rec_].b, st_);
+    }
+}
+
+}  // namespace far
+
+struct far_snapshot {
+    void *table, *points, *cov, *cov_ok, *ctr;
+    size_t b_table, b_points, b_cov, b_ok;
+    uint64_t next_id;
+};
+
+extern "C" {
+
+long long far_launch_count(void) { return far::g_launches.load(); }
+
+void far_profile_enable(int on) { far::g_prof.store(on ? 1 : 0); }
+
+// Synchronises the device, sums the recorded durations per kernel name and clears the records.
+// Writes up to max_entries rows: names[i] (borrowed static strings), total_ms[i], launches[i]; returns the row count.
+int far_profile_collect(const char** names, double* total_ms, long long* launches, int max_entries) {
+    cudaDeviceSynchronize();
+    std::lock_guard<std::mutex> lk(far::g_prof_mu);
+    std::map<std::string, std::pair<double, long long>> acc;
+    std::map<std::string, const char*> ptr;
+    for (auto& r : far::g_recs) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, r.a, r.b) == cudaSuccess) {
+            auto& e = acc[r.name];
+            e.first += ms;
+            e.second += 1;
+            ptr[r.name] = r.name;
+        }
+        cudaEventDestroy(r.a);
+        cudaEventDestroy(r.b);
+    }
+    far::g_recs.clear();
+    int i = 0;
+    for (auto& kv : acc) {
+        if (i >= max_entries) break;
+        if (names) names[i] = ptr[kv.first];
+        if (total_ms) total_ms[i] = kv.second.first;
+        if (launches) launches[i] = kv.second.second;
+        ++i;
+    }
+    return i;
+}
+
+int far_map_snapshot_destroy(far_snapshot_t* s) {
+    if (!s) return FAR_OK;
+    cudaFree(s->table); cudaFree(s->points); cudaFree(s->cov); cudaFree(s->cov_ok); cudaFree(s->ctr);
+    delete s;
+    return FAR_OK;
+}
+
+int far_map_snapshot_create(far_map_t* m, far_snapshot_t** out, void* stream) {
+    if (!m || !out) return FAR_ERR_ARG;
+    *out = nullptr;
+    cudaStream_t st = (cudaStream_t)stream;
+    far_snapshot* s = new (std::nothrow) far_snapshot();
+    if (!s) return FAR_ERR_ARG;
+    memset(s, 0, sizeof(*s));
+    const size_t npts = (size_t)m->view.slots * m->view.cap;
+    s->b_table = (size_t)m->view.slots * sizeof(Entry);
+    s->b_points = npts * sizeof(float4);
+    s->b_cov = m->view.cov ? npts * 6 * sizeof(float) : 0;
+    s->b_ok = m->view.cov_ok ? npts : 0;
+    s->next_id = m->next_id;
+    cudaError_t e = cudaMalloc(&s->table, s->b_table);
+    if (e == cudaSuccess) e = cudaMalloc(&s->points, s->b_points);
+    if (e == cudaSuccess && s->b_cov) e = cudaMalloc(&s->cov, s->b_cov);
+    if (e == cudaSuccess && s->b_ok) e = cudaMalloc(&s->cov_ok, s->b_ok);
+    if (e == cudaSuccess) e = cudaMalloc(&s->ctr, sizeof(Counters));
+    if (e == cudaSuccess) e = cudaMemcpyAsync(s->table, m->view.table, s->b_table, cudaMemcpyDeviceToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(s->points, m->view.points, s->b_points, cudaMemcpyDeviceToDevice, st);
+    if (e == cudaSuccess && s->b_cov) e = cudaMemcpyAsync(s->cov, m->view.cov, s->b_cov, cudaMemcpyDeviceToDevice, st);
+    if (e == cudaSuccess && s->b_ok) e = cudaMemcpyAsync(s->cov_ok, m->view.cov_ok, s->b_ok, cudaMemcpyDeviceToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(s->ctr, m->view.ctr, sizeof(Counters), cudaMemcpyDeviceToDevice, st);
+    if (e != cudaSuccess) {
+        far::set_cuda_error(e, "far_map_snapshot_create");
+        far_map_snapshot_destroy(s);
+        return FAR_ERR_CUDA;
+    }
+    *out = s;
+    return FAR_OK;
+}
+
+int far_map_snapshot_restore(far_map_t* m, const far_snapshot_t* s, void* stream) {
+    if (!m || !s) return FAR_ERR_ARG;
+    const size_t npts = (size_t)m->view.slots * m->view.cap;
+    if (s->b_table != (size_t)m->view.slots * sizeof(Entry) || s->b_points != npts * sizeof(float4)) return FAR_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    FAR_CUDA(cudaMemcpyAsync(m->view.table, s->table, s->b_table, cudaMemcpyDeviceToDevice, st));
+    FAR_CUDA(cudaMemcpyAsync(m->view.points, s->points, s->b_points, cudaMemcpyDeviceToDevice, st));
+    if (s->b_cov && m->view.cov) FAR_CUDA(cudaMemcpyAsync(m->view.cov, s->cov, s->b_cov, cudaMemcpyDeviceToDevice, st));
+    if (s->b_ok && m->view.cov_ok) FAR_CUDA(cudaMemcpyAsync(m->view.cov_ok, s->cov_ok, s->b_ok, cudaMemcpyDeviceToDevice, st));
+    FAR_CUDA(cudaMemcpyAsync(m->view.ctr, s->ctr, sizeof(Counters), cudaMemcpyDeviceToDevice, st));
+    m->next_id = s->next_id;
     return FAR_OK;
 }
 

@@ -67,6 +67,22 @@ __global__ void __launch_bounds__(QWARPS * 32) nn_kernel(MapView m, const float*
     }
 }
 
+__global__ void __launch_bounds__(QWARPS * 32) count27_kernel(MapView m, const float* __restrict__ q, int64_t n, int stride,
+                                                               int32_t* __restrict__ out) {
+    __shared__ int s_off[QWARPS][32];
+    __shared__ uint32_t s_slot[QWARPS][32];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const int64_t nwarps = (int64_t)gridDim.x * QWARPS;
+    for (int64_t i = (int64_t)blockIdx.x * QWARPS + wib; i < n; i += nwarps) {
+        const float* qq = q + i * stride;
+        int k[3];
+        int total = 0;
+        if (voxel_index(__ldg(qq), __ldg(qq + 1), __ldg(qq + 2), m.voxel, k)) total = probe27(m, k, lane, s_off[wib], s_slot[wib]);
+        if (lane == 0) out[i] = total;
+        __syncwarp();
+    }
+}
+
 // ---- A7: k nearest by (d2, id) -> Eq. 1 -----------------------------------------------------------------------
 // dynamic shared memory per warp: double d2[27*cap] | u32 id[27*cap] | int off[32] | u32 slot[32] | int sel[32]
 __host__ __device__ inline size_t knn_smem_per_warp(int cap) { return (size_t)27 * cap * 12 + 3 * 32 * 4; }
@@ -245,7 +261,7 @@ int launch_knn_cov_refs(const far_map* map, const uint32_t* d_refs, const unsign
     KnnLaunch L;
     int rc = knn_launch_cfg(map, knn_cov_refs_kernel, n_max, L);
     if (rc != FAR_OK) return rc;
-    knn_cov_refs_kernel<<<L.grid, L.warps * 32, L.smem, st>>>(map->view, d_refs, d_n, L.warps);
+    FAR_LAUNCH(knn_cov_refs_kernel, L.grid, L.warps * 32, L.smem, st, map->view, d_refs, d_n, L.warps);
     FAR_CUDA(cudaGetLastError());
     return FAR_OK;
 }
@@ -254,7 +270,7 @@ int launch_knn_cov_new_ids(const far_map* map, uint32_t first_id, cudaStream_t s
     KnnLaunch L;
     int rc = knn_launch_cfg(map, knn_cov_new_ids_kernel, map->view.slots, L);
     if (rc != FAR_OK) return rc;
-    knn_cov_new_ids_kernel<<<L.grid, L.warps * 32, L.smem, st>>>(map->view, first_id, L.warps);
+    FAR_LAUNCH(knn_cov_new_ids_kernel, L.grid, L.warps * 32, L.smem, st, map->view, first_id, L.warps);
     FAR_CUDA(cudaGetLastError());
     return FAR_OK;
 }
@@ -269,7 +285,18 @@ int far_map_nn(const far_map_t* map, const float* d_q, int64_t m, int stride, ui
     int64_t grid = (int64_t)map->sm_count * 8;   // 8 blocks x 8 warps = 64 warps per SM: one full wave
     const int64_t need = (m + QWARPS - 1) / QWARPS;
     if (need < grid) grid = need;
-    nn_kernel<<<(int)grid, QWARPS * 32, 0, (cudaStream_t)stream>>>(map->view, d_q, m, stride, d_id, d_d2);
+    FAR_LAUNCH(nn_kernel, (int)grid, QWARPS * 32, 0, (cudaStream_t)stream, map->view, d_q, m, stride, d_id, d_d2);
+    FAR_CUDA(cudaGetLastError());
+    return FAR_OK;
+}
+
+int far_map_count27(const far_map_t* map, const float* d_q, int64_t m, int stride, int32_t* d_count, void* stream) {
+    if (!map || m < 0 || (stride != 3 && stride != 4) || (m > 0 && (!d_q || !d_count))) return FAR_ERR_ARG;
+    if (m == 0) return FAR_OK;
+    int64_t grid = (int64_t)map->sm_count * 8;
+    const int64_t need = (m + QWARPS - 1) / QWARPS;
+    if (need < grid) grid = need;
+    FAR_LAUNCH(count27_kernel, (int)grid, QWARPS * 32, 0, (cudaStream_t)stream, map->view, d_q, m, stride, d_count);
     FAR_CUDA(cudaGetLastError());
     return FAR_OK;
 }
@@ -281,7 +308,7 @@ static int knn_cov_impl(const far_map_t* map, const float* d_q, int64_t m, const
     KnnLaunch L;
     int rc = knn_launch_cfg(map, knn_cov_points_kernel, m, L);
     if (rc != FAR_OK) return rc;
-    knn_cov_points_kernel<<<L.grid, L.warps * 32, L.smem, (cudaStream_t)stream>>>(map->view, d_q, m, d_m, stride, d_cov6,
+    FAR_LAUNCH(knn_cov_points_kernel, L.grid, L.warps * 32, L.smem, (cudaStream_t)stream, map->view, d_q, m, d_m, stride, d_cov6,
                                                                                   d_valid, L.warps);
     FAR_CUDA(cudaGetLastError());
     return FAR_OK;

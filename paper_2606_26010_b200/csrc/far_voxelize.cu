@@ -150,7 +150,7 @@ extern "C" int far_voxelize(const float* d_xyz, int64_t n, int stride, float vox
     if (*workspace_bytes < need || !d_n_out || (n > 0 && (!d_xyz || !d_out_xyz || !d_out_index))) return FAR_ERR_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     if (n == 0) {
-        zero_i64_kernel<<<1, 32, 0, st>>>(d_n_out);
+        FAR_LAUNCH(zero_i64_kernel, 1, 32, 0, st, d_n_out);
         FAR_CUDA(cudaGetLastError());
         return FAR_OK;
     }
@@ -163,10 +163,10 @@ extern "C" int far_voxelize(const float* d_xyz, int64_t n, int stride, float vox
     w.slots = (uint32_t)slots;
     w.mask = (uint32_t)slots - 1;
     FAR_CUDA(cudaMemsetAsync(base, 0xFF, b_keys + b_first, st));   // keys = empty, first = +inf
-    vox_claim_kernel<<<grid_for(n, 256), 256, 0, st>>>(w, d_xyz, n, stride, voxel);
-    vox_count_kernel<<<(int)tiles, VTILE, 0, st>>>(w, n);
-    vox_scan_kernel<<<1, 1024, 0, st>>>(w, (int)tiles, d_n_out);
-    vox_scatter_kernel<<<(int)tiles, VTILE, 0, st>>>(w, d_xyz, n, stride, d_out_xyz, d_out_index);
+    FAR_LAUNCH(vox_claim_kernel, grid_for(n, 256), 256, 0, st, w, d_xyz, n, stride, voxel);
+    FAR_LAUNCH(vox_count_kernel, (int)tiles, VTILE, 0, st, w, n);
+    FAR_LAUNCH(vox_scan_kernel, 1, 1024, 0, st, w, (int)tiles, d_n_out);
+    FAR_LAUNCH(vox_scatter_kernel, (int)tiles, VTILE, 0, st, w, d_xyz, n, stride, d_out_xyz, d_out_index);
     FAR_CUDA(cudaGetLastError());
     return FAR_OK;
 }

@@ -51,6 +51,7 @@ def test_struct_sizes_match_header_layout():
     assert C.sizeof(far.GicpOptions) == 32
     assert C.sizeof(far.GicpResult) == 96 + 36 * 8 + 6 * 8 + 8 + 16
     assert C.sizeof(far.MapConfig) == 48
+    assert C.sizeof(far.FrontendConfig) == 48 + 8 + 8 + 8 + 8 + 32
 
 
 def test_default_options_are_the_papers():

@@ -271,3 +271,37 @@ def test_c2_reduced_frame_end_to_end_device_chain():
     assert np.array_equal(eg["keys"], eo["keys"]) and np.array_equal(eg["counts"], eo["counts"])
     assert np.array_equal(eg["ids"], eo["ids"])
     assert np.abs(eg["xyz"] - eo["xyz"]).max() < 1e-5
+
+
+def test_frontend_chain_equals_manual_chain_and_host_variant():
+    """far_frontend_process (device scan) and far_frontend_process_host (host scan) give the oracle's frame."""
+    c2 = scenes.c2_single_frame(seed=5, n_map_candidates=120_000, map_radius=50.0, rings=16, azimuths=512)
+    v, cap, sigma = c2["voxel"], c2["cap"], c2["sigma"]
+    scan = c2["scan"]
+    mo = oracle.Map(v, cap)
+    mo.insert(c2["map_points"], compute_cov=True)
+    ds_o, _ = oracle.voxelize(scan, v)
+    lo = oracle.Map(v, cap); lo.insert(scan)
+    cov_o, val_o = lo.knn_cov(ds_o, nthreads=8)
+    o = mo.gicp_register(ds_o, cov_o, val_o, c2["T_init"], sigma, 30, nthreads=8)
+    mo.insert(scan, pose=(o["R"], o["t"]), compute_cov=True)
+    mo.prune(o["t"], 35.0)
+    eo = mo.export(with_cov=True)
+    for host in (False, True):
+        fe = far.Frontend(v, cap, 4 * len(c2["map_points"]), len(scan) + 7, prune_radius=35.0, max_iters=30)
+        fe.map.insert(c2["map_points"], compute_cov=True)
+        if host:
+            g = fe.process_host(torch.as_tensor(scan).pin_memory(), c2["T_init"], sigma)
+        else:
+            d_res = torch.zeros(far.GICP_RESULT_BYTES, dtype=torch.uint8, device="cuda")
+            fe.process_enqueue(torch.as_tensor(scan).cuda(), c2["T_init"], sigma, d_result=d_res)
+            torch.cuda.synchronize()
+            g = far.result_to_dict(far.GicpResult.from_buffer_copy(d_res.cpu().numpy().tobytes()))
+        assert g["status"] == 0 and g["iters"] == o["iters"] and g["n_inliers"] == o["n_inliers"]
+        dt, dr = _pose_err(g, o)
+        assert dt < 1e-4 and dr < 1e-5, (dt, dr)
+        eg = fe.map.export(with_cov=True)
+        assert np.array_equal(eg["keys"], eo["keys"]) and np.array_equal(eg["ids"], eo["ids"])
+        assert np.abs(eg["xyz"] - eo["xyz"]).max() < 1e-5
+        assert np.array_equal(eg["cov_valid"], eo["cov_valid"])
+        fe.close()

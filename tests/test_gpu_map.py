@@ -298,3 +298,36 @@ def test_empty_calls():
     assert int(valid[0]) == 0 and cov[0].tolist() == [1, 0, 0, 1, 0, 1]
     assert m.export()["keys"].size == 0
     assert m.prune([0, 0, 0], 1.0) == dict(n_voxels_removed=0, n_points_removed=0, n_voxels_left=0, n_points_left=0)
+
+
+def test_snapshot_restore_count27_and_launch_accounting():
+    rng = np.random.default_rng(21)
+    pts = _cloud(rng, 40_000, scale=12.0)
+    mo, mg = oracle.Map(0.5, 20), far.Map(0.5, 20, 100_000, with_cov=True)
+    mo.insert(pts[:20_000], compute_cov=True); mg.insert(pts[:20_000], compute_cov=True)
+    snap = mg.snapshot()
+    before = mg.export(with_cov=True)
+    n0 = far.launch_count()
+    mg.insert(pts[20_000:], compute_cov=True)
+    mg.prune([0, 0, 0], 5.0)
+    assert far.launch_count() - n0 >= 5            # claim, commit, knn_cov, stats, prune, ...
+    mg.restore(snap)
+    after = mg.export(with_cov=True)
+    for k in ("keys", "counts", "ids", "xyz", "cov", "cov_valid"):
+        assert np.array_equal(before[k].view(np.uint8), after[k].view(np.uint8)), k
+    assert mg.size() == mo.size()
+    # the restored map continues exactly like the oracle (ids continue from the snapshot's counter)
+    assert mg.insert(pts[20_000:]) == mo.insert(pts[20_000:])
+    _assert_same_map(mg.export(), mo.export())
+    far.Map.snapshot_destroy(snap)
+    # count27 = number of candidates the 27-voxel search scans, checked against the oracle's k-NN list length
+    q = pts[:500]
+    cnt = mg.count27(q).cpu().numpy()
+    ids, _ = mo.knn(q, 27 * 20)
+    assert np.array_equal(cnt, (ids != oracle.NO_ID).sum(axis=1))
+    # per-kernel timing facility
+    far.profile_enable(True)
+    mg.nn(q)
+    far.profile_enable(False)
+    prof = far.profile_collect()
+    assert "nn_kernel" in prof and prof["nn_kernel"][1] == 1 and prof["nn_kernel"][0] > 0
