@@ -15,13 +15,10 @@
 // last-arriving block in a fixed order (deterministic, no floating atomics), the 6x6 Cholesky solve, SE(3)
 // exponential and pose update done by one thread of that last block in FP64, and one grid-wide barrier per
 // iteration.  The host is not involved until it reads the result.
-#include <cooperative_groups.h>
-
 #include <cstring>
 
 #include "far_internal.h"
 
-namespace cg = cooperative_groups;
 using namespace far;
 
 namespace far {
@@ -30,10 +27,16 @@ constexpr int GWARPS = 8;        // warps per block
 constexpr int NTERMS = 29;       // 21 (H upper triangle) + 6 (b) + chi2 + inlier count
 constexpr int TSTRIDE = 32;      // padded row of per-block partials
 
+constexpr int GROUP = 32;        // blocks per first-level reduction group
+constexpr int MAX_GROUPS = 64;
+constexpr int GICP_BLOCKS_PER_SM = 5;
+
 struct GicpState {
     Pose pose;
     int done;
-    unsigned int ticket;
+    unsigned int ticket;                    // groups that finished their first-level sum
+    unsigned int epoch;                     // iterations completed (published after the pose)
+    unsigned int group_ticket[MAX_GROUPS];  // blocks of a group that wrote their partial row
 };
 
 struct GicpParams {
@@ -48,6 +51,7 @@ struct GicpParams {
     double tau2, kappa, conv_eps;
     int kernel, max_iters, linearize_only;
     double* partials;           // [gridDim.x][TSTRIDE]
+    double* partials2;          // [groups][TSTRIDE]
     GicpState* state;
     far_gicp_result_t* out;
 };
@@ -143,70 +147,164 @@ __device__ __forceinline__ void correspondence_terms(const Pose& T, const double
     terms[28] = 1.0;
 }
 
-// 6x6 Cholesky solve H x = rhs (FP64); false if H is not positive definite
-__device__ bool chol_solve6(const double* H, const double* rhs, double* x) {
-    double L[36];
-    for (int i = 0; i < 36; ++i) L[i] = 0.0;
-    for (int i = 0; i < 6; ++i)
-        for (int j = 0; j <= i; ++j) {
-            double s = H[6 * i + j];
-            for (int k = 0; k < j; ++k) s -= L[6 * i + k] * L[6 * j + k];
-            if (i == j) {
-                if (!(s > 0.0) || !isfinite(s)) return false;
-                L[6 * i + i] = sqrt(s);
-            } else {
-                L[6 * i + j] = s / L[6 * j + j];
-            }
+// 6x6 Cholesky solve H x = rhs (FP64), fully unrolled so L lives in registers; one rsqrt per pivot and
+// multiplications by the reciprocal pivots instead of 27 divisions (this thread is the serial section of every
+// Gauss-Newton iteration).  false if H is not positive definite.
+__device__ __forceinline__ bool chol_solve6(const double* H, const double* rhs, double* x) {
+    double L[6][6], inv[6];
+#pragma unroll
+    for (int j = 0; j < 6; ++j) {
+        double s = H[6 * j + j];
+#pragma unroll
+        for (int k = 0; k < j; ++k) s -= L[j][k] * L[j][k];
+        if (!(s > 0.0) || !isfinite(s)) return false;
+        inv[j] = rsqrt(s);
+        L[j][j] = s * inv[j];
+#pragma unroll
+        for (int i = j + 1; i < 6; ++i) {
+            double t = H[6 * i + j];
+#pragma unroll
+            for (int k = 0; k < j; ++k) t -= L[i][k] * L[j][k];
+            L[i][j] = t * inv[j];
         }
-    double y[6];
-    for (int i = 0; i < 6; ++i) {
-        double s = rhs[i];
-        for (int k = 0; k < i; ++k) s -= L[6 * i + k] * y[k];
-        y[i] = s / L[6 * i + i];
     }
+    double y[6];
+#pragma unroll
+    for (int i = 0; i < 6; ++i) {
+        double t = rhs[i];
+#pragma unroll
+        for (int k = 0; k < i; ++k) t -= L[i][k] * y[k];
+        y[i] = t * inv[i];
+    }
+#pragma unroll
     for (int i = 5; i >= 0; --i) {
-        double s = y[i];
-        for (int k = i + 1; k < 6; ++k) s -= L[6 * k + i] * x[k];
-        x[i] = s / L[6 * i + i];
+        double t = y[i];
+#pragma unroll
+        for (int k = i + 1; k < 6; ++k) t -= L[k][i] * x[k];
+        x[i] = t * inv[i];
     }
     return true;
 }
 
 // SE(3) exponential of delta = (rho, phi), translation first (R12); series below theta = 1e-8
-__device__ void se3_exp(const double* d, Pose& E) {
-    const double phi[3] = {d[3], d[4], d[5]};
-    const double th2 = phi[0] * phi[0] + phi[1] * phi[1] + phi[2] * phi[2];
+__device__ __forceinline__ void se3_exp(const double* d, Pose& E) {
+    const double px = d[3], py = d[4], pz = d[5];
+    const double th2 = px * px + py * py + pz * pz;
     const double th = sqrt(th2);
     double A, B, C;
     if (th < 1e-8) {
         A = 1.0 - th2 / 6.0; B = 0.5 - th2 / 24.0; C = 1.0 / 6.0 - th2 / 120.0;
     } else {
-        A = sin(th) / th; B = (1.0 - cos(th)) / th2; C = (th - sin(th)) / (th2 * th);
+        double sn, cs;
+        sincos(th, &sn, &cs);
+        const double ith = 1.0 / th, ith2 = ith * ith;
+        A = sn * ith; B = (1.0 - cs) * ith2; C = (th - sn) * ith2 * ith;
     }
-    const double K[9] = {0, -phi[2], phi[1], phi[2], 0, -phi[0], -phi[1], phi[0], 0};
-    double K2[9], V[9];
-    for (int i = 0; i < 3; ++i)
-        for (int j = 0; j < 3; ++j) {
-            double s = 0.0;
-            for (int k = 0; k < 3; ++k) s += K[3 * i + k] * K[3 * k + j];
-            K2[3 * i + j] = s;
-        }
+    const double K[9] = {0, -pz, py, pz, 0, -px, -py, px, 0};
+    // K^2 = phi phi^T - |phi|^2 I
+    const double K2[9] = {px * px - th2, px * py, px * pz, px * py, py * py - th2, py * pz, px * pz, py * pz, pz * pz - th2};
+    double V[9];
+#pragma unroll
     for (int i = 0; i < 9; ++i) {
         const double I = (i % 4 == 0) ? 1.0 : 0.0;
         E.R[i] = I + A * K[i] + B * K2[i];
         V[i] = I + B * K[i] + C * K2[i];
     }
+#pragma unroll
     for (int r = 0; r < 3; ++r) E.t[r] = V[3 * r] * d[0] + V[3 * r + 1] * d[1] + V[3 * r + 2] * d[2];
 }
 
-__global__ void __launch_bounds__(GWARPS * 32, 4) gicp_kernel(MapView m, GicpParams P) {
+// Serial section of one iteration (one thread of the last-arriving block): assemble H, b from the 29 reduced
+// terms, solve, update the pose, decide termination, publish.
+__device__ __noinline__ void solve_and_update(const GicpParams& P, const double* tv, const Pose& T, int it) {
+    double H[36], b[6];
+    {
+        int q = 0;
+#pragma unroll
+        for (int a = 0; a < 6; ++a)
+#pragma unroll
+            for (int c = a; c < 6; ++c) { H[6 * a + c] = tv[q]; H[6 * c + a] = tv[q]; ++q; }
+    }
+#pragma unroll
+    for (int a = 0; a < 6; ++a) b[a] = tv[21 + a];
+    const int n_inl = (int)(tv[28] + 0.5);
+    bool done = false;
+    int converged = 0, status = FAR_OK;
+    Pose Tn = T;
+    if (!P.linearize_only) {
+        double rhs[6], delta[6];
+#pragma unroll
+        for (int a = 0; a < 6; ++a) rhs[a] = -b[a];
+        if (n_inl < 6 || !chol_solve6(H, rhs, delta)) {
+            status = FAR_ERR_DEGENERATE;
+            Tn = P.d_init ? *P.d_init : P.init;
+            done = true;
+        } else {
+            Pose E;
+            se3_exp(delta, E);
+#pragma unroll
+            for (int i = 0; i < 3; ++i)
+#pragma unroll
+                for (int j = 0; j < 3; ++j)
+                    Tn.R[3 * i + j] = E.R[3 * i] * T.R[j] + E.R[3 * i + 1] * T.R[3 + j] + E.R[3 * i + 2] * T.R[6 + j];
+#pragma unroll
+            for (int r = 0; r < 3; ++r)
+                Tn.t[r] = (E.R[3 * r] * T.t[0] + E.R[3 * r + 1] * T.t[1] + E.R[3 * r + 2] * T.t[2]) + E.t[r];
+            double nrm = 0.0;
+#pragma unroll
+            for (int a = 0; a < 6; ++a) nrm += delta[a] * delta[a];
+            if (nrm <= P.conv_eps * P.conv_eps) { converged = 1; done = true; }   // PAPER.md:100, R13: ||delta||_2 <= eps
+        }
+    } else {
+        done = true;
+    }
+    if (it + 1 >= P.max_iters) done = true;
+    P.state->pose = Tn;
+    if (done) {
+        far_gicp_result_t* out = P.out;
+        for (int a = 0; a < 9; ++a) out->pose.R[a] = Tn.R[a];
+        for (int a = 0; a < 3; ++a) out->pose.t[a] = Tn.t[a];
+        for (int a = 0; a < 36; ++a) out->H[a] = H[a];
+        for (int a = 0; a < 6; ++a) out->b[a] = b[a];
+        out->chi2 = tv[27];
+        out->n_inliers = n_inl;
+        out->iters = it + 1;
+        out->converged = converged;
+        out->status = status;
+    }
+    P.state->done = done ? 1 : 0;
+}
+
+// sum rows [first, first + count) of a [rows][TSTRIDE] array of doubles, column = lane; 8 warps x 32 lanes.
+// Every load is independent (one memory latency for up to 32 rows); the additions happen in a fixed order.
+__device__ __forceinline__ double block_sum_rows(const double* rows, int first, int count, int lane, int wib,
+                                                 double (*s_red)[TSTRIDE]) {
+    double v[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const int r = wib + GWARPS * u;
+        v[u] = r < count ? __ldcg(rows + (size_t)(first + r) * TSTRIDE + lane) : 0.0;
+    }
+    double s = (v[0] + v[1]) + (v[2] + v[3]);
+    for (int r = wib + 4 * GWARPS; r < count; r += GWARPS) s += __ldcg(rows + (size_t)(first + r) * TSTRIDE + lane);
+    s_red[wib][lane] = s;
+    __syncthreads();
+    double t = 0.0;
+    if (wib == 0) {
+#pragma unroll
+        for (int w8 = 0; w8 < GWARPS; ++w8) t += s_red[w8][lane];
+    }
+    __syncthreads();
+    return t;   // valid in warp 0
+}
+
+__global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(MapView m, GicpParams P) {
     __shared__ int s_off[GWARPS][32];
     __shared__ uint32_t s_slot[GWARPS][32];
     __shared__ double s_terms[GWARPS][TSTRIDE];
     __shared__ double s_red[GWARPS][TSTRIDE];
     __shared__ Pose s_T;
-    __shared__ int s_last;
-    cg::grid_group grid = cg::this_grid();
+    __shared__ int s_flag;
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const int64_t nwarps = (int64_t)gridDim.x * GWARPS;
     int64_t n = P.n;
@@ -217,6 +315,10 @@ __global__ void __launch_bounds__(GWARPS * 32, 4) gicp_kernel(MapView m, GicpPar
         if (threadIdx.x < 9) s_T.R[threadIdx.x] = vv; else s_T.t[threadIdx.x - 9] = vv;
     }
     __syncthreads();
+    const int n_groups = (gridDim.x + GROUP - 1) / GROUP;
+    const int group = blockIdx.x / GROUP;
+    const int group_rows = min(GROUP, (int)gridDim.x - group * GROUP);
+    const bool have_scan_cov = P.cov6 != nullptr && P.valid != nullptr && m.cov != nullptr;
 
     for (int it = 0; it < P.max_iters; ++it) {
         // ---- A8 + A9: one warp per source point; lane t < 29 accumulates term t ---------------------------------
@@ -225,6 +327,12 @@ __global__ void __launch_bounds__(GWARPS * 32, 4) gicp_kernel(MapView m, GicpPar
             const float* sp = P.scan + i * P.stride;
             const float sx = __ldg(sp), sy = __ldg(sp + 1), sz = __ldg(sp + 2);
             if (!(isfinite(sx) && isfinite(sy) && isfinite(sz))) continue;
+            // the source covariance does not depend on the search: lanes 8..13 fetch it now, lane 14 its flag
+            float cin = 0.f;
+            if (have_scan_cov) {
+                if (lane >= 8 && lane < 14) cin = __ldg(P.cov6 + 6 * i + (lane - 8));
+                if (lane == 14) cin = (float)__ldg(P.valid + i);
+            }
             float pf[3];
             transform_point(s_T, sx, sy, sz, pf);                 // Eq. 2 with the accumulated pose (R11)
             int k[3];
@@ -235,13 +343,14 @@ __global__ void __launch_bounds__(GWARPS * 32, 4) gicp_kernel(MapView m, GicpPar
             best.d2 = __longlong_as_double(0x7FF0000000000000ll);
             best.id = NO_ID;
             best.ref = 0;
+            float bx = 0.f, by = 0.f, bz = 0.f;
             int v = 0;
             for (int j = lane; j < total; j += 32) {
                 const uint32_t ref = g_cand_ref(s_off[wib], s_slot[wib], j, v, m.cap);
                 const float4 q = __ldg(m.points + ref);
                 const double d2 = dist2(pf[0], pf[1], pf[2], q.x, q.y, q.z);
                 const uint32_t id = __float_as_uint(q.w);
-                if (better(d2, id, best)) { best.d2 = d2; best.id = id; best.ref = ref; }
+                if (better(d2, id, best)) { best.d2 = d2; best.id = id; best.ref = ref; bx = q.x; by = q.y; bz = q.z; }
             }
             __syncwarp();
             const int w = warp_argmin(best.d2, best.id);
@@ -249,19 +358,23 @@ __global__ void __launch_bounds__(GWARPS * 32, 4) gicp_kernel(MapView m, GicpPar
             const uint32_t bid = __shfl_sync(FULL, best.id, w);
             const uint32_t bref = __shfl_sync(FULL, best.ref, w);
             if (bid == NO_ID || bd2 > P.tau2) continue;           // adaptive-threshold gate
-            if (lane == 0) {
-                const float4 rp = __ldg(m.points + bref);
-                const double p[3] = {(double)pf[0], (double)pf[1], (double)pf[2]};
-                const double r[3] = {(double)rp.x, (double)rp.y, (double)rp.z};
-                bool full = P.cov6 && P.valid && P.valid[i] != 0 && m.cov_ok && m.cov_ok[bref] != 0;
-                correspondence_terms(s_T, p, r, full, full ? P.cov6 + 6 * i : nullptr, full ? m.cov + (size_t)bref * 6 : nullptr,
-                                     P.kernel, P.kappa, s_terms[wib]);
+            // the winning lane already holds r; lanes 0..5 fetch Sigma_r, lane 6 its flag: one memory level
+            const double r[3] = {(double)__shfl_sync(FULL, bx, w), (double)__shfl_sync(FULL, by, w), (double)__shfl_sync(FULL, bz, w)};
+            if (have_scan_cov) {
+                if (lane < 6) cin = __ldg(m.cov + (size_t)bref * 6 + lane);
+                if (lane == 6) cin = (float)__ldg(m.cov_ok + bref);
             }
+            float cr[6], cs[6];
+#pragma unroll
+            for (int a = 0; a < 6; ++a) { cr[a] = __shfl_sync(FULL, cin, a); cs[a] = __shfl_sync(FULL, cin, 8 + a); }
+            const bool full = have_scan_cov && __shfl_sync(FULL, cin, 6) != 0.f && __shfl_sync(FULL, cin, 14) != 0.f;
+            const double p[3] = {(double)pf[0], (double)pf[1], (double)pf[2]};
+            if (lane == 0) correspondence_terms(s_T, p, r, full, cs, cr, P.kernel, P.kappa, s_terms[wib]);
             __syncwarp();
             if (lane < NTERMS) acc += s_terms[wib][lane];
             __syncwarp();
         }
-        // ---- A10: warp -> block -> last block, fixed order --------------------------------------------------------
+        // ---- A10: warp -> block -> group of 32 blocks -> grid, every level in a fixed order ----------------------
         s_red[wib][lane] = lane < NTERMS ? acc : 0.0;
         __syncthreads();
         if (wib == 0) {
@@ -272,82 +385,41 @@ __global__ void __launch_bounds__(GWARPS * 32, 4) gicp_kernel(MapView m, GicpPar
             __threadfence();
         }
         __syncthreads();
-        if (threadIdx.x == 0) {
-            const unsigned int t = atomicAdd(&P.state->ticket, 1u);
-            s_last = (t == gridDim.x - 1) ? 1 : 0;
-        }
+        if (threadIdx.x == 0) s_flag = (atomicAdd(&P.state->group_ticket[group], 1u) == (unsigned)group_rows - 1) ? 1 : 0;
         __syncthreads();
-        if (s_last) {
+        if (s_flag) {   // last block of its group: fold the group's rows into one
             __threadfence();
-            // 8 warps each sum a strided subset of the blocks, then warp 0 combines them: same order every run
-            double s = 0.0;
-            for (unsigned b = wib; b < gridDim.x; b += GWARPS) s += __ldcg(P.partials + (size_t)b * TSTRIDE + lane);
-            s_red[wib][lane] = s;
-            __syncthreads();
+            const double t = block_sum_rows(P.partials, group * GROUP, group_rows, lane, wib, s_red);
             if (wib == 0) {
-                double tsum = 0.0;
-#pragma unroll
-                for (int w8 = 0; w8 < GWARPS; ++w8) tsum += s_red[w8][lane];
-                s_terms[0][lane] = tsum;
+                P.partials2[(size_t)group * TSTRIDE + lane] = t;
+                __threadfence();
             }
             __syncthreads();
             if (threadIdx.x == 0) {
-                const double* tv = s_terms[0];
-                double H[36], b[6];
-                int q = 0;
-                for (int a = 0; a < 6; ++a)
-                    for (int c = a; c < 6; ++c) { H[6 * a + c] = tv[q]; H[6 * c + a] = tv[q]; ++q; }
-                for (int a = 0; a < 6; ++a) b[a] = tv[21 + a];
-                const int n_inl = (int)(tv[28] + 0.5);
-                far_gicp_result_t* out = P.out;
-                bool done = false;
-                int converged = 0, status = FAR_OK;
-                Pose Tn = s_T;
-                if (!P.linearize_only) {
-                    double rhs[6], delta[6];
-                    for (int a = 0; a < 6; ++a) rhs[a] = -b[a];
-                    if (n_inl < 6 || !chol_solve6(H, rhs, delta)) {
-                        status = FAR_ERR_DEGENERATE;
-                        Tn = P.d_init ? *P.d_init : P.init;
-                        done = true;
-                    } else {
-                        Pose E;
-                        se3_exp(delta, E);
-                        for (int i = 0; i < 3; ++i)
-                            for (int j = 0; j < 3; ++j) {
-                                double s2 = 0.0;
-                                for (int kk = 0; kk < 3; ++kk) s2 += E.R[3 * i + kk] * s_T.R[3 * kk + j];
-                                Tn.R[3 * i + j] = s2;
-                            }
-                        for (int r = 0; r < 3; ++r)
-                            Tn.t[r] = (E.R[3 * r] * s_T.t[0] + E.R[3 * r + 1] * s_T.t[1] + E.R[3 * r + 2] * s_T.t[2]) + E.t[r];
-                        double nrm = 0.0;
-                        for (int a = 0; a < 6; ++a) nrm += delta[a] * delta[a];
-                        if (sqrt(nrm) <= P.conv_eps) { converged = 1; done = true; }   // PAPER.md:100, R13
-                    }
-                } else {
-                    done = true;
-                }
-                if (it + 1 >= P.max_iters) done = true;
-                P.state->pose = Tn;
-                if (done) {
-                    for (int a = 0; a < 9; ++a) out->pose.R[a] = Tn.R[a];
-                    for (int a = 0; a < 3; ++a) out->pose.t[a] = Tn.t[a];
-                    for (int a = 0; a < 36; ++a) out->H[a] = H[a];
-                    for (int a = 0; a < 6; ++a) out->b[a] = b[a];
-                    out->chi2 = tv[27];
-                    out->n_inliers = n_inl;
-                    out->iters = it + 1;
-                    out->converged = converged;
-                    out->status = status;
-                }
-                P.state->done = done ? 1 : 0;
-                P.state->ticket = 0u;
+                P.state->group_ticket[group] = 0u;
+                s_flag = (atomicAdd(&P.state->ticket, 1u) == (unsigned)n_groups - 1) ? 2 : 1;
+            }
+            __syncthreads();
+            if (s_flag == 2) {   // last group: final sum, solve, publish
                 __threadfence();
+                const double t2 = block_sum_rows(P.partials2, 0, n_groups, lane, wib, s_red);
+                if (wib == 0) s_terms[0][lane] = t2;
+                __syncthreads();
+                if (threadIdx.x == 0) {
+                    solve_and_update(P, s_terms[0], s_T, it);
+                    P.state->ticket = 0u;
+                    __threadfence();
+                    atomicExch(&P.state->epoch, (unsigned)(it + 1));
+                }
             }
         }
-        grid.sync();
-        if (*reinterpret_cast<volatile int*>(&P.state->done)) break;
+        // ---- grid-wide wait for the new pose: all blocks are co-resident (cooperative launch) -------------------
+        if (threadIdx.x == 0) {
+            while (*reinterpret_cast<volatile unsigned int*>(&P.state->epoch) < (unsigned)(it + 1)) __nanosleep(32);
+            __threadfence();
+        }
+        __syncthreads();
+        if (__ldcg(&P.state->done)) break;
         if (threadIdx.x < 12) {
             const double vv = __ldcg(threadIdx.x < 9 ? &P.state->pose.R[threadIdx.x] : &P.state->pose.t[threadIdx.x - 9]);
             if (threadIdx.x < 9) s_T.R[threadIdx.x] = vv; else s_T.t[threadIdx.x - 9] = vv;
@@ -389,6 +461,7 @@ static int gicp_launch(const far_map_t* map, const float* d_scan, const float* d
     P.conv_eps = o.conv_eps;
     P.kernel = o.kernel; P.max_iters = max_iters; P.linearize_only = linearize_only;
     P.partials = map->d_gicp_partials;
+    P.partials2 = map->d_gicp_partials + (size_t)map->gicp_max_grid * TSTRIDE;
     P.state = (GicpState*)map->d_gicp_state;
     P.out = d_out;
     int64_t grid = map->gicp_max_grid;
@@ -435,7 +508,8 @@ int gicp_setup(far_map* map) {
     FAR_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gicp_kernel, GWARPS * 32, 0));
     if (per_sm < 1) per_sm = 1;
     map->gicp_max_grid = map->sm_count * per_sm;
-    FAR_CUDA(cudaMalloc((void**)&map->d_gicp_partials, (size_t)map->gicp_max_grid * TSTRIDE * sizeof(double)));
+    if (map->gicp_max_grid > GROUP * MAX_GROUPS) map->gicp_max_grid = GROUP * MAX_GROUPS;
+    FAR_CUDA(cudaMalloc((void**)&map->d_gicp_partials, (size_t)(map->gicp_max_grid + MAX_GROUPS) * TSTRIDE * sizeof(double)));
     FAR_CUDA(cudaMalloc((void**)&map->d_gicp_state, sizeof(GicpState)));
     FAR_CUDA(cudaMemset(map->d_gicp_state, 0, sizeof(GicpState)));
     return FAR_OK;

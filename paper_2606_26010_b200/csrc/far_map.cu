@@ -86,7 +86,15 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
     // ids at a position only ever decrease: if the last position already holds a smaller id, x cannot survive
     const uint32_t last = *reinterpret_cast<volatile uint32_t*>(idw + 4 * (cap - 1));
     if (last < x) return;
-    for (uint32_t pos = c0; pos < cap; ++pos) {
+    // The id words of a bucket are sorted at every instant and only ever decrease, so a position seen holding an
+    // id < x will never take x: gallop over such positions with plain reads (4 independent loads per step)
+    // instead of walking them with dependent atomics.  A stale read only makes the chain start earlier.
+    uint32_t pos = c0;
+    while (pos + 4 <= cap) {
+        const uint32_t a3 = *reinterpret_cast<volatile uint32_t*>(idw + 4 * (pos + 3));
+        if (a3 < x) pos += 4; else break;
+    }
+    for (; pos < cap; ++pos) {
         const uint32_t old = atomicMin(idw + 4 * pos, x);
         if (old == NO_ID) {
             if (pos == c0) touched[atomicAdd(&m.ctr->n_touched, 1u)] = s;   // unique per voxel and chunk
@@ -182,15 +190,23 @@ __global__ void __launch_bounds__(256) prune_kernel(MapView m, double cx, double
             }
         }
     }
-    // warp-aggregate the four statistics
+    // block-aggregate the four statistics: one atomic per counter and block (the four words are a hot spot)
+    __shared__ unsigned long long s_acc[8][4];
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) {
         vr += __shfl_xor_sync(FULL, vr, d); pr += __shfl_xor_sync(FULL, pr, d);
         vl += __shfl_xor_sync(FULL, vl, d); pl += __shfl_xor_sync(FULL, pl, d);
     }
     if ((threadIdx.x & 31) == 0) {
-        if (vr) { atomicAdd(&m.ctr->pr_vox_removed, vr); atomicAdd(&m.ctr->pr_pts_removed, pr); }
-        if (vl) { atomicAdd(&m.ctr->pr_vox_left, vl); atomicAdd(&m.ctr->pr_pts_left, pl); }
+        s_acc[threadIdx.x >> 5][0] = vr; s_acc[threadIdx.x >> 5][1] = pr;
+        s_acc[threadIdx.x >> 5][2] = vl; s_acc[threadIdx.x >> 5][3] = pl;
+    }
+    __syncthreads();
+    if (threadIdx.x < 4) {
+        unsigned long long t = 0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) t += s_acc[w][threadIdx.x];
+        if (t) atomicAdd(&m.ctr->pr_vox_removed + threadIdx.x, t);
     }
 }
 

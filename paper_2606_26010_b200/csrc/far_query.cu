@@ -84,8 +84,21 @@ __global__ void __launch_bounds__(QWARPS * 32) count27_kernel(MapView m, const f
 }
 
 // ---- A7: k nearest by (d2, id) -> Eq. 1 -----------------------------------------------------------------------
-// dynamic shared memory per warp: double d2[27*cap] | u32 id[27*cap] | int off[32] | u32 slot[32] | int sel[32]
-__host__ __device__ inline size_t knn_smem_per_warp(int cap) { return (size_t)27 * cap * 12 + 3 * 32 * 4; }
+// Selection without a sort of all candidates: every lane keeps the k smallest of ITS candidates as a sorted
+// column in shared memory (insertion while the candidates stream in; a candidate that cannot enter the lane's
+// top k costs one comparison).  The k nearest overall are then k rounds of a warp arg-min over the column heads;
+// the winning lane just advances its head.  Shared memory per warp: 32 lanes x k x 16 B, independent of cap.
+struct __align__(16) Cand {
+    double d2;
+    uint32_t id;
+    uint32_t ref;
+};
+
+__host__ __device__ inline size_t knn_smem_per_warp(int k) { return (size_t)32 * k * sizeof(Cand) + 2 * 32 * 4; }
+
+__device__ __forceinline__ bool cand_less(double d2, uint32_t id, const Cand& c) {
+    return d2 < c.d2 || (d2 == c.d2 && id < c.id);
+}
 
 // Eq. 1: C = Sigma_hat + eps I ; Sigma = (C^-1 / ||C^-1||_F)^-1 = ||C^-1||_F C.  FP64 throughout.
 __device__ __forceinline__ bool regularised_cov(const double sc[6], double eps, float out[6]) {
@@ -96,10 +109,9 @@ __device__ __forceinline__ bool regularised_cov(const double sc[6], double eps, 
     const double c02 = a1 * a5 - a4 * a2;
     const double det = a0 * c00 + a1 * c01 + a2 * c02;
     if (!(det != 0.0) || !isfinite(det)) return false;
-    const double id = 1.0 / det;
-    const double i00 = c00 * id, i01 = c01 * id, i02 = c02 * id;
-    const double i11 = (a0 * a8 - a2 * a2) * id, i12 = (a2 * a1 - a0 * a5) * id, i22 = (a0 * a4 - a1 * a1) * id;
-    const double fro = sqrt(i00 * i00 + i11 * i11 + i22 * i22 + 2.0 * (i01 * i01 + i02 * i02 + i12 * i12));
+    // ||C^-1||_F = ||adj(C)||_F / |det|
+    const double c11 = a0 * a8 - a2 * a2, c12 = a2 * a1 - a0 * a5, c22 = a0 * a4 - a1 * a1;
+    const double fro = sqrt(c00 * c00 + c11 * c11 + c22 * c22 + 2.0 * (c01 * c01 + c02 * c02 + c12 * c12)) / fabs(det);
     out[0] = (float)(fro * a0); out[1] = (float)(fro * a1); out[2] = (float)(fro * a2);
     out[3] = (float)(fro * a4); out[4] = (float)(fro * a5); out[5] = (float)(fro * a8);
     return true;
@@ -109,68 +121,76 @@ __device__ __forceinline__ bool regularised_cov(const double sc[6], double eps, 
 __device__ __forceinline__ bool warp_knn_cov(const MapView& m, float qx, float qy, float qz, int lane, char* smem_w,
                                              float cov[6]) {
     const int cap = m.cap, kk = m.k_cov;
-    double* s_d2 = reinterpret_cast<double*>(smem_w);
-    uint32_t* s_id = reinterpret_cast<uint32_t*>(smem_w + (size_t)27 * cap * 8);
-    int* s_off = reinterpret_cast<int*>(smem_w + (size_t)27 * cap * 12);
+    Cand* col = reinterpret_cast<Cand*>(smem_w);                 // col[r * 32 + lane] = r-th smallest of this lane
+    int* s_off = reinterpret_cast<int*>(smem_w + (size_t)32 * kk * sizeof(Cand));
     uint32_t* s_slot = reinterpret_cast<uint32_t*>(s_off + 32);
-    int* s_sel = reinterpret_cast<int*>(s_off + 64);
     cov[0] = 1.f; cov[1] = 0.f; cov[2] = 0.f; cov[3] = 1.f; cov[4] = 0.f; cov[5] = 1.f;
     int k[3];
     if (!voxel_index(qx, qy, qz, m.voxel, k)) return false;
     const int total = probe27(m, k, lane, s_off, s_slot);
     if (total < kk) { __syncwarp(); return false; }
     const double INF = __longlong_as_double(0x7FF0000000000000ll);
-    // stage (d2, id) of every candidate; lane owns candidates j = lane, lane+32, ... and tracks its local minimum
-    double bd = INF; uint32_t bid = NO_ID; int bj = -1;
-    int v = 0;
+    const double dqx = (double)qx, dqy = (double)qy, dqz = (double)qz;
+    int cnt = 0, v = 0;
     for (int j = lane; j < total; j += 32) {
         const uint32_t ref = cand_ref(s_off, s_slot, j, v, cap);
         const float4 p = __ldg(m.points + ref);
-        const double d2 = dist2(qx, qy, qz, p.x, p.y, p.z);
+        const double dx = dqx - (double)p.x, dy = dqy - (double)p.y, dz = dqz - (double)p.z;
+        const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));   // R6
         const uint32_t id = __float_as_uint(p.w);
-        s_d2[j] = d2;
-        s_id[j] = id;
-        if (d2 < bd || (d2 == bd && id < bid)) { bd = d2; bid = id; bj = j; }
-    }
-    __syncwarp();
-    // k rounds of warp arg-min; only the winning lane rescans its own candidates
-    for (int r = 0; r < kk; ++r) {
-        const int w = warp_argmin(bd, bid);
-        const int wj = __shfl_sync(FULL, bj, w);
-        if (lane == 0) s_sel[r] = wj;
-        if (lane == w) {
-            s_d2[bj] = INF;
-            s_id[bj] = NO_ID;
-            bd = INF; bid = NO_ID; bj = -1;
-            for (int j = lane; j < total; j += 32) {
-                const double d2 = s_d2[j];
-                const uint32_t id = s_id[j];
-                if (id != NO_ID && (d2 < bd || (d2 == bd && id < bid))) { bd = d2; bid = id; bj = j; }
-            }
+        int q = cnt;
+        if (cnt == kk) {
+            if (!cand_less(d2, id, col[(kk - 1) * 32 + lane])) continue;    // cannot enter this lane's top k
+            q = kk - 1;
+        } else {
+            ++cnt;
         }
-        __syncwarp();
+        while (q > 0) {
+            const Cand c = col[(q - 1) * 32 + lane];
+            if (!cand_less(d2, id, c)) break;
+            col[q * 32 + lane] = c;
+            --q;
+        }
+        Cand e;
+        e.d2 = d2; e.id = id; e.ref = ref;
+        col[q * 32 + lane] = e;
     }
-    // lanes r < k fetch the r-th neighbour again (L1/L2 hit); mean and centred sums in neighbour order (R7: 1/k)
-    double px = 0.0, py = 0.0, pz = 0.0;
+    // k rounds of warp arg-min over the column heads
+    int h = 0;
+    Cand head;
+    head.d2 = INF; head.id = NO_ID; head.ref = 0;
+    if (cnt > 0) head = col[lane];
+    uint32_t myref = 0;
+    for (int r = 0; r < kk; ++r) {
+        const int w = warp_argmin(head.d2, head.id);
+        const uint32_t wref = __shfl_sync(FULL, head.ref, w);
+        if (lane == r) myref = wref;
+        if (lane == w) {
+            ++h;
+            if (h < cnt) head = col[h * 32 + lane];
+            else { head.d2 = INF; head.id = NO_ID; }
+        }
+    }
+    // lane r < k holds the r-th neighbour; mean and centred sums in neighbour order (R7: 1/k)
+    float px = 0.f, py = 0.f, pz = 0.f;
     if (lane < kk) {
-        int vv = 0;
-        const uint32_t ref = cand_ref(s_off, s_slot, s_sel[lane], vv, cap);
-        const float4 p = __ldg(m.points + ref);
+        const float4 p = __ldg(m.points + myref);
         px = p.x; py = p.y; pz = p.z;
     }
+    const double inv_k = 1.0 / (double)kk;
     double mx = 0.0, my = 0.0, mz = 0.0;
     for (int r = 0; r < kk; ++r) {
-        mx += __shfl_sync(FULL, px, r); my += __shfl_sync(FULL, py, r); mz += __shfl_sync(FULL, pz, r);
+        mx += (double)__shfl_sync(FULL, px, r); my += (double)__shfl_sync(FULL, py, r); mz += (double)__shfl_sync(FULL, pz, r);
     }
-    mx /= (double)kk; my /= (double)kk; mz /= (double)kk;
-    const double dx = px - mx, dy = py - my, dz = pz - mz;
+    mx *= inv_k; my *= inv_k; mz *= inv_k;
     double sc[6] = {0, 0, 0, 0, 0, 0};
     for (int r = 0; r < kk; ++r) {
-        const double x = __shfl_sync(FULL, dx, r), y = __shfl_sync(FULL, dy, r), z = __shfl_sync(FULL, dz, r);
+        const double x = (double)__shfl_sync(FULL, px, r) - mx, y = (double)__shfl_sync(FULL, py, r) - my,
+                     z = (double)__shfl_sync(FULL, pz, r) - mz;
         sc[0] += x * x; sc[1] += x * y; sc[2] += x * z; sc[3] += y * y; sc[4] += y * z; sc[5] += z * z;
     }
 #pragma unroll
-    for (int a = 0; a < 6; ++a) sc[a] /= (double)kk;
+    for (int a = 0; a < 6; ++a) sc[a] *= inv_k;
     __syncwarp();
     float out[6];
     if (!regularised_cov(sc, m.cov_eps, out)) return false;
@@ -184,7 +204,7 @@ __global__ void knn_cov_points_kernel(MapView m, const float* __restrict__ q, in
                                       int stride, float* __restrict__ cov6, uint8_t* __restrict__ valid, int warps_per_block) {
     extern __shared__ __align__(16) char smem[];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    char* smem_w = smem + (size_t)wib * knn_smem_per_warp(m.cap);
+    char* smem_w = smem + (size_t)wib * knn_smem_per_warp(m.k_cov);
     if (d_n) n = min(n, *d_n);
     const int64_t nwarps = (int64_t)gridDim.x * warps_per_block;
     for (int64_t i = (int64_t)blockIdx.x * warps_per_block + wib; i < n; i += nwarps) {
@@ -201,7 +221,7 @@ __global__ void knn_cov_refs_kernel(MapView m, const uint32_t* __restrict__ refs
                                     int warps_per_block) {
     extern __shared__ __align__(16) char smem[];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    char* smem_w = smem + (size_t)wib * knn_smem_per_warp(m.cap);
+    char* smem_w = smem + (size_t)wib * knn_smem_per_warp(m.k_cov);
     const int64_t n = *d_n;
     const int64_t nwarps = (int64_t)gridDim.x * warps_per_block;
     for (int64_t i = (int64_t)blockIdx.x * warps_per_block + wib; i < n; i += nwarps) {
@@ -218,7 +238,7 @@ __global__ void knn_cov_refs_kernel(MapView m, const uint32_t* __restrict__ refs
 __global__ void knn_cov_new_ids_kernel(MapView m, uint32_t first_id, int warps_per_block) {
     extern __shared__ __align__(16) char smem[];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    char* smem_w = smem + (size_t)wib * knn_smem_per_warp(m.cap);
+    char* smem_w = smem + (size_t)wib * knn_smem_per_warp(m.k_cov);
     const int64_t nwarps = (int64_t)gridDim.x * warps_per_block;
     for (int64_t s = (int64_t)blockIdx.x * warps_per_block + wib; s < m.slots; s += nwarps) {
         const Entry e = m.table[s];
@@ -239,7 +259,7 @@ struct KnnLaunch { int warps, grid; size_t smem; };
 
 template <class K>
 static int knn_launch_cfg(const far_map* map, K kernel, int64_t work, KnnLaunch& L) {
-    const size_t per_warp = knn_smem_per_warp(map->view.cap);
+    const size_t per_warp = knn_smem_per_warp(map->view.k_cov);
     int warps = (int)(100 * 1024 / per_warp);
     if (warps > 8) warps = 8;
     if (warps < 1) warps = 1;
