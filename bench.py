@@ -35,13 +35,39 @@ PRUNE_RADIUS = 150.0
 MAX_ITERS = 30
 
 
-def workload_c2():
+def load_workload(name="c2"):
+    """c2 = BASELINE.json configs[1], the configuration the metric is quoted on (the bench line).
+    c1 = configs[0], the tiny case: only for the CPU rank-logic tests and quick checks, never a bench line."""
     import far_scenes as scenes
-    c2 = scenes.c2_single_frame(seed=1)
-    return c2
+    if name == "c1":
+        w = scenes.c1_tiny(seed=0)
+        w["max_voxels"] = 1 << 14
+    else:
+        w = scenes.c2_single_frame(seed=1)
+        w["max_voxels"] = 262144
+    w["name"] = name
+    return w
+
+
+def max_over_ranks(x, dist, device):
+    """max of a per-rank scalar over all ranks (identity without a process group)."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(world, steps, total_ms):
+    """whole-job throughput: replicas only, every rank runs `steps` frames; time = max over ranks."""
+    return world * steps / (total_ms * 1e-3)
 
 
 def workload_name(c2, n_ds=None, n_vox=None, n_stored=None):
+    if c2.get("name") == "c1":
+        return (f"C1 tiny planes (BASELINE.json configs[0], seed 0): {len(c2['map_points'])} map points, "
+                f"{len(c2['scan'])}-point scan, v=0.5 m cap 20 -- test-only workload, not the bench configuration")
     s = (f"C2 single-frame spinning-LiDAR registration (BASELINE.json configs[1], seed 1): 64x2048 rays -> "
          f"{len(c2['scan'])} returns, voxelised at 1.0 m")
     if n_ds is not None:
@@ -130,7 +156,7 @@ def run_reference(args):
         return
     import oracle
     cores = os.cpu_count() or 1
-    c2 = workload_c2()
+    c2 = load_workload(args.workload)
     mo = oracle.Map(c2["voxel"], c2["cap"])
     mo.insert(c2["map_points"], compute_cov=True)
     times = []
@@ -190,9 +216,9 @@ def run_far(args):
     far.lib()
     K, W = args.steps, args.warmup
 
-    c2 = workload_c2()
+    c2 = load_workload(args.workload)
     scan, v, cap, sigma = c2["scan"], c2["voxel"], c2["cap"], c2["sigma"]
-    fe = far.Frontend(v, cap, 262144, len(scan), ds_voxel=v, prune_radius=PRUNE_RADIUS, max_iters=MAX_ITERS)
+    fe = far.Frontend(v, cap, c2["max_voxels"], len(scan), ds_voxel=v, prune_radius=PRUNE_RADIUS, max_iters=MAX_ITERS)
     d_map_pts = torch.as_tensor(c2["map_points"]).cuda()
     build_stats = fe.map.insert(d_map_pts, compute_cov=True)
     map_stats = fe.map.stats()
@@ -231,11 +257,8 @@ def run_far(args):
     barrier()
     sampler.stop_flag = True
     sampler.join()
-    if dist is not None:
-        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
-    value = world * K / (total_ms * 1e-3)
+    total_ms = max_over_ranks(total_ms, dist, "cuda")
+    value = aggregate_value(world, K, total_ms)
     res = far.result_to_dict(far.GicpResult.from_buffer_copy(d_res[K - 1].cpu().numpy().tobytes()))
     post_stats = fe.map.stats()
     dt_gt = float(np.linalg.norm(res["t"] - c2["T_gt"][1]))
@@ -254,11 +277,8 @@ def run_far(args):
         r_e2e = fe.process_host(h_scan, T_init, sigma)
         e2e_t.append(time.perf_counter() - t0)
     e2e_total = float(np.sum(e2e_t))
-    if dist is not None:
-        t = torch.tensor([e2e_total], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_total = float(t.item())
-    e2e_value = world * Ke / e2e_total
+    e2e_total = max_over_ranks(e2e_total, dist, "cuda")
+    e2e_value = aggregate_value(world, Ke, e2e_total * 1e3)
     assert r_e2e["iters"] == res["iters"] and r_e2e["n_inliers"] == res["n_inliers"]
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
@@ -399,6 +419,7 @@ def main():
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="far", choices=["far", "reference"])
+    ap.add_argument("--workload", default="c2", choices=["c2", "c1"], help="c1 is for tests only")
     ap.add_argument("--no-extras", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
