@@ -213,6 +213,41 @@ class UrbanScene:
         pts = d_s[keep] * rng_t[keep, None]
         return pts.astype(F32)
 
+    def _under_a_box(self, q, cell=32.0):
+        """q (n,>=2): True where (x, y) lies strictly inside a box footprint.  Exact test
+        |x - cx| < sx/2 and |y - cy| < sy/2 against every box, evaluated per 32 m grid cell
+        against only the boxes that overlap the cell (same predicate, fewer pairs)."""
+        bx = self.boxes
+        half = self.extent / 2.0
+        nc = int(math.ceil(self.extent / cell))
+        ix = np.clip(np.floor((q[:, 0] + half) / cell).astype(np.int64), 0, nc - 1)
+        iy = np.clip(np.floor((q[:, 1] + half) / cell).astype(np.int64), 0, nc - 1)
+        cid = ix * nc + iy
+        order = np.argsort(cid, kind="stable")
+        cs = cid[order]
+        starts = np.nonzero(np.r_[True, cs[1:] != cs[:-1]])[0]
+        ends = np.r_[starts[1:], cs.size]
+        blo = np.stack([bx[:, 0] - bx[:, 2] / 2, bx[:, 1] - bx[:, 3] / 2], axis=1)
+        bhi = np.stack([bx[:, 0] + bx[:, 2] / 2, bx[:, 1] + bx[:, 3] / 2], axis=1)
+        inside = np.zeros(q.shape[0], dtype=bool)
+        for s, e in zip(starts, ends):
+            c = int(cs[s])
+            cx0 = (c // nc) * cell - half
+            cy0 = (c % nc) * cell - half
+            # boxes whose footprint can contain a point of this cell (clipped points sit in edge cells: pad them)
+            pad = cell if (c // nc in (0, nc - 1) or c % nc in (0, nc - 1)) else 0.0
+            sel = (bhi[:, 0] >= cx0 - pad) & (blo[:, 0] <= cx0 + cell + pad) & \
+                  (bhi[:, 1] >= cy0 - pad) & (blo[:, 1] <= cy0 + cell + pad)
+            if not sel.any():
+                continue
+            b = bx[sel]
+            idx = order[s:e]
+            pts = q[idx]
+            ins = (np.abs(pts[:, None, 0] - b[None, :, 0]) < b[None, :, 2] / 2) & \
+                  (np.abs(pts[:, None, 1] - b[None, :, 1]) < b[None, :, 3] / 2)
+            inside[idx] = ins.any(axis=1)
+        return inside
+
     # ---- area-uniform surface samples ------------------------------------
     def sample_surfaces(self, n, rng, center=(0.0, 0.0), radius=None, noise=0.0):
         """n area-uniform samples of the scene surfaces (ground, box walls and roofs, poles).
@@ -275,13 +310,7 @@ class UrbanScene:
             # ground samples under a building are not visible surfaces: drop them
             gi = np.nonzero(g & keep)[0]
             if gi.size:
-                inside = np.zeros(gi.size, dtype=bool)
-                for s in range(0, gi.size, 65536):
-                    q = p[gi[s:s + 65536]]
-                    ins = (np.abs(q[:, None, 0] - bx[None, :, 0]) < bx[None, :, 2] / 2) & \
-                          (np.abs(q[:, None, 1] - bx[None, :, 1]) < bx[None, :, 3] / 2)
-                    inside[s:s + 65536] = ins.any(axis=1)
-                keep[gi[inside]] = False
+                keep[gi[self._under_a_box(p[gi])]] = False
             out = np.concatenate([out, p[keep]], axis=0)
         out = out[:n]
         if noise > 0:

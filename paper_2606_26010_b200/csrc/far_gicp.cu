@@ -39,6 +39,19 @@ struct GicpState {
     unsigned int group_ticket[MAX_GROUPS];  // blocks of a group that wrote their partial row
 };
 
+#ifdef FAR_GICP_TRACE
+// Debug-only timing probes (never compiled into the product library): globaltimer stamps per iteration.
+__device__ unsigned long long g_trace[64][8];
+__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#define TRACE_MIN(it, slot) do { if (threadIdx.x == 0 && (it) < 64) atomicMin(&g_trace[it][slot], gtime()); } while (0)
+#define TRACE_MAX(it, slot) do { if (threadIdx.x == 0 && (it) < 64) atomicMax(&g_trace[it][slot], gtime()); } while (0)
+#define TRACE_ADD(it, slot) do { if (threadIdx.x == 0 && (it) < 64) atomicAdd(&g_trace[it][slot], gtime()); } while (0)
+#else
+#define TRACE_MIN(it, slot)
+#define TRACE_MAX(it, slot)
+#define TRACE_ADD(it, slot)
+#endif
+
 struct GicpParams {
     const float* scan;
     const float* cov6;          // nullable
@@ -322,6 +335,7 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(M
 
     for (int it = 0; it < P.max_iters; ++it) {
         // ---- A8 + A9: one warp per source point; lane t < 29 accumulates term t ---------------------------------
+        TRACE_MIN(it, 0);
         double acc = 0.0;
         for (int64_t i = (int64_t)blockIdx.x * GWARPS + wib; i < n; i += nwarps) {
             const float* sp = P.scan + i * P.stride;
@@ -377,6 +391,8 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(M
         // ---- A10: warp -> block -> group of 32 blocks -> grid, every level in a fixed order ----------------------
         s_red[wib][lane] = lane < NTERMS ? acc : 0.0;
         __syncthreads();
+        TRACE_MAX(it, 1);
+        TRACE_ADD(it, 2);
         if (wib == 0) {
             double s = 0.0;
 #pragma unroll
@@ -405,12 +421,14 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(M
                 const double t2 = block_sum_rows(P.partials2, 0, n_groups, lane, wib, s_red);
                 if (wib == 0) s_terms[0][lane] = t2;
                 __syncthreads();
+                TRACE_MAX(it, 3);
                 if (threadIdx.x == 0) {
                     solve_and_update(P, s_terms[0], s_T, it);
                     P.state->ticket = 0u;
                     __threadfence();
                     atomicExch(&P.state->epoch, (unsigned)(it + 1));
                 }
+                TRACE_MAX(it, 4);
             }
         }
         // ---- grid-wide wait for the new pose: all blocks are co-resident (cooperative launch) -------------------
@@ -419,6 +437,7 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(M
             __threadfence();
         }
         __syncthreads();
+        TRACE_MAX(it, 5);
         if (__ldcg(&P.state->done)) break;
         if (threadIdx.x < 12) {
             const double vv = __ldcg(threadIdx.x < 9 ? &P.state->pose.R[threadIdx.x] : &P.state->pose.t[threadIdx.x - 9]);
@@ -498,6 +517,16 @@ int far_gicp_register_dev(const far_map_t* map, const float* d_scan, const float
     return gicp_launch(map, d_scan, d_cov6, d_valid, n_max, d_n, stride, nullptr, d_init_pose, sigma, max_iters, 0, opts, d_out,
                        stream);
 }
+
+#ifdef FAR_GICP_TRACE
+// debug build only: reset (all slots 0, min-slot ~0) / read the probes
+void far_gicp_trace_reset(void) {
+    unsigned long long h[64][8];
+    for (int i = 0; i < 64; ++i) for (int j = 0; j < 8; ++j) h[i][j] = (j == 0) ? ~0ull : 0ull;
+    cudaMemcpyToSymbol(far::g_trace, h, sizeof(h));
+}
+void far_gicp_trace_read(unsigned long long* out) { cudaMemcpyFromSymbol(out, far::g_trace, sizeof(unsigned long long) * 64 * 8); }
+#endif
 
 }  // extern "C"
 
