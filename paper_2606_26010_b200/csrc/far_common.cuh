@@ -178,14 +178,17 @@ __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
 }
 
 // The 27-voxel probe of one query by one warp (Fig. 3): lane l < 27 looks up neighbour
-// (l/9-1, (l/3)%3-1, l%3-1); s_off[0..27] receives the exclusive prefix of the counts, s_slot[0..26] the slots.
-// Returns the total number of candidate points.  All 32 lanes must call.
-__device__ __forceinline__ int probe27(const MapView& m, const int k[3], int lane, int* s_off, uint32_t* s_slot) {
-    uint32_t cnt = 0, slot = NO_SLOT;
+// (l/9-1, (l/3)%3-1, l%3-1) and keeps its slot and count in registers.  All 32 lanes must call.
+__device__ __forceinline__ void probe27_regs(const MapView& m, const int k[3], int lane, uint32_t& cnt, uint32_t& slot) {
+    cnt = 0; slot = NO_SLOT;
     if (lane < 27) {
         const int nx = k[0] + lane / 9 - 1, ny = k[1] + (lane / 3) % 3 - 1, nz = k[2] + lane % 3 - 1;
         if (index_in_range(nx) && index_in_range(ny) && index_in_range(nz)) slot = find_voxel(m, pack_key(nx, ny, nz), cnt);
     }
+}
+
+// publishes per-lane counts as an exclusive prefix: s_off[0..27], s_slot[0..26]; returns the total
+__device__ __forceinline__ int publish_prefix(uint32_t cnt, uint32_t slot, int lane, int* s_off, uint32_t* s_slot) {
     const int incl = warp_incl_scan((int)cnt, lane);
     if (lane < 27) {
         s_off[lane + 1] = incl;
@@ -194,6 +197,94 @@ __device__ __forceinline__ int probe27(const MapView& m, const int k[3], int lan
     if (lane == 0) s_off[0] = 0;
     __syncwarp();
     return __shfl_sync(FULL, incl, 31);
+}
+
+__device__ __forceinline__ int probe27(const MapView& m, const int k[3], int lane, int* s_off, uint32_t* s_slot) {
+    uint32_t cnt, slot;
+    probe27_regs(m, k, lane, cnt, slot);
+    return publish_prefix(cnt, slot, lane, s_off, s_slot);
+}
+
+// map flat candidate j -> (voxel v, position) with a monotone walk over the prefix array
+__device__ __forceinline__ uint32_t cand_ref(const int* s_off, const uint32_t* s_slot, int j, int& v, int cap) {
+    while (j >= s_off[v + 1]) ++v;
+    return s_slot[v] * (uint32_t)cap + (uint32_t)(j - s_off[v]);
+}
+
+// warp-wide minimum of a non-negative double (its bit pattern orders like its value): two redux.sync steps
+__device__ __forceinline__ double warp_min_nonneg(double d2) {
+    const unsigned long long bits = (unsigned long long)__double_as_longlong(d2);
+    const uint32_t hi = (uint32_t)(bits >> 32), lo = (uint32_t)bits;
+    const uint32_t mhi = __reduce_min_sync(FULL, hi);
+    const uint32_t mlo = __reduce_min_sync(FULL, hi == mhi ? lo : 0xFFFFFFFFu);
+    return __longlong_as_double((long long)(((unsigned long long)mhi << 32) | mlo));
+}
+
+// Lower bound of the squared distance from q (inside voxel k) to ANY point stored in neighbour voxel
+// k + (ox, oy, oz).  A point of voxel index K along one axis satisfies K v - e <= p < (K + 1) v + e with
+// e < (|K| + 1) v 2^-24 (the key is the floor of ONE rounded fp32 quotient, R1), so the faces are pulled in by a
+// margin of (|k| + 2) v 2^-20, which also covers the rounding of the bound itself.  k v is exact in binary64.
+__device__ __forceinline__ double voxel_lower_bound(float qx, float qy, float qz, const int k[3], float v, int ox, int oy, int oz) {
+    const double dv = (double)v;
+    const double q[3] = {(double)qx, (double)qy, (double)qz};
+    const int o[3] = {ox, oy, oz};
+    double lb = 0.0;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double margin = (double)(abs(k[a]) + 2) * dv * 9.5367431640625e-07;   // 2^-20
+        double gap = 0.0;
+        if (o[a] < 0) gap = q[a] - (double)k[a] * dv - margin;
+        else if (o[a] > 0) gap = (double)(k[a] + 1) * dv - q[a] - margin;
+        gap = fmax(gap, 0.0);
+        lb += gap * gap;
+    }
+    return lb;
+}
+
+// A6 by one warp, all 32 lanes must call; every lane returns the winner (best.id == NO_ID if none) and its
+// coordinates.  Exactly the 27-voxel (d2, id)-minimum of R6, reached with fewer reads: the query's own voxel is
+// swept first, then a neighbour voxel is read only if its lower bound does not exceed the best d2 so far
+// (a skipped voxel holds only points strictly farther than the current best, so it cannot change the result,
+// ties included).  The surviving voxels are swept as ONE flattened candidate list, 32 float4 per step.
+__device__ __forceinline__ Best warp_nearest(const MapView& m, float qx, float qy, float qz, const int k[3], int lane,
+                                             int* s_off, uint32_t* s_slot, float& rx, float& ry, float& rz) {
+    uint32_t cnt, slot;
+    probe27_regs(m, k, lane, cnt, slot);
+    Best best;
+    best.d2 = __longlong_as_double(0x7FF0000000000000ll);
+    best.id = NO_ID;
+    best.ref = 0;
+    float bx = 0.f, by = 0.f, bz = 0.f;
+    const uint32_t c_cnt = __shfl_sync(FULL, cnt, 13), c_slot = __shfl_sync(FULL, slot, 13);
+    for (uint32_t j = lane; j < c_cnt; j += 32) {
+        const uint32_t ref = c_slot * (uint32_t)m.cap + j;
+        const float4 p = __ldg(m.points + ref);
+        const double d2 = dist2(qx, qy, qz, p.x, p.y, p.z);
+        const uint32_t id = __float_as_uint(p.w);
+        if (better(d2, id, best)) { best.d2 = d2; best.id = id; best.ref = ref; bx = p.x; by = p.y; bz = p.z; }
+    }
+    const double bound = warp_min_nonneg(best.d2);
+    uint32_t c2 = 0;
+    if (lane < 27 && lane != 13 && cnt > 0) {
+        const double lb = voxel_lower_bound(qx, qy, qz, k, m.voxel, lane / 9 - 1, (lane / 3) % 3 - 1, lane % 3 - 1);
+        if (lb <= bound) c2 = cnt;
+    }
+    const int total = publish_prefix(c2, slot, lane, s_off, s_slot);
+    int v = 0;
+    for (int j = lane; j < total; j += 32) {
+        const uint32_t ref = cand_ref(s_off, s_slot, j, v, m.cap);
+        const float4 p = __ldg(m.points + ref);
+        const double d2 = dist2(qx, qy, qz, p.x, p.y, p.z);
+        const uint32_t id = __float_as_uint(p.w);
+        if (better(d2, id, best)) { best.d2 = d2; best.id = id; best.ref = ref; bx = p.x; by = p.y; bz = p.z; }
+    }
+    __syncwarp();
+    const int w = warp_argmin(best.d2, best.id);
+    best.d2 = __shfl_sync(FULL, best.d2, w);
+    best.id = __shfl_sync(FULL, best.id, w);
+    best.ref = __shfl_sync(FULL, best.ref, w);
+    rx = __shfl_sync(FULL, bx, w); ry = __shfl_sync(FULL, by, w); rz = __shfl_sync(FULL, bz, w);
+    return best;
 }
 
 }  // namespace far

@@ -9,12 +9,21 @@
 // accumulated in FP64 and always applied to the ORIGINAL scan; stop on ||delta||_2; max_iters replaces the
 // wall-clock limit.
 //
-// B200 design: a registration is a few thousand source points, i.e. latency- not bandwidth-bound, so the whole
-// Gauss-Newton loop is ONE persistent cooperative kernel: one warp per source point (27-voxel probe + flattened
-// candidate sweep, see far_query.cu), the 29 unique terms of (H, b, chi2, n) reduced lane -> warp -> block ->
-// last-arriving block in a fixed order (deterministic, no floating atomics), the 6x6 Cholesky solve, SE(3)
-// exponential and pose update done by one thread of that last block in FP64, and one grid-wide barrier per
-// iteration.  The host is not involved until it reads the result.
+// B200 design: a registration is a few thousand source points, i.e. latency- and issue-bound, never bandwidth-
+// bound, so the whole Gauss-Newton loop is ONE persistent cooperative kernel and every iteration is organised to
+// keep both the instruction count and the serial chain short:
+//   phase A  one warp per source point: FP64 transform, 27-voxel probe, bounded candidate sweep
+//            (far_common.cuh::warp_nearest), gate, fetch of Sigma_r -> one correspondence record in shared memory;
+//   phase B  the block's 8 correspondences are linearised by 8 lanes of warp 0 at once (the ~300 FP64 operations of
+//            M, weight, J^T M J are one instruction stream for 8 points instead of 8 streams with one active lane);
+//   reduce   the 29 unique terms of (H, b, chi2, n) go block -> group of 32 blocks -> grid as TAGGED rows: every
+//            value travels as {lo, tag, hi, tag} (two self-validating 8-byte words, tag = launch sequence and
+//            iteration), so a consumer just polls the rows it needs -- no fence, no ticket atomics -- and sums
+//            them in a fixed order (deterministic, no floating-point atomics);
+//   solve    block 0 / thread 0: 6x6 Cholesky, SE(3) exponential, pose update and stop test in FP64, published as
+//            13 tagged words that every block polls: one L2 round trip from "solved" to "next iteration".
+// The host is not involved until it reads the result.
+#include <atomic>
 #include <cstring>
 
 #include "far_internal.h"
@@ -23,20 +32,30 @@ using namespace far;
 
 namespace far {
 
-constexpr int GWARPS = 8;        // warps per block
+constexpr int GWARPS = 8;        // warps per block = correspondences linearised together in phase B
 constexpr int NTERMS = 29;       // 21 (H upper triangle) + 6 (b) + chi2 + inlier count
-constexpr int TSTRIDE = 32;      // padded row of per-block partials
+constexpr int TSTRIDE = 32;      // padded row
 
 constexpr int GROUP = 32;        // blocks per first-level reduction group
 constexpr int MAX_GROUPS = 64;
 constexpr int GICP_BLOCKS_PER_SM = 5;
+constexpr int NPUB = 13;         // published words: R[9], t[3], done
+constexpr int MAX_ITERS_LIMIT = 1000;   // the iteration index shares the 32-bit tag with the launch sequence
 
-struct GicpState {
-    Pose pose;
-    int done;
-    unsigned int ticket;                    // groups that finished their first-level sum
-    unsigned int epoch;                     // iterations completed (published after the pose)
-    unsigned int group_ticket[MAX_GROUPS];  // blocks of a group that wrote their partial row
+// device scratch of one map: [max_grid] block rows, [MAX_GROUPS] group rows, the published pose
+struct GicpScratch {
+    uint4* rows;      // [max_grid][TSTRIDE]
+    uint4* grows;     // [MAX_GROUPS][TSTRIDE]
+    uint4* pub;       // [16]
+};
+
+// one correspondence, written by its warp in phase A, read by one lane of warp 0 in phase B
+struct Corr {
+    float p[3];       // transformed source point
+    float r[3];       // its nearest map point
+    float cs[6];      // Sigma_s
+    float cr[6];      // Sigma_r
+    int flags;        // bit 0: correspondence accepted, bit 1: both covariances valid
 };
 
 #ifdef FAR_GICP_TRACE
@@ -45,7 +64,7 @@ __device__ unsigned long long g_trace[64][8];
 __device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
 #define TRACE_MIN(it, slot) do { if (threadIdx.x == 0 && (it) < 64) atomicMin(&g_trace[it][slot], gtime()); } while (0)
 #define TRACE_MAX(it, slot) do { if (threadIdx.x == 0 && (it) < 64) atomicMax(&g_trace[it][slot], gtime()); } while (0)
-#define TRACE_ADD(it, slot) do { if (threadIdx.x == 0 && (it) < 64) atomicAdd(&g_trace[it][slot], gtime()); } while (0)
+#define TRACE_ADD(it, slot) do { if (threadIdx.x == 0 && (it) < 64) atomicAdd(&g_trace[it][slot], gtime() & 0xFFFFFFFFull); } while (0)
 #else
 #define TRACE_MIN(it, slot)
 #define TRACE_MAX(it, slot)
@@ -63,16 +82,29 @@ struct GicpParams {
     const Pose* d_init;
     double tau2, kappa, conv_eps;
     int kernel, max_iters, linearize_only;
-    double* partials;           // [gridDim.x][TSTRIDE]
-    double* partials2;          // [groups][TSTRIDE]
-    GicpState* state;
+    uint32_t seq;               // launch sequence number (upper bits of every tag)
+    GicpScratch scratch;
     far_gicp_result_t* out;
 };
 
-// nearest-neighbour core shared in spirit with far_query.cu (kept local so the kernel inlines it)
-__device__ __forceinline__ uint32_t g_cand_ref(const int* s_off, const uint32_t* s_slot, int j, int& v, int cap) {
-    while (j >= s_off[v + 1]) ++v;
-    return s_slot[v] * (uint32_t)cap + (uint32_t)(j - s_off[v]);
+__device__ __forceinline__ void put_tagged(uint4* dst, double v, uint32_t tag) {
+    const unsigned long long b = (unsigned long long)__double_as_longlong(v);
+    asm volatile("st.relaxed.gpu.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "r"((uint32_t)b), "r"(tag),
+                 "r"((uint32_t)(b >> 32)), "r"(tag)
+                 : "memory");
+}
+
+__device__ __forceinline__ uint4 load_tagged(const uint4* src) {
+    uint4 w;
+    asm volatile("ld.relaxed.gpu.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w) : "l"(src) : "memory");
+    return w;
+}
+
+// spins until both halves carry `tag` (volatile asm: the compiler must neither hoist the load nor assume the loop ends)
+__device__ __forceinline__ double wait_tagged(const uint4* src, uint32_t tag) {
+    uint4 w = load_tagged(src);
+    while (w.y != tag || w.w != tag) w = load_tagged(src);
+    return __longlong_as_double((long long)(((unsigned long long)w.z << 32) | w.x));
 }
 
 __device__ __forceinline__ double robust_weight(int kernel, double e2, double kappa) {
@@ -227,9 +259,9 @@ __device__ __forceinline__ void se3_exp(const double* d, Pose& E) {
     for (int r = 0; r < 3; ++r) E.t[r] = V[3 * r] * d[0] + V[3 * r + 1] * d[1] + V[3 * r + 2] * d[2];
 }
 
-// Serial section of one iteration (one thread of the last-arriving block): assemble H, b from the 29 reduced
-// terms, solve, update the pose, decide termination, publish.
-__device__ __noinline__ void solve_and_update(const GicpParams& P, const double* tv, const Pose& T, int it) {
+// Serial section of one iteration (thread 0 of block 0): assemble H, b from the 29 reduced terms, solve, update
+// the pose, decide termination, write the result when done.  Returns the new pose and the done flag.
+__device__ __forceinline__ bool solve_and_update(const GicpParams& P, const double* tv, const Pose& T, int it, Pose& Tn) {
     double H[36], b[6];
     {
         int q = 0;
@@ -243,7 +275,7 @@ __device__ __noinline__ void solve_and_update(const GicpParams& P, const double*
     const int n_inl = (int)(tv[28] + 0.5);
     bool done = false;
     int converged = 0, status = FAR_OK;
-    Pose Tn = T;
+    Tn = T;
     if (!P.linearize_only) {
         double rhs[6], delta[6];
 #pragma unroll
@@ -272,7 +304,6 @@ __device__ __noinline__ void solve_and_update(const GicpParams& P, const double*
         done = true;
     }
     if (it + 1 >= P.max_iters) done = true;
-    P.state->pose = Tn;
     if (done) {
         far_gicp_result_t* out = P.out;
         for (int a = 0; a < 9; ++a) out->pose.R[a] = Tn.R[a];
@@ -285,21 +316,15 @@ __device__ __noinline__ void solve_and_update(const GicpParams& P, const double*
         out->converged = converged;
         out->status = status;
     }
-    P.state->done = done ? 1 : 0;
+    return done;
 }
 
-// sum rows [first, first + count) of a [rows][TSTRIDE] array of doubles, column = lane; 8 warps x 32 lanes.
-// Every load is independent (one memory latency for up to 32 rows); the additions happen in a fixed order.
-__device__ __forceinline__ double block_sum_rows(const double* rows, int first, int count, int lane, int wib,
-                                                 double (*s_red)[TSTRIDE]) {
-    double v[4];
-#pragma unroll
-    for (int u = 0; u < 4; ++u) {
-        const int r = wib + GWARPS * u;
-        v[u] = r < count ? __ldcg(rows + (size_t)(first + r) * TSTRIDE + lane) : 0.0;
-    }
-    double s = (v[0] + v[1]) + (v[2] + v[3]);
-    for (int r = wib + 4 * GWARPS; r < count; r += GWARPS) s += __ldcg(rows + (size_t)(first + r) * TSTRIDE + lane);
+// Polls `count` tagged rows starting at `first` (column = lane) and sums them: warp w takes rows w, w + 8, ... in
+// increasing order, then the 8 warp sums are added in warp order by warp 0.  Every block must call with all threads.
+__device__ __forceinline__ double block_sum_tagged(const uint4* rows, int first, int count, uint32_t tag, int lane, int wib,
+                                                   double (*s_red)[TSTRIDE]) {
+    double s = 0.0;
+    for (int r = wib; r < count; r += GWARPS) s += wait_tagged(rows + (size_t)(first + r) * TSTRIDE + lane, tag);
     s_red[wib][lane] = s;
     __syncthreads();
     double t = 0.0;
@@ -316,8 +341,9 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(M
     __shared__ uint32_t s_slot[GWARPS][32];
     __shared__ double s_terms[GWARPS][TSTRIDE];
     __shared__ double s_red[GWARPS][TSTRIDE];
+    __shared__ Corr s_corr[GWARPS];
     __shared__ Pose s_T;
-    __shared__ int s_flag;
+    __shared__ int s_done;
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const int64_t nwarps = (int64_t)gridDim.x * GWARPS;
     int64_t n = P.n;
@@ -332,118 +358,107 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(M
     const int group = blockIdx.x / GROUP;
     const int group_rows = min(GROUP, (int)gridDim.x - group * GROUP);
     const bool have_scan_cov = P.cov6 != nullptr && P.valid != nullptr && m.cov != nullptr;
+    const int rounds = (int)((n + nwarps - 1) / nwarps);      // source points per warp (1 when n <= resident warps)
 
     for (int it = 0; it < P.max_iters; ++it) {
-        // ---- A8 + A9: one warp per source point; lane t < 29 accumulates term t ---------------------------------
+        const uint32_t tag = (P.seq << 10) | (uint32_t)(it + 1);
         TRACE_MIN(it, 0);
-        double acc = 0.0;
-        for (int64_t i = (int64_t)blockIdx.x * GWARPS + wib; i < n; i += nwarps) {
-            const float* sp = P.scan + i * P.stride;
-            const float sx = __ldg(sp), sy = __ldg(sp + 1), sz = __ldg(sp + 2);
-            if (!(isfinite(sx) && isfinite(sy) && isfinite(sz))) continue;
-            // the source covariance does not depend on the search: lanes 8..13 fetch it now, lane 14 its flag
-            float cin = 0.f;
-            if (have_scan_cov) {
-                if (lane >= 8 && lane < 14) cin = __ldg(P.cov6 + 6 * i + (lane - 8));
-                if (lane == 14) cin = (float)__ldg(P.valid + i);
+        double acc = 0.0;                                     // warp 0, lane t < 29: term t of this block
+        for (int rd = 0; rd < rounds; ++rd) {
+            // ---- phase A (A8): one warp per source point -> correspondence record ---------------------------------
+            const int64_t i = (int64_t)rd * nwarps + (int64_t)blockIdx.x * GWARPS + wib;
+            int flags = 0;
+            if (i < n) {
+                const float* sp = P.scan + i * P.stride;
+                const float sx = __ldg(sp), sy = __ldg(sp + 1), sz = __ldg(sp + 2);
+                float pf[3];
+                int k[3];
+                if (isfinite(sx) && isfinite(sy) && isfinite(sz)) {
+                    // the source covariance does not depend on the search: lanes 8..13 fetch it now, lane 14 its flag
+                    float cin = 0.f;
+                    if (have_scan_cov) {
+                        if (lane >= 8 && lane < 14) cin = __ldg(P.cov6 + 6 * i + (lane - 8));
+                        if (lane == 14) cin = (float)__ldg(P.valid + i);
+                    }
+                    transform_point(s_T, sx, sy, sz, pf);             // Eq. 2 with the accumulated pose (R11)
+                    if (voxel_index(pf[0], pf[1], pf[2], m.voxel, k)) {
+                        // kNN-search, k = 1
+                        float rx, ry, rz;
+                        const Best best = warp_nearest(m, pf[0], pf[1], pf[2], k, lane, s_off[wib], s_slot[wib], rx, ry, rz);
+                        if (best.id != NO_ID && !(best.d2 > P.tau2)) {    // adaptive-threshold gate
+                            // lanes 0..5 fetch Sigma_r, lane 6 its flag: one memory level
+                            if (have_scan_cov) {
+                                if (lane < 6) cin = __ldg(m.cov + (size_t)best.ref * 6 + lane);
+                                if (lane == 6) cin = (float)__ldg(m.cov_ok + best.ref);
+                            }
+                            const bool full = have_scan_cov && __shfl_sync(FULL, cin, 6) != 0.f && __shfl_sync(FULL, cin, 14) != 0.f;
+                            Corr& c = s_corr[wib];
+                            if (lane < 6) c.cr[lane] = cin;
+                            if (lane >= 8 && lane < 14) c.cs[lane - 8] = cin;
+                            if (lane == 16) { c.p[0] = pf[0]; c.p[1] = pf[1]; c.p[2] = pf[2]; c.r[0] = rx; c.r[1] = ry; c.r[2] = rz; }
+                            flags = full ? 3 : 1;
+                        }
+                    }
+                }
             }
-            float pf[3];
-            transform_point(s_T, sx, sy, sz, pf);                 // Eq. 2 with the accumulated pose (R11)
-            int k[3];
-            if (!voxel_index(pf[0], pf[1], pf[2], m.voxel, k)) continue;
-            // kNN-search, k = 1
-            const int total = probe27(m, k, lane, s_off[wib], s_slot[wib]);
-            Best best;
-            best.d2 = __longlong_as_double(0x7FF0000000000000ll);
-            best.id = NO_ID;
-            best.ref = 0;
-            float bx = 0.f, by = 0.f, bz = 0.f;
-            int v = 0;
-            for (int j = lane; j < total; j += 32) {
-                const uint32_t ref = g_cand_ref(s_off[wib], s_slot[wib], j, v, m.cap);
-                const float4 q = __ldg(m.points + ref);
-                const double d2 = dist2(pf[0], pf[1], pf[2], q.x, q.y, q.z);
-                const uint32_t id = __float_as_uint(q.w);
-                if (better(d2, id, best)) { best.d2 = d2; best.id = id; best.ref = ref; bx = q.x; by = q.y; bz = q.z; }
-            }
-            __syncwarp();
-            const int w = warp_argmin(best.d2, best.id);
-            const double bd2 = __shfl_sync(FULL, best.d2, w);
-            const uint32_t bid = __shfl_sync(FULL, best.id, w);
-            const uint32_t bref = __shfl_sync(FULL, best.ref, w);
-            if (bid == NO_ID || bd2 > P.tau2) continue;           // adaptive-threshold gate
-            // the winning lane already holds r; lanes 0..5 fetch Sigma_r, lane 6 its flag: one memory level
-            const double r[3] = {(double)__shfl_sync(FULL, bx, w), (double)__shfl_sync(FULL, by, w), (double)__shfl_sync(FULL, bz, w)};
-            if (have_scan_cov) {
-                if (lane < 6) cin = __ldg(m.cov + (size_t)bref * 6 + lane);
-                if (lane == 6) cin = (float)__ldg(m.cov_ok + bref);
-            }
-            float cr[6], cs[6];
-#pragma unroll
-            for (int a = 0; a < 6; ++a) { cr[a] = __shfl_sync(FULL, cin, a); cs[a] = __shfl_sync(FULL, cin, 8 + a); }
-            const bool full = have_scan_cov && __shfl_sync(FULL, cin, 6) != 0.f && __shfl_sync(FULL, cin, 14) != 0.f;
-            const double p[3] = {(double)pf[0], (double)pf[1], (double)pf[2]};
-            if (lane == 0) correspondence_terms(s_T, p, r, full, cs, cr, P.kernel, P.kappa, s_terms[wib]);
-            __syncwarp();
-            if (lane < NTERMS) acc += s_terms[wib][lane];
-            __syncwarp();
-        }
-        // ---- A10: warp -> block -> group of 32 blocks -> grid, every level in a fixed order ----------------------
-        s_red[wib][lane] = lane < NTERMS ? acc : 0.0;
-        __syncthreads();
-        TRACE_MAX(it, 1);
-        TRACE_ADD(it, 2);
-        if (wib == 0) {
-            double s = 0.0;
-#pragma unroll
-            for (int w8 = 0; w8 < GWARPS; ++w8) s += s_red[w8][lane];
-            P.partials[(size_t)blockIdx.x * TSTRIDE + lane] = s;
-            __threadfence();
-        }
-        __syncthreads();
-        if (threadIdx.x == 0) s_flag = (atomicAdd(&P.state->group_ticket[group], 1u) == (unsigned)group_rows - 1) ? 1 : 0;
-        __syncthreads();
-        if (s_flag) {   // last block of its group: fold the group's rows into one
-            __threadfence();
-            const double t = block_sum_rows(P.partials, group * GROUP, group_rows, lane, wib, s_red);
+            if (lane == 0) s_corr[wib].flags = flags;
+            __syncthreads();
+            // ---- phase B (A9): 8 lanes of warp 0 linearise the block's 8 correspondences together --------------------
             if (wib == 0) {
-                P.partials2[(size_t)group * TSTRIDE + lane] = t;
-                __threadfence();
+                if (lane < GWARPS) {
+                    const Corr c = s_corr[lane];
+                    double* terms = s_terms[lane];
+                    if (c.flags & 1) {
+                        const double p[3] = {(double)c.p[0], (double)c.p[1], (double)c.p[2]};
+                        const double r[3] = {(double)c.r[0], (double)c.r[1], (double)c.r[2]};
+                        correspondence_terms(s_T, p, r, (c.flags & 2) != 0, c.cs, c.cr, P.kernel, P.kappa, terms);
+                    } else {
+#pragma unroll
+                        for (int t = 0; t < NTERMS; ++t) terms[t] = 0.0;
+                    }
+                }
+                __syncwarp();
+                if (lane < NTERMS) {
+#pragma unroll
+                    for (int w8 = 0; w8 < GWARPS; ++w8) acc += s_terms[w8][lane];
+                }
             }
-            __syncthreads();
-            if (threadIdx.x == 0) {
-                P.state->group_ticket[group] = 0u;
-                s_flag = (atomicAdd(&P.state->ticket, 1u) == (unsigned)n_groups - 1) ? 2 : 1;
-            }
-            __syncthreads();
-            if (s_flag == 2) {   // last group: final sum, solve, publish
-                __threadfence();
-                const double t2 = block_sum_rows(P.partials2, 0, n_groups, lane, wib, s_red);
+            if (rd + 1 < rounds) __syncthreads();             // the records are rewritten by the next round
+        }
+        TRACE_MAX(it, 1);
+        // ---- A10: block row -> group of 32 blocks -> grid, tagged words, every level summed in a fixed order --------
+        if (wib == 0) put_tagged(P.scratch.rows + (size_t)blockIdx.x * TSTRIDE + lane, lane < NTERMS ? acc : 0.0, tag);
+        if (blockIdx.x % GROUP == 0) {   // group leader: fold the group's rows into one
+            const double t = block_sum_tagged(P.scratch.rows, group * GROUP, group_rows, tag, lane, wib, s_red);
+            if (wib == 0) put_tagged(P.scratch.grows + (size_t)group * TSTRIDE + lane, t, tag);
+            if (blockIdx.x == 0) {       // block 0: final sum, solve, publish
+                const double t2 = block_sum_tagged(P.scratch.grows, 0, n_groups, tag, lane, wib, s_red);
                 if (wib == 0) s_terms[0][lane] = t2;
                 __syncthreads();
                 TRACE_MAX(it, 3);
                 if (threadIdx.x == 0) {
-                    solve_and_update(P, s_terms[0], s_T, it);
-                    P.state->ticket = 0u;
-                    __threadfence();
-                    atomicExch(&P.state->epoch, (unsigned)(it + 1));
+                    Pose Tn;
+                    const bool done = solve_and_update(P, s_terms[0], s_T, it, Tn);
+#pragma unroll
+                    for (int a = 0; a < 9; ++a) put_tagged(P.scratch.pub + a, Tn.R[a], tag);
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) put_tagged(P.scratch.pub + 9 + a, Tn.t[a], tag);
+                    put_tagged(P.scratch.pub + 12, done ? 1.0 : 0.0, tag);
                 }
                 TRACE_MAX(it, 4);
             }
         }
-        // ---- grid-wide wait for the new pose: all blocks are co-resident (cooperative launch) -------------------
-        if (threadIdx.x == 0) {
-            while (*reinterpret_cast<volatile unsigned int*>(&P.state->epoch) < (unsigned)(it + 1)) __nanosleep(32);
-            __threadfence();
+        // ---- grid-wide wait for the new pose: all blocks are co-resident (cooperative launch) -----------------------
+        __syncthreads();                                      // phase B / the sums have finished reading s_T, s_terms
+        if (threadIdx.x < NPUB) {
+            const double vv = wait_tagged(P.scratch.pub + threadIdx.x, tag);
+            if (threadIdx.x < 9) s_T.R[threadIdx.x] = vv;
+            else if (threadIdx.x < 12) s_T.t[threadIdx.x - 9] = vv;
+            else s_done = vv != 0.0 ? 1 : 0;
         }
         __syncthreads();
         TRACE_MAX(it, 5);
-        if (__ldcg(&P.state->done)) break;
-        if (threadIdx.x < 12) {
-            const double vv = __ldcg(threadIdx.x < 9 ? &P.state->pose.R[threadIdx.x] : &P.state->pose.t[threadIdx.x - 9]);
-            if (threadIdx.x < 9) s_T.R[threadIdx.x] = vv; else s_T.t[threadIdx.x - 9] = vv;
-        }
-        __syncthreads();
+        if (s_done) break;
     }
 }
 
@@ -459,11 +474,13 @@ void far_gicp_default_options(far_gicp_options_t* o) {
     o->kappa_div = 3.0;
 }
 
+static size_t gicp_scratch_bytes(int max_grid) { return ((size_t)(max_grid + MAX_GROUPS) * TSTRIDE + 16) * sizeof(uint4); }
+
 static int gicp_launch(const far_map_t* map, const float* d_scan, const float* d_cov6, const uint8_t* d_valid, int64_t n,
                        const int64_t* d_n, int stride, const far_pose_t* hpose, const far_pose_t* d_pose, double sigma,
                        int max_iters, int linearize_only, const far_gicp_options_t* opts, far_gicp_result_t* d_out,
                        void* stream) {
-    if (!map || !d_out || n < 0 || (n > 0 && !d_scan) || (stride != 3 && stride != 4) || max_iters < 1 || (!hpose && !d_pose))
+    if (!map || !d_out || n < 0 || (n > 0 && !d_scan) || (stride != 3 && stride != 4) || max_iters < 1 || max_iters > MAX_ITERS_LIMIT || (!hpose && !d_pose))
         return FAR_ERR_ARG;
     far_gicp_options_t o;
     if (opts) o = *opts; else far_gicp_default_options(&o);
@@ -479,15 +496,23 @@ static int gicp_launch(const far_map_t* map, const float* d_scan, const float* d
     P.kappa = sigma / o.kappa_div;
     P.conv_eps = o.conv_eps;
     P.kernel = o.kernel; P.max_iters = max_iters; P.linearize_only = linearize_only;
-    P.partials = map->d_gicp_partials;
-    P.partials2 = map->d_gicp_partials + (size_t)map->gicp_max_grid * TSTRIDE;
-    P.state = (GicpState*)map->d_gicp_state;
+    P.scratch.rows = reinterpret_cast<uint4*>(map->d_gicp_partials);
+    P.scratch.grows = P.scratch.rows + (size_t)map->gicp_max_grid * TSTRIDE;
+    P.scratch.pub = P.scratch.grows + (size_t)MAX_GROUPS * TSTRIDE;
     P.out = d_out;
     int64_t grid = map->gicp_max_grid;
     const int64_t need = (n + GWARPS - 1) / GWARPS;
     if (need < grid) grid = need;
     if (grid < 1) grid = 1;
-    FAR_CUDA(cudaMemsetAsync(map->d_gicp_state, 0, sizeof(GicpState), st));
+    // every launch gets its own tag space; on wrap-around of the 22-bit sequence the scratch is wiped once so that no
+    // word written 4 M launches ago can be mistaken for a current one
+    static std::atomic<uint32_t> g_seq{0};
+    uint32_t seq = g_seq.fetch_add(1, std::memory_order_relaxed) + 1;
+    if ((seq & 0x3FFFFFu) == 0) {
+        FAR_CUDA(cudaMemsetAsync(map->d_gicp_partials, 0, gicp_scratch_bytes(map->gicp_max_grid), st));
+        seq = g_seq.fetch_add(1, std::memory_order_relaxed) + 1;
+    }
+    P.seq = seq & 0x3FFFFFu;
     MapView view = map->view;
     void* args[] = {(void*)&view, (void*)&P};
     {
@@ -538,9 +563,10 @@ int gicp_setup(far_map* map) {
     if (per_sm < 1) per_sm = 1;
     map->gicp_max_grid = map->sm_count * per_sm;
     if (map->gicp_max_grid > GROUP * MAX_GROUPS) map->gicp_max_grid = GROUP * MAX_GROUPS;
-    FAR_CUDA(cudaMalloc((void**)&map->d_gicp_partials, (size_t)(map->gicp_max_grid + MAX_GROUPS) * TSTRIDE * sizeof(double)));
-    FAR_CUDA(cudaMalloc((void**)&map->d_gicp_state, sizeof(GicpState)));
-    FAR_CUDA(cudaMemset(map->d_gicp_state, 0, sizeof(GicpState)));
+    const size_t bytes = ((size_t)(map->gicp_max_grid + MAX_GROUPS) * TSTRIDE + 16) * sizeof(uint4);
+    FAR_CUDA(cudaMalloc((void**)&map->d_gicp_partials, bytes));
+    FAR_CUDA(cudaMemset(map->d_gicp_partials, 0, bytes));     // tag 0 is never used by a launch
+    map->d_gicp_state = nullptr;
     return FAR_OK;
 }
 }  // namespace far

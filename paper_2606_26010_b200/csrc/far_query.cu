@@ -4,10 +4,11 @@
 // PAPER.md:80 "closest Euclidean neighbor" (k = 1), PAPER.md:68-76 (k = 10 -> Eq. 1).
 //
 // Warp-cooperative design: lanes 0..26 each probe one neighbour voxel (27 independent hash lookups in flight
-// at once), the counts are prefix-summed across the warp, and the warp then sweeps the *flattened* candidate
-// list 32 points at a time -- consecutive lanes read consecutive float4 of a bucket, so the gathers coalesce and
-// no lane idles on a half-empty voxel.  Distances are FP64 with a fixed operation order (R6) so the arg-min is
-// bit-identical to the definition; the arg-min itself is three redux.sync steps.
+// at once); the query's own voxel is swept first and bounds the search (far_common.cuh::warp_nearest), the
+// counts of the voxels that can still matter are prefix-summed across the warp, and the warp sweeps that
+// *flattened* candidate list 32 points at a time -- consecutive lanes read consecutive float4 of a bucket, so the
+// gathers coalesce and no lane idles on a half-empty voxel.  Distances are FP64 with a fixed operation order (R6)
+// so the arg-min is bit-identical to the definition; the arg-min itself is three redux.sync steps.
 #include "far_internal.h"
 
 using namespace far;
@@ -15,36 +16,6 @@ using namespace far;
 namespace far {
 
 constexpr int QWARPS = 8;   // warps (= queries in flight) per block
-
-// map flat candidate j -> (voxel v, position) with a monotone walk over the prefix array
-__device__ __forceinline__ uint32_t cand_ref(const int* s_off, const uint32_t* s_slot, int j, int& v, int cap) {
-    while (j >= s_off[v + 1]) ++v;
-    return s_slot[v] * (uint32_t)cap + (uint32_t)(j - s_off[v]);
-}
-
-// nearest stored point of q among the 27 voxels around it; every lane returns the warp-wide winner
-__device__ __forceinline__ Best warp_nearest(const MapView& m, float qx, float qy, float qz, const int k[3], int lane,
-                                             int* s_off, uint32_t* s_slot) {
-    const int total = probe27(m, k, lane, s_off, s_slot);
-    Best best;
-    best.d2 = __longlong_as_double(0x7FF0000000000000ll);
-    best.id = NO_ID;
-    best.ref = 0;
-    int v = 0;
-    for (int j = lane; j < total; j += 32) {
-        const uint32_t ref = cand_ref(s_off, s_slot, j, v, m.cap);
-        const float4 p = __ldg(m.points + ref);
-        const double d2 = dist2(qx, qy, qz, p.x, p.y, p.z);
-        const uint32_t id = __float_as_uint(p.w);
-        if (better(d2, id, best)) { best.d2 = d2; best.id = id; best.ref = ref; }
-    }
-    __syncwarp();
-    const int w = warp_argmin(best.d2, best.id);
-    best.d2 = __shfl_sync(FULL, best.d2, w);
-    best.id = __shfl_sync(FULL, best.id, w);
-    best.ref = __shfl_sync(FULL, best.ref, w);
-    return best;
-}
 
 __global__ void __launch_bounds__(QWARPS * 32) nn_kernel(MapView m, const float* __restrict__ q, int64_t n, int stride,
                                                           uint32_t* __restrict__ out_id, float* __restrict__ out_d2) {
@@ -59,7 +30,8 @@ __global__ void __launch_bounds__(QWARPS * 32) nn_kernel(MapView m, const float*
         uint32_t id = NO_ID;
         float d2 = __int_as_float(0x7F800000);
         if (voxel_index(qx, qy, qz, m.voxel, k)) {
-            const Best b = warp_nearest(m, qx, qy, qz, k, lane, s_off[wib], s_slot[wib]);
+            float rx, ry, rz;
+            const Best b = warp_nearest(m, qx, qy, qz, k, lane, s_off[wib], s_slot[wib], rx, ry, rz);
             if (b.id != NO_ID) { id = b.id; d2 = __double2float_rn(b.d2); }
         }
         if (lane == 0) { out_id[i] = id; out_d2[i] = d2; }
