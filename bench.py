@@ -325,9 +325,19 @@ def run_far(args):
     peak = float(peaks.get("hbm_gbs", 6650.0))
     peak_kind = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
     nbytes = algorithmic_bytes(top, units.get(top, 0), cand.get(top, 0.0), n_slots=after["n_slots"])
+    # DRAM bytes per launch of the same kernel from the committed `ncu --set full` capture (never measured live:
+    # a number taken under a profiler is not a bench value)
+    traffic, traffic_src = None, None
+    try:
+        tr = json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json"))).get(top)
+        if tr:
+            traffic, traffic_src = tr["dram_bytes_per_launch"], f"{tr['capture']} ({tr['round']})"
+    except Exception:
+        pass
     dur_s = kern[top]["ms_per_step"] * 1e-3
     roof = {"bound": "hbm", "kernel": top, "achieved": (nbytes / dur_s / 1e9) if nbytes else None, "peak": peak,
-            "unit": "GB/s", "frac": (nbytes / dur_s / 1e9 / peak) if nbytes else None, "traffic": None,
+            "unit": "GB/s", "frac": (nbytes / dur_s / 1e9 / peak) if nbytes else None, "traffic": traffic,
+            "traffic_source": traffic_src,
             "peak_kind": peak_kind, "algorithmic_bytes_per_launch": nbytes, "kernel_ms": kern[top]["ms_per_step"],
             "kernel_share_of_step": kern[top]["share"], "units_per_launch": units.get(top), "candidates_per_query": cand.get(top),
             "note": "latency-bound at this size: a 5k-point registration cannot approach the HBM roofline (SURVEY 8d)"}
