@@ -21,4 +21,5 @@ from .generators import (  # noqa: F401
     c3_racing_frame,
     c4_insert_stress,
     c5_nn_sweep,
+    motion_distorted_scan,
 )

@@ -532,3 +532,60 @@ def c5_nn_sweep(seed=4, n_map=20_000_000, n_query=1_000_000, extent=1000.0):
     code = spread(g[:, 0]) | (spread(g[:, 1]) << 1) | (spread(g[:, 2]) << 2)
     morton = np.argsort(code, kind="stable")
     return dict(map_points=map_pts, queries=q, is_hit=is_hit, order=order, morton_order=morton)
+
+
+# --------------------------------------------------------------------------
+# a scan distorted by ego motion during the sweep
+# --------------------------------------------------------------------------
+def _twist_matrix(xi):
+    """4x4 matrix of the body twist xi = (v, w)"""
+    v, w = xi[:3], xi[3:]
+    return np.array([[0.0, -w[2], w[1], v[0]],
+                     [w[2], 0.0, -w[0], v[1]],
+                     [-w[1], w[0], 0.0, v[2]],
+                     [0.0, 0.0, 0.0, 0.0]])
+
+
+def motion_distorted_scan(seed=5, n=20000, duration=0.1, steps=1000, a=None, b=None, scene_radius=60.0,
+                          history=12, history_span=0.2, history_noise=0.0):
+    """Forward model of a sweep taken while the sensor moves (the INPUT of motion undistortion; none of the
+    method's arithmetic): static world points W, given in the sensor frame at the frame reference time t_ref (the
+    time of the last point), are observed one after the other while the sensor follows the body twist
+    xi(t) = a + b (t - t_ref).  The sensor pose relative to the t_ref pose, G(t), solves dG/dt = G [xi(t)]^ with
+    G(t_ref) = I; it is integrated backwards on a grid of `steps` intervals with scipy's matrix exponential at the
+    interval midpoints (error O(dt^3) per step, far below fp32 resolution) and the point times are grid times, so
+    `observed` is exact to integration error:  observed_i = fl32(G(t_i)^-1 W_i).
+
+    Returns dict(observed f32[n,3], time f32[n] (offset from the first point), dt_ref, world f64[n,3], a, b,
+    hist_times f64[history], hist_vel f64[history,6]) -- the history samples the twist line (+ optional noise)
+    over the `history_span` seconds before t_ref, in absolute time with t_ref = 100.0 s."""
+    from scipy.linalg import expm
+
+    rng = np.random.default_rng(seed)
+    if a is None:
+        a = np.array([69.4, 0.3, -0.1, 0.01, -0.02, 0.25])     # ~250 km/h forward, gentle yaw rate (PAPER.md:153)
+    if b is None:
+        b = np.array([-4.0, 0.5, 0.0, 0.0, 0.0, 0.6])
+    a, b = np.asarray(a, dtype=np.float64), np.asarray(b, dtype=np.float64)
+    dt = duration / steps
+    # G at grid times t_ref - j dt, j = 0..steps (backwards): G(t - dt) = G(t) expm(-[xi(t - dt/2)]^ dt)
+    G = np.empty((steps + 1, 4, 4))
+    G[0] = np.eye(4)
+    for j in range(steps):
+        tm = -(j + 0.5) * dt                                    # midpoint, relative to t_ref
+        G[j + 1] = G[j] @ expm(-_twist_matrix(a + b * tm) * dt)
+    # spinning-LiDAR-like ordering: the point's time grows with its azimuth
+    az = np.sort(rng.uniform(-math.pi, math.pi, n))
+    rad = rng.uniform(2.0, scene_radius, n)
+    z = rng.uniform(-2.0, 8.0, n)
+    world = np.stack([rad * np.cos(az), rad * np.sin(az), z], axis=1)
+    grid = np.minimum((np.arange(n) * (steps + 1)) // n, steps)    # 0 = first point ... steps = last point (t_ref)
+    back = steps - grid                                            # number of intervals before t_ref
+    Gi = np.linalg.inv(G[back])                                    # (n,4,4)
+    obs = np.einsum("nij,nj->ni", Gi[:, :3, :3], world) + Gi[:, :3, 3]
+    time = (grid * dt).astype(F32)
+    t_ref = 100.0
+    ht = t_ref - history_span + history_span * (np.arange(history) + 0.5) / history
+    hv = a[None, :] + b[None, :] * (ht - t_ref)[:, None] + rng.normal(0.0, history_noise, (history, 6))
+    return dict(observed=obs.astype(F32), time=time, dt_ref=float(duration), world=world, a=a, b=b,
+                hist_times=ht, hist_vel=hv, t_ref=t_ref)

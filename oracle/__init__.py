@@ -42,6 +42,21 @@ class PruneStats(C.Structure):
     _fields_ = [(n, C.c_int64) for n in ("n_voxels_removed", "n_points_removed", "n_voxels_left", "n_points_left")]
 
 
+class Motion(C.Structure):
+    """xi(t) = a + b (t - t_ref): body twist, linear velocity first (R15)"""
+    _fields_ = [("a", C.c_double * 6), ("b", C.c_double * 6)]
+
+    @staticmethod
+    def from_ab(a, b):
+        m = Motion()
+        m.a[:] = np.asarray(a, dtype=np.float64).reshape(6).tolist()
+        m.b[:] = np.asarray(b, dtype=np.float64).reshape(6).tolist()
+        return m
+
+    def to_ab(self):
+        return np.array(self.a[:]), np.array(self.b[:])
+
+
 class GicpOptions(C.Structure):
     _fields_ = [("kernel", C.c_int32), ("conv_eps", C.c_double), ("tau_mult", C.c_double), ("kappa_div", C.c_double)]
 
@@ -101,6 +116,12 @@ def lib():
         L.faro_threshold_update.restype = None
         L.faro_threshold_sigma.argtypes = [vp]
         L.faro_threshold_sigma.restype = f64
+        L.faro_motion_fit.argtypes = [vp, vp, i32, f64, vp]
+        L.faro_undistort.argtypes = [vp, vp, i64, C.c_int, f64, vp, vp]
+        L.faro_asmd_density.argtypes = [vp, vp, f64, vp, vp]
+        L.faro_asmd_cap.argtypes = [vp, f32, vp, f64, f64, i32, i32]
+        L.faro_asmd_cap.restype = i32
+        L.faro_map_insert_asmd.argtypes = [vp, vp, i64, C.c_int, vp, f64, f64, C.c_int, vp]
         _lib = L
     return _lib
 
@@ -169,6 +190,32 @@ def cov_from_points(pts, eps=1e-3):
     return out
 
 
+def motion_fit(times, vel6, t_ref):
+    """R15: least-squares line per twist component over the velocity history; returns (a, b)"""
+    t = np.ascontiguousarray(times, dtype=np.float64)
+    v = np.ascontiguousarray(vel6, dtype=np.float64).reshape(len(t), 6)
+    m = Motion()
+    _check(lib().faro_motion_fit(_p(t), _p(v), len(t), float(t_ref), C.byref(m)))
+    return m.to_ab()
+
+
+def undistort(xyz, time, dt_ref, a, b):
+    """R16: every point projected to the frame reference timestamp"""
+    p, n, s = _pts(xyz)
+    t = np.ascontiguousarray(time, dtype=np.float32)
+    assert t.shape == (n,)
+    out = np.empty((n, 3), dtype=np.float32)
+    m = Motion.from_ab(a, b)
+    _check(lib().faro_undistort(_p(p), _p(t), n, s, float(dt_ref), C.byref(m), _p(out)))
+    return out
+
+
+def asmd_cap(k3, voxel, center, n_close, d_max, k_min, cap):
+    k = np.ascontiguousarray(k3, dtype=np.int32)
+    c = np.ascontiguousarray(center, dtype=np.float64)
+    return int(lib().faro_asmd_cap(_p(k), voxel, _p(c), float(n_close), float(d_max), int(k_min), int(cap)))
+
+
 class Map:
     def __init__(self, voxel, cap, k_cov=10, cov_eps=1e-3):
         self.voxel, self.cap, self.k_cov = float(voxel), int(cap), int(k_cov)
@@ -187,6 +234,22 @@ class Map:
         pp = C.byref(Pose.from_rt(pose)) if pose is not None else None
         _check(lib().faro_map_insert(self._h, _p(a), n, s, pp, int(compute_cov), C.byref(st)))
         return {f: getattr(st, f) for f, _ in st._fields_}
+
+    def insert_asmd(self, xyz, n_close, d_max, pose=None, compute_cov=False):
+        """PAPER.md:109 / R17: per-voxel limit N_ASMD instead of the fixed cap"""
+        a, n, s = _pts(xyz)
+        st = InsertStats()
+        pp = C.byref(Pose.from_rt(pose)) if pose is not None else None
+        _check(lib().faro_map_insert_asmd(self._h, _p(a), n, s, pp, float(n_close), float(d_max), int(compute_cov),
+                                          C.byref(st)))
+        return {f: getattr(st, f) for f, _ in st._fields_}
+
+    def asmd_density(self, center, r_close):
+        """mean stored points per voxel within r_close of center, and the number of such voxels"""
+        c = np.ascontiguousarray(center, dtype=np.float64)
+        out, nv = C.c_double(0.0), C.c_int64(0)
+        _check(lib().faro_asmd_density(self._h, _p(c), float(r_close), C.byref(out), C.byref(nv)))
+        return out.value, nv.value
 
     def prune(self, center, radius):
         c = np.ascontiguousarray(center, dtype=np.float64)

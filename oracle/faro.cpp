@@ -283,12 +283,33 @@ faro_map_t* faro_map_create(float voxel, int32_t cap, int32_t k_cov, double cov_
 }
 void faro_map_destroy(faro_map_t* m) { delete m; }
 
-// A3/A4 (reading R3): sequential semantics, lowest id wins, ids = next_id + i
-int faro_map_insert(faro_map_t* m, const float* xyz, int64_t n, int stride, const faro_pose_t* pose,
-                    int compute_cov, faro_insert_stats_t* stats) {
+namespace {
+
+// R17: N_ASMD of a voxel seen from `c`; every operation one rounded binary64 operation
+int32_t asmd_cap(const int32_t k[3], float voxel, const double c[3], double n_close, double d_max, int32_t k_min,
+                 int32_t cap) {
+    const double v = (double)voxel;
+    const double dx = ((double)k[0] + 0.5) * v - c[0];
+    const double dy = ((double)k[1] + 0.5) * v - c[1];
+    const double dz = ((double)k[2] + 0.5) * v - c[2];
+    const double d = std::sqrt((dx * dx + dy * dy) + dz * dz);
+    const double f = 1.0 - d / d_max;                      // linear decay over range
+    const double x = std::floor(n_close * f + 0.5);
+    int32_t lim = k_min;                                   // lower bound: the k points a covariance needs
+    if (x > (double)k_min) lim = (x >= (double)cap) ? cap : (int32_t)x;
+    if (lim > cap) lim = cap;
+    return lim;
+}
+
+// A3/A4 (reading R3): sequential semantics, lowest id wins, ids = next_id + i.
+// asmd: per-voxel limit N_ASMD instead of the fixed cap (reading R17)
+int insert_points(faro_map_t* m, const float* xyz, int64_t n, int stride, const faro_pose_t* pose, bool asmd,
+                  double n_close, double d_max, int compute_cov, faro_insert_stats_t* stats) {
     if (!m || !xyz || n < 0 || (stride != 3 && stride != 4)) return FARO_ERR_ARG;
     if (m->next_id + (uint64_t)n > 0xFFFFFFFFull) return FARO_ERR_RANGE;
     faro_insert_stats_t st = {n, 0, 0, 0, 0};
+    const double origin[3] = {0.0, 0.0, 0.0};
+    const double* centre = pose ? pose->t : origin;
     std::vector<std::pair<uint64_t, uint32_t>> added;   // (key, id) of accepted points
     for (int64_t i = 0; i < n; ++i) {
         const float* s = xyz + i * stride;
@@ -302,7 +323,8 @@ int faro_map_insert(faro_map_t* m, const float* xyz, int64_t n, int stride, cons
         auto ins = m->vox.try_emplace(key);
         if (ins.second) st.n_new_voxels++;
         Voxel& vx = ins.first->second;
-        if ((int32_t)vx.pts.size() < m->cap) {
+        const int32_t limit = asmd ? asmd_cap(k, m->voxel, centre, n_close, d_max, m->k_cov, m->cap) : m->cap;
+        if ((int32_t)vx.pts.size() < limit) {
             Pt pt{p[0], p[1], p[2], id, {1, 0, 0, 1, 0, 1}, 0};
             vx.pts.push_back(pt);
             st.n_accepted++;
@@ -322,6 +344,47 @@ int faro_map_insert(faro_map_t* m, const float* xyz, int64_t n, int stride, cons
             }
     }
     if (stats) *stats = st;
+    return FARO_OK;
+}
+
+}  // namespace
+
+int faro_map_insert(faro_map_t* m, const float* xyz, int64_t n, int stride, const faro_pose_t* pose,
+                    int compute_cov, faro_insert_stats_t* stats) {
+    return insert_points(m, xyz, n, stride, pose, false, 0.0, 1.0, compute_cov, stats);
+}
+
+// SURVEY 8(f)-1, reading R17
+int faro_map_insert_asmd(faro_map_t* m, const float* xyz, int64_t n, int stride, const faro_pose_t* pose,
+                         double n_close, double d_max, int compute_cov, faro_insert_stats_t* stats) {
+    if (!(d_max > 0.0) || !(n_close >= 0.0)) return FARO_ERR_ARG;
+    return insert_points(m, xyz, n, stride, pose, true, n_close, d_max, compute_cov, stats);
+}
+
+int32_t faro_asmd_cap(const int32_t k3[3], float voxel, const double center[3], double n_close, double d_max,
+                      int32_t k_min, int32_t cap) {
+    return asmd_cap(k3, voxel, center, n_close, d_max, k_min, cap);
+}
+
+// PAPER.md:109 "the average amount of points per voxel in a close range of the current scan"
+int faro_asmd_density(const faro_map_t* local, const double center[3], double r_close, double* n_close,
+                      int64_t* n_voxels_close) {
+    if (!local || !center || !n_close) return FARO_ERR_ARG;
+    const double v = (double)local->voxel;
+    const double r2 = r_close * r_close;
+    int64_t nv = 0, np = 0;
+    for (const auto& kv : local->vox) {
+        if (kv.second.pts.empty()) continue;
+        int32_t k[3];
+        unpack(kv.first, k);
+        const double dx = ((double)k[0] + 0.5) * v - center[0];
+        const double dy = ((double)k[1] + 0.5) * v - center[1];
+        const double dz = ((double)k[2] + 0.5) * v - center[2];
+        const double d2 = (dx * dx + dy * dy) + dz * dz;
+        if (d2 <= r2) { nv++; np += (int64_t)kv.second.pts.size(); }
+    }
+    *n_close = nv > 0 ? (double)np / (double)nv : (double)local->cap;
+    if (n_voxels_close) *n_voxels_close = nv;
     return FARO_OK;
 }
 
@@ -744,6 +807,69 @@ void faro_threshold_update(faro_threshold_t* t, const faro_pose_t* pred, const f
 double faro_threshold_sigma(const faro_threshold_t* t) {
     if (t->count == 0) return t->sigma0;
     return std::sqrt(t->sse / (double)t->count);
+}
+
+
+// ---- motion undistortion (readings R15/R16) -----------------------------------
+// R15: ordinary least squares line x(t) = a + b (t - t_ref) per twist component
+int faro_motion_fit(const double* times, const double* vel6, int32_t m, double t_ref, faro_motion_t* out) {
+    if (!times || !vel6 || !out || m < 1) return FARO_ERR_ARG;
+    double sbar = 0.0;
+    for (int32_t j = 0; j < m; ++j) sbar += times[j] - t_ref;
+    sbar /= (double)m;
+    double sxx = 0.0;
+    for (int32_t j = 0; j < m; ++j) { const double ds = (times[j] - t_ref) - sbar; sxx += ds * ds; }
+    for (int c = 0; c < 6; ++c) {
+        double xbar = 0.0;
+        for (int32_t j = 0; j < m; ++j) xbar += vel6[6 * j + c];
+        xbar /= (double)m;
+        double sxy = 0.0;
+        for (int32_t j = 0; j < m; ++j) sxy += ((times[j] - t_ref) - sbar) * (vel6[6 * j + c] - xbar);
+        const double slope = sxx > 0.0 ? sxy / sxx : 0.0;
+        out->b[c] = slope;
+        out->a[c] = xbar - slope * sbar;          // value of the line at t = t_ref
+    }
+    return FARO_OK;
+}
+
+// R16: Magnus expansion (to second order) of the linear twist between the point's time and t_ref.
+// dG/dt = G [xi(t)]^ (body twist), xi(t) = a + b (t - t_ref), Delta = t_ref - t_i:
+//   Omega_1 = int xi = a Delta - b Delta^2 / 2
+//   Omega_2 = +(1/2) int int [xi(s1), xi(s2)] ds2 ds1 (sign of the right-multiplied ODE) = [a, b] Delta^3 / 12
+//   with the se(3) bracket [(v1,w1),(v2,w2)] = (w1 x v2 - w2 x v1, w1 x w2);  G(t_i)^-1 G(t_ref) = Exp(Omega_1 + Omega_2)
+// and the point moves by the inverse: out = fl32(Exp(-(Omega_1 + Omega_2)) p).
+int faro_undistort(const float* xyz, const float* time, int64_t n, int stride, double dt_ref,
+                   const faro_motion_t* motion, float* out_xyz) {
+    if ((!xyz && n > 0) || (!time && n > 0) || !motion || (!out_xyz && n > 0) || n < 0 || (stride != 3 && stride != 4))
+        return FARO_ERR_ARG;
+    const double* a = motion->a;
+    const double* b = motion->b;
+    const double* va = a;      const double* wa = a + 3;
+    const double* vb = b;      const double* wb = b + 3;
+    double br[6];              // [a, b]
+    br[0] = (wa[1] * vb[2] - wa[2] * vb[1]) - (wb[1] * va[2] - wb[2] * va[1]);
+    br[1] = (wa[2] * vb[0] - wa[0] * vb[2]) - (wb[2] * va[0] - wb[0] * va[2]);
+    br[2] = (wa[0] * vb[1] - wa[1] * vb[0]) - (wb[0] * va[1] - wb[1] * va[0]);
+    br[3] = wa[1] * wb[2] - wa[2] * wb[1];
+    br[4] = wa[2] * wb[0] - wa[0] * wb[2];
+    br[5] = wa[0] * wb[1] - wa[1] * wb[0];
+    for (int64_t i = 0; i < n; ++i) {
+        const float* s = xyz + i * stride;
+        float* o = out_xyz + 3 * i;
+        if (!std::isfinite(s[0]) || !std::isfinite(s[1]) || !std::isfinite(s[2]) || !std::isfinite(time[i])) {
+            o[0] = s[0]; o[1] = s[1]; o[2] = s[2];
+            continue;
+        }
+        const double D = dt_ref - (double)time[i];
+        const double h = 0.5 * (D * D);
+        const double g = (D * D) * D / 12.0;
+        double neg_omega[6];
+        for (int c = 0; c < 6; ++c) neg_omega[c] = -((a[c] * D - b[c] * h) + br[c] * g);
+        faro_pose_t E;
+        faro_se3_exp(neg_omega, &E);
+        transform_pt(E, s, o);
+    }
+    return FARO_OK;
 }
 
 }  // extern "C"

@@ -105,6 +105,38 @@ void faro_threshold_destroy(faro_threshold_t*);
 void faro_threshold_update(faro_threshold_t*, const faro_pose_t* predicted, const faro_pose_t* registered);
 double faro_threshold_sigma(const faro_threshold_t*);
 
+/* ---- SURVEY 8(f)-2  PAPER.md:56 (Preprocessing & Undistortion); readings R15/R16 in DESIGN.md --------------
+ * "We perform a linear regression on both the linear and angular velocities ... This continuous motion model is
+ * evaluated ... each raw point is undistorted and projected to the frame reference timestamp, which is equal to
+ * the scan's final point-timestamp."
+ * motion: body twist xi(t) = a + b (t - t_ref), 6-vectors (linear velocity first, then angular velocity). */
+typedef struct { double a[6]; double b[6]; } faro_motion_t;
+/* R15: ordinary least-squares line per component over m history samples (times[j], vel[j*6 .. j*6+5]);
+ * fewer than 2 distinct times -> b = 0, a = mean. */
+int faro_motion_fit(const double* times, const double* vel6, int32_t m, double t_ref, faro_motion_t* out);
+/* R16: point i was measured at t_first + time[i]; Delta_i = dt_ref - (double)time[i] (dt_ref = t_ref - t_first);
+ * Omega_i = a Delta_i - b Delta_i^2 / 2 + [a,b] Delta_i^3 / 12 (Magnus expansion to second order, se(3) bracket);
+ * out_i = fl32(Exp(-Omega_i) p_i)  (SE(3) exponential of R12, transform of R4).
+ * out_xyz: n*3 floats; non-finite points are copied unchanged. */
+int faro_undistort(const float* xyz, const float* time, int64_t n, int stride, double dt_ref,
+                   const faro_motion_t* motion, float* out_xyz);
+
+/* ---- SURVEY 8(f)-1  PAPER.md:109 (Adaptive Submap Density); reading R17 -------------------------------------
+ * "the average amount of points per voxel in a close range of the current scan is computed ... linear decay (with
+ * a lower bound defined by the k = 10 points required to compute the covariances) ... integrated into the
+ * corresponding voxels ... as long as the number of points inside it is below N_ASMD."
+ * density: mean stored points per voxel over the voxels of `local` whose centre is within r_close of `center`
+ * (|(k+0.5)v - c|^2 <= r_close^2, FP64 as in R5); *n_close = cap of `local` if there is no such voxel. */
+int faro_asmd_density(const faro_map_t* local, const double center[3], double r_close, double* n_close,
+                      int64_t* n_voxels_close);
+/* N_ASMD of the voxel with index k3 seen from `center`: clamp(floor(n_close (1 - d/d_max) + 0.5), k_min, cap),
+ * d = |(k+0.5)v - center| ; every operation one rounded binary64 operation. */
+int32_t faro_asmd_cap(const int32_t k3[3], float voxel, const double center[3], double n_close, double d_max,
+                      int32_t k_min, int32_t cap);
+/* faro_map_insert with the per-voxel limit N_ASMD (centre = pose->t, or the origin without a pose; k_min = k_cov) */
+int faro_map_insert_asmd(faro_map_t*, const float* xyz, int64_t n, int stride, const faro_pose_t* pose_or_null,
+                         double n_close, double d_max, int compute_cov, faro_insert_stats_t* stats);
+
 #ifdef __cplusplus
 }
 #endif
