@@ -186,11 +186,55 @@ int far_gicp_register_dev(const far_map_t* map, const float* d_scan, const float
 int far_map_knn_cov_dev(const far_map_t* map, const float* d_q, const int64_t* d_m, int64_t m_max, int stride,
                         float* d_cov6, uint8_t* d_valid, void* stream);
 
+/* ---- motion undistortion ("Preprocessing & Undistortion"; R15/R16) -----------------
+ * "the distortion of the LiDAR scan is corrected using the velocity history of the Sensor Fusion.  We perform a
+ * linear regression on both the linear and angular velocities ...  This continuous motion model is evaluated in
+ * CUDA ... each raw point is undistorted and projected to the frame reference timestamp, which is equal to the
+ * scan's final point-timestamp."
+ * far_motion_t: body twist xi(t) = a + b (t - t_ref), 6-vectors (linear velocity [m/s] first, then angular
+ * velocity [rad/s]), t_ref = frame reference time. */
+typedef struct { double a[6]; double b[6]; } far_motion_t;
+/* R15, HOST-only FP64 helper (a 6-component line fit, boundary logic): ordinary least squares over m history
+ * samples (times[j], vel6[6 j .. 6 j + 5]), all HOST pointers.  Fewer than two distinct times: b = 0, a = mean. */
+int far_motion_fit(const double* times, const double* vel6, int32_t m, double t_ref, far_motion_t* out);
+/* R16: point i was measured at t_first + d_time[i] (fp32 offsets, DEVICE); Delta_i = dt_ref - (double)d_time[i]
+ * with dt_ref = t_ref - t_first (the sweep duration when t_ref is the last point's time).
+ *   Omega_i = a Delta_i - b Delta_i^2/2 + [a,b] Delta_i^3/12      (Magnus expansion of the linear twist to second
+ *                                                                  order; [.,.] the se(3) bracket)
+ *   d_out_xyz[i] = fl32(Exp(-Omega_i) p_i)                        (SE(3) exponential of R12), FP64 arithmetic.
+ * motion: HOST pointer, read during the call.  d_out_xyz: n*3 fp32, may NOT alias d_xyz.  Points with a non-finite
+ * coordinate or time are copied unchanged.  One pass, 16 B read (28 B at stride 4 with .w) + 12 B written a point. */
+int far_undistort(const float* d_xyz, const float* d_time, int64_t n, int stride, double dt_ref,
+                  const far_motion_t* motion, float* d_out_xyz, void* stream);
+
+/* ---- Adaptive Submap Density (R17) ------------------------------------------------
+ * "Before the map is updated, the average amount of points per voxel in a close range of the current scan is
+ * computed ...  we use a linear decay (with a lower bound defined by the k = 10 points required to compute the
+ * covariances) ... integrated into the corresponding voxels ... as long as the number of points inside it is
+ * below N_ASMD."
+ * far_asmd_density: d_out[0] = n_close = mean stored points per live voxel of `local` (the scan-local map of R8)
+ * over the voxels with |(k + 0.5) v - center|^2 <= r_close^2 (FP64, R5 form); = cap of `local` if there is none.
+ * d_out[1] = number of such voxels (as a double).  center: HOST double[3].  d_out: DEVICE double[2]. */
+int far_asmd_density(const far_map_t* local, const double center[3], double r_close, double* d_out, void* stream);
+/* far_map_insert with the per-voxel limit
+ *   N_ASMD(k) = clamp(floor(n_close (1 - d/d_max) + 0.5), k_cov, cap),  d = |(k + 0.5) v - c|,
+ * c = the pose translation (the origin without a pose), every operation one rounded binary64 operation; n_close is
+ * read from DEVICE memory (d_n_close[0], e.g. written by far_asmd_density) in stream order.  Same sequential
+ * semantics as far_map_insert (R3) with `count < N_ASMD(k)` as the acceptance test; points already stored are never
+ * removed, whatever the limit of their voxel has become. */
+int far_map_insert_asmd(far_map_t* map, const float* d_xyz, int64_t n, int stride, const far_pose_t* pose_or_null,
+                        const double* d_n_close, double d_max, int compute_cov, far_insert_stats_t* d_stats,
+                        void* stream);
+int far_map_insert_asmd_dev(far_map_t* map, const float* d_xyz, int64_t n, int stride, const far_pose_t* d_pose,
+                            const double* d_n_close, double d_max, int compute_cov, far_insert_stats_t* d_stats,
+                            void* stream);
+
 /* ---- one frame through the whole path (the LiDAR scan callback) -----------------------------
  * far_frontend_process chains, in stream order and with NO host synchronisation: far_voxelize (ds_voxel) ->
  * scan-local map of the raw scan + far_map_knn_cov of the downsampled points (Sigma_s) ->
  * far_gicp_register against the frontend's map from init_pose -> (update_map) far_map_insert of the raw scan at
- * the registered pose with covariances + far_map_prune about it.  Sizes and the registered pose
+ * the registered pose with covariances (cfg.asmd: far_asmd_density of the scan-local map about the sensor, then
+ * far_map_insert_asmd) + far_map_prune about it.  Sizes and the registered pose
  * flow between the stages through device memory.  d_out (device, nullable = internal buffer) receives the
  * registration result.  The _host variant takes a HOST scan (pinned for a truly asynchronous copy) and a HOST
  * result struct: it uploads, runs the chain, downloads the result and synchronises the stream. */
@@ -202,6 +246,9 @@ typedef struct {
     int32_t max_iters;          /* GICP iteration limit (R14)                                          */
     int32_t update_map;         /* 0: register only                                                    */
     far_gicp_options_t gicp;
+    int32_t asmd;               /* 1: map update with the Adaptive Submap Density limit (R17) */
+    double asmd_r_close;        /* "close range of the current scan" [m] for the density; 0 -> 10         */
+    double asmd_d_max;          /* range at which the linear decay reaches the lower bound; 0 -> 100       */
 } far_frontend_config_t;
 typedef struct far_frontend far_frontend_t;
 int far_frontend_create(far_frontend_t** out, const far_frontend_config_t* cfg);
@@ -211,6 +258,11 @@ int far_frontend_process(far_frontend_t* f, const float* d_scan, int64_t n, int 
                          double sigma, far_gicp_result_t* d_out, void* stream);
 int far_frontend_process_host(far_frontend_t* f, const float* h_scan, int64_t n, int stride,
                               const far_pose_t* init_pose, double sigma, far_gicp_result_t* h_out, void* stream);
+/* the whole LiDAR scan callback of PAPER.md:54-109 including its first step: far_undistort of the raw sweep
+ * (d_time, dt_ref, motion as in far_undistort) into an internal buffer, then far_frontend_process on the result */
+int far_frontend_process_sweep(far_frontend_t* f, const float* d_scan, const float* d_time, int64_t n, int stride,
+                               double dt_ref, const far_motion_t* motion, const far_pose_t* init_pose, double sigma,
+                               far_gicp_result_t* d_out, void* stream);
 
 /* Adaptive threshold of Vizzo et al. [1] as read in R10.  HOST-only FP64 helper (20 lines of
  * boundary logic, not a kernel): sigma = sqrt(mean delta_i^2) over recorded deviations delta_i > min_motion,

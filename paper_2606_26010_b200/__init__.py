@@ -57,7 +57,23 @@ class GicpResult(C.Structure):
 
 class FrontendConfig(C.Structure):
     _fields_ = [("map", MapConfig), ("ds_voxel", C.c_float), ("max_scan_points", C.c_int64), ("prune_radius", C.c_double),
-                ("max_iters", C.c_int32), ("update_map", C.c_int32), ("gicp", GicpOptions)]
+                ("max_iters", C.c_int32), ("update_map", C.c_int32), ("gicp", GicpOptions),
+                ("asmd", C.c_int32), ("asmd_r_close", C.c_double), ("asmd_d_max", C.c_double)]
+
+
+class Motion(C.Structure):
+    """far_motion_t: body twist xi(t) = a + b (t - t_ref), linear velocity first (R15)"""
+    _fields_ = [("a", C.c_double * 6), ("b", C.c_double * 6)]
+
+    @staticmethod
+    def from_ab(a, b):
+        m = Motion()
+        m.a[:] = np.asarray(a, dtype=np.float64).reshape(6).tolist()
+        m.b[:] = np.asarray(b, dtype=np.float64).reshape(6).tolist()
+        return m
+
+    def to_ab(self):
+        return np.array(self.a[:]), np.array(self.b[:])
 
 
 INSERT_STATS_FIELDS = ("n_offered", "n_accepted", "n_new_voxels", "n_dropped_full", "n_invalid")
@@ -118,6 +134,12 @@ def lib():
             "far_frontend_map": (vp, [vp]),
             "far_frontend_process": (ci, [vp, vp, i64, ci, vp, f64, vp, vp]),
             "far_frontend_process_host": (ci, [vp, vp, i64, ci, vp, f64, vp, vp]),
+            "far_frontend_process_sweep": (ci, [vp, vp, vp, i64, ci, f64, vp, vp, f64, vp, vp]),
+            "far_motion_fit": (ci, [vp, vp, i32, f64, vp]),
+            "far_undistort": (ci, [vp, vp, i64, ci, f64, vp, vp, vp]),
+            "far_asmd_density": (ci, [vp, vp, f64, vp, vp]),
+            "far_map_insert_asmd": (ci, [vp, vp, i64, ci, vp, vp, f64, ci, vp, vp]),
+            "far_map_insert_asmd_dev": (ci, [vp, vp, i64, ci, vp, vp, f64, ci, vp, vp]),
             "far_threshold_create": (vp, [f64, f64, f64]),
             "far_threshold_destroy": (None, [vp]),
             "far_threshold_update": (None, [vp, vp, vp]),
@@ -229,6 +251,29 @@ def voxelize(xyz, voxel):
     return Voxelizer(max(n, 1), device=x.device)(x, voxel)
 
 
+def motion_fit(times, vel6, t_ref):
+    """far_motion_fit (host-only FP64 helper, R15): returns (a, b) of xi(t) = a + b (t - t_ref)"""
+    t = np.ascontiguousarray(times, dtype=np.float64)
+    v = np.ascontiguousarray(vel6, dtype=np.float64).reshape(len(t), 6)
+    m = Motion()
+    _check(lib().far_motion_fit(C.c_void_p(t.ctypes.data), C.c_void_p(v.ctypes.data), len(t), float(t_ref), C.byref(m)),
+           "far_motion_fit")
+    return m.to_ab()
+
+
+def undistort(xyz, time, dt_ref, a, b, out=None):
+    """far_undistort (R16): device (n,3|4) points + device (n,) fp32 time offsets -> device (n,3)"""
+    x, n, s = _points(xyz)
+    t = time if isinstance(time, torch.Tensor) else torch.as_tensor(np.ascontiguousarray(time, dtype=np.float32))
+    t = t.to(device="cuda", dtype=torch.float32).contiguous()
+    assert t.shape == (n,)
+    if out is None:
+        out = torch.empty((n, 3), dtype=torch.float32, device="cuda")
+    m = Motion.from_ab(a, b)
+    _check(lib().far_undistort(_ptr(x), _ptr(t), n, s, float(dt_ref), C.byref(m), _ptr(out), _stream()), "far_undistort")
+    return out
+
+
 class Map:
     """A far_map_t handle.  All bulk arguments are CUDA tensors (NumPy arrays are uploaded for convenience)."""
 
@@ -280,6 +325,33 @@ class Map:
 
     def insert(self, xyz, pose=None, compute_cov=False):
         self.insert_enqueue(xyz, pose, compute_cov)
+        return dict(zip(INSERT_STATS_FIELDS, self._insert_stats.tolist()))
+
+    def asmd_density(self, center, r_close, out=None):
+        """far_asmd_density (R17): device double[2] = (n_close, number of close voxels)"""
+        if out is None:
+            out = torch.empty(2, dtype=torch.float64, device="cuda")
+        c = (C.c_double * 3)(*[float(v) for v in center])
+        _check(lib().far_asmd_density(self._h, c, float(r_close), _ptr(out), _stream()), "far_asmd_density")
+        return out
+
+    def insert_asmd_enqueue(self, xyz, d_n_close, d_max, pose=None, compute_cov=False, d_pose=None):
+        """far_map_insert_asmd(_dev): per-voxel limit N_ASMD; d_n_close is a device double tensor"""
+        x, n, s = _points(xyz)
+        if not isinstance(d_n_close, torch.Tensor):
+            d_n_close = torch.tensor([float(d_n_close)], dtype=torch.float64, device="cuda")
+        if d_pose is not None:
+            rc = lib().far_map_insert_asmd_dev(self._h, _ptr(x), n, s, _ptr(d_pose), _ptr(d_n_close), float(d_max),
+                                               int(compute_cov), _ptr(self._insert_stats), _stream())
+        else:
+            pp = C.byref(Pose.from_rt(pose)) if pose is not None else None
+            rc = lib().far_map_insert_asmd(self._h, _ptr(x), n, s, pp, _ptr(d_n_close), float(d_max), int(compute_cov),
+                                           _ptr(self._insert_stats), _stream())
+        _check(rc, "far_map_insert_asmd")
+        self._keep = d_n_close
+
+    def insert_asmd(self, xyz, n_close, d_max, pose=None, compute_cov=False):
+        self.insert_asmd_enqueue(xyz, n_close, d_max, pose, compute_cov)
         return dict(zip(INSERT_STATS_FIELDS, self._insert_stats.tolist()))
 
     def prune_enqueue(self, center=None, radius=0.0, d_pose=None):
@@ -409,12 +481,14 @@ class Frontend:
     """far_frontend_*: one frame through the whole hot path as a single stream-ordered chain."""
 
     def __init__(self, voxel, cap, max_voxels, max_scan_points, ds_voxel=0.0, prune_radius=0.0, max_iters=30,
-                 update_map=True, opts=None, k_cov=10, cov_eps=1e-3, max_load=0.5):
+                 update_map=True, opts=None, k_cov=10, cov_eps=1e-3, max_load=0.5, asmd=False, asmd_r_close=10.0,
+                 asmd_d_max=100.0):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2606_26010_b200 needs a CUDA device: there is no CPU fallback")
         o = opts if opts is not None else default_options()
         cfg = FrontendConfig(MapConfig(voxel, cap, int(max_voxels), max_load, 1, k_cov, cov_eps, 0), ds_voxel,
-                             int(max_scan_points), float(prune_radius), int(max_iters), int(update_map), o)
+                             int(max_scan_points), float(prune_radius), int(max_iters), int(update_map), o,
+                             int(asmd), float(asmd_r_close), float(asmd_d_max))
         h = C.c_void_p()
         _check(lib().far_frontend_create(C.byref(h), C.byref(cfg)), "far_frontend_create")
         self._h = h
@@ -440,6 +514,15 @@ class Frontend:
         po = Pose.from_rt(init_pose) if not isinstance(init_pose, Pose) else init_pose
         _check(lib().far_frontend_process(self._h, _ptr(x), n, s, C.byref(po), float(sigma), _ptr(d_result), _stream()),
                "far_frontend_process")
+
+    def process_sweep_enqueue(self, d_scan, d_time, dt_ref, a, b, init_pose, sigma, d_result=None):
+        """Raw sweep + per-point time offsets in: far_undistort, then the chain of process_enqueue."""
+        x, n, s = _points(d_scan)
+        assert d_time.dtype == torch.float32 and d_time.shape == (n,) and d_time.is_cuda
+        po = Pose.from_rt(init_pose) if not isinstance(init_pose, Pose) else init_pose
+        m = Motion.from_ab(a, b)
+        _check(lib().far_frontend_process_sweep(self._h, _ptr(x), _ptr(d_time), n, s, float(dt_ref), C.byref(m), C.byref(po),
+                                                float(sigma), _ptr(d_result), _stream()), "far_frontend_process_sweep")
 
     def process_host(self, h_scan, init_pose, sigma):
         """HOST scan (a pinned torch CPU tensor or a NumPy array) in, result dict out; uploads, runs, downloads, syncs."""

@@ -24,6 +24,8 @@ struct far_frontend {
     uint8_t* d_valid;
     far_pose_t* d_init;
     far_gicp_result_t* d_result;
+    double* d_asmd;          // [2] n_close, number of close voxels (far_asmd_density)
+    float* d_undist;         // undistorted sweep [max_scan_points * 3] (far_frontend_process_sweep)
 };
 
 extern "C" {
@@ -33,7 +35,7 @@ int far_frontend_destroy(far_frontend_t* f) {
     far_map_destroy(f->map);
     far_map_destroy(f->local);
     cudaFree(f->d_ws); cudaFree(f->d_scan); cudaFree(f->d_ds_xyz); cudaFree(f->d_ds_index); cudaFree(f->d_n_ds);
-    cudaFree(f->d_cov6); cudaFree(f->d_valid); cudaFree(f->d_init); cudaFree(f->d_result);
+    cudaFree(f->d_cov6); cudaFree(f->d_valid); cudaFree(f->d_init); cudaFree(f->d_result); cudaFree(f->d_asmd); cudaFree(f->d_undist);
     delete f;
     return FAR_OK;
 }
@@ -46,6 +48,8 @@ int far_frontend_create(far_frontend_t** out, const far_frontend_config_t* cfg) 
     memset(f, 0, sizeof(*f));
     f->cfg = *cfg;
     if (!(f->cfg.ds_voxel > 0.f)) f->cfg.ds_voxel = cfg->map.voxel_size;
+    if (!(f->cfg.asmd_r_close > 0.0)) f->cfg.asmd_r_close = 10.0;
+    if (!(f->cfg.asmd_d_max > 0.0)) f->cfg.asmd_d_max = 100.0;
     far_map_config_t mc = cfg->map;
     mc.with_cov = 1;
     if (mc.max_batch < cfg->max_scan_points) mc.max_batch = cfg->max_scan_points;
@@ -72,6 +76,8 @@ int far_frontend_create(far_frontend_t** out, const far_frontend_config_t* cfg) 
     alloc((void**)&f->d_valid, (size_t)n);
     alloc((void**)&f->d_init, sizeof(far_pose_t));
     alloc((void**)&f->d_result, sizeof(far_gicp_result_t));
+    alloc((void**)&f->d_asmd, 2 * sizeof(double));
+    alloc((void**)&f->d_undist, (size_t)n * 3 * sizeof(float));
     if (rc != FAR_OK || e != cudaSuccess) {
         if (e != cudaSuccess) far::set_cuda_error(e, "cudaMalloc in far_frontend_create");
         far_frontend_destroy(f);
@@ -103,10 +109,24 @@ int far_frontend_process(far_frontend_t* f, const float* d_scan, int64_t n, int 
                                     f->cfg.max_iters, &f->cfg.gicp, res, stream))) return rc;
     // A3-A5, A7: submap update at the registered pose
     if (f->cfg.update_map) {
-        if ((rc = far_map_insert_dev(f->map, d_scan, n, stride, &res->pose, 1, nullptr, stream))) return rc;
+        if (f->cfg.asmd) {
+            // density "in a close range of the current scan" = scan-local map about the sensor origin
+            const double origin[3] = {0.0, 0.0, 0.0};
+            if ((rc = far_asmd_density(f->local, origin, f->cfg.asmd_r_close, f->d_asmd, stream))) return rc;
+            if ((rc = far_map_insert_asmd_dev(f->map, d_scan, n, stride, &res->pose, f->d_asmd, f->cfg.asmd_d_max, 1, nullptr, stream))) return rc;
+        } else if ((rc = far_map_insert_dev(f->map, d_scan, n, stride, &res->pose, 1, nullptr, stream))) return rc;
         if (f->cfg.prune_radius > 0.0 && (rc = far_map_prune_dev(f->map, &res->pose, f->cfg.prune_radius, nullptr, stream))) return rc;
     }
     return FAR_OK;
+}
+
+int far_frontend_process_sweep(far_frontend_t* f, const float* d_scan, const float* d_time, int64_t n, int stride, double dt_ref,
+                               const far_motion_t* motion, const far_pose_t* init_pose, double sigma, far_gicp_result_t* d_out,
+                               void* stream) {
+    if (!f || n < 0 || n > f->cfg.max_scan_points) return FAR_ERR_ARG;
+    const int rc = far_undistort(d_scan, d_time, n, stride, dt_ref, motion, f->d_undist, stream);
+    if (rc != FAR_OK) return rc;
+    return far_frontend_process(f, f->d_undist, n, 3, init_pose, sigma, d_out, stream);
 }
 
 int far_frontend_process_host(far_frontend_t* f, const float* h_scan, int64_t n, int stride, const far_pose_t* init_pose,

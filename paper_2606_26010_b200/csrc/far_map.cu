@@ -40,11 +40,37 @@ __device__ __forceinline__ bool load_pose_point(const float* __restrict__ xyz, i
     return true;
 }
 
+// ---- Adaptive Submap Density (R17) -----------------------------------------------------
+// per-voxel limit N_ASMD = clamp(floor(n_close (1 - d/d_max) + 0.5), k_cov, cap), d = distance of the voxel centre
+// from the current pose; every operation one rounded binary64 operation so that the integer it decides is the
+// oracle's.  `on == 0`: the fixed cap (plain far_map_insert).
+struct Asmd {
+    const double* d_n_close;   // device: mean points per voxel near the scan (far_asmd_density)
+    double d_max;
+    int on;
+};
+
+__device__ __forceinline__ uint32_t voxel_limit(const MapView& m, const Asmd& A, const int k[3], int pose_mode, const Pose& T) {
+    if (!A.on) return (uint32_t)m.cap;
+    const double v = (double)m.voxel;
+    const double cx = pose_mode ? T.t[0] : 0.0, cy = pose_mode ? T.t[1] : 0.0, cz = pose_mode ? T.t[2] : 0.0;
+    const double dx = __dadd_rn(__dmul_rn(__dadd_rn((double)k[0], 0.5), v), -cx);
+    const double dy = __dadd_rn(__dmul_rn(__dadd_rn((double)k[1], 0.5), v), -cy);
+    const double dz = __dadd_rn(__dmul_rn(__dadd_rn((double)k[2], 0.5), v), -cz);
+    const double d = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz)));
+    const double f = __dadd_rn(1.0, -__ddiv_rn(d, A.d_max));
+    const double x = floor(__dadd_rn(__dmul_rn(__ldg(A.d_n_close), f), 0.5));
+    const double lo = (double)m.k_cov, hi = (double)m.cap;
+    uint32_t lim = (uint32_t)m.k_cov;
+    if (x > lo) lim = (x >= hi) ? (uint32_t)m.cap : (uint32_t)x;
+    return min(lim, (uint32_t)m.cap);
+}
+
 // ---- insert, kernel 1: key -> find-or-claim -> atomicMin chain ---------------------------------------
 __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, const float* __restrict__ xyz, int64_t n,
                                                                   int stride, int pose_mode, Pose hpose,
                                                                   const Pose* __restrict__ d_pose, uint32_t first_id,
-                                                                  uint32_t* __restrict__ touched) {
+                                                                  uint32_t* __restrict__ touched, Asmd asmd) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const Pose& T = (pose_mode == 2) ? *d_pose : hpose;
@@ -79,9 +105,10 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
     }
     // count is only written by the commit kernel, so it is stable here: c0 = points stored before this chunk
     const uint32_t c0 = *reinterpret_cast<volatile uint32_t*>(&m.table[s].count);
-    const uint32_t cap = (uint32_t)m.cap;
+    // cap = this voxel's limit: the fixed cap, or N_ASMD (positions at and beyond it are never written)
+    const uint32_t cap = voxel_limit(m, asmd, k, pose_mode, T);
     if (c0 >= cap) return;
-    uint32_t* idw = reinterpret_cast<uint32_t*>(m.points + (size_t)s * cap) + 3;   // id word of position 0; stride 4
+    uint32_t* idw = reinterpret_cast<uint32_t*>(m.points + (size_t)s * (uint32_t)m.cap) + 3;   // id word of position 0; stride 4
     uint32_t x = first_id + (uint32_t)i;
     // ids at a position only ever decrease: if the last position already holds a smaller id, x cannot survive
     const uint32_t last = *reinterpret_cast<volatile uint32_t*>(idw + 4 * (cap - 1));
@@ -219,6 +246,36 @@ __global__ void prune_stats_kernel(MapView m, far_prune_stats_t* out) {
             out->n_points_left = (int64_t)m.ctr->pr_pts_left;
         }
         m.ctr->pr_vox_removed = m.ctr->pr_pts_removed = m.ctr->pr_vox_left = m.ctr->pr_pts_left = 0ull;
+    }
+}
+
+// ---- ASMD density (R17): integer sums over the live voxels near the centre, one division at the end --
+__global__ void __launch_bounds__(256) asmd_density_kernel(MapView m, double cx, double cy, double cz, double r2,
+                                                            unsigned long long* acc /* [2]: voxels, points */) {
+    const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned long long nv = 0, np = 0;
+    if (s < m.slots) {
+        const Entry e = m.table[s];
+        if (e.key != KEY_EMPTY && e.count > 0) {
+            int k[3];
+            unpack_key(e.key, k);
+            const double v = (double)m.voxel;
+            const double dx = __dadd_rn(__dmul_rn(__dadd_rn((double)k[0], 0.5), v), -cx);
+            const double dy = __dadd_rn(__dmul_rn(__dadd_rn((double)k[1], 0.5), v), -cy);
+            const double dz = __dadd_rn(__dmul_rn(__dadd_rn((double)k[2], 0.5), v), -cz);
+            const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+            if (d2 <= r2) { nv = 1; np = e.count; }
+        }
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) { nv += __shfl_xor_sync(FULL, nv, d); np += __shfl_xor_sync(FULL, np, d); }
+    if ((threadIdx.x & 31) == 0 && nv) { atomicAdd(&acc[0], nv); atomicAdd(&acc[1], np); }
+}
+
+__global__ void asmd_density_out_kernel(MapView m, const unsigned long long* acc, double* out) {
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        out[0] = acc[0] ? __ddiv_rn((double)acc[1], (double)acc[0]) : (double)m.cap;
+        out[1] = (double)acc[0];
     }
 }
 
@@ -446,7 +503,7 @@ int far_map_create(far_map_t** out, const far_map_config_t* cfg) {
         alloc((void**)&v.cov, npts * 6 * sizeof(float));
         alloc((void**)&v.cov_ok, npts);
     }
-    alloc((void**)&v.ctr, sizeof(Counters) + 4 * sizeof(unsigned long long));
+    alloc((void**)&v.ctr, sizeof(Counters) + 8 * sizeof(unsigned long long));
     alloc((void**)&m->d_touched, (size_t)c.max_batch * 4);
     alloc((void**)&m->d_cov_list, (size_t)c.max_batch * 4);
     if (e != cudaSuccess) {
@@ -458,7 +515,7 @@ int far_map_create(far_map_t** out, const far_map_config_t* cfg) {
     FAR_CUDA(cudaMemset(v.points, 0xFF, npts * sizeof(float4)));
     FAR_LAUNCH(table_init_kernel, grid_for((int64_t)slots, 256), 256, 0, 0, v.table, v.slots);
     FAR_CUDA(cudaGetLastError());
-    FAR_CUDA(cudaMemset(v.ctr, 0, sizeof(Counters) + 4 * sizeof(unsigned long long)));
+    FAR_CUDA(cudaMemset(v.ctr, 0, sizeof(Counters) + 8 * sizeof(unsigned long long)));
     if (v.cov_ok) FAR_CUDA(cudaMemset(v.cov_ok, 0, npts));
     {
         const int rc = gicp_setup(m);
@@ -489,7 +546,8 @@ int far_map_clear(far_map_t* m, void* stream) {
 }
 
 static int insert_impl(far_map_t* m, const float* d_xyz, int64_t n, int stride, int pose_mode, const far_pose_t* hpose,
-                       const far_pose_t* d_pose, int compute_cov, far_insert_stats_t* d_stats, void* stream) {
+                       const far_pose_t* d_pose, int compute_cov, far_insert_stats_t* d_stats, void* stream,
+                       Asmd asmd = Asmd{nullptr, 1.0, 0}) {
     if (!m || (!d_xyz && n > 0) || n < 0 || (stride != 3 && stride != 4)) return FAR_ERR_ARG;
     if (compute_cov && !m->view.cov) return FAR_ERR_ARG;
     if (m->next_id + (uint64_t)n > 0xFFFFFFFFull) return FAR_ERR_RANGE;
@@ -510,7 +568,7 @@ static int insert_impl(far_map_t* m, const float* d_xyz, int64_t n, int stride, 
         const float* xyz = d_xyz + off * stride;
         FAR_CUDA(cudaMemsetAsync(&ctr->n_touched, 0, sizeof(unsigned int), st));
         FAR_LAUNCH(insert_claim_chain_kernel, grid_for(nc, 256), 256, 0, st, m->view, xyz, nc, stride, pose_mode, hp,
-                                                                      (const Pose*)d_pose, first_id, m->d_touched);
+                                                                      (const Pose*)d_pose, first_id, m->d_touched, asmd);
         FAR_LAUNCH(insert_commit_kernel, commit_grid, 256, 0, st, m->view, xyz, stride, pose_mode, hp, (const Pose*)d_pose,
                                                            first_id, m->d_touched, cov_by_list ? m->d_cov_list : nullptr,
                                                            m->max_batch);
@@ -539,6 +597,32 @@ int far_map_insert_dev(far_map_t* m, const float* d_xyz, int64_t n, int stride, 
                        int compute_cov, far_insert_stats_t* d_stats, void* stream) {
     if (!d_pose) return FAR_ERR_ARG;
     return insert_impl(m, d_xyz, n, stride, 2, nullptr, d_pose, compute_cov, d_stats, stream);
+}
+
+int far_map_insert_asmd(far_map_t* m, const float* d_xyz, int64_t n, int stride, const far_pose_t* pose,
+                        const double* d_n_close, double d_max, int compute_cov, far_insert_stats_t* d_stats, void* stream) {
+    if (!d_n_close || !(d_max > 0.0)) return FAR_ERR_ARG;
+    return insert_impl(m, d_xyz, n, stride, pose ? 1 : 0, pose, nullptr, compute_cov, d_stats, stream, Asmd{d_n_close, d_max, 1});
+}
+
+int far_map_insert_asmd_dev(far_map_t* m, const float* d_xyz, int64_t n, int stride, const far_pose_t* d_pose,
+                            const double* d_n_close, double d_max, int compute_cov, far_insert_stats_t* d_stats,
+                            void* stream) {
+    if (!d_pose || !d_n_close || !(d_max > 0.0)) return FAR_ERR_ARG;
+    return insert_impl(m, d_xyz, n, stride, 2, nullptr, d_pose, compute_cov, d_stats, stream, Asmd{d_n_close, d_max, 1});
+}
+
+// PAPER.md:109 "the average amount of points per voxel in a close range of the current scan" (R17)
+int far_asmd_density(const far_map_t* local, const double center[3], double r_close, double* d_out, void* stream) {
+    if (!local || !center || !d_out || !(r_close >= 0.0)) return FAR_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned long long* acc = reinterpret_cast<unsigned long long*>(local->view.ctr + 1) + 4;   // 2 words of the tail
+    FAR_CUDA(cudaMemsetAsync(acc, 0, 2 * sizeof(unsigned long long), st));
+    FAR_LAUNCH(asmd_density_kernel, grid_for(local->view.slots, 256), 256, 0, st, local->view, center[0], center[1], center[2],
+                                                                        r_close * r_close, acc);
+    FAR_LAUNCH(asmd_density_out_kernel, 1, 32, 0, st, local->view, acc, d_out);
+    FAR_CUDA(cudaGetLastError());
+    return FAR_OK;
 }
 
 static int prune_impl(far_map_t* m, const double* c, const far_pose_t* d_pose, double radius, far_prune_stats_t* d_stats,

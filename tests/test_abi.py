@@ -51,7 +51,8 @@ def test_struct_sizes_match_header_layout():
     assert C.sizeof(far.GicpOptions) == 32
     assert C.sizeof(far.GicpResult) == 96 + 36 * 8 + 6 * 8 + 8 + 16
     assert C.sizeof(far.MapConfig) == 48
-    assert C.sizeof(far.FrontendConfig) == 48 + 8 + 8 + 8 + 8 + 32
+    assert C.sizeof(far.FrontendConfig) == 48 + 8 + 8 + 8 + 8 + 32 + 8 + 8 + 8
+    assert C.sizeof(far.Motion) == 96
 
 
 def test_default_options_are_the_papers():
@@ -83,6 +84,24 @@ def test_threshold_helper_matches_oracle_and_closed_form():
     s0 = a.sigma()
     a.update(pose_identity(), pose_from_rpy_t(0, 0, 0, [0.01, 0, 0]))
     assert a.sigma() == s0
+
+
+def test_motion_fit_helper_matches_oracle_and_polyfit():
+    """far_motion_fit is host-only FP64 boundary logic (R15): same line as the oracle's and NumPy's polyfit"""
+    import oracle
+    import paper_2606_26010_b200 as far
+    rng = np.random.default_rng(7)
+    t_ref = 50.0
+    times = t_ref - np.sort(rng.uniform(0, 0.25, 20))[::-1]
+    vel = rng.normal(0, 0.5, (20, 6)) + np.array([65.0, 0, 0, 0, 0, 0.3]) + np.outer(times - t_ref, [3, 0, 0, 0, 0, 1.0])
+    a, b = far.motion_fit(times, vel, t_ref)
+    ao, bo = oracle.motion_fit(times, vel, t_ref)
+    assert np.allclose(a, ao, rtol=1e-12, atol=1e-12) and np.allclose(b, bo, rtol=1e-10, atol=1e-10)
+    for c in range(6):
+        slope, icpt = np.polyfit(times - t_ref, vel[:, c], 1)
+        assert abs(b[c] - slope) < 1e-8 and abs(a[c] - icpt) < 1e-9
+    a, b = far.motion_fit(times[:1], vel[:1], t_ref)
+    assert np.array_equal(b, np.zeros(6)) and np.allclose(a, vel[0])
 
 
 def test_compute_calls_fail_loudly_without_a_gpu():
