@@ -378,6 +378,24 @@ def run_far(args):
                             "algorithmic_GBps": len(c2["map_points"]) * 40 / t_ins / 1e9,
                             "note": "1.52 M points in one call into an empty v=1.0 cap-20 map, no covariances"}
         mp.close()
+        # motion undistortion: 8 M points of racing-shaped sweeps, 28 B algorithmic per point (12 + 4 in, 12 out)
+        nu = 8_000_000
+        gen = torch.Generator(device="cuda").manual_seed(0)
+        up = (torch.rand((nu, 3), device="cuda", generator=gen) - 0.5) * 300.0
+        ut = torch.rand(nu, device="cuda", generator=gen) * 0.1
+        uo = torch.empty((nu, 3), dtype=torch.float32, device="cuda")
+        ua, ub = [69.4, 0.3, -0.1, 0.01, -0.02, 0.25], [-4.0, 0.5, 0.0, 0.0, 0.0, 0.6]
+        ts = []
+        for i in range(8):
+            flush.fill_(i)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); far.undistort(up, ut, 0.1, ua, ub, out=uo); b.record(); torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        t_u = float(np.median(ts[3:])) * 1e-3
+        extras["undistort"] = {"points": nu, "points_per_s": nu / t_u, "ms": t_u * 1e3, "algorithmic_GBps": nu * 28 / t_u / 1e9,
+                               "frac_of_hbm_peak": nu * 28 / t_u / 1e9 / peak,
+                               "note": "8 M points in one call (224 MB > L2), FP64 arithmetic, 256 MB flush between repetitions"}
+        del up, ut, uo
 
     # ---- CPU baseline: the oracle, as it stands, on this box's host cores ---------------------------------
     cpu = None
