@@ -129,14 +129,26 @@ __device__ __forceinline__ Entry load_entry(const Entry* table, uint32_t s) {
     return e;
 }
 
-// read-only lookup: slot of `key` and its count, or count = 0 if absent / dead
+// read-only lookup: slot of `key` and its count, or count = 0 if absent / dead.  Linear probing is
+// sequential by definition, but the next slots are known in advance: four consecutive entries are requested at once
+// and examined in probe order, so a lookup costs ONE memory round trip unless its probe sequence is longer than four
+// (the dependent chain of single-slot probes was the longest stall of the 27-voxel search: the warp waits for the
+// slowest of its 27 lookups).
 __device__ __forceinline__ uint32_t find_voxel(const MapView& m, unsigned long long key, uint32_t& count) {
     uint32_t s = hash_key(key) & m.mask;
-    for (uint32_t probes = 0; probes < m.slots; ++probes) {
-        const Entry e = load_entry(m.table, s);
-        if (e.key == key) { count = e.count; return s; }
-        if (e.key == KEY_EMPTY) break;
-        s = (s + 1) & m.mask;
+    for (uint32_t probes = 0; probes < m.slots; probes += 4) {
+        const uint32_t s1 = (s + 1) & m.mask, s2 = (s + 2) & m.mask, s3 = (s + 3) & m.mask;
+        const Entry e0 = load_entry(m.table, s), e1 = load_entry(m.table, s1), e2 = load_entry(m.table, s2),
+                    e3 = load_entry(m.table, s3);
+        if (e0.key == key) { count = e0.count; return s; }
+        if (e0.key == KEY_EMPTY) break;
+        if (e1.key == key) { count = e1.count; return s1; }
+        if (e1.key == KEY_EMPTY) break;
+        if (e2.key == key) { count = e2.count; return s2; }
+        if (e2.key == KEY_EMPTY) break;
+        if (e3.key == key) { count = e3.count; return s3; }
+        if (e3.key == KEY_EMPTY) break;
+        s = (s + 4) & m.mask;
     }
     count = 0;
     return NO_SLOT;
@@ -187,28 +199,51 @@ __device__ __forceinline__ void probe27_regs(const MapView& m, const int k[3], i
     }
 }
 
-// publishes per-lane counts as an exclusive prefix: s_off[0..27], s_slot[0..26]; returns the total
-__device__ __forceinline__ int publish_prefix(uint32_t cnt, uint32_t slot, int lane, int* s_off, uint32_t* s_slot) {
+// ---- the flattened candidate list of one query ---------------------------------------------------------------------
+// The warp sweeps the points of the voxels that matter as ONE list, 32 consecutive candidates per step, so lanes never
+// idle on half-empty voxels.  Per warp in shared memory: the occupied voxels in compact form (slot, first candidate
+// index) and, for every 32-candidate step, a bit mask of the positions where a new voxel starts.  Candidate j of step c
+// then belongs to compact voxel (#starts in earlier steps) + popc(mask_c & lanes <= mine) - 1: two LDS and a popc
+// instead of a per-lane walk over the prefix array.
+constexpr int CAND_STEPS = 27 * 64 / 32;    // cap <= 64
+struct __align__(16) CandList {
+    int off[32];                 // first candidate index of compact voxel c
+    uint32_t slot[32];           // its table slot
+    uint32_t mask[CAND_STEPS];   // voxel-start bits of step c
+};
+
+// all 32 lanes call; lane l < 27 passes the count (0 = skip) and slot of neighbour voxel l; returns the total
+__device__ __forceinline__ int cand_build(CandList& L, uint32_t cnt, uint32_t slot, int lane) {
     const int incl = warp_incl_scan((int)cnt, lane);
-    if (lane < 27) {
-        s_off[lane + 1] = incl;
-        s_slot[lane] = slot;
-    }
-    if (lane == 0) s_off[0] = 0;
+    const int total = __shfl_sync(FULL, incl, 31);
+    const unsigned occ = __ballot_sync(FULL, cnt > 0);
+    const int steps = (total + 31) >> 5;
+    for (int c = lane; c < steps; c += 32) L.mask[c] = 0u;
     __syncwarp();
-    return __shfl_sync(FULL, incl, 31);
+    if (cnt > 0) {
+        const int excl = incl - (int)cnt;
+        const int ci = __popc(occ & ((1u << lane) - 1u));
+        L.off[ci] = excl;
+        L.slot[ci] = slot;
+        atomicOr(&L.mask[excl >> 5], 1u << (excl & 31));
+    }
+    __syncwarp();
+    return total;
 }
 
-__device__ __forceinline__ int probe27(const MapView& m, const int k[3], int lane, int* s_off, uint32_t* s_slot) {
+// iteration state of one lane over the list: call cand_next once per 32-candidate step, in order
+struct CandIter { int before; };   // voxel starts in earlier steps
+__device__ __forceinline__ uint32_t cand_next(const CandList& L, CandIter& it, int step, int j, int lane, int cap) {
+    const uint32_t mk = L.mask[step];
+    const int v = it.before + __popc(mk & (0xFFFFFFFFu >> (31 - lane))) - 1;
+    it.before += __popc(mk);
+    return L.slot[v] * (uint32_t)cap + (uint32_t)(j - L.off[v]);
+}
+
+__device__ __forceinline__ int probe27(const MapView& m, const int k[3], int lane, CandList& L) {
     uint32_t cnt, slot;
     probe27_regs(m, k, lane, cnt, slot);
-    return publish_prefix(cnt, slot, lane, s_off, s_slot);
-}
-
-// map flat candidate j -> (voxel v, position) with a monotone walk over the prefix array
-__device__ __forceinline__ uint32_t cand_ref(const int* s_off, const uint32_t* s_slot, int j, int& v, int cap) {
-    while (j >= s_off[v + 1]) ++v;
-    return s_slot[v] * (uint32_t)cap + (uint32_t)(j - s_off[v]);
+    return cand_build(L, cnt, slot, lane);
 }
 
 // warp-wide minimum of a non-negative double (its bit pattern orders like its value): two redux.sync steps
@@ -247,7 +282,7 @@ __device__ __forceinline__ double voxel_lower_bound(float qx, float qy, float qz
 // (a skipped voxel holds only points strictly farther than the current best, so it cannot change the result,
 // ties included).  The surviving voxels are swept as ONE flattened candidate list, 32 float4 per step.
 __device__ __forceinline__ Best warp_nearest(const MapView& m, float qx, float qy, float qz, const int k[3], int lane,
-                                             int* s_off, uint32_t* s_slot, float& rx, float& ry, float& rz) {
+                                             CandList& L, float& rx, float& ry, float& rz) {
     uint32_t cnt, slot;
     probe27_regs(m, k, lane, cnt, slot);
     Best best;
@@ -269,10 +304,11 @@ __device__ __forceinline__ Best warp_nearest(const MapView& m, float qx, float q
         const double lb = voxel_lower_bound(qx, qy, qz, k, m.voxel, lane / 9 - 1, (lane / 3) % 3 - 1, lane % 3 - 1);
         if (lb <= bound) c2 = cnt;
     }
-    const int total = publish_prefix(c2, slot, lane, s_off, s_slot);
-    int v = 0;
-    for (int j = lane; j < total; j += 32) {
-        const uint32_t ref = cand_ref(s_off, s_slot, j, v, m.cap);
+    const int total = cand_build(L, c2, slot, lane);
+    CandIter ci;
+    ci.before = 0;
+    for (int j = lane, step = 0; j < total; j += 32, ++step) {
+        const uint32_t ref = cand_next(L, ci, step, j, lane, m.cap);
         const float4 p = __ldg(m.points + ref);
         const double d2 = dist2(qx, qy, qz, p.x, p.y, p.z);
         const uint32_t id = __float_as_uint(p.w);

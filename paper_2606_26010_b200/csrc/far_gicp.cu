@@ -337,8 +337,7 @@ __device__ __forceinline__ double block_sum_tagged(const uint4* rows, int first,
 }
 
 __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(MapView m, GicpParams P) {
-    __shared__ int s_off[GWARPS][32];
-    __shared__ uint32_t s_slot[GWARPS][32];
+    __shared__ CandList s_list[GWARPS];
     __shared__ double s_terms[GWARPS][TSTRIDE];
     __shared__ double s_red[GWARPS][TSTRIDE];
     __shared__ Corr s_corr[GWARPS];
@@ -360,6 +359,22 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(M
     const bool have_scan_cov = P.cov6 != nullptr && P.valid != nullptr && m.cov != nullptr;
     const int rounds = (int)((n + nwarps - 1) / nwarps);      // source points per warp (1 when n <= resident warps)
 
+    // one source point per warp (n <= resident warps, the usual case): the point, its covariance and flag are the same
+    // in every iteration, so they are fetched once and stay in registers -- one memory level less per iteration
+    const bool resident = rounds == 1;
+    float sx0 = 0.f, sy0 = 0.f, sz0 = 0.f, cin0 = 0.f;
+    if (resident) {
+        const int64_t i = (int64_t)blockIdx.x * GWARPS + wib;
+        if (i < n) {
+            const float* sp = P.scan + i * P.stride;
+            sx0 = __ldg(sp); sy0 = __ldg(sp + 1); sz0 = __ldg(sp + 2);
+            if (have_scan_cov) {
+                if (lane >= 8 && lane < 14) cin0 = __ldg(P.cov6 + 6 * i + (lane - 8));
+                if (lane == 14) cin0 = (float)__ldg(P.valid + i);
+            }
+        }
+    }
+
     for (int it = 0; it < P.max_iters; ++it) {
         const uint32_t tag = (P.seq << 10) | (uint32_t)(it + 1);
         TRACE_MIN(it, 0);
@@ -369,22 +384,24 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(M
             const int64_t i = (int64_t)rd * nwarps + (int64_t)blockIdx.x * GWARPS + wib;
             int flags = 0;
             if (i < n) {
-                const float* sp = P.scan + i * P.stride;
-                const float sx = __ldg(sp), sy = __ldg(sp + 1), sz = __ldg(sp + 2);
-                float pf[3];
-                int k[3];
-                if (isfinite(sx) && isfinite(sy) && isfinite(sz)) {
+                float sx = sx0, sy = sy0, sz = sz0, cin = cin0;
+                if (!resident) {
+                    const float* sp = P.scan + i * P.stride;
+                    sx = __ldg(sp); sy = __ldg(sp + 1); sz = __ldg(sp + 2);
                     // the source covariance does not depend on the search: lanes 8..13 fetch it now, lane 14 its flag
-                    float cin = 0.f;
                     if (have_scan_cov) {
                         if (lane >= 8 && lane < 14) cin = __ldg(P.cov6 + 6 * i + (lane - 8));
                         if (lane == 14) cin = (float)__ldg(P.valid + i);
                     }
+                }
+                float pf[3];
+                int k[3];
+                if (isfinite(sx) && isfinite(sy) && isfinite(sz)) {
                     transform_point(s_T, sx, sy, sz, pf);             // Eq. 2 with the accumulated pose (R11)
                     if (voxel_index(pf[0], pf[1], pf[2], m.voxel, k)) {
                         // kNN-search, k = 1
                         float rx, ry, rz;
-                        const Best best = warp_nearest(m, pf[0], pf[1], pf[2], k, lane, s_off[wib], s_slot[wib], rx, ry, rz);
+                        const Best best = warp_nearest(m, pf[0], pf[1], pf[2], k, lane, s_list[wib], rx, ry, rz);
                         if (best.id != NO_ID && !(best.d2 > P.tau2)) {    // adaptive-threshold gate
                             // lanes 0..5 fetch Sigma_r, lane 6 its flag: one memory level
                             if (have_scan_cov) {

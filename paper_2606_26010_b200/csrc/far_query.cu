@@ -19,8 +19,7 @@ constexpr int QWARPS = 8;   // warps (= queries in flight) per block
 
 __global__ void __launch_bounds__(QWARPS * 32) nn_kernel(MapView m, const float* __restrict__ q, int64_t n, int stride,
                                                           uint32_t* __restrict__ out_id, float* __restrict__ out_d2) {
-    __shared__ int s_off[QWARPS][32];
-    __shared__ uint32_t s_slot[QWARPS][32];
+    __shared__ CandList s_list[QWARPS];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const int64_t nwarps = (int64_t)gridDim.x * QWARPS;
     for (int64_t i = (int64_t)blockIdx.x * QWARPS + wib; i < n; i += nwarps) {
@@ -31,7 +30,7 @@ __global__ void __launch_bounds__(QWARPS * 32) nn_kernel(MapView m, const float*
         float d2 = __int_as_float(0x7F800000);
         if (voxel_index(qx, qy, qz, m.voxel, k)) {
             float rx, ry, rz;
-            const Best b = warp_nearest(m, qx, qy, qz, k, lane, s_off[wib], s_slot[wib], rx, ry, rz);
+            const Best b = warp_nearest(m, qx, qy, qz, k, lane, s_list[wib], rx, ry, rz);
             if (b.id != NO_ID) { id = b.id; d2 = __double2float_rn(b.d2); }
         }
         if (lane == 0) { out_id[i] = id; out_d2[i] = d2; }
@@ -41,15 +40,14 @@ __global__ void __launch_bounds__(QWARPS * 32) nn_kernel(MapView m, const float*
 
 __global__ void __launch_bounds__(QWARPS * 32) count27_kernel(MapView m, const float* __restrict__ q, int64_t n, int stride,
                                                                int32_t* __restrict__ out) {
-    __shared__ int s_off[QWARPS][32];
-    __shared__ uint32_t s_slot[QWARPS][32];
+    __shared__ CandList s_list[QWARPS];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const int64_t nwarps = (int64_t)gridDim.x * QWARPS;
     for (int64_t i = (int64_t)blockIdx.x * QWARPS + wib; i < n; i += nwarps) {
         const float* qq = q + i * stride;
         int k[3];
         int total = 0;
-        if (voxel_index(__ldg(qq), __ldg(qq + 1), __ldg(qq + 2), m.voxel, k)) total = probe27(m, k, lane, s_off[wib], s_slot[wib]);
+        if (voxel_index(__ldg(qq), __ldg(qq + 1), __ldg(qq + 2), m.voxel, k)) total = probe27(m, k, lane, s_list[wib]);
         if (lane == 0) out[i] = total;
         __syncwarp();
     }
@@ -66,7 +64,7 @@ struct __align__(16) Cand {
     uint32_t ref;
 };
 
-__host__ __device__ inline size_t knn_smem_per_warp(int k) { return (size_t)32 * k * sizeof(Cand) + 2 * 32 * 4; }
+__host__ __device__ inline size_t knn_smem_per_warp(int k) { return (size_t)32 * k * sizeof(Cand) + sizeof(CandList); }
 
 __device__ __forceinline__ bool cand_less(double d2, uint32_t id, const Cand& c) {
     return d2 < c.d2 || (d2 == c.d2 && id < c.id);
@@ -94,18 +92,19 @@ __device__ __forceinline__ bool warp_knn_cov(const MapView& m, float qx, float q
                                              float cov[6]) {
     const int cap = m.cap, kk = m.k_cov;
     Cand* col = reinterpret_cast<Cand*>(smem_w);                 // col[r * 32 + lane] = r-th smallest of this lane
-    int* s_off = reinterpret_cast<int*>(smem_w + (size_t)32 * kk * sizeof(Cand));
-    uint32_t* s_slot = reinterpret_cast<uint32_t*>(s_off + 32);
+    CandList& L = *reinterpret_cast<CandList*>(smem_w + (size_t)32 * kk * sizeof(Cand));
     cov[0] = 1.f; cov[1] = 0.f; cov[2] = 0.f; cov[3] = 1.f; cov[4] = 0.f; cov[5] = 1.f;
     int k[3];
     if (!voxel_index(qx, qy, qz, m.voxel, k)) return false;
-    const int total = probe27(m, k, lane, s_off, s_slot);
+    const int total = probe27(m, k, lane, L);
     if (total < kk) { __syncwarp(); return false; }
     const double INF = __longlong_as_double(0x7FF0000000000000ll);
     const double dqx = (double)qx, dqy = (double)qy, dqz = (double)qz;
-    int cnt = 0, v = 0;
-    for (int j = lane; j < total; j += 32) {
-        const uint32_t ref = cand_ref(s_off, s_slot, j, v, cap);
+    int cnt = 0;
+    CandIter ci;
+    ci.before = 0;
+    for (int j = lane, step = 0; j < total; j += 32, ++step) {
+        const uint32_t ref = cand_next(L, ci, step, j, lane, cap);
         const float4 p = __ldg(m.points + ref);
         const double dx = dqx - (double)p.x, dy = dqy - (double)p.y, dz = dqz - (double)p.z;
         const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));   // R6
