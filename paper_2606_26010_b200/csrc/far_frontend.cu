@@ -24,6 +24,8 @@ struct far_frontend {
     uint8_t* d_valid;
     far_pose_t* d_init;
     far_gicp_result_t* d_result;
+    cudaStream_t side;       // second stream: the downsampling branch runs beside the scan-local map build
+    cudaEvent_t ev_fork, ev_join;
     double* d_asmd;          // [2] n_close, number of close voxels (far_asmd_density)
     float* d_undist;         // undistorted sweep [max_scan_points * 3] (far_frontend_process_sweep)
 };
@@ -34,6 +36,9 @@ int far_frontend_destroy(far_frontend_t* f) {
     if (!f) return FAR_OK;
     far_map_destroy(f->map);
     far_map_destroy(f->local);
+    if (f->ev_fork) cudaEventDestroy(f->ev_fork);
+    if (f->ev_join) cudaEventDestroy(f->ev_join);
+    if (f->side) cudaStreamDestroy(f->side);
     cudaFree(f->d_ws); cudaFree(f->d_scan); cudaFree(f->d_ds_xyz); cudaFree(f->d_ds_index); cudaFree(f->d_n_ds);
     cudaFree(f->d_cov6); cudaFree(f->d_valid); cudaFree(f->d_init); cudaFree(f->d_result); cudaFree(f->d_asmd); cudaFree(f->d_undist);
     delete f;
@@ -78,6 +83,9 @@ int far_frontend_create(far_frontend_t** out, const far_frontend_config_t* cfg) 
     alloc((void**)&f->d_result, sizeof(far_gicp_result_t));
     alloc((void**)&f->d_asmd, 2 * sizeof(double));
     alloc((void**)&f->d_undist, (size_t)n * 3 * sizeof(float));
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&f->side, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&f->ev_fork, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&f->ev_join, cudaEventDisableTiming);
     if (rc != FAR_OK || e != cudaSuccess) {
         if (e != cudaSuccess) far::set_cuda_error(e, "cudaMalloc in far_frontend_create");
         far_frontend_destroy(f);
@@ -96,12 +104,17 @@ int far_frontend_process(far_frontend_t* f, const float* d_scan, int64_t n, int 
     cudaStream_t st = (cudaStream_t)stream;
     far_gicp_result_t* res = d_out ? d_out : f->d_result;
     int rc;
-    // A1/A2: downsample
+    // A1/A2 downsampling and the scan-local map are independent until Cov-Calc needs both: fork the downsampling onto
+    // the side stream, build the local map on the caller's stream, join before far_map_knn_cov (still no host sync)
+    FAR_CUDA(cudaEventRecord(f->ev_fork, st));
+    FAR_CUDA(cudaStreamWaitEvent(f->side, f->ev_fork, 0));
     size_t ws = f->ws_bytes;
-    if ((rc = far_voxelize(d_scan, n, stride, f->cfg.ds_voxel, f->d_ds_xyz, f->d_ds_index, f->d_n_ds, f->d_ws, &ws, stream))) return rc;
+    if ((rc = far_voxelize(d_scan, n, stride, f->cfg.ds_voxel, f->d_ds_xyz, f->d_ds_index, f->d_n_ds, f->d_ws, &ws, (void*)f->side))) return rc;
+    FAR_CUDA(cudaEventRecord(f->ev_join, f->side));
     // A7: Sigma_s from a scan-local map of the raw scan
     if ((rc = far_map_clear(f->local, stream))) return rc;
     if ((rc = far_map_insert(f->local, d_scan, n, stride, nullptr, 0, nullptr, stream))) return rc;
+    FAR_CUDA(cudaStreamWaitEvent(st, f->ev_join, 0));
     if (n > 0 && (rc = far_map_knn_cov_dev(f->local, f->d_ds_xyz, f->d_n_ds, n, 3, f->d_cov6, f->d_valid, stream))) return rc;
     // A6, A8-A10: registration from the predicted pose
     FAR_CUDA(cudaMemcpyAsync(f->d_init, init_pose, sizeof(far_pose_t), cudaMemcpyHostToDevice, st));

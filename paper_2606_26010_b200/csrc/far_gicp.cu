@@ -49,6 +49,13 @@ struct GicpScratch {
     uint4* pub;       // [16]
 };
 
+// one transformed source point, written by one lane of warp 0 in phase A0, read by its warp in phase A
+struct Src {
+    float p[3];       // T s (Eq. 2)
+    int k[3];         // its voxel index
+    int ok;           // 0: no point / non-finite / outside the key range
+};
+
 // one correspondence, written by its warp in phase A, read by one lane of warp 0 in phase B
 struct Corr {
     float p[3];       // transformed source point
@@ -341,6 +348,7 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(M
     __shared__ double s_terms[GWARPS][TSTRIDE];
     __shared__ double s_red[GWARPS][TSTRIDE];
     __shared__ Corr s_corr[GWARPS];
+    __shared__ Src s_src[GWARPS];
     __shared__ Pose s_T;
     __shared__ int s_done;
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
@@ -360,18 +368,23 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(M
     const int rounds = (int)((n + nwarps - 1) / nwarps);      // source points per warp (1 when n <= resident warps)
 
     // one source point per warp (n <= resident warps, the usual case): the point, its covariance and flag are the same
-    // in every iteration, so they are fetched once and stay in registers -- one memory level less per iteration
+    // in every iteration, so they are fetched once and stay in registers -- one memory level less per iteration.
+    // Lane l < 8 of warp 0 holds the point of warp l (phase A0), lanes 8..14 of every warp its own covariance and flag.
     const bool resident = rounds == 1;
     float sx0 = 0.f, sy0 = 0.f, sz0 = 0.f, cin0 = 0.f;
     if (resident) {
-        const int64_t i = (int64_t)blockIdx.x * GWARPS + wib;
-        if (i < n) {
-            const float* sp = P.scan + i * P.stride;
-            sx0 = __ldg(sp); sy0 = __ldg(sp + 1); sz0 = __ldg(sp + 2);
-            if (have_scan_cov) {
-                if (lane >= 8 && lane < 14) cin0 = __ldg(P.cov6 + 6 * i + (lane - 8));
-                if (lane == 14) cin0 = (float)__ldg(P.valid + i);
+        if (wib == 0 && lane < GWARPS) {
+            const int64_t i = (int64_t)blockIdx.x * GWARPS + lane;
+            sx0 = sy0 = sz0 = __int_as_float(0x7FC00000);     // NaN: no point
+            if (i < n) {
+                const float* sp = P.scan + i * P.stride;
+                sx0 = __ldg(sp); sy0 = __ldg(sp + 1); sz0 = __ldg(sp + 2);
             }
+        }
+        const int64_t i = (int64_t)blockIdx.x * GWARPS + wib;
+        if (i < n && have_scan_cov) {
+            if (lane >= 8 && lane < 14) cin0 = __ldg(P.cov6 + 6 * i + (lane - 8));
+            if (lane == 14) cin0 = (float)__ldg(P.valid + i);
         }
     }
 
@@ -380,25 +393,44 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(M
         TRACE_MIN(it, 0);
         double acc = 0.0;                                     // warp 0, lane t < 29: term t of this block
         for (int rd = 0; rd < rounds; ++rd) {
+            // ---- phase A0 (Eq. 2, A1): 8 lanes of warp 0 transform the block's 8 source points with the accumulated pose
+            // (R11) and take their voxel indices: one instruction stream for 8 points instead of 8 redundant warps ------
+            if (wib == 0 && lane < GWARPS) {
+                float sx = sx0, sy = sy0, sz = sz0;
+                if (!resident) {
+                    const int64_t i = (int64_t)rd * nwarps + (int64_t)blockIdx.x * GWARPS + lane;
+                    sx = sy = sz = __int_as_float(0x7FC00000);
+                    if (i < n) {
+                        const float* sp = P.scan + i * P.stride;
+                        sx = __ldg(sp); sy = __ldg(sp + 1); sz = __ldg(sp + 2);
+                    }
+                }
+                Src o;
+                o.ok = 0;
+                o.p[0] = o.p[1] = o.p[2] = 0.f;
+                o.k[0] = o.k[1] = o.k[2] = 0;
+                if (isfinite(sx) && isfinite(sy) && isfinite(sz)) {
+                    transform_point(s_T, sx, sy, sz, o.p);
+                    o.ok = voxel_index(o.p[0], o.p[1], o.p[2], m.voxel, o.k) ? 1 : 0;
+                }
+                s_src[lane] = o;
+            }
+            __syncthreads();
             // ---- phase A (A8): one warp per source point -> correspondence record ---------------------------------
             const int64_t i = (int64_t)rd * nwarps + (int64_t)blockIdx.x * GWARPS + wib;
             int flags = 0;
             if (i < n) {
-                float sx = sx0, sy = sy0, sz = sz0, cin = cin0;
-                if (!resident) {
-                    const float* sp = P.scan + i * P.stride;
-                    sx = __ldg(sp); sy = __ldg(sp + 1); sz = __ldg(sp + 2);
+                float cin = cin0;
+                if (!resident && have_scan_cov) {
                     // the source covariance does not depend on the search: lanes 8..13 fetch it now, lane 14 its flag
-                    if (have_scan_cov) {
-                        if (lane >= 8 && lane < 14) cin = __ldg(P.cov6 + 6 * i + (lane - 8));
-                        if (lane == 14) cin = (float)__ldg(P.valid + i);
-                    }
+                    if (lane >= 8 && lane < 14) cin = __ldg(P.cov6 + 6 * i + (lane - 8));
+                    if (lane == 14) cin = (float)__ldg(P.valid + i);
                 }
-                float pf[3];
-                int k[3];
-                if (isfinite(sx) && isfinite(sy) && isfinite(sz)) {
-                    transform_point(s_T, sx, sy, sz, pf);             // Eq. 2 with the accumulated pose (R11)
-                    if (voxel_index(pf[0], pf[1], pf[2], m.voxel, k)) {
+                const Src src = s_src[wib];
+                const float pf[3] = {src.p[0], src.p[1], src.p[2]};
+                const int k[3] = {src.k[0], src.k[1], src.k[2]};
+                {
+                    if (src.ok) {
                         // kNN-search, k = 1
                         float rx, ry, rz;
                         const Best best = warp_nearest(m, pf[0], pf[1], pf[2], k, lane, s_list[wib], rx, ry, rz);
@@ -420,6 +452,7 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(M
             }
             if (lane == 0) s_corr[wib].flags = flags;
             __syncthreads();
+            TRACE_MAX(it, 2);
             // ---- phase B (A9): 8 lanes of warp 0 linearise the block's 8 correspondences together --------------------
             if (wib == 0) {
                 if (lane < GWARPS) {
