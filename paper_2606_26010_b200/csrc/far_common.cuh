@@ -165,8 +165,8 @@ __device__ __forceinline__ bool better(double d2, uint32_t id, const Best& b) {
     return d2 < b.d2 || (d2 == b.d2 && id < b.id);
 }
 
-// warp arg-min over (d2, id): three redux.sync steps on the 64-bit pattern halves and the id; returns the lane
-// holding the winner (lanes with no candidate carry d2 = +inf, id = NO_ID)
+// warp arg-min over (d2, id): redux.sync steps on the 64-bit pattern halves, and on the id only if two lanes tie on
+// d2 (rare); returns the lane holding the winner (lanes with no candidate carry d2 = +inf, id = NO_ID)
 __device__ __forceinline__ int warp_argmin(double d2, uint32_t id) {
     const unsigned long long bits = (unsigned long long)__double_as_longlong(d2);
     const uint32_t hi = (uint32_t)(bits >> 32), lo = (uint32_t)bits;
@@ -174,9 +174,12 @@ __device__ __forceinline__ int warp_argmin(double d2, uint32_t id) {
     bool c = hi == mhi;
     const uint32_t mlo = __reduce_min_sync(FULL, c ? lo : 0xFFFFFFFFu);
     c = c && lo == mlo;
-    const uint32_t mid = __reduce_min_sync(FULL, c ? id : 0xFFFFFFFFu);
-    c = c && id == mid;
-    const unsigned b = __ballot_sync(FULL, c);
+    unsigned b = __ballot_sync(FULL, c);
+    if (b & (b - 1)) {      // more than one lane holds the minimal d2: lowest id wins (R6)
+        const uint32_t mid = __reduce_min_sync(FULL, c ? id : 0xFFFFFFFFu);
+        c = c && id == mid;
+        b = __ballot_sync(FULL, c);
+    }
     return __ffs(b) - 1;
 }
 

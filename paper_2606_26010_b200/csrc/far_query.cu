@@ -142,26 +142,38 @@ __device__ __forceinline__ bool warp_knn_cov(const MapView& m, float qx, float q
             else { head.d2 = INF; head.id = NO_ID; }
         }
     }
-    // lane r < k holds the r-th neighbour; mean and centred sums in neighbour order (R7: 1/k)
-    float px = 0.f, py = 0.f, pz = 0.f;
+    // lane r < k holds the r-th neighbour.  The neighbours go through shared memory (the candidate columns are no
+    // longer needed) so that the moments are computed once, not by 32 lanes in lockstep through shuffles: lane a < 3
+    // sums coordinate a in neighbour order (R7: 1/k), then lane a < 6 accumulates centred product a, also in order.
+    __syncwarp();
+    double* nb = reinterpret_cast<double*>(smem_w);          // [kk][3] positions, then [3] mean, then [6] moments
     if (lane < kk) {
         const float4 p = __ldg(m.points + myref);
-        px = p.x; py = p.y; pz = p.z;
+        nb[3 * lane] = (double)p.x; nb[3 * lane + 1] = (double)p.y; nb[3 * lane + 2] = (double)p.z;
     }
+    __syncwarp();
     const double inv_k = 1.0 / (double)kk;
-    double mx = 0.0, my = 0.0, mz = 0.0;
-    for (int r = 0; r < kk; ++r) {
-        mx += (double)__shfl_sync(FULL, px, r); my += (double)__shfl_sync(FULL, py, r); mz += (double)__shfl_sync(FULL, pz, r);
+    double* mean = nb + 3 * kk;
+    double* mom = mean + 3;
+    if (lane < 3) {
+        double sacc = 0.0;
+        for (int r = 0; r < kk; ++r) sacc += nb[3 * r + lane];
+        mean[lane] = sacc * inv_k;
     }
-    mx *= inv_k; my *= inv_k; mz *= inv_k;
-    double sc[6] = {0, 0, 0, 0, 0, 0};
-    for (int r = 0; r < kk; ++r) {
-        const double x = (double)__shfl_sync(FULL, px, r) - mx, y = (double)__shfl_sync(FULL, py, r) - my,
-                     z = (double)__shfl_sync(FULL, pz, r) - mz;
-        sc[0] += x * x; sc[1] += x * y; sc[2] += x * z; sc[3] += y * y; sc[4] += y * z; sc[5] += z * z;
+    __syncwarp();
+    if (lane < 6) {
+        // (xx,xy,xz,yy,yz,zz) -> axis pair (i,j)
+        const int i = lane < 3 ? 0 : (lane < 5 ? 1 : 2);
+        const int j = lane < 3 ? lane : (lane < 5 ? lane - 2 : 2);
+        const double mi = mean[i], mj = mean[j];
+        double sacc = 0.0;
+        for (int r = 0; r < kk; ++r) sacc += (nb[3 * r + i] - mi) * (nb[3 * r + j] - mj);
+        mom[lane] = sacc * inv_k;
     }
+    __syncwarp();
+    double sc[6];
 #pragma unroll
-    for (int a = 0; a < 6; ++a) sc[a] *= inv_k;
+    for (int a = 0; a < 6; ++a) sc[a] = mom[a];
     __syncwarp();
     float out[6];
     if (!regularised_cov(sc, m.cov_eps, out)) return false;
