@@ -125,7 +125,7 @@ int far_map_stats(far_map_t* map, far_map_stats_t* d_stats, void* stream);
 int far_map_rehash(far_map_t* map, void* stream);
 
 /* Checkpoint / restore of a map's whole device state (table, buckets, covariances, counters, id counter).
- * create allocates the copy (a maintenance call); restore is five stream-ordered device copies, no sync. */
+ * create allocates the copy (a maintenance call); restore is six stream-ordered device copies, no sync. */
 typedef struct far_snapshot far_snapshot_t;
 int far_map_snapshot_create(far_map_t* map, far_snapshot_t** out, void* stream);
 int far_map_snapshot_restore(far_map_t* map, const far_snapshot_t* snap, void* stream);

@@ -5,8 +5,12 @@
 //                                     AND the number of points, so a lookup is two dependent memory levels
 //                                     (entry -> points), not three.
 //   points  : float4[slots * cap]     bucket of slot s = points[s*cap .. s*cap+cap); .w = id bits.  The bucket
-//                                     index IS the slot index (no indirection, no allocator); unused positions
-//                                     hold id = FAR_NO_ID, which is what the deterministic insert relies on.
+//                                     index IS the slot index (no indirection, no allocator); positions >= count
+//                                     are never read.
+//   ids     : u32[slots * cap]        the id of stored point j of slot s at ids[s*cap + j], FAR_NO_ID if the position is
+//                                     free.  A compact copy of the .w words: it is the working storage of the
+//                                     deterministic insert, whose chain then touches 80 contiguous bytes (one to three
+//                                     32-byte sectors) per voxel instead of up to ten sectors of the float4 bucket.
 //   cov     : float[slots * cap * 6]  (optional) regularised covariance of each stored point (Eq. 1)
 //   cov_ok  : u8[slots * cap]         (optional) 1 if that covariance is valid (>= k neighbours)
 // A pruned voxel keeps its key with count = 0 ("dead key"): it behaves exactly like an absent voxel for every
@@ -46,6 +50,7 @@ struct Counters {
 struct MapView {
     Entry* table;
     float4* points;
+    uint32_t* ids;
     float* cov;          // nullable
     uint8_t* cov_ok;     // nullable
     Counters* ctr;

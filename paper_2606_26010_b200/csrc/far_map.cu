@@ -108,21 +108,21 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
     // cap = this voxel's limit: the fixed cap, or N_ASMD (positions at and beyond it are never written)
     const uint32_t cap = voxel_limit(m, asmd, k, pose_mode, T);
     if (c0 >= cap) return;
-    uint32_t* idw = reinterpret_cast<uint32_t*>(m.points + (size_t)s * (uint32_t)m.cap) + 3;   // id word of position 0; stride 4
+    uint32_t* idw = m.ids + (size_t)s * (uint32_t)m.cap;   // id word of position 0 (compact array)
     uint32_t x = first_id + (uint32_t)i;
     // ids at a position only ever decrease: if the last position already holds a smaller id, x cannot survive
-    const uint32_t last = *reinterpret_cast<volatile uint32_t*>(idw + 4 * (cap - 1));
+    const uint32_t last = *reinterpret_cast<volatile uint32_t*>(idw + (cap - 1));
     if (last < x) return;
     // The id words of a bucket are sorted at every instant and only ever decrease, so a position seen holding an
     // id < x will never take x: gallop over such positions with plain reads (4 independent loads per step)
     // instead of walking them with dependent atomics.  A stale read only makes the chain start earlier.
     uint32_t pos = c0;
     while (pos + 4 <= cap) {
-        const uint32_t a3 = *reinterpret_cast<volatile uint32_t*>(idw + 4 * (pos + 3));
+        const uint32_t a3 = *reinterpret_cast<volatile uint32_t*>(idw + (pos + 3));
         if (a3 < x) pos += 4; else break;
     }
     for (; pos < cap; ++pos) {
-        const uint32_t old = atomicMin(idw + 4 * pos, x);
+        const uint32_t old = atomicMin(idw + pos, x);
         if (old == NO_ID) {
             if (pos == c0) touched[atomicAdd(&m.ctr->n_touched, 1u)] = s;   // unique per voxel and chunk
             break;
@@ -150,7 +150,7 @@ __global__ void __launch_bounds__(256) insert_commit_kernel(MapView m, const flo
         for (uint32_t base = c0; base < cap; base += 32) {
             const uint32_t pos = base + lane;
             uint32_t id = NO_ID;
-            if (pos < cap) id = __float_as_uint(bucket[pos].w);
+            if (pos < cap) id = m.ids[(size_t)s * cap + pos];
             const bool is_new = id != NO_ID;
             if (is_new) {
                 float p[3];
@@ -205,9 +205,8 @@ __global__ void __launch_bounds__(256) prune_kernel(MapView m, double cx, double
             const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
             if (d2 > r2) {
                 // the key stays (dead key, count 0); its id words go back to +inf so a later insert starts clean
-                float4* bucket = m.points + (size_t)s * m.cap;
                 for (uint32_t j = 0; j < e.count; ++j) {
-                    bucket[j].w = __uint_as_float(NO_ID);
+                    m.ids[(size_t)s * m.cap + j] = NO_ID;
                     if (m.cov_ok) m.cov_ok[(size_t)s * m.cap + j] = 0;
                 }
                 m.table[s].count = 0;
@@ -285,8 +284,7 @@ __global__ void __launch_bounds__(256) clear_kernel(MapView m) {
     if (s >= m.slots) return;
     const Entry e = m.table[s];
     if (e.key == KEY_EMPTY) return;
-    float4* bucket = m.points + (size_t)s * m.cap;
-    for (uint32_t j = 0; j < e.count; ++j) bucket[j].w = __uint_as_float(NO_ID);
+    for (uint32_t j = 0; j < e.count; ++j) m.ids[(size_t)s * m.cap + j] = NO_ID;
     Entry z;
     z.key = KEY_EMPTY; z.count = 0; z.pad = 0;
     m.table[s] = z;
@@ -410,7 +408,7 @@ __global__ void __launch_bounds__(256) rehash_gather_kernel(MapView m, unsigned 
             }
         }
     }
-    for (uint32_t j = 0; j < e.count; ++j) bucket[j].w = __uint_as_float(NO_ID);
+    for (uint32_t j = 0; j < e.count; ++j) m.ids[(size_t)s * m.cap + j] = NO_ID;
     Entry z;
     z.key = KEY_EMPTY; z.count = 0; z.pad = 0;
     m.table[s] = z;
@@ -433,6 +431,7 @@ __global__ void __launch_bounds__(256) rehash_scatter_kernel(MapView m, const un
     for (uint32_t j = 0; j < cnt; ++j) {
         const size_t to = (size_t)s * m.cap + j, from = (size_t)r * m.cap + j;
         m.points[to] = pts[from];
+        m.ids[to] = __float_as_uint(pts[from].w);
         if (m.cov) {
             for (int a = 0; a < 6; ++a) m.cov[to * 6 + a] = cov6[from * 6 + a];
             m.cov_ok[to] = cov_ok[from];
@@ -499,6 +498,7 @@ int far_map_create(far_map_t** out, const far_map_config_t* cfg) {
     auto alloc = [&](void** p, size_t bytes) { if (e == cudaSuccess) e = cudaMalloc(p, bytes); };
     alloc((void**)&v.table, slots * sizeof(Entry));
     alloc((void**)&v.points, npts * sizeof(float4));
+    alloc((void**)&v.ids, npts * sizeof(uint32_t));
     if (c.with_cov) {
         alloc((void**)&v.cov, npts * 6 * sizeof(float));
         alloc((void**)&v.cov_ok, npts);
@@ -511,8 +511,8 @@ int far_map_create(far_map_t** out, const far_map_config_t* cfg) {
         far_map_destroy(m);
         return FAR_ERR_CUDA;
     }
-    // empty table: every key = ~0, count = 0; every id word = FAR_NO_ID (0xFF bytes everywhere in the pool)
-    FAR_CUDA(cudaMemset(v.points, 0xFF, npts * sizeof(float4)));
+    // empty table: every key = ~0, count = 0; every id word = FAR_NO_ID
+    FAR_CUDA(cudaMemset(v.ids, 0xFF, npts * sizeof(uint32_t)));
     FAR_LAUNCH(table_init_kernel, grid_for((int64_t)slots, 256), 256, 0, 0, v.table, v.slots);
     FAR_CUDA(cudaGetLastError());
     FAR_CUDA(cudaMemset(v.ctr, 0, sizeof(Counters) + 8 * sizeof(unsigned long long)));
@@ -528,7 +528,7 @@ int far_map_create(far_map_t** out, const far_map_config_t* cfg) {
 
 int far_map_destroy(far_map_t* m) {
     if (!m) return FAR_OK;
-    cudaFree(m->view.table); cudaFree(m->view.points); cudaFree(m->view.cov); cudaFree(m->view.cov_ok);
+    cudaFree(m->view.table); cudaFree(m->view.points); cudaFree(m->view.ids); cudaFree(m->view.cov); cudaFree(m->view.cov_ok);
     cudaFree(m->view.ctr); cudaFree(m->d_touched); cudaFree(m->d_cov_list);
     cudaFree(m->d_gicp_partials); cudaFree(m->d_gicp_state);
     delete m;
@@ -761,8 +761,8 @@ LaunchScope::~LaunchScope() {
 }  // namespace far
 
 struct far_snapshot {
-    void *table, *points, *cov, *cov_ok, *ctr;
-    size_t b_table, b_points, b_cov, b_ok;
+    void *table, *points, *ids, *cov, *cov_ok, *ctr;
+    size_t b_table, b_points, b_ids, b_cov, b_ok;
     uint64_t next_id;
 };
 
@@ -804,7 +804,7 @@ int far_profile_collect(const char** names, double* total_ms, long long* launche
 
 int far_map_snapshot_destroy(far_snapshot_t* s) {
     if (!s) return FAR_OK;
-    cudaFree(s->table); cudaFree(s->points); cudaFree(s->cov); cudaFree(s->cov_ok); cudaFree(s->ctr);
+    cudaFree(s->table); cudaFree(s->points); cudaFree(s->ids); cudaFree(s->cov); cudaFree(s->cov_ok); cudaFree(s->ctr);
     delete s;
     return FAR_OK;
 }
@@ -819,16 +819,19 @@ int far_map_snapshot_create(far_map_t* m, far_snapshot_t** out, void* stream) {
     const size_t npts = (size_t)m->view.slots * m->view.cap;
     s->b_table = (size_t)m->view.slots * sizeof(Entry);
     s->b_points = npts * sizeof(float4);
+    s->b_ids = npts * sizeof(uint32_t);
     s->b_cov = m->view.cov ? npts * 6 * sizeof(float) : 0;
     s->b_ok = m->view.cov_ok ? npts : 0;
     s->next_id = m->next_id;
     cudaError_t e = cudaMalloc(&s->table, s->b_table);
     if (e == cudaSuccess) e = cudaMalloc(&s->points, s->b_points);
+    if (e == cudaSuccess) e = cudaMalloc(&s->ids, s->b_ids);
     if (e == cudaSuccess && s->b_cov) e = cudaMalloc(&s->cov, s->b_cov);
     if (e == cudaSuccess && s->b_ok) e = cudaMalloc(&s->cov_ok, s->b_ok);
     if (e == cudaSuccess) e = cudaMalloc(&s->ctr, sizeof(Counters));
     if (e == cudaSuccess) e = cudaMemcpyAsync(s->table, m->view.table, s->b_table, cudaMemcpyDeviceToDevice, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(s->points, m->view.points, s->b_points, cudaMemcpyDeviceToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(s->ids, m->view.ids, s->b_ids, cudaMemcpyDeviceToDevice, st);
     if (e == cudaSuccess && s->b_cov) e = cudaMemcpyAsync(s->cov, m->view.cov, s->b_cov, cudaMemcpyDeviceToDevice, st);
     if (e == cudaSuccess && s->b_ok) e = cudaMemcpyAsync(s->cov_ok, m->view.cov_ok, s->b_ok, cudaMemcpyDeviceToDevice, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(s->ctr, m->view.ctr, sizeof(Counters), cudaMemcpyDeviceToDevice, st);
@@ -848,6 +851,7 @@ int far_map_snapshot_restore(far_map_t* m, const far_snapshot_t* s, void* stream
     cudaStream_t st = (cudaStream_t)stream;
     FAR_CUDA(cudaMemcpyAsync(m->view.table, s->table, s->b_table, cudaMemcpyDeviceToDevice, st));
     FAR_CUDA(cudaMemcpyAsync(m->view.points, s->points, s->b_points, cudaMemcpyDeviceToDevice, st));
+    FAR_CUDA(cudaMemcpyAsync(m->view.ids, s->ids, s->b_ids, cudaMemcpyDeviceToDevice, st));
     if (s->b_cov && m->view.cov) FAR_CUDA(cudaMemcpyAsync(m->view.cov, s->cov, s->b_cov, cudaMemcpyDeviceToDevice, st));
     if (s->b_ok && m->view.cov_ok) FAR_CUDA(cudaMemcpyAsync(m->view.cov_ok, s->cov_ok, s->b_ok, cudaMemcpyDeviceToDevice, st));
     FAR_CUDA(cudaMemcpyAsync(m->view.ctr, s->ctr, sizeof(Counters), cudaMemcpyDeviceToDevice, st));
