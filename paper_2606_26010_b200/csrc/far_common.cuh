@@ -134,26 +134,26 @@ __device__ __forceinline__ Entry load_entry(const Entry* table, uint32_t s) {
     return e;
 }
 
-// read-only lookup: slot of `key` and its count, or count = 0 if absent / dead.  Linear probing is
-// sequential by definition, but the next slots are known in advance: four consecutive entries are requested at once
-// and examined in probe order, so a lookup costs ONE memory round trip unless its probe sequence is longer than four
-// (the dependent chain of single-slot probes was the longest stall of the 27-voxel search: the warp waits for the
-// slowest of its 27 lookups).
+// read-only lookup: slot of `key` and its count, or count = 0 if absent / dead.  Linear probing, step 1.
+// FAR_PROBE_GROUP consecutive entries are requested per step.  Measured on B200 (profiles/probe_group_r01d.md): really
+// issuing 2 or 4 entries at once shortens the dependent chain but fetches sectors that most lookups never need --
+// the C2 frame gets 2 % / 12 % slower and the NN sweep over 10-17 M-voxel tables (C5, v <= 0.5) 15 % / 45 % slower -- so
+// the default is 1: at load <= 0.5 the first entry decides most lookups.
+#ifndef FAR_PROBE_GROUP
+#define FAR_PROBE_GROUP 1
+#endif
 __device__ __forceinline__ uint32_t find_voxel(const MapView& m, unsigned long long key, uint32_t& count) {
     uint32_t s = hash_key(key) & m.mask;
-    for (uint32_t probes = 0; probes < m.slots; probes += 4) {
-        const uint32_t s1 = (s + 1) & m.mask, s2 = (s + 2) & m.mask, s3 = (s + 3) & m.mask;
-        const Entry e0 = load_entry(m.table, s), e1 = load_entry(m.table, s1), e2 = load_entry(m.table, s2),
-                    e3 = load_entry(m.table, s3);
-        if (e0.key == key) { count = e0.count; return s; }
-        if (e0.key == KEY_EMPTY) break;
-        if (e1.key == key) { count = e1.count; return s1; }
-        if (e1.key == KEY_EMPTY) break;
-        if (e2.key == key) { count = e2.count; return s2; }
-        if (e2.key == KEY_EMPTY) break;
-        if (e3.key == key) { count = e3.count; return s3; }
-        if (e3.key == KEY_EMPTY) break;
-        s = (s + 4) & m.mask;
+    for (uint32_t probes = 0; probes < m.slots; probes += FAR_PROBE_GROUP) {
+        Entry e[FAR_PROBE_GROUP];
+#pragma unroll
+        for (int g = 0; g < FAR_PROBE_GROUP; ++g) e[g] = load_entry(m.table, (s + g) & m.mask);
+#pragma unroll
+        for (int g = 0; g < FAR_PROBE_GROUP; ++g) {
+            if (e[g].key == key) { count = e[g].count; return (s + g) & m.mask; }
+            if (e[g].key == KEY_EMPTY) { count = 0; return NO_SLOT; }
+        }
+        s = (s + FAR_PROBE_GROUP) & m.mask;
     }
     count = 0;
     return NO_SLOT;
