@@ -109,7 +109,7 @@ def test_upsampled_correction_equals_single_correction_for_a_static_linear_syste
     part = _static_filter(10, P0)
     part.push_measurement(z, R, 0)
     part.predict(_rest_input())
-    assert 0.05 < part.x[0] / one.x[0] < 0.5
+    assert 0.05 < part.x[0] / one.x[0] < 0.7          # first of ten steps: K = P/(P + 10 R) = 0.15 of z vs 0.27 in total
 
 
 def test_delay_compensation_eq11_extrapolates_the_measurement_with_the_predicted_motion():
