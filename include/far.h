@@ -2,7 +2,7 @@
  * far.h -- C ABI of the B200-native FAR-LIO front-end hot path (voxel hashmap + sparsity-aware GICP).
  *
  * Source of the method: /root/reference/PAPER.md (FAR-LIO, arxiv/paper_2606_26010), cited below as
- * PAPER.md:<line>.  Readings of passages the paper leaves open are numbered R1..R17 in DESIGN.md.
+ * PAPER.md:<line>.  Readings of passages the paper leaves open are numbered R1..R20 in DESIGN.md.
  * Every entry point below runs hand-written CUDA kernels for sm_100a; there is no CPU fallback.
  *
  * Conventions
@@ -271,6 +271,39 @@ far_threshold_t* far_threshold_create(double sigma0, double min_motion, double m
 void far_threshold_destroy(far_threshold_t*);
 void far_threshold_update(far_threshold_t*, const far_pose_t* predicted, const far_pose_t* registered);
 double far_threshold_sigma(const far_threshold_t*);
+
+/* ---- Sensor Fusion backend (Eq. 7-11; R18-R20).  HOST-only FP64 module, outside the
+ * GPU hot path ("a small host-side module"): kinematic EKF at a fixed rate with the IMU as control input, corrected by the
+ * registered LiDAR pose and velocity with delay compensation and measurement up-sampling.  It supplies what the hot
+ * path consumes: the initial guess T_t of the registration and the velocity history of the undistortion.
+ *   state x = (t, theta, v): position (map), Euler angles (roll, pitch, yaw; R = Rz Ry Rx), velocity (body)   Eq. 8
+ *   predict: x += dt [R(theta) v ; E(theta)(w_m - w_b) ; -[w_m]x v + (a_m - a_b) + g(theta)]                  Eq. 9 (R18)
+ *   measurement z = (t_L, theta_L, [theta_ref], v_L), h = row selection                                     Eq. 10 (R19)
+ *   delayed measurement taken at cycle s: z_k = z_s + h(x_k|k-1) - h(x_s); applied over n_up cycles with
+ *   covariance n_up R (R20)                                                                                  Eq. 11
+ * theta_ref (reference roll/pitch of [31],[32]) is an optional INPUT: its formulas are not in the paper. */
+typedef struct far_ekf far_ekf_t;
+far_ekf_t* far_ekf_create(const double x0[9], const double P0_diag[9], const double Q_diag[9], double dt, int32_t n_up,
+                          const double accel_bias_or_null[3], const double gyro_bias_or_null[3]);
+void far_ekf_destroy(far_ekf_t*);
+/* one cycle: prediction with the IMU sample, then the pending (up-sampled) corrections.  Returns the new cycle index. */
+int64_t far_ekf_predict(far_ekf_t*, const double accel_m[3], const double gyro_m[3]);
+/* queue a LiDAR measurement taken at cycle `cycle_s` (0 <= current - cycle_s < 512): pose T_L, velocity v_L (Eq. 7),
+ * optional reference (roll, pitch), variances in the order of z (9 values, or 11 with theta_ref).  FAR_ERR_ARG if the
+ * cycle is no longer in the state history. */
+int far_ekf_push_lidar(far_ekf_t*, const far_pose_t* T_L, const double v_L[3], const double theta_ref_or_null[2],
+                       const double R_diag[], int64_t cycle_s);
+/* current estimate: x[9], P[81] row-major (nullable), cycle index (nullable) */
+int far_ekf_state(const far_ekf_t*, double x[9], double* P_or_null, int64_t* cycle_or_null);
+/* the state as a pose (R(theta), t): the initial guess T_t of far_gicp_register */
+int far_ekf_pose(const far_ekf_t*, far_pose_t* out);
+/* the last m cycles as (time = cycle * dt, body twist (v, w_m - w_b)) for far_motion_fit ("velocity history
+ * of the Sensor Fusion"); returns the number of samples written (<= m) */
+int far_ekf_velocity_history(const far_ekf_t*, int32_t m, double* times, double* vel6);
+/* Eq. 7: v_L = R_L,t^-1 (t_t - t_{t-1}) / dt */
+int far_lidar_velocity(const far_pose_t* T_t, const far_pose_t* T_prev, double dt, double v_out[3]);
+/* exposed for tests: Eq. 9 and its analytic Jacobian F (row-major 9x9) at (x, u = (a_m, w_m)) with zero biases */
+int far_ekf_model(const double x[9], const double u[6], double dt, double x_next[9], double F[81]);
 
 #ifdef __cplusplus
 }

@@ -140,6 +140,15 @@ def lib():
             "far_asmd_density": (ci, [vp, vp, f64, vp, vp]),
             "far_map_insert_asmd": (ci, [vp, vp, i64, ci, vp, vp, f64, ci, vp, vp]),
             "far_map_insert_asmd_dev": (ci, [vp, vp, i64, ci, vp, vp, f64, ci, vp, vp]),
+            "far_ekf_create": (vp, [vp, vp, vp, f64, i32, vp, vp]),
+            "far_ekf_destroy": (None, [vp]),
+            "far_ekf_predict": (i64, [vp, vp, vp]),
+            "far_ekf_push_lidar": (ci, [vp, vp, vp, vp, vp, i64]),
+            "far_ekf_state": (ci, [vp, vp, vp, vp]),
+            "far_ekf_pose": (ci, [vp, vp]),
+            "far_ekf_velocity_history": (ci, [vp, i32, vp, vp]),
+            "far_lidar_velocity": (ci, [vp, vp, f64, vp]),
+            "far_ekf_model": (ci, [vp, vp, f64, vp, vp]),
             "far_threshold_create": (vp, [f64, f64, f64]),
             "far_threshold_destroy": (None, [vp]),
             "far_threshold_update": (None, [vp, vp, vp]),
@@ -536,6 +545,68 @@ class Frontend:
         _check(lib().far_frontend_process_host(self._h, ptr, n, s, C.byref(po), float(sigma), C.byref(self.h_result), _stream()),
                "far_frontend_process_host")
         return result_to_dict(self.h_result)
+
+
+def _dp(a):
+    return C.c_void_p(a.ctypes.data) if a is not None else None
+
+
+def lidar_velocity(T_t, T_prev, dt):
+    """far_lidar_velocity (Eq. 7)"""
+    v = np.zeros(3)
+    _check(lib().far_lidar_velocity(C.byref(Pose.from_rt(T_t)), C.byref(Pose.from_rt(T_prev)), float(dt), _dp(v)), "far_lidar_velocity")
+    return v
+
+
+def ekf_model(x, u, dt):
+    """far_ekf_model: Eq. 9 step and its analytic Jacobian"""
+    x = np.ascontiguousarray(x, dtype=np.float64); u = np.ascontiguousarray(u, dtype=np.float64)
+    xn, F = np.zeros(9), np.zeros((9, 9))
+    _check(lib().far_ekf_model(_dp(x), _dp(u), float(dt), _dp(xn), _dp(F)), "far_ekf_model")
+    return xn, F
+
+
+class Ekf:
+    """far_ekf_*: host-only FP64 Sensor Fusion backend (Eq. 8-11; R18-R20)"""
+
+    def __init__(self, x0, P0_diag, Q_diag, dt=0.01, n_up=1, accel_bias=None, gyro_bias=None):
+        a = [np.ascontiguousarray(v, dtype=np.float64) for v in (x0, P0_diag, Q_diag)]
+        ab = np.ascontiguousarray(accel_bias, dtype=np.float64) if accel_bias is not None else None
+        wb = np.ascontiguousarray(gyro_bias, dtype=np.float64) if gyro_bias is not None else None
+        self._h = lib().far_ekf_create(_dp(a[0]), _dp(a[1]), _dp(a[2]), float(dt), int(n_up), _dp(ab), _dp(wb))
+        if not self._h:
+            raise ValueError("bad EKF configuration")
+        self.dt = float(dt)
+
+    def __del__(self):
+        if getattr(self, "_h", None) and lib is not None:
+            lib().far_ekf_destroy(self._h)
+            self._h = None
+
+    def predict(self, accel_m, gyro_m):
+        a = np.ascontiguousarray(accel_m, dtype=np.float64); w = np.ascontiguousarray(gyro_m, dtype=np.float64)
+        return int(lib().far_ekf_predict(self._h, _dp(a), _dp(w)))
+
+    def push_lidar(self, T_L, v_L, R_diag, cycle_s, theta_ref=None):
+        v = np.ascontiguousarray(v_L, dtype=np.float64); r = np.ascontiguousarray(R_diag, dtype=np.float64)
+        tr = np.ascontiguousarray(theta_ref, dtype=np.float64) if theta_ref is not None else None
+        assert len(r) == (11 if tr is not None else 9)
+        _check(lib().far_ekf_push_lidar(self._h, C.byref(Pose.from_rt(T_L)), _dp(v), _dp(tr), _dp(r), int(cycle_s)), "far_ekf_push_lidar")
+
+    def state(self):
+        x, P, k = np.zeros(9), np.zeros((9, 9)), C.c_int64(0)
+        _check(lib().far_ekf_state(self._h, _dp(x), _dp(P), C.byref(k)), "far_ekf_state")
+        return x, P, k.value
+
+    def pose(self):
+        p = Pose()
+        _check(lib().far_ekf_pose(self._h, C.byref(p)), "far_ekf_pose")
+        return p.to_rt()
+
+    def velocity_history(self, m):
+        t, v = np.zeros(m), np.zeros((m, 6))
+        n = lib().far_ekf_velocity_history(self._h, int(m), _dp(t), _dp(v))
+        return t[:n], v[:n]
 
 
 class AdaptiveThreshold:
