@@ -182,6 +182,12 @@ int far_gicp_register_dev(const far_map_t* map, const float* d_scan, const float
                           const uint8_t* d_scan_valid, const int64_t* d_n, int64_t n_max, int stride,
                           const far_pose_t* d_init_pose, double sigma, int max_iters,
                           const far_gicp_options_t* opts_or_null, far_gicp_result_t* d_out, void* stream);
+/* same with only n read from DEVICE memory; the initial pose is a HOST pointer passed as a kernel argument (what
+ * far_frontend_process uses: the predicted pose comes from the host-side EKF, the scan size from far_voxelize) */
+int far_gicp_register_dn(const far_map_t* map, const float* d_scan, const float* d_scan_cov6,
+                         const uint8_t* d_scan_valid, const int64_t* d_n, int64_t n_max, int stride,
+                         const far_pose_t* init_pose, double sigma, int max_iters,
+                         const far_gicp_options_t* opts_or_null, far_gicp_result_t* d_out, void* stream);
 /* same as far_map_knn_cov with the query count read from DEVICE memory (for chaining after far_voxelize) */
 int far_map_knn_cov_dev(const far_map_t* map, const float* d_q, const int64_t* d_m, int64_t m_max, int stride,
                         float* d_cov6, uint8_t* d_valid, void* stream);

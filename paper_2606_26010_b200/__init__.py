@@ -129,6 +129,7 @@ def lib():
             "far_gicp_linearize": (ci, [vp, vp, vp, vp, i64, ci, vp, f64, vp, vp, vp]),
             "far_gicp_register": (ci, [vp, vp, vp, vp, i64, ci, vp, f64, ci, vp, vp, vp]),
             "far_gicp_register_dev": (ci, [vp, vp, vp, vp, vp, i64, ci, vp, f64, ci, vp, vp, vp]),
+            "far_gicp_register_dn": (ci, [vp, vp, vp, vp, vp, i64, ci, vp, f64, ci, vp, vp, vp]),
             "far_frontend_create": (ci, [vp, vp]),
             "far_frontend_destroy": (ci, [vp]),
             "far_frontend_map": (vp, [vp]),

@@ -38,10 +38,11 @@ struct __align__(16) Entry {
 // device counters of one map (all zeroed at create / clear)
 struct Counters {
     unsigned long long n_keys;        // claimed keys (live + dead)
-    unsigned int n_touched;           // voxels that received a first new point in the current chunk
-    unsigned int n_cov;               // accepted points queued for covariance in the current call
     unsigned int full_flag;           // sticky: a point was dropped because the table was full
     unsigned int pad;
+    // n_touched .. st_invalid are contiguous: one memset at the start of an insert call zeroes them all
+    unsigned int n_touched;           // voxels that received a first new point in the current chunk
+    unsigned int n_cov;               // accepted points queued for covariance in the current call
     unsigned long long st_accepted, st_new_voxels, st_dropped_full, st_invalid;   // per-call statistics
     unsigned long long pr_vox_removed, pr_pts_removed, pr_vox_left, pr_pts_left;  // per-prune statistics
 };

@@ -117,9 +117,8 @@ int far_frontend_process(far_frontend_t* f, const float* d_scan, int64_t n, int 
     FAR_CUDA(cudaStreamWaitEvent(st, f->ev_join, 0));
     if (n > 0 && (rc = far_map_knn_cov_dev(f->local, f->d_ds_xyz, f->d_n_ds, n, 3, f->d_cov6, f->d_valid, stream))) return rc;
     // A6, A8-A10: registration from the predicted pose
-    FAR_CUDA(cudaMemcpyAsync(f->d_init, init_pose, sizeof(far_pose_t), cudaMemcpyHostToDevice, st));
-    if ((rc = far_gicp_register_dev(f->map, f->d_ds_xyz, f->d_cov6, f->d_valid, f->d_n_ds, n, 3, f->d_init, sigma,
-                                    f->cfg.max_iters, &f->cfg.gicp, res, stream))) return rc;
+    if ((rc = far_gicp_register_dn(f->map, f->d_ds_xyz, f->d_cov6, f->d_valid, f->d_n_ds, n, 3, init_pose, sigma,
+                                   f->cfg.max_iters, &f->cfg.gicp, res, stream))) return rc;
     // A3-A5, A7: submap update at the registered pose
     if (f->cfg.update_map) {
         if (f->cfg.asmd) {

@@ -593,6 +593,15 @@ int far_gicp_register_dev(const far_map_t* map, const float* d_scan, const float
                        stream);
 }
 
+// n from the device, initial pose from the host as a kernel argument (saves far_frontend_process a pageable
+// 96-byte upload per frame)
+int far_gicp_register_dn(const far_map_t* map, const float* d_scan, const float* d_cov6, const uint8_t* d_valid,
+                         const int64_t* d_n, int64_t n_max, int stride, const far_pose_t* init_pose, double sigma, int max_iters,
+                         const far_gicp_options_t* opts, far_gicp_result_t* d_out, void* stream) {
+    if (!d_n || !init_pose) return FAR_ERR_ARG;
+    return gicp_launch(map, d_scan, d_cov6, d_valid, n_max, d_n, stride, init_pose, nullptr, sigma, max_iters, 0, opts, d_out, stream);
+}
+
 #ifdef FAR_GICP_TRACE
 // debug build only: reset (all slots 0, min-slot ~0) / read the probes
 void far_gicp_trace_reset(void) {

@@ -556,9 +556,8 @@ static int insert_impl(far_map_t* m, const float* d_xyz, int64_t n, int stride, 
     memset(&hp, 0, sizeof(hp));
     if (pose_mode == 1) memcpy(&hp, hpose, sizeof(hp));
     Counters* ctr = m->view.ctr;
-    // zero the per-call statistics and the covariance queue
-    FAR_CUDA(cudaMemsetAsync(&ctr->st_accepted, 0, 4 * sizeof(unsigned long long), st));
-    FAR_CUDA(cudaMemsetAsync(&ctr->n_cov, 0, sizeof(unsigned int), st));
+    // zero the touched counter, the covariance queue and the per-call statistics (contiguous: one call)
+    FAR_CUDA(cudaMemsetAsync(&ctr->n_touched, 0, 2 * sizeof(unsigned int) + 4 * sizeof(unsigned long long), st));
     const bool cov_by_list = compute_cov && n <= m->max_batch;
     const uint32_t call_first_id = (uint32_t)m->next_id;
     const int commit_grid = m->sm_count * 8;
@@ -566,7 +565,7 @@ static int insert_impl(far_map_t* m, const float* d_xyz, int64_t n, int stride, 
         const int64_t nc = (n - off < m->max_batch) ? n - off : m->max_batch;
         const uint32_t first_id = (uint32_t)(m->next_id + (uint64_t)off);
         const float* xyz = d_xyz + off * stride;
-        FAR_CUDA(cudaMemsetAsync(&ctr->n_touched, 0, sizeof(unsigned int), st));
+        if (off > 0) FAR_CUDA(cudaMemsetAsync(&ctr->n_touched, 0, sizeof(unsigned int), st));
         FAR_LAUNCH(insert_claim_chain_kernel, grid_for(nc, 256), 256, 0, st, m->view, xyz, nc, stride, pose_mode, hp,
                                                                       (const Pose*)d_pose, first_id, m->d_touched, asmd);
         FAR_LAUNCH(insert_commit_kernel, commit_grid, 256, 0, st, m->view, xyz, stride, pose_mode, hp, (const Pose*)d_pose,

@@ -130,9 +130,13 @@ int far_undistort(const float* d_xyz, const float* d_time, int64_t n, int stride
     M.c[4] = (wa[2] * wb[0] - wa[0] * wb[2]) / 12.0;
     M.c[5] = (wa[0] * wb[1] - wa[1] * wb[0]) / 12.0;
     M.dt_ref = dt_ref;
-    int dev = 0, sms = 148;
-    FAR_CUDA(cudaGetDevice(&dev));
-    FAR_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    static int sms = 0;                       // SM count of the first device used (grid sizing only)
+    if (sms == 0) {
+        int dev = 0, v = 148;
+        FAR_CUDA(cudaGetDevice(&dev));
+        FAR_CUDA(cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev));
+        sms = v;
+    }
     int64_t g = (n + 255) / 256;
     if (g > (int64_t)sms * 32) g = (int64_t)sms * 32;
     FAR_LAUNCH(undistort_kernel, (int)g, 256, 0, (cudaStream_t)stream, d_xyz, d_time, n, stride, M, d_out_xyz);

@@ -240,18 +240,42 @@ __global__ void knn_cov_new_ids_kernel(MapView m, uint32_t first_id, int warps_p
 
 struct KnnLaunch { int warps, grid; size_t smem; };
 
+// The shared-memory opt-in and the occupancy query are slow host calls: done once per (kernel, k_cov, device) and cached
+// (the frame chain launches two of these kernels per scan and is host-enqueue-bound end to end).
 template <class K>
 static int knn_launch_cfg(const far_map* map, K kernel, int64_t work, KnnLaunch& L) {
+    struct Cached { bool have; int warps, per_sm; size_t smem; };
+    static Cached cache[33][8] = {};          // one table per kernel instantiation
+    const int dev = map->device & 7;
+    Cached& c = cache[map->view.k_cov][dev];
+    static size_t attr_bytes[8] = {};         // largest dynamic shared-memory opt-in made for this kernel, per device
+    if (c.have && map->device < 8) {
+        L.warps = c.warps; L.smem = c.smem;
+        if (c.smem > attr_bytes[dev]) {       // another k_cov lowered nothing, but a larger one may be needed now
+            FAR_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem));
+            attr_bytes[dev] = c.smem;
+        }
+        int64_t grid = (int64_t)map->sm_count * c.per_sm;
+        const int64_t need = (work + c.warps - 1) / c.warps;
+        if (need < grid) grid = need;
+        if (grid < 1) grid = 1;
+        L.grid = (int)grid;
+        return FAR_OK;
+    }
     const size_t per_warp = knn_smem_per_warp(map->view.k_cov);
     int warps = (int)(100 * 1024 / per_warp);
     if (warps > 8) warps = 8;
     if (warps < 1) warps = 1;
     L.warps = warps;
     L.smem = per_warp * warps;
-    FAR_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem));
+    if (L.smem > attr_bytes[dev]) {           // the opt-in is per function: only ever raise it
+        FAR_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem));
+        attr_bytes[dev] = L.smem;
+    }
     int per_sm = 0;
     FAR_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, warps * 32, L.smem));
     if (per_sm < 1) per_sm = 1;
+    c.warps = warps; c.per_sm = per_sm; c.smem = L.smem; c.have = true;
     int64_t grid = (int64_t)map->sm_count * per_sm;
     const int64_t need = (work + warps - 1) / warps;
     if (need < grid) grid = need;
