@@ -131,49 +131,70 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
     }
 }
 
-// ---- insert, kernel 2: one warp per touched voxel writes the coordinates of the surviving ids ---------------
+// ---- insert, kernel 2: 8 lanes per touched voxel write the coordinates of the surviving ids -------------------
+// Every step of a voxel's commit is a dependent, usually cold access (touched list -> entry -> id row -> source point ->
+// bucket), and most touched voxels receive a handful of points, so a warp works on FOUR voxels at once: four times the
+// memory-level parallelism of a warp per voxel (C4, where almost every point opens its own voxel in a multi-GB pool,
+// is bound by exactly that).  The statistics are accumulated per warp and flushed once at the end.
+constexpr int COMMIT_LANES = 8;
 __global__ void __launch_bounds__(256) insert_commit_kernel(MapView m, const float* __restrict__ xyz, int stride,
                                                              int pose_mode, Pose hpose, const Pose* __restrict__ d_pose,
                                                              uint32_t first_id, const uint32_t* __restrict__ touched,
                                                              uint32_t* __restrict__ cov_list, int64_t cov_list_cap) {
-    const int lane = threadIdx.x & 31;
+    const int lane = threadIdx.x & 31, sub = lane / COMMIT_LANES, sl = lane % COMMIT_LANES;
+    constexpr int PER_WARP = 32 / COMMIT_LANES;
+    const unsigned gmask = ((1u << COMMIT_LANES) - 1u) << (sub * COMMIT_LANES);
     const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
     const Pose& T = (pose_mode == 2) ? *d_pose : hpose;
     const uint32_t n_touched = m.ctr->n_touched;
     const uint32_t cap = (uint32_t)m.cap;
-    for (int64_t t = warp; t < n_touched; t += nwarps) {
-        const uint32_t s = touched[t];
-        const uint32_t c0 = m.table[s].count;
-        float4* bucket = m.points + (size_t)s * cap;
+    unsigned long long acc_new = 0, acc_vox = 0;          // lane sl == 0 of each group: points accepted, voxels opened
+    for (int64_t t0 = warp * PER_WARP; t0 < n_touched; t0 += nwarps * PER_WARP) {
+        const int64_t t = t0 + sub;
+        const bool active = t < n_touched;
+        uint32_t s = 0, c0 = cap;
+        if (active) {
+            s = touched[t];
+            c0 = m.table[s].count;
+        }
         uint32_t n_new = 0;
-        for (uint32_t base = c0; base < cap; base += 32) {
-            const uint32_t pos = base + lane;
+        for (uint32_t step = 0; step * COMMIT_LANES < cap; ++step) {      // warp-uniform trip count
+            const uint32_t pos = c0 + step * COMMIT_LANES + sl;
             uint32_t id = NO_ID;
-            if (pos < cap) id = m.ids[(size_t)s * cap + pos];
+            if (active && pos < cap) id = m.ids[(size_t)s * cap + pos];
             const bool is_new = id != NO_ID;
             if (is_new) {
                 float p[3];
                 load_pose_point(xyz, (int64_t)(id - first_id), stride, pose_mode, T, p);
-                bucket[pos] = make_float4(p[0], p[1], p[2], __uint_as_float(id));
+                m.points[(size_t)s * cap + pos] = make_float4(p[0], p[1], p[2], __uint_as_float(id));
                 if (m.cov_ok) m.cov_ok[(size_t)s * cap + pos] = 0;
             }
             const unsigned b = __ballot_sync(FULL, is_new);
-            const uint32_t cnt = __popc(b);
-            if (cov_list != nullptr && cnt) {
+            if (b == 0) break;                                             // ids fill positions in order: nothing further
+            if (cov_list != nullptr) {
                 uint32_t at = 0;
-                if (lane == 0) at = atomicAdd(&m.ctr->n_cov, cnt);
+                if (lane == 0) at = atomicAdd(&m.ctr->n_cov, (uint32_t)__popc(b));
                 at = __shfl_sync(FULL, at, 0);
                 const uint32_t mine = at + __popc(b & ((1u << lane) - 1u));
                 if (is_new && mine < cov_list_cap) cov_list[mine] = s * cap + pos;
             }
-            n_new += cnt;
+            n_new += __popc(b & gmask);
         }
-        if (lane == 0) {
+        if (active && sl == 0) {
             m.table[s].count = c0 + n_new;
-            atomicAdd(&m.ctr->st_accepted, (unsigned long long)n_new);
-            if (c0 == 0) atomicAdd(&m.ctr->st_new_voxels, 1ull);
+            acc_new += n_new;
+            if (c0 == 0) acc_vox += 1;
         }
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        acc_new += __shfl_xor_sync(FULL, acc_new, d);
+        acc_vox += __shfl_xor_sync(FULL, acc_vox, d);
+    }
+    if (lane == 0) {
+        if (acc_new) atomicAdd(&m.ctr->st_accepted, acc_new);
+        if (acc_vox) atomicAdd(&m.ctr->st_new_voxels, acc_vox);
     }
 }
 
