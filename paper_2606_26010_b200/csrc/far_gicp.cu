@@ -238,26 +238,15 @@ __device__ __forceinline__ bool chol_solve6(const double* H, const double* rhs, 
     return true;
 }
 
-// SE(3) exponential of delta = (rho, phi), translation first (R12); Taylor series up to theta = 0.5
+// SE(3) exponential of delta = (rho, phi), translation first (R12); series below theta = 1e-8
 __device__ __forceinline__ void se3_exp(const double* d, Pose& E) {
     const double px = d[3], py = d[4], pz = d[5];
     const double th2 = px * px + py * py + pz * pz;
+    const double th = sqrt(th2);
     double A, B, C;
-    if (th2 <= 0.25) {
-        // Gauss-Newton increments are small: A = sin(t)/t, B = (1-cos t)/t^2, C = (t-sin t)/t^3 from their Taylor series
-        // in t^2 (9 terms, remainder < 1e-22) -- no sqrt, sincos or division on the serial path of every iteration
-        const double x = th2;
-        A = -1.0 / 355687428096000.0; B = -1.0 / 6402373705728000.0; C = -1.0 / 121645100408832000.0;
-        A = fma(A, x, 1.0 / 1307674368000.0);   B = fma(B, x, 1.0 / 20922789888000.0);   C = fma(C, x, 1.0 / 355687428096000.0);
-        A = fma(A, x, -1.0 / 6227020800.0);     B = fma(B, x, -1.0 / 87178291200.0);     C = fma(C, x, -1.0 / 1307674368000.0);
-        A = fma(A, x, 1.0 / 39916800.0);        B = fma(B, x, 1.0 / 479001600.0);        C = fma(C, x, 1.0 / 6227020800.0);
-        A = fma(A, x, -1.0 / 362880.0);         B = fma(B, x, -1.0 / 3628800.0);         C = fma(C, x, -1.0 / 39916800.0);
-        A = fma(A, x, 1.0 / 5040.0);            B = fma(B, x, 1.0 / 40320.0);            C = fma(C, x, 1.0 / 362880.0);
-        A = fma(A, x, -1.0 / 120.0);            B = fma(B, x, -1.0 / 720.0);             C = fma(C, x, -1.0 / 5040.0);
-        A = fma(A, x, 1.0 / 6.0);               B = fma(B, x, 1.0 / 24.0);               C = fma(C, x, 1.0 / 120.0);
-        A = fma(A, -x, 1.0);                    B = fma(B, -x, 0.5);                     C = fma(C, -x, 1.0 / 6.0);
+    if (th < 1e-8) {
+        A = 1.0 - th2 / 6.0; B = 0.5 - th2 / 24.0; C = 1.0 / 6.0 - th2 / 120.0;
     } else {
-        const double th = sqrt(th2);
         double sn, cs;
         sincos(th, &sn, &cs);
         const double ith = 1.0 / th, ith2 = ith * ith;
