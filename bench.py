@@ -517,6 +517,24 @@ def run_far(args):
                             "algorithmic_GBps": len(c2["map_points"]) * 40 / t_ins / 1e9,
                             "note": "1.52 M points in one call into an empty v=1.0 cap-20 map, no covariances"}
         mp.close()
+        # the same frame (a) registration only -- the latency to the pose, before the map update (the paper reports the two
+        # separately) -- and (b) with the Adaptive Submap Density limit on the map update
+        for name, kw in (("register_only", dict(update_map=False)), ("asmd_frame", dict(asmd=True, asmd_r_close=10.0, asmd_d_max=100.0))):
+            fx = far.Frontend(v, cap, c2["max_voxels"], len(scan), ds_voxel=v, prune_radius=PRUNE_RADIUS, max_iters=MAX_ITERS, **kw)
+            fx.map.insert(d_map_pts, compute_cov=True)
+            sx = fx.map.snapshot()
+            ts = []
+            for i in range(13):
+                fx.map.restore(sx)
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(); fx.process_enqueue(d_scan, T_init, sigma, d_result=d_res[0]); b.record(); torch.cuda.synchronize()
+                ts.append(a.elapsed_time(b))
+            n0 = fx.map.stats()["n_points"]
+            fx.map.restore(sx)
+            n1 = fx.map.stats()["n_points"]
+            extras[name] = {"ms_per_frame": float(np.median(ts[3:])), "accepted_per_frame": int(n0 - n1)}
+            far.Map.snapshot_destroy(sx)
+            fx.close()
         # motion undistortion: 8 M points of racing-shaped sweeps, 28 B algorithmic per point (12 + 4 in, 12 out)
         nu = 8_000_000
         gen = torch.Generator(device="cuda").manual_seed(0)
