@@ -183,7 +183,7 @@ __device__ __forceinline__ bool warp_knn_cov(const MapView& m, float qx, float q
 }
 
 // queries given as points (far_map_knn_cov); n read from the device if d_n != nullptr
-__global__ void knn_cov_points_kernel(MapView m, const float* __restrict__ q, int64_t n, const int64_t* __restrict__ d_n,
+__global__ void __launch_bounds__(256, 5) knn_cov_points_kernel(MapView m, const float* __restrict__ q, int64_t n, const int64_t* __restrict__ d_n,
                                       int stride, float* __restrict__ cov6, uint8_t* __restrict__ valid, int warps_per_block) {
     extern __shared__ __align__(16) char smem[];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
@@ -200,7 +200,7 @@ __global__ void knn_cov_points_kernel(MapView m, const float* __restrict__ q, in
 }
 
 // queries = stored points named by refs (covariances of the points an insert accepted)
-__global__ void knn_cov_refs_kernel(MapView m, const uint32_t* __restrict__ refs, const unsigned int* __restrict__ d_n,
+__global__ void __launch_bounds__(256, 5) knn_cov_refs_kernel(MapView m, const uint32_t* __restrict__ refs, const unsigned int* __restrict__ d_n,
                                     int warps_per_block) {
     extern __shared__ __align__(16) char smem[];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
@@ -218,7 +218,7 @@ __global__ void knn_cov_refs_kernel(MapView m, const uint32_t* __restrict__ refs
 }
 
 // same for calls larger than the covariance queue: every stored point with id >= first_id is a new point
-__global__ void knn_cov_new_ids_kernel(MapView m, uint32_t first_id, int warps_per_block) {
+__global__ void __launch_bounds__(256, 5) knn_cov_new_ids_kernel(MapView m, uint32_t first_id, int warps_per_block) {
     extern __shared__ __align__(16) char smem[];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     char* smem_w = smem + (size_t)wib * knn_smem_per_warp(m.k_cov);
