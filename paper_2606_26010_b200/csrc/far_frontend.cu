@@ -22,7 +22,6 @@ struct far_frontend {
     int64_t* d_n_ds;
     float* d_cov6;
     uint8_t* d_valid;
-    far_pose_t* d_init;
     far_gicp_result_t* d_result;
     cudaStream_t side;       // second stream: the downsampling branch runs beside the scan-local map build
     cudaEvent_t ev_fork, ev_join;
@@ -40,7 +39,7 @@ int far_frontend_destroy(far_frontend_t* f) {
     if (f->ev_join) cudaEventDestroy(f->ev_join);
     if (f->side) cudaStreamDestroy(f->side);
     cudaFree(f->d_ws); cudaFree(f->d_scan); cudaFree(f->d_ds_xyz); cudaFree(f->d_ds_index); cudaFree(f->d_n_ds);
-    cudaFree(f->d_cov6); cudaFree(f->d_valid); cudaFree(f->d_init); cudaFree(f->d_result); cudaFree(f->d_asmd); cudaFree(f->d_undist);
+    cudaFree(f->d_cov6); cudaFree(f->d_valid); cudaFree(f->d_result); cudaFree(f->d_asmd); cudaFree(f->d_undist);
     delete f;
     return FAR_OK;
 }
@@ -79,7 +78,6 @@ int far_frontend_create(far_frontend_t** out, const far_frontend_config_t* cfg) 
     alloc((void**)&f->d_n_ds, sizeof(int64_t));
     alloc((void**)&f->d_cov6, (size_t)n * 6 * sizeof(float));
     alloc((void**)&f->d_valid, (size_t)n);
-    alloc((void**)&f->d_init, sizeof(far_pose_t));
     alloc((void**)&f->d_result, sizeof(far_gicp_result_t));
     alloc((void**)&f->d_asmd, 2 * sizeof(double));
     alloc((void**)&f->d_undist, (size_t)n * 3 * sizeof(float));

@@ -12,8 +12,11 @@
 // B200 design: a registration is a few thousand source points, i.e. latency- and issue-bound, never bandwidth-
 // bound, so the whole Gauss-Newton loop is ONE persistent cooperative kernel and every iteration is organised to
 // keep both the instruction count and the serial chain short:
-//   phase A  one warp per source point: FP64 transform, 27-voxel probe, bounded candidate sweep
-//            (far_common.cuh::warp_nearest), gate, fetch of Sigma_r -> one correspondence record in shared memory;
+//   phase A0 8 lanes of warp 0 transform the block's 8 source points (FP64) and take their voxel indices: one
+//            instruction stream instead of 8 redundant warps; a warp's source point, covariance and flag stay in
+//            registers across iterations (one memory level less per iteration);
+//   phase A  one warp per source point: 27-voxel probe, bounded candidate sweep (far_common.cuh::warp_nearest), gate,
+//            fetch of Sigma_r -> one correspondence record in shared memory;
 //   phase B  the block's 8 correspondences are linearised by 8 lanes of warp 0 at once (the ~300 FP64 operations of
 //            M, weight, J^T M J are one instruction stream for 8 points instead of 8 streams with one active lane);
 //   reduce   the 29 unique terms of (H, b, chi2, n) go block -> group of 32 blocks -> grid as TAGGED rows: every
@@ -21,7 +24,12 @@
 //            iteration), so a consumer just polls the rows it needs -- no fence, no ticket atomics -- and sums
 //            them in a fixed order (deterministic, no floating-point atomics);
 //   solve    block 0 / thread 0: 6x6 Cholesky, SE(3) exponential, pose update and stop test in FP64, published as
-//            13 tagged words that every block polls: one L2 round trip from "solved" to "next iteration".
+//            13 tagged words; one lane per block polls the `done` word with a short back-off, then twelve lanes fetch
+//            the pose: one L2 round trip from "solved" to "next iteration" without the waiters crowding that slice.
+// Measured per iteration at C2 (5,352 points, debug-only globaltimer probes): A0+A 6.8 us, B 2.1, reduce 1.8, solve 2.2,
+// publish 1.1-2.0.  The arithmetic of B and solve is left exactly as it is: the C3 chain (tests/test_gpu_full_size.py)
+// amplifies a 1e-16 change of one increment to 2 fp32 ulps of a stored coordinate within 12 frames, along the
+// unobservable direction of the corridor.
 // The host is not involved until it reads the result.
 #include <atomic>
 #include <cstring>
@@ -639,7 +647,6 @@ int gicp_setup(far_map* map) {
     const size_t bytes = ((size_t)(map->gicp_max_grid + MAX_GROUPS) * TSTRIDE + 16) * sizeof(uint4);
     FAR_CUDA(cudaMalloc((void**)&map->d_gicp_partials, bytes));
     FAR_CUDA(cudaMemset(map->d_gicp_partials, 0, bytes));     // tag 0 is never used by a launch
-    map->d_gicp_state = nullptr;
     return FAR_OK;
 }
 }  // namespace far

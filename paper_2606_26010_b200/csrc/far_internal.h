@@ -11,7 +11,6 @@ struct far_map {
     uint32_t* d_touched;        // [max_batch] slots that received their first new point in the chunk
     uint32_t* d_cov_list;       // [max_batch] refs (slot*cap+pos) of accepted points awaiting a covariance
     void* d_gicp_partials;      // tagged reduction rows + published pose of the cooperative GICP kernel (far_gicp.cu)
-    void* d_gicp_state;         // unused (kept for layout stability)
     int gicp_max_grid;          // co-resident blocks of the GICP kernel on this device
     int64_t max_batch;
     uint64_t next_id;           // id of the next offered point (host-side: advances by n per insert)

@@ -568,7 +568,7 @@ int far_map_destroy(far_map_t* m) {
     if (!m) return FAR_OK;
     cudaFree(m->view.table); cudaFree(m->view.points); cudaFree(m->view.ids); cudaFree(m->view.cov); cudaFree(m->view.cov_ok);
     cudaFree(m->view.ctr); cudaFree(m->d_touched); cudaFree(m->d_cov_list);
-    cudaFree(m->d_gicp_partials); cudaFree(m->d_gicp_state);
+    cudaFree(m->d_gicp_partials);
     delete m;
     return FAR_OK;
 }
