@@ -1,7 +1,7 @@
 // far_common.cuh -- device-side building blocks shared by the far_* kernels (sm_100a).
 //
 // Layout of the voxel hashmap in HBM ("cuVoxelMap"; re-designed for B200):
-//   table   : Entry[slots]            16 B per slot {u64 key, u32 count, u32 pad}; one LDG.128 yields the key
+//   table   : Entry[slots]            16 B per slot {u64 key, u32 count, u32 reach}; one LDG.128 yields the key
 //                                     AND the number of points, so a lookup is two dependent memory levels
 //                                     (entry -> points), not three.
 //   points  : float4[slots * cap]     bucket of slot s = points[s*cap .. s*cap+cap); .w = id bits.  The bucket
@@ -32,7 +32,7 @@ constexpr unsigned FULL = 0xFFFFFFFFu;
 struct __align__(16) Entry {
     unsigned long long key;
     uint32_t count;
-    uint32_t pad;
+    uint32_t pad;      // reach of this HOME slot: 1 + largest displacement of a key hashing here (see find_voxel)
 };
 
 // device counters of one map (all zeroed at create / clear)
@@ -136,25 +136,24 @@ __device__ __forceinline__ Entry load_entry(const Entry* table, uint32_t s) {
 }
 
 // read-only lookup: slot of `key` and its count, or count = 0 if absent / dead.  Linear probing, step 1.
-// FAR_PROBE_GROUP consecutive entries are requested per step.  Measured on B200 (profiles/probe_group_r01d.md): really
-// issuing 2 or 4 entries at once shortens the dependent chain but fetches sectors that most lookups never need --
-// the C2 frame gets 2 % / 12 % slower and the NN sweep over 10-17 M-voxel tables (C5, v <= 0.5) 15 % / 45 % slower -- so
-// the default is 1: at load <= 0.5 the first entry decides most lookups.
-#ifndef FAR_PROBE_GROUP
-#define FAR_PROBE_GROUP 1
-#endif
+// The spare word of the entry at a key's HOME slot h holds `reach` = 1 + the largest displacement of any key whose home
+// is h (raised with atomicMax when a key is claimed).  A lookup therefore examines at most reach(h) slots: a voxel that
+// is not in the map -- 11 of the 27 neighbours of a typical query -- is usually dismissed by the one home-entry load
+// (no key has that home: reach = 0) instead of a walk to the next empty slot, and the warp no longer waits for the
+// longest of 27 such walks.  (Requesting several consecutive entries per step was measured and rejected:
+// profiles/probe_group_r01d.md.)
 __device__ __forceinline__ uint32_t find_voxel(const MapView& m, unsigned long long key, uint32_t& count) {
-    uint32_t s = hash_key(key) & m.mask;
-    for (uint32_t probes = 0; probes < m.slots; probes += FAR_PROBE_GROUP) {
-        Entry e[FAR_PROBE_GROUP];
-#pragma unroll
-        for (int g = 0; g < FAR_PROBE_GROUP; ++g) e[g] = load_entry(m.table, (s + g) & m.mask);
-#pragma unroll
-        for (int g = 0; g < FAR_PROBE_GROUP; ++g) {
-            if (e[g].key == key) { count = e[g].count; return (s + g) & m.mask; }
-            if (e[g].key == KEY_EMPTY) { count = 0; return NO_SLOT; }
+    const uint32_t h = hash_key(key) & m.mask;
+    Entry e = load_entry(m.table, h);
+    const uint32_t reach = e.pad;
+    uint32_t s = h;
+    for (uint32_t d = 0; d < reach; ++d) {
+        if (d) {
+            s = (h + d) & m.mask;
+            e = load_entry(m.table, s);
         }
-        s = (s + FAR_PROBE_GROUP) & m.mask;
+        if (e.key == key) { count = e.count; return s; }
+        if (e.key == KEY_EMPTY) break;
     }
     count = 0;
     return NO_SLOT;

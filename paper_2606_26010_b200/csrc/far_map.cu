@@ -103,6 +103,8 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
             if (cur == KEY_EMPTY) {
                 new_key = true;
                 found = true;
+                // keep the reach of the key's home slot up to date (far_common.cuh::find_voxel)
+                atomicMax(&m.table[hash_key(key) & m.mask].pad, probes + 1u);
                 break;
             }
         }
@@ -462,7 +464,10 @@ __global__ void __launch_bounds__(256) rehash_scatter_kernel(MapView m, const un
     const unsigned long long key = keys[r];
     uint32_t s = hash_key(key) & m.mask;
     for (uint32_t probes = 0; probes < m.slots; ++probes) {
-        if (atomicCAS(&m.table[s].key, KEY_EMPTY, key) == KEY_EMPTY) break;
+        if (atomicCAS(&m.table[s].key, KEY_EMPTY, key) == KEY_EMPTY) {
+            atomicMax(&m.table[hash_key(key) & m.mask].pad, probes + 1u);
+            break;
+        }
         s = (s + 1) & m.mask;
     }
     const uint32_t cnt = counts[r];
