@@ -309,7 +309,15 @@ extern "C" {
 int far_map_nn(const far_map_t* map, const float* d_q, int64_t m, int stride, uint32_t* d_id, float* d_d2, void* stream) {
     if (!map || m < 0 || (stride != 3 && stride != 4) || (m > 0 && (!d_q || !d_id || !d_d2))) return FAR_ERR_ARG;
     if (m == 0) return FAR_OK;
-    int64_t grid = (int64_t)map->sm_count * 8;   // 8 blocks x 8 warps = 64 warps per SM: one full wave
+    // exactly one resident wave (the kernel is a grid-stride loop): a grid larger than the residency the register
+    // count allows leaves a partial second wave behind
+    static int per_sm = 0;
+    if (per_sm == 0) {
+        int v = 0;
+        FAR_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, nn_kernel, QWARPS * 32, 0));
+        per_sm = v < 1 ? 1 : v;
+    }
+    int64_t grid = (int64_t)map->sm_count * per_sm;
     const int64_t need = (m + QWARPS - 1) / QWARPS;
     if (need < grid) grid = need;
     FAR_LAUNCH(nn_kernel, (int)grid, QWARPS * 32, 0, (cudaStream_t)stream, map->view, d_q, m, stride, d_id, d_d2);
