@@ -298,11 +298,11 @@ def _leg_c5(out, far, scenes, torch, peak, flush):
 
 
 def _leg_c3(out, far, scenes, torch):
-    # ---- C3: racing sequence, 60 frames (of the 200), three forward LiDARs, 250 km/h, insert + prune 200 m per frame --
+    # ---- C3: racing sequence, 200 frames at 10 Hz, three forward LiDARs, 250 km/h (6.94 m per frame), insert + prune 200 m per frame --
     track = scenes.RaceTrack(seed=2)
     rng = np.random.default_rng(2)
-    n_frames, v, cap = 60, 1.0, 20
-    frames = [scenes.c3_racing_frame(track, 700.0 + 6.94 * f, rng) for f in range(n_frames)]
+    n_frames, v, cap = int(os.environ.get("FAR_BENCH_C3_FRAMES", "200")), 1.0, 20
+    frames = [scenes.c3_racing_frame(track, 300.0 + 6.94 * f, rng) for f in range(n_frames)]
     nmax = max(len(f[0]) for f in frames)
     fe = far.Frontend(v, cap, 1 << 19, nmax, ds_voxel=v, prune_radius=200.0, max_iters=30)
     th = far.AdaptiveThreshold(2.0, 0.1, 200.0)
@@ -312,10 +312,13 @@ def _leg_c3(out, far, scenes, torch):
         poses.append(frames[f][1])
     lat, its, errs = [], [], []
     for f in range(2, n_frames):
-        # initial guess = stand-in for the EKF prior the paper feeds the registration: ground truth
-        # perturbed by 0.15 m / 0.3 deg (seeded).  LiDAR-only constant-velocity dead reckoning diverges along-track in
-        # this corridor within ~40 frames (no along-track structure) -- that is what the paper's IMU fusion is for.
-        pred = scenes.perturb_pose(frames[f][1], 0.15, 0.3, rng)
+        # initial guess = stand-in for the EKF prior the paper feeds the registration: the last registered
+        # pose advanced by the TRUE relative motion of the frame (what an IMU integrates well over 0.1 s) and perturbed by
+        # 0.05 m / 0.1 deg (seeded).  A prior taken from the absolute ground truth would disagree with the drifting map
+        # and inflate the adaptive threshold; LiDAR-only constant-velocity dead reckoning diverges along-track in this
+        # corridor within ~40 frames -- that is what the paper's IMU fusion is for.
+        rel = scenes.pose_compose(scenes.pose_inverse(frames[f - 1][1]), frames[f][1])
+        pred = scenes.perturb_pose(scenes.pose_compose(poses[-1], rel), 0.05, 0.1, rng)
         h = torch.as_tensor(frames[f][0]).pin_memory()
         torch.cuda.synchronize()
         t0 = time.perf_counter()
@@ -326,12 +329,16 @@ def _leg_c3(out, far, scenes, torch):
         its.append(g["iters"])
         errs.append(frames[f][1][0].T @ (g["t"] - frames[f][1][1]))
     lateral = np.abs(np.array(errs)).max(axis=0)
+    ms = fe.map.stats()
+    half = len(lat) // 2
     out["c3_racing"] = {"frames": n_frames - 2, "points_per_frame": int(np.mean([len(f[0]) for f in frames])),
                         "e2e_ms_median": float(np.median(lat)), "e2e_ms_p99": float(np.percentile(lat, 99)), "e2e_ms_max": float(np.max(lat)),
+                        "e2e_ms_median_first_half": float(np.median(lat[:half])), "e2e_ms_median_second_half": float(np.median(lat[half:])),
+                        "map_at_end": {"voxels": ms["n_voxels"], "points": ms["n_points"], "dead_keys": ms["n_dead_keys"], "slots": ms["n_slots"]},
                         "registrations_per_s": 1e3 / float(np.mean(lat)), "iters_median": float(np.median(its)), "iters_max": int(np.max(its)),
-                        "max_abs_error_m": {"along": float(lateral[0]), "lateral": float(lateral[1]), "vertical": float(lateral[2])},
+                        "max_abs_drift_m": {"along": float(lateral[0]), "lateral": float(lateral[1]), "vertical": float(lateral[2])},
                         "note": "host scan in, host result out, per-frame sync (the paper's callback, PAPER.md:54-109); initial guess = "
-                                "ground truth perturbed 0.15 m / 0.3 deg (EKF-prior stand-in); the corridor is degenerate along-track (SURVEY 8d)"}
+                                "last registered pose advanced by the true relative motion, perturbed 0.05 m / 0.1 deg (EKF-prior stand-in); errors are accumulated drift vs ground truth"}
     fe.close()
 
 
