@@ -580,8 +580,8 @@ class Ekf:
         self.dt = float(dt)
 
     def __del__(self):
-        if getattr(self, "_h", None) and lib is not None:
-            lib().far_ekf_destroy(self._h)
+        if getattr(self, "_h", None) and lib is not None and _lib is not None:     # not during interpreter teardown
+            _lib.far_ekf_destroy(self._h)
             self._h = None
 
     def predict(self, accel_m, gyro_m):
@@ -617,8 +617,8 @@ class AdaptiveThreshold:
         self._h = C.c_void_p(lib().far_threshold_create(sigma0, min_motion, max_range))
 
     def __del__(self):
-        if getattr(self, "_h", None):
-            lib().far_threshold_destroy(self._h)
+        if getattr(self, "_h", None) and lib is not None and _lib is not None:     # not during interpreter teardown
+            _lib.far_threshold_destroy(self._h)
             self._h = None
 
     def update(self, predicted, registered):
