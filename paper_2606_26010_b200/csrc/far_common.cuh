@@ -39,7 +39,7 @@ struct __align__(16) Entry {
 struct Counters {
     unsigned long long n_keys;        // claimed keys (live + dead)
     unsigned int full_flag;           // sticky: a point was dropped because the table was full
-    unsigned int pad;
+    unsigned int pad;                 // ticket of prune_kernel's last-block-done epilogue (0 between launches)
     // n_touched .. st_invalid are contiguous: one memset at the start of an insert call zeroes them all
     unsigned int n_touched;           // voxels that received a first new point in the current chunk
     unsigned int n_cov;               // accepted points queued for covariance in the current call

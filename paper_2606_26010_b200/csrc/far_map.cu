@@ -229,7 +229,7 @@ __global__ void insert_stats_kernel(MapView m, int64_t n_offered, far_insert_sta
 
 // ---- A5 prune (R5): thread per slot, FP64 squared centre distance, strict > -------------------
 __global__ void __launch_bounds__(256) prune_kernel(MapView m, double cx, double cy, double cz, const Pose* d_pose,
-                                                     double r2) {
+                                                     double r2, far_prune_stats_t* __restrict__ out) {
     const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
     unsigned long long vr = 0, pr = 0, vl = 0, pl = 0;
     if (s < m.slots) {
@@ -273,18 +273,24 @@ __global__ void __launch_bounds__(256) prune_kernel(MapView m, double cx, double
 #pragma unroll
         for (int w = 0; w < 8; ++w) t += s_acc[w][threadIdx.x];
         if (t) atomicAdd(&m.ctr->pr_vox_removed + threadIdx.x, t);
+        __threadfence();
     }
-}
-
-__global__ void prune_stats_kernel(MapView m, far_prune_stats_t* out) {
-    if (threadIdx.x == 0 && blockIdx.x == 0) {
+    // the block that takes the last ticket writes the statistics out and re-arms the counters: no second launch
+    __shared__ bool s_last;
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = atomicAdd(&m.ctr->pad, 1u) == gridDim.x - 1;
+    __syncthreads();
+    if (s_last && threadIdx.x == 0) {
+        __threadfence();
+        volatile unsigned long long* c = &m.ctr->pr_vox_removed;
         if (out) {
-            out->n_voxels_removed = (int64_t)m.ctr->pr_vox_removed;
-            out->n_points_removed = (int64_t)m.ctr->pr_pts_removed;
-            out->n_voxels_left = (int64_t)m.ctr->pr_vox_left;
-            out->n_points_left = (int64_t)m.ctr->pr_pts_left;
+            out->n_voxels_removed = (int64_t)c[0];
+            out->n_points_removed = (int64_t)c[1];
+            out->n_voxels_left = (int64_t)c[2];
+            out->n_points_left = (int64_t)c[3];
         }
-        m.ctr->pr_vox_removed = m.ctr->pr_pts_removed = m.ctr->pr_vox_left = m.ctr->pr_pts_left = 0ull;
+        c[0] = 0ull; c[1] = 0ull; c[2] = 0ull; c[3] = 0ull;
+        m.ctr->pad = 0u;
     }
 }
 
@@ -673,8 +679,7 @@ static int prune_impl(far_map_t* m, const double* c, const far_pose_t* d_pose, d
     cudaStream_t st = (cudaStream_t)stream;
     const double r2 = radius * radius;
     FAR_LAUNCH(prune_kernel, grid_for(m->view.slots, 256), 256, 0, st, m->view, c ? c[0] : 0.0, c ? c[1] : 0.0, c ? c[2] : 0.0,
-                                                                (const Pose*)d_pose, r2);
-    FAR_LAUNCH(prune_stats_kernel, 1, 32, 0, st, m->view, d_stats);
+                                                                (const Pose*)d_pose, r2, d_stats);
     FAR_CUDA(cudaGetLastError());
     return FAR_OK;
 }
