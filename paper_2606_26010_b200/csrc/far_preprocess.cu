@@ -12,7 +12,8 @@
 // arguments (constant bank).  All arithmetic is FP64 -- the result is rounded to fp32 once -- and the rotation is
 // applied as p + A (phi x p) + B (phi x (phi x p)) without ever forming a matrix; for the small angles of a sweep
 // (|phi| <= 0.5 rad) the coefficients A = sin(t)/t, B = (1-cos t)/t^2, C = (t-sin t)/t^3 come from their Taylor
-// series in t^2 (9 terms, remainder < 1e-22), which avoids sincos, the square root and two divisions.
+// series in t^2 (5 terms up to 0.1 rad, 9 terms up to 0.5 rad; remainders < 3e-18), which avoids sincos, the square root
+// and two divisions.
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -29,7 +30,14 @@ struct MotionArgs {
 };
 
 __device__ __forceinline__ void abc_coefficients(double x /* theta^2 */, double& A, double& B, double& C) {
-    if (x <= 0.25) {
+    if (x <= 0.01) {
+        // |phi| <= 0.1 rad (every realistic sweep: 1 rad/s over 0.1 s): 5 terms, remainder x^5 / 11! < 3e-18
+        A = 1.0 / 362880.0;                      B = 1.0 / 3628800.0;                     C = 1.0 / 39916800.0;
+        A = fma(A, x, -1.0 / 5040.0);            B = fma(B, x, -1.0 / 40320.0);           C = fma(C, x, -1.0 / 362880.0);
+        A = fma(A, x, 1.0 / 120.0);              B = fma(B, x, 1.0 / 720.0);              C = fma(C, x, 1.0 / 5040.0);
+        A = fma(A, x, -1.0 / 6.0);               B = fma(B, x, -1.0 / 24.0);              C = fma(C, x, -1.0 / 120.0);
+        A = fma(A, x, 1.0);                      B = fma(B, x, 0.5);                      C = fma(C, x, 1.0 / 6.0);
+    } else if (x <= 0.25) {
         // sum_k (-1)^k x^k / (2k+1)!, / (2k+2)!, / (2k+3)!   for k = 0..8 (Horner)
         A = -1.0 / 355687428096000.0;      // 17!
         B = -1.0 / 6402373705728000.0;     // 18!
