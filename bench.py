@@ -559,7 +559,21 @@ def run_far(args):
         extras["undistort"] = {"points": nu, "points_per_s": nu / t_u, "ms": t_u * 1e3, "algorithmic_GBps": nu * 28 / t_u / 1e9,
                                "frac_of_hbm_peak": nu * 28 / t_u / 1e9 / peak,
                                "note": "8 M points in one call (224 MB > L2), FP64 arithmetic, 256 MB flush between repetitions"}
-        del up, ut, uo
+        # scan downsampling (A2) at the same size: 8 M points in a 300 m cube at v = 1 m
+        vz = far.Voxelizer(nu)
+        ts = []
+        for i in range(8):
+            flush.fill_(i)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); vz.enqueue(up, 1.0); b.record(); torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        t_v = float(np.median(ts[3:])) * 1e-3
+        n_out = int(vz.n_out.item())
+        vbytes = nu * 20 + n_out * 16
+        extras["voxelize"] = {"points": nu, "voxels_out": n_out, "points_per_s": nu / t_v, "ms": t_v * 1e3,
+                              "algorithmic_GBps": vbytes / t_v / 1e9, "frac_of_hbm_peak": vbytes / t_v / 1e9 / peak,
+                              "note": "worst case: 8 M points uniform in a 300 m cube at v = 1 m, nearly every point opens its own voxel (random scatter into a 2^24-slot scratch table); 20 B per point + 16 B per output (SURVEY 8d)"}
+        del up, ut, uo, vz
 
     if args.full_extras:
         extras["full"] = full_extras(far, scenes, torch, peak)
