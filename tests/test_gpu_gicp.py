@@ -273,6 +273,42 @@ def test_c2_reduced_frame_end_to_end_device_chain():
     assert np.abs(eg["xyz"] - eo["xyz"]).max() < 1e-5
 
 
+def test_paper_parameters_v4_cap40_frame_matches_oracle():
+    """The paper's own map parameters (v = 4 m, N_max = 40, k = 10): up to 27 x 40 = 1,080 candidates per
+    query exercise the long candidate lists of the kNN / NN sweeps; Sigma_s, registration and the map update against
+    the oracle on the reduced C2 scene."""
+    c2 = scenes.c2_single_frame(seed=1, n_map_candidates=200_000, map_radius=60.0, rings=16, azimuths=1024)
+    v, cap, sigma = 4.0, 40, c2["sigma"]
+    mo, mg = _build_pair(c2["map_points"], v, cap)
+    scan = c2["scan"]
+    ds_o, idx_o = oracle.voxelize(scan, 1.0)
+    ds_g, idx_g = far.voxelize(scan, 1.0)
+    assert np.array_equal(idx_g.cpu().numpy(), idx_o)
+    lo, lg = oracle.Map(v, cap), far.Map(v, cap, 1 << 14)
+    lo.insert(scan); lg.insert(scan)
+    cov_o, val_o = lo.knn_cov(ds_o, nthreads=8)
+    cov_g, val_g = lg.knn_cov(ds_g)
+    assert np.array_equal(val_g.cpu().numpy(), val_o) and val_o.mean() > 0.9
+    cnt = mg.count27(ds_g).cpu().numpy()
+    assert cnt.max() > 600                                  # the long lists really occur
+    ids_o, d2_o = mo.nn(ds_o)
+    ids_g, d2_g = mg.nn(ds_g)
+    assert np.array_equal(ids_g.cpu().numpy().view(np.uint32), ids_o)
+    assert np.array_equal(d2_g.cpu().numpy().view(np.uint32), d2_o.view(np.uint32))
+    o = mo.gicp_register(ds_o, cov_o, val_o, c2["T_init"], sigma, 30, nthreads=8)
+    g = mg.gicp_register(ds_g, cov_g, val_g, c2["T_init"], sigma, 30)
+    assert g["status"] == o["status"] == 0 and g["iters"] == o["iters"] and g["n_inliers"] == o["n_inliers"]
+    dt, dr = _pose_err(g, o)
+    assert dt < 1e-4 and dr < 1e-5, (dt, dr)
+    assert np.linalg.norm(g["H"] - o["H"]) <= 1e-4 * np.linalg.norm(o["H"])
+    so = mo.insert(scan, pose=(o["R"], o["t"]), compute_cov=True)
+    sg = mg.insert(scan, pose=(g["R"], g["t"]), compute_cov=True)
+    assert sg == so
+    eo, eg = mo.export(with_cov=True), mg.export(with_cov=True)
+    assert np.array_equal(eg["keys"], eo["keys"]) and np.array_equal(eg["ids"], eo["ids"])
+    assert np.array_equal(eg["cov_valid"], eo["cov_valid"])
+
+
 def test_frontend_chain_equals_manual_chain_and_host_variant():
     """far_frontend_process (device scan) and far_frontend_process_host (host scan) give the oracle's frame."""
     c2 = scenes.c2_single_frame(seed=5, n_map_candidates=120_000, map_radius=50.0, rings=16, azimuths=512)
