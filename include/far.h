@@ -32,8 +32,14 @@ enum {
     FAR_OK = 0,
     FAR_ERR_ARG = 1,        /* null pointer, bad stride/size/config */
     FAR_ERR_CUDA = 2,       /* a CUDA runtime call failed (see far_last_cuda_error) */
-    FAR_ERR_FULL = 3,       /* table occupancy limit reached: excess NEW voxels are dropped and counted */
-    FAR_ERR_RANGE = 4,      /* id counter would exceed 2^32-2 */
+    FAR_ERR_FULL = 3,       /* the map's bucket pool (max_voxels) or key table is exhausted: points that would open a NEW
+                               voxel were dropped and counted.  The condition is raised on the device; far_map_insert*,
+                               far_frontend_process* and far_map_status report it from a flag the device mirrors into
+                               pinned host memory, i.e. WITHOUT a synchronisation: a call returns it once the kernels of
+                               an earlier call (or, after a sync, its own) have dropped points.  The call that returns
+                               it has still enqueued all of its work; the flag clears when a prune frees buckets or
+                               the map is cleared */
+    FAR_ERR_RANGE = 4,      /* id counter would exceed 2^32-1 even after renumbering */
     FAR_ERR_DEGENERATE = 5  /* fewer than 6 inliers or H not positive definite; pose returned = init pose */
 };
 
@@ -46,17 +52,28 @@ typedef struct { double R[9]; double t[3]; } far_pose_t;
 typedef struct {
     float voxel_size;      /* v > 0 [m]                      PAPER.md:62,68 (paper: 4 m)                  */
     int32_t cap;           /* max points per voxel, 1..64    PAPER.md:62,68 (paper: N_max = 40)           */
-    int64_t max_voxels;    /* live + pruned voxel keys the table must hold                                */
-    float max_load;        /* table load limit in (0,1); 0 -> 0.5; slots = pow2 >= max_voxels / max_load   */
+    int64_t max_voxels;    /* buckets in the dense pool = live voxels the map can hold (exact limit)       */
+    float max_load;        /* table load limit in (0,0.9]; 0 -> 0.5; slots = pow2 >= max_voxels / max_load */
     int32_t with_cov;      /* 1: allocate per-point covariance storage (needed for GICP targets)           */
     int32_t k_cov;         /* neighbours for Eq. 1; 0 -> 10                                   */
     double cov_eps;        /* regulariser of Eq. 1; 0 -> 1e-3                                 */
     int64_t max_batch;     /* points per internal insert pass; 0 -> 1<<20.  Larger calls are chunked      */
+    int64_t renumber_every;/* offered points between automatic id renumber passes (R22); 0 -> 2^31         */
 } far_map_config_t;
 
 typedef struct { int64_t n_offered, n_accepted, n_new_voxels, n_dropped_full, n_invalid; } far_insert_stats_t;
 typedef struct { int64_t n_voxels_removed, n_points_removed, n_voxels_left, n_points_left; } far_prune_stats_t;
-typedef struct { int64_t n_voxels, n_points, n_dead_keys, n_slots; uint64_t next_id; } far_map_stats_t;
+typedef struct {
+    int64_t n_voxels, n_points;   /* live voxels and the points stored in them                                       */
+    int64_t n_dead_keys;          /* keys of pruned voxels still in the table (dropped by the next rehash)           */
+    int64_t n_slots;
+    uint64_t next_id;             /* the device-resident id counter                                                  */
+    int64_t n_keys;               /* claimed table slots (live + dead)                                               */
+    int64_t n_free_buckets;       /* buckets on the free list (returned by prune)                                    */
+    int64_t n_fresh_buckets;      /* buckets never used yet                                                          */
+    int64_t n_rehash;             /* in-place rehashes since create / clear                                          */
+    int64_t full;                 /* 1: points were dropped since buckets were last freed (see FAR_ERR_FULL)         */
+} far_map_stats_t;
 
 typedef struct {
     int32_t kernel;      /* FAR_KERNEL_*; Cauchy is the paper's (Eq. 5)       */
@@ -103,8 +120,9 @@ int far_map_clear(far_map_t* map, void* stream);
  * compute_cov != 0 (map created with_cov): the covariance (Eq. 1) of every ACCEPTED point is computed against
  * the map after the insert; points already stored keep theirs.
  * d_stats (nullable, device) is overwritten with the totals of this call.
- * Returns FAR_ERR_RANGE (nothing inserted) if next_id + n > 2^32-1.  Table-full is reported through
- * d_stats->n_dropped_full and the sticky flag of far_map_stats (this call itself does not synchronise). */
+ * Returns FAR_ERR_RANGE (nothing inserted) if the id counter cannot take n more ids, FAR_ERR_FULL (work enqueued) as
+ * described at the enum; the exact drop count of this call is d_stats->n_dropped_full.  Two launches per max_batch
+ * chunk (+ one for the covariances); this call itself does not synchronise. */
 int far_map_insert(far_map_t* map, const float* d_xyz, int64_t n, int stride, const far_pose_t* pose_or_null,
                    int compute_cov, far_insert_stats_t* d_stats, void* stream);
 int far_map_insert_dev(far_map_t* map, const float* d_xyz, int64_t n, int stride, const far_pose_t* d_pose,
@@ -117,15 +135,26 @@ int far_map_prune(far_map_t* map, const double center[3], double radius, far_pru
 int far_map_prune_dev(far_map_t* map, const far_pose_t* d_pose, double radius, far_prune_stats_t* d_stats,
                       void* stream);
 
-/* counts live voxels / stored points / dead (pruned) keys; next_id is the host-side counter at call time */
+/* counts live voxels / stored points / dead (pruned) keys and reports the allocator's state (device struct) */
 int far_map_stats(far_map_t* map, far_map_stats_t* d_stats, void* stream);
-/* Maintenance call, not on the per-frame path: re-hashes the live voxels into a clean table, dropping the keys
- * of pruned voxels (they otherwise stay as dead keys that lengthen probe sequences).  Allocates a temporary for
- * the live buckets, synchronises the stream, frees the temporary; map contents are unchanged. */
+/* FAR_OK or FAR_ERR_FULL from the host-visible mirror of the device's sticky flag; never synchronises */
+int far_map_status(const far_map_t* map);
+/* Deletion in open addressing (SURVEY.md:214-216; PAPER.md:109 prunes every frame, :171,186 nothing may allocate):
+ * far_map_prune hands the buckets of removed voxels back to the free list at once and leaves their keys behind as dead
+ * keys; when these pass max(32 + live/8) -- decided on the device in prune's epilogue -- the two rehash kernels that
+ * every prune call enqueues rebuild the 16-byte entries into the preallocated shadow table, recompute the probe bounds and
+ * copy them back.  far_map_rehash forces that rebuild now.  No allocation, no synchronisation; contents unchanged. */
 int far_map_rehash(far_map_t* map, void* stream);
+/* R22 (ids are this library's construct, PAPER.md has none): ids are u32 and advance by the points OFFERED, so a frontend
+ * fed 150k-point scans at 20 Hz would exhaust them in ~20 minutes.  A renumber pass subtracts the smallest live id from
+ * every stored id and from the id counter (order, contents and every (d2, id) comparison are unchanged).  far_map_insert*
+ * enqueues one by itself before the call that would pass `renumber_every` offered points since the last pass; the
+ * device reports the new counter through pinned host memory, so the host-side range check needs no synchronisation
+ * unless two passes would overlap.  Two stream-ordered launches. */
+int far_map_renumber(far_map_t* map, void* stream);
 
-/* Checkpoint / restore of a map's whole device state (table, buckets, covariances, counters, id counter).
- * create allocates the copy (a maintenance call); restore is six stream-ordered device copies, no sync. */
+/* Checkpoint / restore of a map's whole device state (table, bucket pool, free list, covariances, counters).
+ * create allocates the copy (a maintenance call); restore is seven stream-ordered device copies, no sync. */
 typedef struct far_snapshot far_snapshot_t;
 int far_map_snapshot_create(far_map_t* map, far_snapshot_t** out, void* stream);
 int far_map_snapshot_restore(far_map_t* map, const far_snapshot_t* snap, void* stream);
@@ -260,6 +289,10 @@ typedef struct far_frontend far_frontend_t;
 int far_frontend_create(far_frontend_t** out, const far_frontend_config_t* cfg);
 int far_frontend_destroy(far_frontend_t* f);
 far_map_t* far_frontend_map(far_frontend_t* f);   /* borrowed handle, e.g. to preload the map with far_map_insert */
+/* Statistics of the last frame's map update (accepted, new voxels, dropped because full, invalid) copied to HOST memory;
+ * synchronises the stream (a diagnostic read, not part of the frame).  A full submap is also reported as FAR_ERR_FULL
+ * (see the enum): exactly by far_frontend_process_host (it synchronises), from the mirrored flag by far_frontend_process */
+int far_frontend_insert_stats(far_frontend_t* f, far_insert_stats_t* h_out, void* stream);
 int far_frontend_process(far_frontend_t* f, const float* d_scan, int64_t n, int stride, const far_pose_t* init_pose,
                          double sigma, far_gicp_result_t* d_out, void* stream);
 int far_frontend_process_host(far_frontend_t* f, const float* h_scan, int64_t n, int stride,

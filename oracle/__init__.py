@@ -93,6 +93,7 @@ def lib():
         L.faro_map_insert.argtypes = [vp, vp, i64, C.c_int, vp, C.c_int, vp]
         L.faro_map_prune.argtypes = [vp, vp, f64, vp]
         L.faro_map_size.argtypes = [vp, vp, vp, vp]
+        L.faro_map_renumber.argtypes = [vp, vp]
         L.faro_map_export.argtypes = [vp, vp, vp, vp, vp, vp]
         L.faro_map_nn.argtypes = [vp, vp, i64, C.c_int, vp, vp, C.c_int]
         L.faro_map_nn_brute.argtypes = [vp, vp, i64, C.c_int, vp, vp]
@@ -261,6 +262,12 @@ class Map:
         nv, npnt, nid = C.c_int64(), C.c_int64(), C.c_uint64()
         _check(lib().faro_map_size(self._h, C.byref(nv), C.byref(npnt), C.byref(nid)))
         return nv.value, npnt.value, nid.value
+
+    def renumber(self):
+        """R22: ids -= smallest stored id; returns what was subtracted"""
+        sub = C.c_uint64()
+        _check(lib().faro_map_renumber(self._h, C.byref(sub)))
+        return sub.value
 
     def export(self, with_cov=False):
         nv = self.size()[0]

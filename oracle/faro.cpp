@@ -415,6 +415,21 @@ int faro_map_prune(faro_map_t* m, const double center[3], double radius, faro_pr
     return FARO_OK;
 }
 
+// R22: ids are this build's construct (the paper has none).  Renumbering subtracts the smallest stored id from
+// every stored id and from the id counter: order, contents and every (d2, id) comparison are unchanged.  An empty map
+// restarts at 0.
+int faro_map_renumber(faro_map_t* m, uint64_t* subtracted) {
+    if (!m) return FARO_ERR_ARG;
+    uint64_t mn = m->next_id;
+    for (auto& kv : m->vox)
+        for (const Pt& p : kv.second.pts) mn = std::min<uint64_t>(mn, p.id);
+    for (auto& kv : m->vox)
+        for (Pt& p : kv.second.pts) p.id -= (uint32_t)mn;
+    m->next_id -= mn;
+    if (subtracted) *subtracted = mn;
+    return FARO_OK;
+}
+
 int faro_map_size(const faro_map_t* m, int64_t* n_voxels, int64_t* n_points, uint64_t* next_id) {
     if (!m) return FARO_ERR_ARG;
     int64_t np = 0;

@@ -65,6 +65,8 @@ int faro_map_insert(faro_map_t*, const float* xyz, int64_t n, int stride, const 
                     int compute_cov, faro_insert_stats_t* stats);
 int faro_map_prune(faro_map_t*, const double center[3], double radius, faro_prune_stats_t* stats);
 int faro_map_size(const faro_map_t*, int64_t* n_voxels, int64_t* n_points, uint64_t* next_id);
+/* R22: subtract the smallest stored id from every stored id and from the id counter (empty map: counter -> 0) */
+int faro_map_renumber(faro_map_t*, uint64_t* subtracted);
 /* export sorted by key; points: n_voxels*cap*4 floats (x,y,z,id bits), unused entries zero/0xFFFFFFFF */
 int faro_map_export(const faro_map_t*, uint64_t* keys, int32_t* counts, float* points4,
                     float* cov6 /* nullable, n_voxels*cap*6 */, uint8_t* cov_valid /* nullable */);

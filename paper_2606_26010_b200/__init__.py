@@ -43,7 +43,8 @@ class Pose(C.Structure):
 
 class MapConfig(C.Structure):
     _fields_ = [("voxel_size", C.c_float), ("cap", C.c_int32), ("max_voxels", C.c_int64), ("max_load", C.c_float),
-                ("with_cov", C.c_int32), ("k_cov", C.c_int32), ("cov_eps", C.c_double), ("max_batch", C.c_int64)]
+                ("with_cov", C.c_int32), ("k_cov", C.c_int32), ("cov_eps", C.c_double), ("max_batch", C.c_int64),
+                ("renumber_every", C.c_int64)]
 
 
 class GicpOptions(C.Structure):
@@ -78,7 +79,8 @@ class Motion(C.Structure):
 
 INSERT_STATS_FIELDS = ("n_offered", "n_accepted", "n_new_voxels", "n_dropped_full", "n_invalid")
 PRUNE_STATS_FIELDS = ("n_voxels_removed", "n_points_removed", "n_voxels_left", "n_points_left")
-MAP_STATS_FIELDS = ("n_voxels", "n_points", "n_dead_keys", "n_slots", "next_id")
+MAP_STATS_FIELDS = ("n_voxels", "n_points", "n_dead_keys", "n_slots", "next_id", "n_keys", "n_free_buckets", "n_fresh_buckets",
+                    "n_rehash", "full")
 GICP_RESULT_BYTES = C.sizeof(GicpResult)
 POSE_BYTES = C.sizeof(Pose)
 
@@ -116,6 +118,9 @@ def lib():
             "far_map_prune_dev": (ci, [vp, vp, f64, vp, vp]),
             "far_map_stats": (ci, [vp, vp, vp]),
             "far_map_rehash": (ci, [vp, vp]),
+            "far_map_renumber": (ci, [vp, vp]),
+            "far_map_status": (ci, [vp]),
+            "far_frontend_insert_stats": (ci, [vp, vp, vp]),
             "far_map_snapshot_create": (ci, [vp, vp, vp]),
             "far_map_snapshot_restore": (ci, [vp, vp, vp]),
             "far_map_snapshot_destroy": (ci, [vp]),
@@ -164,9 +169,14 @@ def lib():
     return _lib
 
 
-def _check(rc, where):
+def _check(rc, where, full_ok=False):
+    """FAR_ERR_FULL from insert / frontend calls means "work enqueued, the map has dropped points" (far.h): those callers
+    pass full_ok and get the flag back instead of an exception."""
+    if rc == ERR_FULL and full_ok:
+        return True
     if rc != OK:
         raise FarError(rc, where)
+    return False
 
 
 def _stream():
@@ -288,13 +298,13 @@ class Map:
     """A far_map_t handle.  All bulk arguments are CUDA tensors (NumPy arrays are uploaded for convenience)."""
 
     def __init__(self, voxel, cap, max_voxels, with_cov=False, k_cov=10, cov_eps=1e-3, max_load=0.5, max_batch=1 << 20,
-                 _borrowed=None):
+                 renumber_every=0, _borrowed=None):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2606_26010_b200 needs a CUDA device: there is no CPU fallback")
         self.voxel, self.cap, self.k_cov, self.with_cov = float(voxel), int(cap), int(k_cov), bool(with_cov)
         self._owned = _borrowed is None
         if _borrowed is None:
-            cfg = MapConfig(voxel, cap, int(max_voxels), max_load, int(with_cov), k_cov, cov_eps, int(max_batch))
+            cfg = MapConfig(voxel, cap, int(max_voxels), max_load, int(with_cov), k_cov, cov_eps, int(max_batch), int(renumber_every))
             h = C.c_void_p()
             _check(lib().far_map_create(C.byref(h), C.byref(cfg)), "far_map_create")
             self._h = h
@@ -304,7 +314,8 @@ class Map:
         self.device = dev
         self._insert_stats = torch.zeros(5, dtype=torch.int64, device=dev)
         self._prune_stats = torch.zeros(4, dtype=torch.int64, device=dev)
-        self._map_stats = torch.zeros(5, dtype=torch.int64, device=dev)
+        self._map_stats = torch.zeros(len(MAP_STATS_FIELDS), dtype=torch.int64, device=dev)
+        self.full_seen = False
         self._result = torch.zeros(GICP_RESULT_BYTES, dtype=torch.uint8, device=dev)
 
     def close(self):
@@ -331,7 +342,7 @@ class Map:
         else:
             pp = C.byref(Pose.from_rt(pose)) if pose is not None else None
             rc = lib().far_map_insert(self._h, _ptr(x), n, s, pp, int(compute_cov), _ptr(self._insert_stats), _stream())
-        _check(rc, "far_map_insert")
+        self.full_seen = _check(rc, "far_map_insert", full_ok=True)
 
     def insert(self, xyz, pose=None, compute_cov=False):
         self.insert_enqueue(xyz, pose, compute_cov)
@@ -357,7 +368,7 @@ class Map:
             pp = C.byref(Pose.from_rt(pose)) if pose is not None else None
             rc = lib().far_map_insert_asmd(self._h, _ptr(x), n, s, pp, _ptr(d_n_close), float(d_max), int(compute_cov),
                                            _ptr(self._insert_stats), _stream())
-        _check(rc, "far_map_insert_asmd")
+        self.full_seen = _check(rc, "far_map_insert_asmd", full_ok=True)
         self._keep = d_n_close
 
     def insert_asmd(self, xyz, n_close, d_max, pose=None, compute_cov=False):
@@ -405,6 +416,14 @@ class Map:
 
     def rehash(self):
         _check(lib().far_map_rehash(self._h, _stream()), "far_map_rehash")
+
+    def renumber(self):
+        """far_map_renumber (R22): ids -= smallest live id; no host sync."""
+        _check(lib().far_map_renumber(self._h, _stream()), "far_map_renumber")
+
+    def status(self):
+        """far_map_status: OK or ERR_FULL from the host-visible mirror of the device flag (never synchronises)."""
+        return int(lib().far_map_status(self._h))
 
     def export(self, with_cov=False):
         """Live voxels sorted by key (the library's order is unspecified; sorting is presentation only)."""
@@ -496,7 +515,7 @@ class Frontend:
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2606_26010_b200 needs a CUDA device: there is no CPU fallback")
         o = opts if opts is not None else default_options()
-        cfg = FrontendConfig(MapConfig(voxel, cap, int(max_voxels), max_load, 1, k_cov, cov_eps, 0), ds_voxel,
+        cfg = FrontendConfig(MapConfig(voxel, cap, int(max_voxels), max_load, 1, k_cov, cov_eps, 0, 0), ds_voxel,
                              int(max_scan_points), float(prune_radius), int(max_iters), int(update_map), o,
                              int(asmd), float(asmd_r_close), float(asmd_d_max))
         h = C.c_void_p()
@@ -505,6 +524,7 @@ class Frontend:
         self.map = Map(voxel, cap, max_voxels, with_cov=True, k_cov=k_cov, _borrowed=C.c_void_p(lib().far_frontend_map(h)))
         self.max_scan_points = int(max_scan_points)
         self.h_result = GicpResult()
+        self.full_seen = False
 
     def close(self):
         if getattr(self, "_h", None):
@@ -522,8 +542,8 @@ class Frontend:
         """Device scan in, result struct stays on the device; no host synchronisation."""
         x, n, s = _points(d_scan)
         po = Pose.from_rt(init_pose) if not isinstance(init_pose, Pose) else init_pose
-        _check(lib().far_frontend_process(self._h, _ptr(x), n, s, C.byref(po), float(sigma), _ptr(d_result), _stream()),
-               "far_frontend_process")
+        self.full_seen = _check(lib().far_frontend_process(self._h, _ptr(x), n, s, C.byref(po), float(sigma), _ptr(d_result),
+                                                           _stream()), "far_frontend_process", full_ok=True)
 
     def process_sweep_enqueue(self, d_scan, d_time, dt_ref, a, b, init_pose, sigma, d_result=None):
         """Raw sweep + per-point time offsets in: far_undistort, then the chain of process_enqueue."""
@@ -531,8 +551,9 @@ class Frontend:
         assert d_time.dtype == torch.float32 and d_time.shape == (n,) and d_time.is_cuda
         po = Pose.from_rt(init_pose) if not isinstance(init_pose, Pose) else init_pose
         m = Motion.from_ab(a, b)
-        _check(lib().far_frontend_process_sweep(self._h, _ptr(x), _ptr(d_time), n, s, float(dt_ref), C.byref(m), C.byref(po),
-                                                float(sigma), _ptr(d_result), _stream()), "far_frontend_process_sweep")
+        self.full_seen = _check(lib().far_frontend_process_sweep(self._h, _ptr(x), _ptr(d_time), n, s, float(dt_ref), C.byref(m),
+                                                                 C.byref(po), float(sigma), _ptr(d_result), _stream()),
+                                "far_frontend_process_sweep", full_ok=True)
 
     def process_host(self, h_scan, init_pose, sigma):
         """HOST scan (a pinned torch CPU tensor or a NumPy array) in, result dict out; uploads, runs, downloads, syncs."""
@@ -543,9 +564,16 @@ class Frontend:
             h_scan = np.ascontiguousarray(h_scan, dtype=np.float32)
             ptr, n, s = C.c_void_p(h_scan.ctypes.data), h_scan.shape[0], h_scan.shape[1]
         po = Pose.from_rt(init_pose) if not isinstance(init_pose, Pose) else init_pose
-        _check(lib().far_frontend_process_host(self._h, ptr, n, s, C.byref(po), float(sigma), C.byref(self.h_result), _stream()),
-               "far_frontend_process_host")
+        self.full_seen = _check(lib().far_frontend_process_host(self._h, ptr, n, s, C.byref(po), float(sigma),
+                                                                C.byref(self.h_result), _stream()),
+                                "far_frontend_process_host", full_ok=True)
         return result_to_dict(self.h_result)
+
+    def insert_stats(self):
+        """far_frontend_insert_stats: statistics of the last frame's map update (synchronising read of the device struct)."""
+        buf = (C.c_int64 * 5)()
+        _check(lib().far_frontend_insert_stats(self._h, buf, _stream()), "far_frontend_insert_stats")
+        return dict(zip(INSERT_STATS_FIELDS, list(buf)))
 
 
 def _dp(a):

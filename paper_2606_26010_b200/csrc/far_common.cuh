@@ -1,20 +1,24 @@
 // far_common.cuh -- device-side building blocks shared by the far_* kernels (sm_100a).
 //
-// Layout of the voxel hashmap in HBM (PAPER.md:62-68 "cuVoxelMap"; re-designed for B200, see DESIGN.md):
-//   table   : Entry[slots]            16 B per slot {u64 key, u32 count, u32 reach}; one LDG.128 yields the key
-//                                     AND the number of points, so a lookup is two dependent memory levels
-//                                     (entry -> points), not three.
-//   points  : float4[slots * cap]     bucket of slot s = points[s*cap .. s*cap+cap); .w = id bits.  The bucket
-//                                     index IS the slot index (no indirection, no allocator); positions >= count
-//                                     are never read.
-//   ids     : u32[slots * cap]        the id of stored point j of slot s at ids[s*cap + j], FAR_NO_ID if the position is
-//                                     free.  A compact copy of the .w words: it is the working storage of the
-//                                     deterministic insert, whose chain then touches 80 contiguous bytes (one to three
-//                                     32-byte sectors) per voxel instead of up to ten sectors of the float4 bucket.
-//   cov     : float[slots * cap * 6]  (optional) regularised covariance of each stored point (Eq. 1)
-//   cov_ok  : u8[slots * cap]         (optional) 1 if that covariance is valid (>= k neighbours)
-// A pruned voxel keeps its key with count = 0 ("dead key"): it behaves exactly like an absent voxel for every
-// query and is re-used if the voxel is created again, so inserts never have to reason about tombstones.
+// Layout of the voxel hashmap in HBM (PAPER.md:62-68 "cuVoxelMap"; re-designed for B200, see DESIGN.md section 5):
+//   table   : Entry[slots]              16 B per slot {u64 key, u32 bucket, u32 count | reach << 8}; one LDG.128 yields the
+//                                       key, where its points live AND how many there are, so a lookup is two dependent
+//                                       memory levels (entry -> points), not three.
+//   shadow  : Entry[slots]              second table of the same size, empty between calls: the target of the in-place
+//                                       rehash that drops the keys of pruned voxels (rehash_*_kernel in far_map.cu)
+//   points  : float4[max_voxels * cap]  DENSE bucket pool (Fig. 3: points stored apart from the key table);
+//                                       bucket b = points[b*cap .. b*cap+cap); .w = id bits; positions >= count never read.
+//                                       Buckets come from a bump allocator and a free list refilled by pruning, so V live
+//                                       voxels occupy V * cap * 16 B contiguous-ish bytes whatever the table size.
+//   ids     : u32[max_voxels * cap]     the id of stored point j of bucket b at ids[b*cap + j], FAR_NO_ID if the position
+//                                       is free: the working storage of the deterministic insert (its atomicMin chain
+//                                       touches 80 contiguous bytes per voxel at cap 20)
+//   cov     : float[max_voxels*cap*6]   (optional) regularised covariance of each stored point (Eq. 1)
+//   cov_ok  : u8[max_voxels * cap]      (optional) 1 if that covariance is valid (>= k neighbours)
+//   free    : u32[max_voxels]           stack of bucket indices returned by far_map_prune
+// A pruned voxel gives its bucket back at once; its key stays in the table with bucket = NO_BUCKET ("dead key": absent for
+// every query, re-usable by an insert) until the number of dead keys passes a device-side threshold, at which point the
+// prune call itself rebuilds the 16-byte entries into `shadow` and copies them back -- no allocation, no host sync.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -26,48 +30,91 @@ namespace far {
 constexpr unsigned long long KEY_EMPTY = ~0ull;
 constexpr uint32_t NO_ID = 0xFFFFFFFFu;
 constexpr uint32_t NO_SLOT = 0xFFFFFFFFu;
+constexpr uint32_t NO_BUCKET = 0xFFFFFFFFu;        // key present, no points (never had any, or pruned)
+constexpr uint32_t BUCKET_PENDING = 0xFFFFFFFEu;   // a thread is allocating this voxel's bucket right now
 constexpr int KEY_BIAS = 1 << 20;
 constexpr unsigned FULL = 0xFFFFFFFFu;
 
 struct __align__(16) Entry {
     unsigned long long key;
-    uint32_t count;
-    uint32_t pad;      // reach of this HOME slot: 1 + largest displacement of a key hashing here (see find_voxel)
+    uint32_t bucket;   // index into the dense pool, NO_BUCKET, or BUCKET_PENDING (only while an insert kernel runs)
+    uint32_t cr;       // bits 0..7: number of stored points; bits 8..31: reach of this HOME slot = 1 + the largest
+                       // displacement of any key whose home slot this is (see find_voxel)
 };
 
 // device counters of one map (all zeroed at create / clear)
 struct Counters {
-    unsigned long long n_keys;        // claimed keys (live + dead)
-    unsigned int full_flag;           // sticky: a point was dropped because the table was full
-    unsigned int pad;                 // ticket of prune_kernel's last-block-done epilogue (0 between launches)
-    // n_touched .. st_invalid are contiguous: one memset at the start of an insert call zeroes them all
+    unsigned long long next_id;       // id of the next offered point (device-resident: no per-call kernel argument)
+    unsigned long long call_first_id; // first id of the insert call whose last chunk was committed most recently
+    unsigned int n_keys;              // claimed keys (live + dead)
+    unsigned int n_dead;              // keys whose voxel was pruned since the last rehash
+    unsigned int bump;                // buckets ever taken from the fresh end of the pool
+    int n_free;                       // entries on the free list (transiently negative inside an insert kernel)
+    unsigned int full_flag;           // sticky until buckets are freed: a point was dropped (pool or table exhausted)
+    unsigned int rehash_flag;         // written by prune's epilogue: the two rehash kernels that follow do their work
+    unsigned int rehash_moved;        // entries moved by the running rehash
+    unsigned int n_rehash;            // rehashes done since create / clear
+    unsigned int ticket[4];           // last-block-done tickets: 0 insert commit, 1 prune, 2 clear, 3 renumber
     unsigned int n_touched;           // voxels that received a first new point in the current chunk
-    unsigned int n_cov;               // accepted points queued for covariance in the current call
+    unsigned int n_tasks;             // covariance tasks (touched voxels) left by the last commit for knn_cov_tasks_kernel
+    unsigned int min_id;              // far_map_renumber: smallest live id
+    unsigned int pad0;
     unsigned long long st_accepted, st_new_voxels, st_dropped_full, st_invalid;   // per-call statistics
     unsigned long long pr_vox_removed, pr_pts_removed, pr_vox_left, pr_pts_left;  // per-prune statistics
+    unsigned long long scratch[8];    // stats / export / ASMD accumulators
+};
+
+// written by the device into pinned, mapped HOST memory: lets later host calls report conditions without a sync
+struct Mailbox {
+    volatile uint32_t full;             // mirrors Counters::full_flag
+    volatile uint32_t renumber_seq;     // number of far_map_renumber passes completed
+    volatile unsigned long long next_id_after_renumber;
+    volatile unsigned long long offered_at_renumber;   // host-side offered-points counter the pass was enqueued at
 };
 
 // device view of a map, passed by value to kernels
 struct MapView {
     Entry* table;
+    Entry* shadow;
     float4* points;
     uint32_t* ids;
     float* cov;          // nullable
     uint8_t* cov_ok;     // nullable
+    uint32_t* free_list;
     Counters* ctr;
+    Mailbox* mail;       // device pointer to the mapped host mailbox
     uint32_t mask;       // slots - 1
     uint32_t slots;
+    uint32_t max_buckets;
+    uint32_t key_limit;  // new keys are refused beyond this many claimed slots (probe lengths stay bounded)
     int cap;
     int k_cov;
     float voxel;
     double cov_eps;
-    unsigned long long max_keys;
 };
 
 struct Pose {
     double R[9];
     double t[3];
 };
+
+__device__ __forceinline__ uint32_t entry_count(uint32_t cr) { return cr & 0xFFu; }
+__device__ __forceinline__ uint32_t entry_reach(uint32_t cr) { return cr >> 8; }
+
+// true in exactly one block of the grid: the one whose thread 0 takes the last ticket, after every other block has
+// passed this point (its earlier writes are fenced).  All threads of the block must call; the ticket re-arms itself.
+__device__ __forceinline__ bool last_block_done(unsigned int* ticket) {
+    __shared__ bool s_last;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const bool last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+        if (last) { *ticket = 0u; __threadfence(); }
+        s_last = last;
+    }
+    __syncthreads();
+    return s_last;
+}
 
 // ---- A1: voxel key (R1).  One IEEE fp32 division, floor, 21-bit biased pack. -------------
 __device__ __forceinline__ bool voxel_index(float x, float y, float z, float v, int k[3]) {
@@ -130,40 +177,41 @@ __device__ __forceinline__ Entry load_entry(const Entry* table, uint32_t s) {
     const uint4 raw = __ldg(reinterpret_cast<const uint4*>(table + s));
     Entry e;
     e.key = ((unsigned long long)raw.y << 32) | raw.x;
-    e.count = raw.z;
-    e.pad = raw.w;
+    e.bucket = raw.z;
+    e.cr = raw.w;
     return e;
 }
 
-// read-only lookup: slot of `key` and its count, or count = 0 if absent / dead.  Linear probing, step 1.
-// The spare word of the entry at a key's HOME slot h holds `reach` = 1 + the largest displacement of any key whose home
-// is h (raised with atomicMax when a key is claimed).  A lookup therefore examines at most reach(h) slots: a voxel that
-// is not in the map -- 11 of the 27 neighbours of a typical query -- is usually dismissed by the one home-entry load
-// (no key has that home: reach = 0) instead of a walk to the next empty slot, and the warp no longer waits for the
-// longest of 27 such walks.  (Requesting several consecutive entries per step was measured and rejected:
-// profiles/probe_group_r01d.md.)
+// read-only lookup: bucket of `key` and its count, or NO_BUCKET / count = 0 if absent or dead.  Linear probing, step 1
+// (PAPER.md:62).  The upper 24 bits of the entry at a key's HOME slot h hold `reach` = 1 + the largest displacement of any
+// key whose home is h (raised when a key is claimed, recomputed by every rehash).  A lookup therefore examines at most
+// reach(h) slots: a voxel that is not in the map -- 11 of the 27 neighbours of a typical query -- is usually dismissed by
+// the one home-entry load instead of a walk to the next empty slot, and the warp no longer waits for the longest of 27
+// such walks.  An EMPTY home slot means no key has that home (keys are only ever removed by a rebuild).
 __device__ __forceinline__ uint32_t find_voxel(const MapView& m, unsigned long long key, uint32_t& count) {
     const uint32_t h = hash_key(key) & m.mask;
     Entry e = load_entry(m.table, h);
-    const uint32_t reach = e.pad;
-    uint32_t s = h;
+    count = 0;
+    if (e.key == KEY_EMPTY) return NO_BUCKET;
+    const uint32_t reach = entry_reach(e.cr);
     for (uint32_t d = 0; d < reach; ++d) {
         if (d) {
-            s = (h + d) & m.mask;
-            e = load_entry(m.table, s);
+            e = load_entry(m.table, (h + d) & m.mask);
+            if (e.key == KEY_EMPTY) break;
         }
-        if (e.key == key) { count = e.count; return s; }
-        if (e.key == KEY_EMPTY) break;
+        if (e.key == key) {
+            count = entry_count(e.cr);
+            return count ? e.bucket : NO_BUCKET;
+        }
     }
-    count = 0;
-    return NO_SLOT;
+    return NO_BUCKET;
 }
 
 // lexicographic (d2, id) candidate; d2 >= 0 so its bit pattern orders like the value
 struct Best {
     double d2;
     uint32_t id;
-    uint32_t ref;     // slot*cap + position of the stored point
+    uint32_t ref;     // bucket*cap + position of the stored point
 };
 
 __device__ __forceinline__ bool better(double d2, uint32_t id, const Best& b) {
@@ -198,9 +246,9 @@ __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
 }
 
 // The 27-voxel probe of one query by one warp (Fig. 3): lane l < 27 looks up neighbour
-// (l/9-1, (l/3)%3-1, l%3-1) and keeps its slot and count in registers.  All 32 lanes must call.
+// (l/9-1, (l/3)%3-1, l%3-1) and keeps its bucket and count in registers.  All 32 lanes must call.
 __device__ __forceinline__ void probe27_regs(const MapView& m, const int k[3], int lane, uint32_t& cnt, uint32_t& slot) {
-    cnt = 0; slot = NO_SLOT;
+    cnt = 0; slot = NO_BUCKET;
     if (lane < 27) {
         const int nx = k[0] + lane / 9 - 1, ny = k[1] + (lane / 3) % 3 - 1, nz = k[2] + lane % 3 - 1;
         if (index_in_range(nx) && index_in_range(ny) && index_in_range(nz)) slot = find_voxel(m, pack_key(nx, ny, nz), cnt);
@@ -216,7 +264,7 @@ __device__ __forceinline__ void probe27_regs(const MapView& m, const int k[3], i
 constexpr int CAND_STEPS = 27 * 64 / 32;    // cap <= 64
 struct __align__(16) CandList {
     int off[32];                 // first candidate index of compact voxel c
-    uint32_t slot[32];           // its table slot
+    uint32_t slot[32];           // its bucket
     uint32_t mask[CAND_STEPS];   // voxel-start bits of step c
 };
 

@@ -31,7 +31,6 @@
 // amplifies a 1e-16 change of one increment to 2 fp32 ulps of a stored coordinate within 12 frames, along the
 // unobservable direction of the corridor.
 // The host is not involved until it reads the result.
-#include <atomic>
 #include <cstring>
 
 #include "far_internal.h"
@@ -54,7 +53,7 @@ constexpr int MAX_ITERS_LIMIT = 1000;   // the iteration index shares the 32-bit
 struct GicpScratch {
     uint4* rows;      // [max_grid][TSTRIDE]
     uint4* grows;     // [MAX_GROUPS][TSTRIDE]
-    uint4* pub;       // [16]
+    uint4* pub;       // [16]: 13 published words; pub[15].x = launch sequence of this map (device-resident)
 };
 
 // one transformed source point, written by one lane of warp 0 in phase A0, read by its warp in phase A
@@ -73,18 +72,6 @@ struct Corr {
     int flags;        // bit 0: correspondence accepted, bit 1: both covariances valid
 };
 
-#ifdef FAR_GICP_TRACE
-// Debug-only timing probes (never compiled into the product library): globaltimer stamps per iteration.
-__device__ unsigned long long g_trace[64][8];
-__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-#define TRACE_MIN(it, slot) do { if (threadIdx.x == 0 && (it) < 64) atomicMin(&g_trace[it][slot], gtime()); } while (0)
-#define TRACE_MAX(it, slot) do { if (threadIdx.x == 0 && (it) < 64) atomicMax(&g_trace[it][slot], gtime()); } while (0)
-#define TRACE_ADD(it, slot) do { if (threadIdx.x == 0 && (it) < 64) atomicAdd(&g_trace[it][slot], gtime() & 0xFFFFFFFFull); } while (0)
-#else
-#define TRACE_MIN(it, slot)
-#define TRACE_MAX(it, slot)
-#define TRACE_ADD(it, slot)
-#endif
 
 struct GicpParams {
     const float* scan;
@@ -97,7 +84,6 @@ struct GicpParams {
     const Pose* d_init;
     double tau2, kappa, conv_eps;
     int kernel, max_iters, linearize_only;
-    uint32_t seq;               // launch sequence number (upper bits of every tag)
     GicpScratch scratch;
     far_gicp_result_t* out;
 };
@@ -361,6 +347,9 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(M
     __shared__ int s_done;
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const int64_t nwarps = (int64_t)gridDim.x * GWARPS;
+    // launch sequence: read by every block at start, advanced by block 0 at the very end (launches on one map are
+    // stream-ordered), so every launch has its own tag space without a host-side counter or a kernel argument
+    const uint32_t seq = *reinterpret_cast<volatile uint32_t*>(&P.scratch.pub[15].x);
     int64_t n = P.n;
     if (P.d_n) n = min(n, *P.d_n);
     if (threadIdx.x < 12) {
@@ -397,8 +386,7 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(M
     }
 
     for (int it = 0; it < P.max_iters; ++it) {
-        const uint32_t tag = (P.seq << 10) | (uint32_t)(it + 1);
-        TRACE_MIN(it, 0);
+        const uint32_t tag = (seq << 10) | (uint32_t)(it + 1);
         double acc = 0.0;                                     // warp 0, lane t < 29: term t of this block
         for (int rd = 0; rd < rounds; ++rd) {
             // ---- phase A0 (Eq. 2, A1): 8 lanes of warp 0 transform the block's 8 source points with the accumulated pose
@@ -460,7 +448,6 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(M
             }
             if (lane == 0) s_corr[wib].flags = flags;
             __syncthreads();
-            TRACE_MAX(it, 2);
             // ---- phase B (A9): 8 lanes of warp 0 linearise the block's 8 correspondences together --------------------
             if (wib == 0) {
                 if (lane < GWARPS) {
@@ -483,7 +470,6 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(M
             }
             if (rd + 1 < rounds) __syncthreads();             // the records are rewritten by the next round
         }
-        TRACE_MAX(it, 1);
         // ---- A10: block row -> group of 32 blocks -> grid, tagged words, every level summed in a fixed order --------
         if (wib == 0) put_tagged(P.scratch.rows + (size_t)blockIdx.x * TSTRIDE + lane, lane < NTERMS ? acc : 0.0, tag);
         if (blockIdx.x % GROUP == 0) {   // group leader: fold the group's rows into one
@@ -493,7 +479,6 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(M
                 const double t2 = block_sum_tagged(P.scratch.grows, 0, n_groups, tag, lane, wib, s_red);
                 if (wib == 0) s_terms[0][lane] = t2;
                 __syncthreads();
-                TRACE_MAX(it, 3);
                 if (threadIdx.x == 0) {
                     Pose Tn;
                     const bool done = solve_and_update(P, s_terms[0], s_T, it, Tn);
@@ -503,7 +488,6 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(M
                     for (int a = 0; a < 3; ++a) put_tagged(P.scratch.pub + 9 + a, Tn.t[a], tag);
                     put_tagged(P.scratch.pub + 12, done ? 1.0 : 0.0, tag);
                 }
-                TRACE_MAX(it, 4);
             }
         }
         // ---- grid-wide wait for the new pose: all blocks are co-resident (cooperative launch) -----------------------
@@ -529,8 +513,21 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(M
             else if (lane == 12) s_done = vv != 0.0 ? 1 : 0;
         }
         __syncthreads();
-        TRACE_MAX(it, 5);
         if (s_done) break;
+    }
+    // every block has read `seq` before it could pass the first grid-wide wait, which block 0 is now behind
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        uint32_t next = (seq + 1u) & 0x3FFFFFu;
+        if (next == 0u) {
+            // wrap-around of the 22-bit sequence (once per 4 M launches): wipe the block and group rows so that no word
+            // written 4 M launches ago can be mistaken for a current one (every row this launch needed has been read: the
+            // solve came after them; the published words are rewritten by every launch and stay).  Tag 0 is never used
+            const size_t words = (size_t)(P.scratch.pub - P.scratch.rows);
+            for (size_t w = 0; w < words; ++w) P.scratch.rows[w] = make_uint4(0u, 0u, 0u, 0u);
+            next = 1u;
+        }
+        __threadfence();
+        *reinterpret_cast<volatile uint32_t*>(&P.scratch.pub[15].x) = next;
     }
 }
 
@@ -545,8 +542,6 @@ void far_gicp_default_options(far_gicp_options_t* o) {
     o->tau_mult = 3.0;
     o->kappa_div = 3.0;
 }
-
-static size_t gicp_scratch_bytes(int max_grid) { return ((size_t)(max_grid + MAX_GROUPS) * TSTRIDE + 16) * sizeof(uint4); }
 
 static int gicp_launch(const far_map_t* map, const float* d_scan, const float* d_cov6, const uint8_t* d_valid, int64_t n,
                        const int64_t* d_n, int stride, const far_pose_t* hpose, const far_pose_t* d_pose, double sigma,
@@ -576,15 +571,6 @@ static int gicp_launch(const far_map_t* map, const float* d_scan, const float* d
     const int64_t need = (n + GWARPS - 1) / GWARPS;
     if (need < grid) grid = need;
     if (grid < 1) grid = 1;
-    // every launch gets its own tag space; on wrap-around of the 22-bit sequence the scratch is wiped once so that no
-    // word written 4 M launches ago can be mistaken for a current one
-    static std::atomic<uint32_t> g_seq{0};
-    uint32_t seq = g_seq.fetch_add(1, std::memory_order_relaxed) + 1;
-    if ((seq & 0x3FFFFFu) == 0) {
-        FAR_CUDA(cudaMemsetAsync(map->d_gicp_partials, 0, gicp_scratch_bytes(map->gicp_max_grid), st));
-        seq = g_seq.fetch_add(1, std::memory_order_relaxed) + 1;
-    }
-    P.seq = seq & 0x3FFFFFu;
     MapView view = map->view;
     void* args[] = {(void*)&view, (void*)&P};
     {
@@ -624,19 +610,12 @@ int far_gicp_register_dn(const far_map_t* map, const float* d_scan, const float*
     return gicp_launch(map, d_scan, d_cov6, d_valid, n_max, d_n, stride, init_pose, nullptr, sigma, max_iters, 0, opts, d_out, stream);
 }
 
-#ifdef FAR_GICP_TRACE
-// debug build only: reset (all slots 0, min-slot ~0) / read the probes
-void far_gicp_trace_reset(void) {
-    unsigned long long h[64][8];
-    for (int i = 0; i < 64; ++i) for (int j = 0; j < 8; ++j) h[i][j] = (j == 0) ? ~0ull : 0ull;
-    cudaMemcpyToSymbol(far::g_trace, h, sizeof(h));
-}
-void far_gicp_trace_read(unsigned long long* out) { cudaMemcpyFromSymbol(out, far::g_trace, sizeof(unsigned long long) * 64 * 8); }
-#endif
 
 }  // extern "C"
 
 namespace far {
+static size_t gicp_scratch_bytes(int max_grid) { return ((size_t)(max_grid + MAX_GROUPS) * TSTRIDE + 16) * sizeof(uint4); }
+
 // called once from far_map_create: sizes the cooperative grid and allocates the reduction scratch
 int gicp_setup(far_map* map) {
     int per_sm = 0;
@@ -644,9 +623,12 @@ int gicp_setup(far_map* map) {
     if (per_sm < 1) per_sm = 1;
     map->gicp_max_grid = map->sm_count * per_sm;
     if (map->gicp_max_grid > GROUP * MAX_GROUPS) map->gicp_max_grid = GROUP * MAX_GROUPS;
-    const size_t bytes = ((size_t)(map->gicp_max_grid + MAX_GROUPS) * TSTRIDE + 16) * sizeof(uint4);
+    const size_t bytes = gicp_scratch_bytes(map->gicp_max_grid);
     FAR_CUDA(cudaMalloc((void**)&map->d_gicp_partials, bytes));
     FAR_CUDA(cudaMemset(map->d_gicp_partials, 0, bytes));     // tag 0 is never used by a launch
+    const uint32_t one = 1u;                                   // launch sequence starts at 1 (pub[15].x)
+    FAR_CUDA(cudaMemcpy(reinterpret_cast<uint4*>(map->d_gicp_partials) + (size_t)(map->gicp_max_grid + MAX_GROUPS) * TSTRIDE + 15,
+                        &one, sizeof(one), cudaMemcpyHostToDevice));
     return FAR_OK;
 }
 }  // namespace far

@@ -1,8 +1,9 @@
-// far_map.cu -- the voxel hashmap: create / clear / deterministic capped insert / prune / export / stats.
+// far_map.cu -- the voxel hashmap: create / clear / deterministic capped insert / prune + in-place rehash / export / stats.
 //
 // PAPER.md:62-68 (cuVoxelMap: custom key = 3D voxel indices, linear probing, <= N_max points per voxel, built
 // for concurrent access), PAPER.md:109 (submap update: insert at T_L with a per-voxel cap, recompute the
-// covariances of added points only, remove voxels beyond a range limit).
+// covariances of added points only, remove voxels beyond a range limit), PAPER.md:171,186 (everything
+// preallocated: allocations show up as latency peaks).
 //
 // Deterministic capped insert (reading R3: the result equals inserting the points one by one in index order).
 // A bare atomicAdd ticket gives the right counts but timing-dependent contents, so instead each offered point
@@ -15,6 +16,11 @@
 // smaller than the batch's ids (ids grow monotonically), so they stay where they are.  A second kernel walks
 // the voxels that received a point, fetches the coordinates of the surviving ids (index = id - first id of
 // the chunk) and writes them next to their id.
+//
+// Storage (far_common.cuh): 16-byte table entries {key, bucket, count | reach}, buckets in a DENSE pool handed out by a
+// bump allocator + free list.  Pruning returns buckets at once and leaves dead keys behind; when their number passes a
+// device-side threshold the prune call's two follow-up kernels rebuild the entries into the shadow table and copy them
+// back.  Nothing on this path allocates, frees or synchronises.
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -38,6 +44,43 @@ __device__ __forceinline__ bool load_pose_point(const float* __restrict__ xyz, i
     if (pose_mode) transform_point(T, x, y, z, p);
     else { p[0] = x; p[1] = y; p[2] = z; }
     return true;
+}
+
+__device__ __forceinline__ uint32_t ld_volatile(const uint32_t* p) { return *reinterpret_cast<const volatile uint32_t*>(p); }
+
+// raise the reach of home slot h to at least r, leaving the count byte alone (rare: once per claimed key)
+__device__ __forceinline__ void raise_reach(Entry* table, uint32_t h, uint32_t r) {
+    uint32_t* w = &table[h].cr;
+    uint32_t old = ld_volatile(w);
+    while (entry_reach(old) < r) {
+        const uint32_t seen = atomicCAS(w, old, (r << 8) | (old & 0xFFu));
+        if (seen == old) break;
+        old = seen;
+    }
+}
+
+// find `key` or claim an empty slot for it: 64-bit atomicCAS on the key word, linear probing step 1.
+// Returns NO_SLOT if the key is absent and the table takes no more keys.
+__device__ __forceinline__ uint32_t find_or_claim(Entry* table, uint32_t mask, uint32_t slots, unsigned long long key,
+                                                  bool may_claim, bool& claimed) {
+    const uint32_t h = hash_key(key) & mask;
+    uint32_t s = h;
+    claimed = false;
+    for (uint32_t probes = 0; probes < slots; ++probes) {
+        unsigned long long cur = *reinterpret_cast<volatile unsigned long long*>(&table[s].key);
+        if (cur == KEY_EMPTY) {
+            if (!may_claim || probes >= 0xFFFFFEu) return NO_SLOT;
+            cur = atomicCAS(&table[s].key, KEY_EMPTY, key);
+            if (cur == KEY_EMPTY) {
+                claimed = true;
+                raise_reach(table, h, probes + 1u);   // keep the reach of the key's home slot up to date (find_voxel)
+                return s;
+            }
+        }
+        if (cur == key) return s;
+        s = (s + 1) & mask;
+    }
+    return NO_SLOT;
 }
 
 // ---- Adaptive Submap Density (R17) -----------------------------------------------------
@@ -66,175 +109,232 @@ __device__ __forceinline__ uint32_t voxel_limit(const MapView& m, const Asmd& A,
     return min(lim, (uint32_t)m.cap);
 }
 
-// ---- insert, kernel 1: key -> find-or-claim -> atomicMin chain ---------------------------------------
+// ---- insert, kernel 1: key -> find-or-claim -> bucket -> atomicMin chain --------------------------------------------
+// All 32 lanes of a warp stay in the kernel to its end (no early return), so every collective below uses the full mask.
+// Lanes that offer points to the SAME voxel (a LiDAR ring crossing a voxel gives a run of consecutive ids; 73 % of a C2
+// scan falls into voxels that are offered more than cap points, up to 700) elect one leader: only the leader walks the
+// table, and the lanes' ranks `ahead` let each id enter the chain at c0 + ahead instead of at c0 (exact: an id may enter
+// anywhere at or before its final position -- every position still ends up with the minimum of the ids that reach it --
+// and it removes most of the shifting); if c0 + ahead is already past the limit the point cannot survive at all.
 __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, const float* __restrict__ xyz, int64_t n,
                                                                   int stride, int pose_mode, Pose hpose,
-                                                                  const Pose* __restrict__ d_pose, uint32_t first_id,
+                                                                  const Pose* __restrict__ d_pose, uint32_t id_offset,
                                                                   uint32_t* __restrict__ touched, Asmd asmd) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
+    const int lane = threadIdx.x & 31;
+    const unsigned lt = (1u << lane) - 1u;
     const Pose& T = (pose_mode == 2) ? *d_pose : hpose;
-    // the key count is read once, up front (its latency hides behind the point load); the limit is enforced up to the
-    // keys claimed while this kernel runs -- which excess voxels are dropped is unspecified anyway (R3)
-    const unsigned long long keys_before = *reinterpret_cast<volatile unsigned long long*>(&m.ctr->n_keys);
+    Counters* ctr = m.ctr;
     float p[3];
-    int k[3];
-    if (!load_pose_point(xyz, i, stride, pose_mode, T, p) || !voxel_index(p[0], p[1], p[2], m.voxel, k)) {
-        atomicAdd(&m.ctr->st_invalid, 1ull);
-        return;
+    int k[3] = {0, 0, 0};
+    bool valid = false, bad = false;
+    if (i < n) {
+        valid = load_pose_point(xyz, i, stride, pose_mode, T, p) && voxel_index(p[0], p[1], p[2], m.voxel, k);
+        bad = !valid;
     }
-    const unsigned long long key = pack_key(k[0], k[1], k[2]);
-    // Lanes of this warp that offer points to the SAME voxel (a LiDAR ring crossing a voxel gives a run of consecutive
-    // ids; 73 % of a C2 scan falls into voxels that are offered more than cap points, up to 700).  Ids grow with the
-    // lane, so `ahead` of them are smaller than mine: my final position is at least c0 + ahead.  Entering the chain
-    // there instead of at c0 is exact (an id may enter anywhere at or before its final position: every position still
-    // ends up with the minimum of the ids that reach it) and removes most of the shifting; if c0 + ahead is already
-    // past the limit the point cannot survive at all.
-    const unsigned same = __match_any_sync(__activemask(), key);
-    const uint32_t ahead = __popc(same & ((1u << (threadIdx.x & 31)) - 1u));
-    // find or claim the voxel's slot: 64-bit atomicCAS on the key word, linear probing step 1
-    uint32_t s = hash_key(key) & m.mask;
-    bool found = false, new_key = false;
-    for (uint32_t probes = 0; probes < m.slots; ++probes) {
-        unsigned long long cur = *reinterpret_cast<volatile unsigned long long*>(&m.table[s].key);
-        if (cur == KEY_EMPTY) {
-            if (keys_before >= m.max_keys) break;   // table full
-            cur = atomicCAS(&m.table[s].key, KEY_EMPTY, key);
-            if (cur == KEY_EMPTY) {
-                new_key = true;
-                found = true;
-                // keep the reach of the key's home slot up to date (far_common.cuh::find_voxel)
-                atomicMax(&m.table[hash_key(key) & m.mask].pad, probes + 1u);
-                break;
+    // invalid lanes get distinct fake keys (bit 63 is never set by a valid key)
+    const unsigned long long key = valid ? pack_key(k[0], k[1], k[2]) : ((1ull << 63) | (unsigned long long)lane);
+    const unsigned same = __match_any_sync(FULL, key);
+    const int leader = __ffs(same) - 1;
+    const uint32_t ahead = __popc(same & lt);
+    const bool is_leader = valid && lane == leader;
+
+    // phase 1: the leader finds or claims the voxel's table slot
+    uint32_t s = NO_SLOT;
+    bool claimed = false;
+    if (is_leader) {
+        const bool may_claim = ld_volatile(&ctr->n_keys) < m.key_limit;   // enforced up to the keys claimed while this runs
+        s = find_or_claim(m.table, m.mask, m.slots, key, may_claim, claimed);
+    }
+    const unsigned newk = __ballot_sync(FULL, claimed);
+    if (newk && lane == 0) atomicAdd(&ctr->n_keys, (unsigned)__popc(newk));   // one atomic per warp, not one per key
+
+    // phase 2: a voxel without a bucket (new key, or the dead key of a pruned voxel) gets one.  Exactly one thread in the
+    // grid wins the NO_BUCKET -> PENDING exchange; the warp's winners allocate together: free list first, then the bump end
+    uint32_t b = NO_BUCKET;
+    bool want = false;
+    if (is_leader && s != NO_SLOT) {
+        b = ld_volatile(&m.table[s].bucket);
+        if (b == NO_BUCKET) {
+            const uint32_t old = atomicCAS(&m.table[s].bucket, NO_BUCKET, BUCKET_PENDING);
+            if (old == NO_BUCKET) want = true; else b = old;
+        }
+    }
+    const unsigned wm = __ballot_sync(FULL, want);
+    bool opened = false;
+    if (wm) {
+        const int nreq = __popc(wm);
+        int base = 0;
+        uint32_t fresh = 0;
+        if (lane == 0) {
+            base = atomicSub(&ctr->n_free, nreq);              // may go negative: clamped by the commit kernel's epilogue
+            const int take = max(0, min(base, nreq));
+            if (nreq - take > 0) fresh = atomicAdd(&ctr->bump, (unsigned)(nreq - take));
+        }
+        base = __shfl_sync(FULL, base, 0);
+        fresh = __shfl_sync(FULL, fresh, 0);
+        if (want) {
+            const int take = max(0, min(base, nreq));
+            const int r = __popc(wm & lt);
+            if (r < take) b = m.free_list[base - 1 - r];
+            else {
+                b = fresh + (uint32_t)(r - take);
+                if (b >= m.max_buckets) b = NO_BUCKET;             // pool exhausted: the voxel stays without points
+            }
+            atomicExch(&m.table[s].bucket, b);
+            opened = b != NO_BUCKET;
+        }
+    }
+    // phase 3: another warp may be allocating this voxel's bucket right now; it never waits for anything, so this ends
+    if (is_leader && s != NO_SLOT && !want) {
+        while (b == BUCKET_PENDING) b = ld_volatile(&m.table[s].bucket);
+    }
+    uint32_t c0 = 0;
+    if (is_leader && b != NO_BUCKET) c0 = entry_count(ld_volatile(&m.table[s].cr));   // stable: only commit writes counts
+    s = __shfl_sync(same, s, leader);
+    b = __shfl_sync(same, b, leader);
+    c0 = __shfl_sync(same, c0, leader);
+
+    // statistics, one atomic per warp and counter
+    const unsigned m_bad = __ballot_sync(FULL, bad);
+    const unsigned m_drop = __ballot_sync(FULL, valid && b == NO_BUCKET);
+    const unsigned m_open = __ballot_sync(FULL, opened);
+    if (lane == 0) {
+        if (m_bad) atomicAdd(&ctr->st_invalid, (unsigned long long)__popc(m_bad));
+        if (m_open) atomicAdd(&ctr->st_new_voxels, (unsigned long long)__popc(m_open));
+        if (m_drop) {
+            atomicAdd(&ctr->st_dropped_full, (unsigned long long)__popc(m_drop));
+            ctr->full_flag = 1u;
+        }
+    }
+
+    // phase 4: the chain.  cap = this voxel's limit: the fixed cap, or N_ASMD (positions at and beyond it are never written)
+    bool first_of_voxel = false;
+    if (valid && b != NO_BUCKET) {
+        const uint32_t cap = voxel_limit(m, asmd, k, pose_mode, T);
+        uint32_t* idw = m.ids + (size_t)b * (uint32_t)m.cap;   // id word of position 0
+        uint32_t x = (uint32_t)ctr->next_id + id_offset + (uint32_t)i;
+        // ids at a position only ever decrease: if the last position already holds a smaller id, x cannot survive
+        if (c0 + ahead < cap && !(ld_volatile(idw + (cap - 1)) < x)) {
+            // The id words of a bucket are sorted at every instant and only ever decrease, so a position seen holding an
+            // id < x will never take x: gallop over such positions with plain reads (4 independent loads per step)
+            // instead of walking them with dependent atomics.  A stale read only makes the chain start earlier.
+            uint32_t pos = c0 + ahead;
+            while (pos + 4 <= cap) {
+                if (ld_volatile(idw + (pos + 3)) < x) pos += 4; else break;
+            }
+            for (; pos < cap; ++pos) {
+                const uint32_t old = atomicMin(idw + pos, x);
+                if (old == NO_ID) {
+                    first_of_voxel = pos == c0;                // unique per voxel and chunk
+                    break;
+                }
+                if (old > x) x = old;
             }
         }
-        if (cur == key) { found = true; break; }
-        s = (s + 1) & m.mask;
     }
-    if (new_key) {
-        // one atomic per group of lanes that claimed a key together, not one per key: tens of thousands of
-        // same-address atomics per scan serialise in a single L2 slice (C4: 72k per 100k-point batch)
-        const unsigned grp = __activemask();
-        if ((threadIdx.x & 31) == __ffs(grp) - 1) atomicAdd(&m.ctr->n_keys, (unsigned long long)__popc(grp));
-    }
-    if (!found) {
-        atomicAdd(&m.ctr->st_dropped_full, 1ull);
-        m.ctr->full_flag = 1u;
-        return;
-    }
-    // count is only written by the commit kernel, so it is stable here: c0 = points stored before this chunk
-    const uint32_t c0 = *reinterpret_cast<volatile uint32_t*>(&m.table[s].count);
-    // cap = this voxel's limit: the fixed cap, or N_ASMD (positions at and beyond it are never written)
-    const uint32_t cap = voxel_limit(m, asmd, k, pose_mode, T);
-    if (c0 + ahead >= cap) return;
-    uint32_t* idw = m.ids + (size_t)s * (uint32_t)m.cap;   // id word of position 0 (compact array)
-    uint32_t x = first_id + (uint32_t)i;
-    // ids at a position only ever decrease: if the last position already holds a smaller id, x cannot survive
-    const uint32_t last = *reinterpret_cast<volatile uint32_t*>(idw + (cap - 1));
-    if (last < x) return;
-    // The id words of a bucket are sorted at every instant and only ever decrease, so a position seen holding an
-    // id < x will never take x: gallop over such positions with plain reads (4 independent loads per step)
-    // instead of walking them with dependent atomics.  A stale read only makes the chain start earlier.
-    uint32_t pos = c0 + ahead;
-    while (pos + 4 <= cap) {
-        const uint32_t a3 = *reinterpret_cast<volatile uint32_t*>(idw + (pos + 3));
-        if (a3 < x) pos += 4; else break;
-    }
-    for (; pos < cap; ++pos) {
-        const uint32_t old = atomicMin(idw + pos, x);
-        if (old == NO_ID) {
-            if (pos == c0) touched[atomicAdd(&m.ctr->n_touched, 1u)] = s;   // unique per voxel and chunk
-            break;
-        }
-        if (old > x) x = old;
+    const unsigned m_first = __ballot_sync(FULL, first_of_voxel);
+    if (m_first) {
+        uint32_t at = 0;
+        if (lane == 0) at = atomicAdd(&ctr->n_touched, (unsigned)__popc(m_first));
+        at = __shfl_sync(FULL, at, 0);
+        if (first_of_voxel) touched[at + __popc(m_first & lt)] = s;
     }
 }
 
 // ---- insert, kernel 2: 8 lanes per touched voxel write the coordinates of the surviving ids -------------------
 // Every step of a voxel's commit is a dependent, usually cold access (touched list -> entry -> id row -> source point ->
-// bucket), and most touched voxels receive a handful of points, so a warp works on FOUR voxels at once: four times the
-// memory-level parallelism of a warp per voxel (C4, where almost every point opens its own voxel in a multi-GB pool,
-// is bound by exactly that).  The statistics are accumulated per warp and flushed once at the end.
+// bucket), and most touched voxels receive a handful of points, so a warp works on FOUR voxels at once.  The block that
+// finishes last closes the call: statistics out, counters re-armed, id counter advanced -- no separate launch, no memset.
 constexpr int COMMIT_LANES = 8;      // 4 and 16 measure the same within 3 %
 __global__ void __launch_bounds__(256) insert_commit_kernel(MapView m, const float* __restrict__ xyz, int stride,
                                                              int pose_mode, Pose hpose, const Pose* __restrict__ d_pose,
-                                                             uint32_t first_id, const uint32_t* __restrict__ touched,
-                                                             uint32_t* __restrict__ cov_list, int64_t cov_list_cap) {
+                                                             uint32_t id_offset, const uint32_t* __restrict__ touched,
+                                                             uint2* __restrict__ cov_tasks, int64_t n_call, int last_chunk,
+                                                             far_insert_stats_t* __restrict__ d_stats) {
     const int lane = threadIdx.x & 31, sub = lane / COMMIT_LANES, sl = lane % COMMIT_LANES;
     constexpr int PER_WARP = 32 / COMMIT_LANES;
     const unsigned gmask = ((1u << COMMIT_LANES) - 1u) << (sub * COMMIT_LANES);
     const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
     const Pose& T = (pose_mode == 2) ? *d_pose : hpose;
-    const uint32_t n_touched = m.ctr->n_touched;
+    Counters* ctr = m.ctr;
+    const uint32_t n_touched = ctr->n_touched;
+    const uint32_t first_id = (uint32_t)ctr->next_id + id_offset;
     const uint32_t cap = (uint32_t)m.cap;
-    unsigned long long acc_new = 0, acc_vox = 0;          // lane sl == 0 of each group: points accepted, voxels opened
+    unsigned long long acc_new = 0;                       // lane sl == 0 of each group: points accepted
     for (int64_t t0 = warp * PER_WARP; t0 < n_touched; t0 += nwarps * PER_WARP) {
         const int64_t t = t0 + sub;
         const bool active = t < n_touched;
-        uint32_t s = 0, c0 = cap;
+        uint32_t s = 0, b = 0, cr = 0, c0 = cap;
         if (active) {
             s = touched[t];
-            c0 = m.table[s].count;
+            const Entry e = m.table[s];
+            b = e.bucket; cr = e.cr;
+            c0 = entry_count(cr);
         }
         uint32_t n_new = 0;
         for (uint32_t step = 0; step * COMMIT_LANES < cap; ++step) {      // warp-uniform trip count
             const uint32_t pos = c0 + step * COMMIT_LANES + sl;
             uint32_t id = NO_ID;
-            if (active && pos < cap) id = m.ids[(size_t)s * cap + pos];
+            if (active && pos < cap) id = m.ids[(size_t)b * cap + pos];
             const bool is_new = id != NO_ID;
             if (is_new) {
                 float p[3];
                 load_pose_point(xyz, (int64_t)(id - first_id), stride, pose_mode, T, p);
-                m.points[(size_t)s * cap + pos] = make_float4(p[0], p[1], p[2], __uint_as_float(id));
-                if (m.cov_ok) m.cov_ok[(size_t)s * cap + pos] = 0;
+                m.points[(size_t)b * cap + pos] = make_float4(p[0], p[1], p[2], __uint_as_float(id));
+                if (m.cov_ok) m.cov_ok[(size_t)b * cap + pos] = 0;
             }
-            const unsigned b = __ballot_sync(FULL, is_new);
-            if (b == 0) break;                                             // ids fill positions in order: nothing further
-            if (cov_list != nullptr) {
-                uint32_t at = 0;
-                if (lane == 0) at = atomicAdd(&m.ctr->n_cov, (uint32_t)__popc(b));
-                at = __shfl_sync(FULL, at, 0);
-                const uint32_t mine = at + __popc(b & ((1u << lane) - 1u));
-                if (is_new && mine < cov_list_cap) cov_list[mine] = s * cap + pos;
-            }
-            n_new += __popc(b & gmask);
+            const unsigned bal = __ballot_sync(FULL, is_new);
+            if (bal == 0) break;                                           // ids fill positions in order: nothing further
+            n_new += __popc(bal & gmask);
         }
         if (active && sl == 0) {
-            m.table[s].count = c0 + n_new;
+            m.table[s].cr = (cr & ~0xFFu) | (c0 + n_new);
+            if (cov_tasks) cov_tasks[t] = make_uint2(b, c0 | (n_new << 8));
             acc_new += n_new;
-            if (c0 == 0) acc_vox += 1;
         }
     }
 #pragma unroll
-    for (int d = 16; d > 0; d >>= 1) {
-        acc_new += __shfl_xor_sync(FULL, acc_new, d);
-        acc_vox += __shfl_xor_sync(FULL, acc_vox, d);
-    }
-    if (lane == 0) {
-        if (acc_new) atomicAdd(&m.ctr->st_accepted, acc_new);
-        if (acc_vox) atomicAdd(&m.ctr->st_new_voxels, acc_vox);
-    }
-}
+    for (int d = 16; d > 0; d >>= 1) acc_new += __shfl_xor_sync(FULL, acc_new, d);
+    if (lane == 0 && acc_new) atomicAdd(&ctr->st_accepted, acc_new);
 
-__global__ void insert_stats_kernel(MapView m, int64_t n_offered, far_insert_stats_t* out) {
-    if (threadIdx.x == 0 && blockIdx.x == 0 && out) {
-        out->n_offered = n_offered;
-        out->n_accepted = (int64_t)m.ctr->st_accepted;
-        out->n_new_voxels = (int64_t)m.ctr->st_new_voxels;
-        out->n_dropped_full = (int64_t)m.ctr->st_dropped_full;
-        out->n_invalid = (int64_t)m.ctr->st_invalid;
+    if (last_block_done(&ctr->ticket[0]) && threadIdx.x == 0) {
+        volatile Counters* c = ctr;
+        c->n_tasks = c->n_touched;
+        c->n_touched = 0u;
+        if (c->n_free < 0) c->n_free = 0;
+        if (c->bump > m.max_buckets) c->bump = m.max_buckets;
+        if (last_chunk) {
+            c->call_first_id = c->next_id;
+            c->next_id = c->next_id + (unsigned long long)n_call;
+            if (d_stats) {
+                d_stats->n_offered = n_call;
+                d_stats->n_accepted = (int64_t)c->st_accepted;
+                d_stats->n_new_voxels = (int64_t)c->st_new_voxels;
+                d_stats->n_dropped_full = (int64_t)c->st_dropped_full;
+                d_stats->n_invalid = (int64_t)c->st_invalid;
+            }
+            c->st_accepted = 0ull; c->st_new_voxels = 0ull; c->st_dropped_full = 0ull; c->st_invalid = 0ull;
+            if (c->full_flag) m.mail->full = 1u;
+        }
     }
 }
 
 // ---- A5 prune (R5): thread per slot, FP64 squared centre distance, strict > -------------------
+// A removed voxel's bucket goes back to the free list at once (block-aggregated push) and its key stays as a dead key.
+// The last block writes the statistics and decides, from the number of dead keys, whether the two rehash kernels that
+// follow this one in the stream do their work or return immediately.
 __global__ void __launch_bounds__(256) prune_kernel(MapView m, double cx, double cy, double cz, const Pose* d_pose,
                                                      double r2, far_prune_stats_t* __restrict__ out) {
     const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     unsigned long long vr = 0, pr = 0, vl = 0, pl = 0;
+    uint32_t freed = NO_BUCKET;
     if (s < m.slots) {
         const Entry e = m.table[s];
-        if (e.key != KEY_EMPTY && e.count > 0) {
+        const uint32_t cnt = entry_count(e.cr);
+        if (e.key != KEY_EMPTY && e.bucket < BUCKET_PENDING && cnt > 0) {
             if (d_pose) { cx = d_pose->t[0]; cy = d_pose->t[1]; cz = d_pose->t[2]; }
             int k[3];
             unpack_key(e.key, k);
@@ -244,28 +344,33 @@ __global__ void __launch_bounds__(256) prune_kernel(MapView m, double cx, double
             const double dz = __dadd_rn(__dmul_rn(__dadd_rn((double)k[2], 0.5), v), -cz);
             const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
             if (d2 > r2) {
-                // the key stays (dead key, count 0); its id words go back to +inf so a later insert starts clean
-                for (uint32_t j = 0; j < e.count; ++j) {
-                    m.ids[(size_t)s * m.cap + j] = NO_ID;
-                    if (m.cov_ok) m.cov_ok[(size_t)s * m.cap + j] = 0;
+                // the id words go back to +inf so that the bucket's next owner starts clean
+                for (uint32_t j = 0; j < cnt; ++j) {
+                    m.ids[(size_t)e.bucket * m.cap + j] = NO_ID;
+                    if (m.cov_ok) m.cov_ok[(size_t)e.bucket * m.cap + j] = 0;
                 }
-                m.table[s].count = 0;
-                vr = 1; pr = e.count;
+                m.table[s].bucket = NO_BUCKET;
+                m.table[s].cr = e.cr & ~0xFFu;
+                freed = e.bucket;
+                vr = 1; pr = cnt;
             } else {
-                vl = 1; pl = e.count;
+                vl = 1; pl = cnt;
             }
         }
     }
-    // block-aggregate the four statistics: one atomic per counter and block (the four words are a hot spot)
+    // block-aggregate the free-list push and the four statistics: one atomic per block each
     __shared__ unsigned long long s_acc[8][4];
+    __shared__ uint32_t s_wbase[8];
+    __shared__ uint32_t s_base;
+    const unsigned fm = __ballot_sync(FULL, freed != NO_BUCKET);
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) {
         vr += __shfl_xor_sync(FULL, vr, d); pr += __shfl_xor_sync(FULL, pr, d);
         vl += __shfl_xor_sync(FULL, vl, d); pl += __shfl_xor_sync(FULL, pl, d);
     }
-    if ((threadIdx.x & 31) == 0) {
-        s_acc[threadIdx.x >> 5][0] = vr; s_acc[threadIdx.x >> 5][1] = pr;
-        s_acc[threadIdx.x >> 5][2] = vl; s_acc[threadIdx.x >> 5][3] = pl;
+    if (lane == 0) {
+        s_acc[wib][0] = vr; s_acc[wib][1] = pr; s_acc[wib][2] = vl; s_acc[wib][3] = pl;
+        s_wbase[wib] = __popc(fm);
     }
     __syncthreads();
     if (threadIdx.x < 4) {
@@ -273,24 +378,114 @@ __global__ void __launch_bounds__(256) prune_kernel(MapView m, double cx, double
 #pragma unroll
         for (int w = 0; w < 8; ++w) t += s_acc[w][threadIdx.x];
         if (t) atomicAdd(&m.ctr->pr_vox_removed + threadIdx.x, t);
-        __threadfence();
     }
-    // the block that takes the last ticket writes the statistics out and re-arms the counters: no second launch
-    __shared__ bool s_last;
+    if (threadIdx.x == 32) {
+        uint32_t tot = 0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) { const uint32_t c = s_wbase[w]; s_wbase[w] = tot; tot += c; }
+        s_base = tot ? (uint32_t)atomicAdd(&m.ctr->n_free, (int)tot) : 0u;
+    }
     __syncthreads();
-    if (threadIdx.x == 0) s_last = atomicAdd(&m.ctr->pad, 1u) == gridDim.x - 1;
-    __syncthreads();
-    if (s_last && threadIdx.x == 0) {
-        __threadfence();
-        volatile unsigned long long* c = &m.ctr->pr_vox_removed;
+    if (freed != NO_BUCKET) m.free_list[s_base + s_wbase[wib] + __popc(fm & ((1u << lane) - 1u))] = freed;
+
+    if (last_block_done(&m.ctr->ticket[1]) && threadIdx.x == 0) {
+        volatile Counters* c = m.ctr;
+        const unsigned long long removed = c->pr_vox_removed, left = c->pr_vox_left;
         if (out) {
-            out->n_voxels_removed = (int64_t)c[0];
-            out->n_points_removed = (int64_t)c[1];
-            out->n_voxels_left = (int64_t)c[2];
-            out->n_points_left = (int64_t)c[3];
+            out->n_voxels_removed = (int64_t)removed;
+            out->n_points_removed = (int64_t)c->pr_pts_removed;
+            out->n_voxels_left = (int64_t)left;
+            out->n_points_left = (int64_t)c->pr_pts_left;
         }
-        c[0] = 0ull; c[1] = 0ull; c[2] = 0ull; c[3] = 0ull;
-        m.ctr->pad = 0u;
+        c->pr_vox_removed = 0ull; c->pr_pts_removed = 0ull; c->pr_vox_left = 0ull; c->pr_pts_left = 0ull;
+        const unsigned dead = c->n_dead + (unsigned)removed;
+        c->n_dead = dead;
+        // rebuild when dead keys are no longer a small fraction of the live ones, or the table is running out of keys
+        c->rehash_flag = (dead > 0u && (dead >= 32u + (unsigned)(left >> 3) || c->n_keys > m.key_limit - (m.key_limit >> 2))) ? 1u : 0u;
+        if (removed) { c->full_flag = 0u; m.mail->full = 0u; }     // buckets are available again
+    }
+}
+
+// ---- in-place rehash (SURVEY.md:214-216: deletion in open addressing).  Pass 1 re-inserts every entry that owns a
+// bucket into the empty shadow table (16-byte entries only: buckets stay where they are) and recomputes the reach words;
+// pass 2 copies the shadow table back and empties it again.  Both return at once unless prune's epilogue (or
+// far_map_rehash) set the flag: the decision is taken on the device, the launches are unconditional.
+__global__ void __launch_bounds__(256) rehash_move_kernel(MapView m) {
+    if (!m.ctr->rehash_flag) return;
+    const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+    bool moved = false;
+    if (s < m.slots) {
+        const Entry e = m.table[s];
+        if (e.key != KEY_EMPTY && e.bucket < BUCKET_PENDING) {
+            bool claimed;
+            const uint32_t t = find_or_claim(m.shadow, m.mask, m.slots, e.key, true, claimed);
+            m.shadow[t].bucket = e.bucket;
+            atomicOr(&m.shadow[t].cr, entry_count(e.cr));     // the reach bits of slot t may be raised concurrently
+            moved = true;
+        }
+    }
+    const unsigned bm = __ballot_sync(FULL, moved);
+    if (bm && (threadIdx.x & 31) == 0) atomicAdd(&m.ctr->rehash_moved, (unsigned)__popc(bm));
+}
+
+__global__ void __launch_bounds__(256) rehash_swap_kernel(MapView m) {
+    if (!m.ctr->rehash_flag) return;
+    const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < m.slots) {
+        uint4* sh = reinterpret_cast<uint4*>(m.shadow + s);
+        *reinterpret_cast<uint4*>(m.table + s) = *sh;
+        *sh = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, NO_BUCKET, 0u);
+    }
+    if (s == 0) {
+        m.ctr->n_keys = m.ctr->rehash_moved;
+        m.ctr->rehash_moved = 0u;
+        m.ctr->n_dead = 0u;
+        m.ctr->n_rehash += 1u;
+    }
+}
+
+__global__ void set_rehash_flag_kernel(MapView m) {
+    if (threadIdx.x == 0 && blockIdx.x == 0) m.ctr->rehash_flag = 1u;
+}
+
+// ---- far_map_renumber (R22): ids -= smallest live id, next_id likewise; order and contents unchanged ---------------
+__global__ void __launch_bounds__(256) renumber_min_kernel(MapView m) {
+    const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+    uint32_t mn = NO_ID;
+    if (s < m.slots) {
+        const Entry e = m.table[s];
+        if (e.key != KEY_EMPTY && e.bucket < BUCKET_PENDING && entry_count(e.cr) > 0)
+            mn = m.ids[(size_t)e.bucket * m.cap];             // ids ascend inside a bucket
+    }
+    mn = __reduce_min_sync(FULL, mn);
+    if ((threadIdx.x & 31) == 0 && mn != NO_ID) atomicMin(&m.ctr->min_id, mn);
+}
+
+__global__ void __launch_bounds__(256) renumber_apply_kernel(MapView m, unsigned long long offered_at) {
+    const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t mn = m.ctr->min_id;
+    if (s < m.slots && mn != NO_ID && mn != 0u) {
+        const Entry e = m.table[s];
+        if (e.key != KEY_EMPTY && e.bucket < BUCKET_PENDING) {
+            const uint32_t cnt = entry_count(e.cr);
+            for (uint32_t j = 0; j < cnt; ++j) {
+                const size_t at = (size_t)e.bucket * m.cap + j;
+                const uint32_t id = m.ids[at] - mn;
+                m.ids[at] = id;
+                m.points[at].w = __uint_as_float(id);
+            }
+        }
+    }
+    if (last_block_done(&m.ctr->ticket[3]) && threadIdx.x == 0) {
+        volatile Counters* c = m.ctr;
+        const unsigned long long sub = (mn == NO_ID) ? c->next_id : (unsigned long long)mn;   // empty map: restart at 0
+        c->next_id = c->next_id - sub;
+        c->call_first_id = c->call_first_id >= sub ? c->call_first_id - sub : 0ull;
+        c->min_id = NO_ID;
+        m.mail->next_id_after_renumber = c->next_id;
+        m.mail->offered_at_renumber = offered_at;
+        __threadfence_system();
+        m.mail->renumber_seq = m.mail->renumber_seq + 1u;
     }
 }
 
@@ -301,7 +496,8 @@ __global__ void __launch_bounds__(256) asmd_density_kernel(MapView m, double cx,
     unsigned long long nv = 0, np = 0;
     if (s < m.slots) {
         const Entry e = m.table[s];
-        if (e.key != KEY_EMPTY && e.count > 0) {
+        const uint32_t cnt = entry_count(e.cr);
+        if (e.key != KEY_EMPTY && e.bucket < BUCKET_PENDING && cnt > 0) {
             int k[3];
             unpack_key(e.key, k);
             const double v = (double)m.voxel;
@@ -309,7 +505,7 @@ __global__ void __launch_bounds__(256) asmd_density_kernel(MapView m, double cx,
             const double dy = __dadd_rn(__dmul_rn(__dadd_rn((double)k[1], 0.5), v), -cy);
             const double dz = __dadd_rn(__dmul_rn(__dadd_rn((double)k[2], 0.5), v), -cz);
             const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-            if (d2 <= r2) { nv = 1; np = e.count; }
+            if (d2 <= r2) { nv = 1; np = cnt; }
         }
     }
 #pragma unroll
@@ -317,31 +513,34 @@ __global__ void __launch_bounds__(256) asmd_density_kernel(MapView m, double cx,
     if ((threadIdx.x & 31) == 0 && nv) { atomicAdd(&acc[0], nv); atomicAdd(&acc[1], np); }
 }
 
-__global__ void asmd_density_out_kernel(MapView m, const unsigned long long* acc, double* out) {
+__global__ void asmd_density_out_kernel(MapView m, unsigned long long* acc, double* out) {
     if (threadIdx.x == 0 && blockIdx.x == 0) {
         out[0] = acc[0] ? __ddiv_rn((double)acc[1], (double)acc[0]) : (double)m.cap;
         out[1] = (double)acc[0];
+        acc[0] = 0ull; acc[1] = 0ull;
     }
 }
 
-// ---- clear: reset only what is in use (the pool itself is never touched beyond the live buckets) ------------
+// ---- clear: empty the table, give every used bucket a clean id row, re-arm the counters (one launch) ----------------
 __global__ void __launch_bounds__(256) clear_kernel(MapView m) {
-    const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= m.slots) return;
-    const Entry e = m.table[s];
-    if (e.key == KEY_EMPTY) return;
-    for (uint32_t j = 0; j < e.count; ++j) m.ids[(size_t)s * m.cap + j] = NO_ID;
-    Entry z;
-    z.key = KEY_EMPTY; z.count = 0; z.pad = 0;
-    m.table[s] = z;
+    const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nthr = gridDim.x * blockDim.x;
+    for (uint32_t s = tid; s < m.slots; s += nthr)
+        *reinterpret_cast<uint4*>(m.table + s) = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, NO_BUCKET, 0u);
+    const size_t used = (size_t)min(m.ctr->bump, m.max_buckets) * (size_t)m.cap;   // fresh buckets beyond are clean
+    for (size_t j = tid; j < used; j += nthr) m.ids[j] = NO_ID;
+    if (last_block_done(&m.ctr->ticket[2]) && threadIdx.x == 0) {
+        Counters z;
+        memset(&z, 0, sizeof(z));
+        z.min_id = NO_ID;
+        *m.ctr = z;
+        m.mail->full = 0u;
+    }
 }
 
 __global__ void __launch_bounds__(256) table_init_kernel(Entry* table, uint32_t slots) {
     const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= slots) return;
-    Entry z;
-    z.key = KEY_EMPTY; z.count = 0; z.pad = 0;
-    table[s] = z;
+    *reinterpret_cast<uint4*>(table + s) = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, NO_BUCKET, 0u);
 }
 
 // ---- stats / export ----------------------------------------------------------------------------------------
@@ -351,7 +550,8 @@ __global__ void __launch_bounds__(256) stats_kernel(MapView m, unsigned long lon
     if (s < m.slots) {
         const Entry e = m.table[s];
         if (e.key != KEY_EMPTY) {
-            if (e.count > 0) { nv = 1; np = e.count; } else nd = 1;
+            const uint32_t cnt = entry_count(e.cr);
+            if (e.bucket < BUCKET_PENDING && cnt > 0) { nv = 1; np = cnt; } else nd = 1;
         }
     }
 #pragma unroll
@@ -364,13 +564,19 @@ __global__ void __launch_bounds__(256) stats_kernel(MapView m, unsigned long lon
     }
 }
 
-__global__ void stats_out_kernel(MapView m, unsigned long long* acc, unsigned long long next_id, far_map_stats_t* out) {
+__global__ void stats_out_kernel(MapView m, unsigned long long* acc, far_map_stats_t* out) {
     if (threadIdx.x == 0 && blockIdx.x == 0) {
+        const Counters* c = m.ctr;
         out->n_voxels = (int64_t)acc[0];
         out->n_points = (int64_t)acc[1];
         out->n_dead_keys = (int64_t)acc[2];
         out->n_slots = (int64_t)m.slots;
-        out->next_id = next_id;
+        out->next_id = c->next_id;
+        out->n_keys = (int64_t)c->n_keys;
+        out->n_free_buckets = (int64_t)max(c->n_free, 0);
+        out->n_fresh_buckets = (int64_t)m.max_buckets - (int64_t)min(c->bump, m.max_buckets);
+        out->n_rehash = (int64_t)c->n_rehash;
+        out->full = (int64_t)c->full_flag;
         acc[0] = acc[1] = acc[2] = 0ull;
     }
 }
@@ -383,9 +589,10 @@ __global__ void __launch_bounds__(256) export_kernel(MapView m, unsigned long lo
     const int lane = threadIdx.x & 31;
     const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
     Entry e;
-    e.key = KEY_EMPTY; e.count = 0;
+    e.key = KEY_EMPTY; e.bucket = NO_BUCKET; e.cr = 0;
     if (s < m.slots) e = m.table[s];
-    const bool live = e.key != KEY_EMPTY && e.count > 0;
+    const uint32_t my_cnt = entry_count(e.cr);
+    const bool live = e.key != KEY_EMPTY && e.bucket < BUCKET_PENDING && my_cnt > 0;
     const unsigned b = __ballot_sync(FULL, live);
     if (!b) return;
     unsigned long long base = 0;
@@ -394,20 +601,20 @@ __global__ void __launch_bounds__(256) export_kernel(MapView m, unsigned long lo
     const unsigned long long row = base + __popc(b & ((1u << lane) - 1u));
     if (live && (int64_t)row < max_out) {
         keys[row] = e.key;
-        counts[row] = (int32_t)e.count;
+        counts[row] = (int32_t)my_cnt;
     }
     // cooperative copy of each live bucket of this warp
     unsigned rem = b;
     while (rem) {
         const int src = __ffs(rem) - 1;
         rem &= rem - 1;
-        const uint32_t ss = (blockIdx.x * blockDim.x + (threadIdx.x & ~31)) + src;
-        const uint32_t cnt = __shfl_sync(FULL, e.count, src);
+        const uint32_t bk = __shfl_sync(FULL, e.bucket, src);
+        const uint32_t cnt = __shfl_sync(FULL, my_cnt, src);
         const unsigned long long r = __shfl_sync(FULL, row, src);
         if ((int64_t)r >= max_out) continue;
         for (uint32_t j = lane; j < (uint32_t)m.cap; j += 32) {
             const bool have = j < cnt;
-            const size_t from = (size_t)ss * m.cap + j, to = (size_t)r * m.cap + j;
+            const size_t from = (size_t)bk * m.cap + j, to = (size_t)r * m.cap + j;
             if (pts) pts[to] = have ? m.points[from] : make_float4(0.f, 0.f, 0.f, __uint_as_float(NO_ID));
             if (cov6) {
                 for (int a = 0; a < 6; ++a) cov6[to * 6 + a] = (have && m.cov) ? m.cov[from * 6 + a] : 0.f;
@@ -417,8 +624,8 @@ __global__ void __launch_bounds__(256) export_kernel(MapView m, unsigned long lo
     }
 }
 
-__global__ void write_i64_kernel(const unsigned long long* src, int64_t* dst) {
-    if (threadIdx.x == 0 && blockIdx.x == 0) *dst = (int64_t)*src;
+__global__ void write_i64_kernel(unsigned long long* src, int64_t* dst) {
+    if (threadIdx.x == 0 && blockIdx.x == 0) { *dst = (int64_t)*src; *src = 0ull; }
 }
 
 __global__ void __launch_bounds__(256) voxel_keys_kernel(const float* __restrict__ xyz, int64_t n, int stride, float v,
@@ -428,66 +635,6 @@ __global__ void __launch_bounds__(256) voxel_keys_kernel(const float* __restrict
     const float* p = xyz + i * stride;
     int k[3];
     keys[i] = voxel_index(p[0], p[1], p[2], v, k) ? pack_key(k[0], k[1], k[2]) : KEY_EMPTY;
-}
-
-// ---- rehash: move the live voxels into a clean table (drops dead keys) --------------------------------------
-// pass 1 copies every live bucket into a compact temporary; pass 2 re-inserts them after the table was cleared
-__global__ void __launch_bounds__(256) rehash_gather_kernel(MapView m, unsigned long long* __restrict__ keys,
-                                                             uint32_t* __restrict__ counts, float4* __restrict__ pts,
-                                                             float* __restrict__ cov6, uint8_t* __restrict__ cov_ok,
-                                                             unsigned long long* n_out) {
-    const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= m.slots) return;
-    const Entry e = m.table[s];
-    if (e.key == KEY_EMPTY) return;
-    float4* bucket = m.points + (size_t)s * m.cap;
-    if (e.count > 0) {
-        const unsigned long long r = atomicAdd(n_out, 1ull);
-        keys[r] = e.key;
-        counts[r] = e.count;
-        for (uint32_t j = 0; j < e.count; ++j) {
-            const size_t from = (size_t)s * m.cap + j, to = (size_t)r * m.cap + j;
-            pts[to] = bucket[j];
-            if (m.cov) {
-                for (int a = 0; a < 6; ++a) cov6[to * 6 + a] = m.cov[from * 6 + a];
-                cov_ok[to] = m.cov_ok[from];
-            }
-        }
-    }
-    for (uint32_t j = 0; j < e.count; ++j) m.ids[(size_t)s * m.cap + j] = NO_ID;
-    Entry z;
-    z.key = KEY_EMPTY; z.count = 0; z.pad = 0;
-    m.table[s] = z;
-}
-
-__global__ void __launch_bounds__(256) rehash_scatter_kernel(MapView m, const unsigned long long* __restrict__ keys,
-                                                              const uint32_t* __restrict__ counts,
-                                                              const float4* __restrict__ pts, const float* __restrict__ cov6,
-                                                              const uint8_t* __restrict__ cov_ok,
-                                                              const unsigned long long* n_live) {
-    const unsigned long long r = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (r >= *n_live) return;
-    const unsigned long long key = keys[r];
-    uint32_t s = hash_key(key) & m.mask;
-    for (uint32_t probes = 0; probes < m.slots; ++probes) {
-        if (atomicCAS(&m.table[s].key, KEY_EMPTY, key) == KEY_EMPTY) {
-            atomicMax(&m.table[hash_key(key) & m.mask].pad, probes + 1u);
-            break;
-        }
-        s = (s + 1) & m.mask;
-    }
-    const uint32_t cnt = counts[r];
-    for (uint32_t j = 0; j < cnt; ++j) {
-        const size_t to = (size_t)s * m.cap + j, from = (size_t)r * m.cap + j;
-        m.points[to] = pts[from];
-        m.ids[to] = __float_as_uint(pts[from].w);
-        if (m.cov) {
-            for (int a = 0; a < 6; ++a) m.cov[to * 6 + a] = cov6[from * 6 + a];
-            m.cov_ok[to] = cov_ok[from];
-        }
-    }
-    m.table[s].count = cnt;
-    if (r == 0) m.ctr->n_keys = *n_live;
 }
 
 }  // namespace far
@@ -500,7 +647,7 @@ const char* far_strerror(int status) {
         case FAR_OK: return "ok";
         case FAR_ERR_ARG: return "invalid argument";
         case FAR_ERR_CUDA: return "CUDA runtime error";
-        case FAR_ERR_FULL: return "voxel table full";
+        case FAR_ERR_FULL: return "voxel map full: points were dropped";
         case FAR_ERR_RANGE: return "point id counter out of range";
         case FAR_ERR_DEGENERATE: return "degenerate registration (too few inliers or H not positive definite)";
         default: return "unknown status";
@@ -521,50 +668,64 @@ int far_map_create(far_map_t** out, const far_map_config_t* cfg) {
     if (c.cov_eps == 0.0) c.cov_eps = 1e-3;
     if (c.max_batch == 0) c.max_batch = 1 << 20;
     if (c.max_batch < 1 || c.max_batch > (1ll << 30)) return FAR_ERR_ARG;
+    if (c.renumber_every == 0) c.renumber_every = 1ll << 31;
+    if (c.renumber_every < 1 || c.renumber_every > (1ll << 31)) return FAR_ERR_ARG;
     uint64_t slots = 16;
     const double want = (double)c.max_voxels / (double)c.max_load;
     while ((double)slots < want) slots <<= 1;
-    if (slots * (uint64_t)c.cap >= (1ull << 32)) return FAR_ERR_ARG;   // refs (slot*cap+pos) are 32-bit
+    if (slots >= (1ull << 31) || (uint64_t)c.max_voxels * (uint64_t)c.cap >= (1ull << 32)) return FAR_ERR_ARG;   // refs are 32-bit
 
     far_map* m = new (std::nothrow) far_map();
     if (!m) return FAR_ERR_ARG;
     memset(m, 0, sizeof(*m));
     m->cfg = c;
     m->max_batch = c.max_batch;
-    m->next_id = 0;
+    m->renumber_every = (uint64_t)c.renumber_every;
     FAR_CUDA(cudaGetDevice(&m->device));
     FAR_CUDA(cudaDeviceGetAttribute(&m->sm_count, cudaDevAttrMultiProcessorCount, m->device));
     MapView& v = m->view;
     v.slots = (uint32_t)slots;
     v.mask = (uint32_t)slots - 1;
+    v.max_buckets = (uint32_t)c.max_voxels;
+    v.key_limit = (uint32_t)(slots - slots / 16);
     v.cap = c.cap;
     v.k_cov = c.k_cov;
     v.voxel = c.voxel_size;
     v.cov_eps = c.cov_eps;
-    v.max_keys = (unsigned long long)c.max_voxels;
-    const size_t npts = (size_t)slots * c.cap;
+    const size_t npts = (size_t)c.max_voxels * c.cap;
     cudaError_t e = cudaSuccess;
     auto alloc = [&](void** p, size_t bytes) { if (e == cudaSuccess) e = cudaMalloc(p, bytes); };
     alloc((void**)&v.table, slots * sizeof(Entry));
+    alloc((void**)&v.shadow, slots * sizeof(Entry));
     alloc((void**)&v.points, npts * sizeof(float4));
     alloc((void**)&v.ids, npts * sizeof(uint32_t));
+    alloc((void**)&v.free_list, (size_t)c.max_voxels * sizeof(uint32_t));
     if (c.with_cov) {
         alloc((void**)&v.cov, npts * 6 * sizeof(float));
         alloc((void**)&v.cov_ok, npts);
     }
-    alloc((void**)&v.ctr, sizeof(Counters) + 8 * sizeof(unsigned long long));
-    alloc((void**)&m->d_touched, (size_t)c.max_batch * 4);
-    alloc((void**)&m->d_cov_list, (size_t)c.max_batch * 4);
+    alloc((void**)&v.ctr, sizeof(Counters));
+    alloc((void**)&m->d_touched, (size_t)c.max_batch * sizeof(uint32_t));
+    alloc((void**)&m->d_cov_tasks, (size_t)c.max_batch * sizeof(uint2));
+    if (e == cudaSuccess) e = cudaHostAlloc((void**)&m->h_mail, sizeof(Mailbox), cudaHostAllocMapped);
+    if (e == cudaSuccess) {
+        memset((void*)m->h_mail, 0, sizeof(Mailbox));
+        e = cudaHostGetDevicePointer((void**)&v.mail, (void*)m->h_mail, 0);
+    }
     if (e != cudaSuccess) {
-        far::set_cuda_error(e, "cudaMalloc in far_map_create");
+        far::set_cuda_error(e, "allocation in far_map_create");
         far_map_destroy(m);
         return FAR_ERR_CUDA;
     }
-    // empty table: every key = ~0, count = 0; every id word = FAR_NO_ID
+    // empty tables: every key = ~0, no bucket; every id word = FAR_NO_ID
     FAR_CUDA(cudaMemset(v.ids, 0xFF, npts * sizeof(uint32_t)));
     FAR_LAUNCH(table_init_kernel, grid_for((int64_t)slots, 256), 256, 0, 0, v.table, v.slots);
+    FAR_LAUNCH(table_init_kernel, grid_for((int64_t)slots, 256), 256, 0, 0, v.shadow, v.slots);
     FAR_CUDA(cudaGetLastError());
-    FAR_CUDA(cudaMemset(v.ctr, 0, sizeof(Counters) + 8 * sizeof(unsigned long long)));
+    Counters z;
+    memset(&z, 0, sizeof(z));
+    z.min_id = NO_ID;
+    FAR_CUDA(cudaMemcpy(v.ctr, &z, sizeof(z), cudaMemcpyHostToDevice));
     if (v.cov_ok) FAR_CUDA(cudaMemset(v.cov_ok, 0, npts));
     {
         const int rc = gicp_setup(m);
@@ -577,9 +738,11 @@ int far_map_create(far_map_t** out, const far_map_config_t* cfg) {
 
 int far_map_destroy(far_map_t* m) {
     if (!m) return FAR_OK;
-    cudaFree(m->view.table); cudaFree(m->view.points); cudaFree(m->view.ids); cudaFree(m->view.cov); cudaFree(m->view.cov_ok);
-    cudaFree(m->view.ctr); cudaFree(m->d_touched); cudaFree(m->d_cov_list);
+    cudaFree(m->view.table); cudaFree(m->view.shadow); cudaFree(m->view.points); cudaFree(m->view.ids);
+    cudaFree(m->view.free_list); cudaFree(m->view.cov); cudaFree(m->view.cov_ok);
+    cudaFree(m->view.ctr); cudaFree(m->d_touched); cudaFree(m->d_cov_tasks);
     cudaFree(m->d_gicp_partials);
+    if (m->h_mail) cudaFreeHost((void*)m->h_mail);
     delete m;
     return FAR_OK;
 }
@@ -587,53 +750,85 @@ int far_map_destroy(far_map_t* m) {
 int far_map_clear(far_map_t* m, void* stream) {
     if (!m) return FAR_ERR_ARG;
     cudaStream_t st = (cudaStream_t)stream;
-    FAR_LAUNCH(clear_kernel, grid_for(m->view.slots, 256), 256, 0, st, m->view);
+    FAR_LAUNCH(clear_kernel, m->sm_count * 4, 256, 0, st, m->view);
     FAR_CUDA(cudaGetLastError());
-    FAR_CUDA(cudaMemsetAsync(m->view.ctr, 0, sizeof(Counters), st));
-    m->next_id = 0;
+    m->next_id_ub = 0;
+    m->offered_total = 0;
+    m->offered_at_renumber = 0;
     return FAR_OK;
+}
+
+// folds a completed renumber pass (reported through the mailbox) into the host-side bound of the id counter
+static void refresh_id_bound(far_map_t* m) {
+    const uint32_t seq = m->h_mail->renumber_seq;
+    if (seq == m->renumber_seen) return;
+    const uint64_t at = m->h_mail->offered_at_renumber, nid = m->h_mail->next_id_after_renumber;
+    if (m->h_mail->renumber_seq != seq) return;                 // a newer pass is landing: take it next time
+    m->renumber_seen = seq;
+    if (at <= m->offered_total) m->next_id_ub = nid + (m->offered_total - at);
+}
+
+static int renumber_enqueue(far_map_t* m, cudaStream_t st) {
+    FAR_LAUNCH(renumber_min_kernel, grid_for(m->view.slots, 256), 256, 0, st, m->view);
+    FAR_LAUNCH(renumber_apply_kernel, grid_for(m->view.slots, 256), 256, 0, st, m->view, (unsigned long long)m->offered_total);
+    FAR_CUDA(cudaGetLastError());
+    m->offered_at_renumber = m->offered_total;
+    return FAR_OK;
+}
+
+int far_map_renumber(far_map_t* m, void* stream) {
+    if (!m) return FAR_ERR_ARG;
+    return renumber_enqueue(m, (cudaStream_t)stream);
 }
 
 static int insert_impl(far_map_t* m, const float* d_xyz, int64_t n, int stride, int pose_mode, const far_pose_t* hpose,
                        const far_pose_t* d_pose, int compute_cov, far_insert_stats_t* d_stats, void* stream,
                        Asmd asmd = Asmd{nullptr, 1.0, 0}) {
-    if (!m || (!d_xyz && n > 0) || n < 0 || (stride != 3 && stride != 4)) return FAR_ERR_ARG;
+    if (!m || (!d_xyz && n > 0) || n < 0 || n > 0x7FFFFFFFll || (stride != 3 && stride != 4)) return FAR_ERR_ARG;
     if (compute_cov && !m->view.cov) return FAR_ERR_ARG;
-    if (m->next_id + (uint64_t)n > 0xFFFFFFFFull) return FAR_ERR_RANGE;
     cudaStream_t st = (cudaStream_t)stream;
+    // id counter (R3: ids are u32 and advance by the points OFFERED).  The counter lives on the device; the host keeps an
+    // upper bound, enqueues a renumber pass (R22) at a deterministic point of the offered-points count, and only if the
+    // bound would still overflow does it wait for the device to report the renumbered counter.
+    refresh_id_bound(m);
+    if (m->offered_total - m->offered_at_renumber + (uint64_t)n > m->renumber_every && m->offered_total > m->offered_at_renumber) {
+        const int rc = renumber_enqueue(m, st);
+        if (rc != FAR_OK) return rc;
+    }
+    if (m->next_id_ub + (uint64_t)n > 0xFFFFFFFFull) {
+        FAR_CUDA(cudaStreamSynchronize(st));
+        refresh_id_bound(m);
+        if (m->next_id_ub + (uint64_t)n > 0xFFFFFFFFull) return FAR_ERR_RANGE;
+    }
     Pose hp;
     memset(&hp, 0, sizeof(hp));
     if (pose_mode == 1) memcpy(&hp, hpose, sizeof(hp));
-    Counters* ctr = m->view.ctr;
-    // zero the touched counter, the covariance queue and the per-call statistics (contiguous: one call)
-    FAR_CUDA(cudaMemsetAsync(&ctr->n_touched, 0, 2 * sizeof(unsigned int) + 4 * sizeof(unsigned long long), st));
-    const bool cov_by_list = compute_cov && n <= m->max_batch;
-    const uint32_t call_first_id = (uint32_t)m->next_id;
+    const bool cov_by_tasks = compute_cov && n <= m->max_batch;
     const int commit_grid = m->sm_count * 8;
-    for (int64_t off = 0; off < n; off += m->max_batch) {
+    int64_t off = 0;
+    do {
         const int64_t nc = (n - off < m->max_batch) ? n - off : m->max_batch;
-        const uint32_t first_id = (uint32_t)(m->next_id + (uint64_t)off);
         const float* xyz = d_xyz + off * stride;
-        if (off > 0) FAR_CUDA(cudaMemsetAsync(&ctr->n_touched, 0, sizeof(unsigned int), st));
-        FAR_LAUNCH(insert_claim_chain_kernel, grid_for(nc, 256), 256, 0, st, m->view, xyz, nc, stride, pose_mode, hp,
-                                                                      (const Pose*)d_pose, first_id, m->d_touched, asmd);
-        FAR_LAUNCH(insert_commit_kernel, commit_grid, 256, 0, st, m->view, xyz, stride, pose_mode, hp, (const Pose*)d_pose,
-                                                           first_id, m->d_touched, cov_by_list ? m->d_cov_list : nullptr,
-                                                           m->max_batch);
+        const int last = off + nc >= n;
+        if (nc > 0)
+            FAR_LAUNCH(insert_claim_chain_kernel, grid_for(nc, 256), 256, 0, st, m->view, xyz, nc, stride, pose_mode, hp,
+                                                                          (const Pose*)d_pose, (uint32_t)off, m->d_touched, asmd);
+        FAR_LAUNCH(insert_commit_kernel, nc > 0 ? commit_grid : 1, 256, 0, st, m->view, xyz, stride, pose_mode, hp,
+                                                           (const Pose*)d_pose, (uint32_t)off, m->d_touched,
+                                                           cov_by_tasks ? m->d_cov_tasks : nullptr, n, last, d_stats);
         FAR_CUDA(cudaGetLastError());
-    }
-    m->next_id += (uint64_t)n;
+        off += nc;
+    } while (off < n);
+    m->next_id_ub += (uint64_t)n;
+    m->offered_total += (uint64_t)n;
     if (compute_cov && n > 0) {
         // "we recompute the covariances of the added points" -- against the map AFTER the insert
-        int rc = cov_by_list ? launch_knn_cov_refs(m, m->d_cov_list, &ctr->n_cov, n, st)
-                             : launch_knn_cov_new_ids(m, call_first_id, st);
+        int rc = cov_by_tasks ? launch_knn_cov_tasks(m, m->d_cov_tasks, &m->view.ctr->n_tasks, n, st)
+                              : launch_knn_cov_new_ids(m, st);
         if (rc != FAR_OK) return rc;
     }
-    if (d_stats) {
-        FAR_LAUNCH(insert_stats_kernel, 1, 32, 0, st, m->view, n, d_stats);
-        FAR_CUDA(cudaGetLastError());
-    }
-    return FAR_OK;
+    // the device's sticky flag, seen without a synchronisation: set by THIS call only if it has already run
+    return m->h_mail->full ? FAR_ERR_FULL : FAR_OK;
 }
 
 int far_map_insert(far_map_t* m, const float* d_xyz, int64_t n, int stride, const far_pose_t* pose, int compute_cov,
@@ -664,11 +859,17 @@ int far_map_insert_asmd_dev(far_map_t* m, const float* d_xyz, int64_t n, int str
 int far_asmd_density(const far_map_t* local, const double center[3], double r_close, double* d_out, void* stream) {
     if (!local || !center || !d_out || !(r_close >= 0.0)) return FAR_ERR_ARG;
     cudaStream_t st = (cudaStream_t)stream;
-    unsigned long long* acc = reinterpret_cast<unsigned long long*>(local->view.ctr + 1) + 4;   // 2 words of the tail
-    FAR_CUDA(cudaMemsetAsync(acc, 0, 2 * sizeof(unsigned long long), st));
+    unsigned long long* acc = local->view.ctr->scratch + 4;     // two words, left zeroed by the out kernel
     FAR_LAUNCH(asmd_density_kernel, grid_for(local->view.slots, 256), 256, 0, st, local->view, center[0], center[1], center[2],
                                                                         r_close * r_close, acc);
     FAR_LAUNCH(asmd_density_out_kernel, 1, 32, 0, st, local->view, acc, d_out);
+    FAR_CUDA(cudaGetLastError());
+    return FAR_OK;
+}
+
+static int rehash_enqueue(far_map_t* m, cudaStream_t st) {
+    FAR_LAUNCH(rehash_move_kernel, grid_for(m->view.slots, 256), 256, 0, st, m->view);
+    FAR_LAUNCH(rehash_swap_kernel, grid_for(m->view.slots, 256), 256, 0, st, m->view);
     FAR_CUDA(cudaGetLastError());
     return FAR_OK;
 }
@@ -681,7 +882,7 @@ static int prune_impl(far_map_t* m, const double* c, const far_pose_t* d_pose, d
     FAR_LAUNCH(prune_kernel, grid_for(m->view.slots, 256), 256, 0, st, m->view, c ? c[0] : 0.0, c ? c[1] : 0.0, c ? c[2] : 0.0,
                                                                 (const Pose*)d_pose, r2, d_stats);
     FAR_CUDA(cudaGetLastError());
-    return FAR_OK;
+    return rehash_enqueue(m, st);          // both kernels return at once unless prune's epilogue asked for the rebuild
 }
 
 int far_map_prune(far_map_t* m, const double center[3], double radius, far_prune_stats_t* d_stats, void* stream) {
@@ -697,19 +898,23 @@ int far_map_prune_dev(far_map_t* m, const far_pose_t* d_pose, double radius, far
 int far_map_stats(far_map_t* m, far_map_stats_t* d_stats, void* stream) {
     if (!m || !d_stats) return FAR_ERR_ARG;
     cudaStream_t st = (cudaStream_t)stream;
-    unsigned long long* acc = reinterpret_cast<unsigned long long*>(m->view.ctr + 1);
+    unsigned long long* acc = m->view.ctr->scratch;
     FAR_LAUNCH(stats_kernel, grid_for(m->view.slots, 256), 256, 0, st, m->view, acc);
-    FAR_LAUNCH(stats_out_kernel, 1, 32, 0, st, m->view, acc, m->next_id, d_stats);
+    FAR_LAUNCH(stats_out_kernel, 1, 32, 0, st, m->view, acc, d_stats);
     FAR_CUDA(cudaGetLastError());
     return FAR_OK;
+}
+
+int far_map_status(const far_map_t* m) {
+    if (!m) return FAR_ERR_ARG;
+    return m->h_mail->full ? FAR_ERR_FULL : FAR_OK;
 }
 
 int far_map_export(far_map_t* m, uint64_t* d_keys, int32_t* d_counts, float* d_points4, float* d_cov6,
                    uint8_t* d_cov_valid, int64_t max_out, int64_t* d_n_voxels, void* stream) {
     if (!m || !d_keys || !d_counts || !d_n_voxels || max_out < 0) return FAR_ERR_ARG;
     cudaStream_t st = (cudaStream_t)stream;
-    unsigned long long* acc = reinterpret_cast<unsigned long long*>(m->view.ctr + 1) + 3;
-    FAR_CUDA(cudaMemsetAsync(acc, 0, sizeof(unsigned long long), st));
+    unsigned long long* acc = m->view.ctr->scratch + 3;          // left zeroed by write_i64_kernel
     FAR_LAUNCH(export_kernel, grid_for(m->view.slots, 256), 256, 0, st, m->view, (unsigned long long*)d_keys, d_counts,
                                                                  (float4*)d_points4, d_cov6, d_cov_valid, max_out, acc);
     FAR_LAUNCH(write_i64_kernel, 1, 32, 0, st, acc, d_n_voxels);
@@ -726,44 +931,13 @@ int far_voxel_keys(const float* d_xyz, int64_t n, int stride, float voxel, uint6
     return FAR_OK;
 }
 
-// Maintenance call (not on the per-frame hot path): allocates a compact temporary for the live voxels,
-// synchronises the stream once to learn their number, and frees the temporary before returning.
+// Drops the dead keys now, whatever their number: three stream-ordered launches, no allocation, no synchronisation.
+// far_map_prune does the same by itself whenever the dead keys pass its threshold.
 int far_map_rehash(far_map_t* m, void* stream) {
     if (!m) return FAR_ERR_ARG;
     cudaStream_t st = (cudaStream_t)stream;
-    far_map_stats_t hs;
-    far_map_stats_t* d_hs = nullptr;
-    FAR_CUDA(cudaMalloc((void**)&d_hs, sizeof(hs)));
-    int rc = far_map_stats(m, d_hs, stream);
-    if (rc != FAR_OK) { cudaFree(d_hs); return rc; }
-    FAR_CUDA(cudaMemcpyAsync(&hs, d_hs, sizeof(hs), cudaMemcpyDeviceToHost, st));
-    FAR_CUDA(cudaStreamSynchronize(st));
-    cudaFree(d_hs);
-    const size_t nv = (size_t)hs.n_voxels, cap = (size_t)m->view.cap;
-    unsigned long long *t_keys = nullptr, *t_n = nullptr;
-    uint32_t* t_counts = nullptr;
-    float4* t_pts = nullptr;
-    float* t_cov = nullptr;
-    uint8_t* t_ok = nullptr;
-    cudaError_t e = cudaMalloc((void**)&t_keys, (nv + 1) * 8);
-    if (e == cudaSuccess) e = cudaMalloc((void**)&t_counts, (nv + 1) * 4);
-    if (e == cudaSuccess) e = cudaMalloc((void**)&t_pts, (nv * cap + 1) * sizeof(float4));
-    if (e == cudaSuccess) e = cudaMalloc((void**)&t_n, 8);
-    if (e == cudaSuccess && m->view.cov) e = cudaMalloc((void**)&t_cov, (nv * cap + 1) * 6 * sizeof(float));
-    if (e == cudaSuccess && m->view.cov) e = cudaMalloc((void**)&t_ok, nv * cap + 1);
-    if (e == cudaSuccess) e = cudaMemsetAsync(t_n, 0, 8, st);
-    if (e == cudaSuccess) {
-        FAR_LAUNCH(rehash_gather_kernel, grid_for(m->view.slots, 256), 256, 0, st, m->view, t_keys, t_counts, t_pts, t_cov, t_ok, t_n);
-        if (nv > 0)
-            FAR_LAUNCH(rehash_scatter_kernel, grid_for((int64_t)nv, 256), 256, 0, st, m->view, t_keys, t_counts, t_pts, t_cov, t_ok, t_n);
-        else
-            e = cudaMemsetAsync(&m->view.ctr->n_keys, 0, 8, st);
-        if (e == cudaSuccess) e = cudaGetLastError();
-        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    }
-    cudaFree(t_keys); cudaFree(t_counts); cudaFree(t_pts); cudaFree(t_n); cudaFree(t_cov); cudaFree(t_ok);
-    if (e != cudaSuccess) { far::set_cuda_error(e, "far_map_rehash"); return FAR_ERR_CUDA; }
-    return FAR_OK;
+    FAR_LAUNCH(set_rehash_flag_kernel, 1, 32, 0, st, m->view);
+    return rehash_enqueue(m, st);
 }
 
 }  // extern "C"
@@ -808,9 +982,9 @@ LaunchScope::~LaunchScope() {
 }  // namespace far
 
 struct far_snapshot {
-    void *table, *points, *ids, *cov, *cov_ok, *ctr;
-    size_t b_table, b_points, b_ids, b_cov, b_ok;
-    uint64_t next_id;
+    void *table, *points, *ids, *cov, *cov_ok, *free_list, *ctr;
+    size_t b_table, b_points, b_ids, b_cov, b_ok, b_free;
+    uint64_t next_id_ub, offered_total, offered_at_renumber;
 };
 
 extern "C" {
@@ -851,7 +1025,8 @@ int far_profile_collect(const char** names, double* total_ms, long long* launche
 
 int far_map_snapshot_destroy(far_snapshot_t* s) {
     if (!s) return FAR_OK;
-    cudaFree(s->table); cudaFree(s->points); cudaFree(s->ids); cudaFree(s->cov); cudaFree(s->cov_ok); cudaFree(s->ctr);
+    cudaFree(s->table); cudaFree(s->points); cudaFree(s->ids); cudaFree(s->cov); cudaFree(s->cov_ok); cudaFree(s->free_list);
+    cudaFree(s->ctr);
     delete s;
     return FAR_OK;
 }
@@ -863,25 +1038,26 @@ int far_map_snapshot_create(far_map_t* m, far_snapshot_t** out, void* stream) {
     far_snapshot* s = new (std::nothrow) far_snapshot();
     if (!s) return FAR_ERR_ARG;
     memset(s, 0, sizeof(*s));
-    const size_t npts = (size_t)m->view.slots * m->view.cap;
+    const size_t npts = (size_t)m->view.max_buckets * m->view.cap;
     s->b_table = (size_t)m->view.slots * sizeof(Entry);
     s->b_points = npts * sizeof(float4);
     s->b_ids = npts * sizeof(uint32_t);
     s->b_cov = m->view.cov ? npts * 6 * sizeof(float) : 0;
     s->b_ok = m->view.cov_ok ? npts : 0;
-    s->next_id = m->next_id;
-    cudaError_t e = cudaMalloc(&s->table, s->b_table);
-    if (e == cudaSuccess) e = cudaMalloc(&s->points, s->b_points);
-    if (e == cudaSuccess) e = cudaMalloc(&s->ids, s->b_ids);
-    if (e == cudaSuccess && s->b_cov) e = cudaMalloc(&s->cov, s->b_cov);
-    if (e == cudaSuccess && s->b_ok) e = cudaMalloc(&s->cov_ok, s->b_ok);
-    if (e == cudaSuccess) e = cudaMalloc(&s->ctr, sizeof(Counters));
-    if (e == cudaSuccess) e = cudaMemcpyAsync(s->table, m->view.table, s->b_table, cudaMemcpyDeviceToDevice, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(s->points, m->view.points, s->b_points, cudaMemcpyDeviceToDevice, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(s->ids, m->view.ids, s->b_ids, cudaMemcpyDeviceToDevice, st);
-    if (e == cudaSuccess && s->b_cov) e = cudaMemcpyAsync(s->cov, m->view.cov, s->b_cov, cudaMemcpyDeviceToDevice, st);
-    if (e == cudaSuccess && s->b_ok) e = cudaMemcpyAsync(s->cov_ok, m->view.cov_ok, s->b_ok, cudaMemcpyDeviceToDevice, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(s->ctr, m->view.ctr, sizeof(Counters), cudaMemcpyDeviceToDevice, st);
+    s->b_free = (size_t)m->view.max_buckets * sizeof(uint32_t);
+    s->next_id_ub = m->next_id_ub;
+    s->offered_total = m->offered_total;
+    s->offered_at_renumber = m->offered_at_renumber;
+    struct { void** dst; const void* src; size_t bytes; } parts[] = {
+        {&s->table, m->view.table, s->b_table}, {&s->points, m->view.points, s->b_points}, {&s->ids, m->view.ids, s->b_ids},
+        {&s->cov, m->view.cov, s->b_cov}, {&s->cov_ok, m->view.cov_ok, s->b_ok}, {&s->free_list, m->view.free_list, s->b_free},
+        {&s->ctr, m->view.ctr, sizeof(Counters)}};
+    cudaError_t e = cudaSuccess;
+    for (auto& p : parts) {
+        if (!p.bytes || e != cudaSuccess) continue;
+        e = cudaMalloc(p.dst, p.bytes);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(*p.dst, p.src, p.bytes, cudaMemcpyDeviceToDevice, st);
+    }
     if (e != cudaSuccess) {
         far::set_cuda_error(e, "far_map_snapshot_create");
         far_map_snapshot_destroy(s);
@@ -891,9 +1067,10 @@ int far_map_snapshot_create(far_map_t* m, far_snapshot_t** out, void* stream) {
     return FAR_OK;
 }
 
+// the shadow table is empty between calls and the GICP scratch carries its own launch sequence: neither is part of a snapshot
 int far_map_snapshot_restore(far_map_t* m, const far_snapshot_t* s, void* stream) {
     if (!m || !s) return FAR_ERR_ARG;
-    const size_t npts = (size_t)m->view.slots * m->view.cap;
+    const size_t npts = (size_t)m->view.max_buckets * m->view.cap;
     if (s->b_table != (size_t)m->view.slots * sizeof(Entry) || s->b_points != npts * sizeof(float4)) return FAR_ERR_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     FAR_CUDA(cudaMemcpyAsync(m->view.table, s->table, s->b_table, cudaMemcpyDeviceToDevice, st));
@@ -901,8 +1078,11 @@ int far_map_snapshot_restore(far_map_t* m, const far_snapshot_t* s, void* stream
     FAR_CUDA(cudaMemcpyAsync(m->view.ids, s->ids, s->b_ids, cudaMemcpyDeviceToDevice, st));
     if (s->b_cov && m->view.cov) FAR_CUDA(cudaMemcpyAsync(m->view.cov, s->cov, s->b_cov, cudaMemcpyDeviceToDevice, st));
     if (s->b_ok && m->view.cov_ok) FAR_CUDA(cudaMemcpyAsync(m->view.cov_ok, s->cov_ok, s->b_ok, cudaMemcpyDeviceToDevice, st));
+    FAR_CUDA(cudaMemcpyAsync(m->view.free_list, s->free_list, s->b_free, cudaMemcpyDeviceToDevice, st));
     FAR_CUDA(cudaMemcpyAsync(m->view.ctr, s->ctr, sizeof(Counters), cudaMemcpyDeviceToDevice, st));
-    m->next_id = s->next_id;
+    m->next_id_ub = s->next_id_ub;
+    m->offered_total = s->offered_total;
+    m->offered_at_renumber = s->offered_at_renumber;
     return FAR_OK;
 }
 

@@ -199,8 +199,8 @@ __global__ void __launch_bounds__(256, 5) knn_cov_points_kernel(MapView m, const
     }
 }
 
-// queries = stored points named by refs (covariances of the points an insert accepted)
-__global__ void __launch_bounds__(256, 5) knn_cov_refs_kernel(MapView m, const uint32_t* __restrict__ refs, const unsigned int* __restrict__ d_n,
+// queries = the points an insert accepted, one task per touched voxel: bucket, first new position, count
+__global__ void __launch_bounds__(256, 5) knn_cov_tasks_kernel(MapView m, const uint2* __restrict__ tasks, const unsigned int* __restrict__ d_n,
                                     int warps_per_block) {
     extern __shared__ __align__(16) char smem[];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
@@ -208,26 +208,32 @@ __global__ void __launch_bounds__(256, 5) knn_cov_refs_kernel(MapView m, const u
     const int64_t n = *d_n;
     const int64_t nwarps = (int64_t)gridDim.x * warps_per_block;
     for (int64_t i = (int64_t)blockIdx.x * warps_per_block + wib; i < n; i += nwarps) {
-        const uint32_t ref = refs[i];
-        const float4 p = m.points[ref];
-        float c[6];
-        const bool ok = warp_knn_cov(m, p.x, p.y, p.z, lane, smem_w, c);
-        if (lane < 6) m.cov[(size_t)ref * 6 + lane] = c[lane];
-        if (lane == 0) m.cov_ok[ref] = ok ? 1 : 0;
+        const uint2 t = tasks[i];
+        const uint32_t c0 = t.y & 0xFFu, n_new = t.y >> 8;
+        for (uint32_t j = c0; j < c0 + n_new; ++j) {
+            const uint32_t ref = t.x * (uint32_t)m.cap + j;
+            const float4 p = m.points[ref];
+            float c[6];
+            const bool ok = warp_knn_cov(m, p.x, p.y, p.z, lane, smem_w, c);
+            if (lane < 6) m.cov[(size_t)ref * 6 + lane] = c[lane];
+            if (lane == 0) m.cov_ok[ref] = ok ? 1 : 0;
+        }
     }
 }
 
-// same for calls larger than the covariance queue: every stored point with id >= first_id is a new point
-__global__ void __launch_bounds__(256, 5) knn_cov_new_ids_kernel(MapView m, uint32_t first_id, int warps_per_block) {
+// same for calls larger than the task list: every stored point with id >= the call's first id is a new point
+__global__ void __launch_bounds__(256, 5) knn_cov_new_ids_kernel(MapView m, int warps_per_block) {
     extern __shared__ __align__(16) char smem[];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     char* smem_w = smem + (size_t)wib * knn_smem_per_warp(m.k_cov);
+    const uint32_t first_id = (uint32_t)m.ctr->call_first_id;
     const int64_t nwarps = (int64_t)gridDim.x * warps_per_block;
     for (int64_t s = (int64_t)blockIdx.x * warps_per_block + wib; s < m.slots; s += nwarps) {
         const Entry e = m.table[s];
-        if (e.key == KEY_EMPTY || e.count == 0) continue;
-        for (uint32_t j = 0; j < e.count; ++j) {
-            const uint32_t ref = (uint32_t)s * m.cap + j;
+        const uint32_t cnt = entry_count(e.cr);
+        if (e.key == KEY_EMPTY || e.bucket >= BUCKET_PENDING || cnt == 0) continue;
+        for (uint32_t j = 0; j < cnt; ++j) {
+            const uint32_t ref = e.bucket * (uint32_t)m.cap + j;
             const float4 p = m.points[ref];
             if (__float_as_uint(p.w) < first_id) continue;
             float c[6];
@@ -284,20 +290,20 @@ static int knn_launch_cfg(const far_map* map, K kernel, int64_t work, KnnLaunch&
     return FAR_OK;
 }
 
-int launch_knn_cov_refs(const far_map* map, const uint32_t* d_refs, const unsigned int* d_n, int64_t n_max, cudaStream_t st) {
+int launch_knn_cov_tasks(const far_map* map, const uint2* d_tasks, const unsigned int* d_n, int64_t n_max, cudaStream_t st) {
     KnnLaunch L;
-    int rc = knn_launch_cfg(map, knn_cov_refs_kernel, n_max, L);
+    int rc = knn_launch_cfg(map, knn_cov_tasks_kernel, n_max, L);
     if (rc != FAR_OK) return rc;
-    FAR_LAUNCH(knn_cov_refs_kernel, L.grid, L.warps * 32, L.smem, st, map->view, d_refs, d_n, L.warps);
+    FAR_LAUNCH(knn_cov_tasks_kernel, L.grid, L.warps * 32, L.smem, st, map->view, d_tasks, d_n, L.warps);
     FAR_CUDA(cudaGetLastError());
     return FAR_OK;
 }
 
-int launch_knn_cov_new_ids(const far_map* map, uint32_t first_id, cudaStream_t st) {
+int launch_knn_cov_new_ids(const far_map* map, cudaStream_t st) {
     KnnLaunch L;
     int rc = knn_launch_cfg(map, knn_cov_new_ids_kernel, map->view.slots, L);
     if (rc != FAR_OK) return rc;
-    FAR_LAUNCH(knn_cov_new_ids_kernel, L.grid, L.warps * 32, L.smem, st, map->view, first_id, L.warps);
+    FAR_LAUNCH(knn_cov_new_ids_kernel, L.grid, L.warps * 32, L.smem, st, map->view, L.warps);
     FAR_CUDA(cudaGetLastError());
     return FAR_OK;
 }

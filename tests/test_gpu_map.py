@@ -178,16 +178,35 @@ def test_insert_is_deterministic_across_runs():
 
 
 def test_table_full_is_reported_not_fatal():
+    """FAR_ERR_FULL (far.h): the bucket pool is an exact limit; excess NEW voxels are dropped and counted; the status is
+    raised on the device, mirrored into pinned host memory and returned by later calls without a sync; pruning clears it."""
     rng = np.random.default_rng(12)
     pts = _cloud(rng, 20_000, scale=50.0, clustered=False)
     m = far.Map(0.5, 4, 1000)       # far fewer voxels than the cloud occupies
-    st = m.insert(pts)
-    assert st["n_dropped_full"] > 0
-    assert st["n_accepted"] + st["n_dropped_full"] <= st["n_offered"]
+    assert m.status() == far.OK
+    st = m.insert(pts)              # reads the statistics back: the kernels have run
+    assert st["n_dropped_full"] > 0 and st["n_new_voxels"] == 1000
+    assert st["n_accepted"] + st["n_dropped_full"] + st["n_invalid"] <= st["n_offered"]
     s = m.stats()
-    assert s["n_voxels"] <= 1000 + 256 * 148   # racy pre-check may overshoot by the threads in flight, never unbounded
+    assert s["n_voxels"] == 1000 and s["full"] == 1 and s["n_fresh_buckets"] == 0
+    assert m.status() == far.ERR_FULL
+    rc = far.lib().far_map_insert(m._h, None, 0, 3, None, 0, None, None)     # the C call itself reports it
+    assert rc == far.ERR_FULL
     e = m.export()
-    assert (e["counts"] <= 4).all() and (e["counts"] >= 1).all()
+    assert (e["counts"] <= 4).all() and (e["counts"] >= 1).all() and len(e["keys"]) == 1000
+    # every stored voxel holds exactly what the oracle stores for it (which voxels were dropped is unspecified, R3)
+    mo = oracle.Map(0.5, 4)
+    mo.insert(pts)
+    eo = mo.export()
+    pos = np.searchsorted(eo["keys"], e["keys"])
+    assert np.array_equal(eo["keys"][pos], e["keys"]) and np.array_equal(eo["ids"][pos], e["ids"])
+    # pruning frees buckets: the flag clears and new voxels are accepted again
+    pr = m.prune([0.0, 0.0, 0.0], 20.0)
+    assert pr["n_voxels_removed"] > 0
+    assert m.status() == far.OK and m.stats()["full"] == 0
+    near = (rng.uniform(-5, 5, size=(pr["n_voxels_removed"] // 4, 3)) + np.array([30.0, 30.0, 30.0])).astype(np.float32)
+    st2 = m.insert(near)
+    assert st2["n_dropped_full"] == 0 and st2["n_new_voxels"] > 0 and not m.full_seen
 
 
 # ---- A5 ---------------------------------------------------------------------------------------------------
@@ -215,27 +234,127 @@ def test_prune_matches_oracle_and_reinsert():
     _assert_same_map(mg.export(), mo.export())
 
 
-def test_rehash_and_clear_keep_contents_semantics():
+def test_dead_keys_rehash_and_clear_keep_contents_semantics():
     rng = np.random.default_rng(14)
     pts = _cloud(rng, 60_000, scale=30.0)
     mo, mg = oracle.Map(1.0, 20), far.Map(1.0, 20, 200_000, with_cov=True)
     mo.insert(pts, compute_cov=True); mg.insert(pts, compute_cov=True)
-    mo.prune([0, 0, 0], 20.0); mg.prune([0, 0, 0], 20.0)
-    dead_before = mg.stats()["n_dead_keys"]
-    assert dead_before > 0
-    mg.rehash()
+    n_live0 = mg.stats()["n_voxels"]
+    # a small prune leaves dead keys behind (below the rebuild threshold 32 + live / 8): absent for every query, re-usable
+    assert mo.prune([0, 0, 0], 49.0) == mg.prune([0, 0, 0], 49.0)
     st = mg.stats()
-    assert st["n_dead_keys"] == 0 and st["n_voxels"] == mo.size()[0]
+    assert 0 < st["n_dead_keys"] < 32 + st["n_voxels"] // 8 and st["n_rehash"] == 0
+    assert st["n_free_buckets"] == st["n_dead_keys"] and st["n_keys"] == n_live0
     _assert_same_map(mg.export(with_cov=True), mo.export(with_cov=True), with_cov=True)
-    q = _cloud(rng, 5000, scale=25.0)
+    q = _cloud(rng, 5000, scale=32.0)
     ids_o, d2_o = mo.nn(q)
     ids_g, d2_g = mg.nn(q)
     assert np.array_equal(ids_g.cpu().numpy().view(np.uint32), ids_o)
+    # a large prune passes the threshold: the prune call rebuilds the table itself (no dead keys afterwards)
+    assert mo.prune([0, 0, 0], 20.0) == mg.prune([0, 0, 0], 20.0)
+    st = mg.stats()
+    assert st["n_dead_keys"] == 0 and st["n_rehash"] == 1 and st["n_voxels"] == mo.size()[0] and st["n_keys"] == st["n_voxels"]
+    _assert_same_map(mg.export(with_cov=True), mo.export(with_cov=True), with_cov=True)
+    ids_o, d2_o = mo.nn(q)
+    ids_g, d2_g = mg.nn(q)
+    assert np.array_equal(ids_g.cpu().numpy().view(np.uint32), ids_o)
+    assert np.array_equal(d2_g.cpu().numpy().view(np.uint32), d2_o.view(np.uint32))
+    # freed buckets are re-used by later inserts (new voxels and re-created ones), contents still the oracle's
+    more = _cloud(rng, 30_000, scale=30.0)
+    assert mg.insert(more, compute_cov=True) == mo.insert(more, compute_cov=True)
+    _assert_same_map(mg.export(with_cov=True), mo.export(with_cov=True), with_cov=True)
+    # explicit rehash with a few dead keys
+    assert mo.prune([1, 0, 0], 29.0) == mg.prune([1, 0, 0], 29.0)
+    mg.rehash()
+    st = mg.stats()
+    assert st["n_dead_keys"] == 0 and st["n_keys"] == st["n_voxels"] == mo.size()[0]
+    _assert_same_map(mg.export(), mo.export())
     mg.clear()
     assert mg.size() == (0, 0, 0)
     mo2 = oracle.Map(1.0, 20)
     mo2.insert(pts[:1000]); mg.insert(pts[:1000])
     _assert_same_map(mg.export(), mo2.export())
+
+
+def test_renumber_matches_oracle_and_keeps_order():
+    """R22: ids -= smallest live id (also triggered automatically every `renumber_every` offered points)"""
+    rng = np.random.default_rng(15)
+    mo, mg = oracle.Map(1.0, 8), far.Map(1.0, 8, 100_000, renumber_every=50_000)
+    offered_since = 0
+    for b in range(12):
+        pts = (rng.uniform(-10, 10, size=(20_000, 3)) + np.array([8.0 * b, 0, 0])).astype(np.float32)
+        if offered_since > 0 and offered_since + len(pts) > 50_000:       # the library's deterministic trigger, restated
+            mo.renumber()
+            offered_since = 0
+        assert mg.insert(pts) == mo.insert(pts)
+        offered_since += len(pts)
+        c = [8.0 * b, 0.0, 0.0]
+        assert mg.prune(c, 12.0) == mo.prune(c, 12.0)
+        assert mg.size() == mo.size(), b
+    assert mo.size()[2] < 12 * 20_000                                  # the counter really was pulled back
+    _assert_same_map(mg.export(), mo.export())
+    sub = mo.renumber()
+    mg.renumber()
+    assert sub > 0 and mg.size() == mo.size()
+    e = mg.export()
+    _assert_same_map(e, mo.export())
+    assert e["ids"][e["counts"][:, None] > np.arange(8)[None, :]].min() == 0
+    q = (rng.uniform(-10, 10, size=(3000, 3)) + np.array([88.0, 0, 0])).astype(np.float32)
+    ids_g, _ = mg.nn(q)
+    assert np.array_equal(ids_g.cpu().numpy().view(np.uint32), mo.nn(q)[0])
+    mg.prune([0, 0, 0], 1.0); mo.prune([0, 0, 0], 1.0)                  # empties the map
+    mg.renumber(); mo.renumber()
+    assert mg.size() == mo.size() == (0, 0, 0)
+
+
+def test_sliding_window_5000_frames_never_fills_and_matches_oracle():
+    """PAPER.md:109 prunes every frame, :171,186 nothing may allocate: a 200 m window slides for 5,000 frames through a map
+    sized for the window only.  Buckets are recycled through the free list, dead keys are dropped by the prune calls'
+    own rebuilds, ids are renumbered on the way; the map never reports full and ends equal to the oracle's."""
+    rng = np.random.default_rng(16)
+    v, cap, step, radius, n_pts, frames = 1.0, 20, 7.0, 100.0, 1500, 5000
+    mo = oracle.Map(v, cap)
+    mg = far.Map(v, cap, 40_000, max_batch=4096, renumber_every=1_000_000)
+    assert mg.stats()["n_slots"] == 131072
+    offered_since, peak_dead, peak_live = 0, 0, 0
+    q0 = None
+    t_nn = {}
+
+    def time_nn(center):
+        q = torch.as_tensor((rng.uniform(-1, 1, size=(200_000, 3)) * np.array([90.0, 12.0, 3.0]) + center).astype(np.float32)).cuda()
+        ts = []
+        for _ in range(7):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); mg.nn(q); b.record(); torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        return float(np.median(ts[2:]))
+
+    for f in range(frames):
+        c = np.array([step * f, 0.0, 0.0])
+        # a corridor-shaped "scan": points up to 95 m ahead of and behind the sensor, 24 m wide, 6 m high
+        pts = (rng.uniform(-1, 1, size=(n_pts, 3)) * np.array([95.0, 12.0, 3.0]) + c).astype(np.float32)
+        if offered_since > 0 and offered_since + n_pts > 1_000_000:
+            mo.renumber()
+            offered_since = 0
+        mo.insert(pts)
+        mg.insert_enqueue(pts)
+        offered_since += n_pts
+        mo.prune(c, radius)
+        mg.prune_enqueue(c, radius)
+        if f % 250 == 249 or f == frames - 1:
+            st = mg.stats()
+            assert st["full"] == 0 and mg.status() == far.OK, f
+            assert (st["n_voxels"], st["n_points"], st["next_id"]) == mo.size(), f
+            peak_dead, peak_live = max(peak_dead, st["n_dead_keys"]), max(peak_live, st["n_voxels"])
+            assert st["n_dead_keys"] < 64 + st["n_voxels"] // 4, (f, st)
+            assert st["n_keys"] == st["n_voxels"] + st["n_dead_keys"]
+        if f in (249, frames - 1):
+            t_nn[f] = time_nn(c)
+    st = mg.stats()
+    assert st["n_rehash"] > 50 and peak_live <= 40_000 and mo.size()[2] < 2_500_000
+    _assert_same_map(mg.export(), mo.export())
+    # lookups are as fast at the end as at the start: dead keys and probe bounds do not accumulate
+    assert t_nn[frames - 1] < 1.15 * t_nn[249], t_nn
 
 
 # ---- A6 ---------------------------------------------------------------------------------------------------

@@ -283,3 +283,37 @@ def test_nn_multithreaded_equals_single():
     a = m.nn(c1["scan"], nthreads=1)
     b = m.nn(c1["scan"], nthreads=4)
     assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+
+
+def test_renumber_shifts_ids_by_the_minimum_and_nothing_else():
+    """R22 pin: after renumbering, the stored ids are the old ones minus their minimum (so order, contents, NN winners and
+    tie-breaks are those of the old ids), the counter moves by the same amount, and later ids continue from it."""
+    rng = np.random.default_rng(31)
+    pts = rng.uniform(-6, 6, size=(5000, 3)).astype(np.float32)
+    m = oracle.Map(1.0, 4)
+    m.insert(pts)
+    m.prune([20.0, 0.0, 0.0], 16.5)          # removes the voxels that hold the earliest ids near x = -6 ... some survive elsewhere
+    m.insert(pts[:100] + np.float32(0.01))
+    before = m.export()
+    stored = before["counts"][:, None] > np.arange(4)[None, :]
+    mn = int(before["ids"][stored].min())
+    nid = m.size()[2]
+    q = rng.uniform(-6, 6, size=(500, 3)).astype(np.float32)
+    ids0, d0 = m.nn(q)
+    sub = m.renumber()
+    after = m.export()
+    assert sub == mn and m.size()[2] == nid - mn
+    assert np.array_equal(after["keys"], before["keys"]) and np.array_equal(after["counts"], before["counts"])
+    assert np.array_equal(after["xyz"], before["xyz"])
+    assert np.array_equal(after["ids"][stored].astype(np.int64), before["ids"][stored].astype(np.int64) - mn)
+    ids1, d1 = m.nn(q)
+    hit = ids0 != oracle.NO_ID
+    assert np.array_equal(ids1[hit].astype(np.int64), ids0[hit].astype(np.int64) - mn) and np.array_equal(d1, d0)
+    assert np.array_equal(ids1[~hit], ids0[~hit])
+    assert m.renumber() == 0                  # idempotent: the minimum is now 0
+    st = m.insert(pts[:7])
+    e = m.export()
+    assert int(e["ids"][e["counts"][:, None] > np.arange(4)[None, :]].max()) <= nid - mn + 6
+    # an empty map restarts at 0
+    m.prune([1000.0, 0.0, 0.0], 1.0)
+    assert m.size()[0] == 0 and m.renumber() == nid - mn + 7 and m.size()[2] == 0
