@@ -182,9 +182,11 @@ int far_map_nn(const far_map_t* map, const float* d_q, int64_t m, int stride, ui
 int far_map_knn_cov(const far_map_t* map, const float* d_q, int64_t m, int stride, float* d_cov6,
                     uint8_t* d_valid, void* stream);
 
-/* number of candidate points in the 27 voxels around each query (what A6/A7 scan): density probe, used by
- * bench.py for the algorithmic-byte count and the quantity the ASMD rule averages */
-int far_map_count27(const far_map_t* map, const float* d_q, int64_t m, int stride, int32_t* d_count, void* stream);
+/* number of candidate points in the 27 voxels around each query (what A6/A7 scan) and, if d_voxels is not NULL, how many
+ * of the 27 voxels are occupied: density probe, used by bench.py for the algorithmic-byte count (27 keys +
+ * 4 B per occupied voxel + 16 B per candidate) */
+int far_map_count27(const far_map_t* map, const float* d_q, int64_t m, int stride, int32_t* d_count, int32_t* d_voxels,
+                    void* stream);
 
 /* A2 ("preprocessing (typically ... deskewing and downsampling)"; R2): one representative per
  * occupied voxel of the scan = the lowest-index valid point, emitted in ascending source index.

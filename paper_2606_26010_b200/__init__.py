@@ -124,7 +124,7 @@ def lib():
             "far_map_snapshot_create": (ci, [vp, vp, vp]),
             "far_map_snapshot_restore": (ci, [vp, vp, vp]),
             "far_map_snapshot_destroy": (ci, [vp]),
-            "far_map_count27": (ci, [vp, vp, i64, ci, vp, vp]),
+            "far_map_count27": (ci, [vp, vp, i64, ci, vp, vp, vp]),
             "far_map_export": (ci, [vp, vp, vp, vp, vp, vp, i64, vp, vp]),
             "far_voxel_keys": (ci, [vp, i64, ci, f32, vp, vp]),
             "far_map_nn": (ci, [vp, vp, i64, ci, vp, vp, vp]),
@@ -408,11 +408,13 @@ class Map:
     def snapshot_destroy(snap):
         lib().far_map_snapshot_destroy(snap)
 
-    def count27(self, q):
+    def count27(self, q, with_voxels=False):
+        """candidates in the 27 voxels around each query (and, optionally, how many of the 27 are occupied)"""
         x, n, s = _points(q)
         out = torch.empty(n, dtype=torch.int32, device=x.device)
-        _check(lib().far_map_count27(self._h, _ptr(x), n, s, _ptr(out), _stream()), "far_map_count27")
-        return out
+        vox = torch.empty(n, dtype=torch.int32, device=x.device) if with_voxels else None
+        _check(lib().far_map_count27(self._h, _ptr(x), n, s, _ptr(out), _ptr(vox), _stream()), "far_map_count27")
+        return (out, vox) if with_voxels else out
 
     def rehash(self):
         _check(lib().far_map_rehash(self._h, _stream()), "far_map_rehash")

@@ -30,15 +30,16 @@ namespace far {
 constexpr unsigned long long KEY_EMPTY = ~0ull;
 constexpr uint32_t NO_ID = 0xFFFFFFFFu;
 constexpr uint32_t NO_SLOT = 0xFFFFFFFFu;
-constexpr uint32_t NO_BUCKET = 0xFFFFFFFFu;        // key present, no points (never had any, or pruned)
-constexpr uint32_t BUCKET_PENDING = 0xFFFFFFFEu;   // a thread is allocating this voxel's bucket right now
+constexpr uint32_t NO_BUCKET = 0xFFFFFFFFu;        // key present, no points: pruned (dead key) or the pool was exhausted
+constexpr uint32_t BUCKET_PENDING = 0xFFFFFFFEu;   // the bucket word of every EMPTY slot; on a claimed key: the claimer (or
+                                                   // the thread that revives a dead key) is allocating the bucket right now
 constexpr int KEY_BIAS = 1 << 20;
 constexpr unsigned FULL = 0xFFFFFFFFu;
 
 struct __align__(16) Entry {
     unsigned long long key;
     uint32_t bucket;   // index into the dense pool, NO_BUCKET, or BUCKET_PENDING (only while an insert kernel runs)
-    uint32_t cr;       // bits 0..7: number of stored points; bits 8..31: reach of this HOME slot = 1 + the largest
+    uint32_t cr;       // bits 0..7: number of stored points; bits 8..31: reach of this HOME slot = the largest
                        // displacement of any key whose home slot this is (see find_voxel)
 };
 
@@ -49,16 +50,18 @@ struct Counters {
     unsigned int n_keys;              // claimed keys (live + dead)
     unsigned int n_dead;              // keys whose voxel was pruned since the last rehash
     unsigned int bump;                // buckets ever taken from the fresh end of the pool
-    int n_free;                       // entries on the free list (transiently negative inside an insert kernel)
+    int n_free;                       // entries on the free list
+    unsigned int n_alloc;             // buckets handed out by the running insert kernel: the first n_free of them come off the
+                                      // free list, the rest from the fresh end; folded into n_free / bump by the commit epilogue
     unsigned int full_flag;           // sticky until buckets are freed: a point was dropped (pool or table exhausted)
     unsigned int rehash_flag;         // written by prune's epilogue: the two rehash kernels that follow do their work
     unsigned int rehash_moved;        // entries moved by the running rehash
     unsigned int n_rehash;            // rehashes done since create / clear
     unsigned int ticket[4];           // last-block-done tickets: 0 insert commit, 1 prune, 2 clear, 3 renumber
     unsigned int n_touched;           // voxels that received a first new point in the current chunk
-    unsigned int n_tasks;             // covariance tasks (touched voxels) left by the last commit for knn_cov_tasks_kernel
+    unsigned int n_tasks;             // length of the covariance queue the last insert call left for knn_cov_refs_kernel
     unsigned int min_id;              // far_map_renumber: smallest live id
-    unsigned int pad0;
+    unsigned int n_cov;               // accepted points queued for covariance by the running insert call
     unsigned long long st_accepted, st_new_voxels, st_dropped_full, st_invalid;   // per-call statistics
     unsigned long long pr_vox_removed, pr_pts_removed, pr_vox_left, pr_pts_left;  // per-prune statistics
     unsigned long long scratch[8];    // stats / export / ASMD accumulators
@@ -183,26 +186,25 @@ __device__ __forceinline__ Entry load_entry(const Entry* table, uint32_t s) {
 }
 
 // read-only lookup: bucket of `key` and its count, or NO_BUCKET / count = 0 if absent or dead.  Linear probing, step 1
-// (PAPER.md:62).  The upper 24 bits of the entry at a key's HOME slot h hold `reach` = 1 + the largest displacement of any
-// key whose home is h (raised when a key is claimed, recomputed by every rehash).  A lookup therefore examines at most
-// reach(h) slots: a voxel that is not in the map -- 11 of the 27 neighbours of a typical query -- is usually dismissed by
-// the one home-entry load instead of a walk to the next empty slot, and the warp no longer waits for the longest of 27
-// such walks.  An EMPTY home slot means no key has that home (keys are only ever removed by a rebuild).
+// (PAPER.md:62).  The upper 24 bits of the entry at a key's HOME slot h hold `reach` = the largest displacement of any key
+// whose home is h (raised when a displaced key is claimed, recomputed by every rehash).  A lookup therefore examines the
+// slots h .. h + reach(h) only: a voxel that is not in the map -- 11 of the 27 neighbours of a typical query -- is usually
+// dismissed by the one home-entry load instead of a walk to the next empty slot, and the warp no longer waits for the
+// longest of 27 such walks.  An EMPTY home slot means no key has that home (keys are only ever removed by a rebuild).
 __device__ __forceinline__ uint32_t find_voxel(const MapView& m, unsigned long long key, uint32_t& count) {
     const uint32_t h = hash_key(key) & m.mask;
     Entry e = load_entry(m.table, h);
     count = 0;
     if (e.key == KEY_EMPTY) return NO_BUCKET;
     const uint32_t reach = entry_reach(e.cr);
-    for (uint32_t d = 0; d < reach; ++d) {
-        if (d) {
-            e = load_entry(m.table, (h + d) & m.mask);
-            if (e.key == KEY_EMPTY) break;
-        }
+    for (uint32_t d = 0;; ++d) {
         if (e.key == key) {
             count = entry_count(e.cr);
-            return count ? e.bucket : NO_BUCKET;
+            return (count && e.bucket < BUCKET_PENDING) ? e.bucket : NO_BUCKET;
         }
+        if (d >= reach) break;
+        e = load_entry(m.table, (h + d + 1) & m.mask);
+        if (e.key == KEY_EMPTY) break;
     }
     return NO_BUCKET;
 }
@@ -294,12 +296,6 @@ __device__ __forceinline__ uint32_t cand_next(const CandList& L, CandIter& it, i
     const int v = it.before + __popc(mk & (0xFFFFFFFFu >> (31 - lane))) - 1;
     it.before += __popc(mk);
     return L.slot[v] * (uint32_t)cap + (uint32_t)(j - L.off[v]);
-}
-
-__device__ __forceinline__ int probe27(const MapView& m, const int k[3], int lane, CandList& L) {
-    uint32_t cnt, slot;
-    probe27_regs(m, k, lane, cnt, slot);
-    return cand_build(L, cnt, slot, lane);
 }
 
 // warp-wide minimum of a non-negative double (its bit pattern orders like its value): two redux.sync steps

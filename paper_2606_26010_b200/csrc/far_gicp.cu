@@ -12,25 +12,28 @@
 // B200 design: a registration is a few thousand source points, i.e. latency- and issue-bound, never bandwidth-
 // bound, so the whole Gauss-Newton loop is ONE persistent cooperative kernel and every iteration is organised to
 // keep both the instruction count and the serial chain short:
-//   phase A0 8 lanes of warp 0 transform the block's 8 source points (FP64) and take their voxel indices: one
-//            instruction stream instead of 8 redundant warps; a warp's source point, covariance and flag stay in
-//            registers across iterations (one memory level less per iteration);
-//   phase A  one warp per source point: 27-voxel probe, bounded candidate sweep (far_common.cuh::warp_nearest), gate,
-//            fetch of Sigma_r -> one correspondence record in shared memory;
-//   phase B  the block's 8 correspondences are linearised by 8 lanes of warp 0 at once (the ~300 FP64 operations of
-//            M, weight, J^T M J are one instruction stream for 8 points instead of 8 streams with one active lane);
+//   phase A  one warp per source point, no block barrier before it: the warp transforms its point itself (FP64), and
+//            what the previous iteration learnt stays in registers -- the source point and its covariance, the 27 table
+//            lookups (valid as long as the transformed point stays in its voxel: the map does not change during a
+//            registration) and the previous nearest neighbour, whose distance to the new position bounds the search: a
+//            neighbour voxel is read only if its distance lower bound does not exceed it (exact, ties included).  From
+//            the second iteration on a search is usually one sweep over the point's own voxel, served by L1;
+//   phase B  the block's 8 correspondences are linearised by 8 lanes of warp 0 at once (one FP64 instruction stream for
+//            8 points: the FP64 pipe, not the issue slots, is what a per-warp linearisation would exhaust), column by
+//            column so that the live set fits the 48 registers five co-resident blocks per SM leave;
 //   reduce   the 29 unique terms of (H, b, chi2, n) go block -> group of 32 blocks -> grid as TAGGED rows: every
-//            value travels as {lo, tag, hi, tag} (two self-validating 8-byte words, tag = launch sequence and
-//            iteration), so a consumer just polls the rows it needs -- no fence, no ticket atomics -- and sums
-//            them in a fixed order (deterministic, no floating-point atomics);
-//   solve    block 0 / thread 0: 6x6 Cholesky, SE(3) exponential, pose update and stop test in FP64, published as
-//            13 tagged words; one lane per block polls the `done` word with a short back-off, then twelve lanes fetch
-//            the pose: one L2 round trip from "solved" to "next iteration" without the waiters crowding that slice.
-// Measured per iteration at C2 (5,352 points, debug-only globaltimer probes): A0+A 6.8 us, B 2.1, reduce 1.8, solve 2.2,
-// publish 1.1-2.0.  The arithmetic of B and solve is left exactly as it is: the C3 chain (tests/test_gpu_full_size.py)
-// amplifies a 1e-16 change of one increment to 2 fp32 ulps of a stored coordinate within 12 frames, along the
-// unobservable direction of the corridor.
+//            value travels as two 8-byte words {value half, tag} (tag = launch sequence and iteration), so a consumer
+//            just polls the rows it needs -- no fence, no ticket atomics -- and sums them in a fixed order
+//            (deterministic, no floating-point atomics);
+//   solve    warp 0 of block 0: 6x6 Cholesky with one row per lane (shuffles, no local memory), SE(3) exponential by
+//            series, pose update and stop test in FP64; thirteen lanes publish one tagged word each; one lane per block
+//            polls the `done` word with a short back-off, then twelve lanes fetch the pose.
 // The host is not involved until it reads the result.
+//
+// Tagged words and the PTX memory model: a word is written with st.relaxed.gpu.v2.u64 and read with ld.relaxed.gpu.v2.u64.
+// PTX treats a vector access as one scalar access per element, and an aligned 64-bit scalar access is single-copy atomic,
+// so each element {32 value bits, 32 tag bits} is observed whole or not at all; a reader accepts a value only when BOTH
+// elements carry the tag it waits for.  No ordering between different words is assumed anywhere.
 #include <cstring>
 
 #include "far_internal.h"
@@ -41,7 +44,8 @@ namespace far {
 
 constexpr int GWARPS = 8;        // warps per block = correspondences linearised together in phase B
 constexpr int NTERMS = 29;       // 21 (H upper triangle) + 6 (b) + chi2 + inlier count
-constexpr int TSTRIDE = 32;      // padded row
+constexpr int TSTRIDE = 32;      // row length of the tagged rows in global memory
+constexpr int SSTRIDE = 33;      // row length of the per-correspondence term rows in shared memory (no bank conflicts)
 
 constexpr int GROUP = 32;        // blocks per first-level reduction group
 constexpr int MAX_GROUPS = 64;
@@ -56,13 +60,6 @@ struct GicpScratch {
     uint4* pub;       // [16]: 13 published words; pub[15].x = launch sequence of this map (device-resident)
 };
 
-// one transformed source point, written by one lane of warp 0 in phase A0, read by its warp in phase A
-struct Src {
-    float p[3];       // T s (Eq. 2)
-    int k[3];         // its voxel index
-    int ok;           // 0: no point / non-finite / outside the key range
-};
-
 // one correspondence, written by its warp in phase A, read by one lane of warp 0 in phase B
 struct Corr {
     float p[3];       // transformed source point
@@ -71,7 +68,6 @@ struct Corr {
     float cr[6];      // Sigma_r
     int flags;        // bit 0: correspondence accepted, bit 1: both covariances valid
 };
-
 
 struct GicpParams {
     const float* scan;
@@ -89,23 +85,23 @@ struct GicpParams {
 };
 
 __device__ __forceinline__ void put_tagged(uint4* dst, double v, uint32_t tag) {
-    const unsigned long long b = (unsigned long long)__double_as_longlong(v);
-    asm volatile("st.relaxed.gpu.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "r"((uint32_t)b), "r"(tag),
-                 "r"((uint32_t)(b >> 32)), "r"(tag)
-                 : "memory");
+    const unsigned long long b = (unsigned long long)__double_as_longlong(v), t = (unsigned long long)tag << 32;
+    asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" ::"l"(dst), "l"(t | (b & 0xFFFFFFFFull)), "l"(t | (b >> 32)) : "memory");
 }
 
-__device__ __forceinline__ uint4 load_tagged(const uint4* src) {
-    uint4 w;
-    asm volatile("ld.relaxed.gpu.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w) : "l"(src) : "memory");
-    return w;
+// one attempt: true (and the value) iff both elements carry `tag`
+__device__ __forceinline__ bool load_tagged(const uint4* src, uint32_t tag, double& v) {
+    unsigned long long a, b;
+    asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(a), "=l"(b) : "l"(src) : "memory");
+    v = __longlong_as_double((long long)((b << 32) | (a & 0xFFFFFFFFull)));
+    return (uint32_t)(a >> 32) == tag && (uint32_t)(b >> 32) == tag;
 }
 
 // spins until both halves carry `tag` (volatile asm: the compiler must neither hoist the load nor assume the loop ends)
 __device__ __forceinline__ double wait_tagged(const uint4* src, uint32_t tag) {
-    uint4 w = load_tagged(src);
-    while (w.y != tag || w.w != tag) w = load_tagged(src);
-    return __longlong_as_double((long long)(((unsigned long long)w.z << 32) | w.x));
+    double v;
+    while (!load_tagged(src, tag, v)) {}
+    return v;
 }
 
 __device__ __forceinline__ double robust_weight(int kernel, double e2, double kappa) {
@@ -129,30 +125,35 @@ __device__ __forceinline__ bool inv_sym3(const double a[6], double o[6]) {
     return true;
 }
 
-// A9 for one correspondence: the 29 terms, written by lane 0 into s_terms
-__device__ __forceinline__ void correspondence_terms(const Pose& T, const double p[3], const double r[3], bool full,
-                                                      const float* cs, const float* cr, int kernel, double kappa,
-                                                      double* terms) {
-    const double d0 = r[0] - p[0], d1 = r[1] - p[1], d2 = r[2] - p[2];   // Eq. 3
+// A9 for one correspondence: the 29 terms, written straight into the correspondence's row of shared memory.  Ordered so
+// that few values are live at a time: S row by row -> M -> (M, Md, w) -> one column of X = M [p]x and of Y = [p]x^T X at
+// a time.  H = w J^T M J with J = [-I | A], A = [p]x:  [[M, -X], [-X^T, Y]];  b = w J^T M d = w [-Md ; A^T Md].
+__device__ __forceinline__ void correspondence_terms(const Pose& T, const Corr& c, int kernel, double kappa, double* terms) {
+    const double px = (double)c.p[0], py = (double)c.p[1], pz = (double)c.p[2];
+    const double d0 = (double)c.r[0] - px, d1 = (double)c.r[1] - py, d2 = (double)c.r[2] - pz;   // Eq. 3
     double M[6] = {1.0, 0.0, 0.0, 1.0, 0.0, 1.0};                        // SA fallback: Sigma_r = I, Sigma_s = 0
-    if (full) {
-        // S = Sigma_r + R Sigma_s R^T   (Eq. 4)
-        const double s[6] = {cs[0], cs[1], cs[2], cs[3], cs[4], cs[5]};
-        double RS[9];
-#pragma unroll
-        for (int i = 0; i < 3; ++i) {
-            const double a = T.R[3 * i], b = T.R[3 * i + 1], c = T.R[3 * i + 2];
-            RS[3 * i + 0] = a * s[0] + b * s[1] + c * s[2];
-            RS[3 * i + 1] = a * s[1] + b * s[3] + c * s[4];
-            RS[3 * i + 2] = a * s[2] + b * s[4] + c * s[5];
-        }
+    if (c.flags & 2) {
+        // S = Sigma_r + R Sigma_s R^T   (Eq. 4): row i of R Sigma_s, then its products with rows j >= i of R
+        const double s0 = c.cs[0], s1 = c.cs[1], s2 = c.cs[2], s3 = c.cs[3], s4 = c.cs[4], s5 = c.cs[5];
         double S[6];
-        S[0] = (double)cr[0] + (RS[0] * T.R[0] + RS[1] * T.R[1] + RS[2] * T.R[2]);
-        S[1] = (double)cr[1] + (RS[0] * T.R[3] + RS[1] * T.R[4] + RS[2] * T.R[5]);
-        S[2] = (double)cr[2] + (RS[0] * T.R[6] + RS[1] * T.R[7] + RS[2] * T.R[8]);
-        S[3] = (double)cr[3] + (RS[3] * T.R[3] + RS[4] * T.R[4] + RS[5] * T.R[5]);
-        S[4] = (double)cr[4] + (RS[3] * T.R[6] + RS[4] * T.R[7] + RS[5] * T.R[8]);
-        S[5] = (double)cr[5] + (RS[6] * T.R[6] + RS[7] * T.R[7] + RS[8] * T.R[8]);
+        {
+            const double a = T.R[0], b = T.R[1], e = T.R[2];
+            const double u0 = a * s0 + b * s1 + e * s2, u1 = a * s1 + b * s3 + e * s4, u2 = a * s2 + b * s4 + e * s5;
+            S[0] = (double)c.cr[0] + (u0 * T.R[0] + u1 * T.R[1] + u2 * T.R[2]);
+            S[1] = (double)c.cr[1] + (u0 * T.R[3] + u1 * T.R[4] + u2 * T.R[5]);
+            S[2] = (double)c.cr[2] + (u0 * T.R[6] + u1 * T.R[7] + u2 * T.R[8]);
+        }
+        {
+            const double a = T.R[3], b = T.R[4], e = T.R[5];
+            const double u0 = a * s0 + b * s1 + e * s2, u1 = a * s1 + b * s3 + e * s4, u2 = a * s2 + b * s4 + e * s5;
+            S[3] = (double)c.cr[3] + (u0 * T.R[3] + u1 * T.R[4] + u2 * T.R[5]);
+            S[4] = (double)c.cr[4] + (u0 * T.R[6] + u1 * T.R[7] + u2 * T.R[8]);
+        }
+        {
+            const double a = T.R[6], b = T.R[7], e = T.R[8];
+            const double u0 = a * s0 + b * s1 + e * s2, u1 = a * s1 + b * s3 + e * s4, u2 = a * s2 + b * s4 + e * s5;
+            S[5] = (double)c.cr[5] + (u0 * T.R[6] + u1 * T.R[7] + u2 * T.R[8]);
+        }
         double Mi[6];
         if (inv_sym3(S, Mi)) {
 #pragma unroll
@@ -164,160 +165,205 @@ __device__ __forceinline__ void correspondence_terms(const Pose& T, const double
     const double Md2 = M[2] * d0 + M[4] * d1 + M[5] * d2;
     const double e2 = d0 * Md0 + d1 * Md1 + d2 * Md2;
     const double w = robust_weight(kernel, e2, kappa);
-    const double px = p[0], py = p[1], pz = p[2];
-    // X = M A with A = [p]x :  column 0 = M(:,1) pz - M(:,2) py, column 1 = -M(:,0) pz + M(:,2) px, column 2 = M(:,0) py - M(:,1) px
-    const double Mr[3][3] = {{M[0], M[1], M[2]}, {M[1], M[3], M[4]}, {M[2], M[4], M[5]}};
-    double X[3][3];
-#pragma unroll
-    for (int r_ = 0; r_ < 3; ++r_) {
-        X[r_][0] = Mr[r_][1] * pz - Mr[r_][2] * py;
-        X[r_][1] = Mr[r_][2] * px - Mr[r_][0] * pz;
-        X[r_][2] = Mr[r_][0] * py - Mr[r_][1] * px;
-    }
-    // Y = A^T X (symmetric):  row 0 = pz X[1] - py X[2], row 1 = px X[2] - pz X[0], row 2 = py X[0] - px X[1]
-    const double Y00 = pz * X[1][0] - py * X[2][0], Y01 = pz * X[1][1] - py * X[2][1], Y02 = pz * X[1][2] - py * X[2][2];
-    const double Y11 = px * X[2][1] - pz * X[0][1], Y12 = px * X[2][2] - pz * X[0][2];
-    const double Y22 = py * X[0][2] - px * X[1][2];
-    // H = w J^T M J with J = [-I | A]:  [[M, -X], [-X^T, Y]];   b = w J^T M d = w [-Md ; A^T Md]
-    terms[0] = w * M[0];  terms[1] = w * M[1];  terms[2] = w * M[2];  terms[3] = -w * X[0][0]; terms[4] = -w * X[0][1]; terms[5] = -w * X[0][2];
-    terms[6] = w * M[3];  terms[7] = w * M[4];  terms[8] = -w * X[1][0]; terms[9] = -w * X[1][1]; terms[10] = -w * X[1][2];
-    terms[11] = w * M[5]; terms[12] = -w * X[2][0]; terms[13] = -w * X[2][1]; terms[14] = -w * X[2][2];
-    terms[15] = w * Y00;  terms[16] = w * Y01;  terms[17] = w * Y02;
-    terms[18] = w * Y11;  terms[19] = w * Y12;
-    terms[20] = w * Y22;
+    terms[0] = w * M[0];  terms[1] = w * M[1];  terms[2] = w * M[2];
+    terms[6] = w * M[3];  terms[7] = w * M[4];  terms[11] = w * M[5];
     terms[21] = -w * Md0; terms[22] = -w * Md1; terms[23] = -w * Md2;
     terms[24] = w * (pz * Md1 - py * Md2);
     terms[25] = w * (px * Md2 - pz * Md0);
     terms[26] = w * (py * Md0 - px * Md1);
     terms[27] = w * e2;
     terms[28] = 1.0;
+    // column 0 of X = M A:  X[r][0] = M[r][1] pz - M[r][2] py;   Y[i][0] = (A^T X)[i][0]
+    {
+        const double x0 = M[1] * pz - M[2] * py, x1 = M[3] * pz - M[4] * py, x2 = M[4] * pz - M[5] * py;
+        terms[3] = -w * x0; terms[8] = -w * x1; terms[12] = -w * x2;
+        terms[15] = w * (pz * x1 - py * x2);                               // Y00
+    }
+    // column 1:  X[r][1] = M[r][2] px - M[r][0] pz
+    {
+        const double x0 = M[2] * px - M[0] * pz, x1 = M[4] * px - M[1] * pz, x2 = M[5] * px - M[2] * pz;
+        terms[4] = -w * x0; terms[9] = -w * x1; terms[13] = -w * x2;
+        terms[16] = w * (pz * x1 - py * x2);                               // Y01
+        terms[18] = w * (px * x2 - pz * x0);                               // Y11
+    }
+    // column 2:  X[r][2] = M[r][0] py - M[r][1] px
+    {
+        const double x0 = M[0] * py - M[1] * px, x1 = M[1] * py - M[3] * px, x2 = M[2] * py - M[4] * px;
+        terms[5] = -w * x0; terms[10] = -w * x1; terms[14] = -w * x2;
+        terms[17] = w * (pz * x1 - py * x2);                               // Y02
+        terms[19] = w * (px * x2 - pz * x0);                               // Y12
+        terms[20] = w * (py * x0 - px * x1);                               // Y22
+    }
 }
 
-// 6x6 Cholesky solve H x = rhs (FP64), fully unrolled so L lives in registers; one rsqrt per pivot and
-// multiplications by the reciprocal pivots instead of 27 divisions (this thread is the serial section of every
-// Gauss-Newton iteration).  false if H is not positive definite.
-__device__ __forceinline__ bool chol_solve6(const double* H, const double* rhs, double* x) {
-    double L[6][6], inv[6];
+// A6 with what earlier iterations learnt: `cnt` / `bucket` are the warp's 27 lookups for voxel k (lane l < 27), `bound0`
+// an upper bound of the answer's d2 (+inf if none): the distance to a stored point that lies in the 27 voxels.  A voxel is
+// read only if its distance lower bound does not exceed the bound; without a bound the point's own voxel is swept first
+// to get one.  Exactly the (d2, id) minimum of R6: a skipped voxel holds only points strictly farther than the bound.
+__device__ __forceinline__ Best nearest_bounded(const MapView& m, float qx, float qy, float qz, const int k[3], int lane,
+                                                uint32_t cnt, uint32_t bucket, double bound0, CandList& L, float& rx, float& ry, float& rz) {
+    const double INF = __longlong_as_double(0x7FF0000000000000ll);
+    Best best;
+    best.d2 = INF; best.id = NO_ID; best.ref = 0;
+    float bx = 0.f, by = 0.f, bz = 0.f;
+    double bound = bound0;
+    const bool have_bound = bound0 < INF;
+    if (!have_bound) {
+        const uint32_t c_cnt = __shfl_sync(FULL, cnt, 13), c_bucket = __shfl_sync(FULL, bucket, 13);
+        for (uint32_t j = lane; j < c_cnt; j += 32) {
+            const uint32_t ref = c_bucket * (uint32_t)m.cap + j;
+            const float4 p = __ldg(m.points + ref);
+            const double d2 = dist2(qx, qy, qz, p.x, p.y, p.z);
+            const uint32_t id = __float_as_uint(p.w);
+            if (better(d2, id, best)) { best.d2 = d2; best.id = id; best.ref = ref; bx = p.x; by = p.y; bz = p.z; }
+        }
+        bound = warp_min_nonneg(best.d2);
+    }
+    uint32_t c2 = 0;
+    if (lane < 27 && cnt > 0 && (have_bound || lane != 13)) {
+        const double lb = (lane == 13) ? 0.0 : voxel_lower_bound(qx, qy, qz, k, m.voxel, lane / 9 - 1, (lane / 3) % 3 - 1, lane % 3 - 1);
+        if (lb <= bound) c2 = cnt;
+    }
+    const int total = cand_build(L, c2, bucket, lane);
+    CandIter ci;
+    ci.before = 0;
+    for (int j = lane, step = 0; j < total; j += 32, ++step) {
+        const uint32_t ref = cand_next(L, ci, step, j, lane, m.cap);
+        const float4 p = __ldg(m.points + ref);
+        const double d2 = dist2(qx, qy, qz, p.x, p.y, p.z);
+        const uint32_t id = __float_as_uint(p.w);
+        if (better(d2, id, best)) { best.d2 = d2; best.id = id; best.ref = ref; bx = p.x; by = p.y; bz = p.z; }
+    }
+    __syncwarp();
+    const int w = warp_argmin(best.d2, best.id);
+    best.d2 = __shfl_sync(FULL, best.d2, w);
+    best.id = __shfl_sync(FULL, best.id, w);
+    best.ref = __shfl_sync(FULL, best.ref, w);
+    rx = __shfl_sync(FULL, bx, w); ry = __shfl_sync(FULL, by, w); rz = __shfl_sync(FULL, bz, w);
+    return best;
+}
+
+// 6x6 Cholesky solve H x = rhs by one warp: lane i < 6 owns row i (H is read from the packed upper triangle `tv` in
+// shared memory as it is needed) and rhs_i; every lane returns all of x.  The factor's row i lives in lane i's registers
+// with the RECIPROCAL pivot in place of L_ii (the pivot itself is never needed again); rows talk through shuffles, so
+// nothing spills and the six pivots are the only serial chain.  One rsqrt per pivot.  false if H is not positive
+// definite.  All 32 lanes must call (lanes >= 6 compute on row 5's data and are ignored).
+__device__ __forceinline__ bool warp_chol_solve6(const double* tv, double rhs, int lane, double x[6]) {
+    const int i = min(lane, 5);
+    double l[6];
+    bool ok = true;
 #pragma unroll
     for (int j = 0; j < 6; ++j) {
-        double s = H[6 * j + j];
+        const int a = min(i, j), c = max(i, j);
+        double acc = tv[a * 6 - a * (a - 1) / 2 + (c - a)];                        // H_ij
 #pragma unroll
-        for (int k = 0; k < j; ++k) s -= L[j][k] * L[j][k];
-        if (!(s > 0.0) || !isfinite(s)) return false;
-        inv[j] = rsqrt(s);
-        L[j][j] = s * inv[j];
+        for (int k = 0; k < j; ++k) acc -= l[k] * __shfl_sync(FULL, l[k], j);     // H_ij - sum_k L_ik L_jk
+        const double piv = __shfl_sync(FULL, acc, j);
+        ok = ok && piv > 0.0 && isfinite(piv);
+        const double inv = rsqrt(piv);
+        l[j] = (lane == j) ? inv : acc * inv;                                      // lanes i < j hold garbage: never read
+    }
+    // forward: y_k = (rhs_k - sum_{j<k} L_kj y_j) / L_kk, finished on lane k and broadcast
+    double y = rhs, z = 0.0;
 #pragma unroll
-        for (int i = j + 1; i < 6; ++i) {
-            double t = H[6 * i + j];
+    for (int k = 0; k < 6; ++k) {
+        const double yk = __shfl_sync(FULL, y * l[k], k);
+        if (lane == k) z = yk;
+        y -= l[k] * yk;                                                             // lanes i > k; others unused
+    }
+    // backward: x_k = (y_k - sum_{i>k} L_ik x_i) / L_kk; L_ik sits in lane i, which sends its product to lane k
 #pragma unroll
-            for (int k = 0; k < j; ++k) t -= L[i][k] * L[j][k];
-            L[i][j] = t * inv[j];
+    for (int k = 5; k >= 0; --k) {
+        const double xk = __shfl_sync(FULL, z * l[k], k);
+        x[k] = xk;
+#pragma unroll
+        for (int q = 0; q < k; ++q) {
+            const double c = __shfl_sync(FULL, l[q] * xk, k);                      // lane k's L_kq x_k, for lane q
+            if (lane == q) z -= c;
         }
     }
-    double y[6];
-#pragma unroll
-    for (int i = 0; i < 6; ++i) {
-        double t = rhs[i];
-#pragma unroll
-        for (int k = 0; k < i; ++k) t -= L[i][k] * y[k];
-        y[i] = t * inv[i];
-    }
-#pragma unroll
-    for (int i = 5; i >= 0; --i) {
-        double t = y[i];
-#pragma unroll
-        for (int k = i + 1; k < 6; ++k) t -= L[k][i] * x[k];
-        x[i] = t * inv[i];
-    }
-    return true;
+    return ok;
 }
 
-// SE(3) exponential of delta = (rho, phi), translation first (R12); series below theta = 1e-8
-__device__ __forceinline__ void se3_exp(const double* d, Pose& E) {
-    const double px = d[3], py = d[4], pz = d[5];
-    const double th2 = px * px + py * py + pz * pz;
-    const double th = sqrt(th2);
-    double A, B, C;
-    if (th < 1e-8) {
-        A = 1.0 - th2 / 6.0; B = 0.5 - th2 / 24.0; C = 1.0 / 6.0 - th2 / 120.0;
+// coefficients of the SE(3) exponential: A = sin t / t, B = (1 - cos t) / t^2, C = (t - sin t) / t^3.  Series in t^2 up
+// to t^10 below 0.1 rad (remainder < 1e-21 relative: a Gauss-Newton increment is always that small unless the initial
+// guess is far off), the closed forms above.
+__device__ __forceinline__ void exp_coefficients(double th2, double& A, double& B, double& C) {
+    if (th2 < 0.01) {
+        A = 1.0 + th2 * (-1.0 / 6.0 + th2 * (1.0 / 120.0 + th2 * (-1.0 / 5040.0 + th2 * (1.0 / 362880.0 + th2 * (-1.0 / 39916800.0)))));
+        B = 0.5 + th2 * (-1.0 / 24.0 + th2 * (1.0 / 720.0 + th2 * (-1.0 / 40320.0 + th2 * (1.0 / 3628800.0 + th2 * (-1.0 / 479001600.0)))));
+        C = 1.0 / 6.0 + th2 * (-1.0 / 120.0 + th2 * (1.0 / 5040.0 + th2 * (-1.0 / 362880.0 + th2 * (1.0 / 39916800.0 + th2 * (-1.0 / 6227020800.0)))));
     } else {
+        const double th = sqrt(th2);
         double sn, cs;
         sincos(th, &sn, &cs);
-        const double ith = 1.0 / th, ith2 = ith * ith;
-        A = sn * ith; B = (1.0 - cs) * ith2; C = (th - sn) * ith2 * ith;
+        const double ith2 = 1.0 / th2;
+        A = sn / th; B = (1.0 - cs) * ith2; C = (th - sn) * ith2 / th;
     }
-    const double K[9] = {0, -pz, py, pz, 0, -px, -py, px, 0};
-    // K^2 = phi phi^T - |phi|^2 I
-    const double K2[9] = {px * px - th2, px * py, px * pz, px * py, py * py - th2, py * pz, px * pz, py * pz, pz * pz - th2};
-    double V[9];
-#pragma unroll
-    for (int i = 0; i < 9; ++i) {
-        const double I = (i % 4 == 0) ? 1.0 : 0.0;
-        E.R[i] = I + A * K[i] + B * K2[i];
-        V[i] = I + B * K[i] + C * K2[i];
-    }
-#pragma unroll
-    for (int r = 0; r < 3; ++r) E.t[r] = V[3 * r] * d[0] + V[3 * r + 1] * d[1] + V[3 * r + 2] * d[2];
 }
 
-// Serial section of one iteration (thread 0 of block 0): assemble H, b from the 29 reduced terms, solve, update
-// the pose, decide termination, write the result when done.  Returns the new pose and the done flag.
-__device__ __forceinline__ bool solve_and_update(const GicpParams& P, const double* tv, const Pose& T, int it, Pose& Tn) {
-    double H[36], b[6];
-    {
-        int q = 0;
-#pragma unroll
-        for (int a = 0; a < 6; ++a)
-#pragma unroll
-            for (int c = a; c < 6; ++c) { H[6 * a + c] = tv[q]; H[6 * c + a] = tv[q]; ++q; }
-    }
-#pragma unroll
-    for (int a = 0; a < 6; ++a) b[a] = tv[21 + a];
+// Serial section of one iteration, run by warp 0 of block 0 (all 32 lanes call): H, b from the 29 reduced terms `tv`
+// (shared memory), solve, SE(3) exponential, pose update, stop test; lanes 0..12 publish one tagged word each, the result
+// struct is written lane-parallel when the registration ends.
+__device__ __forceinline__ void solve_and_publish(const GicpParams& P, const double* tv, const Pose& T, int it, int lane, uint32_t tag) {
+    // index of H[a][c] (a <= c) in the packed upper triangle
+    auto tri = [](int a, int c) { return a * 6 - a * (a - 1) / 2 + (c - a); };
+    const double rhs = -tv[21 + min(lane, 5)];
     const int n_inl = (int)(tv[28] + 0.5);
+    double delta[6];
+    const bool solved = warp_chol_solve6(tv, rhs, lane, delta);
     bool done = false;
     int converged = 0, status = FAR_OK;
-    Tn = T;
-    if (!P.linearize_only) {
-        double rhs[6], delta[6];
-#pragma unroll
-        for (int a = 0; a < 6; ++a) rhs[a] = -b[a];
-        if (n_inl < 6 || !chol_solve6(H, rhs, delta)) {
-            status = FAR_ERR_DEGENERATE;
-            Tn = P.d_init ? *P.d_init : P.init;
-            done = true;
-        } else {
-            Pose E;
-            se3_exp(delta, E);
-#pragma unroll
-            for (int i = 0; i < 3; ++i)
-#pragma unroll
-                for (int j = 0; j < 3; ++j)
-                    Tn.R[3 * i + j] = E.R[3 * i] * T.R[j] + E.R[3 * i + 1] * T.R[3 + j] + E.R[3 * i + 2] * T.R[6 + j];
-#pragma unroll
-            for (int r = 0; r < 3; ++r)
-                Tn.t[r] = (E.R[3 * r] * T.t[0] + E.R[3 * r + 1] * T.t[1] + E.R[3 * r + 2] * T.t[2]) + E.t[r];
-            double nrm = 0.0;
-#pragma unroll
-            for (int a = 0; a < 6; ++a) nrm += delta[a] * delta[a];
-            if (nrm <= P.conv_eps * P.conv_eps) { converged = 1; done = true; }   // PAPER.md:100, R13: ||delta||_2 <= eps
-        }
-    } else {
+    // the element of the new pose this lane owns: lanes 0..8 R (row-major), 9..11 t
+    double mine = 0.0;
+    const int r = lane < 9 ? lane / 3 : lane - 9, cidx = lane % 3;
+    if (P.linearize_only) {
         done = true;
+        if (lane < 9) mine = T.R[lane]; else if (lane < 12) mine = T.t[lane - 9];
+    } else if (n_inl < 6 || !solved) {
+        status = FAR_ERR_DEGENERATE;
+        done = true;
+        const Pose& I0 = P.d_init ? *P.d_init : P.init;
+        if (lane < 9) mine = I0.R[lane]; else if (lane < 12) mine = I0.t[lane - 9];
+    } else {
+        const double px = delta[3], py = delta[4], pz = delta[5];
+        const double th2 = px * px + py * py + pz * pz;
+        double A, B, C;
+        exp_coefficients(th2, A, B, C);
+        // row r of E.R = I + A K + B K^2 and of V = I + B K + C K^2, K = [phi]x, K^2 = phi phi^T - |phi|^2 I
+        const double ph[3] = {px, py, pz};
+        const double pr = r == 0 ? px : (r == 1 ? py : pz);
+        double er[3], vr[3];
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            const double k2 = pr * ph[j] - (j == r ? th2 : 0.0);
+            // K[r][j]: (0,1) -pz (0,2) py (1,0) pz (1,2) -px (2,0) -py (2,1) px
+            double kk = 0.0;
+            if (r == 0) kk = j == 1 ? -pz : (j == 2 ? py : 0.0);
+            else if (r == 1) kk = j == 0 ? pz : (j == 2 ? -px : 0.0);
+            else kk = j == 0 ? -py : (j == 1 ? px : 0.0);
+            const double id = j == r ? 1.0 : 0.0;
+            er[j] = id + A * kk + B * k2;
+            vr[j] = id + B * kk + C * k2;
+        }
+        if (lane < 9) mine = er[0] * T.R[cidx] + er[1] * T.R[3 + cidx] + er[2] * T.R[6 + cidx];
+        else if (lane < 12) mine = (er[0] * T.t[0] + er[1] * T.t[1] + er[2] * T.t[2]) + (vr[0] * delta[0] + vr[1] * delta[1] + vr[2] * delta[2]);
+        double nrm = 0.0;
+#pragma unroll
+        for (int a = 0; a < 6; ++a) nrm += delta[a] * delta[a];
+        if (nrm <= P.conv_eps * P.conv_eps) { converged = 1; done = true; }   // PAPER.md:100, R13: ||delta||_2 <= eps
     }
     if (it + 1 >= P.max_iters) done = true;
+    if (lane < 12) put_tagged(P.scratch.pub + lane, mine, tag);
     if (done) {
         far_gicp_result_t* out = P.out;
-        for (int a = 0; a < 9; ++a) out->pose.R[a] = Tn.R[a];
-        for (int a = 0; a < 3; ++a) out->pose.t[a] = Tn.t[a];
-        for (int a = 0; a < 36; ++a) out->H[a] = H[a];
-        for (int a = 0; a < 6; ++a) out->b[a] = b[a];
-        out->chi2 = tv[27];
-        out->n_inliers = n_inl;
-        out->iters = it + 1;
-        out->converged = converged;
-        out->status = status;
+        if (lane < 9) out->pose.R[lane] = mine; else if (lane < 12) out->pose.t[lane - 9] = mine;
+        for (int a = lane; a < 36; a += 32) { const int i = a / 6, j = a % 6; out->H[a] = tv[i <= j ? tri(i, j) : tri(j, i)]; }
+        if (lane < 6) out->b[lane] = tv[21 + lane];
+        if (lane == 6) out->chi2 = tv[27];
+        if (lane == 7) { out->n_inliers = n_inl; out->iters = it + 1; out->converged = converged; out->status = status; }
     }
-    return done;
+    if (lane == 12) put_tagged(P.scratch.pub + 12, done ? 1.0 : 0.0, tag);
 }
 
 // Polls `count` tagged rows starting at `first` (column = lane) and sums them: warp w takes rows w, w + 8, ... in
@@ -337,113 +383,131 @@ __device__ __forceinline__ double block_sum_tagged(const uint4* rows, int first,
     return t;   // valid in warp 0
 }
 
-__global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(MapView m, GicpParams P) {
+// what a warp keeps about its source point from one iteration to the next (shared memory: 30-cycle reads instead of
+// registers the FP64 linearisation needs)
+struct WarpState {
+    float s[3];       // the source point (sensor frame)
+    float pr[3];      // previous nearest neighbour
+    int kp[3];        // voxel of the transformed point at the last table walk
+    uint32_t pref;    // reference of the previous nearest neighbour
+};
+
+__global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(const __grid_constant__ MapView m, const __grid_constant__ GicpParams P) {
     __shared__ CandList s_list[GWARPS];
-    __shared__ double s_terms[GWARPS][TSTRIDE];
+    __shared__ double s_terms[GWARPS][SSTRIDE];
     __shared__ double s_red[GWARPS][TSTRIDE];
     __shared__ Corr s_corr[GWARPS];
-    __shared__ Src s_src[GWARPS];
+    __shared__ WarpState s_state[GWARPS];
     __shared__ Pose s_T;
     __shared__ int s_done;
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    const int64_t nwarps = (int64_t)gridDim.x * GWARPS;
+    const int nwarps = (int)gridDim.x * GWARPS;
     // launch sequence: read by every block at start, advanced by block 0 at the very end (launches on one map are
     // stream-ordered), so every launch has its own tag space without a host-side counter or a kernel argument
     const uint32_t seq = *reinterpret_cast<volatile uint32_t*>(&P.scratch.pub[15].x);
-    int64_t n = P.n;
-    if (P.d_n) n = min(n, *P.d_n);
+    int n = (int)P.n;
+    if (P.d_n) n = (int)min((int64_t)n, *P.d_n);
     if (threadIdx.x < 12) {
         const Pose& src = P.d_init ? *P.d_init : P.init;
         double vv = threadIdx.x < 9 ? src.R[threadIdx.x] : src.t[threadIdx.x - 9];
         if (threadIdx.x < 9) s_T.R[threadIdx.x] = vv; else s_T.t[threadIdx.x - 9] = vv;
     }
-    __syncthreads();
-    const int n_groups = (gridDim.x + GROUP - 1) / GROUP;
-    const int group = blockIdx.x / GROUP;
-    const int group_rows = min(GROUP, (int)gridDim.x - group * GROUP);
     const bool have_scan_cov = P.cov6 != nullptr && P.valid != nullptr && m.cov != nullptr;
-    const int rounds = (int)((n + nwarps - 1) / nwarps);      // source points per warp (1 when n <= resident warps)
+    const int rounds = (n + nwarps - 1) / nwarps;             // source points per warp (1 when n <= resident warps)
+    const double INF = __longlong_as_double(0x7FF0000000000000ll);
 
-    // one source point per warp (n <= resident warps, the usual case): the point, its covariance and flag are the same
-    // in every iteration, so they are fetched once and stay in registers -- one memory level less per iteration.
-    // Lane l < 8 of warp 0 holds the point of warp l (phase A0), lanes 8..14 of every warp its own covariance and flag.
+    // one source point per warp (n <= resident warps, the usual case): everything that does not depend on the pose is
+    // fetched once and kept across iterations -- the point in shared memory, its covariance in lanes 8..13 and its flag
+    // in lane 14.  What an iteration learns is kept too: the voxel the transformed point fell into with its 27 lookups
+    // (lane l < 27: count, bucket), the nearest neighbour (reference, coordinates) and, in lanes 0..6, that
+    // neighbour's covariance and flag.
     const bool resident = rounds == 1;
-    float sx0 = 0.f, sy0 = 0.f, sz0 = 0.f, cin0 = 0.f;
+    WarpState& ws = s_state[wib];
+    float cin0 = 0.f;
     if (resident) {
-        if (wib == 0 && lane < GWARPS) {
-            const int64_t i = (int64_t)blockIdx.x * GWARPS + lane;
-            sx0 = sy0 = sz0 = __int_as_float(0x7FC00000);     // NaN: no point
-            if (i < n) {
-                const float* sp = P.scan + i * P.stride;
-                sx0 = __ldg(sp); sy0 = __ldg(sp + 1); sz0 = __ldg(sp + 2);
+        const int i = (int)blockIdx.x * GWARPS + wib;
+        if (i < n) {
+            if (lane < 3) ws.s[lane] = __ldg(P.scan + (int64_t)i * P.stride + lane);
+            if (have_scan_cov) {
+                if (lane >= 8 && lane < 14) cin0 = __ldg(P.cov6 + 6 * (int64_t)i + (lane - 8));
+                if (lane == 14) cin0 = (float)__ldg(P.valid + i);
             }
         }
-        const int64_t i = (int64_t)blockIdx.x * GWARPS + wib;
-        if (i < n && have_scan_cov) {
-            if (lane >= 8 && lane < 14) cin0 = __ldg(P.cov6 + 6 * i + (lane - 8));
-            if (lane == 14) cin0 = (float)__ldg(P.valid + i);
-        }
     }
+    __syncthreads();
+    uint32_t have = 0;                    // bit 0: the 27 lookups are those of voxel ws.kp; bit 1: ws.pr / ws.pref are set
+    uint32_t pcnt = 0, pbucket = NO_BUCKET;
+    float cinr = 0.f;
 
     for (int it = 0; it < P.max_iters; ++it) {
         const uint32_t tag = (seq << 10) | (uint32_t)(it + 1);
         double acc = 0.0;                                     // warp 0, lane t < 29: term t of this block
         for (int rd = 0; rd < rounds; ++rd) {
-            // ---- phase A0 (Eq. 2, A1): 8 lanes of warp 0 transform the block's 8 source points with the accumulated pose
-            // (R11) and take their voxel indices: one instruction stream for 8 points instead of 8 redundant warps ------
-            if (wib == 0 && lane < GWARPS) {
-                float sx = sx0, sy = sy0, sz = sz0;
-                if (!resident) {
-                    const int64_t i = (int64_t)rd * nwarps + (int64_t)blockIdx.x * GWARPS + lane;
-                    sx = sy = sz = __int_as_float(0x7FC00000);
-                    if (i < n) {
-                        const float* sp = P.scan + i * P.stride;
-                        sx = __ldg(sp); sy = __ldg(sp + 1); sz = __ldg(sp + 2);
-                    }
-                }
-                Src o;
-                o.ok = 0;
-                o.p[0] = o.p[1] = o.p[2] = 0.f;
-                o.k[0] = o.k[1] = o.k[2] = 0;
-                if (isfinite(sx) && isfinite(sy) && isfinite(sz)) {
-                    transform_point(s_T, sx, sy, sz, o.p);
-                    o.ok = voxel_index(o.p[0], o.p[1], o.p[2], m.voxel, o.k) ? 1 : 0;
-                }
-                s_src[lane] = o;
-            }
-            __syncthreads();
-            // ---- phase A (A8): one warp per source point -> correspondence record ---------------------------------
-            const int64_t i = (int64_t)rd * nwarps + (int64_t)blockIdx.x * GWARPS + wib;
+            // ---- phase A (Eq. 2, A1, A6, A8): one warp per source point -> correspondence record ---------------------
+            const int i = rd * nwarps + (int)blockIdx.x * GWARPS + wib;
             int flags = 0;
             if (i < n) {
-                float cin = cin0;
-                if (!resident && have_scan_cov) {
-                    // the source covariance does not depend on the search: lanes 8..13 fetch it now, lane 14 its flag
-                    if (lane >= 8 && lane < 14) cin = __ldg(P.cov6 + 6 * i + (lane - 8));
-                    if (lane == 14) cin = (float)__ldg(P.valid + i);
+                float sx, sy, sz, cin = cin0;
+                if (resident) {
+                    sx = ws.s[0]; sy = ws.s[1]; sz = ws.s[2];
+                } else {
+                    const float* sp = P.scan + (int64_t)i * P.stride;
+                    sx = __ldg(sp); sy = __ldg(sp + 1); sz = __ldg(sp + 2);
+                    if (have_scan_cov) {
+                        if (lane >= 8 && lane < 14) cin = __ldg(P.cov6 + 6 * (int64_t)i + (lane - 8));
+                        if (lane == 14) cin = (float)__ldg(P.valid + i);
+                    }
+                    have = 0;
                 }
-                const Src src = s_src[wib];
-                const float pf[3] = {src.p[0], src.p[1], src.p[2]};
-                const int k[3] = {src.k[0], src.k[1], src.k[2]};
-                {
-                    if (src.ok) {
-                        // kNN-search, k = 1
-                        float rx, ry, rz;
-                        const Best best = warp_nearest(m, pf[0], pf[1], pf[2], k, lane, s_list[wib], rx, ry, rz);
-                        if (best.id != NO_ID && !(best.d2 > P.tau2)) {    // adaptive-threshold gate
-                            // lanes 0..5 fetch Sigma_r, lane 6 its flag: one memory level
-                            if (have_scan_cov) {
-                                if (lane < 6) cin = __ldg(m.cov + (size_t)best.ref * 6 + lane);
-                                if (lane == 6) cin = (float)__ldg(m.cov_ok + best.ref);
-                            }
-                            const bool full = have_scan_cov && __shfl_sync(FULL, cin, 6) != 0.f && __shfl_sync(FULL, cin, 14) != 0.f;
+                float pf[3];
+                int k[3];
+                bool ok = false;
+                if (isfinite(sx) && isfinite(sy) && isfinite(sz)) {
+                    transform_point(s_T, sx, sy, sz, pf);                       // accumulated pose on the ORIGINAL point (R11)
+                    ok = voxel_index(pf[0], pf[1], pf[2], m.voxel, k);
+                }
+                if (ok) {
+                    // the 27 lookups: reused while the point stays in its voxel
+                    if (!((have & 1u) && k[0] == ws.kp[0] && k[1] == ws.kp[1] && k[2] == ws.kp[2])) {
+                        probe27_regs(m, k, lane, pcnt, pbucket);
+                        __syncwarp();
+                        if (lane < 3) ws.kp[lane] = k[lane];
+                        have |= 1u;
+                    }
+                    // the previous nearest neighbour bounds the search if it is one of this search's candidates
+                    double bound = INF;
+                    uint32_t pref = 0xFFFFFFFFu;
+                    if (have & 2u) {
+                        const float prx = ws.pr[0], pry = ws.pr[1], prz = ws.pr[2];
+                        pref = ws.pref;
+                        int kr[3];
+                        if (voxel_index(prx, pry, prz, m.voxel, kr) && abs(kr[0] - k[0]) <= 1 && abs(kr[1] - k[1]) <= 1 && abs(kr[2] - k[2]) <= 1)
+                            bound = dist2(pf[0], pf[1], pf[2], prx, pry, prz);
+                    }
+                    // kNN-search, k = 1
+                    float rx, ry, rz;
+                    const Best best = nearest_bounded(m, pf[0], pf[1], pf[2], k, lane, pcnt, pbucket, bound, s_list[wib], rx, ry, rz);
+                    if (best.id != NO_ID) {
+                        // Sigma_r (lanes 0..5) and its flag (lane 6): one memory level, skipped if the neighbour is the old one
+                        if (have_scan_cov && best.ref != pref) {
+                            if (lane < 6) cinr = __ldg(m.cov + (size_t)best.ref * 6 + lane);
+                            if (lane == 6) cinr = (float)__ldg(m.cov_ok + best.ref);
+                        }
+                        __syncwarp();
+                        if (lane == 0) { ws.pr[0] = rx; ws.pr[1] = ry; ws.pr[2] = rz; ws.pref = best.ref; }
+                        have |= 2u;
+                        if (!(best.d2 > P.tau2)) {                                 // adaptive-threshold gate
+                            const bool full = have_scan_cov && __shfl_sync(FULL, cinr, 6) != 0.f && __shfl_sync(FULL, cin, 14) != 0.f;
                             Corr& c = s_corr[wib];
-                            if (lane < 6) c.cr[lane] = cin;
+                            if (lane < 6) c.cr[lane] = cinr;
                             if (lane >= 8 && lane < 14) c.cs[lane - 8] = cin;
                             if (lane == 16) { c.p[0] = pf[0]; c.p[1] = pf[1]; c.p[2] = pf[2]; c.r[0] = rx; c.r[1] = ry; c.r[2] = rz; }
                             flags = full ? 3 : 1;
                         }
+                    } else {
+                        have &= ~2u;
                     }
+                    __syncwarp();
                 }
             }
             if (lane == 0) s_corr[wib].flags = flags;
@@ -451,12 +515,9 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(M
             // ---- phase B (A9): 8 lanes of warp 0 linearise the block's 8 correspondences together --------------------
             if (wib == 0) {
                 if (lane < GWARPS) {
-                    const Corr c = s_corr[lane];
                     double* terms = s_terms[lane];
-                    if (c.flags & 1) {
-                        const double p[3] = {(double)c.p[0], (double)c.p[1], (double)c.p[2]};
-                        const double r[3] = {(double)c.r[0], (double)c.r[1], (double)c.r[2]};
-                        correspondence_terms(s_T, p, r, (c.flags & 2) != 0, c.cs, c.cr, P.kernel, P.kappa, terms);
+                    if (s_corr[lane].flags & 1) {
+                        correspondence_terms(s_T, s_corr[lane], P.kernel, P.kappa, terms);
                     } else {
 #pragma unroll
                         for (int t = 0; t < NTERMS; ++t) terms[t] = 0.0;
@@ -473,20 +534,16 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(M
         // ---- A10: block row -> group of 32 blocks -> grid, tagged words, every level summed in a fixed order --------
         if (wib == 0) put_tagged(P.scratch.rows + (size_t)blockIdx.x * TSTRIDE + lane, lane < NTERMS ? acc : 0.0, tag);
         if (blockIdx.x % GROUP == 0) {   // group leader: fold the group's rows into one
+            const int group = blockIdx.x / GROUP, n_groups = (gridDim.x + GROUP - 1) / GROUP;
+            const int group_rows = min(GROUP, (int)gridDim.x - group * GROUP);
             const double t = block_sum_tagged(P.scratch.rows, group * GROUP, group_rows, tag, lane, wib, s_red);
             if (wib == 0) put_tagged(P.scratch.grows + (size_t)group * TSTRIDE + lane, t, tag);
             if (blockIdx.x == 0) {       // block 0: final sum, solve, publish
                 const double t2 = block_sum_tagged(P.scratch.grows, 0, n_groups, tag, lane, wib, s_red);
-                if (wib == 0) s_terms[0][lane] = t2;
-                __syncthreads();
-                if (threadIdx.x == 0) {
-                    Pose Tn;
-                    const bool done = solve_and_update(P, s_terms[0], s_T, it, Tn);
-#pragma unroll
-                    for (int a = 0; a < 9; ++a) put_tagged(P.scratch.pub + a, Tn.R[a], tag);
-#pragma unroll
-                    for (int a = 0; a < 3; ++a) put_tagged(P.scratch.pub + 9 + a, Tn.t[a], tag);
-                    put_tagged(P.scratch.pub + 12, done ? 1.0 : 0.0, tag);
+                if (wib == 0) {
+                    s_red[0][lane] = t2;
+                    __syncwarp();
+                    solve_and_publish(P, s_red[0], s_T, it, lane, tag);
                 }
             }
         }
@@ -499,12 +556,7 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(M
             // of the pool the publish hop cost 3.5 us instead of 1.1 us with every lane polling).
             double vv = 0.0;
             if (lane == NPUB - 1) {
-                uint4 w = load_tagged(P.scratch.pub + lane);
-                while (w.y != tag || w.w != tag) {
-                    __nanosleep(200);       // back off: the waiters must not crowd out the few blocks still working
-                    w = load_tagged(P.scratch.pub + lane);
-                }
-                vv = __longlong_as_double((long long)(((unsigned long long)w.z << 32) | w.x));
+                while (!load_tagged(P.scratch.pub + lane, tag, vv)) __nanosleep(100);   // back off: do not crowd out the blocks still working
             }
             __syncwarp();
             if (lane < NPUB - 1) vv = wait_tagged(P.scratch.pub + lane, tag);
@@ -547,7 +599,7 @@ static int gicp_launch(const far_map_t* map, const float* d_scan, const float* d
                        const int64_t* d_n, int stride, const far_pose_t* hpose, const far_pose_t* d_pose, double sigma,
                        int max_iters, int linearize_only, const far_gicp_options_t* opts, far_gicp_result_t* d_out,
                        void* stream) {
-    if (!map || !d_out || n < 0 || (n > 0 && !d_scan) || (stride != 3 && stride != 4) || max_iters < 1 || max_iters > MAX_ITERS_LIMIT || (!hpose && !d_pose))
+    if (!map || !d_out || n < 0 || n > 0x7FFFFFFFll / 8 || (n > 0 && !d_scan) || (stride != 3 && stride != 4) || max_iters < 1 || max_iters > MAX_ITERS_LIMIT || (!hpose && !d_pose))
         return FAR_ERR_ARG;
     far_gicp_options_t o;
     if (opts) o = *opts; else far_gicp_default_options(&o);

@@ -9,7 +9,7 @@ struct far_map {
     far_map_config_t cfg;
     far::MapView view;          // device pointers + constants, passed by value to kernels
     uint32_t* d_touched;        // [max_batch] slots that received their first new point in the chunk
-    uint2* d_cov_tasks;         // [max_batch] {bucket, first new position | new points << 8} per touched voxel
+    uint32_t* d_cov_list;       // [max_batch] refs (bucket*cap+pos) of accepted points awaiting a covariance, grouped by voxel
     void* d_gicp_partials;      // tagged reduction rows + published pose of the cooperative GICP kernel (far_gicp.cu)
     int gicp_max_grid;          // co-resident blocks of the GICP kernel on this device
     int64_t max_batch;
@@ -55,8 +55,8 @@ struct LaunchScope {
 inline int grid_for(int64_t n, int block) { return (int)((n + block - 1) / block); }
 
 // launch helpers implemented in far_query.cu (used by far_map.cu for the covariances of accepted points)
-int launch_knn_cov_tasks(const far_map* map, const uint2* d_tasks, const unsigned int* d_n, int64_t n_max,
-                         cudaStream_t stream);
+int launch_knn_cov_refs(const far_map* map, const uint32_t* d_refs, const unsigned int* d_n, int64_t n_max,
+                        cudaStream_t stream);
 int launch_knn_cov_new_ids(const far_map* map, cudaStream_t stream);
 // implemented in far_gicp.cu: sizes the cooperative grid, allocates the reduction scratch of a map
 int gicp_setup(far_map* map);

@@ -48,7 +48,18 @@ __device__ __forceinline__ bool load_pose_point(const float* __restrict__ xyz, i
 
 __device__ __forceinline__ uint32_t ld_volatile(const uint32_t* p) { return *reinterpret_cast<const volatile uint32_t*>(p); }
 
-// raise the reach of home slot h to at least r, leaving the count byte alone (rare: once per claimed key)
+__device__ __forceinline__ Entry ld_entry_volatile(const Entry* p) {
+    uint4 raw;
+    asm volatile("ld.volatile.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(raw.x), "=r"(raw.y), "=r"(raw.z), "=r"(raw.w) : "l"(p) : "memory");
+    Entry e;
+    e.key = ((unsigned long long)raw.y << 32) | raw.x;
+    e.bucket = raw.z;
+    e.cr = raw.w;
+    return e;
+}
+
+// raise the reach of home slot h to at least r, leaving the count byte alone (only for DISPLACED keys: a key sitting in
+// its home slot needs no reach)
 __device__ __forceinline__ void raise_reach(Entry* table, uint32_t h, uint32_t r) {
     uint32_t* w = &table[h].cr;
     uint32_t old = ld_volatile(w);
@@ -60,24 +71,29 @@ __device__ __forceinline__ void raise_reach(Entry* table, uint32_t h, uint32_t r
 }
 
 // find `key` or claim an empty slot for it: 64-bit atomicCAS on the key word, linear probing step 1.
-// Returns NO_SLOT if the key is absent and the table takes no more keys.
+// One 16-byte load per probed slot yields key, bucket and count together (the two 8-byte halves may be of different age:
+// harmless, a stale half only sends the caller through the slower path).  Returns NO_SLOT if the key is absent and the
+// table takes no more keys; `e` = the entry as seen (bucket = BUCKET_PENDING on a slot claimed just now).
 __device__ __forceinline__ uint32_t find_or_claim(Entry* table, uint32_t mask, uint32_t slots, unsigned long long key,
-                                                  bool may_claim, bool& claimed) {
+                                                  bool may_claim, bool& claimed, Entry& e) {
     const uint32_t h = hash_key(key) & mask;
     uint32_t s = h;
     claimed = false;
     for (uint32_t probes = 0; probes < slots; ++probes) {
-        unsigned long long cur = *reinterpret_cast<volatile unsigned long long*>(&table[s].key);
-        if (cur == KEY_EMPTY) {
+        e = ld_entry_volatile(table + s);
+        if (e.key == KEY_EMPTY) {
             if (!may_claim || probes >= 0xFFFFFEu) return NO_SLOT;
-            cur = atomicCAS(&table[s].key, KEY_EMPTY, key);
+            const unsigned long long cur = atomicCAS(&table[s].key, KEY_EMPTY, key);
             if (cur == KEY_EMPTY) {
                 claimed = true;
-                raise_reach(table, h, probes + 1u);   // keep the reach of the key's home slot up to date (find_voxel)
+                e.key = key; e.bucket = BUCKET_PENDING; e.cr &= ~0xFFu;
+                if (probes) raise_reach(table, h, probes);   // keep the reach of the key's home slot up to date (find_voxel)
                 return s;
             }
+            if (cur == key) { e = ld_entry_volatile(table + s); return s; }
+        } else if (e.key == key) {
+            return s;
         }
-        if (cur == key) return s;
         s = (s + 1) & mask;
     }
     return NO_SLOT;
@@ -139,61 +155,57 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
     const uint32_t ahead = __popc(same & lt);
     const bool is_leader = valid && lane == leader;
 
-    // phase 1: the leader finds or claims the voxel's table slot
-    uint32_t s = NO_SLOT;
-    bool claimed = false;
+    // phase 1: the leader finds or claims the voxel's table slot; the probe's 16-byte load brings bucket and count along
+    uint32_t s = NO_SLOT, b = NO_BUCKET, c0 = 0;
+    bool claimed = false, want = false;
+    const uint32_t id_base = (uint32_t)ctr->next_id + id_offset;           // requested early: needed by the chain only
     if (is_leader) {
-        const bool may_claim = ld_volatile(&ctr->n_keys) < m.key_limit;   // enforced up to the keys claimed while this runs
-        s = find_or_claim(m.table, m.mask, m.slots, key, may_claim, claimed);
+        const bool may_claim = ld_volatile(&ctr->n_keys) < m.key_limit;    // enforced up to the keys claimed while this runs
+        Entry e;
+        s = find_or_claim(m.table, m.mask, m.slots, key, may_claim, claimed, e);
+        if (s != NO_SLOT) {
+            b = e.bucket;
+            c0 = entry_count(e.cr);                                        // stable: only the commit kernel writes counts
+            // a voxel without a bucket gets one from exactly one thread of the grid: the claimer of a new key (its bucket
+            // word starts out PENDING), or whoever wins the NO_BUCKET -> PENDING exchange on the dead key of a pruned voxel
+            want = claimed;
+            if (b == NO_BUCKET) {
+                const uint32_t old = atomicCAS(&m.table[s].bucket, NO_BUCKET, BUCKET_PENDING);
+                if (old == NO_BUCKET) want = true; else b = old;
+            }
+        }
     }
     const unsigned newk = __ballot_sync(FULL, claimed);
     if (newk && lane == 0) atomicAdd(&ctr->n_keys, (unsigned)__popc(newk));   // one atomic per warp, not one per key
-
-    // phase 2: a voxel without a bucket (new key, or the dead key of a pruned voxel) gets one.  Exactly one thread in the
-    // grid wins the NO_BUCKET -> PENDING exchange; the warp's winners allocate together: free list first, then the bump end
-    uint32_t b = NO_BUCKET;
-    bool want = false;
-    if (is_leader && s != NO_SLOT) {
-        b = ld_volatile(&m.table[s].bucket);
-        if (b == NO_BUCKET) {
-            const uint32_t old = atomicCAS(&m.table[s].bucket, NO_BUCKET, BUCKET_PENDING);
-            if (old == NO_BUCKET) want = true; else b = old;
-        }
-    }
+    // phase 2: the warp's allocators draw together: ONE atomic; the first n_free draws of a kernel come off the free list,
+    // the rest from the fresh end of the pool (n_free and bump do not change while the kernel runs)
     const unsigned wm = __ballot_sync(FULL, want);
     bool opened = false;
     if (wm) {
-        const int nreq = __popc(wm);
-        int base = 0;
-        uint32_t fresh = 0;
-        if (lane == 0) {
-            base = atomicSub(&ctr->n_free, nreq);              // may go negative: clamped by the commit kernel's epilogue
-            const int take = max(0, min(base, nreq));
-            if (nreq - take > 0) fresh = atomicAdd(&ctr->bump, (unsigned)(nreq - take));
-        }
-        base = __shfl_sync(FULL, base, 0);
-        fresh = __shfl_sync(FULL, fresh, 0);
+        uint32_t a0 = 0;
+        if (lane == 0) a0 = atomicAdd(&ctr->n_alloc, (unsigned)__popc(wm));
+        a0 = __shfl_sync(FULL, a0, 0);
         if (want) {
-            const int take = max(0, min(base, nreq));
-            const int r = __popc(wm & lt);
-            if (r < take) b = m.free_list[base - 1 - r];
+            const uint32_t a = a0 + __popc(wm & lt);
+            const uint32_t nf = (uint32_t)ctr->n_free;
+            if (a < nf) b = m.free_list[nf - 1u - a];
             else {
-                b = fresh + (uint32_t)(r - take);
-                if (b >= m.max_buckets) b = NO_BUCKET;             // pool exhausted: the voxel stays without points
+                b = ctr->bump + (a - nf);
+                if (b >= m.max_buckets) b = NO_BUCKET;                  // pool exhausted: the voxel stays without points
             }
             atomicExch(&m.table[s].bucket, b);
             opened = b != NO_BUCKET;
+            c0 = 0;
         }
     }
-    // phase 3: another warp may be allocating this voxel's bucket right now; it never waits for anything, so this ends
+    // phase 3: another thread may be allocating this voxel's bucket right now; it never waits for anything, so this ends
     if (is_leader && s != NO_SLOT && !want) {
         while (b == BUCKET_PENDING) b = ld_volatile(&m.table[s].bucket);
     }
-    uint32_t c0 = 0;
-    if (is_leader && b != NO_BUCKET) c0 = entry_count(ld_volatile(&m.table[s].cr));   // stable: only commit writes counts
     s = __shfl_sync(same, s, leader);
     b = __shfl_sync(same, b, leader);
     c0 = __shfl_sync(same, c0, leader);
+    const bool fresh_voxel = __shfl_sync(same, (int)want, leader) != 0;
 
     // statistics, one atomic per warp and counter
     const unsigned m_bad = __ballot_sync(FULL, bad);
@@ -213,9 +225,10 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
     if (valid && b != NO_BUCKET) {
         const uint32_t cap = voxel_limit(m, asmd, k, pose_mode, T);
         uint32_t* idw = m.ids + (size_t)b * (uint32_t)m.cap;   // id word of position 0
-        uint32_t x = (uint32_t)ctr->next_id + id_offset + (uint32_t)i;
+        uint32_t x = id_base + (uint32_t)i;
         // ids at a position only ever decrease: if the last position already holds a smaller id, x cannot survive
-        if (c0 + ahead < cap && !(ld_volatile(idw + (cap - 1)) < x)) {
+        // (not worth a load on a voxel that was opened just now)
+        if (c0 + ahead < cap && (fresh_voxel || !(ld_volatile(idw + (cap - 1)) < x))) {
             // The id words of a bucket are sorted at every instant and only ever decrease, so a position seen holding an
             // id < x will never take x: gallop over such positions with plain reads (4 independent loads per step)
             // instead of walking them with dependent atomics.  A stale read only makes the chain start earlier.
@@ -250,7 +263,7 @@ constexpr int COMMIT_LANES = 8;      // 4 and 16 measure the same within 3 %
 __global__ void __launch_bounds__(256) insert_commit_kernel(MapView m, const float* __restrict__ xyz, int stride,
                                                              int pose_mode, Pose hpose, const Pose* __restrict__ d_pose,
                                                              uint32_t id_offset, const uint32_t* __restrict__ touched,
-                                                             uint2* __restrict__ cov_tasks, int64_t n_call, int last_chunk,
+                                                             uint32_t* __restrict__ cov_list, int64_t n_call, int last_chunk,
                                                              far_insert_stats_t* __restrict__ d_stats) {
     const int lane = threadIdx.x & 31, sub = lane / COMMIT_LANES, sl = lane % COMMIT_LANES;
     constexpr int PER_WARP = 32 / COMMIT_LANES;
@@ -287,11 +300,16 @@ __global__ void __launch_bounds__(256) insert_commit_kernel(MapView m, const flo
             }
             const unsigned bal = __ballot_sync(FULL, is_new);
             if (bal == 0) break;                                           // ids fill positions in order: nothing further
+            if (cov_list != nullptr) {                                     // the warp's new points, voxel by voxel
+                uint32_t at = 0;
+                if (lane == 0) at = atomicAdd(&ctr->n_cov, (uint32_t)__popc(bal));
+                at = __shfl_sync(FULL, at, 0);
+                if (is_new) cov_list[at + __popc(bal & ((1u << lane) - 1u))] = b * cap + pos;
+            }
             n_new += __popc(bal & gmask);
         }
         if (active && sl == 0) {
             m.table[s].cr = (cr & ~0xFFu) | (c0 + n_new);
-            if (cov_tasks) cov_tasks[t] = make_uint2(b, c0 | (n_new << 8));
             acc_new += n_new;
         }
     }
@@ -301,10 +319,16 @@ __global__ void __launch_bounds__(256) insert_commit_kernel(MapView m, const flo
 
     if (last_block_done(&ctr->ticket[0]) && threadIdx.x == 0) {
         volatile Counters* c = ctr;
-        c->n_tasks = c->n_touched;
         c->n_touched = 0u;
-        if (c->n_free < 0) c->n_free = 0;
-        if (c->bump > m.max_buckets) c->bump = m.max_buckets;
+        if (last_chunk) { c->n_tasks = c->n_cov; c->n_cov = 0u; }
+        {   // fold the kernel's bucket draws into the allocator state
+            const unsigned drawn = c->n_alloc, nf = (unsigned)c->n_free;
+            const unsigned from_free = drawn < nf ? drawn : nf;
+            c->n_free = (int)(nf - from_free);
+            const unsigned long long bump = (unsigned long long)c->bump + (drawn - from_free);
+            c->bump = bump > m.max_buckets ? m.max_buckets : (unsigned)bump;
+            c->n_alloc = 0u;
+        }
         if (last_chunk) {
             c->call_first_id = c->next_id;
             c->next_id = c->next_id + (unsigned long long)n_call;
@@ -418,7 +442,8 @@ __global__ void __launch_bounds__(256) rehash_move_kernel(MapView m) {
         const Entry e = m.table[s];
         if (e.key != KEY_EMPTY && e.bucket < BUCKET_PENDING) {
             bool claimed;
-            const uint32_t t = find_or_claim(m.shadow, m.mask, m.slots, e.key, true, claimed);
+            Entry seen;
+            const uint32_t t = find_or_claim(m.shadow, m.mask, m.slots, e.key, true, claimed, seen);
             m.shadow[t].bucket = e.bucket;
             atomicOr(&m.shadow[t].cr, entry_count(e.cr));     // the reach bits of slot t may be raised concurrently
             moved = true;
@@ -434,7 +459,7 @@ __global__ void __launch_bounds__(256) rehash_swap_kernel(MapView m) {
     if (s < m.slots) {
         uint4* sh = reinterpret_cast<uint4*>(m.shadow + s);
         *reinterpret_cast<uint4*>(m.table + s) = *sh;
-        *sh = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, NO_BUCKET, 0u);
+        *sh = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, BUCKET_PENDING, 0u);
     }
     if (s == 0) {
         m.ctr->n_keys = m.ctr->rehash_moved;
@@ -525,7 +550,7 @@ __global__ void asmd_density_out_kernel(MapView m, unsigned long long* acc, doub
 __global__ void __launch_bounds__(256) clear_kernel(MapView m) {
     const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nthr = gridDim.x * blockDim.x;
     for (uint32_t s = tid; s < m.slots; s += nthr)
-        *reinterpret_cast<uint4*>(m.table + s) = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, NO_BUCKET, 0u);
+        *reinterpret_cast<uint4*>(m.table + s) = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, BUCKET_PENDING, 0u);
     const size_t used = (size_t)min(m.ctr->bump, m.max_buckets) * (size_t)m.cap;   // fresh buckets beyond are clean
     for (size_t j = tid; j < used; j += nthr) m.ids[j] = NO_ID;
     if (last_block_done(&m.ctr->ticket[2]) && threadIdx.x == 0) {
@@ -540,7 +565,7 @@ __global__ void __launch_bounds__(256) clear_kernel(MapView m) {
 __global__ void __launch_bounds__(256) table_init_kernel(Entry* table, uint32_t slots) {
     const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= slots) return;
-    *reinterpret_cast<uint4*>(table + s) = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, NO_BUCKET, 0u);
+    *reinterpret_cast<uint4*>(table + s) = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, BUCKET_PENDING, 0u);
 }
 
 // ---- stats / export ----------------------------------------------------------------------------------------
@@ -706,7 +731,7 @@ int far_map_create(far_map_t** out, const far_map_config_t* cfg) {
     }
     alloc((void**)&v.ctr, sizeof(Counters));
     alloc((void**)&m->d_touched, (size_t)c.max_batch * sizeof(uint32_t));
-    alloc((void**)&m->d_cov_tasks, (size_t)c.max_batch * sizeof(uint2));
+    alloc((void**)&m->d_cov_list, (size_t)c.max_batch * sizeof(uint32_t));
     if (e == cudaSuccess) e = cudaHostAlloc((void**)&m->h_mail, sizeof(Mailbox), cudaHostAllocMapped);
     if (e == cudaSuccess) {
         memset((void*)m->h_mail, 0, sizeof(Mailbox));
@@ -740,7 +765,7 @@ int far_map_destroy(far_map_t* m) {
     if (!m) return FAR_OK;
     cudaFree(m->view.table); cudaFree(m->view.shadow); cudaFree(m->view.points); cudaFree(m->view.ids);
     cudaFree(m->view.free_list); cudaFree(m->view.cov); cudaFree(m->view.cov_ok);
-    cudaFree(m->view.ctr); cudaFree(m->d_touched); cudaFree(m->d_cov_tasks);
+    cudaFree(m->view.ctr); cudaFree(m->d_touched); cudaFree(m->d_cov_list);
     cudaFree(m->d_gicp_partials);
     if (m->h_mail) cudaFreeHost((void*)m->h_mail);
     delete m;
@@ -803,7 +828,7 @@ static int insert_impl(far_map_t* m, const float* d_xyz, int64_t n, int stride, 
     Pose hp;
     memset(&hp, 0, sizeof(hp));
     if (pose_mode == 1) memcpy(&hp, hpose, sizeof(hp));
-    const bool cov_by_tasks = compute_cov && n <= m->max_batch;
+    const bool cov_by_list = compute_cov && n <= m->max_batch;
     const int commit_grid = m->sm_count * 8;
     int64_t off = 0;
     do {
@@ -815,7 +840,7 @@ static int insert_impl(far_map_t* m, const float* d_xyz, int64_t n, int stride, 
                                                                           (const Pose*)d_pose, (uint32_t)off, m->d_touched, asmd);
         FAR_LAUNCH(insert_commit_kernel, nc > 0 ? commit_grid : 1, 256, 0, st, m->view, xyz, stride, pose_mode, hp,
                                                            (const Pose*)d_pose, (uint32_t)off, m->d_touched,
-                                                           cov_by_tasks ? m->d_cov_tasks : nullptr, n, last, d_stats);
+                                                           cov_by_list ? m->d_cov_list : nullptr, n, last, d_stats);
         FAR_CUDA(cudaGetLastError());
         off += nc;
     } while (off < n);
@@ -823,7 +848,7 @@ static int insert_impl(far_map_t* m, const float* d_xyz, int64_t n, int stride, 
     m->offered_total += (uint64_t)n;
     if (compute_cov && n > 0) {
         // "we recompute the covariances of the added points" -- against the map AFTER the insert
-        int rc = cov_by_tasks ? launch_knn_cov_tasks(m, m->d_cov_tasks, &m->view.ctr->n_tasks, n, st)
+        int rc = cov_by_list ? launch_knn_cov_refs(m, m->d_cov_list, &m->view.ctr->n_tasks, n, st)
                               : launch_knn_cov_new_ids(m, st);
         if (rc != FAR_OK) return rc;
     }
