@@ -224,6 +224,27 @@ __device__ __forceinline__ Best nearest_bounded(const MapView& m, float qx, floa
         const double lb = (lane == 13) ? 0.0 : voxel_lower_bound(qx, qy, qz, k, m.voxel, lane / 9 - 1, (lane / 3) % 3 - 1, lane % 3 - 1);
         if (lb <= bound) c2 = cnt;
     }
+    const unsigned surv = __ballot_sync(FULL, c2 > 0);
+    if ((surv & ~(1u << 13)) == 0) {
+        // the usual case from the second iteration on: no neighbour voxel can hold a nearer point.  With a bound the own
+        // voxel is still to be swept (one step: cap <= 64 points, two lanes' worth at most); without, it was swept above
+        if (surv) {
+            const uint32_t c_cnt = __shfl_sync(FULL, c2, 13), c_bucket = __shfl_sync(FULL, bucket, 13);
+            for (uint32_t j = lane; j < c_cnt; j += 32) {
+                const uint32_t ref = c_bucket * (uint32_t)m.cap + j;
+                const float4 p = __ldg(m.points + ref);
+                const double d2 = dist2(qx, qy, qz, p.x, p.y, p.z);
+                const uint32_t id = __float_as_uint(p.w);
+                if (better(d2, id, best)) { best.d2 = d2; best.id = id; best.ref = ref; bx = p.x; by = p.y; bz = p.z; }
+            }
+        }
+        const int w = warp_argmin(best.d2, best.id);
+        best.d2 = __shfl_sync(FULL, best.d2, w);
+        best.id = __shfl_sync(FULL, best.id, w);
+        best.ref = __shfl_sync(FULL, best.ref, w);
+        rx = __shfl_sync(FULL, bx, w); ry = __shfl_sync(FULL, by, w); rz = __shfl_sync(FULL, bz, w);
+        return best;
+    }
     const int total = cand_build(L, c2, bucket, lane);
     CandIter ci;
     ci.before = 0;
@@ -370,8 +391,25 @@ __device__ __forceinline__ void solve_and_publish(const GicpParams& P, const dou
 // increasing order, then the 8 warp sums are added in warp order by warp 0.  Every block must call with all threads.
 __device__ __forceinline__ double block_sum_tagged(const uint4* rows, int first, int count, uint32_t tag, int lane, int wib,
                                                    double (*s_red)[TSTRIDE]) {
+    // a warp's rows are requested together before the first is examined: they arrive within a microsecond of each other,
+    // and one L2 round trip per row would be most of the reduction
+    constexpr int POLL = 4;
     double s = 0.0;
-    for (int r = wib; r < count; r += GWARPS) s += wait_tagged(rows + (size_t)(first + r) * TSTRIDE + lane, tag);
+    for (int r0 = wib; r0 < count; r0 += GWARPS * POLL) {
+        double v[POLL];
+        unsigned pending = 0;
+#pragma unroll
+        for (int u = 0; u < POLL; ++u) {
+            const int r = r0 + u * GWARPS;
+            v[u] = 0.0;
+            if (r < count && !load_tagged(rows + (size_t)(first + r) * TSTRIDE + lane, tag, v[u])) pending |= 1u << u;
+        }
+#pragma unroll
+        for (int u = 0; u < POLL; ++u) {
+            if (pending & (1u << u)) v[u] = wait_tagged(rows + (size_t)(first + r0 + u * GWARPS) * TSTRIDE + lane, tag);
+            s += v[u];                                       // fixed order: rows ascending
+        }
+    }
     s_red[wib][lane] = s;
     __syncthreads();
     double t = 0.0;
@@ -388,6 +426,7 @@ __device__ __forceinline__ double block_sum_tagged(const uint4* rows, int first,
 struct WarpState {
     float s[3];       // the source point (sensor frame)
     float pr[3];      // previous nearest neighbour
+    int kr[3];        // its voxel
     int kp[3];        // voxel of the transformed point at the last table walk
     uint32_t pref;    // reference of the previous nearest neighbour
 };
@@ -478,11 +517,9 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(c
                     double bound = INF;
                     uint32_t pref = 0xFFFFFFFFu;
                     if (have & 2u) {
-                        const float prx = ws.pr[0], pry = ws.pr[1], prz = ws.pr[2];
                         pref = ws.pref;
-                        int kr[3];
-                        if (voxel_index(prx, pry, prz, m.voxel, kr) && abs(kr[0] - k[0]) <= 1 && abs(kr[1] - k[1]) <= 1 && abs(kr[2] - k[2]) <= 1)
-                            bound = dist2(pf[0], pf[1], pf[2], prx, pry, prz);
+                        if (abs(ws.kr[0] - k[0]) <= 1 && abs(ws.kr[1] - k[1]) <= 1 && abs(ws.kr[2] - k[2]) <= 1)
+                            bound = dist2(pf[0], pf[1], pf[2], ws.pr[0], ws.pr[1], ws.pr[2]);
                     }
                     // kNN-search, k = 1
                     float rx, ry, rz;
@@ -494,7 +531,12 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(c
                             if (lane == 6) cinr = (float)__ldg(m.cov_ok + best.ref);
                         }
                         __syncwarp();
-                        if (lane == 0) { ws.pr[0] = rx; ws.pr[1] = ry; ws.pr[2] = rz; ws.pref = best.ref; }
+                        if (best.ref != pref && lane == 0) {
+                            ws.pr[0] = rx; ws.pr[1] = ry; ws.pr[2] = rz; ws.pref = best.ref;
+                            int kr[3];
+                            voxel_index(rx, ry, rz, m.voxel, kr);                 // a stored point: always valid
+                            ws.kr[0] = kr[0]; ws.kr[1] = kr[1]; ws.kr[2] = kr[2];
+                        }
                         have |= 2u;
                         if (!(best.d2 > P.tau2)) {                                 // adaptive-threshold gate
                             const bool full = have_scan_cov && __shfl_sync(FULL, cinr, 6) != 0.f && __shfl_sync(FULL, cin, 14) != 0.f;
@@ -556,7 +598,7 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(c
             // of the pool the publish hop cost 3.5 us instead of 1.1 us with every lane polling).
             double vv = 0.0;
             if (lane == NPUB - 1) {
-                while (!load_tagged(P.scratch.pub + lane, tag, vv)) __nanosleep(100);   // back off: do not crowd out the blocks still working
+                while (!load_tagged(P.scratch.pub + lane, tag, vv)) __nanosleep(40);    // back off: do not crowd out the blocks still working
             }
             __syncwarp();
             if (lane < NPUB - 1) vv = wait_tagged(P.scratch.pub + lane, tag);

@@ -151,15 +151,31 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
     // invalid lanes get distinct fake keys (bit 63 is never set by a valid key)
     const unsigned long long key = valid ? pack_key(k[0], k[1], k[2]) : ((1ull << 63) | (unsigned long long)lane);
     const unsigned same = __match_any_sync(FULL, key);
-    const int leader = __ffs(same) - 1;
     const uint32_t ahead = __popc(same & lt);
-    const bool is_leader = valid && lane == leader;
 
-    // phase 1: the leader finds or claims the voxel's table slot; the probe's 16-byte load brings bucket and count along
+    // phase 1: every lane looks its voxel up by itself, read-only; the probe's 16-byte load brings bucket and count along.
+    // On a map that already holds the scan's voxels (the submap update of a frame) every lane is done here and goes
+    // straight to its chain -- nobody waits for a neighbour's slower walk.
     uint32_t s = NO_SLOT, b = NO_BUCKET, c0 = 0;
-    bool claimed = false, want = false;
+    bool claimed = false, want = false, resolved = !valid;
     const uint32_t id_base = (uint32_t)ctr->next_id + id_offset;           // requested early: needed by the chain only
-    if (is_leader) {
+    if (valid) {
+        uint32_t t = hash_key(key) & m.mask;
+        for (uint32_t probes = 0; probes < m.slots; ++probes) {
+            const Entry e = ld_entry_volatile(m.table + t);
+            if (e.key == key) {
+                if (e.bucket < BUCKET_PENDING) { s = t; b = e.bucket; c0 = entry_count(e.cr); resolved = true; }
+                break;
+            }
+            if (e.key == KEY_EMPTY) break;
+            t = (t + 1) & m.mask;
+        }
+    }
+    // phase 1b (only warps with an unresolved lane): the voxel is new, dead or being opened by someone else.  One leader
+    // per voxel claims the key / the right to allocate; the others of its group get the result by shuffle.
+    const unsigned unresolved = __ballot_sync(FULL, !resolved);
+    const bool is_leader = !resolved && (__ffs(same & unresolved) - 1) == lane;
+    if (unresolved && is_leader) {
         const bool may_claim = ld_volatile(&ctr->n_keys) < m.key_limit;    // enforced up to the keys claimed while this runs
         Entry e;
         s = find_or_claim(m.table, m.mask, m.slots, key, may_claim, claimed, e);
@@ -199,13 +215,20 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
         }
     }
     // phase 3: another thread may be allocating this voxel's bucket right now; it never waits for anything, so this ends
-    if (is_leader && s != NO_SLOT && !want) {
-        while (b == BUCKET_PENDING) b = ld_volatile(&m.table[s].bucket);
+    bool fresh_voxel = false;
+    if (unresolved) {
+        if (is_leader && s != NO_SLOT && !want) {
+            while (b == BUCKET_PENDING) b = ld_volatile(&m.table[s].bucket);
+        }
+        const unsigned grp = same & unresolved;                 // the lanes that wait for this voxel's leader (or nobody)
+        const int leader = __ffs(grp) - 1;
+        if (!resolved) {
+            s = __shfl_sync(grp, s, leader);
+            b = __shfl_sync(grp, b, leader);
+            c0 = __shfl_sync(grp, c0, leader);
+            fresh_voxel = __shfl_sync(grp, (int)want, leader) != 0;
+        }
     }
-    s = __shfl_sync(same, s, leader);
-    b = __shfl_sync(same, b, leader);
-    c0 = __shfl_sync(same, c0, leader);
-    const bool fresh_voxel = __shfl_sync(same, (int)want, leader) != 0;
 
     // statistics, one atomic per warp and counter
     const unsigned m_bad = __ballot_sync(FULL, bad);
@@ -436,9 +459,8 @@ __global__ void __launch_bounds__(256) prune_kernel(MapView m, double cx, double
 // far_map_rehash) set the flag: the decision is taken on the device, the launches are unconditional.
 __global__ void __launch_bounds__(256) rehash_move_kernel(MapView m) {
     if (!m.ctr->rehash_flag) return;
-    const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
-    bool moved = false;
-    if (s < m.slots) {
+    unsigned n_moved = 0;
+    for (uint32_t s = blockIdx.x * blockDim.x + threadIdx.x; s < m.slots; s += gridDim.x * blockDim.x) {
         const Entry e = m.table[s];
         if (e.key != KEY_EMPTY && e.bucket < BUCKET_PENDING) {
             bool claimed;
@@ -446,22 +468,21 @@ __global__ void __launch_bounds__(256) rehash_move_kernel(MapView m) {
             const uint32_t t = find_or_claim(m.shadow, m.mask, m.slots, e.key, true, claimed, seen);
             m.shadow[t].bucket = e.bucket;
             atomicOr(&m.shadow[t].cr, entry_count(e.cr));     // the reach bits of slot t may be raised concurrently
-            moved = true;
+            ++n_moved;
         }
     }
-    const unsigned bm = __ballot_sync(FULL, moved);
-    if (bm && (threadIdx.x & 31) == 0) atomicAdd(&m.ctr->rehash_moved, (unsigned)__popc(bm));
+    n_moved = __reduce_add_sync(FULL, n_moved);
+    if (n_moved && (threadIdx.x & 31) == 0) atomicAdd(&m.ctr->rehash_moved, n_moved);
 }
 
 __global__ void __launch_bounds__(256) rehash_swap_kernel(MapView m) {
     if (!m.ctr->rehash_flag) return;
-    const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s < m.slots) {
+    for (uint32_t s = blockIdx.x * blockDim.x + threadIdx.x; s < m.slots; s += gridDim.x * blockDim.x) {
         uint4* sh = reinterpret_cast<uint4*>(m.shadow + s);
         *reinterpret_cast<uint4*>(m.table + s) = *sh;
         *sh = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, BUCKET_PENDING, 0u);
     }
-    if (s == 0) {
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
         m.ctr->n_keys = m.ctr->rehash_moved;
         m.ctr->rehash_moved = 0u;
         m.ctr->n_dead = 0u;
@@ -893,8 +914,12 @@ int far_asmd_density(const far_map_t* local, const double center[3], double r_cl
 }
 
 static int rehash_enqueue(far_map_t* m, cudaStream_t st) {
-    FAR_LAUNCH(rehash_move_kernel, grid_for(m->view.slots, 256), 256, 0, st, m->view);
-    FAR_LAUNCH(rehash_swap_kernel, grid_for(m->view.slots, 256), 256, 0, st, m->view);
+    // grid-stride over the table with one resident wave: when the flag is clear (most frames) the launch costs a few
+    // hundred empty blocks, not one per 256 slots
+    int grid = grid_for(m->view.slots, 256);
+    if (grid > m->sm_count * 8) grid = m->sm_count * 8;
+    FAR_LAUNCH(rehash_move_kernel, grid, 256, 0, st, m->view);
+    FAR_LAUNCH(rehash_swap_kernel, grid, 256, 0, st, m->view);
     FAR_CUDA(cudaGetLastError());
     return FAR_OK;
 }
