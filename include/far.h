@@ -267,7 +267,10 @@ int far_map_insert_asmd_dev(far_map_t* map, const float* d_xyz, int64_t n, int s
                             void* stream);
 
 /* ---- one frame through the whole path (the LiDAR scan callback) -----------------------------
- * far_frontend_process chains, in stream order and with NO host synchronisation: far_voxelize (ds_voxel) ->
+ * far_frontend_process runs the frame as ONE CUDA GRAPH (cfg.use_graph; captured on the second frame that uses the same
+ * scan buffer, stride and result pointer, replayed from then on: per frame a 120-byte parameter upload and one graph
+ * launch) or, equivalently, as a stream of launches.  Either way, in stream order and with NO host synchronisation:
+ * far_voxelize (ds_voxel) ->
  * scan-local map of the raw scan + far_map_knn_cov of the downsampled points (Sigma_s) ->
  * far_gicp_register against the frontend's map from init_pose -> (update_map) far_map_insert of the raw scan at
  * the registered pose with covariances (cfg.asmd: far_asmd_density of the scan-local map about the sensor, then
@@ -286,11 +289,16 @@ typedef struct {
     int32_t asmd;               /* 1: map update with the Adaptive Submap Density limit (R17) */
     double asmd_r_close;        /* "close range of the current scan" [m] for the density; 0 -> 10         */
     double asmd_d_max;          /* range at which the linear decay reaches the lower bound; 0 -> 100       */
+    int32_t use_graph;          /* 1: the frame is captured as ONE CUDA graph and replayed; 0: stream of launches */
 } far_frontend_config_t;
 typedef struct far_frontend far_frontend_t;
 int far_frontend_create(far_frontend_t** out, const far_frontend_config_t* cfg);
 int far_frontend_destroy(far_frontend_t* f);
 far_map_t* far_frontend_map(far_frontend_t* f);   /* borrowed handle, e.g. to preload the map with far_map_insert */
+/* 1: frames are being replayed from the captured CUDA graph; 0: no graph yet (it is captured when a frame repeats the
+ * previous frame's scan buffer, stride and result pointer); -1: the runtime refused the capture, frames run as a stream of
+ * launches */
+int far_frontend_graph_state(const far_frontend_t* f);
 /* Statistics of the last frame's map update (accepted, new voxels, dropped because full, invalid) copied to HOST memory;
  * synchronises the stream (a diagnostic read, not part of the frame).  A full submap is also reported as FAR_ERR_FULL
  * (see the enum): exactly by far_frontend_process_host (it synchronises), from the mirrored flag by far_frontend_process */

@@ -59,7 +59,7 @@ class GicpResult(C.Structure):
 class FrontendConfig(C.Structure):
     _fields_ = [("map", MapConfig), ("ds_voxel", C.c_float), ("max_scan_points", C.c_int64), ("prune_radius", C.c_double),
                 ("max_iters", C.c_int32), ("update_map", C.c_int32), ("gicp", GicpOptions),
-                ("asmd", C.c_int32), ("asmd_r_close", C.c_double), ("asmd_d_max", C.c_double)]
+                ("asmd", C.c_int32), ("asmd_r_close", C.c_double), ("asmd_d_max", C.c_double), ("use_graph", C.c_int32)]
 
 
 class Motion(C.Structure):
@@ -121,6 +121,7 @@ def lib():
             "far_map_renumber": (ci, [vp, vp]),
             "far_map_status": (ci, [vp]),
             "far_frontend_insert_stats": (ci, [vp, vp, vp]),
+            "far_frontend_graph_state": (ci, [vp]),
             "far_map_snapshot_create": (ci, [vp, vp, vp]),
             "far_map_snapshot_restore": (ci, [vp, vp, vp]),
             "far_map_snapshot_destroy": (ci, [vp]),
@@ -513,13 +514,13 @@ class Frontend:
 
     def __init__(self, voxel, cap, max_voxels, max_scan_points, ds_voxel=0.0, prune_radius=0.0, max_iters=30,
                  update_map=True, opts=None, k_cov=10, cov_eps=1e-3, max_load=0.5, asmd=False, asmd_r_close=10.0,
-                 asmd_d_max=100.0):
+                 asmd_d_max=100.0, use_graph=True):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2606_26010_b200 needs a CUDA device: there is no CPU fallback")
         o = opts if opts is not None else default_options()
         cfg = FrontendConfig(MapConfig(voxel, cap, int(max_voxels), max_load, 1, k_cov, cov_eps, 0, 0), ds_voxel,
                              int(max_scan_points), float(prune_radius), int(max_iters), int(update_map), o,
-                             int(asmd), float(asmd_r_close), float(asmd_d_max))
+                             int(asmd), float(asmd_r_close), float(asmd_d_max), int(use_graph))
         h = C.c_void_p()
         _check(lib().far_frontend_create(C.byref(h), C.byref(cfg)), "far_frontend_create")
         self._h = h
@@ -570,6 +571,10 @@ class Frontend:
                                                                 C.byref(self.h_result), _stream()),
                                 "far_frontend_process_host", full_ok=True)
         return result_to_dict(self.h_result)
+
+    def graph_state(self):
+        """far_frontend_graph_state: 1 replaying the captured frame graph, 0 not captured yet, -1 capture refused"""
+        return int(lib().far_frontend_graph_state(self._h))
 
     def insert_stats(self):
         """far_frontend_insert_stats: statistics of the last frame's map update (synchronising read of the device struct)."""

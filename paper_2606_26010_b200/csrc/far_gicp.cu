@@ -79,6 +79,8 @@ struct GicpParams {
     Pose init;                  // used when d_init == nullptr
     const Pose* d_init;
     double tau2, kappa, conv_eps;
+    const double* d_sigma;      // nullable: tau2 = (tau_mult sigma)^2 and kappa = sigma / kappa_div from the DEVICE value
+    double tau_mult, kappa_div;
     int kernel, max_iters, linearize_only;
     GicpScratch scratch;
     far_gicp_result_t* out;
@@ -452,6 +454,12 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(c
         if (threadIdx.x < 9) s_T.R[threadIdx.x] = vv; else s_T.t[threadIdx.x - 9] = vv;
     }
     const bool have_scan_cov = P.cov6 != nullptr && P.valid != nullptr && m.cov != nullptr;
+    double tau2 = P.tau2, kappa = P.kappa;
+    if (P.d_sigma) {                                          // frame graph: sigma is part of the device-side frame parameters
+        const double sg = *P.d_sigma;
+        tau2 = (P.tau_mult * sg) * (P.tau_mult * sg);
+        kappa = sg / P.kappa_div;
+    }
     const int rounds = (n + nwarps - 1) / nwarps;             // source points per warp (1 when n <= resident warps)
     const double INF = __longlong_as_double(0x7FF0000000000000ll);
 
@@ -538,7 +546,7 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(c
                             ws.kr[0] = kr[0]; ws.kr[1] = kr[1]; ws.kr[2] = kr[2];
                         }
                         have |= 2u;
-                        if (!(best.d2 > P.tau2)) {                                 // adaptive-threshold gate
+                        if (!(best.d2 > tau2)) {                                 // adaptive-threshold gate
                             const bool full = have_scan_cov && __shfl_sync(FULL, cinr, 6) != 0.f && __shfl_sync(FULL, cin, 14) != 0.f;
                             Corr& c = s_corr[wib];
                             if (lane < 6) c.cr[lane] = cinr;
@@ -559,7 +567,7 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(c
                 if (lane < GWARPS) {
                     double* terms = s_terms[lane];
                     if (s_corr[lane].flags & 1) {
-                        correspondence_terms(s_T, s_corr[lane], P.kernel, P.kappa, terms);
+                        correspondence_terms(s_T, s_corr[lane], P.kernel, kappa, terms);
                     } else {
 #pragma unroll
                         for (int t = 0; t < NTERMS; ++t) terms[t] = 0.0;
@@ -637,15 +645,17 @@ void far_gicp_default_options(far_gicp_options_t* o) {
     o->kappa_div = 3.0;
 }
 
-static int gicp_launch(const far_map_t* map, const float* d_scan, const float* d_cov6, const uint8_t* d_valid, int64_t n,
-                       const int64_t* d_n, int stride, const far_pose_t* hpose, const far_pose_t* d_pose, double sigma,
-                       int max_iters, int linearize_only, const far_gicp_options_t* opts, far_gicp_result_t* d_out,
-                       void* stream) {
+}  // extern "C"
+
+int far::gicp_launch(const far_map_t* map, const float* d_scan, const float* d_cov6, const uint8_t* d_valid, int64_t n,
+                     const int64_t* d_n, int stride, const far_pose_t* hpose, const far_pose_t* d_pose, double sigma,
+                     const double* d_sigma, int max_iters, int linearize_only, const far_gicp_options_t* opts, far_gicp_result_t* d_out,
+                     void* stream) {
     if (!map || !d_out || n < 0 || n > 0x7FFFFFFFll / 8 || (n > 0 && !d_scan) || (stride != 3 && stride != 4) || max_iters < 1 || max_iters > MAX_ITERS_LIMIT || (!hpose && !d_pose))
         return FAR_ERR_ARG;
     far_gicp_options_t o;
     if (opts) o = *opts; else far_gicp_default_options(&o);
-    if (o.kernel < 0 || o.kernel > 2 || !(sigma > 0.0)) return FAR_ERR_ARG;
+    if (o.kernel < 0 || o.kernel > 2 || (!d_sigma && !(sigma > 0.0))) return FAR_ERR_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     GicpParams P;
     memset(&P, 0, sizeof(P));
@@ -656,6 +666,7 @@ static int gicp_launch(const far_map_t* map, const float* d_scan, const float* d
     P.tau2 = tau * tau;
     P.kappa = sigma / o.kappa_div;
     P.conv_eps = o.conv_eps;
+    P.d_sigma = d_sigma; P.tau_mult = o.tau_mult; P.kappa_div = o.kappa_div;
     P.kernel = o.kernel; P.max_iters = max_iters; P.linearize_only = linearize_only;
     P.scratch.rows = reinterpret_cast<uint4*>(map->d_gicp_partials);
     P.scratch.grows = P.scratch.rows + (size_t)map->gicp_max_grid * TSTRIDE;
@@ -674,25 +685,27 @@ static int gicp_launch(const far_map_t* map, const float* d_scan, const float* d
     return FAR_OK;
 }
 
+extern "C" {
+
 int far_gicp_linearize(const far_map_t* map, const float* d_scan, const float* d_cov6, const uint8_t* d_valid, int64_t n,
                        int stride, const far_pose_t* pose, double sigma, const far_gicp_options_t* opts,
                        far_gicp_result_t* d_out, void* stream) {
-    return gicp_launch(map, d_scan, d_cov6, d_valid, n, nullptr, stride, pose, nullptr, sigma, 1, 1, opts, d_out, stream);
+    return far::gicp_launch(map, d_scan, d_cov6, d_valid, n, nullptr, stride, pose, nullptr, sigma, nullptr, 1, 1, opts, d_out, stream);
 }
 
 int far_gicp_register(const far_map_t* map, const float* d_scan, const float* d_cov6, const uint8_t* d_valid, int64_t n,
                       int stride, const far_pose_t* init_pose, double sigma, int max_iters, const far_gicp_options_t* opts,
                       far_gicp_result_t* d_out, void* stream) {
-    return gicp_launch(map, d_scan, d_cov6, d_valid, n, nullptr, stride, init_pose, nullptr, sigma, max_iters, 0, opts, d_out,
-                       stream);
+    return far::gicp_launch(map, d_scan, d_cov6, d_valid, n, nullptr, stride, init_pose, nullptr, sigma, nullptr, max_iters, 0, opts,
+                            d_out, stream);
 }
 
 int far_gicp_register_dev(const far_map_t* map, const float* d_scan, const float* d_cov6, const uint8_t* d_valid,
                           const int64_t* d_n, int64_t n_max, int stride, const far_pose_t* d_init_pose, double sigma,
                           int max_iters, const far_gicp_options_t* opts, far_gicp_result_t* d_out, void* stream) {
     if (!d_n || !d_init_pose) return FAR_ERR_ARG;
-    return gicp_launch(map, d_scan, d_cov6, d_valid, n_max, d_n, stride, nullptr, d_init_pose, sigma, max_iters, 0, opts, d_out,
-                       stream);
+    return far::gicp_launch(map, d_scan, d_cov6, d_valid, n_max, d_n, stride, nullptr, d_init_pose, sigma, nullptr, max_iters, 0, opts,
+                            d_out, stream);
 }
 
 // n from the device, initial pose from the host as a kernel argument (saves far_frontend_process a pageable
@@ -701,7 +714,7 @@ int far_gicp_register_dn(const far_map_t* map, const float* d_scan, const float*
                          const int64_t* d_n, int64_t n_max, int stride, const far_pose_t* init_pose, double sigma, int max_iters,
                          const far_gicp_options_t* opts, far_gicp_result_t* d_out, void* stream) {
     if (!d_n || !init_pose) return FAR_ERR_ARG;
-    return gicp_launch(map, d_scan, d_cov6, d_valid, n_max, d_n, stride, init_pose, nullptr, sigma, max_iters, 0, opts, d_out, stream);
+    return far::gicp_launch(map, d_scan, d_cov6, d_valid, n_max, d_n, stride, init_pose, nullptr, sigma, nullptr, max_iters, 0, opts, d_out, stream);
 }
 
 

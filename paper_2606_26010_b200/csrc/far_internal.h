@@ -61,4 +61,19 @@ int launch_knn_cov_new_ids(const far_map* map, cudaStream_t stream);
 // implemented in far_gicp.cu: sizes the cooperative grid, allocates the reduction scratch of a map
 int gicp_setup(far_map* map);
 
+// internal forms of the public calls with the point count (and sigma) read from DEVICE memory in stream order: what the
+// frame graph of far_frontend.cu replays.  n is then the capacity the launch is sized for, the work is min(n, *d_n)
+int voxelize_impl(const float* d_xyz, int64_t n, const int64_t* d_n, int stride, float voxel, float* d_out_xyz, int32_t* d_out_index,
+                  int64_t* d_n_out, void* d_workspace, size_t* workspace_bytes, void* stream);
+int insert_impl(far_map* m, const float* d_xyz, int64_t n, const int64_t* d_n, int stride, int pose_mode, const far_pose_t* hpose,
+                const far_pose_t* d_pose, int compute_cov, far_insert_stats_t* d_stats, void* stream, const double* d_n_close,
+                double d_max);
+int gicp_launch(const far_map* map, const float* d_scan, const float* d_cov6, const uint8_t* d_valid, int64_t n, const int64_t* d_n,
+                int stride, const far_pose_t* hpose, const far_pose_t* d_pose, double sigma, const double* d_sigma, int max_iters,
+                int linearize_only, const far_gicp_options_t* opts, far_gicp_result_t* d_out, void* stream);
+// kernels launched through FAR_LAUNCH so far (also counts what a replayed frame graph launches)
+long long launch_counter();
+void launch_counter_add(long long n);
+bool profiling_enabled();
+
 }  // namespace far

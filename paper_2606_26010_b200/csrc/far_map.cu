@@ -133,7 +133,7 @@ __device__ __forceinline__ uint32_t voxel_limit(const MapView& m, const Asmd& A,
 // anywhere at or before its final position -- every position still ends up with the minimum of the ids that reach it --
 // and it removes most of the shifting); if c0 + ahead is already past the limit the point cannot survive at all.
 __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, const float* __restrict__ xyz, int64_t n,
-                                                                  int stride, int pose_mode, Pose hpose,
+                                                                  const int64_t* __restrict__ d_n, int stride, int pose_mode, Pose hpose,
                                                                   const Pose* __restrict__ d_pose, uint32_t id_offset,
                                                                   uint32_t* __restrict__ touched, Asmd asmd) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -141,6 +141,7 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
     const unsigned lt = (1u << lane) - 1u;
     const Pose& T = (pose_mode == 2) ? *d_pose : hpose;
     Counters* ctr = m.ctr;
+    if (d_n) n = min(n, *d_n);                  // frame graph: launch sized for the largest scan, count on the device
     float p[3];
     int k[3] = {0, 0, 0};
     bool valid = false, bad = false;
@@ -286,8 +287,8 @@ constexpr int COMMIT_LANES = 8;      // 4 and 16 measure the same within 3 %
 __global__ void __launch_bounds__(256) insert_commit_kernel(MapView m, const float* __restrict__ xyz, int stride,
                                                              int pose_mode, Pose hpose, const Pose* __restrict__ d_pose,
                                                              uint32_t id_offset, const uint32_t* __restrict__ touched,
-                                                             uint32_t* __restrict__ cov_list, int64_t n_call, int last_chunk,
-                                                             far_insert_stats_t* __restrict__ d_stats) {
+                                                             uint32_t* __restrict__ cov_list, int64_t n_call, const int64_t* __restrict__ d_n,
+                                                             int last_chunk, far_insert_stats_t* __restrict__ d_stats) {
     const int lane = threadIdx.x & 31, sub = lane / COMMIT_LANES, sl = lane % COMMIT_LANES;
     constexpr int PER_WARP = 32 / COMMIT_LANES;
     const unsigned gmask = ((1u << COMMIT_LANES) - 1u) << (sub * COMMIT_LANES);
@@ -298,6 +299,7 @@ __global__ void __launch_bounds__(256) insert_commit_kernel(MapView m, const flo
     const uint32_t n_touched = ctr->n_touched;
     const uint32_t first_id = (uint32_t)ctr->next_id + id_offset;
     const uint32_t cap = (uint32_t)m.cap;
+    if (d_n) n_call = min(n_call, *d_n);
     unsigned long long acc_new = 0;                       // lane sl == 0 of each group: points accepted
     for (int64_t t0 = warp * PER_WARP; t0 < n_touched; t0 += nwarps * PER_WARP) {
         const int64_t t = t0 + sub;
@@ -827,9 +829,14 @@ int far_map_renumber(far_map_t* m, void* stream) {
     return renumber_enqueue(m, (cudaStream_t)stream);
 }
 
-static int insert_impl(far_map_t* m, const float* d_xyz, int64_t n, int stride, int pose_mode, const far_pose_t* hpose,
-                       const far_pose_t* d_pose, int compute_cov, far_insert_stats_t* d_stats, void* stream,
-                       Asmd asmd = Asmd{nullptr, 1.0, 0}) {
+} // extern "C"
+
+// n = min(n, *d_n) if d_n is given (single chunk only: n <= max_batch); the host-side id bound advances by n
+int far::insert_impl(far_map_t* m, const float* d_xyz, int64_t n, const int64_t* d_n, int stride, int pose_mode, const far_pose_t* hpose,
+                     const far_pose_t* d_pose, int compute_cov, far_insert_stats_t* d_stats, void* stream, const double* d_n_close,
+                     double d_max) {
+    Asmd asmd{d_n_close, d_n_close ? d_max : 1.0, d_n_close ? 1 : 0};
+    if (d_n && n > m->max_batch) return FAR_ERR_ARG;
     if (!m || (!d_xyz && n > 0) || n < 0 || n > 0x7FFFFFFFll || (stride != 3 && stride != 4)) return FAR_ERR_ARG;
     if (compute_cov && !m->view.cov) return FAR_ERR_ARG;
     cudaStream_t st = (cudaStream_t)stream;
@@ -857,11 +864,11 @@ static int insert_impl(far_map_t* m, const float* d_xyz, int64_t n, int stride, 
         const float* xyz = d_xyz + off * stride;
         const int last = off + nc >= n;
         if (nc > 0)
-            FAR_LAUNCH(insert_claim_chain_kernel, grid_for(nc, 256), 256, 0, st, m->view, xyz, nc, stride, pose_mode, hp,
+            FAR_LAUNCH(insert_claim_chain_kernel, grid_for(nc, 256), 256, 0, st, m->view, xyz, nc, d_n, stride, pose_mode, hp,
                                                                           (const Pose*)d_pose, (uint32_t)off, m->d_touched, asmd);
         FAR_LAUNCH(insert_commit_kernel, nc > 0 ? commit_grid : 1, 256, 0, st, m->view, xyz, stride, pose_mode, hp,
                                                            (const Pose*)d_pose, (uint32_t)off, m->d_touched,
-                                                           cov_by_list ? m->d_cov_list : nullptr, n, last, d_stats);
+                                                           cov_by_list ? m->d_cov_list : nullptr, n, d_n, last, d_stats);
         FAR_CUDA(cudaGetLastError());
         off += nc;
     } while (off < n);
@@ -877,28 +884,30 @@ static int insert_impl(far_map_t* m, const float* d_xyz, int64_t n, int stride, 
     return m->h_mail->full ? FAR_ERR_FULL : FAR_OK;
 }
 
+extern "C" {
+
 int far_map_insert(far_map_t* m, const float* d_xyz, int64_t n, int stride, const far_pose_t* pose, int compute_cov,
                    far_insert_stats_t* d_stats, void* stream) {
-    return insert_impl(m, d_xyz, n, stride, pose ? 1 : 0, pose, nullptr, compute_cov, d_stats, stream);
+    return far::insert_impl(m, d_xyz, n, nullptr, stride, pose ? 1 : 0, pose, nullptr, compute_cov, d_stats, stream, nullptr, 1.0);
 }
 
 int far_map_insert_dev(far_map_t* m, const float* d_xyz, int64_t n, int stride, const far_pose_t* d_pose,
                        int compute_cov, far_insert_stats_t* d_stats, void* stream) {
     if (!d_pose) return FAR_ERR_ARG;
-    return insert_impl(m, d_xyz, n, stride, 2, nullptr, d_pose, compute_cov, d_stats, stream);
+    return far::insert_impl(m, d_xyz, n, nullptr, stride, 2, nullptr, d_pose, compute_cov, d_stats, stream, nullptr, 1.0);
 }
 
 int far_map_insert_asmd(far_map_t* m, const float* d_xyz, int64_t n, int stride, const far_pose_t* pose,
                         const double* d_n_close, double d_max, int compute_cov, far_insert_stats_t* d_stats, void* stream) {
     if (!d_n_close || !(d_max > 0.0)) return FAR_ERR_ARG;
-    return insert_impl(m, d_xyz, n, stride, pose ? 1 : 0, pose, nullptr, compute_cov, d_stats, stream, Asmd{d_n_close, d_max, 1});
+    return far::insert_impl(m, d_xyz, n, nullptr, stride, pose ? 1 : 0, pose, nullptr, compute_cov, d_stats, stream, d_n_close, d_max);
 }
 
 int far_map_insert_asmd_dev(far_map_t* m, const float* d_xyz, int64_t n, int stride, const far_pose_t* d_pose,
                             const double* d_n_close, double d_max, int compute_cov, far_insert_stats_t* d_stats,
                             void* stream) {
     if (!d_pose || !d_n_close || !(d_max > 0.0)) return FAR_ERR_ARG;
-    return insert_impl(m, d_xyz, n, stride, 2, nullptr, d_pose, compute_cov, d_stats, stream, Asmd{d_n_close, d_max, 1});
+    return far::insert_impl(m, d_xyz, n, nullptr, stride, 2, nullptr, d_pose, compute_cov, d_stats, stream, d_n_close, d_max);
 }
 
 // PAPER.md:109 "the average amount of points per voxel in a close range of the current scan" (R17)
@@ -1021,6 +1030,10 @@ LaunchScope::LaunchScope(const char* name, cudaStream_t st) : rec_(-1), st_(st) 
         }
     }
 }
+
+long long launch_counter() { return g_launches.load(std::memory_order_relaxed); }
+void launch_counter_add(long long n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+bool profiling_enabled() { return g_prof.load(std::memory_order_relaxed) != 0; }
 
 LaunchScope::~LaunchScope() {
     if (rec_ >= 0) {

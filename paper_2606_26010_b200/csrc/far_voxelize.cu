@@ -23,8 +23,10 @@ struct VoxWs {
     uint32_t slots, mask;
 };
 
-__global__ void __launch_bounds__(256) vox_claim_kernel(VoxWs w, const float* __restrict__ xyz, int64_t n, int stride, float v) {
+__global__ void __launch_bounds__(256) vox_claim_kernel(VoxWs w, const float* __restrict__ xyz, int64_t n, const int64_t* __restrict__ d_n,
+                                                         int stride, float v) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (d_n) n = min(n, *d_n);                  // frame graph: the launch is sized for the largest scan, the count is on the device
     if (i >= n) return;
     const float* p = xyz + i * stride;
     int k[3];
@@ -49,8 +51,9 @@ __device__ __forceinline__ bool vox_is_first(const VoxWs& w, int64_t i, int64_t 
     return s != NO_SLOT && w.first[s] == (uint32_t)i;
 }
 
-__global__ void __launch_bounds__(VTILE) vox_count_kernel(VoxWs w, int64_t n) {
+__global__ void __launch_bounds__(VTILE) vox_count_kernel(VoxWs w, int64_t n, const int64_t* __restrict__ d_n) {
     __shared__ int s_cnt[VTILE / 32];
+    if (d_n) n = min(n, *d_n);
     const int64_t i = (int64_t)blockIdx.x * VTILE + threadIdx.x;
     const unsigned b = __ballot_sync(FULL, vox_is_first(w, i, n));
     if ((threadIdx.x & 31) == 0) s_cnt[threadIdx.x >> 5] = __popc(b);
@@ -101,9 +104,10 @@ __global__ void __launch_bounds__(1024) vox_scan_kernel(VoxWs w, int tiles, int6
     if (threadIdx.x == 0) *n_out = (int64_t)s_carry;
 }
 
-__global__ void __launch_bounds__(VTILE) vox_scatter_kernel(VoxWs w, const float* __restrict__ xyz, int64_t n, int stride,
-                                                             float* __restrict__ out_xyz, int32_t* __restrict__ out_index) {
+__global__ void __launch_bounds__(VTILE) vox_scatter_kernel(VoxWs w, const float* __restrict__ xyz, int64_t n, const int64_t* __restrict__ d_n,
+                                                             int stride, float* __restrict__ out_xyz, int32_t* __restrict__ out_index) {
     __shared__ int s_cnt[VTILE / 32];
+    if (d_n) n = min(n, *d_n);
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int64_t i = (int64_t)blockIdx.x * VTILE + threadIdx.x;
     const bool f = vox_is_first(w, i, n);
@@ -137,8 +141,19 @@ static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 }  // namespace far
 
+namespace far {
+int voxelize_impl(const float* d_xyz, int64_t n, const int64_t* d_n, int stride, float voxel, float* d_out_xyz, int32_t* d_out_index,
+                  int64_t* d_n_out, void* d_workspace, size_t* workspace_bytes, void* stream);
+}
+
 extern "C" int far_voxelize(const float* d_xyz, int64_t n, int stride, float voxel, float* d_out_xyz, int32_t* d_out_index,
                             int64_t* d_n_out, void* d_workspace, size_t* workspace_bytes, void* stream) {
+    return far::voxelize_impl(d_xyz, n, nullptr, stride, voxel, d_out_xyz, d_out_index, d_n_out, d_workspace, workspace_bytes, stream);
+}
+
+// n = min(n, *d_n) if d_n is given (read on the device in stream order)
+int far::voxelize_impl(const float* d_xyz, int64_t n, const int64_t* d_n, int stride, float voxel, float* d_out_xyz, int32_t* d_out_index,
+                       int64_t* d_n_out, void* d_workspace, size_t* workspace_bytes, void* stream) {
     if (n < 0 || n > (1ll << 30) || (stride != 3 && stride != 4) || !(voxel > 0.f) || !workspace_bytes) return FAR_ERR_ARG;
     uint64_t slots = 64;
     while (slots < 2 * (uint64_t)n) slots <<= 1;
@@ -163,10 +178,10 @@ extern "C" int far_voxelize(const float* d_xyz, int64_t n, int stride, float vox
     w.slots = (uint32_t)slots;
     w.mask = (uint32_t)slots - 1;
     FAR_CUDA(cudaMemsetAsync(base, 0xFF, b_keys + b_first, st));   // keys = empty, first = +inf
-    FAR_LAUNCH(vox_claim_kernel, grid_for(n, 256), 256, 0, st, w, d_xyz, n, stride, voxel);
-    FAR_LAUNCH(vox_count_kernel, (int)tiles, VTILE, 0, st, w, n);
+    FAR_LAUNCH(vox_claim_kernel, grid_for(n, 256), 256, 0, st, w, d_xyz, n, d_n, stride, voxel);
+    FAR_LAUNCH(vox_count_kernel, (int)tiles, VTILE, 0, st, w, n, d_n);
     FAR_LAUNCH(vox_scan_kernel, 1, 1024, 0, st, w, (int)tiles, d_n_out);
-    FAR_LAUNCH(vox_scatter_kernel, (int)tiles, VTILE, 0, st, w, d_xyz, n, stride, d_out_xyz, d_out_index);
+    FAR_LAUNCH(vox_scatter_kernel, (int)tiles, VTILE, 0, st, w, d_xyz, n, d_n, stride, d_out_xyz, d_out_index);
     FAR_CUDA(cudaGetLastError());
     return FAR_OK;
 }

@@ -43,6 +43,14 @@ def _cov_close(g, o, tol=1e-4):
     assert rel.max() < tol, rel.max()
 
 
+# Stored coordinates after an insert at a REGISTERED pose: the two sides' poses agree to ~1e-10 m (different summation
+# orders of the same FP64 terms, amplified by the chain of frames), and a coordinate is that pose applied to the point,
+# rounded to fp32 once.  Where the 1e-10 straddles a rounding boundary the stored values differ by one fp32 ulp -- 6.1e-5 m
+# at the 1 km coordinates of the race track -- so the bar is two ulps there, far inside north_star's pose tolerance
+# (1e-4 m + 1e-5 rad x 200 m range).  At a GIVEN pose the same insert is bit-exact (tests/test_gpu_map.py).
+XYZ_TOL_1KM = 1.3e-4
+
+
 def _result(d_res):
     return far.result_to_dict(far.GicpResult.from_buffer_copy(d_res.cpu().numpy().tobytes()))
 
@@ -105,7 +113,7 @@ def test_c2_full_frame_as_benched():
     eo1, eg1 = mo.export(with_cov=True), fe.map.export(with_cov=True)
     assert np.array_equal(eg1["keys"], eo1["keys"]) and np.array_equal(eg1["counts"], eo1["counts"])
     assert np.array_equal(eg1["ids"], eo1["ids"])
-    assert np.abs(eg1["xyz"] - eo1["xyz"]).max() < 1e-5          # poses agree to ~1e-12, fp32 rounding may differ
+    assert np.abs(eg1["xyz"] - eo1["xyz"]).max() < 3.1e-5        # two fp32 ulps at the scene's 150 m (see XYZ_TOL_1KM)
     assert np.array_equal(eg1["cov_valid"], eo1["cov_valid"])
     fe.close()
 
@@ -157,7 +165,7 @@ def test_c3_racing_frames_chain_matches_oracle_frame_by_frame():
     assert min(iters) < 10 and max(iters) > 10          # both quick and long registrations were exercised
     eo, eg = mo.export(with_cov=True), fe.map.export(with_cov=True)
     assert np.array_equal(eg["keys"], eo["keys"]) and np.array_equal(eg["ids"], eo["ids"])
-    assert np.abs(eg["xyz"] - eo["xyz"]).max() < 1e-5
+    assert np.abs(eg["xyz"] - eo["xyz"]).max() < XYZ_TOL_1KM
     assert np.array_equal(eg["cov_valid"], eo["cov_valid"])
     # the corridor is degenerate along-track (expect it, report it, do not tune it away):
     # only lateral / vertical / heading errors are bounded
@@ -232,7 +240,7 @@ def test_c3_racing_sequence_200_frames_ekf_prior_matches_oracle_every_frame():
     eo, eg = mo.export(with_cov=True), fe.map.export(with_cov=True)
     assert np.array_equal(eg["keys"], eo["keys"]) and np.array_equal(eg["counts"], eo["counts"])
     assert np.array_equal(eg["ids"], eo["ids"])
-    assert np.abs(eg["xyz"] - eo["xyz"]).max() < 1e-5
+    assert np.abs(eg["xyz"] - eo["xyz"]).max() < XYZ_TOL_1KM
     assert np.array_equal(eg["cov_valid"], eo["cov_valid"])
     st = fe.map.stats()
     assert st["full"] == 0 and st["n_rehash"] > 0 and st["n_dead_keys"] < 64 + st["n_voxels"] // 4    # 2^16-bucket map, 198 prunes

@@ -341,3 +341,63 @@ def test_frontend_chain_equals_manual_chain_and_host_variant():
         assert np.abs(eg["xyz"] - eo["xyz"]).max() < 1e-5
         assert np.array_equal(eg["cov_valid"], eo["cov_valid"])
         fe.close()
+
+
+def test_frame_graph_replay_equals_stream_of_launches_and_oracle():
+    """the frame as ONE CUDA graph.  Three frames of different sizes and poses through the same buffers: the
+    first runs as a stream of launches, the second captures, the third replays; every frame's result and the final map
+    equal those of the stream path (use_graph = 0) bit for bit and the oracle's within tolerance.  Per replayed frame the
+    library launches no more kernels than the stream path does."""
+    c2 = scenes.c2_single_frame(seed=6, n_map_candidates=100_000, map_radius=45.0, rings=16, azimuths=512)
+    v, cap, sigma, scan = c2["voxel"], c2["cap"], c2["sigma"], c2["scan"]
+    rng = np.random.default_rng(3)
+    sizes = [len(scan), len(scan) - 1777, len(scan) - 31]
+    poses = [c2["T_init"], scenes.perturb_pose(c2["T_gt"], 0.2, 1.0, rng), scenes.perturb_pose(c2["T_gt"], 0.1, 0.5, rng)]
+    sig = [sigma, 1.0, 0.7]
+    # oracle: three frames in a row on one map
+    mo = oracle.Map(v, cap)
+    mo.insert(c2["map_points"], compute_cov=True)
+    res_o = []
+    for n, T, sg in zip(sizes, poses, sig):
+        s = scan[:n]
+        ds_o, _ = oracle.voxelize(s, v)
+        lo = oracle.Map(v, cap); lo.insert(s)
+        cov_o, val_o = lo.knn_cov(ds_o, nthreads=8)
+        o = mo.gicp_register(ds_o, cov_o, val_o, T, sg, 30, nthreads=8)
+        mo.insert(s, pose=(o["R"], o["t"]), compute_cov=True)
+        mo.prune(o["t"], 30.0)
+        res_o.append(o)
+    eo = mo.export(with_cov=True)
+    outs = {}
+    for use_graph in (False, True):
+        fe = far.Frontend(v, cap, 4 * len(c2["map_points"]), len(scan), prune_radius=30.0, max_iters=30, use_graph=use_graph)
+        fe.map.insert(c2["map_points"], compute_cov=True)
+        buf = torch.zeros((len(scan), 3), dtype=torch.float32, device="cuda")      # ONE scan buffer, as a driver would keep
+        d_res = torch.zeros(far.GICP_RESULT_BYTES, dtype=torch.uint8, device="cuda")
+        rs, launches = [], []
+        for n, T, sg in zip(sizes, poses, sig):
+            buf[:n] = torch.as_tensor(scan[:n]).cuda()
+            l0 = far.launch_count()
+            rc = far.lib().far_frontend_process(fe._h, buf.data_ptr(), n, 3, far.C.byref(far.Pose.from_rt(T)), sg, d_res.data_ptr(),
+                                                torch.cuda.current_stream().cuda_stream)
+            assert rc == far.OK
+            launches.append(far.launch_count() - l0)
+            torch.cuda.synchronize()
+            rs.append(d_res.cpu().numpy().tobytes())
+        assert fe.graph_state() == (1 if use_graph else 0)
+        assert launches[2] == launches[0] and launches[0] <= 20
+        outs[use_graph] = (rs, fe.map.export(with_cov=True), fe.map.stats())
+        fe.close()
+    (ra, ea, sa), (rb, eb, sb) = outs[False], outs[True]
+    assert ra == rb                                           # far_gicp_result_t bytes of every frame
+    for k in ("keys", "counts", "ids", "xyz", "cov", "cov_valid"):
+        assert np.array_equal(ea[k].view(np.uint8), eb[k].view(np.uint8)), k
+    assert sa == sb
+    for raw, o in zip(rb, res_o):
+        g = far.result_to_dict(far.GicpResult.from_buffer_copy(raw))
+        assert g["status"] == 0 and g["iters"] == o["iters"] and g["n_inliers"] == o["n_inliers"]
+        dt, dr = _pose_err(g, o)
+        assert dt < 1e-4 and dr < 1e-5, (dt, dr)
+    assert np.array_equal(eb["keys"], eo["keys"]) and np.array_equal(eb["ids"], eo["ids"])
+    assert np.abs(eb["xyz"] - eo["xyz"]).max() < 1e-5
+    assert np.array_equal(eb["cov_valid"], eo["cov_valid"])
