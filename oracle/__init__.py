@@ -94,6 +94,8 @@ def lib():
         L.faro_map_prune.argtypes = [vp, vp, f64, vp]
         L.faro_map_size.argtypes = [vp, vp, vp, vp]
         L.faro_map_renumber.argtypes = [vp, vp]
+        L.faro_map_set_min_spacing.argtypes = [vp, f64]
+        L.faro_map_set_min_spacing.restype = None
         L.faro_map_export.argtypes = [vp, vp, vp, vp, vp, vp]
         L.faro_map_nn.argtypes = [vp, vp, i64, C.c_int, vp, vp, C.c_int]
         L.faro_map_nn_brute.argtypes = [vp, vp, i64, C.c_int, vp, vp]
@@ -218,11 +220,13 @@ def asmd_cap(k3, voxel, center, n_close, d_max, k_min, cap):
 
 
 class Map:
-    def __init__(self, voxel, cap, k_cov=10, cov_eps=1e-3):
+    def __init__(self, voxel, cap, k_cov=10, cov_eps=1e-3, min_spacing=0.0):
         self.voxel, self.cap, self.k_cov = float(voxel), int(cap), int(k_cov)
         self._h = lib().faro_map_create(voxel, cap, k_cov, cov_eps)
         if not self._h:
             raise ValueError("bad map config")
+        if min_spacing > 0.0:
+            lib().faro_map_set_min_spacing(self._h, float(min_spacing))
 
     def __del__(self):
         if getattr(self, "_h", None):

@@ -164,6 +164,7 @@ struct faro_map {
     int32_t k_cov;
     double cov_eps;
     uint64_t next_id;
+    double min_spacing = 0.0;   // R21: > 0: a point is stored only if no point already in ITS OWN voxel is closer than this
     std::unordered_map<uint64_t, Voxel> vox;
 
     // A6 candidate enumeration: the query's voxel and its 26 neighbours (Fig. 3)
@@ -282,6 +283,7 @@ faro_map_t* faro_map_create(float voxel, int32_t cap, int32_t k_cov, double cov_
     return m;
 }
 void faro_map_destroy(faro_map_t* m) { delete m; }
+void faro_map_set_min_spacing(faro_map_t* m, double s) { if (m) m->min_spacing = s > 0.0 ? s : 0.0; }
 
 namespace {
 
@@ -324,7 +326,18 @@ int insert_points(faro_map_t* m, const float* xyz, int64_t n, int stride, const 
         if (ins.second) st.n_new_voxels++;
         Voxel& vx = ins.first->second;
         const int32_t limit = asmd ? asmd_cap(k, m->voxel, centre, n_close, d_max, m->k_cov, m->cap) : m->cap;
-        if ((int32_t)vx.pts.size() < limit) {
+        bool spaced = true;
+        if (m->min_spacing > 0.0) {
+            // R21 ("regularly spaced ... a minimum point-to-point distance of ~65 cm" at v = 4 m, N_max = 40,
+            // i.e. v / sqrt(N_max)): sequential rule, points in index order; squared distance as R6, strict <
+            const double s2 = m->min_spacing * m->min_spacing;
+            for (const Pt& q : vx.pts) {
+                const double dx = (double)p[0] - (double)q.x, dy = (double)p[1] - (double)q.y, dz = (double)p[2] - (double)q.z;
+                const double d2 = (dx * dx + dy * dy) + dz * dz;
+                if (d2 < s2) { spaced = false; break; }
+            }
+        }
+        if ((int32_t)vx.pts.size() < limit && spaced) {
             Pt pt{p[0], p[1], p[2], id, {1, 0, 0, 1, 0, 1}, 0};
             vx.pts.push_back(pt);
             st.n_accepted++;

@@ -263,3 +263,74 @@ def test_asmd_insert_with_pose_uses_pose_translation_as_centre_and_keeps_existin
     got2 = {int(k): [int(i) for i in e2["ids"][v, :e2["counts"][v]]] for v, k in enumerate(e2["keys"])}
     for k, v in before.items():
         assert got2[k][:len(v)] == v
+
+
+# ---- R21: regular spacing ("regularly spaced, with a minimum point-to-point distance of ~65 cm") -------------
+def _spaced_restatement(xyz, voxel, cap, s):
+    """the sequential rule written out with a dict and NumPy float64: {key: [ids]}"""
+    from helpers import np_pack, np_voxel_index
+    keys = np_pack(np_voxel_index(xyz, voxel))
+    P = np.asarray(xyz, dtype=np.float64)
+    out = {}
+    for i, k in enumerate(keys.tolist()):
+        ids = out.setdefault(k, [])
+        if len(ids) >= cap:
+            continue
+        if ids:
+            d = P[i] - P[ids]
+            d2 = (d[:, 0] * d[:, 0] + d[:, 1] * d[:, 1]) + d[:, 2] * d[:, 2]
+            if (d2 < s * s).any():
+                continue
+        ids.append(i)
+    return out
+
+
+def test_min_spacing_hand_example():
+    """v = 4, s = 1: (0.5,0.5,0.5) stored; (1.0,0.5,0.5) is 0.5 away -> dropped; (1.5,0.5,0.5) is exactly 1.0 away -> stored
+    (strict <); (1.9,0.5,0.5) is 0.4 from the third -> dropped; (4.1,0.5,0.5) lies 2.6 from the third but in the NEXT voxel,
+    where nothing is stored -> stored; (4.3,0.5,0.5) is 0.2 from it -> dropped.  Ids are consumed by dropped points."""
+    pts = np.array([[0.5, 0.5, 0.5], [1.0, 0.5, 0.5], [1.5, 0.5, 0.5], [1.9, 0.5, 0.5], [4.1, 0.5, 0.5], [4.3, 0.5, 0.5],
+                    [3.9, 0.5, 0.5]], dtype=np.float32)
+    m = oracle.Map(4.0, 40, min_spacing=1.0)
+    st = m.insert(pts)
+    e = m.export()
+    stored = {int(k): [int(i) for i in ids[:c]] for k, c, ids in zip(e["keys"], e["counts"], e["ids"])}
+    assert stored == {oracle.pack_key(0, 0, 0): [0, 2, 6], oracle.pack_key(1, 0, 0): [4]}     # 3.9 is 0.2 from 4.1 but in the other voxel
+    assert st["n_accepted"] == 4 and st["n_new_voxels"] == 2 and m.size()[2] == 7
+
+
+def test_min_spacing_matches_sequential_restatement_and_invariants():
+    rng = np.random.default_rng(41)
+    pts = np.concatenate([rng.uniform(-8, 8, size=(3000, 3)), rng.normal(0, 0.3, size=(3000, 3)) + [2.0, 2.0, 2.0]]).astype(np.float32)
+    rng.shuffle(pts)
+    v, cap, s = 4.0, 40, 4.0 / np.sqrt(40.0)                     # the paper's parameters: s = v / sqrt(N_max) = 0.632 m
+    m = oracle.Map(v, cap, min_spacing=s)
+    st = m.insert(pts[:3500])
+    st2 = m.insert(pts[3500:])                                   # a second batch tests against what the first stored
+    e = m.export()
+    want = _spaced_restatement(pts, v, cap, s)
+    got = {int(k): [int(i) for i in ids[:c]] for k, c, ids in zip(e["keys"], e["counts"], e["ids"])}
+    assert got == want
+    assert st["n_accepted"] + st2["n_accepted"] == sum(len(x) for x in want.values())
+    # invariant: no two stored points of a voxel closer than s; the cap is never exceeded; ids ascend
+    for v_i in range(len(e["keys"])):
+        c = int(e["counts"][v_i])
+        assert c <= cap
+        P = e["xyz"][v_i, :c].astype(np.float64)
+        if c > 1:
+            d = np.linalg.norm(P[:, None, :] - P[None, :, :], axis=2) + np.eye(c) * 1e9
+            assert d.min() >= s * (1 - 1e-12)
+        assert (np.diff(e["ids"][v_i, :c].astype(np.int64)) > 0).all()
+    # the clump at (2,2,2) would fill its voxel with near-duplicates without the rule
+    plain = oracle.Map(v, cap)
+    plain.insert(pts)
+    assert plain.size()[1] > m.size()[1]
+
+
+def test_min_spacing_zero_is_the_plain_insert():
+    rng = np.random.default_rng(42)
+    pts = rng.uniform(-5, 5, size=(4000, 3)).astype(np.float32)
+    a, b = oracle.Map(1.0, 6), oracle.Map(1.0, 6, min_spacing=0.0)
+    assert a.insert(pts) == b.insert(pts)
+    ea, eb = a.export(), b.export()
+    assert np.array_equal(ea["keys"], eb["keys"]) and np.array_equal(ea["ids"], eb["ids"])
