@@ -59,6 +59,10 @@ typedef struct {
     double cov_eps;        /* regulariser of Eq. 1; 0 -> 1e-3                                 */
     int64_t max_batch;     /* points per internal insert pass; 0 -> 1<<20.  Larger calls are chunked      */
     int64_t renumber_every;/* offered points between automatic id renumber passes (R22); 0 -> 2^31         */
+    double min_spacing;    /* > 0: regular spacing ("regularly spaced ... ~65 cm" at v = 4 m, N_max = 40,
+                              i.e. v / sqrt(N_max); R21): an offered point is stored only if no point already stored in
+                              ITS OWN voxel is closer (FP64 d2 of R6, strict <), decided in index order after the cap /
+                              N_ASMD test.  0: the plain capped insert */
 } far_map_config_t;
 
 typedef struct { int64_t n_offered, n_accepted, n_new_voxels, n_dropped_full, n_invalid; } far_insert_stats_t;

@@ -44,7 +44,7 @@ class Pose(C.Structure):
 class MapConfig(C.Structure):
     _fields_ = [("voxel_size", C.c_float), ("cap", C.c_int32), ("max_voxels", C.c_int64), ("max_load", C.c_float),
                 ("with_cov", C.c_int32), ("k_cov", C.c_int32), ("cov_eps", C.c_double), ("max_batch", C.c_int64),
-                ("renumber_every", C.c_int64)]
+                ("renumber_every", C.c_int64), ("min_spacing", C.c_double)]
 
 
 class GicpOptions(C.Structure):
@@ -299,13 +299,14 @@ class Map:
     """A far_map_t handle.  All bulk arguments are CUDA tensors (NumPy arrays are uploaded for convenience)."""
 
     def __init__(self, voxel, cap, max_voxels, with_cov=False, k_cov=10, cov_eps=1e-3, max_load=0.5, max_batch=1 << 20,
-                 renumber_every=0, _borrowed=None):
+                 renumber_every=0, min_spacing=0.0, _borrowed=None):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2606_26010_b200 needs a CUDA device: there is no CPU fallback")
         self.voxel, self.cap, self.k_cov, self.with_cov = float(voxel), int(cap), int(k_cov), bool(with_cov)
         self._owned = _borrowed is None
         if _borrowed is None:
-            cfg = MapConfig(voxel, cap, int(max_voxels), max_load, int(with_cov), k_cov, cov_eps, int(max_batch), int(renumber_every))
+            cfg = MapConfig(voxel, cap, int(max_voxels), max_load, int(with_cov), k_cov, cov_eps, int(max_batch), int(renumber_every),
+                            float(min_spacing))
             h = C.c_void_p()
             _check(lib().far_map_create(C.byref(h), C.byref(cfg)), "far_map_create")
             self._h = h
@@ -514,11 +515,11 @@ class Frontend:
 
     def __init__(self, voxel, cap, max_voxels, max_scan_points, ds_voxel=0.0, prune_radius=0.0, max_iters=30,
                  update_map=True, opts=None, k_cov=10, cov_eps=1e-3, max_load=0.5, asmd=False, asmd_r_close=10.0,
-                 asmd_d_max=100.0, use_graph=True):
+                 asmd_d_max=100.0, use_graph=True, min_spacing=0.0):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2606_26010_b200 needs a CUDA device: there is no CPU fallback")
         o = opts if opts is not None else default_options()
-        cfg = FrontendConfig(MapConfig(voxel, cap, int(max_voxels), max_load, 1, k_cov, cov_eps, 0, 0), ds_voxel,
+        cfg = FrontendConfig(MapConfig(voxel, cap, int(max_voxels), max_load, 1, k_cov, cov_eps, 0, 0, float(min_spacing)), ds_voxel,
                              int(max_scan_points), float(prune_radius), int(max_iters), int(update_map), o,
                              int(asmd), float(asmd_r_close), float(asmd_d_max), int(use_graph))
         h = C.c_void_p()

@@ -89,6 +89,7 @@ int far_frontend_create(far_frontend_t** out, const far_frontend_config_t* cfg) 
     if (rc == FAR_OK) {
         far_map_config_t lc = cfg->map;
         lc.with_cov = 0;
+        lc.min_spacing = 0.0;       // R8/R21: Cov-Calc looks for the k nearest RAW scan points; spacing shapes the submap only
         lc.max_voxels = cfg->max_scan_points;
         lc.max_load = 0.5f;
         lc.max_batch = cfg->max_scan_points;

@@ -109,6 +109,21 @@ struct Asmd {
     int on;
 };
 
+// ---- regular spacing ("regularly spaced ... minimum point-to-point distance of ~65 cm"; R21) --
+// With min_spacing > 0 acceptance depends on the points accepted before, so the atomicMin chain cannot decide it.  The
+// claim kernel then only LISTS every offered point for its voxel (count per bucket, bucket per point); the offers of a
+// voxel are gathered into one contiguous segment (scan + scatter) and one block per touched voxel sorts them by id and
+// walks them in order, 32 at a time against the stored points (spaced_commit_kernel).  Scratch allocated at create.
+struct Spaced {
+    uint32_t* offer_cnt;       // [max_voxels] offers per bucket in the running chunk (all zero between chunks)
+    uint32_t* voxel_t;         // [max_voxels] index of the bucket's voxel in the touched list
+    uint32_t* pt_bucket;       // [max_batch]  bucket of point i of the chunk, NO_BUCKET if it is not offered
+    uint32_t* seg_start;       // [max_batch + 1] first entry of touched voxel t in `seg`
+    uint32_t* seg;             // [max_batch]  point indices, grouped by voxel
+    double s2;                 // min_spacing^2
+    int on;
+};
+
 __device__ __forceinline__ uint32_t voxel_limit(const MapView& m, const Asmd& A, const int k[3], int pose_mode, const Pose& T) {
     if (!A.on) return (uint32_t)m.cap;
     const double v = (double)m.voxel;
@@ -135,7 +150,7 @@ __device__ __forceinline__ uint32_t voxel_limit(const MapView& m, const Asmd& A,
 __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, const float* __restrict__ xyz, int64_t n,
                                                                   const int64_t* __restrict__ d_n, int stride, int pose_mode, Pose hpose,
                                                                   const Pose* __restrict__ d_pose, uint32_t id_offset,
-                                                                  uint32_t* __restrict__ touched, Asmd asmd) {
+                                                                  uint32_t* __restrict__ touched, Asmd asmd, Spaced sp) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
@@ -246,7 +261,15 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
 
     // phase 4: the chain.  cap = this voxel's limit: the fixed cap, or N_ASMD (positions at and beyond it are never written)
     bool first_of_voxel = false;
-    if (valid && b != NO_BUCKET) {
+    if (sp.on) {
+        // regular spacing: no chain -- the point is listed for its voxel (one atomic per group of lanes with the same key)
+        uint32_t pb = NO_BUCKET;
+        if (valid && b != NO_BUCKET) {
+            pb = b;
+            if (ahead == 0) first_of_voxel = atomicAdd(&sp.offer_cnt[b], (unsigned)__popc(same)) == 0u;
+        }
+        if (i < n) sp.pt_bucket[i] = pb;
+    } else if (valid && b != NO_BUCKET) {
         const uint32_t cap = voxel_limit(m, asmd, k, pose_mode, T);
         uint32_t* idw = m.ids + (size_t)b * (uint32_t)m.cap;   // id word of position 0
         uint32_t x = id_base + (uint32_t)i;
@@ -275,7 +298,44 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
         uint32_t at = 0;
         if (lane == 0) at = atomicAdd(&ctr->n_touched, (unsigned)__popc(m_first));
         at = __shfl_sync(FULL, at, 0);
-        if (first_of_voxel) touched[at + __popc(m_first & lt)] = s;
+        if (first_of_voxel) {
+            const uint32_t t = at + __popc(m_first & lt);
+            touched[t] = s;
+            if (sp.on) sp.voxel_t[b] = t;
+        }
+    }
+}
+
+// The block that finishes last closes the chunk (all threads of all blocks call): touched list and allocator re-armed; after
+// the last chunk the call's statistics go out, the counters are zeroed and the id counter advances -- no separate launch,
+// no memset.
+__device__ __forceinline__ void insert_epilogue(const MapView& m, int64_t n_call, int last_chunk, far_insert_stats_t* __restrict__ d_stats) {
+    Counters* ctr = m.ctr;
+    if (last_block_done(&ctr->ticket[0]) && threadIdx.x == 0) {
+        volatile Counters* c = ctr;
+        c->n_touched = 0u;
+        if (last_chunk) { c->n_tasks = c->n_cov; c->n_cov = 0u; }
+        {   // fold the kernel's bucket draws into the allocator state
+            const unsigned drawn = c->n_alloc, nf = (unsigned)c->n_free;
+            const unsigned from_free = drawn < nf ? drawn : nf;
+            c->n_free = (int)(nf - from_free);
+            const unsigned long long bump = (unsigned long long)c->bump + (drawn - from_free);
+            c->bump = bump > m.max_buckets ? m.max_buckets : (unsigned)bump;
+            c->n_alloc = 0u;
+        }
+        if (last_chunk) {
+            c->call_first_id = c->next_id;
+            c->next_id = c->next_id + (unsigned long long)n_call;
+            if (d_stats) {
+                d_stats->n_offered = n_call;
+                d_stats->n_accepted = (int64_t)c->st_accepted;
+                d_stats->n_new_voxels = (int64_t)c->st_new_voxels;
+                d_stats->n_dropped_full = (int64_t)c->st_dropped_full;
+                d_stats->n_invalid = (int64_t)c->st_invalid;
+            }
+            c->st_accepted = 0ull; c->st_new_voxels = 0ull; c->st_dropped_full = 0ull; c->st_invalid = 0ull;
+            if (c->full_flag) m.mail->full = 1u;
+        }
     }
 }
 
@@ -342,32 +402,188 @@ __global__ void __launch_bounds__(256) insert_commit_kernel(MapView m, const flo
     for (int d = 16; d > 0; d >>= 1) acc_new += __shfl_xor_sync(FULL, acc_new, d);
     if (lane == 0 && acc_new) atomicAdd(&ctr->st_accepted, acc_new);
 
-    if (last_block_done(&ctr->ticket[0]) && threadIdx.x == 0) {
-        volatile Counters* c = ctr;
-        c->n_touched = 0u;
-        if (last_chunk) { c->n_tasks = c->n_cov; c->n_cov = 0u; }
-        {   // fold the kernel's bucket draws into the allocator state
-            const unsigned drawn = c->n_alloc, nf = (unsigned)c->n_free;
-            const unsigned from_free = drawn < nf ? drawn : nf;
-            c->n_free = (int)(nf - from_free);
-            const unsigned long long bump = (unsigned long long)c->bump + (drawn - from_free);
-            c->bump = bump > m.max_buckets ? m.max_buckets : (unsigned)bump;
-            c->n_alloc = 0u;
+    insert_epilogue(m, n_call, last_chunk, d_stats);
+}
+
+// ---- regular spacing, kernel 2: exclusive scan of the offers per touched voxel (one block; a few thousand voxels) -----
+__global__ void __launch_bounds__(1024) spaced_scan_kernel(MapView m, const uint32_t* __restrict__ touched, Spaced sp) {
+    __shared__ uint32_t s_warp[32];
+    __shared__ uint32_t s_carry;
+    if (threadIdx.x == 0) s_carry = 0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const uint32_t n_touched = m.ctr->n_touched;
+    for (uint32_t base = 0; base < n_touched; base += 1024) {
+        const uint32_t t = base + threadIdx.x;
+        const uint32_t c = t < n_touched ? sp.offer_cnt[m.table[touched[t]].bucket] : 0u;
+        uint32_t incl = c;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t o = __shfl_up_sync(FULL, incl, d);
+            if (lane >= d) incl += o;
         }
-        if (last_chunk) {
-            c->call_first_id = c->next_id;
-            c->next_id = c->next_id + (unsigned long long)n_call;
-            if (d_stats) {
-                d_stats->n_offered = n_call;
-                d_stats->n_accepted = (int64_t)c->st_accepted;
-                d_stats->n_new_voxels = (int64_t)c->st_new_voxels;
-                d_stats->n_dropped_full = (int64_t)c->st_dropped_full;
-                d_stats->n_invalid = (int64_t)c->st_invalid;
+        if (lane == 31) s_warp[wid] = incl;
+        __syncthreads();
+        if (wid == 0) {
+            uint32_t x = s_warp[lane];
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const uint32_t o = __shfl_up_sync(FULL, x, d);
+                if (lane >= d) x += o;
             }
-            c->st_accepted = 0ull; c->st_new_voxels = 0ull; c->st_dropped_full = 0ull; c->st_invalid = 0ull;
-            if (c->full_flag) m.mail->full = 1u;
+            s_warp[lane] = x;
         }
+        __syncthreads();
+        const uint32_t excl = s_carry + (wid ? s_warp[wid - 1] : 0u) + incl - c;
+        if (t < n_touched) sp.seg_start[t] = excl;
+        __syncthreads();
+        if (threadIdx.x == 1023) s_carry = excl + c;
+        __syncthreads();
     }
+    if (threadIdx.x == 0) sp.seg_start[n_touched] = s_carry;
+}
+
+// ---- regular spacing, kernel 3: every offered point goes into its voxel's segment (order inside a segment arbitrary) --
+__global__ void __launch_bounds__(256) spaced_scatter_kernel(MapView m, int64_t n, const int64_t* __restrict__ d_n, Spaced sp) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (d_n) n = min(n, *d_n);
+    if (i >= n) return;
+    const uint32_t b = sp.pt_bucket[i];
+    if (b == NO_BUCKET) return;
+    const uint32_t pos = atomicSub(&sp.offer_cnt[b], 1u) - 1u;          // counts down to zero: clean for the next chunk
+    sp.seg[sp.seg_start[sp.voxel_t[b]] + pos] = (uint32_t)i;
+}
+
+// ---- regular spacing, kernel 4: one block per touched voxel sorts its offers by id and walks them in order -----------
+// The walk is the sequential rule of R21 (accept iff the voxel holds fewer points than its limit and none of them is
+// closer than min_spacing, FP64 d2 of R6, strict <), 32 offers at a time: every lane tests its offer against the stored
+// points; the lowest passing lane is accepted, the lanes after it re-test against that one point, and so on.  Segments
+// longer than the sort buffer are cut into id ranges (halved until they fit).
+constexpr int SP_THREADS = 128;
+constexpr int SP_SORT = 4096;        // offers sorted at a time
+__global__ void __launch_bounds__(SP_THREADS) spaced_commit_kernel(MapView m, const float* __restrict__ xyz, int64_t n_chunk, int stride,
+                                                                   int pose_mode, Pose hpose, const Pose* __restrict__ d_pose,
+                                                                   uint32_t id_offset, const uint32_t* __restrict__ touched,
+                                                                   uint32_t* __restrict__ cov_list, int64_t n_call,
+                                                                   const int64_t* __restrict__ d_n, int last_chunk,
+                                                                   far_insert_stats_t* __restrict__ d_stats, Asmd asmd, Spaced sp) {
+    __shared__ uint32_t s_buf[SP_SORT];
+    __shared__ float4 s_pts[64];
+    __shared__ uint32_t s_acc[64];       // positions accepted in this voxel (for the covariance queue)
+    __shared__ uint32_t s_count, s_n, s_nacc;
+    const Pose& T = (pose_mode == 2) ? *d_pose : hpose;
+    Counters* ctr = m.ctr;
+    if (d_n) { n_call = min(n_call, *d_n); n_chunk = min(n_chunk, *d_n); }
+    const uint32_t first_id = (uint32_t)ctr->next_id + id_offset;
+    const uint32_t n_touched = ctr->n_touched;
+    const uint32_t cap = (uint32_t)m.cap;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    for (uint32_t t = blockIdx.x; t < n_touched; t += gridDim.x) {
+        const uint32_t s = touched[t];
+        const Entry e = m.table[s];
+        const uint32_t b = e.bucket, c0 = entry_count(e.cr);
+        int k[3];
+        unpack_key(e.key, k);
+        const uint32_t limit = voxel_limit(m, asmd, k, pose_mode, T);
+        const uint32_t seg0 = sp.seg_start[t], L = sp.seg_start[t + 1] - seg0;
+        __syncthreads();
+        if (threadIdx.x < c0) s_pts[threadIdx.x] = m.points[(size_t)b * cap + threadIdx.x];
+        if (threadIdx.x == 0) { s_count = c0; s_nacc = 0; }
+        __syncthreads();
+        // id ranges [lo, hi) of point indices, each holding at most SP_SORT of the voxel's offers
+        uint32_t lo = 0;
+        while (lo < (uint32_t)n_chunk && s_count < limit) {
+            uint32_t hi = (uint32_t)n_chunk;
+            for (;;) {
+                if (threadIdx.x == 0) s_n = 0;
+                __syncthreads();
+                uint32_t mine = 0;
+                for (uint32_t j = threadIdx.x; j < L; j += SP_THREADS) { const uint32_t v = sp.seg[seg0 + j]; mine += (v >= lo && v < hi); }
+                mine = __reduce_add_sync(FULL, mine);
+                if (lane == 0 && mine) atomicAdd(&s_n, mine);
+                __syncthreads();
+                const uint32_t cnt = s_n;
+                __syncthreads();
+                if (cnt <= SP_SORT) break;
+                hi = lo + (hi - lo) / 2;                      // cnt > SP_SORT >= 1 distinct indices: the range can be halved
+            }
+            // gather the range, pad to a power of two, bitonic sort ascending
+            if (threadIdx.x == 0) s_n = 0;
+            __syncthreads();
+            for (uint32_t j = threadIdx.x; j < L; j += SP_THREADS) {
+                const uint32_t v = sp.seg[seg0 + j];
+                if (v >= lo && v < hi) s_buf[atomicAdd(&s_n, 1u)] = v;
+            }
+            __syncthreads();
+            const uint32_t cnt = s_n;
+            uint32_t np2 = 32;
+            while (np2 < cnt) np2 <<= 1;
+            for (uint32_t j = cnt + threadIdx.x; j < np2; j += SP_THREADS) s_buf[j] = NO_ID;
+            __syncthreads();
+            for (uint32_t kk = 2; kk <= np2; kk <<= 1) {
+                for (uint32_t jj = kk >> 1; jj > 0; jj >>= 1) {
+                    for (uint32_t idx = threadIdx.x; idx < np2; idx += SP_THREADS) {
+                        const uint32_t ixj = idx ^ jj;
+                        if (ixj > idx) {
+                            const uint32_t a = s_buf[idx], c = s_buf[ixj];
+                            const bool up = (idx & kk) == 0;
+                            if ((a > c) == up) { s_buf[idx] = c; s_buf[ixj] = a; }
+                        }
+                    }
+                    __syncthreads();
+                }
+            }
+            // the walk, by warp 0
+            if (wid == 0) {
+                uint32_t count = s_count, nacc = s_nacc;
+                for (uint32_t base = 0; base < cnt && count < limit; base += 32) {
+                    const uint32_t i = base + lane < cnt ? s_buf[base + lane] : NO_ID;
+                    float p[3] = {0.f, 0.f, 0.f};
+                    bool pass = false;
+                    if (i != NO_ID) {
+                        load_pose_point(xyz, (int64_t)i, stride, pose_mode, T, p);     // valid: it has a key
+                        pass = true;
+                        for (uint32_t j = 0; j < count; ++j) {
+                            const float4 q = s_pts[j];
+                            if (dist2(p[0], p[1], p[2], q.x, q.y, q.z) < sp.s2) { pass = false; break; }
+                        }
+                    }
+                    unsigned pm = __ballot_sync(FULL, pass);
+                    while (pm && count < limit) {
+                        const int w = __ffs(pm) - 1;                                   // lowest id that still passes: accepted
+                        const float ax = __shfl_sync(FULL, p[0], w), ay = __shfl_sync(FULL, p[1], w), az = __shfl_sync(FULL, p[2], w);
+                        if (lane == w) {
+                            const uint32_t id = first_id + i;
+                            const float4 np = make_float4(p[0], p[1], p[2], __uint_as_float(id));
+                            s_pts[count] = np;
+                            m.points[(size_t)b * cap + count] = np;
+                            m.ids[(size_t)b * cap + count] = id;
+                            if (m.cov_ok) m.cov_ok[(size_t)b * cap + count] = 0;
+                            s_acc[nacc] = count;
+                            pass = false;
+                        }
+                        ++count; ++nacc;
+                        if (pass && lane > w && dist2(p[0], p[1], p[2], ax, ay, az) < sp.s2) pass = false;
+                        __syncwarp();
+                        pm = __ballot_sync(FULL, pass) & ~((2u << w) - 1u);            // lanes after w that still pass
+                    }
+                }
+                if (lane == 0) { s_count = count; s_nacc = nacc; }
+            }
+            __syncthreads();
+            lo = hi;
+        }
+        // the voxel's new count, its accepted points into the covariance queue, the statistics
+        const uint32_t nacc = s_nacc;
+        if (threadIdx.x == 0) {
+            m.table[s].cr = (e.cr & ~0xFFu) | s_count;
+            if (nacc) atomicAdd(&ctr->st_accepted, (unsigned long long)nacc);
+            if (cov_list != nullptr && nacc) s_n = atomicAdd(&ctr->n_cov, nacc);
+        }
+        __syncthreads();
+        if (cov_list != nullptr && threadIdx.x < nacc) cov_list[s_n + threadIdx.x] = b * cap + s_acc[threadIdx.x];
+    }
+    insert_epilogue(m, n_call, last_chunk, d_stats);
 }
 
 // ---- A5 prune (R5): thread per slot, FP64 squared centre distance, strict > -------------------
@@ -716,6 +932,7 @@ int far_map_create(far_map_t** out, const far_map_config_t* cfg) {
     if (c.cov_eps == 0.0) c.cov_eps = 1e-3;
     if (c.max_batch == 0) c.max_batch = 1 << 20;
     if (c.max_batch < 1 || c.max_batch > (1ll << 30)) return FAR_ERR_ARG;
+    if (!(c.min_spacing >= 0.0)) return FAR_ERR_ARG;
     if (c.renumber_every == 0) c.renumber_every = 1ll << 31;
     if (c.renumber_every < 1 || c.renumber_every > (1ll << 31)) return FAR_ERR_ARG;
     uint64_t slots = 16;
@@ -755,6 +972,13 @@ int far_map_create(far_map_t** out, const far_map_config_t* cfg) {
     alloc((void**)&v.ctr, sizeof(Counters));
     alloc((void**)&m->d_touched, (size_t)c.max_batch * sizeof(uint32_t));
     alloc((void**)&m->d_cov_list, (size_t)c.max_batch * sizeof(uint32_t));
+    if (c.min_spacing > 0.0) {            // scratch of the regular-spacing insert (R21)
+        alloc((void**)&m->d_sp_cnt, (size_t)c.max_voxels * sizeof(uint32_t));
+        alloc((void**)&m->d_sp_vt, (size_t)c.max_voxels * sizeof(uint32_t));
+        alloc((void**)&m->d_sp_ptb, (size_t)c.max_batch * sizeof(uint32_t));
+        alloc((void**)&m->d_sp_start, ((size_t)c.max_batch + 1) * sizeof(uint32_t));
+        alloc((void**)&m->d_sp_seg, (size_t)c.max_batch * sizeof(uint32_t));
+    }
     if (e == cudaSuccess) e = cudaHostAlloc((void**)&m->h_mail, sizeof(Mailbox), cudaHostAllocMapped);
     if (e == cudaSuccess) {
         memset((void*)m->h_mail, 0, sizeof(Mailbox));
@@ -775,6 +999,7 @@ int far_map_create(far_map_t** out, const far_map_config_t* cfg) {
     z.min_id = NO_ID;
     FAR_CUDA(cudaMemcpy(v.ctr, &z, sizeof(z), cudaMemcpyHostToDevice));
     if (v.cov_ok) FAR_CUDA(cudaMemset(v.cov_ok, 0, npts));
+    if (m->d_sp_cnt) FAR_CUDA(cudaMemset(m->d_sp_cnt, 0, (size_t)c.max_voxels * sizeof(uint32_t)));
     {
         const int rc = gicp_setup(m);
         if (rc != FAR_OK) { far_map_destroy(m); return rc; }
@@ -790,6 +1015,7 @@ int far_map_destroy(far_map_t* m) {
     cudaFree(m->view.free_list); cudaFree(m->view.cov); cudaFree(m->view.cov_ok);
     cudaFree(m->view.ctr); cudaFree(m->d_touched); cudaFree(m->d_cov_list);
     cudaFree(m->d_gicp_partials);
+    cudaFree(m->d_sp_cnt); cudaFree(m->d_sp_vt); cudaFree(m->d_sp_ptb); cudaFree(m->d_sp_start); cudaFree(m->d_sp_seg);
     if (m->h_mail) cudaFreeHost((void*)m->h_mail);
     delete m;
     return FAR_OK;
@@ -837,6 +1063,13 @@ int far::insert_impl(far_map_t* m, const float* d_xyz, int64_t n, const int64_t*
                      double d_max) {
     Asmd asmd{d_n_close, d_n_close ? d_max : 1.0, d_n_close ? 1 : 0};
     if (d_n && n > m->max_batch) return FAR_ERR_ARG;
+    Spaced sp;
+    memset(&sp, 0, sizeof(sp));
+    if (m->cfg.min_spacing > 0.0) {
+        sp.offer_cnt = m->d_sp_cnt; sp.voxel_t = m->d_sp_vt; sp.pt_bucket = m->d_sp_ptb; sp.seg_start = m->d_sp_start; sp.seg = m->d_sp_seg;
+        sp.s2 = m->cfg.min_spacing * m->cfg.min_spacing;
+        sp.on = 1;
+    }
     if (!m || (!d_xyz && n > 0) || n < 0 || n > 0x7FFFFFFFll || (stride != 3 && stride != 4)) return FAR_ERR_ARG;
     if (compute_cov && !m->view.cov) return FAR_ERR_ARG;
     cudaStream_t st = (cudaStream_t)stream;
@@ -865,7 +1098,17 @@ int far::insert_impl(far_map_t* m, const float* d_xyz, int64_t n, const int64_t*
         const int last = off + nc >= n;
         if (nc > 0)
             FAR_LAUNCH(insert_claim_chain_kernel, grid_for(nc, 256), 256, 0, st, m->view, xyz, nc, d_n, stride, pose_mode, hp,
-                                                                          (const Pose*)d_pose, (uint32_t)off, m->d_touched, asmd);
+                                                                          (const Pose*)d_pose, (uint32_t)off, m->d_touched, asmd, sp);
+        if (sp.on) {
+            // R21: list -> scan -> scatter -> per-voxel sort and sequential walk (closes the chunk like the commit kernel)
+            if (nc > 0) {
+                FAR_LAUNCH(spaced_scan_kernel, 1, 1024, 0, st, m->view, m->d_touched, sp);
+                FAR_LAUNCH(spaced_scatter_kernel, grid_for(nc, 256), 256, 0, st, m->view, nc, d_n, sp);
+            }
+            FAR_LAUNCH(spaced_commit_kernel, nc > 0 ? m->sm_count * 8 : 1, SP_THREADS, 0, st, m->view, xyz, nc, stride, pose_mode, hp,
+                                                               (const Pose*)d_pose, (uint32_t)off, m->d_touched,
+                                                               cov_by_list ? m->d_cov_list : nullptr, n, d_n, last, d_stats, asmd, sp);
+        } else
         FAR_LAUNCH(insert_commit_kernel, nc > 0 ? commit_grid : 1, 256, 0, st, m->view, xyz, stride, pose_mode, hp,
                                                            (const Pose*)d_pose, (uint32_t)off, m->d_touched,
                                                            cov_by_list ? m->d_cov_list : nullptr, n, d_n, last, d_stats);

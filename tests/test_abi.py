@@ -50,8 +50,8 @@ def test_struct_sizes_match_header_layout():
     assert C.sizeof(far.Pose) == 96
     assert C.sizeof(far.GicpOptions) == 32
     assert C.sizeof(far.GicpResult) == 96 + 36 * 8 + 6 * 8 + 8 + 16
-    assert C.sizeof(far.MapConfig) == 56
-    assert C.sizeof(far.FrontendConfig) == 56 + 8 + 8 + 8 + 8 + 32 + 8 + 8 + 8 + 8
+    assert C.sizeof(far.MapConfig) == 64
+    assert C.sizeof(far.FrontendConfig) == 64 + 8 + 8 + 8 + 8 + 32 + 8 + 8 + 8 + 8
     assert C.sizeof(far.Motion) == 96
 
 

@@ -6,6 +6,8 @@ is FP64 on both sides with a different but equivalent evaluation order (series v
 matrix) -> results agree to ~1e-15 relative before the single rounding to fp32, so outputs are identical except
 where that tiny difference straddles an fp32 rounding boundary: at most 1 ulp, on a vanishing fraction of values.
 """
+import math
+
 import numpy as np
 import pytest
 import torch
@@ -216,3 +218,117 @@ def test_frontend_sweep_with_asmd_matches_oracle_chain():
     eo, eg = mo.export(with_cov=True), fe.map.export(with_cov=True)
     _same_contents(eg, eo)
     assert np.array_equal(eg["cov_valid"], eo["cov_valid"])
+
+
+# ---- R21: regular spacing -- contents bit-exact against the oracle's sequential rule ------------------------
+def _spaced_cloud(rng, n):
+    pts = np.concatenate([rng.uniform(-20, 20, size=(n, 3)), rng.normal(0, 0.4, size=(n // 2, 3)) + [3.0, 2.0, 1.0],
+                          rng.normal(0, 0.05, size=(n // 4, 3)) + [-9.0, 7.0, 0.5]]).astype(np.float32)
+    rng.shuffle(pts)
+    return pts
+
+
+def _same_map(g, o):
+    assert np.array_equal(g["keys"], o["keys"]) and np.array_equal(g["counts"], o["counts"])
+    assert np.array_equal(g["ids"], o["ids"])
+    assert np.array_equal(g["xyz"].view(np.uint32), o["xyz"].view(np.uint32))
+
+
+@pytest.mark.parametrize("voxel,cap,s", [(4.0, 40, 4.0 / math.sqrt(40.0)), (1.0, 20, 0.2), (2.0, 64, 0.05), (0.5, 3, 0.3)])
+def test_min_spacing_insert_bit_exact(voxel, cap, s):
+    rng = np.random.default_rng(50)
+    pts = _spaced_cloud(rng, 60_000)
+    mo = oracle.Map(voxel, cap, min_spacing=s)
+    mg = far.Map(voxel, cap, 200_000, min_spacing=s, max_batch=25_000)      # calls are chunked internally
+    T = scenes.pose_from_rpy_t(0.02, -0.01, 0.4, [3.0, -2.0, 0.5])
+    for part, pose in ((pts[:40_000], None), (pts[40_000:90_000], T), (pts[90_000:], None)):
+        assert mg.insert(part, pose=pose) == mo.insert(part, pose=pose)
+    eg, eo = mg.export(), mo.export()
+    _same_map(eg, eo)
+    assert mg.size() == mo.size()
+    # the rule's invariant on the CUDA side: no two stored points of a voxel closer than s
+    for v_i in np.random.default_rng(0).choice(len(eg["keys"]), min(400, len(eg["keys"])), replace=False):
+        c = int(eg["counts"][v_i])
+        if c > 1:
+            P = eg["xyz"][v_i, :c].astype(np.float64)
+            d = np.linalg.norm(P[:, None] - P[None, :], axis=2) + np.eye(c) * 1e9
+            assert d.min() >= s * (1 - 1e-12)
+    # prune + re-insert keeps working on the recycled buckets
+    assert mg.prune([0, 0, 0], 12.0) == mo.prune([0, 0, 0], 12.0)
+    more = _spaced_cloud(rng, 10_000)
+    assert mg.insert(more) == mo.insert(more)
+    _same_map(mg.export(), mo.export())
+    mg.close()
+
+
+def test_min_spacing_one_voxel_offered_more_points_than_the_sort_buffer():
+    """20,000 offers for ONE voxel (sort buffer: 4,096): the id ranges are split; with a tiny spacing the walk goes on to the cap"""
+    rng = np.random.default_rng(51)
+    pts = rng.uniform(0.01, 3.99, size=(20_000, 3)).astype(np.float32)
+    pts[::7] = pts[0]                                                    # exact duplicates: d2 = 0 < s2
+    for s, cap in ((1e-3, 64), (1.5, 64), (0.6, 40)):
+        mo, mg = oracle.Map(4.0, cap, min_spacing=s), far.Map(4.0, cap, 64, min_spacing=s)
+        assert mg.insert(pts) == mo.insert(pts)
+        _same_map(mg.export(), mo.export())
+        mg.close()
+
+
+def test_min_spacing_with_asmd_and_covariances_on_a_lidar_scan_at_the_papers_parameters():
+    """v = 4 m, N_max = 40, s = v / sqrt(N_max) = 0.632 m on a ring-structured scan: contents, ids, covariance flags
+    equal the oracle's; stored points really are >= 0.63 m apart; the plain insert would store clumps of consecutive ring points"""
+    c2 = scenes.c2_single_frame(seed=8, n_map_candidates=60_000, map_radius=60.0, rings=32, azimuths=1024)
+    v, cap, s = 4.0, 40, 4.0 / math.sqrt(40.0)
+    scan, T = c2["scan"], c2["T_gt"]
+    mo = oracle.Map(v, cap, min_spacing=s)
+    mg = far.Map(v, cap, 1 << 14, with_cov=True, min_spacing=s)
+    assert mg.insert(c2["map_points"], compute_cov=True) == mo.insert(c2["map_points"], compute_cov=True)
+    assert mg.insert_asmd(scan, 30.0, 80.0, pose=T, compute_cov=True) == mo.insert_asmd(scan, 30.0, 80.0, pose=T, compute_cov=True)
+    eg, eo = mg.export(with_cov=True), mo.export(with_cov=True)
+    _same_map(eg, eo)
+    assert np.array_equal(eg["cov_valid"], eo["cov_valid"])
+    vmask = eo["cov_valid"].astype(bool)
+    a, b = eg["cov"][vmask].astype(np.float64), eo["cov"][vmask].astype(np.float64)
+    assert (np.linalg.norm(a - b, axis=1) / np.linalg.norm(b, axis=1)).max() < 1e-4
+    dmin = np.inf
+    for v_i in range(len(eg["keys"])):
+        c = int(eg["counts"][v_i])
+        if c > 1:
+            P = eg["xyz"][v_i, :c].astype(np.float64)
+            d = np.linalg.norm(P[:, None] - P[None, :], axis=2) + np.eye(c) * 1e9
+            dmin = min(dmin, d.min())
+    assert dmin >= 0.63
+    plain = oracle.Map(v, cap)
+    plain.insert(scan, pose=T)
+    ep = plain.export()
+    pmin = np.inf
+    for v_i in range(len(ep["keys"])):
+        c = int(ep["counts"][v_i])
+        if c > 1:
+            P = ep["xyz"][v_i, :c].astype(np.float64)
+            pmin = min(pmin, (np.linalg.norm(P[:, None] - P[None, :], axis=2) + np.eye(c) * 1e9).min())
+    assert pmin < 0.1                                  # consecutive ring points, centimetres apart, without the rule
+    mg.close()
+
+
+def test_frontend_with_regular_spacing_matches_oracle_frame():
+    c2 = scenes.c2_single_frame(seed=9, n_map_candidates=80_000, map_radius=50.0, rings=16, azimuths=512)
+    v, cap, s, sigma, scan = 2.0, 40, 2.0 / math.sqrt(40.0), c2["sigma"], c2["scan"]
+    mo = oracle.Map(v, cap, min_spacing=s)
+    mo.insert(c2["map_points"], compute_cov=True)
+    ds_o, _ = oracle.voxelize(scan, 1.0)
+    lo = oracle.Map(v, cap); lo.insert(scan)                              # the scan-local map of Cov-Calc is plain (R8 / R21)
+    cov_o, val_o = lo.knn_cov(ds_o, nthreads=8)
+    o = mo.gicp_register(ds_o, cov_o, val_o, c2["T_init"], sigma, 30, nthreads=8)
+    so = mo.insert(scan, pose=(o["R"], o["t"]), compute_cov=True)
+    mo.prune(o["t"], 40.0)
+    fe = far.Frontend(v, cap, 1 << 15, len(scan), ds_voxel=1.0, prune_radius=40.0, max_iters=30, min_spacing=s)
+    fe.map.insert(c2["map_points"], compute_cov=True)
+    g = fe.process_host(scan, c2["T_init"], sigma)
+    assert g["status"] == 0 and g["iters"] == o["iters"] and g["n_inliers"] == o["n_inliers"]
+    assert np.linalg.norm(g["t"] - o["t"]) < 1e-4
+    assert fe.insert_stats() == so
+    eg, eo = fe.map.export(with_cov=True), mo.export(with_cov=True)
+    assert np.array_equal(eg["keys"], eo["keys"]) and np.array_equal(eg["ids"], eo["ids"])
+    assert np.abs(eg["xyz"] - eo["xyz"]).max() < 1e-5
+    assert np.array_equal(eg["cov_valid"], eo["cov_valid"])
+    fe.close()
