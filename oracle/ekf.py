@@ -60,12 +60,15 @@ def f(x, u, dt, a_b=np.zeros(3), w_b=np.zeros(3)):
     return x + dx * dt
 
 
-def jacobian_f(x, u, dt, eps=1e-6):
+def jacobian_f(x, u, dt, a_b=None, w_b=None, eps=1e-6):
+    """F = d f / d x of the step ACTUALLY taken (Eq. 9 with the bias-corrected inputs where it uses them), by central
+    differences"""
+    kw = {} if a_b is None and w_b is None else dict(a_b=a_b, w_b=w_b)
     F = np.zeros((9, 9))
     for j in range(9):
         d = np.zeros(9)
         d[j] = eps
-        F[:, j] = (f(x + d, u, dt) - f(x - d, u, dt)) / (2 * eps)
+        F[:, j] = (f(x + d, u, dt, **kw) - f(x - d, u, dt, **kw)) / (2 * eps)
     return F
 
 
@@ -101,7 +104,7 @@ class Ekf:
 
     def predict(self, u):
         """one 100 Hz cycle: x_k|k-1 = f(x_k-1, u_k), P = F P F^T + Q; then the pending (up-sampled) corrections"""
-        F = jacobian_f(self.x, u, self.dt)
+        F = jacobian_f(self.x, u, self.dt, self.a_b, self.w_b)
         self.x = f(self.x, u, self.dt, self.a_b, self.w_b)
         self.P = F @ self.P @ F.T + self.Q
         self.k += 1

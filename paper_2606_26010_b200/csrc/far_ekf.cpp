@@ -221,18 +221,20 @@ void far_ekf_destroy(far_ekf_t* e) { delete e; }
 int64_t far_ekf_predict(far_ekf_t* e, const double accel_m[3], const double gyro_m[3]) {
     if (!e || !accel_m || !gyro_m) return -1;
     double F[81], xn[NX], FP[81], Pn[81];
-    // R18: the Jacobian is taken with the raw inputs, the state step with the bias-corrected ones (as the oracle does)
-    model(e->x, accel_m, gyro_m, e->dt, xn, F);
     const double a[3] = {accel_m[0] - e->ab[0], accel_m[1] - e->ab[1], accel_m[2] - e->ab[2]};
     const double w[3] = {gyro_m[0] - e->wb[0], gyro_m[1] - e->wb[1], gyro_m[2] - e->wb[2]};
     {
-        // Eq. 9 prints -[w_m]x v with the measured rate and E(theta)(w_m - w_b), a_m - a_b with the corrected ones
-        double xb[NX];
-        model(e->x, a, w, e->dt, xb, nullptr);
-        double xr[NX];
-        model(e->x, a, gyro_m, e->dt, xr, nullptr);
+        // Eq. 9 prints -[w_m]x v with the measured rate and E(theta)(w_m - w_b), a_m - a_b with the corrected ones (R18).
+        // The Jacobian is that of the step actually taken: its position / attitude rows with the corrected rate, its
+        // velocity rows with the measured one
+        double xb[NX], Fb[81];
+        model(e->x, a, w, e->dt, xb, Fb);
+        double xr[NX], Fr[81];
+        model(e->x, a, gyro_m, e->dt, xr, Fr);
         for (int i = 0; i < 6; ++i) xn[i] = xb[i];
         for (int i = 6; i < 9; ++i) xn[i] = xr[i];
+        std::memcpy(F, Fb, 6 * 9 * sizeof(double));
+        std::memcpy(F + 6 * 9, Fr + 6 * 9, 3 * 9 * sizeof(double));
     }
     for (int i = 0; i < NX; ++i)
         for (int j = 0; j < NX; ++j) {

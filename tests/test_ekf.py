@@ -91,3 +91,35 @@ def test_push_rejects_measurements_outside_the_history():
         g.push_lidar(T, [0, 0, 0], [1.0] * 9, cycle_s=5)          # the future
     with pytest.raises(far.FarError):
         g.push_lidar(T, [0, 0, 0], [0.0] * 9, cycle_s=0)          # non-positive variance
+
+
+def test_covariance_propagates_with_the_jacobian_of_the_step_actually_taken():
+    """Pin independent of the oracle (R18): with non-zero biases, P after one cycle must be F P F^T + Q with F the finite
+    difference of the PRODUCT's own state step (same inputs, perturbed states).  A Jacobian evaluated at the raw gyro rate
+    in the E(theta) w block -- the step uses w_m - w_b there -- fails this."""
+    rng = np.random.default_rng(12)
+    x0 = np.r_[1.0, -2.0, 0.5, 0.05, -0.08, 0.7, 25.0, 0.4, -0.2]
+    P0 = np.r_[[0.2] * 3, [2e-3] * 3, [0.1] * 3]
+    Q = np.r_[[1e-6] * 3, [1e-7] * 3, [1e-4] * 3]
+    ab, wb = np.array([0.3, -0.2, 0.1]), np.array([0.2, -0.3, 0.25])          # large gyro bias: the two Jacobians differ visibly
+    a_m, w_m = np.array([0.5, 1.0, 9.6]), np.array([0.3, 0.2, 0.6])
+    dt = 0.01
+
+    def step(x):
+        e = far.Ekf(x, P0, Q, dt=dt, accel_bias=ab, gyro_bias=wb)
+        e.predict(a_m, w_m)
+        return e.state()
+
+    xn, Pn, _ = step(x0)
+    F = np.zeros((9, 9))
+    h = 1e-6
+    for j in range(9):
+        d = np.zeros(9); d[j] = h
+        F[:, j] = (step(x0 + d)[0] - step(x0 - d)[0]) / (2 * h)
+    want = F @ np.diag(P0) @ F.T + np.diag(Q)
+    assert np.allclose(Pn, want, rtol=1e-6, atol=1e-10)
+    # and it is not the raw-rate Jacobian: that one differs in the attitude block by dt * d(E(theta) w_b)/d(theta)
+    _, F_raw = far.ekf_model(x0, np.r_[a_m, w_m], dt)
+    assert np.abs(F_raw - F).max() > 1e-4
+    # the oracle takes the same Jacobian
+    assert np.allclose(oekf.jacobian_f(x0, np.r_[a_m, w_m], dt, ab, wb), F, atol=1e-7)

@@ -401,3 +401,37 @@ def test_frame_graph_replay_equals_stream_of_launches_and_oracle():
     assert np.array_equal(eb["keys"], eo["keys"]) and np.array_equal(eb["ids"], eo["ids"])
     assert np.abs(eb["xyz"] - eo["xyz"]).max() < 1e-5
     assert np.array_equal(eb["cov_valid"], eo["cov_valid"])
+
+
+def test_ten_thousand_registrations_are_bitwise_reproducible():
+    """The reduction is a fixed-order sum of tagged words (far_gicp.cu): 10,000 back-to-back registrations, two maps
+    alternating (each with its own scratch and launch sequence), no host synchronisation in between -- every
+    far_gicp_result_t must be byte-identical to the first one of its map.  A torn or stale tagged word, a reused tag or a
+    summation order that depends on arrival would show up here."""
+    c1 = scenes.c1_tiny(seed=0)
+    v, cap = c1["voxel"], c1["cap"]
+    maps, scans, poses = [], [], []
+    for j in range(2):
+        m = far.Map(v, cap, 1 << 14, with_cov=True)
+        m.insert(c1["map_points"], compute_cov=True)
+        lm = far.Map(v, cap, 1 << 13)
+        sc = c1["scan"] if j == 0 else c1["scan"][::-1].copy()
+        lm.insert(sc)
+        ds = torch.as_tensor(sc).cuda()
+        cov, val = lm.knn_cov(ds)
+        maps.append(m); scans.append((ds, cov, val))
+        poses.append(c1["T_init"] if j == 0 else scenes.perturb_pose(c1["T_init"], 0.05, 0.5, np.random.default_rng(1)))
+    n_rep = 5000
+    out = torch.zeros((2, n_rep, far.GICP_RESULT_BYTES), dtype=torch.uint8, device="cuda")
+    for r in range(n_rep):
+        for j in range(2):
+            ds, cov, val = scans[j]
+            maps[j].gicp_register_enqueue(ds, cov, val, poses[j], c1["sigma"], 30, d_result=out[j, r])
+    torch.cuda.synchronize()
+    h = out.cpu().numpy()
+    for j in range(2):
+        first = far.result_to_dict(far.GicpResult.from_buffer_copy(h[j, 0].tobytes()))
+        assert first["status"] == 0 and first["iters"] > 3
+        assert (h[j] == h[j, 0]).all(), np.nonzero((h[j] != h[j, 0]).any(axis=1))[0][:5]
+    for m in maps:
+        m.close()
