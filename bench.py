@@ -203,6 +203,17 @@ def algorithmic_bytes(kernel, units, cand=0.0, occ=0.0, n_slots=0, n_removed=0):
     return None
 
 
+def _hbm_peak():
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    if "hbm_gbs" in peaks:
+        return float(peaks["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback 6650 GB/s (B200_PROFILING.md)"
+
+
 def _ev_ms(torch, fn):
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     a.record(); fn(); b.record(); torch.cuda.synchronize()
@@ -286,14 +297,14 @@ def _leg_c4(out, far, scenes, torch, peak):
     mg.close(); del pts
 
 
-def _leg_c5(out, far, scenes, torch, peak, flush):
+def _leg_c5(out, far, scenes, torch, peak, flush, voxels=(0.25, 0.5, 1.0, 2.0)):
     # ---- C5: 1 M queries against a 20 M-point map at four voxel sizes, random and Morton order -------------------
     c5 = scenes.c5_nn_sweep(seed=4)
     d_pts = torch.as_tensor(c5["map_points"]).cuda()
     ids = torch.empty(1_000_000, dtype=torch.int32, device="cuda")
     d2 = torch.empty(1_000_000, dtype=torch.float32, device="cuda")
     out["c5_nn"] = {}
-    for v in (0.25, 0.5, 1.0, 2.0):
+    for v in voxels:
         mg = far.Map(v, 20, 20_000_000 if v <= 0.5 else 4_000_000, with_cov=False, max_batch=1 << 22)
         t_build = _ev_ms(torch, lambda: mg.insert_enqueue(d_pts))
         st = mg.stats()
@@ -313,6 +324,26 @@ def _leg_c5(out, far, scenes, torch, peak, flush):
         out["c5_nn"][f"v={v}"] = row
         mg.close()
     del d_pts
+
+
+def _leg_voxelize(out, far, torch, peak, flush, up=None):
+    # scan downsampling (A2): 8 M points in a 300 m cube at v = 1 m
+    nu = 8_000_000
+    if up is None:
+        gen = torch.Generator(device="cuda").manual_seed(0)
+        up = (torch.rand((nu, 3), device="cuda", generator=gen) - 0.5) * 300.0
+    vz = far.Voxelizer(nu)
+    ts = []
+    for i in range(8):
+        flush.fill_(i)
+        ts.append(_ev_ms(torch, lambda: vz.enqueue(up, 1.0)))
+    t_v = float(np.median(ts[3:])) * 1e-3
+    n_out = int(vz.n_out.item())
+    vbytes = nu * 20 + n_out * 16
+    out["voxelize"] = {"points": nu, "voxels_out": n_out, "points_per_s": nu / t_v, "ms": t_v * 1e3,
+                       "algorithmic_GBps": vbytes / t_v / 1e9, "frac_of_hbm_peak": vbytes / t_v / 1e9 / peak,
+                       "note": "worst case: 8 M points uniform in a 300 m cube at v = 1 m, nearly every point opens its own voxel (random scatter into a 2^24-slot scratch table); 20 B per point + 16 B per output (SURVEY 8d)"}
+    del vz
 
 
 def _leg_c3(out, far, scenes, torch):
@@ -394,6 +425,30 @@ def run_far(args):
         dist.init_process_group("nccl")
     far.lib()
     K, W = args.steps, args.warmup
+
+    if args.legs:
+        # only the named legs, nothing else: what the `ncu --set full -k <kernel>` captures under profiles/ are taken on
+        # (the map is far larger than L2 there); prints {"legs": {...}}, not a bench line
+        peak = _hbm_peak()[0]
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+        out = {}
+        for leg in args.legs.split(","):
+            if leg == "c4":
+                _leg_c4(out, far, scenes, torch, peak)
+            elif leg.startswith("c5"):
+                vox = tuple(float(x) for x in leg.split(":")[1].split("/")) if ":" in leg else (0.25, 0.5, 1.0, 2.0)
+                _leg_c5(out, far, scenes, torch, peak, flush, vox)
+            elif leg == "voxelize":
+                _leg_voxelize(out, far, torch, peak, flush)
+            elif leg == "c3":
+                _leg_c3(out, far, scenes, torch)
+            elif leg == "c2p":
+                _leg_c2_paper_params(out, far, scenes, torch)
+            else:
+                raise SystemExit(f"unknown leg {leg!r}")
+        if rank == 0:
+            print(json.dumps({"legs": out}))
+        return
 
     c2 = load_workload(args.workload)
     scan, v, cap, sigma = c2["scan"], c2["voxel"], c2["cap"], c2["sigma"]
@@ -507,13 +562,7 @@ def run_far(args):
              "insert_claim_chain_kernel": 2 * len(scan), "insert_commit_kernel": accepted + int(local_stats["n_accepted"]),
              "vox_claim_kernel": len(scan)}
     cand = {"gicp_kernel": (cand_gicp, occ_gicp), "knn_cov_refs_kernel": (cand_refs, occ_refs), "knn_cov_points_kernel": (cand_pts, occ_pts)}
-    peaks = {}
-    try:
-        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
-    except Exception:
-        pass
-    peak = float(peaks.get("hbm_gbs", 6650.0))
-    peak_kind = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
+    peak, peak_kind = _hbm_peak()
     # per-kernel facts from the committed `ncu --set full` captures (never measured live: a number taken under a profiler
     # is not a bench value): DRAM bytes per launch, issue-slot utilisation, what bounds the kernel
     try:
@@ -614,21 +663,8 @@ def run_far(args):
         extras["undistort"] = {"points": nu, "points_per_s": nu / t_u, "ms": t_u * 1e3, "algorithmic_GBps": nu * 28 / t_u / 1e9,
                                "frac_of_hbm_peak": nu * 28 / t_u / 1e9 / peak,
                                "note": "8 M points in one call (224 MB > L2), FP64 arithmetic, 256 MB flush between repetitions"}
-        # scan downsampling (A2) at the same size: 8 M points in a 300 m cube at v = 1 m
-        vz = far.Voxelizer(nu)
-        ts = []
-        for i in range(8):
-            flush.fill_(i)
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(); vz.enqueue(up, 1.0); b.record(); torch.cuda.synchronize()
-            ts.append(a.elapsed_time(b))
-        t_v = float(np.median(ts[3:])) * 1e-3
-        n_out = int(vz.n_out.item())
-        vbytes = nu * 20 + n_out * 16
-        extras["voxelize"] = {"points": nu, "voxels_out": n_out, "points_per_s": nu / t_v, "ms": t_v * 1e3,
-                              "algorithmic_GBps": vbytes / t_v / 1e9, "frac_of_hbm_peak": vbytes / t_v / 1e9 / peak,
-                              "note": "worst case: 8 M points uniform in a 300 m cube at v = 1 m, nearly every point opens its own voxel (random scatter into a 2^24-slot scratch table); 20 B per point + 16 B per output (SURVEY 8d)"}
-        del up, ut, uo, vz
+        _leg_voxelize(extras, far, torch, peak, flush, up)
+        del up, ut, uo
 
         # BASELINE.json's other throughput metrics at the full sizes of configs[3] and configs[4]: hash insert and NN queries
         flush.fill_(0)
@@ -698,6 +734,7 @@ def main():
     ap.add_argument("--no-extras", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--full-extras", action="store_true", help="also time C3/C4/C5 at full size (minutes)")
+    ap.add_argument("--legs", default="", help="run ONLY these legs (c4, c5[:v/v..], voxelize, c3, c2p) and print {'legs': ...}: for ncu captures")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
