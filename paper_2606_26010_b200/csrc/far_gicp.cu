@@ -9,25 +9,33 @@
 // accumulated in FP64 and always applied to the ORIGINAL scan; stop on ||delta||_2; max_iters replaces the
 // wall-clock limit.
 //
-// B200 design: a registration is a few thousand source points, i.e. latency- and issue-bound, never bandwidth-
-// bound, so the whole Gauss-Newton loop is ONE persistent cooperative kernel and every iteration is organised to
-// keep both the instruction count and the serial chain short:
-//   phase A  one warp per source point, no block barrier before it: the warp transforms its point itself (FP64), and
-//            what the previous iteration learnt stays in registers -- the source point and its covariance, the 27 table
-//            lookups (valid as long as the transformed point stays in its voxel: the map does not change during a
+// B200 design: a registration is a few thousand source points, i.e. latency- and issue-bound, never bandwidth-bound, so
+// the whole Gauss-Newton loop is ONE persistent cooperative kernel and an iteration is organised to keep both the
+// instruction count per scheduler and the serial chain short (round 2 profile: with a warp per point, 10 warps per
+// scheduler each issued ~950 instructions per iteration -- 5-7 us -- and seven warps of a block waited at a barrier
+// while 8 lanes of the eighth linearised):
+//   groups   EIGHT LANES per source point, four points per warp; points are dealt round-robin over the blocks of the
+//            grid (two 512-thread blocks per SM), so a 5,000-point scan puts ~2.5 busy warps on a scheduler instead of 10
+//            and the per-point scalar work (transform, voxel index, bounds) is issued once per 4 points;
+//   search   what the previous iteration learnt stays with the group: the 27 table lookups (lane g keeps neighbours g,
+//            g + 8, g + 16, g + 24; valid while the transformed point stays in its voxel: the map does not change during a
 //            registration) and the previous nearest neighbour, whose distance to the new position bounds the search: a
-//            neighbour voxel is read only if its distance lower bound does not exceed it (exact, ties included).  From
-//            the second iteration on a search is usually one sweep over the point's own voxel, served by L1;
-//   phase B  the block's 8 correspondences are linearised by 8 lanes of warp 0 at once (one FP64 instruction stream for
-//            8 points: the FP64 pipe, not the issue slots, is what a per-warp linearisation would exhaust), column by
-//            column so that the live set fits the 48 registers five co-resident blocks per SM leave;
-//   reduce   the 29 unique terms of (H, b, chi2, n) go block -> group of 32 blocks -> grid as TAGGED rows: every
-//            value travels as two 8-byte words {value half, tag} (tag = launch sequence and iteration), so a consumer
-//            just polls the rows it needs -- no fence, no ticket atomics -- and sums them in a fixed order
-//            (deterministic, no floating-point atomics);
-//   solve    warp 0 of block 0: 6x6 Cholesky with one row per lane (shuffles, no local memory), SE(3) exponential by
-//            series, pose update and stop test in FP64; thirteen lanes publish one tagged word each; one lane per block
-//            polls the `done` word with a short back-off, then twelve lanes fetch the pose.
+//            neighbour voxel is read only if its distance lower bound does not exceed it (exact, ties included).  From the
+//            second iteration on a search is usually one sweep over the point's own voxel, served by L1;
+//   A9       every group linearises its own correspondence at once -- no block barrier, no serial section: the six
+//            entries of Sigma_r + R Sigma_s R^T one per lane, M = S^-1, M d and the weight in every lane, and the 29
+//            terms of (H, b, chi2, n) as ONE uniform expression  coef (u[a] u[b] - u[c] u[d])  over a small vector u
+//            = (M, M d, p, 0, 1, e2, X) in shared memory with a constant index table (four terms per lane), so the
+//            lanes do not diverge;
+//   reduce   lane-wise across the 4 groups of a warp (shuffles), across the warps of the block (shared memory), then
+//            block -> group of 16 blocks -> grid as TAGGED rows: every value travels as two 8-byte words {value half,
+//            tag} (tag = launch sequence and iteration), so a consumer just polls the rows it needs -- no fence, no
+//            ticket atomics -- and sums them in a fixed order (deterministic, no floating-point atomics);
+//   solve    warp 0 of block 0: 6x6 Gauss-Jordan on [H | -b] with one row per lane (pivots = those of Cholesky, so
+//            "not positive definite" is detected identically; six reciprocals are the serial chain, no square roots, no
+//            substitution passes), SE(3) exponential by series, pose update and stop test in FP64; thirteen lanes publish
+//            one tagged word each; one lane per block polls the `done` word with a short back-off, then twelve lanes
+//            fetch the pose.
 // The host is not involved until it reads the result.
 //
 // Tagged words and the PTX memory model: a word is written with st.relaxed.gpu.v2.u64 and read with ld.relaxed.gpu.v2.u64.
@@ -42,31 +50,26 @@ using namespace far;
 
 namespace far {
 
-constexpr int GWARPS = 8;        // warps per block = correspondences linearised together in phase B
-constexpr int NTERMS = 29;       // 21 (H upper triangle) + 6 (b) + chi2 + inlier count
-constexpr int TSTRIDE = 32;      // row length of the tagged rows in global memory
-constexpr int SSTRIDE = 33;      // row length of the per-correspondence term rows in shared memory (no bank conflicts)
-
-constexpr int GROUP = 32;        // blocks per first-level reduction group
+constexpr int GLANES = 16;                // lanes per source point (8 or 16)
+constexpr int GWARPS = 20;                // warps per block
+constexpr int GTHREADS = GWARPS * 32;
+constexpr int GPTS = GTHREADS / GLANES;   // source points per block and round
+constexpr int NBR_PER_LANE = (27 + GLANES - 1) / GLANES;   // neighbour voxels a lane looks after: l = g + GLANES j
+constexpr int SWEEP_U = 32 / GLANES;                      // candidate loads in flight per lane: 32 per group and round trip
+constexpr int TERM_SLOTS = (24 + GLANES - 1) / GLANES + 1;               // term columns per lane: entries g, g + GLANES, .. < 24, then 24 + g
+constexpr int GICP_BLOCKS_PER_SM = 1;
+constexpr int NTERMS = 29;                // 21 (H upper triangle) + 6 (b) + chi2 + inlier count
+constexpr int TSTRIDE = 32;               // row length of the tagged rows in global memory
+constexpr int GROUP = 16;                 // blocks per first-level reduction group
 constexpr int MAX_GROUPS = 64;
-constexpr int GICP_BLOCKS_PER_SM = 5;
-constexpr int NPUB = 13;         // published words: R[9], t[3], done
-constexpr int MAX_ITERS_LIMIT = 1000;   // the iteration index shares the 32-bit tag with the launch sequence
+constexpr int NPUB = 13;                  // published words: R[9], t[3], done
+constexpr int MAX_ITERS_LIMIT = 1000;     // the iteration index shares the 32-bit tag with the launch sequence
 
 // device scratch of one map: [max_grid] block rows, [MAX_GROUPS] group rows, the published pose
 struct GicpScratch {
     uint4* rows;      // [max_grid][TSTRIDE]
     uint4* grows;     // [MAX_GROUPS][TSTRIDE]
     uint4* pub;       // [16]: 13 published words; pub[15].x = launch sequence of this map (device-resident)
-};
-
-// one correspondence, written by its warp in phase A, read by one lane of warp 0 in phase B
-struct Corr {
-    float p[3];       // transformed source point
-    float r[3];       // its nearest map point
-    float cs[6];      // Sigma_s
-    float cr[6];      // Sigma_r
-    int flags;        // bit 0: correspondence accepted, bit 1: both covariances valid
 };
 
 struct GicpParams {
@@ -82,6 +85,7 @@ struct GicpParams {
     const double* d_sigma;      // nullable: tau2 = (tau_mult sigma)^2 and kappa = sigma / kappa_div from the DEVICE value
     double tau_mult, kappa_div;
     int kernel, max_iters, linearize_only;
+    int sm_count;
     GicpScratch scratch;
     far_gicp_result_t* out;
 };
@@ -127,186 +131,76 @@ __device__ __forceinline__ bool inv_sym3(const double a[6], double o[6]) {
     return true;
 }
 
-// A9 for one correspondence: the 29 terms, written straight into the correspondence's row of shared memory.  Ordered so
-// that few values are live at a time: S row by row -> M -> (M, Md, w) -> one column of X = M [p]x and of Y = [p]x^T X at
-// a time.  H = w J^T M J with J = [-I | A], A = [p]x:  [[M, -X], [-X^T, Y]];  b = w J^T M d = w [-Md ; A^T Md].
-__device__ __forceinline__ void correspondence_terms(const Pose& T, const Corr& c, int kernel, double kappa, double* terms) {
-    const double px = (double)c.p[0], py = (double)c.p[1], pz = (double)c.p[2];
-    const double d0 = (double)c.r[0] - px, d1 = (double)c.r[1] - py, d2 = (double)c.r[2] - pz;   // Eq. 3
-    double M[6] = {1.0, 0.0, 0.0, 1.0, 0.0, 1.0};                        // SA fallback: Sigma_r = I, Sigma_s = 0
-    if (c.flags & 2) {
-        // S = Sigma_r + R Sigma_s R^T   (Eq. 4): row i of R Sigma_s, then its products with rows j >= i of R
-        const double s0 = c.cs[0], s1 = c.cs[1], s2 = c.cs[2], s3 = c.cs[3], s4 = c.cs[4], s5 = c.cs[5];
-        double S[6];
-        {
-            const double a = T.R[0], b = T.R[1], e = T.R[2];
-            const double u0 = a * s0 + b * s1 + e * s2, u1 = a * s1 + b * s3 + e * s4, u2 = a * s2 + b * s4 + e * s5;
-            S[0] = (double)c.cr[0] + (u0 * T.R[0] + u1 * T.R[1] + u2 * T.R[2]);
-            S[1] = (double)c.cr[1] + (u0 * T.R[3] + u1 * T.R[4] + u2 * T.R[5]);
-            S[2] = (double)c.cr[2] + (u0 * T.R[6] + u1 * T.R[7] + u2 * T.R[8]);
-        }
-        {
-            const double a = T.R[3], b = T.R[4], e = T.R[5];
-            const double u0 = a * s0 + b * s1 + e * s2, u1 = a * s1 + b * s3 + e * s4, u2 = a * s2 + b * s4 + e * s5;
-            S[3] = (double)c.cr[3] + (u0 * T.R[3] + u1 * T.R[4] + u2 * T.R[5]);
-            S[4] = (double)c.cr[4] + (u0 * T.R[6] + u1 * T.R[7] + u2 * T.R[8]);
-        }
-        {
-            const double a = T.R[6], b = T.R[7], e = T.R[8];
-            const double u0 = a * s0 + b * s1 + e * s2, u1 = a * s1 + b * s3 + e * s4, u2 = a * s2 + b * s4 + e * s5;
-            S[5] = (double)c.cr[5] + (u0 * T.R[6] + u1 * T.R[7] + u2 * T.R[8]);
-        }
-        double Mi[6];
-        if (inv_sym3(S, Mi)) {
-#pragma unroll
-            for (int a = 0; a < 6; ++a) M[a] = Mi[a];
-        }
+// ---- A9 as one uniform expression ---------------------------------------------------------------------------------------
+// H = w J^T M J with J = [-I | A], A = [p]x:  [[M, -X], [-X^T, Y]], X = M A, Y = A^T X;  b = w J^T M d = w [-Md ; A^T Md].
+// Every one of the 29 terms is coef * (u[a] u[b] - u[c] u[d]) over the group's vector
+//   u = (M0..M5 | Md0..Md2 | px py pz | 0 | 1 | e2 | X00 X01 X02 X10 .. X22)          (24 doubles in shared memory)
+// with coef in {+w, -w, 1}.  Lane g of a group evaluates entries g, 8 + g, 16 + g of the first round (the nine X, which it
+// also stores into u, the six M, -Md, A^T Md, chi2, n) and entry g of the second (the six Y, which need X).  An entry packs
+// a | b << 5 | c << 10 | d << 15 | coef << 20 | (1 + X index) << 22; c_term_store maps the entry to its column in the
+// 29-term row (H upper triangle row-wise, b, chi2, n).
+constexpr int U_MD = 6, U_P = 9, U_ZERO = 12, U_ONE = 13, U_E2 = 14, U_X = 15, U_LEN = 24;
+constexpr uint32_t term_enc(int a, int b, int c, int d, int coef, int xs) {
+    return (uint32_t)a | ((uint32_t)b << 5) | ((uint32_t)c << 10) | ((uint32_t)d << 15) | ((uint32_t)coef << 20) | ((uint32_t)xs << 22);
+}
+constexpr int sym3(int r, int c) { return r == c ? (r == 0 ? 0 : (r == 1 ? 3 : 5)) : (r + c == 1 ? 1 : (r + c == 2 ? 2 : 4)); }
+constexpr int COEF_W = 0, COEF_MW = 1, COEF_ONE = 2;
+// X[r][0] = M[r][1] pz - M[r][2] py;  X[r][1] = M[r][2] px - M[r][0] pz;  X[r][2] = M[r][0] py - M[r][1] px
+constexpr uint32_t x_enc(int r, int c) {
+    return c == 0 ? term_enc(sym3(r, 1), U_P + 2, sym3(r, 2), U_P + 1, COEF_MW, 1 + 3 * r + c)
+         : c == 1 ? term_enc(sym3(r, 2), U_P + 0, sym3(r, 0), U_P + 2, COEF_MW, 1 + 3 * r + c)
+                  : term_enc(sym3(r, 0), U_P + 1, sym3(r, 1), U_P + 0, COEF_MW, 1 + 3 * r + c);
+}
+constexpr uint32_t plain_enc(int a, int coef) { return term_enc(a, U_ONE, U_ZERO, U_ZERO, coef, 0); }
+constexpr int XI(int r, int c) { return U_X + 3 * r + c; }
+__constant__ uint32_t c_term_enc[32] = {
+    // round 1, slot 0
+    x_enc(0, 0), x_enc(0, 1), x_enc(0, 2), x_enc(1, 0), x_enc(1, 1), x_enc(1, 2), x_enc(2, 0), x_enc(2, 1),
+    // slot 1
+    x_enc(2, 2), plain_enc(0, COEF_W), plain_enc(1, COEF_W), plain_enc(2, COEF_W), plain_enc(3, COEF_W), plain_enc(4, COEF_W),
+    plain_enc(5, COEF_W), plain_enc(U_MD + 0, COEF_MW),
+    // slot 2:  b_phi = w A^T Md = w (pz Md1 - py Md2, px Md2 - pz Md0, py Md0 - px Md1)
+    plain_enc(U_MD + 1, COEF_MW), plain_enc(U_MD + 2, COEF_MW),
+    term_enc(U_P + 2, U_MD + 1, U_P + 1, U_MD + 2, COEF_W, 0), term_enc(U_P + 0, U_MD + 2, U_P + 2, U_MD + 0, COEF_W, 0),
+    term_enc(U_P + 1, U_MD + 0, U_P + 0, U_MD + 1, COEF_W, 0), plain_enc(U_E2, COEF_W), plain_enc(U_ONE, COEF_ONE),
+    term_enc(U_ZERO, U_ZERO, U_ZERO, U_ZERO, COEF_ONE, 0),
+    // round 2 (slot 3):  Y[0][j] = pz X[1][j] - py X[2][j];  Y[1][j] = px X[2][j] - pz X[0][j];  Y[2][j] = py X[0][j] - px X[1][j]
+    term_enc(U_P + 2, XI(1, 0), U_P + 1, XI(2, 0), COEF_W, 0), term_enc(U_P + 2, XI(1, 1), U_P + 1, XI(2, 1), COEF_W, 0),
+    term_enc(U_P + 2, XI(1, 2), U_P + 1, XI(2, 2), COEF_W, 0), term_enc(U_P + 0, XI(2, 1), U_P + 2, XI(0, 1), COEF_W, 0),
+    term_enc(U_P + 0, XI(2, 2), U_P + 2, XI(0, 2), COEF_W, 0), term_enc(U_P + 1, XI(0, 2), U_P + 0, XI(1, 2), COEF_W, 0),
+    term_enc(U_ZERO, U_ZERO, U_ZERO, U_ZERO, COEF_ONE, 0), term_enc(U_ZERO, U_ZERO, U_ZERO, U_ZERO, COEF_ONE, 0)};
+__constant__ uint8_t c_term_store[32] = {
+    3, 4, 5, 8, 9, 10, 12, 13,
+    14, 0, 1, 2, 6, 7, 11, 21,
+    22, 23, 24, 25, 26, 27, 28, 29,
+    15, 16, 17, 18, 19, 20, 30, 31};
+
+// group-wide arg-min over (d2, id) (lanes of `gmask`): returns the warp lane holding the winner
+__device__ __forceinline__ int group_argmin(unsigned gmask, double d2, uint32_t id) {
+    const unsigned long long bits = (unsigned long long)__double_as_longlong(d2);
+    const uint32_t hi = (uint32_t)(bits >> 32), lo = (uint32_t)bits;
+    const uint32_t mhi = __reduce_min_sync(gmask, hi);
+    bool c = hi == mhi;
+    const uint32_t mlo = __reduce_min_sync(gmask, c ? lo : 0xFFFFFFFFu);
+    c = c && lo == mlo;
+    unsigned b = __ballot_sync(gmask, c);
+    if (b & (b - 1)) {      // more than one lane holds the minimal d2: lowest id wins (R6)
+        const uint32_t mid = __reduce_min_sync(gmask, c ? id : 0xFFFFFFFFu);
+        c = c && id == mid;
+        b = __ballot_sync(gmask, c);
     }
-    const double Md0 = M[0] * d0 + M[1] * d1 + M[2] * d2;
-    const double Md1 = M[1] * d0 + M[3] * d1 + M[4] * d2;
-    const double Md2 = M[2] * d0 + M[4] * d1 + M[5] * d2;
-    const double e2 = d0 * Md0 + d1 * Md1 + d2 * Md2;
-    const double w = robust_weight(kernel, e2, kappa);
-    terms[0] = w * M[0];  terms[1] = w * M[1];  terms[2] = w * M[2];
-    terms[6] = w * M[3];  terms[7] = w * M[4];  terms[11] = w * M[5];
-    terms[21] = -w * Md0; terms[22] = -w * Md1; terms[23] = -w * Md2;
-    terms[24] = w * (pz * Md1 - py * Md2);
-    terms[25] = w * (px * Md2 - pz * Md0);
-    terms[26] = w * (py * Md0 - px * Md1);
-    terms[27] = w * e2;
-    terms[28] = 1.0;
-    // column 0 of X = M A:  X[r][0] = M[r][1] pz - M[r][2] py;   Y[i][0] = (A^T X)[i][0]
-    {
-        const double x0 = M[1] * pz - M[2] * py, x1 = M[3] * pz - M[4] * py, x2 = M[4] * pz - M[5] * py;
-        terms[3] = -w * x0; terms[8] = -w * x1; terms[12] = -w * x2;
-        terms[15] = w * (pz * x1 - py * x2);                               // Y00
-    }
-    // column 1:  X[r][1] = M[r][2] px - M[r][0] pz
-    {
-        const double x0 = M[2] * px - M[0] * pz, x1 = M[4] * px - M[1] * pz, x2 = M[5] * px - M[2] * pz;
-        terms[4] = -w * x0; terms[9] = -w * x1; terms[13] = -w * x2;
-        terms[16] = w * (pz * x1 - py * x2);                               // Y01
-        terms[18] = w * (px * x2 - pz * x0);                               // Y11
-    }
-    // column 2:  X[r][2] = M[r][0] py - M[r][1] px
-    {
-        const double x0 = M[0] * py - M[1] * px, x1 = M[1] * py - M[3] * px, x2 = M[2] * py - M[4] * px;
-        terms[5] = -w * x0; terms[10] = -w * x1; terms[14] = -w * x2;
-        terms[17] = w * (pz * x1 - py * x2);                               // Y02
-        terms[19] = w * (px * x2 - pz * x0);                               // Y12
-        terms[20] = w * (py * x0 - px * x1);                               // Y22
-    }
+    return __ffs(b) - 1;
 }
 
-// A6 with what earlier iterations learnt: `cnt` / `bucket` are the warp's 27 lookups for voxel k (lane l < 27), `bound0`
-// an upper bound of the answer's d2 (+inf if none): the distance to a stored point that lies in the 27 voxels.  A voxel is
-// read only if its distance lower bound does not exceed the bound; without a bound the point's own voxel is swept first
-// to get one.  Exactly the (d2, id) minimum of R6: a skipped voxel holds only points strictly farther than the bound.
-__device__ __forceinline__ Best nearest_bounded(const MapView& m, float qx, float qy, float qz, const int k[3], int lane,
-                                                uint32_t cnt, uint32_t bucket, double bound0, CandList& L, float& rx, float& ry, float& rz) {
-    const double INF = __longlong_as_double(0x7FF0000000000000ll);
-    Best best;
-    best.d2 = INF; best.id = NO_ID; best.ref = 0;
-    float bx = 0.f, by = 0.f, bz = 0.f;
-    double bound = bound0;
-    const bool have_bound = bound0 < INF;
-    if (!have_bound) {
-        const uint32_t c_cnt = __shfl_sync(FULL, cnt, 13), c_bucket = __shfl_sync(FULL, bucket, 13);
-        for (uint32_t j = lane; j < c_cnt; j += 32) {
-            const uint32_t ref = c_bucket * (uint32_t)m.cap + j;
-            const float4 p = __ldg(m.points + ref);
-            const double d2 = dist2(qx, qy, qz, p.x, p.y, p.z);
-            const uint32_t id = __float_as_uint(p.w);
-            if (better(d2, id, best)) { best.d2 = d2; best.id = id; best.ref = ref; bx = p.x; by = p.y; bz = p.z; }
-        }
-        bound = warp_min_nonneg(best.d2);
-    }
-    uint32_t c2 = 0;
-    if (lane < 27 && cnt > 0 && (have_bound || lane != 13)) {
-        const double lb = (lane == 13) ? 0.0 : voxel_lower_bound(qx, qy, qz, k, m.voxel, lane / 9 - 1, (lane / 3) % 3 - 1, lane % 3 - 1);
-        if (lb <= bound) c2 = cnt;
-    }
-    const unsigned surv = __ballot_sync(FULL, c2 > 0);
-    if ((surv & ~(1u << 13)) == 0) {
-        // the usual case from the second iteration on: no neighbour voxel can hold a nearer point.  With a bound the own
-        // voxel is still to be swept (one step: cap <= 64 points, two lanes' worth at most); without, it was swept above
-        if (surv) {
-            const uint32_t c_cnt = __shfl_sync(FULL, c2, 13), c_bucket = __shfl_sync(FULL, bucket, 13);
-            for (uint32_t j = lane; j < c_cnt; j += 32) {
-                const uint32_t ref = c_bucket * (uint32_t)m.cap + j;
-                const float4 p = __ldg(m.points + ref);
-                const double d2 = dist2(qx, qy, qz, p.x, p.y, p.z);
-                const uint32_t id = __float_as_uint(p.w);
-                if (better(d2, id, best)) { best.d2 = d2; best.id = id; best.ref = ref; bx = p.x; by = p.y; bz = p.z; }
-            }
-        }
-        const int w = warp_argmin(best.d2, best.id);
-        best.d2 = __shfl_sync(FULL, best.d2, w);
-        best.id = __shfl_sync(FULL, best.id, w);
-        best.ref = __shfl_sync(FULL, best.ref, w);
-        rx = __shfl_sync(FULL, bx, w); ry = __shfl_sync(FULL, by, w); rz = __shfl_sync(FULL, bz, w);
-        return best;
-    }
-    const int total = cand_build(L, c2, bucket, lane);
-    CandIter ci;
-    ci.before = 0;
-    for (int j = lane, step = 0; j < total; j += 32, ++step) {
-        const uint32_t ref = cand_next(L, ci, step, j, lane, m.cap);
-        const float4 p = __ldg(m.points + ref);
-        const double d2 = dist2(qx, qy, qz, p.x, p.y, p.z);
-        const uint32_t id = __float_as_uint(p.w);
-        if (better(d2, id, best)) { best.d2 = d2; best.id = id; best.ref = ref; bx = p.x; by = p.y; bz = p.z; }
-    }
-    __syncwarp();
-    const int w = warp_argmin(best.d2, best.id);
-    best.d2 = __shfl_sync(FULL, best.d2, w);
-    best.id = __shfl_sync(FULL, best.id, w);
-    best.ref = __shfl_sync(FULL, best.ref, w);
-    rx = __shfl_sync(FULL, bx, w); ry = __shfl_sync(FULL, by, w); rz = __shfl_sync(FULL, bz, w);
-    return best;
+__device__ __forceinline__ double group_min_nonneg(unsigned gmask, double d2) {
+    const unsigned long long bits = (unsigned long long)__double_as_longlong(d2);
+    const uint32_t hi = (uint32_t)(bits >> 32), lo = (uint32_t)bits;
+    const uint32_t mhi = __reduce_min_sync(gmask, hi);
+    const uint32_t mlo = __reduce_min_sync(gmask, hi == mhi ? lo : 0xFFFFFFFFu);
+    return __longlong_as_double((long long)(((unsigned long long)mhi << 32) | mlo));
 }
 
-// 6x6 Cholesky solve H x = rhs by one warp: lane i < 6 owns row i (H is read from the packed upper triangle `tv` in
-// shared memory as it is needed) and rhs_i; every lane returns all of x.  The factor's row i lives in lane i's registers
-// with the RECIPROCAL pivot in place of L_ii (the pivot itself is never needed again); rows talk through shuffles, so
-// nothing spills and the six pivots are the only serial chain.  One rsqrt per pivot.  false if H is not positive
-// definite.  All 32 lanes must call (lanes >= 6 compute on row 5's data and are ignored).
-__device__ __forceinline__ bool warp_chol_solve6(const double* tv, double rhs, int lane, double x[6]) {
-    const int i = min(lane, 5);
-    double l[6];
-    bool ok = true;
-#pragma unroll
-    for (int j = 0; j < 6; ++j) {
-        const int a = min(i, j), c = max(i, j);
-        double acc = tv[a * 6 - a * (a - 1) / 2 + (c - a)];                        // H_ij
-#pragma unroll
-        for (int k = 0; k < j; ++k) acc -= l[k] * __shfl_sync(FULL, l[k], j);     // H_ij - sum_k L_ik L_jk
-        const double piv = __shfl_sync(FULL, acc, j);
-        ok = ok && piv > 0.0 && isfinite(piv);
-        const double inv = rsqrt(piv);
-        l[j] = (lane == j) ? inv : acc * inv;                                      // lanes i < j hold garbage: never read
-    }
-    // forward: y_k = (rhs_k - sum_{j<k} L_kj y_j) / L_kk, finished on lane k and broadcast
-    double y = rhs, z = 0.0;
-#pragma unroll
-    for (int k = 0; k < 6; ++k) {
-        const double yk = __shfl_sync(FULL, y * l[k], k);
-        if (lane == k) z = yk;
-        y -= l[k] * yk;                                                             // lanes i > k; others unused
-    }
-    // backward: x_k = (y_k - sum_{i>k} L_ik x_i) / L_kk; L_ik sits in lane i, which sends its product to lane k
-#pragma unroll
-    for (int k = 5; k >= 0; --k) {
-        const double xk = __shfl_sync(FULL, z * l[k], k);
-        x[k] = xk;
-#pragma unroll
-        for (int q = 0; q < k; ++q) {
-            const double c = __shfl_sync(FULL, l[q] * xk, k);                      // lane k's L_kq x_k, for lane q
-            if (lane == q) z -= c;
-        }
-    }
-    return ok;
-}
+__device__ __forceinline__ double shfl_d(unsigned mask, double v, int src) { return __shfl_sync(mask, v, src); }
 
 // coefficients of the SE(3) exponential: A = sin t / t, B = (1 - cos t) / t^2, C = (t - sin t) / t^3.  Series in t^2 up
 // to t^10 below 0.1 rad (remainder < 1e-21 relative: a Gauss-Newton increment is always that small unless the initial
@@ -325,6 +219,38 @@ __device__ __forceinline__ void exp_coefficients(double th2, double& A, double& 
     }
 }
 
+// 6x6 solve H x = rhs by one warp, Gauss-Jordan on the augmented rows: lane i < 6 owns row i of [H | rhs] (H from the
+// packed upper triangle `tv`); step k broadcasts row k, every other row eliminates column k, row k is normalised.  H is
+// symmetric positive definite in every non-degenerate registration, so no row exchange is needed and pivot k is exactly
+// the k-th pivot of the Cholesky factorisation squared: "some pivot <= 0" is the same verdict.  Serial chain: six
+// reciprocals.  Every lane returns all of x; false if H is not positive definite.  All 32 lanes must call.
+__device__ __forceinline__ bool warp_solve6(const double* tv, double rhs, int lane, double x[6]) {
+    const int i = min(lane, 5);
+    double a[7];
+#pragma unroll
+    for (int j = 0; j < 6; ++j) {
+        const int lo = min(i, j), hi = max(i, j);
+        a[j] = tv[lo * 6 - lo * (lo - 1) / 2 + (hi - lo)];
+    }
+    a[6] = rhs;
+    bool ok = true;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        double pk[7];
+#pragma unroll
+        for (int j = k; j < 7; ++j) pk[j] = __shfl_sync(FULL, a[j], k);
+        const double piv = pk[k];
+        ok = ok && piv > 0.0 && isfinite(piv);
+        const double r = 1.0 / piv;
+        const double f = a[k] * r;
+#pragma unroll
+        for (int j = k; j < 7; ++j) a[j] = (lane == k) ? pk[j] * r : a[j] - f * pk[j];
+    }
+#pragma unroll
+    for (int j = 0; j < 6; ++j) x[j] = __shfl_sync(FULL, a[6], j);
+    return ok;
+}
+
 // Serial section of one iteration, run by warp 0 of block 0 (all 32 lanes call): H, b from the 29 reduced terms `tv`
 // (shared memory), solve, SE(3) exponential, pose update, stop test; lanes 0..12 publish one tagged word each, the result
 // struct is written lane-parallel when the registration ends.
@@ -334,7 +260,7 @@ __device__ __forceinline__ void solve_and_publish(const GicpParams& P, const dou
     const double rhs = -tv[21 + min(lane, 5)];
     const int n_inl = (int)(tv[28] + 0.5);
     double delta[6];
-    const bool solved = warp_chol_solve6(tv, rhs, lane, delta);
+    const bool solved = warp_solve6(tv, rhs, lane, delta);
     bool done = false;
     int converged = 0, status = FAR_OK;
     // the element of the new pose this lane owns: lanes 0..8 R (row-major), 9..11 t
@@ -389,8 +315,8 @@ __device__ __forceinline__ void solve_and_publish(const GicpParams& P, const dou
     if (lane == 12) put_tagged(P.scratch.pub + 12, done ? 1.0 : 0.0, tag);
 }
 
-// Polls `count` tagged rows starting at `first` (column = lane) and sums them: warp w takes rows w, w + 8, ... in
-// increasing order, then the 8 warp sums are added in warp order by warp 0.  Every block must call with all threads.
+// Polls `count` tagged rows starting at `first` (column = lane) and sums them: warp w takes rows w, w + GWARPS, ... in
+// increasing order, then the warp sums are added in warp order by warp 0.  Every thread of the block must call.
 __device__ __forceinline__ double block_sum_tagged(const uint4* rows, int first, int count, uint32_t tag, int lane, int wib,
                                                    double (*s_red)[TSTRIDE]) {
     // a warp's rows are requested together before the first is examined: they arrive within a microsecond of each other,
@@ -423,31 +349,40 @@ __device__ __forceinline__ double block_sum_tagged(const uint4* rows, int first,
     return t;   // valid in warp 0
 }
 
-// what a warp keeps about its source point from one iteration to the next (shared memory: 30-cycle reads instead of
-// registers the FP64 linearisation needs)
-struct WarpState {
+// what a group keeps in shared memory about its source point (read once per iteration; the registers go to the FP64 work)
+struct PointState {
     float s[3];       // the source point (sensor frame)
     float pr[3];      // previous nearest neighbour
     int kr[3];        // its voxel
-    int kp[3];        // voxel of the transformed point at the last table walk
-    uint32_t pref;    // reference of the previous nearest neighbour
 };
 
-__global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(const __grid_constant__ MapView m, const __grid_constant__ GicpParams P) {
-    __shared__ CandList s_list[GWARPS];
-    __shared__ double s_terms[GWARPS][SSTRIDE];
+__global__ void __launch_bounds__(GTHREADS, GICP_BLOCKS_PER_SM) gicp_kernel(const __grid_constant__ MapView m, const __grid_constant__ GicpParams P) {
+    __shared__ double s_u[GPTS][U_LEN];
+    __shared__ double s_part[GWARPS][32];
     __shared__ double s_red[GWARPS][TSTRIDE];
-    __shared__ Corr s_corr[GWARPS];
-    __shared__ WarpState s_state[GWARPS];
+    __shared__ float s_cs[GPTS][6];
+    __shared__ uint32_t s_lb[GPTS][28], s_lo[GPTS][28];       // a group's surviving voxels: bucket, first candidate index
+    __shared__ PointState s_state[GPTS];
     __shared__ Pose s_T;
     __shared__ int s_done;
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    const int nwarps = (int)gridDim.x * GWARPS;
+    const int gl = lane & (GLANES - 1), base = lane & ~(GLANES - 1);
+    const unsigned gmask = (GLANES == 32 ? 0xFFFFFFFFu : ((1u << GLANES) - 1u)) << base;
+    const int slot = threadIdx.x / GLANES;                    // the group's index in the block
     // launch sequence: read by every block at start, advanced by block 0 at the very end (launches on one map are
     // stream-ordered), so every launch has its own tag space without a host-side counter or a kernel argument
     const uint32_t seq = *reinterpret_cast<volatile uint32_t*>(&P.scratch.pub[15].x);
     int n = (int)P.n;
     if (P.d_n) n = (int)min((int64_t)n, *P.d_n);
+    // blocks in use: one per SM while that holds the scan (fewer rows to reduce), never fewer than a warp's worth of
+    // points per block; the others leave at once (nothing below synchronises through the grid's size)
+    int G = (int)gridDim.x;
+    {
+        const int per_sm = (n + P.sm_count * GPTS - 1) / (P.sm_count * GPTS);
+        G = min(G, max(1, P.sm_count * max(per_sm, 1)));
+        G = min(G, max(1, (n + 3) / 4));
+    }
+    if ((int)blockIdx.x >= G) return;
     if (threadIdx.x < 12) {
         const Pose& src = P.d_init ? *P.d_init : P.init;
         double vv = threadIdx.x < 9 ? src.R[threadIdx.x] : src.t[threadIdx.x - 9];
@@ -460,132 +395,300 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(c
         tau2 = (P.tau_mult * sg) * (P.tau_mult * sg);
         kappa = sg / P.kappa_div;
     }
-    const int rounds = (n + nwarps - 1) / nwarps;             // source points per warp (1 when n <= resident warps)
+    // points are dealt round-robin over the blocks: point i of round rd sits in block i mod grid, so a scan smaller than
+    // the grid's capacity (the usual case) spreads evenly over all SMs instead of filling the first blocks
+    const int per_round = G * GPTS;
+    const int rounds = (n + per_round - 1) / per_round;
+    const bool resident = rounds <= 1;                        // every group keeps ONE point for the whole registration
     const double INF = __longlong_as_double(0x7FF0000000000000ll);
+    const double dv = (double)m.voxel;
+    PointState& ps = s_state[slot];
+    double* u = s_u[slot];
 
-    // one source point per warp (n <= resident warps, the usual case): everything that does not depend on the pose is
-    // fetched once and kept across iterations -- the point in shared memory, its covariance in lanes 8..13 and its flag
-    // in lane 14.  What an iteration learns is kept too: the voxel the transformed point fell into with its 27 lookups
-    // (lane l < 27: count, bucket), the nearest neighbour (reference, coordinates) and, in lanes 0..6, that
-    // neighbour's covariance and flag.
-    const bool resident = rounds == 1;
-    WarpState& ws = s_state[wib];
-    float cin0 = 0.f;
-    if (resident) {
-        const int i = (int)blockIdx.x * GWARPS + wib;
-        if (i < n) {
-            if (lane < 3) ws.s[lane] = __ldg(P.scan + (int64_t)i * P.stride + lane);
-            if (have_scan_cov) {
-                if (lane >= 8 && lane < 14) cin0 = __ldg(P.cov6 + 6 * (int64_t)i + (lane - 8));
-                if (lane == 14) cin0 = (float)__ldg(P.valid + i);
-            }
+    // what does not depend on the pose is fetched once: the point and its covariance (shared memory), its flag (lane 6)
+    float cin = 0.f;                                          // lane 6: Sigma_s valid
+    auto load_point = [&](int i) {
+        if (gl < 3) ps.s[gl] = __ldg(P.scan + (int64_t)i * P.stride + gl);
+        cin = 0.f;
+        if (have_scan_cov) {
+            if (gl < 6) s_cs[slot][gl] = __ldg(P.cov6 + 6 * (int64_t)i + gl);
+            if (gl == 6) cin = (float)__ldg(P.valid + i);
         }
+        __syncwarp(gmask);
+    };
+    {
+        const int i = slot * G + (int)blockIdx.x;
+        if (resident && i < n) load_point(i);
     }
     __syncthreads();
-    uint32_t have = 0;                    // bit 0: the 27 lookups are those of voxel ws.kp; bit 1: ws.pr / ws.pref are set
-    uint32_t pcnt = 0, pbucket = NO_BUCKET;
+    // what an iteration learns: the voxel the transformed point fell into with its 27 lookups (lane g: neighbours g + 8 j;
+    // counts packed one byte each), the nearest neighbour (reference; coordinates and voxel in shared memory) and, in lanes
+    // 0..6, that neighbour's covariance and flag
+    uint32_t have = 0;                    // bit 0: the lookups are those of voxel kp; bit 1: the previous neighbour is set
+    int kp0 = 0, kp1 = 0, kp2 = 0;
+    uint32_t pcnt[NBR_PER_LANE], pbk[NBR_PER_LANE], pref = 0xFFFFFFFFu;
+#pragma unroll
+    for (int j = 0; j < NBR_PER_LANE; ++j) { pcnt[j] = 0; pbk[j] = NO_BUCKET; }
     float cinr = 0.f;
 
     for (int it = 0; it < P.max_iters; ++it) {
         const uint32_t tag = (seq << 10) | (uint32_t)(it + 1);
-        double acc = 0.0;                                     // warp 0, lane t < 29: term t of this block
+        double acc[TERM_SLOTS];                                     // this lane's term columns, summed over its points
+#pragma unroll
+        for (int q = 0; q < TERM_SLOTS; ++q) acc[q] = 0.0;
         for (int rd = 0; rd < rounds; ++rd) {
-            // ---- phase A (Eq. 2, A1, A6, A8): one warp per source point -> correspondence record ---------------------
-            const int i = rd * nwarps + (int)blockIdx.x * GWARPS + wib;
-            int flags = 0;
-            if (i < n) {
-                float sx, sy, sz, cin = cin0;
-                if (resident) {
-                    sx = ws.s[0]; sy = ws.s[1]; sz = ws.s[2];
-                } else {
-                    const float* sp = P.scan + (int64_t)i * P.stride;
-                    sx = __ldg(sp); sy = __ldg(sp + 1); sz = __ldg(sp + 2);
-                    if (have_scan_cov) {
-                        if (lane >= 8 && lane < 14) cin = __ldg(P.cov6 + 6 * (int64_t)i + (lane - 8));
-                        if (lane == 14) cin = (float)__ldg(P.valid + i);
-                    }
-                    have = 0;
+            const int i = (rd * GPTS + slot) * G + (int)blockIdx.x;
+            if (i >= n) continue;                                   // group-uniform: everything below uses gmask
+            if (!resident) { load_point(i); have = 0; }
+            // ---- Eq. 2: the accumulated pose on the ORIGINAL point (R11); lane g computes coordinate g mod 3 ---------
+            const float sx = ps.s[0], sy = ps.s[1], sz = ps.s[2];
+            const int r3 = gl % 3;
+            float pmine;
+            {
+                double a = __dadd_rn(__dmul_rn(s_T.R[3 * r3 + 0], (double)sx), __dmul_rn(s_T.R[3 * r3 + 1], (double)sy));
+                a = __dadd_rn(a, __dmul_rn(s_T.R[3 * r3 + 2], (double)sz));
+                a = __dadd_rn(a, s_T.t[r3]);
+                pmine = __double2float_rn(a);
+            }
+            // A1 of my coordinate
+            const float fq = floorf(__fdiv_rn(pmine, m.voxel));
+            const bool inr = fq >= -1048576.0f && fq < 1048576.0f;
+            const int kmine = inr ? (int)fq : 0;
+            const float pfx = __shfl_sync(gmask, pmine, base), pfy = __shfl_sync(gmask, pmine, base + 1), pfz = __shfl_sync(gmask, pmine, base + 2);
+            const int k0 = __shfl_sync(gmask, kmine, base), k1 = __shfl_sync(gmask, kmine, base + 1), k2 = __shfl_sync(gmask, kmine, base + 2);
+            const bool ok = isfinite(sx) && isfinite(sy) && isfinite(sz) && ((__ballot_sync(gmask, inr) >> base) & 7u) == 7u;
+            if (!ok) continue;
+            // ---- the 27 lookups: reused while the point stays in its voxel ---------------------------------------------
+            if (!((have & 1u) && k0 == kp0 && k1 == kp1 && k2 == kp2)) {
+                // home entries of this lane's neighbours first, all in flight together (a walk beyond the home slot is rare)
+                unsigned long long key[NBR_PER_LANE];
+                Entry he[NBR_PER_LANE];
+                uint32_t hs[NBR_PER_LANE];
+#pragma unroll
+                for (int j = 0; j < NBR_PER_LANE; ++j) {
+                    const int l = gl + GLANES * j;
+                    const int nx = k0 + l / 9 - 1, ny = k1 + (l / 3) % 3 - 1, nz = k2 + l % 3 - 1;
+                    const bool in = l < 27 && index_in_range(nx) && index_in_range(ny) && index_in_range(nz);
+                    key[j] = in ? pack_key(nx, ny, nz) : KEY_EMPTY;
+                    hs[j] = hash_key(key[j]) & m.mask;
+                    he[j].key = KEY_EMPTY; he[j].bucket = NO_BUCKET; he[j].cr = 0;
+                    if (in) he[j] = load_entry(m.table, hs[j]);
                 }
-                float pf[3];
-                int k[3];
-                bool ok = false;
-                if (isfinite(sx) && isfinite(sy) && isfinite(sz)) {
-                    transform_point(s_T, sx, sy, sz, pf);                       // accumulated pose on the ORIGINAL point (R11)
-                    ok = voxel_index(pf[0], pf[1], pf[2], m.voxel, k);
+#pragma unroll
+                for (int j = 0; j < NBR_PER_LANE; ++j) {
+                    pcnt[j] = 0; pbk[j] = NO_BUCKET;
+                    if (key[j] != KEY_EMPTY && he[j].key != KEY_EMPTY) {
+                        Entry e = he[j];
+                        const uint32_t reach = entry_reach(e.cr);
+                        for (uint32_t d = 0;; ++d) {                           // find_voxel from the loaded home entry on
+                            if (e.key == key[j]) {
+                                const uint32_t c = entry_count(e.cr);
+                                if (c && e.bucket < BUCKET_PENDING) { pcnt[j] = c; pbk[j] = e.bucket; }
+                                break;
+                            }
+                            if (d >= reach) break;
+                            e = load_entry(m.table, (hs[j] + d + 1) & m.mask);
+                            if (e.key == KEY_EMPTY) break;
+                        }
+                    }
                 }
-                if (ok) {
-                    // the 27 lookups: reused while the point stays in its voxel
-                    if (!((have & 1u) && k[0] == ws.kp[0] && k[1] == ws.kp[1] && k[2] == ws.kp[2])) {
-                        probe27_regs(m, k, lane, pcnt, pbucket);
-                        __syncwarp();
-                        if (lane < 3) ws.kp[lane] = k[lane];
-                        have |= 1u;
+                kp0 = k0; kp1 = k1; kp2 = k2;
+                have |= 1u;
+            }
+            // ---- A6: bounded search (k = 1) ----------------------------------------------------------------
+            Best best;
+            best.d2 = INF; best.id = NO_ID; best.ref = 0;
+            float bx = 0.f, by = 0.f, bz = 0.f;
+            auto consider = [&](const float4& p, uint32_t ref) {
+                const double d2 = dist2(pfx, pfy, pfz, p.x, p.y, p.z);
+                const uint32_t id = __float_as_uint(p.w);
+                if (better(d2, id, best)) { best.d2 = d2; best.id = id; best.ref = ref; bx = p.x; by = p.y; bz = p.z; }
+            };
+            // the previous nearest neighbour bounds the search if it is one of this search's candidates
+            double bound = INF;
+            uint32_t pref_seen = 0xFFFFFFFFu;
+            if (have & 2u) {
+                pref_seen = pref;
+                if (abs(ps.kr[0] - k0) <= 1 && abs(ps.kr[1] - k1) <= 1 && abs(ps.kr[2] - k2) <= 1)
+                    bound = dist2(pfx, pfy, pfz, ps.pr[0], ps.pr[1], ps.pr[2]);
+            }
+            // without one, the point's own voxel (neighbour 13) is swept first to get a bound
+            bool own_swept = false;
+            if (!(bound < INF)) {
+                const uint32_t c = __shfl_sync(gmask, pcnt[13 / GLANES], base + 13 % GLANES), b = __shfl_sync(gmask, pbk[13 / GLANES], base + 13 % GLANES);
+                for (uint32_t j0 = 0; j0 < c; j0 += SWEEP_U * GLANES) {
+                    float4 p[SWEEP_U];
+#pragma unroll
+                    for (int t = 0; t < SWEEP_U; ++t) if (j0 + t * GLANES + gl < c) p[t] = __ldg(m.points + b * (uint32_t)m.cap + j0 + t * GLANES + gl);
+#pragma unroll
+                    for (int t = 0; t < SWEEP_U; ++t) if (j0 + t * GLANES + gl < c) consider(p[t], b * (uint32_t)m.cap + j0 + t * GLANES + gl);
+                }
+                bound = group_min_nonneg(gmask, best.d2);
+                own_swept = true;
+            }
+            {
+                // squared face gaps of the point inside its voxel, pulled in by the fp32 key-rounding margin (far_common.cuh)
+                double lo2[3], hi2[3];
+                const double q[3] = {(double)pfx, (double)pfy, (double)pfz};
+                const int kk[3] = {k0, k1, k2};
+#pragma unroll
+                for (int a = 0; a < 3; ++a) {
+                    const double margin = (double)(abs(kk[a]) + 2) * dv * 9.5367431640625e-07;   // 2^-20
+                    const double lo = fmax(q[a] - (double)kk[a] * dv - margin, 0.0);
+                    const double hi = fmax((double)(kk[a] + 1) * dv - q[a] - margin, 0.0);
+                    lo2[a] = lo * lo; hi2[a] = hi * hi;
+                }
+                // a voxel is read only if its distance lower bound does not exceed the bound (a skipped voxel holds only
+                // strictly farther points).  The survivors' points are swept as ONE flattened list per group -- compact
+                // (bucket, first candidate) pairs in shared memory, built with one packed scan over the 8 lanes -- so that
+                // candidate q goes to lane q mod GLANES and 32 loads per group are in flight whatever the voxels' sizes
+                uint32_t sc[NBR_PER_LANE];
+                uint32_t nsurv = 0, tsum = 0;
+#pragma unroll
+                for (int j = 0; j < NBR_PER_LANE; ++j) {
+                    const int l = gl + GLANES * j;
+                    const uint32_t c = pcnt[j];
+                    sc[j] = 0;
+                    if (l < 27 && c > 0 && !(l == 13 && own_swept)) {
+                        const int ox = l / 9 - 1, oy = (l / 3) % 3 - 1, oz = l % 3 - 1;
+                        double lb = 0.0;
+                        lb += ox < 0 ? lo2[0] : (ox > 0 ? hi2[0] : 0.0);
+                        lb += oy < 0 ? lo2[1] : (oy > 0 ? hi2[1] : 0.0);
+                        lb += oz < 0 ? lo2[2] : (oz > 0 ? hi2[2] : 0.0);
+                        if (lb <= bound) { sc[j] = c; ++nsurv; tsum += c; }
                     }
-                    // the previous nearest neighbour bounds the search if it is one of this search's candidates
-                    double bound = INF;
-                    uint32_t pref = 0xFFFFFFFFu;
-                    if (have & 2u) {
-                        pref = ws.pref;
-                        if (abs(ws.kr[0] - k[0]) <= 1 && abs(ws.kr[1] - k[1]) <= 1 && abs(ws.kr[2] - k[2]) <= 1)
-                            bound = dist2(pf[0], pf[1], pf[2], ws.pr[0], ws.pr[1], ws.pr[2]);
+                }
+                const uint32_t packed = (nsurv << 16) | tsum;
+                uint32_t incl = packed;
+#pragma unroll
+                for (int d = 1; d < GLANES; d <<= 1) {
+                    const uint32_t o = __shfl_up_sync(gmask, incl, d, GLANES);
+                    if (gl >= d) incl += o;
+                }
+                const uint32_t total = __shfl_sync(gmask, incl, base + GLANES - 1) & 0xFFFFu;
+                uint32_t pos = (incl - packed) >> 16, off = (incl - packed) & 0xFFFFu;
+                uint32_t* lb_ = s_lb[slot];
+                uint32_t* lo_ = s_lo[slot];
+#pragma unroll
+                for (int j = 0; j < NBR_PER_LANE; ++j) {
+                    if (sc[j]) {
+                        lb_[pos] = pbk[j];
+                        lo_[pos] = off;
+                        off += sc[j]; ++pos;
                     }
-                    // kNN-search, k = 1
-                    float rx, ry, rz;
-                    const Best best = nearest_bounded(m, pf[0], pf[1], pf[2], k, lane, pcnt, pbucket, bound, s_list[wib], rx, ry, rz);
-                    if (best.id != NO_ID) {
-                        // Sigma_r (lanes 0..5) and its flag (lane 6): one memory level, skipped if the neighbour is the old one
-                        if (have_scan_cov && best.ref != pref) {
-                            if (lane < 6) cinr = __ldg(m.cov + (size_t)best.ref * 6 + lane);
-                            if (lane == 6) cinr = (float)__ldg(m.cov_ok + best.ref);
+                }
+                if (gl == GLANES - 1) lo_[pos] = off;                       // sentinel = total
+                __syncwarp(gmask);
+                uint32_t v = 0;
+                for (uint32_t q0 = 0; q0 < total; q0 += SWEEP_U * GLANES) {
+                    float4 p[SWEEP_U];
+                    uint32_t ref[SWEEP_U];
+#pragma unroll
+                    for (int t = 0; t < SWEEP_U; ++t) {
+                        const uint32_t q = q0 + t * GLANES + gl;
+                        if (q < total) {
+                            while (lo_[v + 1] <= q) ++v;
+                            ref[t] = lb_[v] * (uint32_t)m.cap + (q - lo_[v]);
+                            p[t] = __ldg(m.points + ref[t]);
                         }
-                        __syncwarp();
-                        if (best.ref != pref && lane == 0) {
-                            ws.pr[0] = rx; ws.pr[1] = ry; ws.pr[2] = rz; ws.pref = best.ref;
-                            int kr[3];
-                            voxel_index(rx, ry, rz, m.voxel, kr);                 // a stored point: always valid
-                            ws.kr[0] = kr[0]; ws.kr[1] = kr[1]; ws.kr[2] = kr[2];
-                        }
-                        have |= 2u;
-                        if (!(best.d2 > tau2)) {                                 // adaptive-threshold gate
-                            const bool full = have_scan_cov && __shfl_sync(FULL, cinr, 6) != 0.f && __shfl_sync(FULL, cin, 14) != 0.f;
-                            Corr& c = s_corr[wib];
-                            if (lane < 6) c.cr[lane] = cinr;
-                            if (lane >= 8 && lane < 14) c.cs[lane - 8] = cin;
-                            if (lane == 16) { c.p[0] = pf[0]; c.p[1] = pf[1]; c.p[2] = pf[2]; c.r[0] = rx; c.r[1] = ry; c.r[2] = rz; }
-                            flags = full ? 3 : 1;
-                        }
-                    } else {
-                        have &= ~2u;
                     }
-                    __syncwarp();
+#pragma unroll
+                    for (int t = 0; t < SWEEP_U; ++t) if (q0 + t * GLANES + gl < total) consider(p[t], ref[t]);
+                }
+                __syncwarp(gmask);                                          // the list is rebuilt by the group's next point
+            }
+            const int w = group_argmin(gmask, best.d2, best.id);
+            best.d2 = __shfl_sync(gmask, best.d2, w);
+            best.id = __shfl_sync(gmask, best.id, w);
+            best.ref = __shfl_sync(gmask, best.ref, w);
+            const float rx = __shfl_sync(gmask, bx, w), ry = __shfl_sync(gmask, by, w), rz = __shfl_sync(gmask, bz, w);
+            if (best.id == NO_ID) { have &= ~2u; continue; }
+            if (best.ref != pref_seen) {
+                // Sigma_r (lanes 0..5) and its flag (lane 6): one memory level, skipped if the neighbour is the old one
+                if (have_scan_cov) {
+                    if (gl < 6) cinr = __ldg(m.cov + (size_t)best.ref * 6 + gl);
+                    if (gl == 6) cinr = (float)__ldg(m.cov_ok + best.ref);
+                }
+                // its voxel (a stored point: always valid), one coordinate per lane
+                const float rmine = r3 == 0 ? rx : (r3 == 1 ? ry : rz);
+                const int krm = (int)floorf(__fdiv_rn(rmine, m.voxel));
+                __syncwarp(gmask);                                  // the reads of ps above are done
+                if (gl < 3) { ps.kr[gl] = krm; ps.pr[gl] = rmine; }
+                __syncwarp(gmask);
+                pref = best.ref;
+            }
+            have |= 2u;
+            if (best.d2 > tau2) continue;                           // adaptive-threshold gate
+            // ---- A9: this group's correspondence -> its 29 terms ------------------------------------------------------
+            const bool full = have_scan_cov && __shfl_sync(gmask, cinr, base + 6) != 0.f && __shfl_sync(gmask, cin, base + 6) != 0.f;
+            const double px = (double)pfx, py = (double)pfy, pz = (double)pfz;
+            const double d0 = (double)rx - px, d1 = (double)ry - py, d2 = (double)rz - pz;   // Eq. 3
+            double M[6] = {1.0, 0.0, 0.0, 1.0, 0.0, 1.0};                // SA fallback: Sigma_r = I, Sigma_s = 0
+            if (full) {
+                // S = Sigma_r + R Sigma_s R^T (Eq. 4): lane e < 6 computes entry e = (i, j) of the upper triangle
+                const int e = min(gl, 5);
+                const int ei = e < 3 ? 0 : (e < 5 ? 1 : 2), ej = e < 3 ? e : (e < 5 ? e - 2 : 2);
+                const double a = s_T.R[3 * ei], b = s_T.R[3 * ei + 1], c = s_T.R[3 * ei + 2];
+                const float* cs = s_cs[slot];
+                const double s0 = cs[0], s1 = cs[1], s2 = cs[2], s3 = cs[3], s4 = cs[4], s5 = cs[5];
+                const double u0 = a * s0 + b * s1 + c * s2, u1 = a * s1 + b * s3 + c * s4, u2 = a * s2 + b * s4 + c * s5;
+                const double cr_mine = (double)__shfl_sync(gmask, cinr, base + e);
+                const double Sm = cr_mine + (u0 * s_T.R[3 * ej] + u1 * s_T.R[3 * ej + 1] + u2 * s_T.R[3 * ej + 2]);
+                double S[6];
+#pragma unroll
+                for (int q = 0; q < 6; ++q) S[q] = shfl_d(gmask, Sm, base + q);
+                double Mi[6];
+                if (inv_sym3(S, Mi)) {
+#pragma unroll
+                    for (int q = 0; q < 6; ++q) M[q] = Mi[q];
                 }
             }
-            if (lane == 0) s_corr[wib].flags = flags;
-            __syncthreads();
-            // ---- phase B (A9): 8 lanes of warp 0 linearise the block's 8 correspondences together --------------------
-            if (wib == 0) {
-                if (lane < GWARPS) {
-                    double* terms = s_terms[lane];
-                    if (s_corr[lane].flags & 1) {
-                        correspondence_terms(s_T, s_corr[lane], P.kernel, kappa, terms);
-                    } else {
+            const double Md0 = M[0] * d0 + M[1] * d1 + M[2] * d2;
+            const double Md1 = M[1] * d0 + M[3] * d1 + M[4] * d2;
+            const double Md2 = M[2] * d0 + M[4] * d1 + M[5] * d2;
+            const double e2 = d0 * Md0 + d1 * Md1 + d2 * Md2;
+            const double wgt = robust_weight(P.kernel, e2, kappa);
+            // the group's vector u: one or two entries per lane
+            if (gl < 6) {
 #pragma unroll
-                        for (int t = 0; t < NTERMS; ++t) terms[t] = 0.0;
-                    }
-                }
-                __syncwarp();
-                if (lane < NTERMS) {
+                for (int q = 0; q < 6; ++q) if (gl == q) u[q] = M[q];       // (no dynamic register indexing)
+            } else if (gl == 6) { u[U_MD] = Md0; u[U_MD + 1] = Md1; u[U_MD + 2] = Md2; u[U_E2] = e2; }
+            else { u[U_P] = px; u[U_P + 1] = py; u[U_P + 2] = pz; u[U_ZERO] = 0.0; u[U_ONE] = 1.0; }
+            __syncwarp(gmask);
+            auto term = [&](int slot_e, bool store_x) -> double {
+                const uint32_t en = c_term_enc[slot_e];
+                const double val = u[en & 31u] * u[(en >> 5) & 31u] - u[(en >> 10) & 31u] * u[(en >> 15) & 31u];
+                const uint32_t xs = en >> 22;
+                if (store_x && xs) u[U_X + xs - 1] = val;
+                const uint32_t ck = (en >> 20) & 3u;
+                return (ck == COEF_W ? wgt : (ck == COEF_MW ? -wgt : 1.0)) * val;
+            };
 #pragma unroll
-                    for (int w8 = 0; w8 < GWARPS; ++w8) acc += s_terms[w8][lane];
-                }
-            }
-            if (rd + 1 < rounds) __syncthreads();             // the records are rewritten by the next round
+            for (int q = 0; q < TERM_SLOTS - 1; ++q) if (q * GLANES + gl < 24) acc[q] += term(q * GLANES + gl, true);   // round 1
+            __syncwarp(gmask);                                      // the nine X are in u
+            if (gl < 8) acc[TERM_SLOTS - 1] += term(24 + gl, false);
+            __syncwarp(gmask);                                      // u is rewritten by the group's next point
         }
-        // ---- A10: block row -> group of 32 blocks -> grid, tagged words, every level summed in a fixed order --------
-        if (wib == 0) put_tagged(P.scratch.rows + (size_t)blockIdx.x * TSTRIDE + lane, lane < NTERMS ? acc : 0.0, tag);
+        // ---- A10: lane-wise over the warp's 4 groups, over the block's warps, then block row -> group of 16 blocks -> grid
+        // as tagged words; every level summed in a fixed order
+#pragma unroll
+        for (int q = 0; q < TERM_SLOTS; ++q) {
+            double v = acc[q];
+#pragma unroll
+            for (int d = GLANES; d < 32; d <<= 1) v += __shfl_xor_sync(FULL, v, d);
+            const int col = q < TERM_SLOTS - 1 ? q * GLANES + lane : 24 + lane;
+            if (q < TERM_SLOTS - 1 ? (lane < GLANES && col < 24) : lane < 8) s_part[wib][col] = v;
+        }
+        __syncthreads();
+        if (wib == 0) {
+            double t = 0.0;
+#pragma unroll
+            for (int w8 = 0; w8 < GWARPS; ++w8) t += s_part[w8][lane];
+            put_tagged(P.scratch.rows + (size_t)blockIdx.x * TSTRIDE + c_term_store[lane], t, tag);
+        }
         if (blockIdx.x % GROUP == 0) {   // group leader: fold the group's rows into one
-            const int group = blockIdx.x / GROUP, n_groups = (gridDim.x + GROUP - 1) / GROUP;
-            const int group_rows = min(GROUP, (int)gridDim.x - group * GROUP);
+            const int group = blockIdx.x / GROUP, n_groups = (G + GROUP - 1) / GROUP;
+            const int group_rows = min(GROUP, G - group * GROUP);
             const double t = block_sum_tagged(P.scratch.rows, group * GROUP, group_rows, tag, lane, wib, s_red);
             if (wib == 0) put_tagged(P.scratch.grows + (size_t)group * TSTRIDE + lane, t, tag);
             if (blockIdx.x == 0) {       // block 0: final sum, solve, publish
@@ -598,12 +701,11 @@ __global__ void __launch_bounds__(GWARPS * 32, GICP_BLOCKS_PER_SM) gicp_kernel(c
             }
         }
         // ---- grid-wide wait for the new pose: all blocks are co-resident (cooperative launch) -----------------------
-        __syncthreads();                                      // phase B / the sums have finished reading s_T, s_terms
+        __syncthreads();                                      // the groups / the sums have finished reading s_T, s_part
         if (wib == 0) {
             // ONE lane per block polls the `done` word (written last); only when it carries this iteration's tag do the
-            // other twelve lanes fetch their words (each still self-validating).  740 pollers on one line instead of
-            // 9,620 on two: the solver's stores no longer queue behind the poll traffic in that L2 slice (on some B200s
-            // of the pool the publish hop cost 3.5 us instead of 1.1 us with every lane polling).
+            // other twelve lanes fetch their words (each still self-validating): the solver's stores do not queue behind
+            // poll traffic in that L2 slice
             double vv = 0.0;
             if (lane == NPUB - 1) {
                 while (!load_tagged(P.scratch.pub + lane, tag, vv)) __nanosleep(40);    // back off: do not crowd out the blocks still working
@@ -672,10 +774,12 @@ int far::gicp_launch(const far_map_t* map, const float* d_scan, const float* d_c
     P.scratch.grows = P.scratch.rows + (size_t)map->gicp_max_grid * TSTRIDE;
     P.scratch.pub = P.scratch.grows + (size_t)MAX_GROUPS * TSTRIDE;
     P.out = d_out;
+    // sized for the capacity n; the kernel works with min(n, *d_n) points and the blocks it does not need leave at once
     int64_t grid = map->gicp_max_grid;
-    const int64_t need = (n + GWARPS - 1) / GWARPS;
+    const int64_t need = (n + 3) / 4;
     if (need < grid) grid = need;
     if (grid < 1) grid = 1;
+    P.sm_count = map->sm_count;
     MapView view = map->view;
     void* args[] = {(void*)&view, (void*)&P};
     {

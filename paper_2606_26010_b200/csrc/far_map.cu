@@ -385,17 +385,23 @@ __global__ void __launch_bounds__(256) insert_commit_kernel(MapView m, const flo
             }
             const unsigned bal = __ballot_sync(FULL, is_new);
             if (bal == 0) break;                                           // ids fill positions in order: nothing further
-            if (cov_list != nullptr) {                                     // the warp's new points, voxel by voxel
-                uint32_t at = 0;
-                if (lane == 0) at = atomicAdd(&ctr->n_cov, (uint32_t)__popc(bal));
-                at = __shfl_sync(FULL, at, 0);
-                if (is_new) cov_list[at + __popc(bal & ((1u << lane) - 1u))] = b * cap + pos;
-            }
             n_new += __popc(bal & gmask);
         }
         if (active && sl == 0) {
             m.table[s].cr = (cr & ~0xFFu) | (c0 + n_new);
             acc_new += n_new;
+        }
+        if (cov_list != nullptr) {
+            // one covariance task per voxel that received points: {bucket, c0 | n_new << 8} (far_query.cu serves a voxel's
+            // new points together: they share their 27-voxel candidate set)
+            const bool has = active && sl == 0 && n_new > 0;
+            const unsigned tb = __ballot_sync(FULL, has);
+            if (tb) {
+                uint32_t at = 0;
+                if (lane == 0) at = atomicAdd(&ctr->n_cov, (uint32_t)__popc(tb));
+                at = __shfl_sync(FULL, at, 0);
+                if (has) reinterpret_cast<uint2*>(cov_list)[at + __popc(tb & ((1u << lane) - 1u))] = make_uint2(b, c0 | (n_new << 8));
+            }
         }
     }
 #pragma unroll
@@ -578,10 +584,10 @@ __global__ void __launch_bounds__(SP_THREADS) spaced_commit_kernel(MapView m, co
         if (threadIdx.x == 0) {
             m.table[s].cr = (e.cr & ~0xFFu) | s_count;
             if (nacc) atomicAdd(&ctr->st_accepted, (unsigned long long)nacc);
-            if (cov_list != nullptr && nacc) s_n = atomicAdd(&ctr->n_cov, nacc);
+            // accepted points take consecutive positions c0 .. c0 + nacc - 1: one covariance task for the voxel
+            if (cov_list != nullptr && nacc) reinterpret_cast<uint2*>(cov_list)[atomicAdd(&ctr->n_cov, 1u)] = make_uint2(b, c0 | (nacc << 8));
         }
         __syncthreads();
-        if (cov_list != nullptr && threadIdx.x < nacc) cov_list[s_n + threadIdx.x] = b * cap + s_acc[threadIdx.x];
     }
     insert_epilogue(m, n_call, last_chunk, d_stats);
 }
@@ -971,7 +977,7 @@ int far_map_create(far_map_t** out, const far_map_config_t* cfg) {
     }
     alloc((void**)&v.ctr, sizeof(Counters));
     alloc((void**)&m->d_touched, (size_t)c.max_batch * sizeof(uint32_t));
-    alloc((void**)&m->d_cov_list, (size_t)c.max_batch * sizeof(uint32_t));
+    alloc((void**)&m->d_cov_list, (size_t)c.max_batch * sizeof(uint2));
     if (c.min_spacing > 0.0) {            // scratch of the regular-spacing insert (R21)
         alloc((void**)&m->d_sp_cnt, (size_t)c.max_voxels * sizeof(uint32_t));
         alloc((void**)&m->d_sp_vt, (size_t)c.max_voxels * sizeof(uint32_t));

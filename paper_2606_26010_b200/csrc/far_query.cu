@@ -58,16 +58,22 @@ __global__ void __launch_bounds__(QWARPS * 32) count27_kernel(MapView m, const f
 
 // ---- A7: k nearest by (d2, id) -> Eq. 1 -----------------------------------------------------------------------
 // Two mappings of the same selection.
-//  (a) Covariances of the points an insert accepted: ONE THREAD PER QUERY.  The accepted points arrive
-//      grouped by voxel, so consecutive lanes of a warp are (mostly) points of the same voxel: they walk the same 27
-//      voxels, their loads of table entries and candidate points coalesce into a few sectors served by L1, and they
-//      run in lockstep.  A lane walks its 27 voxels in NEAR-FIRST order (own voxel, 6 face, 12 edge, 8 corner
-//      neighbours) so that its k-th best is tight after the first voxel, tests every candidate in FP32 against that
-//      bound (relative error of the FP32 d2 < 3e-7, margin 1e-6) and only appends the survivors to a short list; the
-//      exact FP64 distance of R6 and the sorted insertion run over the list when it fills (all lanes together), so the
-//      warp does not walk the insertion code for every candidate some lane accepts.  The neighbours chosen are exactly
-//      those of the definition.  ~300 candidates x 12 instructions per 32 queries instead of ~2,000 instructions per
-//      query for a warp per query (measured: profiles/).
+//  (a) Covariances of the points an insert accepted: ONE WARP PER TOUCHED VOXEL.  The accepted points of a
+//      voxel are positions c0 .. c0 + n_new - 1 of its bucket and they all share the same 27-voxel candidate set, so the
+//      warp probes the 27 neighbours once (27 lanes, one lookup each), stages every candidate point in shared memory with
+//      coalesced loads that are all in flight together (north_star: "points staged in shared memory"), and then serves the
+//      voxel's queries from there: G = 32 / pow2(n_new) lanes per query, each scanning a strided share of the staged list.
+//      A lane keeps its KP = 12 best candidates as ONE 32-bit key each, in registers: the FP32 squared distance with its
+//      11 low mantissa bits replaced by the candidate's index in the staged list, so unsigned order = distance order
+//      (coarsened to 2^-12 relative) and inserting is a branch-free min/max chain; the G partial lists are merged with a
+//      shuffle butterfly.  The exact FP64 (d2, id) selection of R6 then runs on those 12 only: the (count - k) largest are
+//      dropped.  The result is PROVEN to be the definition's before it is used: a candidate that was not kept has a coarse
+//      key >= the 12th kept one, hence an exact d2 >= W (1 - 3e-7) with W that key's distance bits; if the exact k-th
+//      distance is below W (1 - 1e-6) no such candidate can precede it.  Otherwise (a near-tie across the 10th..12th
+//      neighbour, ~1e-3 of the queries; always on lattice data; always when k > 10) the warp selects that query's k nearest
+//      exactly, as k successive (d2, id) minima over the staged list.
+//      Round-2 profile of the previous mapping (one thread per query: 1,414 warps for a C2 frame, 8 per SM, every lane
+//      walking ~230 candidates behind 27 dependent lookups): 92 us, 41 % long-scoreboard stalls at 12.7 % warps active.
 //  (b) A free-standing query (far_map_knn_cov: a downsampled scan point against the scan-local map; one query per
 //      voxel, nothing to share): one WARP per query, lane l keeps the k smallest of its candidates as a sorted column,
 //      then k rounds of warp arg-min over the column heads.
@@ -76,8 +82,6 @@ struct __align__(16) Cand {
     uint32_t id;
     uint32_t idx;      // reference bucket * cap + position of the candidate
 };
-
-constexpr int LCAP = 24;   // entries of a lane's survivor list
 
 __device__ __forceinline__ bool cand_less(double d2, uint32_t id, const Cand& c) {
     return d2 < c.d2 || (d2 == c.d2 && id < c.id);
@@ -100,259 +104,255 @@ __device__ __forceinline__ bool regularised_cov(const double sc[6], double eps, 
     return true;
 }
 
-// neighbour l of the near-first order: l = 0 the voxel itself, 1..6 face, 7..18 edge, 19..26 corner neighbours;
-// packed as (dx + 1) | (dy + 1) << 2 | (dz + 1) << 4
-__constant__ uint8_t c_near_first[27] = {
-    0x15,
-    0x14, 0x16, 0x11, 0x19, 0x05, 0x25,
-    0x10, 0x12, 0x18, 0x1A, 0x04, 0x06, 0x24, 0x26, 0x01, 0x09, 0x21, 0x29,
-    0x00, 0x02, 0x08, 0x0A, 0x20, 0x22, 0x28, 0x2A};
+constexpr int KP = 12;              // candidates a lane keeps (coarse keys)
+constexpr int STAGE_U = 4;          // staging loads in flight per lane
 
-// R7: mean and centred second moments of the k neighbours in a lane's sorted column, summed in neighbour order, 1/k;
-// then Eq. 1.  One lane, FP64.
-__device__ __forceinline__ bool column_cov(const MapView& m, const Cand* col, int lane, float cov[6]) {
+// per-warp shared memory of mapping (a): the staged candidates, the list bookkeeping, the indices an exact selection picks
+__host__ __device__ inline size_t cov_task_bytes(int cap) {
+    return (size_t)27 * cap * sizeof(float4) + ((sizeof(CandList) + 15) & ~(size_t)15) + 32 * sizeof(int);
+}
+
+// R7 for the staged candidates named by sel[0 .. kk): mean and centred second moments in that order (1/k), then Eq. 1
+__device__ __forceinline__ bool cov_of_selection(const MapView& m, const float4* cand, const int* sel, float out[6]) {
     const int kk = m.k_cov;
     const double inv_k = 1.0 / (double)kk;
     double mx = 0.0, my = 0.0, mz = 0.0;
-    for (int r = 0; r < kk; ++r) {
-        const float4 p = __ldg(m.points + col[r * 32 + lane].idx);
-        mx += (double)p.x; my += (double)p.y; mz += (double)p.z;
-    }
+    for (int r = 0; r < kk; ++r) { const float4 p = cand[sel[r]]; mx += (double)p.x; my += (double)p.y; mz += (double)p.z; }
     mx *= inv_k; my *= inv_k; mz *= inv_k;
     double sc[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
     for (int r = 0; r < kk; ++r) {
-        const float4 p = __ldg(m.points + col[r * 32 + lane].idx);
+        const float4 p = cand[sel[r]];
         const double dx = (double)p.x - mx, dy = (double)p.y - my, dz = (double)p.z - mz;
         sc[0] += dx * dx; sc[1] += dx * dy; sc[2] += dx * dz; sc[3] += dy * dy; sc[4] += dy * dz; sc[5] += dz * dz;
     }
 #pragma unroll
     for (int a = 0; a < 6; ++a) sc[a] *= inv_k;
-    return regularised_cov(sc, m.cov_eps, cov);
+    return regularised_cov(sc, m.cov_eps, out);
 }
 
-// (a) one thread = one query at (qx, qy, qz); `col` = this warp's [k][32] columns, `lst` = its [LCAP][32] survivor lists.
-// Returns validity; cov = Eq. 1 or the identity.
-// All lanes named in `act` must call together: the walk over the 27 voxels is kept in lockstep (trip counts are the
-// warp's maxima) so that the survivor lists are flushed by all lanes at once.
-__device__ __noinline__ bool thread_knn_cov_exact(const MapView& m, unsigned act, float qx, float qy, float qz, int lane, Cand* col,
-                                                  uint32_t* lst, uint32_t* vox, float cov[6]) {
-    const int kk = m.k_cov, cap = m.cap;
-    cov[0] = 1.f; cov[1] = 0.f; cov[2] = 0.f; cov[3] = 1.f; cov[4] = 0.f; cov[5] = 1.f;
-    int k[3];
-    const bool qok = voxel_index(qx, qy, qz, m.voxel, k);      // always true for a stored point
-    int cnt = 0, nl = 0;
-    float thr = __int_as_float(0x7F800000);            // FP32 bound of the k-th best (+inf until there are k)
-    uint32_t* my = lst + lane;
-    // exact distance (R6) + sorted insertion of the listed survivors
-    auto flush = [&]() {
-        for (int e = 0; e < nl; ++e) {
-            const uint32_t ref = my[e * 32];
-            const float4 p = __ldg(m.points + ref);
+// exact selection for ONE query by the whole warp: k successive minima of (d2, id) over the staged list (R6 order); the
+// chosen indices land in sel[], lane 0 computes Eq. 1.  total >= k.  All 32 lanes must call.
+__device__ __noinline__ bool warp_cov_exact(const MapView& m, const float4* cand, int total, float qx, float qy, float qz, int lane, int* sel,
+                                            float out[6]) {
+    const int kk = m.k_cov;
+    const double INF = __longlong_as_double(0x7FF0000000000000ll);
+    double ld = -1.0;                    // last chosen (d2, id): every d2 >= 0 follows it
+    uint32_t lid = 0;
+    for (int r = 0; r < kk; ++r) {
+        double bd = INF;
+        uint32_t bid = NO_ID;
+        int bj = 0;
+        for (int j = lane; j < total; j += 32) {
+            const float4 p = cand[j];
             const double d2 = dist2(qx, qy, qz, p.x, p.y, p.z);
             const uint32_t id = __float_as_uint(p.w);
-            int q = cnt;
-            if (cnt == kk) {
-                if (!cand_less(d2, id, col[(kk - 1) * 32 + lane])) continue;
-                q = kk - 1;
-            } else {
-                ++cnt;
-            }
-            while (q > 0) {
-                const Cand c = col[(q - 1) * 32 + lane];
-                if (!cand_less(d2, id, c)) break;
-                col[q * 32 + lane] = c;
-                --q;
-            }
-            Cand en;
-            en.d2 = d2; en.id = id; en.idx = ref;
-            col[q * 32 + lane] = en;
+            const bool after = d2 > ld || (d2 == ld && id > lid);
+            if (after && (d2 < bd || (d2 == bd && id < bid))) { bd = d2; bid = id; bj = j; }
         }
-        nl = 0;
-        if (cnt == kk) thr = __double2float_ru(col[(kk - 1) * 32 + lane].d2) * 1.000001f;
-    };
-    // pass 1: the 27 table lookups, all in flight at once (they are independent); bucket and count parked in shared memory
-    uint32_t* myv = vox + lane;
-#pragma unroll 9
-    for (int l = 0; l < 27; ++l) {
-        const int o = c_near_first[l];
-        const int nx = k[0] + (o & 3) - 1, ny = k[1] + ((o >> 2) & 3) - 1, nz = k[2] + ((o >> 4) & 3) - 1;
-        uint32_t c = 0, b = 0;
-        if (qok && index_in_range(nx) && index_in_range(ny) && index_in_range(nz)) {
-            b = find_voxel(m, pack_key(nx, ny, nz), c);
-            if (c == 0) b = 0;
-        }
-        myv[l * 32] = b;
-        myv[(27 + l) * 32] = c;
+        const int w = warp_argmin(bd, bid);
+        ld = __shfl_sync(FULL, bd, w);
+        lid = __shfl_sync(FULL, bid, w);
+        if (lane == w) sel[r] = bj;
     }
-    // pass 2: the candidates, eight loads in flight per lane
-    constexpr int U = 8;
-    for (int l = 0; l < 27; ++l) {
-        const uint32_t b = myv[l * 32], c = myv[(27 + l) * 32];
-        const uint32_t cmax = __reduce_max_sync(act, c);
-        const float4* bp = m.points + (size_t)b * cap;
-        for (uint32_t j0 = 0; j0 < cmax; j0 += U) {
-            float4 p[U];
-#pragma unroll
-            for (int u = 0; u < U; ++u) if (j0 + u < c) p[u] = __ldg(bp + j0 + u);
-#pragma unroll
-            for (int u = 0; u < U; ++u) {
-                if (j0 + u < c) {
-                    const float fx = qx - p[u].x, fy = qy - p[u].y, fz = qz - p[u].z;
-                    if (fmaf(fz, fz, fmaf(fy, fy, fx * fx)) <= thr) { my[nl * 32] = b * (uint32_t)cap + j0 + u; ++nl; }
-                }
-            }
-            if (__any_sync(act, nl > LCAP - U)) flush();          // all lanes together
-        }
-    }
-    flush();
-    if (cnt < kk) return false;                        // fewer than k candidates in the 27 voxels
-    float out[6];
-    if (!column_cov(m, col, lane, out)) return false;
-#pragma unroll
-    for (int a = 0; a < 6; ++a) cov[a] = out[a];
-    return true;
+    __syncwarp();
+    bool ok = false;
+    if (lane == 0) ok = cov_of_selection(m, cand, sel, out);
+    __syncwarp();
+    return ok;                            // valid in lane 0
 }
 
-// The fast form of (a) for k <= 10.  A lane keeps its KP = 12 best candidates as ONE 32-bit key each, in registers:
-// the FP32 squared distance with its 11 low mantissa bits replaced by the candidate's local index (neighbour 0..26 times
-// 64 + position), so unsigned order = distance order (coarsened to 2^-12 relative) and inserting is a branch-free min/max
-// chain -- no shared memory, no loop, nothing for the other lanes of the warp to wait for.  The exact FP64 (d2, id)
-// selection of R6 then runs on those 12 only.  The result is PROVEN to be the definition's before it is used: a
-// candidate that was not kept has a coarse key >= the 12th kept one, hence an exact d2 >= W (1 - 3e-7) with W that key's
-// distance bits; if the exact k-th distance is below W (1 - 1e-6) no such candidate can precede it.  Otherwise (a
-// near-tie across the 10th..12th neighbour, ~1e-3 of the queries; always on lattice data) the warp redoes its queries
-// with thread_knn_cov_exact.
-constexpr int KP = 12;
-__device__ __forceinline__ bool thread_knn_cov(const MapView& m, unsigned act, float qx, float qy, float qz, int lane, Cand* col,
-                                               uint32_t* lst, uint32_t* vox, float cov[6]) {
-    const int kk = m.k_cov, cap = m.cap;
-    if (kk > KP - 2) return thread_knn_cov_exact(m, act, qx, qy, qz, lane, col, lst, vox, cov);
-    cov[0] = 1.f; cov[1] = 0.f; cov[2] = 0.f; cov[3] = 1.f; cov[4] = 0.f; cov[5] = 1.f;
+// mapping (a): the covariances of stored points c0 .. c0 + n_new - 1 of bucket b, by one warp (all 32 lanes must call)
+__device__ __forceinline__ void warp_cov_task(const MapView& m, uint32_t b, uint32_t c0, uint32_t n_new, int lane, float4* cand, CandList& L,
+                                              int* sel) {
+    const int cap = m.cap, kk = m.k_cov;
+    const size_t first = (size_t)b * cap + c0;
+    auto write_out = [&](uint32_t q, bool ok, const float c[6]) {
+        float* o = m.cov + (first + q) * 6;
+        o[0] = ok ? c[0] : 1.f; o[1] = ok ? c[1] : 0.f; o[2] = ok ? c[2] : 0.f; o[3] = ok ? c[3] : 1.f; o[4] = ok ? c[4] : 0.f; o[5] = ok ? c[5] : 1.f;
+        m.cov_ok[first + q] = ok ? 1 : 0;
+    };
+    // the voxel: that of any stored point of the bucket (stored points are always valid)
     int k[3];
-    const bool qok = voxel_index(qx, qy, qz, m.voxel, k);      // always true for a stored point
-    // pass 1: the 27 table lookups, all in flight at once; bucket and count parked in shared memory
-    uint32_t* myv = vox + lane;
-#pragma unroll 9
-    for (int l = 0; l < 27; ++l) {
-        const int o = c_near_first[l];
-        const int nx = k[0] + (o & 3) - 1, ny = k[1] + ((o >> 2) & 3) - 1, nz = k[2] + ((o >> 4) & 3) - 1;
-        uint32_t c = 0, b = 0;
-        if (qok && index_in_range(nx) && index_in_range(ny) && index_in_range(nz)) {
-            b = find_voxel(m, pack_key(nx, ny, nz), c);
-            if (c == 0) b = 0;
-        }
-        myv[l * 32] = b;
-        myv[(27 + l) * 32] = c;
+    {
+        const float4 p0 = m.points[first];
+        voxel_index(p0.x, p0.y, p0.z, m.voxel, k);
     }
-    // pass 2: every candidate -> key -> branch-free insertion into the sorted register array
-    uint32_t key[KP];
+    uint32_t cnt, bucket;
+    probe27_regs(m, k, lane, cnt, bucket);
+    const unsigned occ = __ballot_sync(FULL, cnt > 0);
+    const int total = cand_build(L, cnt, bucket, lane);
+    if (total < kk) {                    // fewer than k candidates in the 27 voxels: every query of the voxel is invalid
+        const float none[6] = {1.f, 0.f, 0.f, 1.f, 0.f, 1.f};
+        for (uint32_t q = lane; q < n_new; q += 32) write_out(q, false, none);
+        __syncwarp();
+        return;
+    }
+    // stage every candidate (x, y, z, id bits): STAGE_U x 32 independent loads in flight
+    {
+        CandIter ci;
+        ci.before = 0;
+        for (int j0 = 0, step = 0; j0 < total; j0 += 32 * STAGE_U) {
+            float4 p[STAGE_U];
 #pragma unroll
-    for (int i = 0; i < KP; ++i) key[i] = 0xFFFFFFFFu;
-    constexpr int U = 8;
-    for (int l = 0; l < 27; ++l) {
-        const uint32_t b = myv[l * 32], c = myv[(27 + l) * 32];
-        const float4* bp = m.points + (size_t)b * cap;
-        for (uint32_t j0 = 0; j0 < c; j0 += U) {
-            float4 p[U];
+            for (int u = 0; u < STAGE_U; ++u) {
+                const int j = j0 + 32 * u + lane;
+                if (j0 + 32 * u < total) {                       // warp-uniform: cand_next wants every step, in order
+                    const uint32_t ref = cand_next(L, ci, step, j, lane, cap);
+                    ++step;
+                    if (j < total) p[u] = __ldg(m.points + ref);
+                }
+            }
 #pragma unroll
-            for (int u = 0; u < U; ++u) if (j0 + u < c) p[u] = __ldg(bp + j0 + u);
+            for (int u = 0; u < STAGE_U; ++u) {
+                const int j = j0 + 32 * u + lane;
+                if (j < total) cand[j] = p[u];
+            }
+        }
+    }
+    __syncwarp();
+    const int own = L.off[__popc(occ & ((1u << 13) - 1u))] + (int)c0;     // staged index of the voxel's first new point
+    for (uint32_t q0 = 0; q0 < n_new; q0 += 32) {
+        const uint32_t nq = min(32u, n_new - q0);
+        int G = 1;                                                     // lanes per query: the largest power of two that fits
+        while (2 * G * nq <= 32) G *= 2;
+        const uint32_t qi = lane / G;
+        const int sub = lane % G;
+        const bool act = qi < nq;
+        float qx = 0.f, qy = 0.f, qz = 0.f;
+        if (act) { const float4 qp = cand[own + q0 + qi]; qx = qp.x; qy = qp.y; qz = qp.z; }
+        bool need_exact = act && sub == 0 && kk > KP - 2;
+        if (kk <= KP - 2) {
+            // coarse keys of this lane's share of the list, sorted ascending in registers
+            uint32_t key[KP];
 #pragma unroll
-            for (int u = 0; u < U; ++u) {
-                if (j0 + u < c) {
-                    const float fx = qx - p[u].x, fy = qy - p[u].y, fz = qz - p[u].z;
-                    uint32_t x = (__float_as_uint(fmaf(fz, fz, fmaf(fy, fy, fx * fx))) & 0xFFFFF800u) | ((uint32_t)l << 6) | (j0 + u);
+            for (int i = 0; i < KP; ++i) key[i] = 0xFFFFFFFFu;
+            if (act) {
+                for (int j = sub; j < total; j += G) {
+                    const float4 p = cand[j];
+                    const float fx = qx - p.x, fy = qy - p.y, fz = qz - p.z;
+                    uint32_t x = (__float_as_uint(fmaf(fz, fz, fmaf(fy, fy, fx * fx))) & 0xFFFFF800u) | (uint32_t)j;
                     if (x < key[KP - 1]) {
 #pragma unroll
                         for (int i = 0; i < KP; ++i) { const uint32_t lo = min(key[i], x); x = max(key[i], x); key[i] = lo; }
                     }
                 }
             }
-        }
-    }
-    // pass 3: exact (d2, id) order of the kept candidates (R6), through the lane's sorted column in shared memory
-    int cnt = 0;
+            // merge the G partial lists (disjoint shares): after the butterfly every lane of a group holds the group's best KP
+            for (int d = 1; d < G; d <<= 1) {
+                uint32_t other[KP];
 #pragma unroll
-    for (int i = 0; i < KP; ++i) {
-        if (key[i] != 0xFFFFFFFFu) {
-            const uint32_t li = key[i] & 0x7FFu;
-            const uint32_t ref = myv[(li >> 6) * 32] * (uint32_t)cap + (li & 63u);
-            const float4 p = __ldg(m.points + ref);
-            const double d2 = dist2(qx, qy, qz, p.x, p.y, p.z);
-            const uint32_t id = __float_as_uint(p.w);
-            int q = cnt;
-            bool take = true;
-            if (cnt == kk) {
-                take = cand_less(d2, id, col[(kk - 1) * 32 + lane]);
-                q = kk - 1;
-            } else {
-                ++cnt;
-            }
-            if (take) {
-                while (q > 0) {
-                    const Cand c = col[(q - 1) * 32 + lane];
-                    if (!cand_less(d2, id, c)) break;
-                    col[q * 32 + lane] = c;
-                    --q;
+                for (int i = 0; i < KP; ++i) other[i] = __shfl_xor_sync(FULL, key[i], d);
+#pragma unroll
+                for (int i = 0; i < KP; ++i) {
+                    uint32_t x = other[i];
+                    if (x < key[KP - 1]) {
+#pragma unroll
+                        for (int t = 0; t < KP; ++t) { const uint32_t lo = min(key[t], x); x = max(key[t], x); key[t] = lo; }
+                    }
                 }
-                Cand en;
-                en.d2 = d2; en.id = id; en.idx = ref;
-                col[q * 32 + lane] = en;
+            }
+            if (act && sub == 0) {
+                // exact (d2, id) of the kept candidates (R6); drop the (count - k) largest; prove; Eq. 1
+                double d2e[KP];
+                uint32_t ide[KP];
+                int n_kept = 0;
+#pragma unroll
+                for (int i = 0; i < KP; ++i) {
+                    d2e[i] = -1.0; ide[i] = 0;
+                    if (key[i] != 0xFFFFFFFFu) {
+                        const float4 p = cand[key[i] & 0x7FFu];
+                        d2e[i] = dist2(qx, qy, qz, p.x, p.y, p.z);
+                        ide[i] = __float_as_uint(p.w);
+                        ++n_kept;
+                    }
+                }
+                unsigned out_mask = 0;                                  // dropped or absent
+#pragma unroll
+                for (int i = 0; i < KP; ++i) if (key[i] == 0xFFFFFFFFu) out_mask |= 1u << i;
+                for (int r = n_kept; r > kk; --r) {
+                    double wd = -1.0;
+                    uint32_t wid = 0;
+                    int wi = 0;
+#pragma unroll
+                    for (int i = 0; i < KP; ++i) {
+                        if (!(out_mask & (1u << i)) && (d2e[i] > wd || (d2e[i] == wd && ide[i] > wid))) { wd = d2e[i]; wid = ide[i]; wi = i; }
+                    }
+                    out_mask |= 1u << wi;
+                }
+                double kth = -1.0;                                      // exact k-th smallest distance
+#pragma unroll
+                for (int i = 0; i < KP; ++i) if (!(out_mask & (1u << i))) kth = fmax(kth, d2e[i]);
+                bool proven = true;                                     // fewer than KP candidates in all: nothing was ever rejected
+                if (key[KP - 1] != 0xFFFFFFFFu) proven = kth < (double)__uint_as_float(key[KP - 1] & 0xFFFFF800u) * (1.0 - 1e-6);
+                if (!proven) {
+                    need_exact = true;
+                } else {
+                    // mean and centred moments over the k chosen, in key order (fixed), 1/k; Eq. 1
+                    const double inv_k = 1.0 / (double)kk;
+                    double mx = 0.0, my = 0.0, mz = 0.0;
+#pragma unroll
+                    for (int i = 0; i < KP; ++i) {
+                        if (!(out_mask & (1u << i))) { const float4 p = cand[key[i] & 0x7FFu]; mx += (double)p.x; my += (double)p.y; mz += (double)p.z; }
+                    }
+                    mx *= inv_k; my *= inv_k; mz *= inv_k;
+                    double sc[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+                    for (int i = 0; i < KP; ++i) {
+                        if (!(out_mask & (1u << i))) {
+                            const float4 p = cand[key[i] & 0x7FFu];
+                            const double dx = (double)p.x - mx, dy = (double)p.y - my, dz = (double)p.z - mz;
+                            sc[0] += dx * dx; sc[1] += dx * dy; sc[2] += dx * dz; sc[3] += dy * dy; sc[4] += dy * dz; sc[5] += dz * dz;
+                        }
+                    }
+#pragma unroll
+                    for (int a = 0; a < 6; ++a) sc[a] *= inv_k;
+                    float c[6];
+                    const bool ok = regularised_cov(sc, m.cov_eps, c);
+                    write_out(q0 + qi, ok, c);
+                }
             }
         }
+        // the queries the coarse keys could not settle: exact selection, one query at a time by the whole warp
+        unsigned todo = __ballot_sync(FULL, need_exact);
+        while (todo) {
+            const int src = __ffs(todo) - 1;
+            todo &= todo - 1;
+            const float ex = __shfl_sync(FULL, qx, src), ey = __shfl_sync(FULL, qy, src), ez = __shfl_sync(FULL, qz, src);
+            const uint32_t eq = __shfl_sync(FULL, q0 + qi, src);
+            float c[6];
+            const bool ok = warp_cov_exact(m, cand, total, ex, ey, ez, lane, sel, c);
+            if (lane == 0) write_out(eq, ok, c);
+        }
+        __syncwarp();
     }
-    // the proof (see above); fewer than KP candidates in all: nothing was ever rejected
-    bool proven = true;
-    if (cnt == kk && key[KP - 1] != 0xFFFFFFFFu) {
-        const double W = (double)__uint_as_float(key[KP - 1] & 0xFFFFF800u);
-        proven = col[(kk - 1) * 32 + lane].d2 < W * (1.0 - 1e-6);
-    }
-    if (__any_sync(act, !proven)) return thread_knn_cov_exact(m, act, qx, qy, qz, lane, col, lst, vox, cov);
-    if (cnt < kk) return false;                        // fewer than k candidates in the 27 voxels
-    float out[6];
-    if (!column_cov(m, col, lane, out)) return false;
-#pragma unroll
-    for (int a = 0; a < 6; ++a) cov[a] = out[a];
-    return true;
 }
 
-__host__ __device__ inline size_t knn_thread_bytes(int k) { return (size_t)32 * k * sizeof(Cand) + (size_t)(LCAP + 54) * 32 * sizeof(uint32_t); }
-
-// queries = stored points named by refs: the points an insert accepted, grouped by voxel
-__global__ void __launch_bounds__(256) knn_cov_refs_kernel(MapView m, const uint32_t* __restrict__ refs, const unsigned int* __restrict__ d_n,
+// tasks = the voxels an insert call added points to, queued by its commit kernel: {bucket, c0 | n_new << 8}
+__global__ void __launch_bounds__(256) knn_cov_refs_kernel(MapView m, const uint2* __restrict__ tasks, const unsigned int* __restrict__ d_n,
                                     int warps_per_block) {
     extern __shared__ __align__(16) char smem[];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    char* wbase = smem + (size_t)wib * knn_thread_bytes(m.k_cov);
-    Cand* col = reinterpret_cast<Cand*>(wbase);
-    uint32_t* lst = reinterpret_cast<uint32_t*>(wbase + (size_t)32 * m.k_cov * sizeof(Cand));
-    uint32_t* vox = lst + LCAP * 32;
+    char* wbase = smem + (size_t)wib * cov_task_bytes(m.cap);
+    float4* cand = reinterpret_cast<float4*>(wbase);
+    CandList& L = *reinterpret_cast<CandList*>(wbase + (size_t)27 * m.cap * sizeof(float4));
+    int* sel = reinterpret_cast<int*>(wbase + (size_t)27 * m.cap * sizeof(float4) + ((sizeof(CandList) + 15) & ~(size_t)15));
     const int64_t n = *d_n;
     const int64_t nwarps = (int64_t)gridDim.x * warps_per_block;
-    for (int64_t base = ((int64_t)blockIdx.x * warps_per_block + wib) * 32; base < n; base += nwarps * 32) {
-        const int64_t i = base + lane;
-        const unsigned act = __ballot_sync(FULL, i < n);
-        if (i < n) {
-            const uint32_t ref = refs[i];
-            const float4 p = m.points[ref];
-            float c[6];
-            const bool ok = thread_knn_cov(m, act, p.x, p.y, p.z, lane, col, lst, vox, c);
-            float* o = m.cov + (size_t)ref * 6;
-#pragma unroll
-            for (int a = 0; a < 6; ++a) o[a] = c[a];
-            m.cov_ok[ref] = ok ? 1 : 0;
-        }
+    for (int64_t t = (int64_t)blockIdx.x * warps_per_block + wib; t < n; t += nwarps) {
+        const uint2 task = tasks[t];
+        warp_cov_task(m, task.x, task.y & 0xFFu, task.y >> 8, lane, cand, L, sel);
     }
 }
 
-// same for calls larger than the reference list: every stored point with id >= the call's first id is a new point.
-// A warp takes 32 table slots, lists the new points of their voxels in shared memory and serves them 32 at a time.
+// same for calls larger than the task list: every stored point with id >= the call's first id is a new point.  A warp
+// takes 32 table slots and serves the voxels among them that hold new points one after the other.
 __global__ void __launch_bounds__(256) knn_cov_new_ids_kernel(MapView m, int warps_per_block) {
     extern __shared__ __align__(16) char smem[];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    char* wbase = smem + (size_t)wib * knn_thread_bytes(m.k_cov);
-    Cand* col = reinterpret_cast<Cand*>(wbase);
-    uint32_t* lst = reinterpret_cast<uint32_t*>(wbase + (size_t)32 * m.k_cov * sizeof(Cand));
-    uint32_t* vox = lst + LCAP * 32;
+    char* wbase = smem + (size_t)wib * cov_task_bytes(m.cap);
+    float4* cand = reinterpret_cast<float4*>(wbase);
+    CandList& L = *reinterpret_cast<CandList*>(wbase + (size_t)27 * m.cap * sizeof(float4));
+    int* sel = reinterpret_cast<int*>(wbase + (size_t)27 * m.cap * sizeof(float4) + ((sizeof(CandList) + 15) & ~(size_t)15));
     const uint32_t first_id = (uint32_t)m.ctr->call_first_id;
     const int64_t nwarps = (int64_t)gridDim.x * warps_per_block;
     for (int64_t s0 = ((int64_t)blockIdx.x * warps_per_block + wib) * 32; s0 < m.slots; s0 += nwarps * 32) {
@@ -362,31 +362,12 @@ __global__ void __launch_bounds__(256) knn_cov_new_ids_kernel(MapView m, int war
         uint32_t cnt = entry_count(e.cr), c0 = cnt;
         if (e.key == KEY_EMPTY || e.bucket >= BUCKET_PENDING) cnt = c0 = 0;
         while (c0 > 0 && m.ids[(size_t)e.bucket * m.cap + c0 - 1] >= first_id) --c0;     // ids ascend: the new points are a suffix
-        // flatten the warp's new points: lane l's voxel contributes cnt - c0 of them
-        const int mine = (int)(cnt - c0);
-        const int incl = warp_incl_scan(mine, lane);
-        const int total = __shfl_sync(FULL, incl, 31);
-        for (int q0 = 0; q0 < total; q0 += 32) {
-            const int q = q0 + lane;
-            // owner of flattened query q: the lane whose [incl - mine, incl) holds it
-            uint32_t ref = 0;
-            bool have = false;
-            for (int src = 0; src < 32; ++src) {
-                const int hi = __shfl_sync(FULL, incl, src), n_src = __shfl_sync(FULL, mine, src);
-                const uint32_t b_src = __shfl_sync(FULL, e.bucket, src), c0_src = __shfl_sync(FULL, c0, src);
-                if (!have && q < total && q >= hi - n_src && q < hi) { ref = b_src * (uint32_t)m.cap + c0_src + (uint32_t)(q - (hi - n_src)); have = true; }
-            }
-            const unsigned act = __ballot_sync(FULL, have);
-            if (have) {
-                const float4 p = m.points[ref];
-                float c[6];
-                const bool ok = thread_knn_cov(m, act, p.x, p.y, p.z, lane, col, lst, vox, c);
-                float* o = m.cov + (size_t)ref * 6;
-#pragma unroll
-                for (int a = 0; a < 6; ++a) o[a] = c[a];
-                m.cov_ok[ref] = ok ? 1 : 0;
-            }
-            __syncwarp();
+        unsigned todo = __ballot_sync(FULL, cnt > c0);
+        while (todo) {
+            const int src = __ffs(todo) - 1;
+            todo &= todo - 1;
+            const uint32_t b = __shfl_sync(FULL, e.bucket, src), f = __shfl_sync(FULL, c0, src), c = __shfl_sync(FULL, cnt, src);
+            warp_cov_task(m, b, f, c - f, lane, cand, L, sel);
         }
     }
 }
@@ -511,12 +492,12 @@ struct KnnLaunch { int warps, grid; size_t smem; };
 // The shared-memory opt-in and the occupancy query are slow host calls: done once per (kernel, k_cov, device) and cached
 // (the frame chain launches two of these kernels per scan).
 template <class K>
-static int knn_launch_cfg(const far_map* map, K kernel, size_t per_warp, int64_t work_warps, KnnLaunch& L) {
+static int knn_launch_cfg(const far_map* map, K kernel, size_t per_warp, int64_t work_warps, KnnLaunch& L, int cache_key) {
     struct Cached { bool have; int warps, per_sm; size_t smem; };
-    static Cached cache[33][8] = {};          // one table per kernel instantiation
+    static Cached cache[65][8] = {};          // one table per kernel instantiation; key = what sizes the warp's shared memory
     static size_t attr_bytes[8] = {};         // largest dynamic shared-memory opt-in made for this kernel, per device
     const int dev = map->device & 7;
-    Cached& c = cache[map->view.k_cov][dev];
+    Cached& c = cache[cache_key][dev];
     if (!c.have || map->device >= 8) {
         per_warp = (per_warp + 15) & ~(size_t)15;
         int warps = (int)(100 * 1024 / per_warp);
@@ -545,18 +526,18 @@ static int knn_launch_cfg(const far_map* map, K kernel, size_t per_warp, int64_t
     return FAR_OK;
 }
 
-int launch_knn_cov_refs(const far_map* map, const uint32_t* d_refs, const unsigned int* d_n, int64_t n_max, cudaStream_t st) {
+int launch_knn_cov_refs(const far_map* map, const uint32_t* d_tasks, const unsigned int* d_n, int64_t n_max, cudaStream_t st) {
     KnnLaunch L;
-    int rc = knn_launch_cfg(map, knn_cov_refs_kernel, knn_thread_bytes(map->view.k_cov), (n_max + 31) / 32, L);
+    int rc = knn_launch_cfg(map, knn_cov_refs_kernel, cov_task_bytes(map->view.cap), n_max, L, map->view.cap);
     if (rc != FAR_OK) return rc;
-    FAR_LAUNCH(knn_cov_refs_kernel, L.grid, L.warps * 32, L.smem, st, map->view, d_refs, d_n, L.warps);
+    FAR_LAUNCH(knn_cov_refs_kernel, L.grid, L.warps * 32, L.smem, st, map->view, reinterpret_cast<const uint2*>(d_tasks), d_n, L.warps);
     FAR_CUDA(cudaGetLastError());
     return FAR_OK;
 }
 
 int launch_knn_cov_new_ids(const far_map* map, cudaStream_t st) {
     KnnLaunch L;
-    int rc = knn_launch_cfg(map, knn_cov_new_ids_kernel, knn_thread_bytes(map->view.k_cov), (map->view.slots + 31) / 32, L);
+    int rc = knn_launch_cfg(map, knn_cov_new_ids_kernel, cov_task_bytes(map->view.cap), (map->view.slots + 31) / 32, L, map->view.cap);
     if (rc != FAR_OK) return rc;
     FAR_LAUNCH(knn_cov_new_ids_kernel, L.grid, L.warps * 32, L.smem, st, map->view, L.warps);
     FAR_CUDA(cudaGetLastError());
@@ -603,7 +584,7 @@ static int knn_cov_impl(const far_map_t* map, const float* d_q, int64_t m, const
     if (!map || m < 0 || (stride != 3 && stride != 4) || (m > 0 && (!d_q || !d_cov6 || !d_valid))) return FAR_ERR_ARG;
     if (m == 0) return FAR_OK;
     KnnLaunch L;
-    int rc = knn_launch_cfg(map, knn_cov_points_kernel, knn_warp_bytes(map->view.k_cov), m, L);
+    int rc = knn_launch_cfg(map, knn_cov_points_kernel, knn_warp_bytes(map->view.k_cov), m, L, map->view.k_cov);
     if (rc != FAR_OK) return rc;
     FAR_LAUNCH(knn_cov_points_kernel, L.grid, L.warps * 32, L.smem, (cudaStream_t)stream, map->view, d_q, m, d_m, stride, d_cov6,
                                                                                   d_valid, L.warps);
