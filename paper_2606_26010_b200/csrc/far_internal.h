@@ -9,7 +9,7 @@ struct far_map {
     far_map_config_t cfg;
     far::MapView view;          // device pointers + constants, passed by value to kernels
     uint32_t* d_touched;        // [max_batch] slots that received their first new point in the chunk
-    uint32_t* d_cov_list;       // [max_batch] uint2 covariance tasks {bucket, c0 | n_new << 8}: the voxels an insert added points to
+    uint32_t* d_cov_list;       // [max_batch] uint4 covariance tasks {key, bucket, c0 | n_new << 8}: the voxels an insert added points to
     uint32_t *d_sp_cnt, *d_sp_vt, *d_sp_ptb, *d_sp_start, *d_sp_seg;   // scratch of the regular-spacing insert (min_spacing > 0)
     void* d_gicp_partials;      // tagged reduction rows + published pose of the cooperative GICP kernel (far_gicp.cu)
     int gicp_max_grid;          // co-resident blocks of the GICP kernel on this device

@@ -365,10 +365,11 @@ __global__ void __launch_bounds__(256) insert_commit_kernel(MapView m, const flo
         const int64_t t = t0 + sub;
         const bool active = t < n_touched;
         uint32_t s = 0, b = 0, cr = 0, c0 = cap;
+        unsigned long long vkey = 0;
         if (active) {
             s = touched[t];
             const Entry e = m.table[s];
-            b = e.bucket; cr = e.cr;
+            b = e.bucket; cr = e.cr; vkey = e.key;
             c0 = entry_count(cr);
         }
         uint32_t n_new = 0;
@@ -392,7 +393,7 @@ __global__ void __launch_bounds__(256) insert_commit_kernel(MapView m, const flo
             acc_new += n_new;
         }
         if (cov_list != nullptr) {
-            // one covariance task per voxel that received points: {bucket, c0 | n_new << 8} (far_query.cu serves a voxel's
+            // one covariance task per voxel that received points: {key, bucket, c0 | n_new << 8} (far_query.cu serves a voxel's
             // new points together: they share their 27-voxel candidate set)
             const bool has = active && sl == 0 && n_new > 0;
             const unsigned tb = __ballot_sync(FULL, has);
@@ -400,7 +401,7 @@ __global__ void __launch_bounds__(256) insert_commit_kernel(MapView m, const flo
                 uint32_t at = 0;
                 if (lane == 0) at = atomicAdd(&ctr->n_cov, (uint32_t)__popc(tb));
                 at = __shfl_sync(FULL, at, 0);
-                if (has) reinterpret_cast<uint2*>(cov_list)[at + __popc(tb & ((1u << lane) - 1u))] = make_uint2(b, c0 | (n_new << 8));
+                if (has) reinterpret_cast<uint4*>(cov_list)[at + __popc(tb & ((1u << lane) - 1u))] = make_uint4((uint32_t)vkey, (uint32_t)(vkey >> 32), b, c0 | (n_new << 8));
             }
         }
     }
@@ -585,7 +586,7 @@ __global__ void __launch_bounds__(SP_THREADS) spaced_commit_kernel(MapView m, co
             m.table[s].cr = (e.cr & ~0xFFu) | s_count;
             if (nacc) atomicAdd(&ctr->st_accepted, (unsigned long long)nacc);
             // accepted points take consecutive positions c0 .. c0 + nacc - 1: one covariance task for the voxel
-            if (cov_list != nullptr && nacc) reinterpret_cast<uint2*>(cov_list)[atomicAdd(&ctr->n_cov, 1u)] = make_uint2(b, c0 | (nacc << 8));
+            if (cov_list != nullptr && nacc) reinterpret_cast<uint4*>(cov_list)[atomicAdd(&ctr->n_cov, 1u)] = make_uint4((uint32_t)e.key, (uint32_t)(e.key >> 32), b, c0 | (nacc << 8));
         }
         __syncthreads();
     }
@@ -977,7 +978,7 @@ int far_map_create(far_map_t** out, const far_map_config_t* cfg) {
     }
     alloc((void**)&v.ctr, sizeof(Counters));
     alloc((void**)&m->d_touched, (size_t)c.max_batch * sizeof(uint32_t));
-    alloc((void**)&m->d_cov_list, (size_t)c.max_batch * sizeof(uint2));
+    alloc((void**)&m->d_cov_list, (size_t)c.max_batch * sizeof(uint4));
     if (c.min_spacing > 0.0) {            // scratch of the regular-spacing insert (R21)
         alloc((void**)&m->d_sp_cnt, (size_t)c.max_voxels * sizeof(uint32_t));
         alloc((void**)&m->d_sp_vt, (size_t)c.max_voxels * sizeof(uint32_t));

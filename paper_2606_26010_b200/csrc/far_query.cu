@@ -109,7 +109,7 @@ constexpr int STAGE_U = 4;          // staging loads in flight per lane
 
 // per-warp shared memory of mapping (a): the staged candidates, the list bookkeeping, the indices an exact selection picks
 __host__ __device__ inline size_t cov_task_bytes(int cap) {
-    return (size_t)27 * cap * sizeof(float4) + ((sizeof(CandList) + 15) & ~(size_t)15) + 32 * sizeof(int);
+    return (size_t)27 * cap * sizeof(float4) + ((sizeof(CandList) + 15) & ~(size_t)15) + 64 * sizeof(int);
 }
 
 // R7 for the staged candidates named by sel[0 .. kk): mean and centred second moments in that order (1/k), then Eq. 1
@@ -162,8 +162,16 @@ __device__ __noinline__ bool warp_cov_exact(const MapView& m, const float4* cand
 }
 
 // mapping (a): the covariances of stored points c0 .. c0 + n_new - 1 of bucket b, by one warp (all 32 lanes must call)
-__device__ __forceinline__ void warp_cov_task(const MapView& m, uint32_t b, uint32_t c0, uint32_t n_new, int lane, float4* cand, CandList& L,
-                                              int* sel) {
+// neighbour l of the near-first order: l = 0 the voxel itself, 1..6 face, 7..18 edge, 19..26 corner neighbours;
+// packed as (dx + 1) | (dy + 1) << 2 | (dz + 1) << 4
+__constant__ uint8_t c_near_first[27] = {
+    0x15,
+    0x14, 0x16, 0x11, 0x19, 0x05, 0x25,
+    0x10, 0x12, 0x18, 0x1A, 0x04, 0x06, 0x24, 0x26, 0x01, 0x09, 0x21, 0x29,
+    0x00, 0x02, 0x08, 0x0A, 0x20, 0x22, 0x28, 0x2A};
+
+__device__ __forceinline__ void warp_cov_task(const MapView& m, unsigned long long vkey, uint32_t b, uint32_t c0, uint32_t n_new, int lane,
+                                              float4* cand, CandList& L, int* sel) {
     const int cap = m.cap, kk = m.k_cov;
     const size_t first = (size_t)b * cap + c0;
     auto write_out = [&](uint32_t q, bool ok, const float c[6]) {
@@ -171,16 +179,22 @@ __device__ __forceinline__ void warp_cov_task(const MapView& m, uint32_t b, uint
         o[0] = ok ? c[0] : 1.f; o[1] = ok ? c[1] : 0.f; o[2] = ok ? c[2] : 0.f; o[3] = ok ? c[3] : 1.f; o[4] = ok ? c[4] : 0.f; o[5] = ok ? c[5] : 1.f;
         m.cov_ok[first + q] = ok ? 1 : 0;
     };
-    // the voxel: that of any stored point of the bucket (stored points are always valid)
+    // the 27 lookups in NEAR-FIRST order (lane 0 the voxel itself, then face, edge, corner neighbours): the staged list
+    // starts with the voxel's own points and a query's 12th-best distance is tight before the far voxels come up
     int k[3];
-    {
-        const float4 p0 = m.points[first];
-        voxel_index(p0.x, p0.y, p0.z, m.voxel, k);
+    unpack_key(vkey, k);
+    uint32_t cnt = 0, bucket = NO_BUCKET;
+    int nbr = 0;
+    if (lane < 27) {
+        nbr = c_near_first[lane];
+        const int nx = k[0] + (nbr & 3) - 1, ny = k[1] + ((nbr >> 2) & 3) - 1, nz = k[2] + ((nbr >> 4) & 3) - 1;
+        if (index_in_range(nx) && index_in_range(ny) && index_in_range(nz)) bucket = find_voxel(m, pack_key(nx, ny, nz), cnt);
     }
-    uint32_t cnt, bucket;
-    probe27_regs(m, k, lane, cnt, bucket);
     const unsigned occ = __ballot_sync(FULL, cnt > 0);
     const int total = cand_build(L, cnt, bucket, lane);
+    int* nb = sel + 32;                  // offset code of compact voxel c
+    if (cnt > 0) nb[__popc(occ & ((1u << lane) - 1u))] = nbr;
+    const int nvox = __popc(occ);
     if (total < kk) {                    // fewer than k candidates in the 27 voxels: every query of the voxel is invalid
         const float none[6] = {1.f, 0.f, 0.f, 1.f, 0.f, 1.f};
         for (uint32_t q = lane; q < n_new; q += 32) write_out(q, false, none);
@@ -210,7 +224,7 @@ __device__ __forceinline__ void warp_cov_task(const MapView& m, uint32_t b, uint
         }
     }
     __syncwarp();
-    const int own = L.off[__popc(occ & ((1u << 13) - 1u))] + (int)c0;     // staged index of the voxel's first new point
+    const int own = (int)c0;                                               // staged index of the voxel's first new point (its voxel is compact voxel 0)
     for (uint32_t q0 = 0; q0 < n_new; q0 += 32) {
         const uint32_t nq = min(32u, n_new - q0);
         int G = 1;                                                     // lanes per query: the largest power of two that fits
@@ -227,13 +241,35 @@ __device__ __forceinline__ void warp_cov_task(const MapView& m, uint32_t b, uint
 #pragma unroll
             for (int i = 0; i < KP; ++i) key[i] = 0xFFFFFFFFu;
             if (act) {
-                for (int j = sub; j < total; j += G) {
-                    const float4 p = cand[j];
-                    const float fx = qx - p.x, fy = qy - p.y, fz = qz - p.z;
-                    uint32_t x = (__float_as_uint(fmaf(fz, fz, fmaf(fy, fy, fx * fx))) & 0xFFFFF800u) | (uint32_t)j;
-                    if (x < key[KP - 1]) {
+                // squared FP32 gaps from the query to the six faces of its voxel, pulled in by 2^-19 |k| v (key rounding and
+                // the FP32 arithmetic here): a neighbour voxel's distance lower bound is a sum of up to three of them
+                float glo[3], ghi[3];
+                const float qq[3] = {qx, qy, qz};
 #pragma unroll
-                        for (int i = 0; i < KP; ++i) { const uint32_t lo = min(key[i], x); x = max(key[i], x); key[i] = lo; }
+                for (int a = 0; a < 3; ++a) {
+                    const float mg = (float)(abs(k[a]) + 2) * m.voxel * 1.9073486328125e-06f;
+                    const float lo = fmaxf(qq[a] - (float)k[a] * m.voxel - mg, 0.f), hi = fmaxf((float)(k[a] + 1) * m.voxel - qq[a] - mg, 0.f);
+                    glo[a] = lo * lo; ghi[a] = hi * hi;
+                }
+                for (int c = 0; c < nvox; ++c) {
+                    const int j0 = L.off[c], j1 = c + 1 < nvox ? L.off[c + 1] : total;
+                    if (c > 0 && key[KP - 1] != 0xFFFFFFFFu) {
+                        // skip the voxel if even its nearest possible point cannot enter this lane's list: every candidate
+                        // in it then has a coarse key above key[KP - 1] (0.2 % slack covers the key's 2^-12 coarsening)
+                        const int o = nb[c];
+                        const int ox = (o & 3) - 1, oy = ((o >> 2) & 3) - 1, oz = ((o >> 4) & 3) - 1;
+                        const float lb = (ox < 0 ? glo[0] : (ox > 0 ? ghi[0] : 0.f)) + (oy < 0 ? glo[1] : (oy > 0 ? ghi[1] : 0.f)) +
+                                         (oz < 0 ? glo[2] : (oz > 0 ? ghi[2] : 0.f));
+                        if (lb * 0.998f > __uint_as_float(key[KP - 1] | 0x7FFu)) continue;
+                    }
+                    for (int j = j0 + sub; j < j1; j += G) {
+                        const float4 p = cand[j];
+                        const float fx = qx - p.x, fy = qy - p.y, fz = qz - p.z;
+                        uint32_t x = (__float_as_uint(fmaf(fz, fz, fmaf(fy, fy, fx * fx))) & 0xFFFFF800u) | (uint32_t)j;
+                        if (x < key[KP - 1]) {
+#pragma unroll
+                            for (int i = 0; i < KP; ++i) { const uint32_t lo = min(key[i], x); x = max(key[i], x); key[i] = lo; }
+                        }
                     }
                 }
             }
@@ -327,8 +363,10 @@ __device__ __forceinline__ void warp_cov_task(const MapView& m, uint32_t b, uint
     }
 }
 
-// tasks = the voxels an insert call added points to, queued by its commit kernel: {bucket, c0 | n_new << 8}
-__global__ void __launch_bounds__(256) knn_cov_refs_kernel(MapView m, const uint2* __restrict__ tasks, const unsigned int* __restrict__ d_n,
+// tasks = the voxels an insert call added points to, queued by its commit kernel: {key lo, key hi, bucket, c0 | n_new << 8}.
+// Two sweeps over the queue, the voxels with many new points first: they are the long jobs (a query gets 32 / pow2(n_new)
+// lanes), and a warp that picks one up last would finish long after the others.
+__global__ void __launch_bounds__(256, 3) knn_cov_refs_kernel(MapView m, const uint4* __restrict__ tasks, const unsigned int* __restrict__ d_n,
                                     int warps_per_block) {
     extern __shared__ __align__(16) char smem[];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
@@ -338,9 +376,13 @@ __global__ void __launch_bounds__(256) knn_cov_refs_kernel(MapView m, const uint
     int* sel = reinterpret_cast<int*>(wbase + (size_t)27 * m.cap * sizeof(float4) + ((sizeof(CandList) + 15) & ~(size_t)15));
     const int64_t n = *d_n;
     const int64_t nwarps = (int64_t)gridDim.x * warps_per_block;
-    for (int64_t t = (int64_t)blockIdx.x * warps_per_block + wib; t < n; t += nwarps) {
-        const uint2 task = tasks[t];
-        warp_cov_task(m, task.x, task.y & 0xFFu, task.y >> 8, lane, cand, L, sel);
+    for (int sweep = 0; sweep < 2; ++sweep) {
+        for (int64_t t = (int64_t)blockIdx.x * warps_per_block + wib; t < n; t += nwarps) {
+            const uint4 task = tasks[t];
+            const uint32_t c0 = task.w & 0xFFu, n_new = task.w >> 8;
+            if ((n_new > 8) == (sweep == 0))
+                warp_cov_task(m, ((unsigned long long)task.y << 32) | task.x, task.z, c0, n_new, lane, cand, L, sel);
+        }
     }
 }
 
@@ -367,7 +409,8 @@ __global__ void __launch_bounds__(256) knn_cov_new_ids_kernel(MapView m, int war
             const int src = __ffs(todo) - 1;
             todo &= todo - 1;
             const uint32_t b = __shfl_sync(FULL, e.bucket, src), f = __shfl_sync(FULL, c0, src), c = __shfl_sync(FULL, cnt, src);
-            warp_cov_task(m, b, f, c - f, lane, cand, L, sel);
+            const uint32_t klo = __shfl_sync(FULL, (uint32_t)e.key, src), khi = __shfl_sync(FULL, (uint32_t)(e.key >> 32), src);
+            warp_cov_task(m, ((unsigned long long)khi << 32) | klo, b, f, c - f, lane, cand, L, sel);
         }
     }
 }
@@ -530,7 +573,7 @@ int launch_knn_cov_refs(const far_map* map, const uint32_t* d_tasks, const unsig
     KnnLaunch L;
     int rc = knn_launch_cfg(map, knn_cov_refs_kernel, cov_task_bytes(map->view.cap), n_max, L, map->view.cap);
     if (rc != FAR_OK) return rc;
-    FAR_LAUNCH(knn_cov_refs_kernel, L.grid, L.warps * 32, L.smem, st, map->view, reinterpret_cast<const uint2*>(d_tasks), d_n, L.warps);
+    FAR_LAUNCH(knn_cov_refs_kernel, L.grid, L.warps * 32, L.smem, st, map->view, reinterpret_cast<const uint4*>(d_tasks), d_n, L.warps);
     FAR_CUDA(cudaGetLastError());
     return FAR_OK;
 }
