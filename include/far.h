@@ -145,9 +145,9 @@ int far_map_stats(far_map_t* map, far_map_stats_t* d_stats, void* stream);
 int far_map_status(const far_map_t* map);
 /* Deletion in open addressing (SURVEY.md:214-216; PAPER.md:109 prunes every frame, :171,186 nothing may allocate):
  * far_map_prune hands the buckets of removed voxels back to the free list at once and leaves their keys behind as dead
- * keys; when these pass max(32 + live/8) -- decided on the device in prune's epilogue -- the two rehash kernels that
- * every prune call enqueues rebuild the 16-byte entries into the preallocated shadow table, recompute the probe bounds and
- * copy them back.  far_map_rehash forces that rebuild now.  No allocation, no synchronisation; contents unchanged. */
+ * keys; when these pass max(32 + live/8) -- decided on the device in prune's epilogue -- the rehash kernel that
+ * every prune call enqueues rebuilds the 16-byte entries into the preallocated shadow table, recomputes the probe bounds and
+ * copies them back.  far_map_rehash forces that rebuild now.  No allocation, no synchronisation; contents unchanged. */
 int far_map_rehash(far_map_t* map, void* stream);
 /* R22 (ids are this library's construct, PAPER.md has none): ids are u32 and advance by the points OFFERED, so a frontend
  * fed 150k-point scans at 20 Hz would exhaust them in ~20 minutes.  A renumber pass subtracts the smallest live id from

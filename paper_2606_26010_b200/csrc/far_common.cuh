@@ -18,7 +18,7 @@
 //   free    : u32[max_voxels]           stack of bucket indices returned by far_map_prune
 // A pruned voxel gives its bucket back at once; its key stays in the table with bucket = NO_BUCKET ("dead key": absent for
 // every query, re-usable by an insert) until the number of dead keys passes a device-side threshold, at which point the
-// prune call itself rebuilds the 16-byte entries into `shadow` and copies them back -- no allocation, no host sync.
+// prune call's rehash kernel rebuilds the 16-byte entries into `shadow` and copies them back -- no allocation, no host sync.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -54,10 +54,11 @@ struct Counters {
     unsigned int n_alloc;             // buckets handed out by the running insert kernel: the first n_free of them come off the
                                       // free list, the rest from the fresh end; folded into n_free / bump by the commit epilogue
     unsigned int full_flag;           // sticky until buckets are freed: a point was dropped (pool or table exhausted)
-    unsigned int rehash_flag;         // written by prune's epilogue: the two rehash kernels that follow do their work
+    unsigned int rehash_flag;         // written by prune's epilogue: the rehash kernel that follows does its work (and clears it)
     unsigned int rehash_moved;        // entries moved by the running rehash
     unsigned int n_rehash;            // rehashes done since create / clear
-    unsigned int ticket[4];           // last-block-done tickets: 0 insert commit, 1 prune, 2 clear, 3 renumber
+    unsigned int ticket[6];           // last-block-done tickets: 0 insert commit, 1 prune, 2 clear, 3 renumber, 4 rehash
+    unsigned int rehash_barrier;      // arrivals at the grid-wide barrier between the two passes of the rehash
     unsigned int n_touched;           // voxels that received a first new point in the current chunk
     unsigned int n_tasks;             // length of the covariance queue the last insert call left for knn_cov_refs_kernel
     unsigned int min_id;              // far_map_renumber: smallest live id

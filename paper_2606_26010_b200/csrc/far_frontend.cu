@@ -36,7 +36,7 @@ struct far_frontend {
     far_gicp_result_t* d_result;
     cudaStream_t side;       // second stream: the downsampling branch runs beside the scan-local map build
     cudaStream_t side2;      // third: takes that role while `side` captures the frame graph
-    cudaEvent_t ev_fork, ev_join;
+    cudaEvent_t ev_fork, ev_join, ev_fork2, ev_join2;
     double* d_asmd;          // [2] n_close, number of close voxels (far_asmd_density)
     float* d_undist;         // undistorted sweep [max_scan_points * 3] (far_frontend_process_sweep)
     far_insert_stats_t* d_insert_stats;   // statistics of the frame's map update (far_frontend_insert_stats)
@@ -51,6 +51,7 @@ struct far_frontend {
     int graph_state;         // 0: not captured yet (the next frame with a repeated key captures), 1: usable, -1: capture refused
     const float* last_scan;  // key of the previous frame (a graph is captured when a key repeats)
     int last_stride;
+    int local_dirty;         // 1: a frame aborted between the scan-local insert and its clear (the next frame clears first)
     far_gicp_result_t* last_out;
 };
 
@@ -64,6 +65,8 @@ int far_frontend_destroy(far_frontend_t* f) {
     if (f->graph) cudaGraphDestroy(f->graph);
     if (f->ev_fork) cudaEventDestroy(f->ev_fork);
     if (f->ev_join) cudaEventDestroy(f->ev_join);
+    if (f->ev_fork2) cudaEventDestroy(f->ev_fork2);
+    if (f->ev_join2) cudaEventDestroy(f->ev_join2);
     if (f->side) cudaStreamDestroy(f->side);
     if (f->side2) cudaStreamDestroy(f->side2);
     cudaFree(f->d_ws); cudaFree(f->d_scan); cudaFree(f->d_ds_xyz); cudaFree(f->d_ds_index); cudaFree(f->d_n_ds);
@@ -116,6 +119,8 @@ int far_frontend_create(far_frontend_t** out, const far_frontend_config_t* cfg) 
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&f->side2, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&f->ev_fork, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&f->ev_join, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&f->ev_fork2, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&f->ev_join2, cudaEventDisableTiming);
     if (rc != FAR_OK || e != cudaSuccess) {
         if (e != cudaSuccess) far::set_cuda_error(e, "cudaMalloc in far_frontend_create");
         far_frontend_destroy(f);
@@ -160,27 +165,37 @@ static int frame_chain(far_frontend* f, const float* d_scan, int64_t n_cap, int 
     size_t ws = f->ws_bytes;
     FAR_STAGE(far::voxelize_impl(d_scan, n_cap, d_n, stride, f->cfg.ds_voxel, f->d_ds_xyz, f->d_ds_index, f->d_n_ds, f->d_ws, &ws, (void*)f->side));
     FAR_CUDA(cudaEventRecord(f->ev_join, f->side));
-    // A7: Sigma_s from a scan-local map of the raw scan
-    FAR_STAGE(far_map_clear(f->local, stream));
+    // A7: Sigma_s from a scan-local map of the raw scan.  The scan-local map is EMPTY here: it is created
+    // empty and every frame clears it again once it has been used (below, beside the submap update)
+    if (f->local_dirty) FAR_STAGE(far_map_clear(f->local, stream));
+    f->local_dirty = 1;
     FAR_STAGE(far::insert_impl(f->local, d_scan, n_cap, d_n, stride, 0, nullptr, nullptr, 0, nullptr, stream, nullptr, 1.0));
     FAR_CUDA(cudaStreamWaitEvent(st, f->ev_join, 0));
     if (n_cap > 0) FAR_STAGE(far_map_knn_cov_dev(f->local, f->d_ds_xyz, f->d_n_ds, n_cap, 3, f->d_cov6, f->d_valid, stream));
     // A6, A8-A10: registration from the predicted pose
     FAR_STAGE(far::gicp_launch(f->map, f->d_ds_xyz, f->d_cov6, f->d_valid, n_cap, f->d_n_ds, 3, nullptr, &f->d_fp->init, 0.0, &f->d_fp->sigma,
                                f->cfg.max_iters, 0, &f->cfg.gicp, res, stream));
+    const double* d_n_close = nullptr;
+    if (f->cfg.update_map && f->cfg.asmd) {
+        // density "in a close range of the current scan" = scan-local map about the sensor origin
+        const double origin[3] = {0.0, 0.0, 0.0};
+        FAR_STAGE(far_asmd_density(f->local, origin, f->cfg.asmd_r_close, f->d_asmd, stream));
+        d_n_close = f->d_asmd;
+    }
+    // the scan-local map has served: it is emptied for the next frame on the side stream, beside the submap update (off
+    // the critical path; forked AFTER the registration so that it never delays the cooperative launch)
+    FAR_CUDA(cudaEventRecord(f->ev_fork2, st));
+    FAR_CUDA(cudaStreamWaitEvent(f->side, f->ev_fork2, 0));
+    FAR_STAGE(far_map_clear(f->local, (void*)f->side));
+    FAR_CUDA(cudaEventRecord(f->ev_join2, f->side));
+    f->local_dirty = 0;
     // A3-A5, A7: submap update at the registered pose
     if (f->cfg.update_map) {
-        const double* d_n_close = nullptr;
-        if (f->cfg.asmd) {
-            // density "in a close range of the current scan" = scan-local map about the sensor origin
-            const double origin[3] = {0.0, 0.0, 0.0};
-            FAR_STAGE(far_asmd_density(f->local, origin, f->cfg.asmd_r_close, f->d_asmd, stream));
-            d_n_close = f->d_asmd;
-        }
         FAR_STAGE(far::insert_impl(f->map, d_scan, n_cap, d_n, stride, 2, nullptr, &res->pose, 1, f->d_insert_stats, stream, d_n_close,
                                    f->cfg.asmd_d_max));
         if (f->cfg.prune_radius > 0.0) FAR_STAGE(far_map_prune_dev(f->map, &res->pose, f->cfg.prune_radius, nullptr, stream));
     }
+    FAR_CUDA(cudaStreamWaitEvent(st, f->ev_join2, 0));
     return full ? FAR_ERR_FULL : FAR_OK;
 }
 
@@ -241,7 +256,7 @@ int far_frontend_process(far_frontend_t* f, const float* d_scan, int64_t n, int 
             FAR_CUDA(cudaGraphLaunch(f->gexec, st));
             far::launch_counter_add(f->g_kernels);
             if (f->cfg.update_map) { M->next_id_ub += (uint64_t)n_cap; M->offered_total += (uint64_t)n_cap; }
-            f->local->next_id_ub = (uint64_t)n_cap; f->local->offered_total = (uint64_t)n_cap; f->local->offered_at_renumber = 0;
+            f->local->next_id_ub = 0; f->local->offered_total = 0; f->local->offered_at_renumber = 0;     // inserted, then cleared
             return far_map_status(M);
         }
     }

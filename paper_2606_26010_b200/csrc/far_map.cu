@@ -19,8 +19,9 @@
 //
 // Storage (far_common.cuh): 16-byte table entries {key, bucket, count | reach}, buckets in a DENSE pool handed out by a
 // bump allocator + free list.  Pruning returns buckets at once and leaves dead keys behind; when their number passes a
-// device-side threshold the prune call's two follow-up kernels rebuild the entries into the shadow table and copy them
+// device-side threshold the prune call's follow-up kernel rebuilds the entries into the shadow table and copies them
 // back.  Nothing on this path allocates, frees or synchronises.
+#include <algorithm>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -595,55 +596,61 @@ __global__ void __launch_bounds__(SP_THREADS) spaced_commit_kernel(MapView m, co
 
 // ---- A5 prune (R5): thread per slot, FP64 squared centre distance, strict > -------------------
 // A removed voxel's bucket goes back to the free list at once (block-aggregated push) and its key stays as a dead key.
-// The last block writes the statistics and decides, from the number of dead keys, whether the two rehash kernels that
-// follow this one in the stream do their work or return immediately.
+// The last block writes the statistics and decides, from the number of dead keys, whether the rehash kernel that
+// follows this one in the stream does its work or returns immediately.
 __global__ void __launch_bounds__(256) prune_kernel(MapView m, double cx, double cy, double cz, const Pose* d_pose,
                                                      double r2, far_prune_stats_t* __restrict__ out) {
-    const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     unsigned long long vr = 0, pr = 0, vl = 0, pl = 0;
-    uint32_t freed = NO_BUCKET;
-    if (s < m.slots) {
-        const Entry e = m.table[s];
-        const uint32_t cnt = entry_count(e.cr);
-        if (e.key != KEY_EMPTY && e.bucket < BUCKET_PENDING && cnt > 0) {
-            if (d_pose) { cx = d_pose->t[0]; cy = d_pose->t[1]; cz = d_pose->t[2]; }
-            int k[3];
-            unpack_key(e.key, k);
-            const double v = (double)m.voxel;
-            const double dx = __dadd_rn(__dmul_rn(__dadd_rn((double)k[0], 0.5), v), -cx);
-            const double dy = __dadd_rn(__dmul_rn(__dadd_rn((double)k[1], 0.5), v), -cy);
-            const double dz = __dadd_rn(__dmul_rn(__dadd_rn((double)k[2], 0.5), v), -cz);
-            const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-            if (d2 > r2) {
-                // the id words go back to +inf so that the bucket's next owner starts clean
-                for (uint32_t j = 0; j < cnt; ++j) {
-                    m.ids[(size_t)e.bucket * m.cap + j] = NO_ID;
-                    if (m.cov_ok) m.cov_ok[(size_t)e.bucket * m.cap + j] = 0;
+    if (d_pose) { cx = d_pose->t[0]; cy = d_pose->t[1]; cz = d_pose->t[2]; }
+    const double v = (double)m.voxel;
+    // grid-stride over the table with one resident wave: the fence + ticket of the epilogue is paid once per block, and a
+    // block's statistics are summed in registers before they touch shared memory
+    for (uint32_t s0 = blockIdx.x * blockDim.x; s0 < m.slots; s0 += gridDim.x * blockDim.x) {
+        const uint32_t s = s0 + threadIdx.x;
+        uint32_t freed = NO_BUCKET;
+        if (s < m.slots) {
+            const Entry e = m.table[s];
+            const uint32_t cnt = entry_count(e.cr);
+            if (e.key != KEY_EMPTY && e.bucket < BUCKET_PENDING && cnt > 0) {
+                int k[3];
+                unpack_key(e.key, k);
+                const double dx = __dadd_rn(__dmul_rn(__dadd_rn((double)k[0], 0.5), v), -cx);
+                const double dy = __dadd_rn(__dmul_rn(__dadd_rn((double)k[1], 0.5), v), -cy);
+                const double dz = __dadd_rn(__dmul_rn(__dadd_rn((double)k[2], 0.5), v), -cz);
+                const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+                if (d2 > r2) {
+                    // the id words go back to +inf so that the bucket's next owner starts clean
+                    for (uint32_t j = 0; j < cnt; ++j) {
+                        m.ids[(size_t)e.bucket * m.cap + j] = NO_ID;
+                        if (m.cov_ok) m.cov_ok[(size_t)e.bucket * m.cap + j] = 0;
+                    }
+                    m.table[s].bucket = NO_BUCKET;
+                    m.table[s].cr = e.cr & ~0xFFu;
+                    freed = e.bucket;
+                    vr += 1; pr += cnt;
+                } else {
+                    vl += 1; pl += cnt;
                 }
-                m.table[s].bucket = NO_BUCKET;
-                m.table[s].cr = e.cr & ~0xFFu;
-                freed = e.bucket;
-                vr = 1; pr = cnt;
-            } else {
-                vl = 1; pl = cnt;
             }
         }
+        // free-list push: one atomic per warp that freed something (rare in a frame, every lane in a bulk prune)
+        const unsigned fm = __ballot_sync(FULL, freed != NO_BUCKET);
+        if (fm) {
+            uint32_t at = 0;
+            if (lane == 0) at = (uint32_t)atomicAdd(&m.ctr->n_free, (int)__popc(fm));
+            at = __shfl_sync(FULL, at, 0);
+            if (freed != NO_BUCKET) m.free_list[at + __popc(fm & ((1u << lane) - 1u))] = freed;
+        }
     }
-    // block-aggregate the free-list push and the four statistics: one atomic per block each
+    // block-aggregate the four statistics: one atomic per block each
     __shared__ unsigned long long s_acc[8][4];
-    __shared__ uint32_t s_wbase[8];
-    __shared__ uint32_t s_base;
-    const unsigned fm = __ballot_sync(FULL, freed != NO_BUCKET);
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) {
         vr += __shfl_xor_sync(FULL, vr, d); pr += __shfl_xor_sync(FULL, pr, d);
         vl += __shfl_xor_sync(FULL, vl, d); pl += __shfl_xor_sync(FULL, pl, d);
     }
-    if (lane == 0) {
-        s_acc[wib][0] = vr; s_acc[wib][1] = pr; s_acc[wib][2] = vl; s_acc[wib][3] = pl;
-        s_wbase[wib] = __popc(fm);
-    }
+    if (lane == 0) { s_acc[wib][0] = vr; s_acc[wib][1] = pr; s_acc[wib][2] = vl; s_acc[wib][3] = pl; }
     __syncthreads();
     if (threadIdx.x < 4) {
         unsigned long long t = 0;
@@ -651,14 +658,6 @@ __global__ void __launch_bounds__(256) prune_kernel(MapView m, double cx, double
         for (int w = 0; w < 8; ++w) t += s_acc[w][threadIdx.x];
         if (t) atomicAdd(&m.ctr->pr_vox_removed + threadIdx.x, t);
     }
-    if (threadIdx.x == 32) {
-        uint32_t tot = 0;
-#pragma unroll
-        for (int w = 0; w < 8; ++w) { const uint32_t c = s_wbase[w]; s_wbase[w] = tot; tot += c; }
-        s_base = tot ? (uint32_t)atomicAdd(&m.ctr->n_free, (int)tot) : 0u;
-    }
-    __syncthreads();
-    if (freed != NO_BUCKET) m.free_list[s_base + s_wbase[wib] + __popc(fm & ((1u << lane) - 1u))] = freed;
 
     if (last_block_done(&m.ctr->ticket[1]) && threadIdx.x == 0) {
         volatile Counters* c = m.ctr;
@@ -678,11 +677,12 @@ __global__ void __launch_bounds__(256) prune_kernel(MapView m, double cx, double
     }
 }
 
-// ---- in-place rehash (SURVEY.md:214-216: deletion in open addressing).  Pass 1 re-inserts every entry that owns a
-// bucket into the empty shadow table (16-byte entries only: buckets stay where they are) and recomputes the reach words;
-// pass 2 copies the shadow table back and empties it again.  Both return at once unless prune's epilogue (or
-// far_map_rehash) set the flag: the decision is taken on the device, the launches are unconditional.
-__global__ void __launch_bounds__(256) rehash_move_kernel(MapView m) {
+// ---- in-place rehash (SURVEY.md:214-216: deletion in open addressing), ONE cooperative kernel.  Pass 1 re-inserts every
+// entry that owns a bucket into the empty shadow table (16-byte entries only: buckets stay where they are) and recomputes
+// the reach words; a grid-wide barrier; pass 2 copies the shadow table back and empties it again.  The kernel returns at
+// once unless prune's epilogue (or far_map_rehash) set the flag: the decision is taken on the device, the launch is
+// unconditional.
+__global__ void __launch_bounds__(256) rehash_kernel(MapView m) {
     if (!m.ctr->rehash_flag) return;
     unsigned n_moved = 0;
     for (uint32_t s = blockIdx.x * blockDim.x + threadIdx.x; s < m.slots; s += gridDim.x * blockDim.x) {
@@ -698,20 +698,29 @@ __global__ void __launch_bounds__(256) rehash_move_kernel(MapView m) {
     }
     n_moved = __reduce_add_sync(FULL, n_moved);
     if (n_moved && (threadIdx.x & 31) == 0) atomicAdd(&m.ctr->rehash_moved, n_moved);
-}
-
-__global__ void __launch_bounds__(256) rehash_swap_kernel(MapView m) {
-    if (!m.ctr->rehash_flag) return;
+    // grid-wide barrier between the two passes (cooperative launch: every block is resident).  The arrival counter
+    // returns to zero by itself: the last block to LEAVE resets it.
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        atomicAdd(&m.ctr->rehash_barrier, 1u);
+        while (ld_volatile(&m.ctr->rehash_barrier) < gridDim.x) __nanosleep(64);
+        __threadfence();
+    }
+    __syncthreads();
     for (uint32_t s = blockIdx.x * blockDim.x + threadIdx.x; s < m.slots; s += gridDim.x * blockDim.x) {
         uint4* sh = reinterpret_cast<uint4*>(m.shadow + s);
         *reinterpret_cast<uint4*>(m.table + s) = *sh;
         *sh = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, BUCKET_PENDING, 0u);
     }
-    if (blockIdx.x == 0 && threadIdx.x == 0) {
-        m.ctr->n_keys = m.ctr->rehash_moved;
-        m.ctr->rehash_moved = 0u;
-        m.ctr->n_dead = 0u;
-        m.ctr->n_rehash += 1u;
+    if (last_block_done(&m.ctr->ticket[4]) && threadIdx.x == 0) {
+        volatile Counters* c = m.ctr;
+        c->n_keys = c->rehash_moved;
+        c->rehash_moved = 0u;
+        c->n_dead = 0u;
+        c->n_rehash = c->n_rehash + 1u;
+        c->rehash_barrier = 0u;
+        c->rehash_flag = 0u;
     }
 }
 
@@ -1175,11 +1184,22 @@ int far_asmd_density(const far_map_t* local, const double center[3], double r_cl
 static int rehash_enqueue(far_map_t* m, cudaStream_t st) {
     // grid-stride over the table with one resident wave: when the flag is clear (most frames) the launch costs a few
     // hundred empty blocks, not one per 256 slots
+    // ONE cooperative launch (the two passes are separated by a grid-wide barrier inside the kernel), sized to a resident
+    // wave: when the flag is clear (most frames) it costs a few hundred blocks that return at once
+    static int per_sm = 0;
+    if (per_sm == 0) {
+        int v = 0;
+        FAR_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, rehash_kernel, 256, 0));
+        per_sm = v < 1 ? 1 : (v > 4 ? 4 : v);
+    }
     int grid = grid_for(m->view.slots, 256);
-    if (grid > m->sm_count * 8) grid = m->sm_count * 8;
-    FAR_LAUNCH(rehash_move_kernel, grid, 256, 0, st, m->view);
-    FAR_LAUNCH(rehash_swap_kernel, grid, 256, 0, st, m->view);
-    FAR_CUDA(cudaGetLastError());
+    if (grid > m->sm_count * per_sm) grid = m->sm_count * per_sm;
+    MapView view = m->view;
+    void* args[] = {(void*)&view};
+    {
+        far::LaunchScope ls_("rehash_kernel", st);
+        FAR_CUDA(cudaLaunchCooperativeKernel((const void*)rehash_kernel, dim3((unsigned)grid), dim3(256), args, 0, st));
+    }
     return FAR_OK;
 }
 
@@ -1188,10 +1208,10 @@ static int prune_impl(far_map_t* m, const double* c, const far_pose_t* d_pose, d
     if (!m || (!c && !d_pose)) return FAR_ERR_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     const double r2 = radius * radius;
-    FAR_LAUNCH(prune_kernel, grid_for(m->view.slots, 256), 256, 0, st, m->view, c ? c[0] : 0.0, c ? c[1] : 0.0, c ? c[2] : 0.0,
+    FAR_LAUNCH(prune_kernel, std::min(grid_for(m->view.slots, 256), m->sm_count * 8), 256, 0, st, m->view, c ? c[0] : 0.0, c ? c[1] : 0.0, c ? c[2] : 0.0,
                                                                 (const Pose*)d_pose, r2, d_stats);
     FAR_CUDA(cudaGetLastError());
-    return rehash_enqueue(m, st);          // both kernels return at once unless prune's epilogue asked for the rebuild
+    return rehash_enqueue(m, st);          // returns at once unless prune's epilogue asked for the rebuild
 }
 
 int far_map_prune(far_map_t* m, const double center[3], double radius, far_prune_stats_t* d_stats, void* stream) {
@@ -1240,7 +1260,7 @@ int far_voxel_keys(const float* d_xyz, int64_t n, int stride, float voxel, uint6
     return FAR_OK;
 }
 
-// Drops the dead keys now, whatever their number: three stream-ordered launches, no allocation, no synchronisation.
+// Drops the dead keys now, whatever their number: two stream-ordered launches, no allocation, no synchronisation.
 // far_map_prune does the same by itself whenever the dead keys pass its threshold.
 int far_map_rehash(far_map_t* m, void* stream) {
     if (!m) return FAR_ERR_ARG;
