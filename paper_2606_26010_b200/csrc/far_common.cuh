@@ -35,6 +35,7 @@ constexpr uint32_t BUCKET_PENDING = 0xFFFFFFFEu;   // the bucket word of every E
                                                    // the thread that revives a dead key) is allocating the bucket right now
 constexpr int KEY_BIAS = 1 << 20;
 constexpr unsigned FULL = 0xFFFFFFFFu;
+constexpr uint32_t TOUCHED_SUBS = 32;             // sub-lists of the insert's touched list (far_map.cu)
 
 struct __align__(16) Entry {
     unsigned long long key;
@@ -59,7 +60,6 @@ struct Counters {
     unsigned int n_rehash;            // rehashes done since create / clear
     unsigned int ticket[6];           // last-block-done tickets: 0 insert commit, 1 prune, 2 clear, 3 renumber, 4 rehash
     unsigned int rehash_barrier;      // arrivals at the grid-wide barrier between the two passes of the rehash
-    unsigned int n_touched;           // voxels that received a first new point in the current chunk
     unsigned int n_tasks;             // length of the covariance queue the last insert call left for knn_cov_refs_kernel
     unsigned int min_id;              // far_map_renumber: smallest live id
     unsigned int n_cov;               // accepted points queued for covariance by the running insert call
@@ -87,6 +87,8 @@ struct MapView {
     uint32_t* free_list;
     Counters* ctr;
     Mailbox* mail;       // device pointer to the mapped host mailbox
+    uint32_t* touched_cnt;   // [TOUCHED_SUBS][32]: lengths of the sub-lists of the insert's touched list, one 128-byte line each
+    uint32_t touched_sub_cap;   // capacity of one sub-list
     uint32_t mask;       // slots - 1
     uint32_t slots;
     uint32_t max_buckets;

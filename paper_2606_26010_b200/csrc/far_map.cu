@@ -152,11 +152,18 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
                                                                   const int64_t* __restrict__ d_n, int stride, int pose_mode, Pose hpose,
                                                                   const Pose* __restrict__ d_pose, uint32_t id_offset,
                                                                   uint32_t* __restrict__ touched, Asmd asmd, Spaced sp) {
+    // Every counter of the map sits in one 128-byte line of L2, and the L2 retires about one atomic per 1.3 cycles on a line:
+    // one atomic per WARP and counter (3,656 warps for a 117k-point scan, six counters) held the whole kernel back by ~14 us.
+    // So everything is summed per BLOCK in shared memory first: the block draws its buckets with ONE atomic after a barrier
+    // that only waits for the lookups, and its statistics go out with one atomic each from whichever warp finishes last.
+    __shared__ uint32_t s_cnt[8];               // 0 buckets wanted, 1 new keys, 2 invalid, 3 opened, 4 dropped, 5 warps done, 6 draw base
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
     const Pose& T = (pose_mode == 2) ? *d_pose : hpose;
     Counters* ctr = m.ctr;
+    if (threadIdx.x < 8) s_cnt[threadIdx.x] = 0u;
+    __syncthreads();
     if (d_n) n = min(n, *d_n);                  // frame graph: launch sized for the largest scan, count on the device
     float p[3];
     int k[3] = {0, 0, 0};
@@ -193,7 +200,7 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
     const unsigned unresolved = __ballot_sync(FULL, !resolved);
     const bool is_leader = !resolved && (__ffs(same & unresolved) - 1) == lane;
     if (unresolved && is_leader) {
-        const bool may_claim = ld_volatile(&ctr->n_keys) < m.key_limit;    // enforced up to the keys claimed while this runs
+        const bool may_claim = ctr->n_keys < m.key_limit;                  // enforced up to the keys claimed while this runs
         Entry e;
         s = find_or_claim(m.table, m.mask, m.slots, key, may_claim, claimed, e);
         if (s != NO_SLOT) {
@@ -208,18 +215,26 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
             }
         }
     }
-    const unsigned newk = __ballot_sync(FULL, claimed);
-    if (newk && lane == 0) atomicAdd(&ctr->n_keys, (unsigned)__popc(newk));   // one atomic per warp, not one per key
-    // phase 2: the warp's allocators draw together: ONE atomic; the first n_free draws of a kernel come off the free list,
+    // phase 2: the BLOCK's allocators draw together: ONE atomic; the first n_free draws of a kernel come off the free list,
     // the rest from the fresh end of the pool (n_free and bump do not change while the kernel runs)
+    const unsigned newk = __ballot_sync(FULL, claimed);
     const unsigned wm = __ballot_sync(FULL, want);
+    uint32_t woff = 0;
+    if (lane == 0) {
+        if (newk) atomicAdd(&s_cnt[1], (uint32_t)__popc(newk));
+        if (wm) woff = atomicAdd(&s_cnt[0], (uint32_t)__popc(wm));
+    }
+    woff = __shfl_sync(FULL, woff, 0);
+    __syncthreads();                            // (nobody waits for anybody before this point: the lookups and claims only)
+    if (threadIdx.x == 0) {
+        if (s_cnt[0]) s_cnt[6] = atomicAdd(&ctr->n_alloc, s_cnt[0]);
+        if (s_cnt[1]) atomicAdd(&ctr->n_keys, s_cnt[1]);
+    }
+    __syncthreads();
     bool opened = false;
     if (wm) {
-        uint32_t a0 = 0;
-        if (lane == 0) a0 = atomicAdd(&ctr->n_alloc, (unsigned)__popc(wm));
-        a0 = __shfl_sync(FULL, a0, 0);
         if (want) {
-            const uint32_t a = a0 + __popc(wm & lt);
+            const uint32_t a = s_cnt[6] + woff + __popc(wm & lt);
             const uint32_t nf = (uint32_t)ctr->n_free;
             if (a < nf) b = m.free_list[nf - 1u - a];
             else {
@@ -247,17 +262,14 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
         }
     }
 
-    // statistics, one atomic per warp and counter
+    // statistics: per block in shared memory; flushed at the end of the kernel by the warp that finishes last
     const unsigned m_bad = __ballot_sync(FULL, bad);
     const unsigned m_drop = __ballot_sync(FULL, valid && b == NO_BUCKET);
     const unsigned m_open = __ballot_sync(FULL, opened);
     if (lane == 0) {
-        if (m_bad) atomicAdd(&ctr->st_invalid, (unsigned long long)__popc(m_bad));
-        if (m_open) atomicAdd(&ctr->st_new_voxels, (unsigned long long)__popc(m_open));
-        if (m_drop) {
-            atomicAdd(&ctr->st_dropped_full, (unsigned long long)__popc(m_drop));
-            ctr->full_flag = 1u;
-        }
+        if (m_bad) atomicAdd(&s_cnt[2], (uint32_t)__popc(m_bad));
+        if (m_open) atomicAdd(&s_cnt[3], (uint32_t)__popc(m_open));
+        if (m_drop) atomicAdd(&s_cnt[4], (uint32_t)__popc(m_drop));
     }
 
     // phase 4: the chain.  cap = this voxel's limit: the fixed cap, or N_ASMD (positions at and beyond it are never written)
@@ -294,16 +306,34 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
             }
         }
     }
+    // the touched list: TOUCHED_SUBS sub-lists with their counters on separate lines (a block appends to sub-list
+    // blockIdx mod TOUCHED_SUBS), so that this per-warp atomic meets ~1/32 of the grid on its line; the regular-spacing path
+    // wants one flat list (its scan kernel walks it) and keeps to sub-list 0
     const unsigned m_first = __ballot_sync(FULL, first_of_voxel);
     if (m_first) {
+        const uint32_t sub = sp.on ? 0u : (blockIdx.x % TOUCHED_SUBS);
         uint32_t at = 0;
-        if (lane == 0) at = atomicAdd(&ctr->n_touched, (unsigned)__popc(m_first));
+        if (lane == 0) at = atomicAdd(&m.touched_cnt[sub * 32u], (unsigned)__popc(m_first));
         at = __shfl_sync(FULL, at, 0);
         if (first_of_voxel) {
             const uint32_t t = at + __popc(m_first & lt);
-            touched[t] = s;
+            touched[(size_t)sub * m.touched_sub_cap + t] = s;
             if (sp.on) sp.voxel_t[b] = t;
         }
+    }
+    // the block's statistics: whichever warp finishes last sends them (no barrier: nobody waits for the slowest chain)
+    __syncwarp();
+    bool last_warp = false;
+    if (lane == 0) {
+        __threadfence_block();
+        last_warp = atomicAdd(&s_cnt[5], 1u) == (blockDim.x >> 5) - 1u;
+    }
+    if (__shfl_sync(FULL, (int)last_warp, 0) && lane == 0) {
+        __threadfence_block();
+        const uint32_t nb = *(volatile uint32_t*)&s_cnt[2], no = *(volatile uint32_t*)&s_cnt[3], nd = *(volatile uint32_t*)&s_cnt[4];
+        if (nb) atomicAdd(&ctr->st_invalid, (unsigned long long)nb);
+        if (no) atomicAdd(&ctr->st_new_voxels, (unsigned long long)no);
+        if (nd) { atomicAdd(&ctr->st_dropped_full, (unsigned long long)nd); ctr->full_flag = 1u; }
     }
 }
 
@@ -314,7 +344,7 @@ __device__ __forceinline__ void insert_epilogue(const MapView& m, int64_t n_call
     Counters* ctr = m.ctr;
     if (last_block_done(&ctr->ticket[0]) && threadIdx.x == 0) {
         volatile Counters* c = ctr;
-        c->n_touched = 0u;
+        for (uint32_t j = 0; j < TOUCHED_SUBS; ++j) m.touched_cnt[j * 32u] = 0u;
         if (last_chunk) { c->n_tasks = c->n_cov; c->n_cov = 0u; }
         {   // fold the kernel's bucket draws into the allocator state
             const unsigned drawn = c->n_alloc, nf = (unsigned)c->n_free;
@@ -357,12 +387,16 @@ __global__ void __launch_bounds__(256) insert_commit_kernel(MapView m, const flo
     const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
     const Pose& T = (pose_mode == 2) ? *d_pose : hpose;
     Counters* ctr = m.ctr;
-    const uint32_t n_touched = ctr->n_touched;
+    // warp w serves sub-list w mod TOUCHED_SUBS (the claim kernel dealt its blocks over the sub-lists: they are balanced)
+    const uint32_t sub_list = (uint32_t)(warp % TOUCHED_SUBS);
+    const int64_t per_list = nwarps / TOUCHED_SUBS;      // warps per sub-list (warps beyond per_list * TOUCHED_SUBS idle)
+    const uint32_t n_touched = warp < per_list * TOUCHED_SUBS ? m.touched_cnt[sub_list * 32u] : 0u;
+    touched += (size_t)sub_list * m.touched_sub_cap;
     const uint32_t first_id = (uint32_t)ctr->next_id + id_offset;
     const uint32_t cap = (uint32_t)m.cap;
     if (d_n) n_call = min(n_call, *d_n);
     unsigned long long acc_new = 0;                       // lane sl == 0 of each group: points accepted
-    for (int64_t t0 = warp * PER_WARP; t0 < n_touched; t0 += nwarps * PER_WARP) {
+    for (int64_t t0 = (warp / TOUCHED_SUBS) * PER_WARP; t0 < n_touched; t0 += per_list * PER_WARP) {
         const int64_t t = t0 + sub;
         const bool active = t < n_touched;
         uint32_t s = 0, b = 0, cr = 0, c0 = cap;
@@ -406,9 +440,15 @@ __global__ void __launch_bounds__(256) insert_commit_kernel(MapView m, const flo
             }
         }
     }
+    // accepted points: per block in shared memory, one atomic on the map's counter line per block
+    __shared__ unsigned long long s_accepted;
+    if (threadIdx.x == 0) s_accepted = 0ull;
+    __syncthreads();
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) acc_new += __shfl_xor_sync(FULL, acc_new, d);
-    if (lane == 0 && acc_new) atomicAdd(&ctr->st_accepted, acc_new);
+    if (lane == 0 && acc_new) atomicAdd(&s_accepted, acc_new);
+    __syncthreads();
+    if (threadIdx.x == 0 && s_accepted) atomicAdd(&ctr->st_accepted, s_accepted);
 
     insert_epilogue(m, n_call, last_chunk, d_stats);
 }
@@ -420,7 +460,7 @@ __global__ void __launch_bounds__(1024) spaced_scan_kernel(MapView m, const uint
     if (threadIdx.x == 0) s_carry = 0;
     __syncthreads();
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const uint32_t n_touched = m.ctr->n_touched;
+    const uint32_t n_touched = m.touched_cnt[0];              // regular spacing: the flat list = sub-list 0
     for (uint32_t base = 0; base < n_touched; base += 1024) {
         const uint32_t t = base + threadIdx.x;
         const uint32_t c = t < n_touched ? sp.offer_cnt[m.table[touched[t]].bucket] : 0u;
@@ -483,7 +523,7 @@ __global__ void __launch_bounds__(SP_THREADS) spaced_commit_kernel(MapView m, co
     Counters* ctr = m.ctr;
     if (d_n) { n_call = min(n_call, *d_n); n_chunk = min(n_chunk, *d_n); }
     const uint32_t first_id = (uint32_t)ctr->next_id + id_offset;
-    const uint32_t n_touched = ctr->n_touched;
+    const uint32_t n_touched = m.touched_cnt[0];
     const uint32_t cap = (uint32_t)m.cap;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     for (uint32_t t = blockIdx.x; t < n_touched; t += gridDim.x) {
@@ -986,7 +1026,9 @@ int far_map_create(far_map_t** out, const far_map_config_t* cfg) {
         alloc((void**)&v.cov_ok, npts);
     }
     alloc((void**)&v.ctr, sizeof(Counters));
-    alloc((void**)&m->d_touched, (size_t)c.max_batch * sizeof(uint32_t));
+    v.touched_sub_cap = (uint32_t)((((c.max_batch + 255) / 256 + TOUCHED_SUBS - 1) / TOUCHED_SUBS + 1) * 256);
+    alloc((void**)&m->d_touched, (size_t)TOUCHED_SUBS * v.touched_sub_cap * sizeof(uint32_t));
+    alloc((void**)&v.touched_cnt, (size_t)TOUCHED_SUBS * 32 * sizeof(uint32_t));
     alloc((void**)&m->d_cov_list, (size_t)c.max_batch * sizeof(uint4));
     if (c.min_spacing > 0.0) {            // scratch of the regular-spacing insert (R21)
         alloc((void**)&m->d_sp_cnt, (size_t)c.max_voxels * sizeof(uint32_t));
@@ -1015,6 +1057,7 @@ int far_map_create(far_map_t** out, const far_map_config_t* cfg) {
     z.min_id = NO_ID;
     FAR_CUDA(cudaMemcpy(v.ctr, &z, sizeof(z), cudaMemcpyHostToDevice));
     if (v.cov_ok) FAR_CUDA(cudaMemset(v.cov_ok, 0, npts));
+    FAR_CUDA(cudaMemset(v.touched_cnt, 0, (size_t)TOUCHED_SUBS * 32 * sizeof(uint32_t)));
     if (m->d_sp_cnt) FAR_CUDA(cudaMemset(m->d_sp_cnt, 0, (size_t)c.max_voxels * sizeof(uint32_t)));
     {
         const int rc = gicp_setup(m);
@@ -1029,7 +1072,7 @@ int far_map_destroy(far_map_t* m) {
     if (!m) return FAR_OK;
     cudaFree(m->view.table); cudaFree(m->view.shadow); cudaFree(m->view.points); cudaFree(m->view.ids);
     cudaFree(m->view.free_list); cudaFree(m->view.cov); cudaFree(m->view.cov_ok);
-    cudaFree(m->view.ctr); cudaFree(m->d_touched); cudaFree(m->d_cov_list);
+    cudaFree(m->view.ctr); cudaFree(m->d_touched); cudaFree(m->view.touched_cnt); cudaFree(m->d_cov_list);
     cudaFree(m->d_gicp_partials);
     cudaFree(m->d_sp_cnt); cudaFree(m->d_sp_vt); cudaFree(m->d_sp_ptb); cudaFree(m->d_sp_start); cudaFree(m->d_sp_seg);
     if (m->h_mail) cudaFreeHost((void*)m->h_mail);
