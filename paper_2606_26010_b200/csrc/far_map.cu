@@ -640,6 +640,8 @@ __global__ void __launch_bounds__(SP_THREADS) spaced_commit_kernel(MapView m, co
 // follows this one in the stream does its work or returns immediately.
 __global__ void __launch_bounds__(256) prune_kernel(MapView m, double cx, double cy, double cz, const Pose* d_pose,
                                                      double r2, far_prune_stats_t* __restrict__ out) {
+    __shared__ uint32_t s_wbase[8];
+    __shared__ uint32_t s_base;
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     unsigned long long vr = 0, pr = 0, vl = 0, pl = 0;
     if (d_pose) { cx = d_pose->t[0]; cy = d_pose->t[1]; cz = d_pose->t[2]; }
@@ -674,14 +676,20 @@ __global__ void __launch_bounds__(256) prune_kernel(MapView m, double cx, double
                 }
             }
         }
-        // free-list push: one atomic per warp that freed something (rare in a frame, every lane in a bulk prune)
+        // free-list push, aggregated over the block: ONE atomic on the map's counter line per block and pass (a bulk prune
+        // frees a bucket in almost every lane: one atomic per warp there is a million atomics on one line of L2)
         const unsigned fm = __ballot_sync(FULL, freed != NO_BUCKET);
-        if (fm) {
-            uint32_t at = 0;
-            if (lane == 0) at = (uint32_t)atomicAdd(&m.ctr->n_free, (int)__popc(fm));
-            at = __shfl_sync(FULL, at, 0);
-            if (freed != NO_BUCKET) m.free_list[at + __popc(fm & ((1u << lane) - 1u))] = freed;
+        if (lane == 0) s_wbase[wib] = __popc(fm);
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            uint32_t tot = 0;
+#pragma unroll
+            for (int w = 0; w < 8; ++w) { const uint32_t c = s_wbase[w]; s_wbase[w] = tot; tot += c; }
+            s_base = tot ? (uint32_t)atomicAdd(&m.ctr->n_free, (int)tot) : 0u;
         }
+        __syncthreads();
+        if (freed != NO_BUCKET) m.free_list[s_base + s_wbase[wib] + __popc(fm & ((1u << lane) - 1u))] = freed;
+        __syncthreads();                                    // s_wbase is rewritten by the next pass
     }
     // block-aggregate the four statistics: one atomic per block each
     __shared__ unsigned long long s_acc[8][4];
@@ -1233,7 +1241,7 @@ static int rehash_enqueue(far_map_t* m, cudaStream_t st) {
     if (per_sm == 0) {
         int v = 0;
         FAR_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, rehash_kernel, 256, 0));
-        per_sm = v < 1 ? 1 : (v > 4 ? 4 : v);
+        per_sm = v < 1 ? 1 : v;
     }
     int grid = grid_for(m->view.slots, 256);
     if (grid > m->sm_count * per_sm) grid = m->sm_count * per_sm;
