@@ -111,7 +111,7 @@ __device__ __forceinline__ double wait_tagged(const uint4* src, uint32_t tag) {
 }
 
 __device__ __forceinline__ double robust_weight(int kernel, double e2, double kappa) {
-    if (kernel == FAR_KERNEL_CAUCHY) return 1.0 / (1.0 + e2 / (kappa * kappa));          // Eq. 5 as IRLS weight (R9)
+    if (kernel == FAR_KERNEL_CAUCHY) { const double k2 = kappa * kappa; return k2 / (k2 + e2); }   // Eq. 5 as IRLS weight (R9): 1 / (1 + e2 / kappa^2), one division
     if (kernel == FAR_KERNEL_GEMAN_MCCLURE) { const double s = kappa + e2; return (kappa * kappa) / (s * s); }
     return 1.0;
 }
@@ -424,6 +424,11 @@ __global__ void __launch_bounds__(GTHREADS, GICP_BLOCKS_PER_SM) gicp_kernel(cons
     // what an iteration learns: the voxel the transformed point fell into with its 27 lookups (lane g: neighbours g + 8 j;
     // counts packed one byte each), the nearest neighbour (reference; coordinates and voxel in shared memory) and, in lanes
     // 0..6, that neighbour's covariance and flag
+    // this lane's entries of the term table, fetched once (a lane-dependent index into constant memory is replayed per
+    // distinct address: 16 replays per access inside the loop)
+    uint32_t enc[TERM_SLOTS];
+#pragma unroll
+    for (int q = 0; q < TERM_SLOTS; ++q) enc[q] = c_term_enc[(q < TERM_SLOTS - 1 ? q * GLANES + gl : 24 + (gl & 7)) & 31];
     uint32_t have = 0;                    // bit 0: the lookups are those of voxel kp; bit 1: the previous neighbour is set
     int kp0 = 0, kp1 = 0, kp2 = 0;
     uint32_t pcnt[NBR_PER_LANE], pbk[NBR_PER_LANE], pref = 0xFFFFFFFFu;
@@ -655,8 +660,7 @@ __global__ void __launch_bounds__(GTHREADS, GICP_BLOCKS_PER_SM) gicp_kernel(cons
             } else if (gl == 6) { u[U_MD] = Md0; u[U_MD + 1] = Md1; u[U_MD + 2] = Md2; u[U_E2] = e2; }
             else { u[U_P] = px; u[U_P + 1] = py; u[U_P + 2] = pz; u[U_ZERO] = 0.0; u[U_ONE] = 1.0; }
             __syncwarp(gmask);
-            auto term = [&](int slot_e, bool store_x) -> double {
-                const uint32_t en = c_term_enc[slot_e];
+            auto term = [&](uint32_t en, bool store_x) -> double {
                 const double val = u[en & 31u] * u[(en >> 5) & 31u] - u[(en >> 10) & 31u] * u[(en >> 15) & 31u];
                 const uint32_t xs = en >> 22;
                 if (store_x && xs) u[U_X + xs - 1] = val;
@@ -664,9 +668,9 @@ __global__ void __launch_bounds__(GTHREADS, GICP_BLOCKS_PER_SM) gicp_kernel(cons
                 return (ck == COEF_W ? wgt : (ck == COEF_MW ? -wgt : 1.0)) * val;
             };
 #pragma unroll
-            for (int q = 0; q < TERM_SLOTS - 1; ++q) if (q * GLANES + gl < 24) acc[q] += term(q * GLANES + gl, true);   // round 1
+            for (int q = 0; q < TERM_SLOTS - 1; ++q) if (q * GLANES + gl < 24) acc[q] += term(enc[q], true);   // round 1
             __syncwarp(gmask);                                      // the nine X are in u
-            if (gl < 8) acc[TERM_SLOTS - 1] += term(24 + gl, false);
+            if (gl < 8) acc[TERM_SLOTS - 1] += term(enc[TERM_SLOTS - 1], false);
             __syncwarp(gmask);                                      // u is rewritten by the group's next point
         }
         // ---- A10: lane-wise over the warp's 4 groups, over the block's warps, then block row -> group of 16 blocks -> grid

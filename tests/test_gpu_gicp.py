@@ -118,6 +118,46 @@ def test_insert_compute_cov_matches_oracle_across_batches():
     assert _rel_cov(ec["cov"][v], eo["cov"][v]).max() < 1e-4
 
 
+@pytest.mark.parametrize("voxel,cap,k", [(0.5, 20, 12), (1.0, 64, 10), (2.0, 64, 16), (0.5, 8, 3), (1.0, 33, 10)])
+def test_insert_compute_cov_task_kernel_paths(voxel, cap, k):
+    """The one-warp-per-touched-voxel covariance kernel off its main road: k > 10 (every query takes the warp-level exact
+    selection), cap 64 with voxels that receive more than 32 points in one call (two passes of queries, one lane per query),
+    small k, a cap that is not a multiple of 4 -- in two batches, both through the task list and through the oversize path."""
+    c1 = scenes.c1_tiny(seed=6, n_map=40_000)
+    pts = c1["map_points"]
+    mo = oracle.Map(voxel, cap, k_cov=k)
+    mg = far.Map(voxel, cap, 100_000, with_cov=True, k_cov=k)
+    mc = far.Map(voxel, cap, 100_000, with_cov=True, k_cov=k, max_batch=4096)      # oversize path: knn_cov_new_ids_kernel
+    for a, b in [(0, 25_000), (25_000, 40_000)]:
+        assert mg.insert(pts[a:b], compute_cov=True) == mo.insert(pts[a:b], compute_cov=True)
+        mc.insert(pts[a:b], compute_cov=True)
+    eo, eg, ec = mo.export(with_cov=True), mg.export(with_cov=True), mc.export(with_cov=True)
+    assert np.array_equal(eg["keys"], eo["keys"]) and np.array_equal(eg["ids"], eo["ids"])
+    assert np.array_equal(eg["cov_valid"], eo["cov_valid"]) and np.array_equal(ec["cov_valid"], eo["cov_valid"])
+    v = eo["cov_valid"].astype(bool)
+    assert v.any()
+    if cap == 64:
+        assert eo["counts"].max() > 32                                   # a voxel did receive more than a warp's worth
+    assert _rel_cov(eg["cov"][v], eo["cov"][v]).max() < 1e-4
+    assert _rel_cov(ec["cov"][v], eo["cov"][v]).max() < 1e-4
+
+
+def test_insert_compute_cov_on_a_lattice_with_distance_ties():
+    """Lattice points: every query has exact distance ties across its 10th..12th neighbours, so the coarse-key proof fails
+    everywhere and the exact selection (ties broken by the lowest id, R6) decides -- valid flags and covariances as the oracle's."""
+    g = np.arange(-6, 6, dtype=np.float32) * np.float32(0.25)
+    pts = np.stack(np.meshgrid(g, g, g[:6], indexing="ij"), axis=-1).reshape(-1, 3).astype(np.float32)
+    rng = np.random.default_rng(0)
+    pts = pts[rng.permutation(len(pts))]
+    mo, mg = oracle.Map(1.0, 20), far.Map(1.0, 20, 4096, with_cov=True)
+    assert mg.insert(pts, compute_cov=True) == mo.insert(pts, compute_cov=True)
+    eo, eg = mo.export(with_cov=True), mg.export(with_cov=True)
+    assert np.array_equal(eg["ids"], eo["ids"]) and np.array_equal(eg["cov_valid"], eo["cov_valid"])
+    v = eo["cov_valid"].astype(bool)
+    assert v.any()
+    assert _rel_cov(eg["cov"][v], eo["cov"][v]).max() < 1e-4
+
+
 # ---- A8-A10 ----------------------------------------------------------------------------------------------
 def test_single_correspondence_and_robust_weight_golden():
     g = load_golden("gicp_single_correspondence.json")
