@@ -2,7 +2,7 @@
  * far.h -- C ABI of the B200-native FAR-LIO front-end hot path (voxel hashmap + sparsity-aware GICP).
  *
  * Source of the method: /root/reference/PAPER.md (FAR-LIO, arxiv/paper_2606_26010), cited below as
- * PAPER.md:<line>.  Readings of passages the paper leaves open are numbered R1..R20 in DESIGN.md.
+ * PAPER.md:<line>.  Readings of passages the paper leaves open are numbered R1..R22 in DESIGN.md.
  * Every entry point below runs hand-written CUDA kernels for sm_100a; there is no CPU fallback.
  *
  * Conventions
