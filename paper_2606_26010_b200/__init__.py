@@ -210,8 +210,9 @@ def default_options(kernel=KERNEL_CAUCHY, conv_eps=5e-3, tau_mult=3.0, kappa_div
 
 
 def result_to_dict(res: GicpResult):
-    R, t = res.pose.to_rt()
-    return dict(R=R, t=t, H=np.array(res.H[:]).reshape(6, 6), b=np.array(res.b[:]), chi2=res.chi2,
+    # one copy of the 456-byte struct: 55 doubles (pose 12, H 36, b 6, chi2) then four int32
+    d = np.frombuffer(res, dtype=np.float64, count=55).copy()
+    return dict(R=d[0:9].reshape(3, 3), t=d[9:12], H=d[12:48].reshape(6, 6), b=d[48:54], chi2=float(d[54]),
                 n_inliers=res.n_inliers, iters=res.iters, converged=res.converged, status=res.status)
 
 

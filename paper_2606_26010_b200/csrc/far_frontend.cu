@@ -41,6 +41,8 @@ struct far_frontend {
     float* d_undist;         // undistorted sweep [max_scan_points * 3] (far_frontend_process_sweep)
     far_insert_stats_t* d_insert_stats;   // statistics of the frame's map update (far_frontend_insert_stats)
     FrameParams* d_fp;
+    FrameParams* h_fp;       // pinned staging of the frame parameters and of the result for the _host variant (which
+    far_gicp_result_t* h_res; //   synchronises every frame, so one slot each is enough): a pageable source or target makes the copy a slow one
     // the captured frame
     cudaGraph_t graph;
     cudaGraphExec_t gexec;
@@ -71,6 +73,8 @@ int far_frontend_destroy(far_frontend_t* f) {
     if (f->side2) cudaStreamDestroy(f->side2);
     cudaFree(f->d_ws); cudaFree(f->d_scan); cudaFree(f->d_ds_xyz); cudaFree(f->d_ds_index); cudaFree(f->d_n_ds);
     cudaFree(f->d_cov6); cudaFree(f->d_valid); cudaFree(f->d_result); cudaFree(f->d_asmd); cudaFree(f->d_undist); cudaFree(f->d_insert_stats); cudaFree(f->d_fp);
+    if (f->h_fp) cudaFreeHost(f->h_fp);
+    if (f->h_res) cudaFreeHost(f->h_res);
     delete f;
     return FAR_OK;
 }
@@ -115,6 +119,8 @@ int far_frontend_create(far_frontend_t** out, const far_frontend_config_t* cfg) 
     alloc((void**)&f->d_undist, (size_t)n * 3 * sizeof(float));
     alloc((void**)&f->d_insert_stats, sizeof(far_insert_stats_t));
     alloc((void**)&f->d_fp, sizeof(FrameParams));
+    if (e == cudaSuccess) e = cudaHostAlloc((void**)&f->h_fp, sizeof(FrameParams), cudaHostAllocDefault);
+    if (e == cudaSuccess) e = cudaHostAlloc((void**)&f->h_res, sizeof(far_gicp_result_t), cudaHostAllocDefault);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&f->side, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&f->side2, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&f->ev_fork, cudaEventDisableTiming);
@@ -201,16 +207,20 @@ static int frame_chain(far_frontend* f, const float* d_scan, int64_t n_cap, int 
 
 extern "C" {
 
-int far_frontend_process(far_frontend_t* f, const float* d_scan, int64_t n, int stride, const far_pose_t* init_pose,
-                         double sigma, far_gicp_result_t* d_out, void* stream) {
+}  // extern "C"
+
+// pinned_params: the caller synchronises before the next frame, so the parameters may go through the frontend's one
+// pinned slot (a truly asynchronous copy); otherwise they are staged by the runtime from the stack before the call returns
+static int frontend_process_impl(far_frontend_t* f, const float* d_scan, int64_t n, int stride, const far_pose_t* init_pose,
+                                 double sigma, far_gicp_result_t* d_out, void* stream, bool pinned_params) {
     if (!f || !init_pose || n < 0 || n > f->cfg.max_scan_points || (n > 0 && !d_scan) || (stride != 3 && stride != 4) || !(sigma > 0.0))
         return FAR_ERR_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     far_gicp_result_t* res = d_out ? d_out : f->d_result;
-    // this frame's parameters (a pageable source is staged by the runtime before the call returns)
     FrameParams hp;
-    hp.n = n; hp.init = *init_pose; hp.sigma = sigma;
-    FAR_CUDA(cudaMemcpyAsync(f->d_fp, &hp, sizeof(hp), cudaMemcpyHostToDevice, st));
+    FrameParams* src = pinned_params ? f->h_fp : &hp;
+    src->n = n; src->init = *init_pose; src->sigma = sigma;
+    FAR_CUDA(cudaMemcpyAsync(f->d_fp, src, sizeof(hp), cudaMemcpyHostToDevice, st));
     const int64_t n_cap = f->cfg.max_scan_points;
     far_map_t* M = f->map;
     // replay is possible when nothing the host decides per frame is due: id renumbering (R22) and the id-range check
@@ -263,6 +273,13 @@ int far_frontend_process(far_frontend_t* f, const float* d_scan, int64_t n, int 
     return frame_chain(f, d_scan, n_cap, stride, res, st);
 }
 
+extern "C" {
+
+int far_frontend_process(far_frontend_t* f, const float* d_scan, int64_t n, int stride, const far_pose_t* init_pose,
+                         double sigma, far_gicp_result_t* d_out, void* stream) {
+    return frontend_process_impl(f, d_scan, n, stride, init_pose, sigma, d_out, stream, false);
+}
+
 int far_frontend_process_sweep(far_frontend_t* f, const float* d_scan, const float* d_time, int64_t n, int stride, double dt_ref,
                                const far_motion_t* motion, const far_pose_t* init_pose, double sigma, far_gicp_result_t* d_out,
                                void* stream) {
@@ -277,10 +294,11 @@ int far_frontend_process_host(far_frontend_t* f, const float* h_scan, int64_t n,
     if (!f || !h_out || n < 0 || n > f->cfg.max_scan_points || (n > 0 && !h_scan) || (stride != 3 && stride != 4)) return FAR_ERR_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     if (n > 0) FAR_CUDA(cudaMemcpyAsync(f->d_scan, h_scan, (size_t)n * stride * sizeof(float), cudaMemcpyHostToDevice, st));
-    const int rc = far_frontend_process(f, f->d_scan, n, stride, init_pose, sigma, f->d_result, stream);
+    const int rc = frontend_process_impl(f, f->d_scan, n, stride, init_pose, sigma, f->d_result, stream, true);
     if (rc != FAR_OK && rc != FAR_ERR_FULL) return rc;
-    FAR_CUDA(cudaMemcpyAsync(h_out, f->d_result, sizeof(far_gicp_result_t), cudaMemcpyDeviceToHost, st));
+    FAR_CUDA(cudaMemcpyAsync(f->h_res, f->d_result, sizeof(far_gicp_result_t), cudaMemcpyDeviceToHost, st));
     FAR_CUDA(cudaStreamSynchronize(st));
+    memcpy(h_out, f->h_res, sizeof(far_gicp_result_t));
     return far_map_status(f->map);      // after the sync the mirrored flag is this frame's: FAR_ERR_FULL if it dropped points
 }
 
