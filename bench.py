@@ -214,6 +214,22 @@ def _hbm_peak():
     return 6650.0, "fallback 6650 GB/s (B200_PROFILING.md)"
 
 
+def _ncu(name):
+    """entry of profiles/ncu_traffic.json (committed `ncu --set full` captures; never measured live) or {}"""
+    try:
+        return json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json"))).get(name) or {}
+    except Exception:
+        return {}
+
+
+def _traffic_ratio(name, algorithmic_bytes_per_launch):
+    t = _ncu(name)
+    if not t.get("dram_bytes_per_launch") or not algorithmic_bytes_per_launch:
+        return None
+    return {"dram_bytes_per_launch": t["dram_bytes_per_launch"], "traffic_over_algorithmic": t["dram_bytes_per_launch"] / algorithmic_bytes_per_launch,
+            "issue_slots_busy_pct": t.get("issue_slots_busy_pct"), "l2_hit_pct": t.get("l2_hit_pct"), "bound": t.get("bound"), "capture": t.get("capture")}
+
+
 def _ev_ms(torch, fn):
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     a.record(); fn(); b.record(); torch.cuda.synchronize()
@@ -293,7 +309,12 @@ def _leg_c4(out, far, scenes, torch, peak):
                         "prune_slots_per_s": st["n_slots"] / (t_pr * 1e-3),
                         "prune_algorithmic_GBps": pr_bytes / (t_pr * 1e-3) / 1e9, "prune_frac_of_hbm_peak": pr_bytes / (t_pr * 1e-3) / 1e9 / peak,
                         "note": "prune_ms includes the in-place rehash that drops the dead keys of the removed voxels (two more "
-                                "passes over the table); nothing allocates or synchronises"}
+                                "passes over the table); nothing allocates or synchronises",
+                        # DRAM traffic of the committed captures (batch 90 of 100; the prune) over SURVEY 8(d)'s bytes per launch
+                        "ncu": {"insert_claim_chain_kernel": _traffic_ratio("insert_claim_chain_kernel@c4", 100_000 * 24),
+                                "insert_commit_kernel": _traffic_ratio("insert_commit_kernel@c4", st["n_points"] / 100 * 16),
+                                "prune_kernel": _traffic_ratio("prune_kernel@c4", pr_bytes),
+                                "rehash_kernel": _traffic_ratio("rehash_kernel@c4", st["n_slots"] * 32)}}
     mg.close(); del pts
 
 
@@ -321,6 +342,11 @@ def _leg_c5(out, far, scenes, torch, peak, flush, voxels=(0.25, 0.5, 1.0, 2.0)):
             nb = algorithmic_bytes("nn_kernel", 1_000_000, cq, oq)
             row[name] = {"queries_per_s": 1e6 / t, "ms": t * 1e3, "candidates_per_query": cq, "occupied_voxels_per_query": oq,
                          "algorithmic_GBps": nb / t / 1e9, "frac_of_hbm_peak": nb / t / 1e9 / peak}
+            if name == "random":
+                tr = _traffic_ratio(f"nn_kernel@c5_v{v}", nb)
+                if tr:
+                    tr["dram_frac_of_hbm_peak"] = tr["dram_bytes_per_launch"] / t / 1e9 / peak    # capture's bytes over this run's time
+                    row[name]["ncu"] = tr
         out["c5_nn"][f"v={v}"] = row
         mg.close()
     del d_pts

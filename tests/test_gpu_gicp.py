@@ -235,6 +235,30 @@ def test_register_matches_oracle_c1(kernel):
     assert dt < 0.01 and dr < math.radians(0.1)
 
 
+@pytest.mark.parametrize("n_scan", [5921, 12_000, 40_003])
+def test_register_more_source_points_than_the_grid_holds_at_once(n_scan):
+    """gicp_kernel keeps one source point per 16-lane group while the scan fits the grid (148 blocks x 40 points on a
+    B200); beyond that it serves the points in rounds and fetches them again every iteration.  Linearisation and the whole
+    registration against the oracle on scans of one point past that limit, two rounds and seven rounds, stride 3 and 4."""
+    c1 = scenes.c1_tiny(seed=7, n_map=30_000, n_scan=n_scan)
+    mo, mg = _build_pair(c1["map_points"], c1["voxel"], c1["cap"])
+    (cov_o, val_o), (cov_g, val_g) = _scan_cov(c1["scan"], c1["scan"], c1["voxel"], c1["cap"])
+    lo = mo.gicp_linearize(c1["scan"], cov_o, val_o, c1["T_init"], c1["sigma"], oracle.default_options())
+    lg = mg.gicp_linearize(c1["scan"], cov_g, val_g, c1["T_init"], c1["sigma"], far.default_options())
+    assert lg["n_inliers"] == lo["n_inliers"] > n_scan // 2
+    eh, eb = _hb_err(lg, lo, np.linalg.norm(lo["H"]))
+    assert eh < 1e-4 and eb < 1e-4
+    o = mo.gicp_register(c1["scan"], cov_o, val_o, c1["T_init"], c1["sigma"], c1["max_iters"], oracle.default_options(), nthreads=16)
+    g = mg.gicp_register(c1["scan"], cov_g, val_g, c1["T_init"], c1["sigma"], c1["max_iters"], far.default_options())
+    assert g["status"] == o["status"] == 0 and g["iters"] == o["iters"] and g["converged"] == o["converged"] == 1
+    assert g["n_inliers"] == o["n_inliers"]
+    dt, dr = _pose_err(g, o)
+    assert dt < 1e-4 and dr < 1e-5
+    scan4 = np.concatenate([c1["scan"], np.full((n_scan, 1), 7.0, np.float32)], axis=1)
+    g4 = mg.gicp_register(scan4, cov_g, val_g, c1["T_init"], c1["sigma"], c1["max_iters"], far.default_options())
+    assert g4["iters"] == g["iters"] and np.array_equal(g4["t"], g["t"]) and np.array_equal(g4["H"], g["H"])
+
+
 def test_noise_free_recovery_and_point_to_point():
     c1 = scenes.c1_tiny(seed=0, noise_free=True)
     mo, mg = _build_pair(c1["map_points"], c1["voxel"], c1["cap"])
