@@ -110,7 +110,8 @@ void far_gicp_default_options(far_gicp_options_t* out);
 
 /* ---- voxel hashmap: PAPER.md:62-68 (cuVoxelMap, Fig. 3), :109 (local submap) -------------------------
  * Open addressing with linear probing on packed 64-bit voxel keys (R1: k = floor(fp32 p / fp32 v), three
- * 21-bit biased indices), one fixed bucket of `cap` float4 (x,y,z,id bits) per table slot.
+ * 21-bit biased indices); 16-byte table entries {key, bucket, count}; buckets of `cap` float4 (x,y,z,id bits) in a dense
+ * pool of max_voxels buckets (bump allocator + free list refilled by far_map_prune).
  * far_map_create allocates and initialises all device memory on the current device and synchronises. */
 int far_map_create(far_map_t** out, const far_map_config_t* cfg);
 int far_map_destroy(far_map_t* map);
@@ -126,7 +127,7 @@ int far_map_clear(far_map_t* map, void* stream);
  * d_stats (nullable, device) is overwritten with the totals of this call.
  * Returns FAR_ERR_RANGE (nothing inserted) if the id counter cannot take n more ids, FAR_ERR_FULL (work enqueued) as
  * described at the enum; the exact drop count of this call is d_stats->n_dropped_full.  Two launches per max_batch
- * chunk (+ one for the covariances); this call itself does not synchronise. */
+ * chunk (+ one for the covariances, served voxel by voxel from a task list the commit kernel leaves); this call itself does not synchronise. */
 int far_map_insert(far_map_t* map, const float* d_xyz, int64_t n, int stride, const far_pose_t* pose_or_null,
                    int compute_cov, far_insert_stats_t* d_stats, void* stream);
 int far_map_insert_dev(far_map_t* map, const float* d_xyz, int64_t n, int stride, const far_pose_t* d_pose,

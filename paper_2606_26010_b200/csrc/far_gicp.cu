@@ -58,7 +58,7 @@ constexpr int NBR_PER_LANE = (27 + GLANES - 1) / GLANES;   // neighbour voxels a
 constexpr int SWEEP_U = 32 / GLANES;                      // candidate loads in flight per lane: 32 per group and round trip
 constexpr int TERM_SLOTS = (24 + GLANES - 1) / GLANES + 1;               // term columns per lane: entries g, g + GLANES, .. < 24, then 24 + g
 constexpr int GICP_BLOCKS_PER_SM = 1;
-constexpr int NTERMS = 29;                // 21 (H upper triangle) + 6 (b) + chi2 + inlier count
+// (a row of the reduction carries 29 terms: 21 of H's upper triangle, 6 of b, chi2, inlier count; 3 columns idle)
 constexpr int TSTRIDE = 32;               // row length of the tagged rows in global memory
 constexpr int GROUP = 16;                 // blocks per first-level reduction group (one hop over all 148 rows measured 2 % slower)
 constexpr int MAX_GROUPS = 64;

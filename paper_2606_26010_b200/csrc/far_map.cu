@@ -517,7 +517,6 @@ __global__ void __launch_bounds__(SP_THREADS) spaced_commit_kernel(MapView m, co
                                                                    far_insert_stats_t* __restrict__ d_stats, Asmd asmd, Spaced sp) {
     __shared__ uint32_t s_buf[SP_SORT];
     __shared__ float4 s_pts[64];
-    __shared__ uint32_t s_acc[64];       // positions accepted in this voxel (for the covariance queue)
     __shared__ uint32_t s_count, s_n, s_nacc;
     const Pose& T = (pose_mode == 2) ? *d_pose : hpose;
     Counters* ctr = m.ctr;
@@ -607,7 +606,6 @@ __global__ void __launch_bounds__(SP_THREADS) spaced_commit_kernel(MapView m, co
                             m.points[(size_t)b * cap + count] = np;
                             m.ids[(size_t)b * cap + count] = id;
                             if (m.cov_ok) m.cov_ok[(size_t)b * cap + count] = 0;
-                            s_acc[nacc] = count;
                             pass = false;
                         }
                         ++count; ++nacc;
