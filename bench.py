@@ -731,6 +731,7 @@ def run_far(args):
                    "occupied_voxels_per_query_27": {"gicp": occ_gicp, "knn_cov_refs": occ_refs, "knn_cov_points": occ_pts}},
         "clocks": sampler.summary(),
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": 1e3 * e2e_total / Ke, "steps": Ke,
+                "ms_median": 1e3 * float(np.median(e2e_t)), "ms_min": 1e3 * float(np.min(e2e_t)), "ms_max": 1e3 * float(np.max(e2e_t)),
                 "h2d_bytes_per_step": int(scan.nbytes + 96), "d2h_bytes_per_step": int(far.GICP_RESULT_BYTES)},
         "gpu_launches": int(launches),
         "frame_graph": {"state": graph_state, "note": "1 = every timed frame was one cudaGraphLaunch of the captured chain"},

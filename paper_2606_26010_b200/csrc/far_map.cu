@@ -645,12 +645,25 @@ __global__ void __launch_bounds__(256) prune_kernel(MapView m, double cx, double
     if (d_pose) { cx = d_pose->t[0]; cy = d_pose->t[1]; cz = d_pose->t[2]; }
     const double v = (double)m.voxel;
     // grid-stride over the table with one resident wave: the fence + ticket of the epilogue is paid once per block, and a
-    // block's statistics are summed in registers before they touch shared memory
-    for (uint32_t s0 = blockIdx.x * blockDim.x; s0 < m.slots; s0 += gridDim.x * blockDim.x) {
-        const uint32_t s = s0 + threadIdx.x;
-        uint32_t freed = NO_BUCKET;
-        if (s < m.slots) {
-            const Entry e = m.table[s];
+    // block's statistics are summed in registers before they touch shared memory.  A thread takes PRUNE_U slots per pass,
+    // their entries requested together (a 16-byte load per thread and pass left the kernel waiting on one DRAM round trip
+    // after the other: 0.6 TB/s on a frame-sized table)
+    constexpr int PRUNE_U = 4;
+    for (uint32_t s0 = blockIdx.x * blockDim.x * PRUNE_U; s0 < m.slots; s0 += gridDim.x * blockDim.x * PRUNE_U) {
+        Entry ent[PRUNE_U];
+#pragma unroll
+        for (int u = 0; u < PRUNE_U; ++u) {
+            const uint32_t s = s0 + u * blockDim.x + threadIdx.x;
+            ent[u].key = KEY_EMPTY; ent[u].bucket = NO_BUCKET; ent[u].cr = 0;
+            if (s < m.slots) ent[u] = m.table[s];
+        }
+        uint32_t freed[PRUNE_U];
+        bool any_freed = false;
+#pragma unroll
+        for (int u = 0; u < PRUNE_U; ++u) {
+            const uint32_t s = s0 + u * blockDim.x + threadIdx.x;
+            const Entry e = ent[u];
+            freed[u] = NO_BUCKET;
             const uint32_t cnt = entry_count(e.cr);
             if (e.key != KEY_EMPTY && e.bucket < BUCKET_PENDING && cnt > 0) {
                 int k[3];
@@ -667,7 +680,8 @@ __global__ void __launch_bounds__(256) prune_kernel(MapView m, double cx, double
                     }
                     m.table[s].bucket = NO_BUCKET;
                     m.table[s].cr = e.cr & ~0xFFu;
-                    freed = e.bucket;
+                    freed[u] = e.bucket;
+                    any_freed = true;
                     vr += 1; pr += cnt;
                 } else {
                     vl += 1; pl += cnt;
@@ -675,19 +689,27 @@ __global__ void __launch_bounds__(256) prune_kernel(MapView m, double cx, double
             }
         }
         // free-list push, aggregated over the block: ONE atomic on the map's counter line per block and pass (a bulk prune
-        // frees a bucket in almost every lane: one atomic per warp there is a million atomics on one line of L2)
-        const unsigned fm = __ballot_sync(FULL, freed != NO_BUCKET);
-        if (lane == 0) s_wbase[wib] = __popc(fm);
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            uint32_t tot = 0;
+        // frees a bucket in almost every lane: one atomic per warp there is a million atomics on one line of L2); a pass
+        // that frees nothing -- nearly every pass of a frame's prune -- costs one barrier
+        if (__syncthreads_or(any_freed)) {
+            uint32_t mine = 0;
 #pragma unroll
-            for (int w = 0; w < 8; ++w) { const uint32_t c = s_wbase[w]; s_wbase[w] = tot; tot += c; }
-            s_base = tot ? (uint32_t)atomicAdd(&m.ctr->n_free, (int)tot) : 0u;
+            for (int u = 0; u < PRUNE_U; ++u) mine += freed[u] != NO_BUCKET;
+            const uint32_t incl = (uint32_t)warp_incl_scan((int)mine, lane);
+            if (lane == 31) s_wbase[wib] = incl;
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                uint32_t tot = 0;
+#pragma unroll
+                for (int w = 0; w < 8; ++w) { const uint32_t c = s_wbase[w]; s_wbase[w] = tot; tot += c; }
+                s_base = tot ? (uint32_t)atomicAdd(&m.ctr->n_free, (int)tot) : 0u;
+            }
+            __syncthreads();
+            uint32_t at = s_base + s_wbase[wib] + incl - mine;
+#pragma unroll
+            for (int u = 0; u < PRUNE_U; ++u) if (freed[u] != NO_BUCKET) m.free_list[at++] = freed[u];
+            __syncthreads();                                // s_wbase is rewritten by the next pass
         }
-        __syncthreads();
-        if (freed != NO_BUCKET) m.free_list[s_base + s_wbase[wib] + __popc(fm & ((1u << lane) - 1u))] = freed;
-        __syncthreads();                                    // s_wbase is rewritten by the next pass
     }
     // block-aggregate the four statistics: one atomic per block each
     __shared__ unsigned long long s_acc[8][4];
@@ -1257,7 +1279,7 @@ static int prune_impl(far_map_t* m, const double* c, const far_pose_t* d_pose, d
     if (!m || (!c && !d_pose)) return FAR_ERR_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     const double r2 = radius * radius;
-    FAR_LAUNCH(prune_kernel, std::min(grid_for(m->view.slots, 256), m->sm_count * 8), 256, 0, st, m->view, c ? c[0] : 0.0, c ? c[1] : 0.0, c ? c[2] : 0.0,
+    FAR_LAUNCH(prune_kernel, std::min(grid_for(m->view.slots, 256 * 4), m->sm_count * 8), 256, 0, st, m->view, c ? c[0] : 0.0, c ? c[1] : 0.0, c ? c[2] : 0.0,
                                                                 (const Pose*)d_pose, r2, d_stats);
     FAR_CUDA(cudaGetLastError());
     return rehash_enqueue(m, st);          // returns at once unless prune's epilogue asked for the rebuild

@@ -508,17 +508,24 @@ __device__ __forceinline__ bool warp_knn_cov(const MapView& m, float qx, float q
     return true;
 }
 
-__host__ __device__ inline size_t knn_warp_bytes(int k) { return (size_t)32 * k * sizeof(Cand) + (size_t)(3 * k + 9) * sizeof(double) + 8 + sizeof(CandList); }
+// per-warp shared memory of mapping (b).  The candidate list comes last, only as many of its step masks as this cap
+// needs are allocated, and the moments of Eq. 1 later take its place: at k = 10, cap 20 a warp then takes 5.4 KB, five 8-warp blocks fit an SM, and the 5,352 queries of
+// a C2 frame run as ONE wave of 5,920 warps (at 5.9 KB it was four blocks: 4,736 warps and a second wave for the rest)
+__host__ __device__ inline size_t knn_warp_bytes(int k, int cap) {
+    const size_t mask_words = ((size_t)27 * cap + 31) / 32;
+    const size_t list = sizeof(CandList) - (CAND_STEPS - mask_words) * sizeof(uint32_t), mom = (size_t)(3 * k + 9) * sizeof(double);
+    return (size_t)32 * k * sizeof(Cand) + (list > mom ? list : mom);      // the moments reuse the list's place: it has served by then
+}
 
 // queries given as points (far_map_knn_cov); n read from the device if d_n != nullptr
 __global__ void __launch_bounds__(256, 5) knn_cov_points_kernel(MapView m, const float* __restrict__ q, int64_t n, const int64_t* __restrict__ d_n,
                                       int stride, float* __restrict__ cov6, uint8_t* __restrict__ valid, int warps_per_block) {
     extern __shared__ __align__(16) char smem[];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    char* wbase = smem + (size_t)wib * ((knn_warp_bytes(m.k_cov) + 15) & ~(size_t)15);
+    char* wbase = smem + (size_t)wib * ((knn_warp_bytes(m.k_cov, m.cap) + 15) & ~(size_t)15);
     Cand* col = reinterpret_cast<Cand*>(wbase);
     double* mom = reinterpret_cast<double*>(wbase + (size_t)32 * m.k_cov * sizeof(Cand));
-    CandList& L = *reinterpret_cast<CandList*>(wbase + (((size_t)32 * m.k_cov * sizeof(Cand) + (size_t)(3 * m.k_cov + 9) * sizeof(double)) + 15 & ~(size_t)15));
+    CandList& L = *reinterpret_cast<CandList*>(wbase + (size_t)32 * m.k_cov * sizeof(Cand));
     if (d_n) n = min(n, *d_n);
     const int64_t nwarps = (int64_t)gridDim.x * warps_per_block;
     for (int64_t i = (int64_t)blockIdx.x * warps_per_block + wib; i < n; i += nwarps) {
@@ -532,33 +539,35 @@ __global__ void __launch_bounds__(256, 5) knn_cov_points_kernel(MapView m, const
 
 struct KnnLaunch { int warps, grid; size_t smem; };
 
-// The shared-memory opt-in and the occupancy query are slow host calls: done once per (kernel, k_cov, device) and cached
-// (the frame chain launches two of these kernels per scan).
+// The shared-memory opt-in and the occupancy query are slow host calls: done once per (kernel, bytes per warp, device) and
+// cached (the frame chain launches two of these kernels per scan).
 template <class K>
-static int knn_launch_cfg(const far_map* map, K kernel, size_t per_warp, int64_t work_warps, KnnLaunch& L, int cache_key) {
-    struct Cached { bool have; int warps, per_sm; size_t smem; };
-    static Cached cache[65][8] = {};          // one table per kernel instantiation; key = what sizes the warp's shared memory
+static int knn_launch_cfg(const far_map* map, K kernel, size_t per_warp, int64_t work_warps, KnnLaunch& L) {
+    struct Cached { size_t per_warp; int dev; int warps, per_sm; size_t smem; };
+    static Cached cache[16] = {};             // one table per kernel instantiation
+    static int n_cached = 0;
     static size_t attr_bytes[8] = {};         // largest dynamic shared-memory opt-in made for this kernel, per device
-    const int dev = map->device & 7;
-    Cached& c = cache[cache_key][dev];
-    if (!c.have || map->device >= 8) {
-        per_warp = (per_warp + 15) & ~(size_t)15;
+    per_warp = (per_warp + 15) & ~(size_t)15;
+    const int dev = map->device;
+    Cached fresh;
+    Cached* hit = nullptr;
+    for (int q = 0; q < n_cached; ++q) if (cache[q].per_warp == per_warp && cache[q].dev == dev) hit = &cache[q];
+    if (!hit) {
         int warps = (int)(100 * 1024 / per_warp);
         if (warps > 8) warps = 8;
         if (warps < 1) warps = 1;
-        c.warps = warps;
-        c.smem = per_warp * warps;
-        c.have = false;
+        fresh.per_warp = per_warp; fresh.dev = dev; fresh.warps = warps; fresh.smem = per_warp * warps; fresh.per_sm = 0;
     }
-    if (c.smem > attr_bytes[dev]) {           // the opt-in is per function: only ever raise it
+    Cached& c = hit ? *hit : fresh;
+    if (c.smem > attr_bytes[dev & 7] || dev >= 8) {   // the opt-in is per function: only ever raise it
         FAR_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem));
-        attr_bytes[dev] = c.smem;
+        attr_bytes[dev & 7] = c.smem;
     }
-    if (!c.have) {
+    if (!hit) {
         int per_sm = 0;
         FAR_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, c.warps * 32, c.smem));
         c.per_sm = per_sm < 1 ? 1 : per_sm;
-        c.have = true;
+        if (n_cached < 16) cache[n_cached++] = c;
     }
     L.warps = c.warps; L.smem = c.smem;
     int64_t grid = (int64_t)map->sm_count * c.per_sm;
@@ -571,7 +580,7 @@ static int knn_launch_cfg(const far_map* map, K kernel, size_t per_warp, int64_t
 
 int launch_knn_cov_refs(const far_map* map, const uint32_t* d_tasks, const unsigned int* d_n, int64_t n_max, cudaStream_t st) {
     KnnLaunch L;
-    int rc = knn_launch_cfg(map, knn_cov_refs_kernel, cov_task_bytes(map->view.cap), n_max, L, map->view.cap);
+    int rc = knn_launch_cfg(map, knn_cov_refs_kernel, cov_task_bytes(map->view.cap), n_max, L);
     if (rc != FAR_OK) return rc;
     FAR_LAUNCH(knn_cov_refs_kernel, L.grid, L.warps * 32, L.smem, st, map->view, reinterpret_cast<const uint4*>(d_tasks), d_n, L.warps);
     FAR_CUDA(cudaGetLastError());
@@ -580,7 +589,7 @@ int launch_knn_cov_refs(const far_map* map, const uint32_t* d_tasks, const unsig
 
 int launch_knn_cov_new_ids(const far_map* map, cudaStream_t st) {
     KnnLaunch L;
-    int rc = knn_launch_cfg(map, knn_cov_new_ids_kernel, cov_task_bytes(map->view.cap), (map->view.slots + 31) / 32, L, map->view.cap);
+    int rc = knn_launch_cfg(map, knn_cov_new_ids_kernel, cov_task_bytes(map->view.cap), (map->view.slots + 31) / 32, L);
     if (rc != FAR_OK) return rc;
     FAR_LAUNCH(knn_cov_new_ids_kernel, L.grid, L.warps * 32, L.smem, st, map->view, L.warps);
     FAR_CUDA(cudaGetLastError());
@@ -627,7 +636,7 @@ static int knn_cov_impl(const far_map_t* map, const float* d_q, int64_t m, const
     if (!map || m < 0 || (stride != 3 && stride != 4) || (m > 0 && (!d_q || !d_cov6 || !d_valid))) return FAR_ERR_ARG;
     if (m == 0) return FAR_OK;
     KnnLaunch L;
-    int rc = knn_launch_cfg(map, knn_cov_points_kernel, knn_warp_bytes(map->view.k_cov), m, L, map->view.k_cov);
+    int rc = knn_launch_cfg(map, knn_cov_points_kernel, knn_warp_bytes(map->view.k_cov, map->view.cap), m, L);
     if (rc != FAR_OK) return rc;
     FAR_LAUNCH(knn_cov_points_kernel, L.grid, L.warps * 32, L.smem, (cudaStream_t)stream, map->view, d_q, m, d_m, stride, d_cov6,
                                                                                   d_valid, L.warps);
