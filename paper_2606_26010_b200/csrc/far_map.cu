@@ -76,11 +76,12 @@ __device__ __forceinline__ void raise_reach(Entry* table, uint32_t h, uint32_t r
 // harmless, a stale half only sends the caller through the slower path).  Returns NO_SLOT if the key is absent and the
 // table takes no more keys; `e` = the entry as seen (bucket = BUCKET_PENDING on a slot claimed just now).
 __device__ __forceinline__ uint32_t find_or_claim(Entry* table, uint32_t mask, uint32_t slots, unsigned long long key,
-                                                  bool may_claim, bool& claimed, Entry& e) {
+                                                  bool may_claim, bool& claimed, Entry& e, uint32_t first_probe = 0) {
+    // first_probe: slots h .. h + first_probe - 1 are known to hold other keys (keys never leave a slot while inserts run)
     const uint32_t h = hash_key(key) & mask;
-    uint32_t s = h;
+    uint32_t s = (h + first_probe) & mask;
     claimed = false;
-    for (uint32_t probes = 0; probes < slots; ++probes) {
+    for (uint32_t probes = first_probe; probes < slots; ++probes) {
         e = ld_entry_volatile(table + s);
         if (e.key == KEY_EMPTY) {
             if (!may_claim || probes >= 0xFFFFFEu) return NO_SLOT;
@@ -183,6 +184,10 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
     uint32_t s = NO_SLOT, b = NO_BUCKET, c0 = 0;
     bool claimed = false, want = false, resolved = !valid;
     const uint32_t id_base = (uint32_t)ctr->next_id + id_offset;           // requested early: needed by the chain only
+    uint32_t walked = 0;                        // slots of the read-only walk that held OTHER keys: the claim resumes behind them
+    // the allocator's state does not change while the kernel runs: fetched now, with the id counter (same line), not when
+    // a bucket is drawn
+    const uint32_t nf = (uint32_t)ctr->n_free, bump0 = ctr->bump;
     if (valid) {
         uint32_t t = hash_key(key) & m.mask;
         for (uint32_t probes = 0; probes < m.slots; ++probes) {
@@ -193,6 +198,7 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
             }
             if (e.key == KEY_EMPTY) break;
             t = (t + 1) & m.mask;
+            walked = probes + 1;
         }
     }
     // phase 1b (only warps with an unresolved lane): the voxel is new, dead or being opened by someone else.  One leader
@@ -202,7 +208,7 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
     if (unresolved && is_leader) {
         const bool may_claim = ctr->n_keys < m.key_limit;                  // enforced up to the keys claimed while this runs
         Entry e;
-        s = find_or_claim(m.table, m.mask, m.slots, key, may_claim, claimed, e);
+        s = find_or_claim(m.table, m.mask, m.slots, key, may_claim, claimed, e, walked);
         if (s != NO_SLOT) {
             b = e.bucket;
             c0 = entry_count(e.cr);                                        // stable: only the commit kernel writes counts
@@ -235,10 +241,9 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
     if (wm) {
         if (want) {
             const uint32_t a = s_cnt[6] + woff + __popc(wm & lt);
-            const uint32_t nf = (uint32_t)ctr->n_free;
             if (a < nf) b = m.free_list[nf - 1u - a];
             else {
-                b = ctr->bump + (a - nf);
+                b = bump0 + (a - nf);
                 if (b >= m.max_buckets) b = NO_BUCKET;                  // pool exhausted: the voxel stays without points
             }
             atomicExch(&m.table[s].bucket, b);
