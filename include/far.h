@@ -159,7 +159,7 @@ int far_map_rehash(far_map_t* map, void* stream);
 int far_map_renumber(far_map_t* map, void* stream);
 
 /* Checkpoint / restore of a map's whole device state (table, bucket pool, free list, covariances, counters).
- * create allocates the copy (a maintenance call); restore is seven stream-ordered device copies, no sync. */
+ * create allocates the copy (a maintenance call); restore is eight stream-ordered device copies, no sync. */
 typedef struct far_snapshot far_snapshot_t;
 int far_map_snapshot_create(far_map_t* map, far_snapshot_t** out, void* stream);
 int far_map_snapshot_restore(far_map_t* map, const far_snapshot_t* snap, void* stream);

@@ -16,6 +16,8 @@
 //   cov     : float[max_voxels*cap*6]   (optional) regularised covariance of each stored point (Eq. 1)
 //   cov_ok  : u8[max_voxels * cap]      (optional) 1 if that covariance is valid (>= k neighbours)
 //   free    : u32[max_voxels]           stack of bucket indices returned by far_map_prune
+//   occ     : u32[slots / 32]           one bit per table slot "holds a key" (set when a key is claimed, recomputed by the
+//                                       rehash): L2-resident filter in front of the table for the NN sweep
 // A pruned voxel gives its bucket back at once; its key stays in the table with bucket = NO_BUCKET ("dead key": absent for
 // every query, re-usable by an insert) until the number of dead keys passes a device-side threshold, at which point the
 // prune call's rehash kernel rebuilds the 16-byte entries into `shadow` and copies them back -- no allocation, no host sync.
@@ -85,6 +87,8 @@ struct MapView {
     float* cov;          // nullable
     uint8_t* cov_ok;     // nullable
     uint32_t* free_list;
+    uint32_t* occ;       // [slots / 32] one bit per table slot: the slot holds a key.  8 MB for the 2^26-slot table of a 20 M-voxel map:
+                         // it stays in the 126 MB L2, so a lookup whose home slot is empty costs no DRAM access at all (find_voxel<true>)
     Counters* ctr;
     Mailbox* mail;       // device pointer to the mapped host mailbox
     uint32_t* touched_cnt;   // [TOUCHED_SUBS][32]: lengths of the sub-lists of the insert's touched list, one 128-byte line each
@@ -194,10 +198,16 @@ __device__ __forceinline__ Entry load_entry(const Entry* table, uint32_t s) {
 // slots h .. h + reach(h) only: a voxel that is not in the map -- 11 of the 27 neighbours of a typical query -- is usually
 // dismissed by the one home-entry load instead of a walk to the next empty slot, and the warp no longer waits for the
 // longest of 27 such walks.  An EMPTY home slot means no key has that home (keys are only ever removed by a rebuild).
+// USE_OCC: the home slot's bit of the occupancy bitmap is looked at first (an L2 hit) and an empty home slot is settled
+// without touching the table -- for throughput-bound sweeps over maps far larger than L2 (nn_kernel at C5: 25 of the 27
+// neighbours of a query are absent at v = 0.25 and three quarters of them have an empty home slot); the latency-bound
+// frame kernels go straight to the entry (the bitmap would be one more dependent level for the voxels that exist).
+template <bool USE_OCC = false>
 __device__ __forceinline__ uint32_t find_voxel(const MapView& m, unsigned long long key, uint32_t& count) {
     const uint32_t h = hash_key(key) & m.mask;
-    Entry e = load_entry(m.table, h);
     count = 0;
+    if (USE_OCC && !((__ldg(m.occ + (h >> 5)) >> (h & 31u)) & 1u)) return NO_BUCKET;
+    Entry e = load_entry(m.table, h);
     if (e.key == KEY_EMPTY) return NO_BUCKET;
     const uint32_t reach = entry_reach(e.cr);
     for (uint32_t d = 0;; ++d) {
@@ -252,11 +262,12 @@ __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
 
 // The 27-voxel probe of one query by one warp (Fig. 3): lane l < 27 looks up neighbour
 // (l/9-1, (l/3)%3-1, l%3-1) and keeps its bucket and count in registers.  All 32 lanes must call.
+template <bool USE_OCC = false>
 __device__ __forceinline__ void probe27_regs(const MapView& m, const int k[3], int lane, uint32_t& cnt, uint32_t& slot) {
     cnt = 0; slot = NO_BUCKET;
     if (lane < 27) {
         const int nx = k[0] + lane / 9 - 1, ny = k[1] + (lane / 3) % 3 - 1, nz = k[2] + lane % 3 - 1;
-        if (index_in_range(nx) && index_in_range(ny) && index_in_range(nz)) slot = find_voxel(m, pack_key(nx, ny, nz), cnt);
+        if (index_in_range(nx) && index_in_range(ny) && index_in_range(nz)) slot = find_voxel<USE_OCC>(m, pack_key(nx, ny, nz), cnt);
     }
 }
 
@@ -336,10 +347,11 @@ __device__ __forceinline__ double voxel_lower_bound(float qx, float qy, float qz
 // swept first, then a neighbour voxel is read only if its lower bound does not exceed the best d2 so far
 // (a skipped voxel holds only points strictly farther than the current best, so it cannot change the result,
 // ties included).  The surviving voxels are swept as ONE flattened candidate list, 32 float4 per step.
+template <bool USE_OCC = false>
 __device__ __forceinline__ Best warp_nearest(const MapView& m, float qx, float qy, float qz, const int k[3], int lane,
                                              CandList& L, float& rx, float& ry, float& rz) {
     uint32_t cnt, slot;
-    probe27_regs(m, k, lane, cnt, slot);
+    probe27_regs<USE_OCC>(m, k, lane, cnt, slot);
     Best best;
     best.d2 = __longlong_as_double(0x7FF0000000000000ll);
     best.id = NO_ID;

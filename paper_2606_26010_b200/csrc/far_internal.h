@@ -22,6 +22,7 @@ struct far_map {
     uint32_t renumber_seen;     // mailbox sequence already folded into next_id_ub
     int device;
     int sm_count;
+    int l2_bytes;               // size of the device's L2 (chooses the occupancy-bitmap path of far_map_nn)
 };
 
 namespace far {

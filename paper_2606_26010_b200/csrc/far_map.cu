@@ -76,7 +76,8 @@ __device__ __forceinline__ void raise_reach(Entry* table, uint32_t h, uint32_t r
 // harmless, a stale half only sends the caller through the slower path).  Returns NO_SLOT if the key is absent and the
 // table takes no more keys; `e` = the entry as seen (bucket = BUCKET_PENDING on a slot claimed just now).
 __device__ __forceinline__ uint32_t find_or_claim(Entry* table, uint32_t mask, uint32_t slots, unsigned long long key,
-                                                  bool may_claim, bool& claimed, Entry& e, uint32_t first_probe = 0) {
+                                                  bool may_claim, bool& claimed, Entry& e, uint32_t first_probe = 0,
+                                                  uint32_t* occ = nullptr) {
     // first_probe: slots h .. h + first_probe - 1 are known to hold other keys (keys never leave a slot while inserts run)
     const uint32_t h = hash_key(key) & mask;
     uint32_t s = (h + first_probe) & mask;
@@ -88,6 +89,7 @@ __device__ __forceinline__ uint32_t find_or_claim(Entry* table, uint32_t mask, u
             const unsigned long long cur = atomicCAS(&table[s].key, KEY_EMPTY, key);
             if (cur == KEY_EMPTY) {
                 claimed = true;
+                if (occ) atomicOr(&occ[s >> 5], 1u << (s & 31u));   // the slot holds a key from now on (far_common.cuh)
                 e.key = key; e.bucket = BUCKET_PENDING; e.cr &= ~0xFFu;
                 if (probes) raise_reach(table, h, probes);   // keep the reach of the key's home slot up to date (find_voxel)
                 return s;
@@ -208,7 +210,7 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
     if (unresolved && is_leader) {
         const bool may_claim = ctr->n_keys < m.key_limit;                  // enforced up to the keys claimed while this runs
         Entry e;
-        s = find_or_claim(m.table, m.mask, m.slots, key, may_claim, claimed, e, walked);
+        s = find_or_claim(m.table, m.mask, m.slots, key, may_claim, claimed, e, walked, m.occ);
         if (s != NO_SLOT) {
             b = e.bucket;
             c0 = entry_count(e.cr);                                        // stable: only the commit kernel writes counts
@@ -781,10 +783,18 @@ __global__ void __launch_bounds__(256) rehash_kernel(MapView m) {
         __threadfence();
     }
     __syncthreads();
-    for (uint32_t s = blockIdx.x * blockDim.x + threadIdx.x; s < m.slots; s += gridDim.x * blockDim.x) {
-        uint4* sh = reinterpret_cast<uint4*>(m.shadow + s);
-        *reinterpret_cast<uint4*>(m.table + s) = *sh;
-        *sh = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, BUCKET_PENDING, 0u);
+    for (uint32_t s0 = blockIdx.x * blockDim.x + (threadIdx.x & ~31u); s0 < m.slots; s0 += gridDim.x * blockDim.x) {
+        const uint32_t s = s0 + (threadIdx.x & 31u);
+        uint4 ent = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, BUCKET_PENDING, 0u);
+        if (s < m.slots) {
+            uint4* sh = reinterpret_cast<uint4*>(m.shadow + s);
+            ent = *sh;
+            *reinterpret_cast<uint4*>(m.table + s) = ent;
+            *sh = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, BUCKET_PENDING, 0u);
+        }
+        // the occupancy bitmap of the rebuilt table: 32 consecutive slots are one word
+        const unsigned word = __ballot_sync(FULL, !(ent.x == 0xFFFFFFFFu && ent.y == 0xFFFFFFFFu));
+        if ((threadIdx.x & 31u) == 0) m.occ[s0 >> 5] = word;
     }
     if (last_block_done(&m.ctr->ticket[4]) && threadIdx.x == 0) {
         volatile Counters* c = m.ctr;
@@ -879,6 +889,7 @@ __global__ void __launch_bounds__(256) clear_kernel(MapView m) {
     const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nthr = gridDim.x * blockDim.x;
     for (uint32_t s = tid; s < m.slots; s += nthr)
         *reinterpret_cast<uint4*>(m.table + s) = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, BUCKET_PENDING, 0u);
+    for (uint32_t w = tid; w < (m.slots + 31u) / 32u; w += nthr) m.occ[w] = 0u;
     const size_t used = (size_t)min(m.ctr->bump, m.max_buckets) * (size_t)m.cap;   // fresh buckets beyond are clean
     for (size_t j = tid; j < used; j += nthr) m.ids[j] = NO_ID;
     if (last_block_done(&m.ctr->ticket[2]) && threadIdx.x == 0) {
@@ -1037,6 +1048,7 @@ int far_map_create(far_map_t** out, const far_map_config_t* cfg) {
     m->renumber_every = (uint64_t)c.renumber_every;
     FAR_CUDA(cudaGetDevice(&m->device));
     FAR_CUDA(cudaDeviceGetAttribute(&m->sm_count, cudaDevAttrMultiProcessorCount, m->device));
+    FAR_CUDA(cudaDeviceGetAttribute(&m->l2_bytes, cudaDevAttrL2CacheSize, m->device));
     MapView& v = m->view;
     v.slots = (uint32_t)slots;
     v.mask = (uint32_t)slots - 1;
@@ -1054,6 +1066,7 @@ int far_map_create(far_map_t** out, const far_map_config_t* cfg) {
     alloc((void**)&v.points, npts * sizeof(float4));
     alloc((void**)&v.ids, npts * sizeof(uint32_t));
     alloc((void**)&v.free_list, (size_t)c.max_voxels * sizeof(uint32_t));
+    alloc((void**)&v.occ, ((slots + 31) / 32) * sizeof(uint32_t));
     if (c.with_cov) {
         alloc((void**)&v.cov, npts * 6 * sizeof(float));
         alloc((void**)&v.cov_ok, npts);
@@ -1091,6 +1104,7 @@ int far_map_create(far_map_t** out, const far_map_config_t* cfg) {
     FAR_CUDA(cudaMemcpy(v.ctr, &z, sizeof(z), cudaMemcpyHostToDevice));
     if (v.cov_ok) FAR_CUDA(cudaMemset(v.cov_ok, 0, npts));
     FAR_CUDA(cudaMemset(v.touched_cnt, 0, (size_t)TOUCHED_SUBS * 32 * sizeof(uint32_t)));
+    FAR_CUDA(cudaMemset(v.occ, 0, ((slots + 31) / 32) * sizeof(uint32_t)));
     if (m->d_sp_cnt) FAR_CUDA(cudaMemset(m->d_sp_cnt, 0, (size_t)c.max_voxels * sizeof(uint32_t)));
     {
         const int rc = gicp_setup(m);
@@ -1104,7 +1118,7 @@ int far_map_create(far_map_t** out, const far_map_config_t* cfg) {
 int far_map_destroy(far_map_t* m) {
     if (!m) return FAR_OK;
     cudaFree(m->view.table); cudaFree(m->view.shadow); cudaFree(m->view.points); cudaFree(m->view.ids);
-    cudaFree(m->view.free_list); cudaFree(m->view.cov); cudaFree(m->view.cov_ok);
+    cudaFree(m->view.free_list); cudaFree(m->view.occ); cudaFree(m->view.cov); cudaFree(m->view.cov_ok);
     cudaFree(m->view.ctr); cudaFree(m->d_touched); cudaFree(m->view.touched_cnt); cudaFree(m->d_cov_list);
     cudaFree(m->d_gicp_partials);
     cudaFree(m->d_sp_cnt); cudaFree(m->d_sp_vt); cudaFree(m->d_sp_ptb); cudaFree(m->d_sp_start); cudaFree(m->d_sp_seg);
@@ -1391,8 +1405,8 @@ LaunchScope::~LaunchScope() {
 }  // namespace far
 
 struct far_snapshot {
-    void *table, *points, *ids, *cov, *cov_ok, *free_list, *ctr;
-    size_t b_table, b_points, b_ids, b_cov, b_ok, b_free;
+    void *table, *points, *ids, *cov, *cov_ok, *free_list, *ctr, *occ;
+    size_t b_table, b_points, b_ids, b_cov, b_ok, b_free, b_occ;
     uint64_t next_id_ub, offered_total, offered_at_renumber;
 };
 
@@ -1435,7 +1449,7 @@ int far_profile_collect(const char** names, double* total_ms, long long* launche
 int far_map_snapshot_destroy(far_snapshot_t* s) {
     if (!s) return FAR_OK;
     cudaFree(s->table); cudaFree(s->points); cudaFree(s->ids); cudaFree(s->cov); cudaFree(s->cov_ok); cudaFree(s->free_list);
-    cudaFree(s->ctr);
+    cudaFree(s->ctr); cudaFree(s->occ);
     delete s;
     return FAR_OK;
 }
@@ -1454,13 +1468,14 @@ int far_map_snapshot_create(far_map_t* m, far_snapshot_t** out, void* stream) {
     s->b_cov = m->view.cov ? npts * 6 * sizeof(float) : 0;
     s->b_ok = m->view.cov_ok ? npts : 0;
     s->b_free = (size_t)m->view.max_buckets * sizeof(uint32_t);
+    s->b_occ = (((size_t)m->view.slots + 31) / 32) * sizeof(uint32_t);
     s->next_id_ub = m->next_id_ub;
     s->offered_total = m->offered_total;
     s->offered_at_renumber = m->offered_at_renumber;
     struct { void** dst; const void* src; size_t bytes; } parts[] = {
         {&s->table, m->view.table, s->b_table}, {&s->points, m->view.points, s->b_points}, {&s->ids, m->view.ids, s->b_ids},
         {&s->cov, m->view.cov, s->b_cov}, {&s->cov_ok, m->view.cov_ok, s->b_ok}, {&s->free_list, m->view.free_list, s->b_free},
-        {&s->ctr, m->view.ctr, sizeof(Counters)}};
+        {&s->ctr, m->view.ctr, sizeof(Counters)}, {&s->occ, m->view.occ, s->b_occ}};
     cudaError_t e = cudaSuccess;
     for (auto& p : parts) {
         if (!p.bytes || e != cudaSuccess) continue;
@@ -1489,6 +1504,7 @@ int far_map_snapshot_restore(far_map_t* m, const far_snapshot_t* s, void* stream
     if (s->b_ok && m->view.cov_ok) FAR_CUDA(cudaMemcpyAsync(m->view.cov_ok, s->cov_ok, s->b_ok, cudaMemcpyDeviceToDevice, st));
     FAR_CUDA(cudaMemcpyAsync(m->view.free_list, s->free_list, s->b_free, cudaMemcpyDeviceToDevice, st));
     FAR_CUDA(cudaMemcpyAsync(m->view.ctr, s->ctr, sizeof(Counters), cudaMemcpyDeviceToDevice, st));
+    FAR_CUDA(cudaMemcpyAsync(m->view.occ, s->occ, s->b_occ, cudaMemcpyDeviceToDevice, st));
     m->next_id_ub = s->next_id_ub;
     m->offered_total = s->offered_total;
     m->offered_at_renumber = s->offered_at_renumber;
