@@ -357,6 +357,29 @@ __device__ __forceinline__ Best warp_nearest(const MapView& m, float qx, float q
     best.id = NO_ID;
     best.ref = 0;
     float bx = 0.f, by = 0.f, bz = 0.f;
+    // few occupied voxels (the rule at small voxel sizes: 2 of 27 on the 20 M-point map at v = 0.25): sweep them one after
+    // the other -- bounding and flattening would cost more instructions than the handful of candidates they could save
+    unsigned occv = __ballot_sync(FULL, cnt > 0);
+    if (__popc(occv) <= 4) {
+        while (occv) {
+            const int l = __ffs(occv) - 1;
+            occv &= occv - 1;
+            const uint32_t c = __shfl_sync(FULL, cnt, l), b = __shfl_sync(FULL, slot, l);
+            for (uint32_t j = lane; j < c; j += 32) {
+                const uint32_t ref = b * (uint32_t)m.cap + j;
+                const float4 p = __ldg(m.points + ref);
+                const double d2 = dist2(qx, qy, qz, p.x, p.y, p.z);
+                const uint32_t id = __float_as_uint(p.w);
+                if (better(d2, id, best)) { best.d2 = d2; best.id = id; best.ref = ref; bx = p.x; by = p.y; bz = p.z; }
+            }
+        }
+        const int w = warp_argmin(best.d2, best.id);
+        best.d2 = __shfl_sync(FULL, best.d2, w);
+        best.id = __shfl_sync(FULL, best.id, w);
+        best.ref = __shfl_sync(FULL, best.ref, w);
+        rx = __shfl_sync(FULL, bx, w); ry = __shfl_sync(FULL, by, w); rz = __shfl_sync(FULL, bz, w);
+        return best;
+    }
     const uint32_t c_cnt = __shfl_sync(FULL, cnt, 13), c_slot = __shfl_sync(FULL, slot, 13);
     for (uint32_t j = lane; j < c_cnt; j += 32) {
         const uint32_t ref = c_slot * (uint32_t)m.cap + j;
