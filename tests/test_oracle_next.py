@@ -334,3 +334,38 @@ def test_min_spacing_zero_is_the_plain_insert():
     assert a.insert(pts) == b.insert(pts)
     ea, eb = a.export(), b.export()
     assert np.array_equal(ea["keys"], eb["keys"]) and np.array_equal(ea["ids"], eb["ids"])
+
+
+def test_min_spacing_turns_ring_clumps_into_surface_patches():
+    """Why PAPER.md:68 wants "regularly spaced" points.  A spinning LiDAR crosses a 4 m ground voxel with a few rings of
+    densely sampled points; with the plain cap (lowest ids win) the 40 slots fill with consecutive points of the first one
+    or two rings, so the k = 10 neighbourhood of a stored point is a piece of a LINE and Eq. 1's covariance has one large
+    and two small eigenvalues -- its "normal" is arbitrary in the plane across the ring.  With s = v / sqrt(N_max) the
+    stored points spread over the voxel and the neighbourhoods become surface patches: two comparable eigenvalues, the
+    smallest eigenvector along the true normal (0, 0, 1)."""
+    rng = np.random.default_rng(5)
+    h = 1.8                                                          # sensor height over the plane z = 0
+    elev = np.radians(np.linspace(-24.8, -3.0, 40))                  # rings that reach the ground within ~35 m
+    az = np.radians(np.arange(0.0, 360.0, 360.0 / 2048))
+    rings = []
+    for e in elev:                                                   # ring-major order, as the sensor delivers it
+        r = h / np.tan(-e)
+        rings.append(np.stack([r * np.cos(az), r * np.sin(az), np.zeros_like(az)], axis=1))
+    pts = (np.concatenate(rings) + rng.normal(0, 0.01, (len(elev) * len(az), 3))).astype(np.float32)
+    v, cap = 4.0, 40
+    quality = {}
+    for name, s in (("plain", 0.0), ("spaced", v / np.sqrt(cap))):
+        m = oracle.Map(v, cap, min_spacing=s)
+        m.insert(pts, compute_cov=True)
+        e = m.export(with_cov=True)
+        ok = e["cov_valid"].astype(bool)
+        C = e["cov"][ok].astype(np.float64)                          # (xx, xy, xz, yy, yz, zz)
+        S = np.stack([C[:, [0, 1, 2]], C[:, [1, 3, 4]], C[:, [2, 4, 5]]], axis=1)
+        w, V = np.linalg.eigh(S)                                     # ascending eigenvalues
+        planarity = w[:, 1] / w[:, 2]                                # ~0 on a line, ~1 on an isotropic patch
+        tilt = np.degrees(np.arccos(np.clip(np.abs(V[:, 2, 0]), 0, 1)))   # angle of the smallest eigenvector to z
+        quality[name] = (float(np.median(planarity)), float(np.median(tilt)), int(ok.sum()))
+    (p0, t0, n0), (p1, t1, n1) = quality["plain"], quality["spaced"]
+    assert n0 > 1000 and n1 > 1000
+    assert p0 < 0.05 and p1 > 5 * p0          # line-like without the rule, patches with it
+    assert t1 < 2.0 and t1 < t0               # and the normals point up
