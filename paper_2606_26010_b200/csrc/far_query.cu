@@ -278,19 +278,29 @@ __device__ __forceinline__ void warp_cov_task(const MapView& m, unsigned long lo
                     }
                 }
             }
-            // merge the G partial lists (disjoint shares): after the butterfly every lane of a group holds the group's best KP
+            // merge the G partial lists (disjoint shares): after the butterfly every lane of a group holds the group's best KP.
+            // Two ascending lists a, b of KP keys: c[i] = min(a[i], b[KP-1-i]) are the KP smallest of the union, as a sequence
+            // that rises and then falls; padded with four zeros at the end it is bitonic as a cycle, and one bitonic merge
+            // network over 16 (the zeros are compile-time constants: their exchanges fold away) sorts it -- about 70
+            // instructions a level, where inserting the partner's keys one by one through the min/max chain took ~190
             for (int d = 1; d < G; d <<= 1) {
-                uint32_t other[KP];
+                uint32_t c[16];
 #pragma unroll
-                for (int i = 0; i < KP; ++i) other[i] = __shfl_xor_sync(FULL, key[i], d);
+                for (int i = 0; i < KP; ++i) c[i] = min(key[i], __shfl_xor_sync(FULL, key[KP - 1 - i], d));
 #pragma unroll
-                for (int i = 0; i < KP; ++i) {
-                    uint32_t x = other[i];
-                    if (x < key[KP - 1]) {
+                for (int i = KP; i < 16; ++i) c[i] = 0u;
 #pragma unroll
-                        for (int t = 0; t < KP; ++t) { const uint32_t lo = min(key[t], x); x = max(key[t], x); key[t] = lo; }
+                for (int stride = 8; stride > 0; stride >>= 1) {
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) {
+                        if ((i & stride) == 0) {
+                            const uint32_t lo = min(c[i], c[i + stride]), hi = max(c[i], c[i + stride]);
+                            c[i] = lo; c[i + stride] = hi;
+                        }
                     }
                 }
+#pragma unroll
+                for (int i = 0; i < KP; ++i) key[i] = c[i + 16 - KP];       // the zeros sort to the front
             }
             if (act && sub == 0) {
                 // exact (d2, id) of the kept candidates (R6); drop the (count - k) largest; prove; Eq. 1
