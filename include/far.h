@@ -205,7 +205,10 @@ int far_voxelize(const float* d_xyz, int64_t n, int stride, float voxel, float* 
  * sigma is the adaptive threshold of [1]: gate tau = tau_mult*sigma, kappa = sigma/kappa_div.
  * linearize: one pass at `pose` -> H, b, chi2, n_inliers (pose copied to out, iters = 1).
  * register: Gauss-Newton, T <- Exp(delta) T with H delta = -b, until ||delta|| <= conv_eps or max_iters;
- * the whole loop runs in one cooperative kernel, no host synchronisation inside.  d_out: device-accessible. */
+ * the whole loop runs in one cooperative kernel, no host synchronisation inside.  d_out: device-accessible.
+ * The map is read-only for the registration, but its handle carries the kernel's reduction scratch and launch sequence:
+ * registrations on ONE map must be issued in one stream order (two in flight at once are undefined); registrations on
+ * different maps are independent. */
 int far_gicp_linearize(const far_map_t* map, const float* d_scan, const float* d_scan_cov6,
                        const uint8_t* d_scan_valid, int64_t n, int stride, const far_pose_t* pose, double sigma,
                        const far_gicp_options_t* opts_or_null, far_gicp_result_t* d_out, void* stream);
