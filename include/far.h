@@ -200,6 +200,44 @@ int far_map_count27(const far_map_t* map, const float* d_q, int64_t m, int strid
 int far_voxelize(const float* d_xyz, int64_t n, int stride, float voxel, float* d_out_xyz, int32_t* d_out_index,
                  int64_t* d_n_out, void* d_workspace, size_t* workspace_bytes, void* stream);
 
+/* far_voxelize for callers that must not allocate device memory: same operation (A2, R2), same outputs bit for bit,
+ * but with no workspace argument and no allocation of any kind inside the call (no cudaMalloc / cudaFree, no pool, no
+ * allocating library routine -- only a cudaMemsetAsync and the four kernel launches of far_voxelize).
+ *
+ * Who this is for.  far_voxelize needs about 28 bytes of scratch per point (a throw-away hash table of the scan's voxels,
+ * one slot word per point, the tile offsets), and asks the caller to size and provide it.  Some callers cannot: a
+ * LiDAR callback that runs inside a hard real-time loop may not call cudaMalloc at all, because the call takes
+ * driver-wide locks and can synchronise the whole device for an unbounded time; a component that lives inside
+ * somebody else's process (a plug-in of a perception stack, a node whose GPU memory budget was handed out at start-up
+ * by a supervisor) often receives its input and output buffers from the host application and has no allocator it is
+ * allowed to use; and glue code written in a language binding may have no way to keep a device buffer alive between
+ * calls.  For them the scratch lives INSIDE the library, in a file-scope `static __device__` array of
+ * FAR_VOXELIZE_STATIC_BYTES bytes (7,341,568 B, about 7 MiB) that every GPU that loads libfar.so carries from the
+ * moment the module is loaded on it until the process exits, whether or not this function is ever called.
+ *
+ * Limit.  n <= FAR_VOXELIZE_STATIC_MAX_POINTS (262,144: two 64 x 2,048 scans, or the three 60k-point racing LiDARs
+ * of BASELINE configs[2]).  A larger n is refused with FAR_ERR_ARG before anything is enqueued, and
+ * far_last_cuda_error() then names the limit; use far_voxelize with your own workspace for larger scans.
+ *
+ * First call on a device.  The address of the array is looked up once per device (cudaGetSymbolAddress, with that
+ * device current) the first time this function is called while that device is current, and cached.  The look-up is a
+ * host-side query, not an allocation, but it may initialise the CUDA context and load the module: make this first call
+ * (n = 0 is enough) during set-up, on each device you will use, before the latency-critical part of your program and
+ * before any stream capture is begun.  Later calls only enqueue work on `stream`.  At most 64 devices.
+ *
+ * Sharing.  There is ONE array per device and every call on that device uses it.  It keeps whatever the previous call
+ * left in it; the function resets the parts that have to start clean (hash keys and first-index words) on `stream` at
+ * the start of every call, so back-to-back calls in one stream are correct.  Two calls whose work can overlap on the
+ * same GPU (different streams without an event between them, or two host threads) race on the scratch and produce
+ * garbage silently: serialise them, or use far_voxelize with separate workspaces.
+ *
+ * d_xyz, d_out_xyz, d_out_index, d_n_out: DEVICE pointers owned by the caller, as in far_voxelize (d_out_xyz n*3 fp32,
+ * d_out_index n int32, *d_n_out the count).  FAR_ERR_CUDA if the address look-up or a launch fails. */
+#define FAR_VOXELIZE_STATIC_MAX_POINTS 262144
+#define FAR_VOXELIZE_STATIC_BYTES 7341568
+int far_voxelize_static(const float* d_xyz, int64_t n, int stride, float voxel, float* d_out_xyz, int32_t* d_out_index,
+                        int64_t* d_n_out, void* stream);
+
 /* A8-A10 (Eq. 2-6; R9-R14).  scan: n source points in the sensor frame with their covariances
  * (d_scan_cov6 n*6 fp32, d_scan_valid n bytes; both nullable = all invalid -> point-to-point).
  * sigma is the adaptive threshold of [1]: gate tau = tau_mult*sigma, kappa = sigma/kappa_div.

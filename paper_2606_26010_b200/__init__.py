@@ -132,6 +132,7 @@ def lib():
             "far_map_knn_cov": (ci, [vp, vp, i64, ci, vp, vp, vp]),
             "far_map_knn_cov_dev": (ci, [vp, vp, vp, i64, ci, vp, vp, vp]),
             "far_voxelize": (ci, [vp, i64, ci, f32, vp, vp, vp, vp, vp, vp]),
+            "far_voxelize_static": (ci, [vp, i64, ci, f32, vp, vp, vp, vp]),
             "far_gicp_linearize": (ci, [vp, vp, vp, vp, i64, ci, vp, f64, vp, vp, vp]),
             "far_gicp_register": (ci, [vp, vp, vp, vp, i64, ci, vp, f64, ci, vp, vp, vp]),
             "far_gicp_register_dev": (ci, [vp, vp, vp, vp, vp, i64, ci, vp, f64, ci, vp, vp, vp]),
@@ -271,6 +272,31 @@ class Voxelizer:
 def voxelize(xyz, voxel):
     x, n, _ = _points(xyz)
     return Voxelizer(max(n, 1), device=x.device)(x, voxel)
+
+
+VOXELIZE_STATIC_MAX_POINTS = 262144   # FAR_VOXELIZE_STATIC_MAX_POINTS
+VOXELIZE_STATIC_BYTES = 7341568       # FAR_VOXELIZE_STATIC_BYTES: held by every GPU that loads libfar.so
+
+
+def voxelize_static(xyz, voxel, out_xyz, out_index, n_out):
+    """far_voxelize_static: far_voxelize for callers that may not allocate device memory.
+
+    Meant for code that gets its buffers from somewhere else and has no allocator of its own to call: a LiDAR callback
+    in a real-time loop (cudaMalloc takes driver locks and may stall the whole device), a plug-in living on its host
+    application's GPU memory budget.  The library's own fixed scratch array (about 7 MiB per GPU, shared by all calls)
+    replaces the workspace, so the scan is limited to VOXELIZE_STATIC_MAX_POINTS points; more raises FarError(ERR_ARG).
+    The caller passes every buffer: `xyz` a CUDA fp32 (n,3|4) tensor, `out_xyz` (>= n,3) fp32, `out_index` (>= n,) int32,
+    `n_out` (1,) int64, all on the device; this wrapper creates no tensor and does not synchronise -- results are valid in
+    stream order, the count is n_out[0].  Call it once per device at start-up (n = 0 will do): the first call on a device
+    looks the scratch address up.  Calls that overlap on one GPU share the scratch and corrupt each other."""
+    assert isinstance(xyz, torch.Tensor) and xyz.is_cuda and xyz.dtype == torch.float32 and xyz.is_contiguous()
+    assert xyz.dim() == 2 and xyz.shape[1] in (3, 4), tuple(xyz.shape)
+    n, s = xyz.shape
+    assert out_xyz.is_cuda and out_xyz.dtype == torch.float32 and out_xyz.is_contiguous() and out_xyz.numel() >= 3 * n
+    assert out_index.is_cuda and out_index.dtype == torch.int32 and out_index.is_contiguous() and out_index.numel() >= n
+    assert n_out.is_cuda and n_out.dtype == torch.int64 and n_out.numel() >= 1
+    _check(lib().far_voxelize_static(_ptr(xyz), n, s, voxel, _ptr(out_xyz), _ptr(out_index), _ptr(n_out), _stream()),
+           "far_voxelize_static")
 
 
 def motion_fit(times, vel6, t_ref):

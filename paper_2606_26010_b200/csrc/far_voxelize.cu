@@ -7,6 +7,8 @@
 // Four small kernels, no sort:  (1) find-or-claim the point's key in a scratch open-addressing table and
 // atomicMin its index into the voxel's "first index" word;  (2) flag the points that are their voxel's first
 // and count flags per tile;  (3) one block scans the tile counts;  (4) stable compaction of the flagged points.
+#include <mutex>
+
 #include "far_internal.h"
 
 using namespace far;
@@ -184,4 +186,75 @@ int far::voxelize_impl(const float* d_xyz, int64_t n, const int64_t* d_n, int st
     FAR_LAUNCH(vox_scatter_kernel, (int)tiles, VTILE, 0, st, w, d_xyz, n, d_n, stride, d_out_xyz, d_out_index);
     FAR_CUDA(cudaGetLastError());
     return FAR_OK;
+}
+
+// ---- far_voxelize_static: the same four kernels with their scratch inside the library ---------------------------
+//
+// For callers that are not allowed to allocate device memory (see include/far.h: a hard real-time LiDAR callback that
+// must stay clear of cudaMalloc's driver locks and device-wide synchronisation, a plug-in whose GPU memory budget is
+// owned by its host application, a binding that cannot keep a device buffer between calls).  The scratch far_voxelize
+// takes from its caller is here a file-scope device array: it costs FAR_VOXELIZE_STATIC_BYTES on every GPU that loads
+// libfar.so, for the life of the process, used or not -- which is why the limit is a modest 262,144 points.
+//
+// In HOST code the name `g_vox_static` is only a stand-in the runtime registers for the symbol; it is not a device
+// address (a kernel handed `g_vox_static` from the host would fault, or on a machine where the GPU can reach host
+// memory would quietly scribble over the stand-in).  The address a kernel can use comes from cudaGetSymbolAddress,
+// asked once per device with that device current.
+namespace far {
+
+constexpr size_t vox_static_need(uint64_t n) {
+    uint64_t slots = 64;
+    while (slots < 2 * n) slots <<= 1;
+    const uint64_t tiles = (n + VTILE - 1) / VTILE;
+    return (size_t)(((slots * 8 + 255) & ~255ull) + ((slots * 4 + 255) & ~255ull) + ((n * 4 + 4 + 255) & ~255ull) +
+                    (((tiles + 1) * 4 + 255) & ~255ull));
+}
+static_assert(vox_static_need(FAR_VOXELIZE_STATIC_MAX_POINTS) == FAR_VOXELIZE_STATIC_BYTES,
+              "FAR_VOXELIZE_STATIC_BYTES must be the workspace far_voxelize asks for at FAR_VOXELIZE_STATIC_MAX_POINTS");
+
+static __device__ __align__(256) unsigned char g_vox_static[FAR_VOXELIZE_STATIC_BYTES];
+
+constexpr int VOX_STATIC_MAX_DEVICES = 64;
+static std::mutex g_vox_static_mu;
+static void* g_vox_static_addr[VOX_STATIC_MAX_DEVICES];   // device address of g_vox_static on device i, nullptr = not asked yet
+
+// device address of the scratch on the CURRENT device; the first call on a device asks the runtime, later calls read the cache
+static int vox_static_scratch(void** out) {
+    int dev = -1;
+    FAR_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= VOX_STATIC_MAX_DEVICES) {
+        set_cuda_error(cudaErrorInvalidDevice, "far_voxelize_static: supports device ordinals 0..63");
+        return FAR_ERR_ARG;
+    }
+    std::lock_guard<std::mutex> lock(g_vox_static_mu);
+    if (!g_vox_static_addr[dev]) {
+        void* p = nullptr;
+        FAR_CUDA(cudaGetSymbolAddress(&p, g_vox_static));
+        if (!p || (reinterpret_cast<uintptr_t>(p) & 255u)) {
+            set_cuda_error(cudaErrorInvalidSymbol, "far_voxelize_static: scratch symbol has no 256-byte aligned device address");
+            return FAR_ERR_CUDA;
+        }
+        g_vox_static_addr[dev] = p;
+    }
+    *out = g_vox_static_addr[dev];
+    return FAR_OK;
+}
+
+}  // namespace far
+
+extern "C" int far_voxelize_static(const float* d_xyz, int64_t n, int stride, float voxel, float* d_out_xyz, int32_t* d_out_index,
+                                   int64_t* d_n_out, void* stream) {
+    if (n > (int64_t)FAR_VOXELIZE_STATIC_MAX_POINTS) {
+        far::set_cuda_error(cudaErrorInvalidValue,
+                            "far_voxelize_static: n exceeds FAR_VOXELIZE_STATIC_MAX_POINTS (262144); use far_voxelize with a caller workspace");
+        return FAR_ERR_ARG;
+    }
+    if (n < 0 || !d_n_out) return FAR_ERR_ARG;
+    void* scratch = nullptr;
+    const int rc = far::vox_static_scratch(&scratch);   // first call on this device: cudaGetSymbolAddress; afterwards a table read
+    if (rc != FAR_OK) return rc;
+    // voxelize_impl resets keys / first-index words (cudaMemsetAsync on `stream`) before the claim kernel and writes every
+    // slot_of / tile_off word it later reads, so what the previous call left in the array does not matter
+    size_t bytes = FAR_VOXELIZE_STATIC_BYTES;
+    return far::voxelize_impl(d_xyz, n, nullptr, stride, voxel, d_out_xyz, d_out_index, d_n_out, scratch, &bytes, stream);
 }
