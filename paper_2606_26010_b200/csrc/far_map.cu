@@ -1167,6 +1167,7 @@ int far_map_renumber(far_map_t* m, void* stream) {
 int far::insert_impl(far_map_t* m, const float* d_xyz, int64_t n, const int64_t* d_n, int stride, int pose_mode, const far_pose_t* hpose,
                      const far_pose_t* d_pose, int compute_cov, far_insert_stats_t* d_stats, void* stream, const double* d_n_close,
                      double d_max) {
+    if (!m || (!d_xyz && n > 0) || n < 0 || n > 0x7FFFFFFFll || (stride != 3 && stride != 4)) return FAR_ERR_ARG;
     Asmd asmd{d_n_close, d_n_close ? d_max : 1.0, d_n_close ? 1 : 0};
     if (d_n && n > m->max_batch) return FAR_ERR_ARG;
     Spaced sp;
@@ -1176,7 +1177,6 @@ int far::insert_impl(far_map_t* m, const float* d_xyz, int64_t n, const int64_t*
         sp.s2 = m->cfg.min_spacing * m->cfg.min_spacing;
         sp.on = 1;
     }
-    if (!m || (!d_xyz && n > 0) || n < 0 || n > 0x7FFFFFFFll || (stride != 3 && stride != 4)) return FAR_ERR_ARG;
     if (compute_cov && !m->view.cov) return FAR_ERR_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     // id counter (R3: ids are u32 and advance by the points OFFERED).  The counter lives on the device; the host keeps an

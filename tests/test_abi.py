@@ -111,3 +111,17 @@ def test_compute_calls_fail_loudly_without_a_gpu():
         pytest.skip("GPU present")
     with pytest.raises(RuntimeError):
         far.Map(0.5, 20, 1024)
+
+
+def test_insert_calls_reject_a_null_map_instead_of_dereferencing_it():
+    """FAR_ERR_ARG = "null pointer, bad stride/size/config" (far.h): the four insert entry points check the handle before
+    they read anything through it (host-side argument check only: no GPU needed, nothing is enqueued)."""
+    import paper_2606_26010_b200 as far
+    L = far.lib()
+    dummy = (C.c_double * 16)()                      # stands in for the non-null pose / n_close pointers; never read
+    d = C.cast(dummy, C.c_void_p)
+    assert L.far_map_insert(None, d, 4, 3, None, 0, None, None) == far.ERR_ARG
+    assert L.far_map_insert(None, None, 0, 3, None, 0, None, None) == far.ERR_ARG
+    assert L.far_map_insert_dev(None, d, 4, 3, d, 0, None, None) == far.ERR_ARG
+    assert L.far_map_insert_asmd(None, d, 4, 3, None, d, 50.0, 0, None, None) == far.ERR_ARG
+    assert L.far_map_insert_asmd_dev(None, d, 4, 3, d, d, 50.0, 0, None, None) == far.ERR_ARG
