@@ -73,7 +73,7 @@ struct Counters {
 // written by the device into pinned, mapped HOST memory: lets later host calls report conditions without a sync
 struct Mailbox {
     volatile uint32_t full;             // mirrors Counters::full_flag
-    volatile uint32_t renumber_seq;     // number of far_map_renumber passes completed
+    volatile uint32_t renumber_seq;     // 2 x far_map_renumber passes completed; odd while a pass writes the two words below
     volatile unsigned long long next_id_after_renumber;
     volatile unsigned long long offered_at_renumber;   // host-side offered-points counter the pass was enqueued at
 };

@@ -19,7 +19,9 @@ struct far_map {
     uint64_t offered_total;     // points offered since create / clear
     uint64_t offered_at_renumber;   // value of offered_total when the last renumber pass was enqueued
     uint64_t renumber_every;    // a renumber pass is enqueued before the insert that would exceed this many offered points
-    uint32_t renumber_seen;     // mailbox sequence already folded into next_id_ub
+    uint32_t renumber_seen;     // mailbox sequence word (2 x passes completed) already looked at
+    uint32_t renumber_enqueued; // renumber passes enqueued on this map since create
+    uint32_t renumber_ignore;   // passes up to this ordinal were enqueued before the last snapshot restore: never folded
     int device;
     int sm_count;
     int l2_bytes;               // size of the device's L2 (chooses the occupancy-bitmap path of far_map_nn)

@@ -22,6 +22,7 @@
 // device-side threshold the prune call's follow-up kernel rebuilds the entries into the shadow table and copies them
 // back.  Nothing on this path allocates, frees or synchronises.
 #include <algorithm>
+#include <atomic>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -845,11 +846,20 @@ __global__ void __launch_bounds__(256) renumber_apply_kernel(MapView m, unsigned
         c->next_id = c->next_id - sub;
         c->call_first_id = c->call_first_id >= sub ? c->call_first_id - sub : 0ull;
         c->min_id = NO_ID;
+        // seqlock towards the host (refresh_id_bound): odd while the record is being written, even = 2 x passes completed
+        const uint32_t seq = m.mail->renumber_seq;
+        m.mail->renumber_seq = seq + 1u;
+        __threadfence_system();
         m.mail->next_id_after_renumber = c->next_id;
         m.mail->offered_at_renumber = offered_at;
         __threadfence_system();
-        m.mail->renumber_seq = m.mail->renumber_seq + 1u;
+        m.mail->renumber_seq = seq + 2u;
     }
+}
+
+// far_map_snapshot_restore: the pinned mailbox follows the restored sticky flag
+__global__ void mirror_full_kernel(MapView m) {
+    if (blockIdx.x == 0 && threadIdx.x == 0) m.mail->full = *reinterpret_cast<volatile unsigned int*>(&m.ctr->full_flag) ? 1u : 0u;
 }
 
 // ---- ASMD density (R17): integer sums over the live voxels near the centre, one division at the end --
@@ -1139,12 +1149,19 @@ int far_map_clear(far_map_t* m, void* stream) {
 }
 
 // folds a completed renumber pass (reported through the mailbox) into the host-side bound of the id counter
+// The mailbox record {next_id_after_renumber, offered_at_renumber} is guarded by a sequence word the device makes odd
+// before it writes the record and even (2 x passes completed) after: the host takes a record only if it read the same
+// even value before and after the two fields.  Passes enqueued before the last far_map_snapshot_restore describe a counter
+// the restore has overwritten: they are marked seen and not folded (the restored bound stays a valid upper bound).
 static void refresh_id_bound(far_map_t* m) {
     const uint32_t seq = m->h_mail->renumber_seq;
-    if (seq == m->renumber_seen) return;
+    if ((seq & 1u) || seq == m->renumber_seen) return;          // a record is being written, or nothing new
+    std::atomic_thread_fence(std::memory_order_acquire);
     const uint64_t at = m->h_mail->offered_at_renumber, nid = m->h_mail->next_id_after_renumber;
+    std::atomic_thread_fence(std::memory_order_acquire);
     if (m->h_mail->renumber_seq != seq) return;                 // a newer pass is landing: take it next time
     m->renumber_seen = seq;
+    if (seq / 2u <= m->renumber_ignore) return;                 // enqueued before the last snapshot restore
     if (at <= m->offered_total) m->next_id_ub = nid + (m->offered_total - at);
 }
 
@@ -1153,6 +1170,7 @@ static int renumber_enqueue(far_map_t* m, cudaStream_t st) {
     FAR_LAUNCH(renumber_apply_kernel, grid_for(m->view.slots, 256), 256, 0, st, m->view, (unsigned long long)m->offered_total);
     FAR_CUDA(cudaGetLastError());
     m->offered_at_renumber = m->offered_total;
+    m->renumber_enqueued += 1u;
     return FAR_OK;
 }
 
@@ -1505,6 +1523,11 @@ int far_map_snapshot_restore(far_map_t* m, const far_snapshot_t* s, void* stream
     FAR_CUDA(cudaMemcpyAsync(m->view.free_list, s->free_list, s->b_free, cudaMemcpyDeviceToDevice, st));
     FAR_CUDA(cudaMemcpyAsync(m->view.ctr, s->ctr, sizeof(Counters), cudaMemcpyDeviceToDevice, st));
     FAR_CUDA(cudaMemcpyAsync(m->view.occ, s->occ, s->b_occ, cudaMemcpyDeviceToDevice, st));
+    // the host-visible mirror of the sticky full flag follows the restored counters (a map that filled up after the snapshot
+    // would otherwise keep answering FAR_ERR_FULL), and renumber passes enqueued so far no longer describe this counter
+    FAR_LAUNCH(mirror_full_kernel, 1, 32, 0, st, m->view);
+    FAR_CUDA(cudaGetLastError());
+    m->renumber_ignore = m->renumber_enqueued;
     m->next_id_ub = s->next_id_ub;
     m->offered_total = s->offered_total;
     m->offered_at_renumber = s->offered_at_renumber;

@@ -419,6 +419,79 @@ def test_empty_calls():
     assert m.prune([0, 0, 0], 1.0) == dict(n_voxels_removed=0, n_points_removed=0, n_voxels_left=0, n_points_left=0)
 
 
+def test_snapshot_restore_brings_back_the_full_status():
+    """far_map_status / the return code of insert are served from a host-visible mirror of the device's sticky full flag
+    (far.h).  Restoring a snapshot taken BEFORE the map filled up must bring that mirror back with the counters: the
+    restored map has free buckets and says so; and it can fill up (and say so) again."""
+    rng = np.random.default_rng(31)
+    few = (rng.uniform(-3, 3, size=(200, 3))).astype(np.float32)
+    many = _cloud(rng, 20_000, scale=50.0, clustered=False)
+    m = far.Map(0.5, 4, 1000)
+    m.insert(few)
+    assert m.status() == far.OK
+    snap = m.snapshot()
+    before = m.export()
+    assert m.insert(many)["n_dropped_full"] > 0
+    assert m.status() == far.ERR_FULL and m.stats()["full"] == 1
+    m.restore(snap)
+    torch.cuda.synchronize()
+    assert m.stats()["full"] == 0 and m.status() == far.OK
+    assert far.lib().far_map_insert(m._h, None, 0, 3, None, 0, None, None) == far.OK
+    _assert_same_map(m.export(), before)
+    assert m.insert(many)["n_dropped_full"] > 0 and m.status() == far.ERR_FULL
+    # ... and the other way round: a snapshot of a FULL map restored onto the map after pruning made room
+    full_snap = m.snapshot()
+    assert m.prune([0.0, 0.0, 0.0], 10.0)["n_voxels_removed"] > 0 and m.status() == far.OK
+    m.restore(full_snap)
+    torch.cuda.synchronize()
+    assert m.status() == far.ERR_FULL and m.stats()["full"] == 1
+    far.Map.snapshot_destroy(snap); far.Map.snapshot_destroy(full_snap)
+
+
+def test_id_range_check_survives_a_renumber_undone_by_a_restore():
+    """R3/R22 at the top of the u32 id range (FAR_ERR_RANGE, far.h).  Ids advance by the points OFFERED, so 3 x 2^30 rows
+    of NaN take the counter to 3.2e9 without storing anything.  A renumber pass enqueued after a snapshot reports a small
+    counter to the host; restoring the snapshot puts the large counter back, and the host-side bound must not fold that
+    stale report: the next 2^30-row insert would wrap the ids past 2^32 and has to be refused, nothing inserted.  After an
+    explicit renumber of the restored map the same insert goes through and the ids are the renumbered ones."""
+    big = 1 << 30
+    nan = torch.full((big, 3), float("nan"), dtype=torch.float32, device="cuda")      # 12.9 GB of invalid rows
+    L, st = far.lib(), far._stream()
+
+    def offer_nan():
+        return L.far_map_insert(m._h, far._ptr(nan), big, 3, None, 0, None, st)
+
+    rng = np.random.default_rng(32)
+    m = far.Map(1.0, 8, 10_000)
+    anchor = np.array([[500.5, 500.5, 0.5]], dtype=np.float32)        # id 0 stays alive: automatic renumbering subtracts 0
+    assert m.insert(anchor)["n_accepted"] == 1
+    for _ in range(3):
+        assert offer_nan() == far.OK
+    pts = (rng.uniform(-4, 4, size=(1000, 3))).astype(np.float32)
+    first = 1 + 3 * big
+    assert m.insert(pts)["n_accepted"] > 900
+    assert m.size()[2] == first + 1000
+    e = m.export()
+    live = np.sort(e["ids"][e["ids"] != far.NO_ID].astype(np.int64))
+    assert live[0] == 0 and live[1] == first and live[-1] <= first + 999
+    assert m.prune([0.0, 0.0, 0.0], 50.0)["n_voxels_removed"] == 1    # the anchor goes: smallest live id is now ~3.2e9
+    snap = m.snapshot()
+    m.renumber()
+    torch.cuda.synchronize()                                         # the pass has reported next_id = 1000 to the host
+    assert m.size()[2] == 1000
+    m.restore(snap)
+    assert m.size()[2] == first + 1000
+    assert offer_nan() == far.ERR_RANGE                              # 3.2e9 + 1001 + 2^30 > 2^32 - 1
+    assert m.size()[2] == first + 1000                               # nothing was offered
+    m.renumber()
+    assert offer_nan() == far.OK
+    assert m.size()[2] == 1000 + big
+    e2 = m.export()
+    live2 = np.sort(e2["ids"][e2["ids"] != far.NO_ID].astype(np.int64))
+    assert np.array_equal(live2, live[1:] - first)
+    far.Map.snapshot_destroy(snap)
+
+
 def test_snapshot_restore_count27_and_launch_accounting():
     rng = np.random.default_rng(21)
     pts = _cloud(rng, 40_000, scale=12.0)
