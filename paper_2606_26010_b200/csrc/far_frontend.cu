@@ -216,6 +216,10 @@ static int frontend_process_impl(far_frontend_t* f, const float* d_scan, int64_t
     if (!f || !init_pose || n < 0 || n > f->cfg.max_scan_points || (n > 0 && !d_scan) || (stride != 3 && stride != 4) || !(sigma > 0.0))
         return FAR_ERR_ARG;
     cudaStream_t st = (cudaStream_t)stream;
+    // an empty frame may come without a scan pointer.  Every stage is sized for max_scan_points and reads the real count
+    // (0) on the device, so the launches still want a valid address: the frontend's own staging buffer stands in (it holds
+    // max_scan_points x 4 floats, enough for either stride, and is never read when the count is 0)
+    if (!d_scan) d_scan = f->d_scan;
     far_gicp_result_t* res = d_out ? d_out : f->d_result;
     FrameParams hp;
     FrameParams* src = pinned_params ? f->h_fp : &hp;
@@ -258,7 +262,9 @@ static int frontend_process_impl(far_frontend_t* f, const float* d_scan, int64_t
             } else {
                 if (f->graph) { cudaGraphDestroy(f->graph); f->graph = nullptr; }
                 f->gexec = nullptr;
-                f->graph_state = -1;                     // this driver refuses the capture: stay on the stream path
+                // the runtime refused the capture: stay on the stream path for good.  A stage that rejected its ARGUMENTS
+                // says nothing about capturing: this frame runs (and fails) on the stream path, a later one may capture
+                f->graph_state = (e == cudaSuccess && rc == FAR_ERR_ARG) ? 0 : -1;
                 cudaGetLastError();
             }
         }

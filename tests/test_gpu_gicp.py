@@ -467,6 +467,49 @@ def test_frame_graph_replay_equals_stream_of_launches_and_oracle():
     assert np.array_equal(eb["cov_valid"], eo["cov_valid"])
 
 
+def test_empty_frame_without_a_scan_pointer_is_a_frame_like_any_other():
+    """far_frontend_process accepts n == 0 with a NULL scan (far.h: "(n > 0 && !d_scan)" is the error).  The frame runs its
+    whole chain on zero points: the registration reports FAR_ERR_DEGENERATE with the initial pose (fewer than 6 inliers,
+    PAPER.md:84-100 has nothing to solve), the map is untouched, and neither the stream path nor the captured graph is
+    disturbed -- the frames after it give the bytes they give without the empty frame in between."""
+    c1 = scenes.c1_tiny(seed=0)
+    v, cap, scan = c1["voxel"], c1["cap"], c1["scan"]
+    st = torch.cuda.current_stream().cuda_stream
+    runs = {}
+    for with_empty in (False, True):
+        fe = far.Frontend(v, cap, 1 << 14, len(scan), ds_voxel=v, prune_radius=50.0, max_iters=c1["max_iters"])
+        fe.map.insert(c1["map_points"], compute_cov=True)
+        buf = torch.as_tensor(scan).cuda()
+        d_res = torch.zeros(far.GICP_RESULT_BYTES, dtype=torch.uint8, device="cuda")
+        po = far.Pose.from_rt(c1["T_init"])
+        frames = []
+        for k in range(5):
+            if with_empty and k in (0, 3):          # before anything ran, and after the graph was captured
+                before = fe.map.export(with_cov=True)
+                rc = far.lib().far_frontend_process(fe._h, None, 0, 3, far.C.byref(po), c1["sigma"], d_res.data_ptr(), st)
+                assert rc == far.OK
+                torch.cuda.synchronize()
+                g = far.result_to_dict(far.GicpResult.from_buffer_copy(d_res.cpu().numpy().tobytes()))
+                assert g["status"] == far.ERR_DEGENERATE and g["n_inliers"] == 0
+                assert np.array_equal(g["R"], np.asarray(c1["T_init"][0])) and np.array_equal(g["t"], np.asarray(c1["T_init"][1]))
+                after = fe.map.export(with_cov=True)
+                for key in ("keys", "counts", "ids", "xyz", "cov", "cov_valid"):
+                    assert np.array_equal(before[key].view(np.uint8), after[key].view(np.uint8)), key
+                assert fe.graph_state() >= 0
+            rc = far.lib().far_frontend_process(fe._h, buf.data_ptr(), len(scan), 3, far.C.byref(po), c1["sigma"], d_res.data_ptr(), st)
+            assert rc == far.OK
+            torch.cuda.synchronize()
+            frames.append(d_res.cpu().numpy().tobytes())
+        assert fe.graph_state() == 1
+        runs[with_empty] = (frames, fe.map.export(with_cov=True))
+        fe.close()
+    assert runs[False][0] == runs[True][0]
+    for key in ("keys", "counts", "ids", "xyz", "cov", "cov_valid"):
+        assert np.array_equal(runs[False][1][key].view(np.uint8), runs[True][1][key].view(np.uint8)), key
+    first = far.result_to_dict(far.GicpResult.from_buffer_copy(runs[True][0][0]))
+    assert first["status"] == 0 and first["n_inliers"] > 100
+
+
 def test_ten_thousand_registrations_are_bitwise_reproducible():
     """The reduction is a fixed-order sum of tagged words (far_gicp.cu): 10,000 back-to-back registrations, two maps
     alternating (each with its own scratch and launch sequence), no host synchronisation in between -- every
