@@ -51,7 +51,8 @@ struct Counters {
     unsigned long long next_id;       // id of the next offered point (device-resident: no per-call kernel argument)
     unsigned long long call_first_id; // first id of the insert call whose last chunk was committed most recently
     unsigned int n_keys;              // claimed keys (live + dead)
-    unsigned int n_dead;              // keys whose voxel was pruned since the last rehash
+    unsigned int n_dead;              // keys in the table that own no bucket: voxels pruned since the last rehash and not opened
+                                      // again since, plus keys claimed when the bucket pool was exhausted
     unsigned int bump;                // buckets ever taken from the fresh end of the pool
     int n_free;                       // entries on the free list
     unsigned int n_alloc;             // buckets handed out by the running insert kernel: the first n_free of them come off the

@@ -160,13 +160,14 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
     // one atomic per WARP and counter (3,656 warps for a 117k-point scan, six counters) held the whole kernel back by ~14 us.
     // So everything is summed per BLOCK in shared memory first: the block draws its buckets with ONE atomic after a barrier
     // that only waits for the lookups, and its statistics go out with one atomic each from whichever warp finishes last.
-    __shared__ uint32_t s_cnt[8];               // 0 buckets wanted, 1 new keys, 2 invalid, 3 opened, 4 dropped, 5 warps done, 6 draw base
+    __shared__ uint32_t s_cnt[10];              // 0 buckets wanted, 1 new keys, 2 invalid, 3 opened, 4 dropped, 5 warps done, 6 draw base,
+                                                // 7 dead keys revived, 8 new keys left without a bucket
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
     const Pose& T = (pose_mode == 2) ? *d_pose : hpose;
     Counters* ctr = m.ctr;
-    if (threadIdx.x < 8) s_cnt[threadIdx.x] = 0u;
+    if (threadIdx.x < 10) s_cnt[threadIdx.x] = 0u;
     __syncthreads();
     if (d_n) n = min(n, *d_n);                  // frame graph: launch sized for the largest scan, count on the device
     float p[3];
@@ -274,10 +275,16 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
     const unsigned m_bad = __ballot_sync(FULL, bad);
     const unsigned m_drop = __ballot_sync(FULL, valid && b == NO_BUCKET);
     const unsigned m_open = __ballot_sync(FULL, opened);
+    // Counters::n_dead = keys in the table that own no bucket: the dead key of a pruned voxel that got a bucket again leaves
+    // that set, a new key the exhausted pool had no bucket for is born into it
+    const unsigned m_rev = __ballot_sync(FULL, want && !claimed && opened);
+    const unsigned m_still = __ballot_sync(FULL, want && claimed && !opened);
     if (lane == 0) {
         if (m_bad) atomicAdd(&s_cnt[2], (uint32_t)__popc(m_bad));
         if (m_open) atomicAdd(&s_cnt[3], (uint32_t)__popc(m_open));
         if (m_drop) atomicAdd(&s_cnt[4], (uint32_t)__popc(m_drop));
+        if (m_rev) atomicAdd(&s_cnt[7], (uint32_t)__popc(m_rev));
+        if (m_still) atomicAdd(&s_cnt[8], (uint32_t)__popc(m_still));
     }
 
     // phase 4: the chain.  cap = this voxel's limit: the fixed cap, or N_ASMD (positions at and beyond it are never written)
@@ -342,6 +349,9 @@ __global__ void __launch_bounds__(256) insert_claim_chain_kernel(MapView m, cons
         if (nb) atomicAdd(&ctr->st_invalid, (unsigned long long)nb);
         if (no) atomicAdd(&ctr->st_new_voxels, (unsigned long long)no);
         if (nd) { atomicAdd(&ctr->st_dropped_full, (unsigned long long)nd); ctr->full_flag = 1u; }
+        const uint32_t nr = *(volatile uint32_t*)&s_cnt[7], ns = *(volatile uint32_t*)&s_cnt[8];
+        if (nr) atomicSub(&ctr->n_dead, nr);
+        if (ns) atomicAdd(&ctr->n_dead, ns);
     }
 }
 

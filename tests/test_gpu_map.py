@@ -6,7 +6,7 @@ import torch
 
 import far_scenes as scenes
 import oracle
-from helpers import load_golden
+from helpers import load_golden, np_pack, np_voxel_index
 
 pytestmark = pytest.mark.gpu
 
@@ -417,6 +417,53 @@ def test_empty_calls():
     assert int(valid[0]) == 0 and cov[0].tolist() == [1, 0, 0, 1, 0, 1]
     assert m.export()["keys"].size == 0
     assert m.prune([0, 0, 0], 1.0) == dict(n_voxels_removed=0, n_points_removed=0, n_voxels_left=0, n_points_left=0)
+
+
+def test_dead_key_count_follows_revived_and_bucketless_keys():
+    """The table is rebuilt (in-place rehash inside far_map_prune) when the keys that own no bucket stop being a small
+    fraction of the live ones.  That count has to follow the table: a pruned voxel that is opened again is no longer dead,
+    and a key claimed while the bucket pool was exhausted is dead from the start.
+    (a) a vehicle going back and forth over the same ground: each lap prunes and re-opens the same ~8 % of the voxels; no
+        lap leaves more dead keys than the first one did, so no lap may trigger a rebuild;
+    (b) a map whose pool ran out: the bucket-less keys are reclaimed by the next prune even if it removes nothing."""
+    rng = np.random.default_rng(41)
+    # (a) 12,000 voxels on a 0.5 m lattice plane, one point each; the strip x < 4 m holds 960 of them (8 %)
+    ij = np.stack(np.meshgrid(np.arange(100), np.arange(120), indexing="ij"), axis=-1).reshape(-1, 2)
+    pts = np.concatenate([ij * 0.5 + 0.25, np.full((len(ij), 1), 0.25)], axis=1).astype(np.float32)
+    pts = pts[rng.permutation(len(pts))]
+    mo, mg = oracle.Map(0.5, 4), far.Map(0.5, 4, 20_000)
+    assert mg.insert(pts) == mo.insert(pts)
+    centre, radius = [1000.0, 30.0, 0.25], 996.0          # keeps x >= 4 m, up to the curvature of a 1 km circle
+    strip = None
+    for lap in range(6):
+        assert mg.prune(centre, radius) == mo.prune(centre, radius)
+        if strip is None:                                # the points of the voxels the prune removes: the same every lap
+            gone = ~np.isin(np_pack(np_voxel_index(pts, 0.5)), mo.export()["keys"])
+            strip = pts[gone]
+            assert 900 < len(strip) < 1100
+        s = mg.stats()
+        assert 800 < s["n_dead_keys"] < 32 + s["n_voxels"] // 8, s
+        assert s["n_rehash"] == 0, (lap, s)
+        assert mg.insert(strip) == mo.insert(strip)
+        s = mg.stats()
+        assert s["n_dead_keys"] == 0 and s["n_voxels"] == 12_000 and s["n_keys"] == 12_000, s
+        _assert_same_map(mg.export(), mo.export())
+    # one more prune, now of a larger part (x < 12 m, 24 %): the rebuild is due and happens
+    assert mg.prune(centre, 988.0) == mo.prune(centre, 988.0)
+    s = mg.stats()
+    assert s["n_rehash"] == 1 and s["n_dead_keys"] == 0 and s["n_keys"] == s["n_voxels"], s
+    _assert_same_map(mg.export(), mo.export())
+    # (b) 1,000 buckets, a cloud that wants ~15,000 voxels
+    m = far.Map(0.5, 4, 1000)
+    st = m.insert(_cloud(rng, 20_000, scale=50.0, clustered=False))
+    assert st["n_new_voxels"] == 1000 and st["n_dropped_full"] > 0
+    s = m.stats()
+    assert s["n_dead_keys"] > 0 and s["n_keys"] == 1000 + s["n_dead_keys"], s
+    before = m.export()
+    assert m.prune([0.0, 0.0, 0.0], 1e4)["n_voxels_removed"] == 0
+    s = m.stats()
+    assert s["n_rehash"] == 1 and s["n_dead_keys"] == 0 and s["n_keys"] == 1000 and s["n_voxels"] == 1000, s
+    _assert_same_map(m.export(), before)
 
 
 def test_snapshot_restore_brings_back_the_full_status():
