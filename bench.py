@@ -150,32 +150,115 @@ def oracle_frame(oracle, mo, c2, n_threads, register_reps):
     return float(np.mean(t_reg)) + t_upd, res, dict(register_s=float(np.mean(t_reg)), update_s=t_upd, accepted=st["n_accepted"])
 
 
+def cpu_model():
+    """model string of the host CPU the oracle is timed on (/proc/cpuinfo), "" if unreadable"""
+    try:
+        with open("/proc/cpuinfo") as f:
+            for ln in f:
+                if ln.lower().startswith("model name"):
+                    return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return ""
+
+
 def run_reference(args):
+    """The oracle timed on the SAME step as the GPU arm: every step starts from a copy of the freshly built local map
+    (faro_map_clone, untimed -- the counterpart of the GPU arm's untimed snapshot restore), so each frame inserts the
+    scan's ~45k accepted points and recomputes their covariances, which is most of the oracle's frame time."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     import oracle
     cores = os.cpu_count() or 1
     c2 = load_workload(args.workload)
-    mo = oracle.Map(c2["voxel"], c2["cap"])
-    mo.insert(c2["map_points"], compute_cov=True)
-    times = []
-    res = None
+    base = oracle.Map(c2["voxel"], c2["cap"])
+    t0 = time.perf_counter()
+    base.insert(c2["map_points"], compute_cov=True)
+    t_build = time.perf_counter() - t0
+    n_vox, n_stored, _ = base.size()
+    n_ds = len(oracle.voxelize(c2["scan"], c2["voxel"])[0])
+    times, res, detail = [], None, None
     for i in range(args.warmup + args.steps):
-        t, res, _ = oracle_frame(oracle, mo, c2, cores, 1)
+        mo = base.clone()
+        t, res, detail = oracle_frame(oracle, mo, c2, cores, 1)
+        del mo
         if i >= args.warmup:
             times.append(t)
     total = float(np.sum(times))
     value = len(times) / total
-    sample = (f"{args.steps} whole frames of the C2 workload on one oracle map (the map keeps the inserted scans between "
-              f"frames, so later frames insert less: this favours the reference)")
+    sample = (f"{args.steps} whole C2 frames (voxelise + Sigma_s + GICP with {cores} OpenMP threads over source points; insert with "
+              f"covariances + prune single-threaded), each on a fresh copy of the built local map (copy and the {t_build:.1f} s map "
+              f"build untimed): the same step the GPU arm times after its snapshot restore")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times), "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_name(c2), "iters": int(res["iters"])},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "config": {"workload": workload_name(c2, n_ds, n_vox, n_stored), "parallelism": "host cores",
+                       "scan_points": len(c2["scan"]), "source_points": n_ds, "map_points": n_stored, "map_voxels": n_vox,
+                       "gicp_iters": int(res["iters"]), "accepted_per_frame": int(detail["accepted"])},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                             "cpu_model": cpu_model(), "detail": detail},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
+
+
+def cpu_baseline_legs(extras, host, cores):
+    """The oracle timed beside every throughput leg of `extras` (north_star: "shown next to the oracle timed on the same
+    box's host cores in the same run"; SURVEY.md:529-532), on the SAME inputs the GPU legs used (`host`: their host copies).
+    Single-threaded, and with OpenMP where the oracle has a parallel loop (the NN query; insert, voxelise and undistort are
+    sequential by definition).  One repetition each: they take seconds.  Bounded samples are named in `sample`."""
+    import oracle
+    model = cpu_model()
+
+    def entry(value, unit, threads, sample, **kw):
+        return dict({"value": value, "unit": unit, "cores": threads, "kind": "oracle", "sample": sample, "cpu_model": model}, **kw)
+
+    if "c4_insert" in extras and "c4" in host:
+        pts = host["c4"]
+        mo = oracle.Map(0.5, 20)
+        t0 = time.perf_counter()
+        for b in range(100):
+            mo.insert(pts[b * 100_000:(b + 1) * 100_000])
+        t_ins = time.perf_counter() - t0
+        nv, npts, _ = mo.size()
+        t0 = time.perf_counter()
+        pr = mo.prune([0.0, 0.0, 0.0], 150.0)
+        t_pr = time.perf_counter() - t0
+        extras["c4_insert"]["cpu_baseline"] = entry(
+            1e7 / t_ins, "points/s", 1, "all 10 M points in 100 batches of 100k (the oracle's insert is one sequential loop), then the prune",
+            seconds=t_ins, prune_seconds=t_pr, prune_voxels_per_s=nv / t_pr,
+            parity={"stored_equal": bool(npts == extras["c4_insert"]["stored"]), "voxels_equal": bool(nv == extras["c4_insert"]["voxels"]),
+                    "pruned_equal": bool(pr["n_voxels_removed"] == extras["c4_insert"]["prune_voxels_removed"])})
+        del mo
+    if "c5_nn" in extras and "c5" in host:
+        c5 = host["c5"]
+        n_q = int(os.environ.get("FAR_BENCH_C5_ORACLE_QUERIES", "200000"))
+        q = np.ascontiguousarray(c5["queries"][c5["order"]][:n_q])
+        for key, row in extras["c5_nn"].items():
+            v = float(key.split("=")[1])
+            mo = oracle.Map(v, 20)
+            t0 = time.perf_counter()
+            mo.insert(c5["map_points"])
+            t_build = time.perf_counter() - t0
+            t0 = time.perf_counter(); mo.nn(q, nthreads=1); t1 = time.perf_counter() - t0
+            t0 = time.perf_counter(); mo.nn(q, nthreads=cores); tn = time.perf_counter() - t0
+            row["cpu_baseline"] = entry(
+                n_q / min(t1, tn), "queries/s", cores if tn < t1 else 1,
+                f"the first {n_q} of the 1 M random-order queries against the full 20 M-point oracle map (std::unordered_map), 1 repetition",
+                single_thread_queries_per_s=n_q / t1, openmp_queries_per_s=n_q / tn, openmp_threads=cores,
+                build_points_per_s=2e7 / t_build, build_seconds=t_build)
+            del mo
+    if "voxelize" in extras and "up" in host:
+        t0 = time.perf_counter()
+        o_xyz, _ = oracle.voxelize(host["up"], 1.0)
+        t_v = time.perf_counter() - t0
+        extras["voxelize"]["cpu_baseline"] = entry(len(host["up"]) / t_v, "points/s", 1, "the same 8 M points, 1 repetition", seconds=t_v,
+                                                   parity={"voxels_out_equal": bool(len(o_xyz) == extras["voxelize"]["voxels_out"])})
+    if "undistort" in extras and "up" in host and "ut" in host:
+        t0 = time.perf_counter()
+        oracle.undistort(host["up"], host["ut"], 0.1, host["ua"], host["ub"])
+        t_u = time.perf_counter() - t0
+        extras["undistort"]["cpu_baseline"] = entry(len(host["up"]) / t_u, "points/s", 1, "the same 8 M points, 1 repetition", seconds=t_u)
 
 
 # ---------------------------------------------------------------------------------------------------------
@@ -278,9 +361,13 @@ def _leg_c2_paper_params(out, far, scenes, torch):
     fe.close()
 
 
+HOST_INPUTS = {}      # host copies of the legs' inputs, for cpu_baseline_legs (the oracle runs after every GPU timing is done)
+
+
 def _leg_c4(out, far, scenes, torch, peak):
     # ---- C4: 10 M points in 100 batches of 100k into v = 0.5, cap 20; then prune r = 150 m -------------------------
-    pts = torch.as_tensor(scenes.c4_insert_stress(seed=3)).cuda()
+    HOST_INPUTS["c4"] = scenes.c4_insert_stress(seed=3)
+    pts = torch.as_tensor(HOST_INPUTS["c4"]).cuda()
     mg = far.Map(0.5, 20, 9_000_000, with_cov=False, max_batch=100_000)
     per = []
     for b in range(100):
@@ -321,6 +408,7 @@ def _leg_c4(out, far, scenes, torch, peak):
 def _leg_c5(out, far, scenes, torch, peak, flush, voxels=(0.25, 0.5, 1.0, 2.0)):
     # ---- C5: 1 M queries against a 20 M-point map at four voxel sizes, random and Morton order -------------------
     c5 = scenes.c5_nn_sweep(seed=4)
+    HOST_INPUTS["c5"] = c5
     d_pts = torch.as_tensor(c5["map_points"]).cuda()
     ids = torch.empty(1_000_000, dtype=torch.int32, device="cuda")
     d2 = torch.empty(1_000_000, dtype=torch.float32, device="cuda")
@@ -690,6 +778,7 @@ def run_far(args):
                                "frac_of_hbm_peak": nu * 28 / t_u / 1e9 / peak,
                                "note": "8 M points in one call (224 MB > L2), FP64 arithmetic, 256 MB flush between repetitions"}
         _leg_voxelize(extras, far, torch, peak, flush, up)
+        HOST_INPUTS.update(up=up.cpu().numpy(), ut=ut.cpu().numpy(), ua=ua, ub=ub)
         del up, ut, uo
 
         # BASELINE.json's other throughput metrics at the full sizes of configs[3] and configs[4]: hash insert and NN queries
@@ -710,7 +799,8 @@ def run_far(args):
         mo.insert(c2["map_points"], compute_cov=True)
         t_build = time.perf_counter() - t0
         t_frame, o_res, detail = oracle_frame(oracle, mo, c2, cores, 5)
-        cpu = {"value": 1.0 / t_frame, "unit": UNIT, "cores": cores, "kind": "oracle",
+        cpu_baseline_legs(extras, HOST_INPUTS, cores)
+        cpu = {"value": 1.0 / t_frame, "unit": UNIT, "cores": cores, "kind": "oracle", "cpu_model": cpu_model(),
                "sample": (f"one whole C2 frame: 5 x (voxelise + Sigma_s + GICP, {cores} OpenMP threads over source points) "
                           f"averaged + 1 x (insert with covariances + prune, SINGLE-THREADED and the larger part of the frame: "
                           f"detail.update_s); map build ({t_build:.1f} s) untimed; a deliberately plain checker, not a tuned CPU code"),

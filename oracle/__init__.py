@@ -84,6 +84,8 @@ def lib():
         L.faro_map_create.argtypes = [f32, i32, i32, f64]
         L.faro_map_destroy.argtypes = [vp]
         L.faro_map_destroy.restype = None
+        L.faro_map_clone.restype = vp
+        L.faro_map_clone.argtypes = [vp]
         L.faro_pack_key.restype = C.c_uint64
         L.faro_pack_key.argtypes = [i32, i32, i32]
         L.faro_unpack_key.restype = None
@@ -232,6 +234,15 @@ class Map:
         if getattr(self, "_h", None):
             lib().faro_map_destroy(self._h)
             self._h = None
+
+    def clone(self):
+        """faro_map_clone: an independent deep copy (contents, covariances, id counter, configuration)."""
+        c = Map.__new__(Map)
+        c.voxel, c.cap, c.k_cov = self.voxel, self.cap, self.k_cov
+        c._h = lib().faro_map_clone(self._h)
+        if not c._h:
+            raise MemoryError("faro_map_clone")
+        return c
 
     def insert(self, xyz, pose=None, compute_cov=False):
         a, n, s = _pts(xyz)

@@ -283,6 +283,9 @@ faro_map_t* faro_map_create(float voxel, int32_t cap, int32_t k_cov, double cov_
     return m;
 }
 void faro_map_destroy(faro_map_t* m) { delete m; }
+// a deep copy (the struct's own copy constructor: configuration, id counter and every voxel's point list): bookkeeping
+// for callers that replay one step on the same map several times (bench.py --impl reference); no arithmetic of the method
+faro_map_t* faro_map_clone(const faro_map_t* m) { return m ? new faro_map(*m) : nullptr; }
 void faro_map_set_min_spacing(faro_map_t* m, double s) { if (m) m->min_spacing = s > 0.0 ? s : 0.0; }
 
 namespace {

@@ -61,6 +61,8 @@ int faro_voxelize(const float* xyz, int64_t n, int stride, float voxel,
 /* A3/A4/A5 */
 faro_map_t* faro_map_create(float voxel, int32_t cap, int32_t k_cov, double cov_eps);
 void faro_map_destroy(faro_map_t*);
+/* deep copy of a map (contents, covariances, id counter, configuration); NULL in -> NULL out.  Bookkeeping only. */
+faro_map_t* faro_map_clone(const faro_map_t*);
 /* R21: s > 0: an offered point is stored only if no point already stored in its own voxel is closer than s
  * (FP64 squared distance as R6, strict <), tested in index order after the cap; s = 0 (default): the plain capped insert */
 void faro_map_set_min_spacing(faro_map_t*, double s);

@@ -317,3 +317,26 @@ def test_renumber_shifts_ids_by_the_minimum_and_nothing_else():
     # an empty map restarts at 0
     m.prune([1000.0, 0.0, 0.0], 1.0)
     assert m.size()[0] == 0 and m.renumber() == nid - mn + 7 and m.size()[2] == 0
+
+
+def test_clone_is_a_deep_independent_copy():
+    """faro_map_clone (bookkeeping for bench.py --impl reference): the copy has the same contents, covariances and id
+    counter; inserting into or pruning one of the two leaves the other as it was."""
+    rng = np.random.default_rng(77)
+    pts = rng.uniform(-6, 6, size=(5000, 3)).astype(np.float32)
+    a = oracle.Map(0.5, 6)
+    a.insert(pts[:3000], compute_cov=True)
+    b = a.clone()
+    ea, eb = a.export(with_cov=True), b.export(with_cov=True)
+    assert a.size() == b.size() and (b.voxel, b.cap, b.k_cov) == (a.voxel, a.cap, a.k_cov)
+    for k in ea:
+        assert np.array_equal(ea[k], eb[k]), k
+    assert b.insert(pts[3000:]) == oracle.Map.clone(a).insert(pts[3000:])      # the counter and the counts came along
+    a.prune([0.0, 0.0, 0.0], 2.0)
+    e2 = b.export(with_cov=True)
+    assert b.size()[1] > a.size()[1] and len(e2["keys"]) > len(ea["keys"])
+    ref = oracle.Map(0.5, 6)
+    ref.insert(pts[:3000], compute_cov=True); ref.insert(pts[3000:])
+    er = ref.export(with_cov=True)
+    for k in er:
+        assert np.array_equal(er[k], e2[k]), k
