@@ -31,7 +31,7 @@ def build(force=False, verbose=False):
            "-Xcompiler", "-fPIC", "-shared", "-I", INCLUDE, "-o", OUT] + sources()
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
-    extra = os.environ.get("FAR_NVCC_FLAGS", "").split()      # e.g. -DFAR_PROBE_GROUP=2 for experiments
+    extra = os.environ.get("FAR_NVCC_FLAGS", "").split()      # extra nvcc flags for experiments, e.g. -Xptxas=-v or -G
     cmd[1:1] = extra
     subprocess.check_call(cmd)
     return OUT

@@ -14,20 +14,21 @@
 // instruction count per scheduler and the serial chain short (round 2 profile: with a warp per point, 10 warps per
 // scheduler each issued ~950 instructions per iteration -- 5-7 us -- and seven warps of a block waited at a barrier
 // while 8 lanes of the eighth linearised):
-//   groups   EIGHT LANES per source point, four points per warp; points are dealt round-robin over the blocks of the
-//            grid (two 512-thread blocks per SM), so a 5,000-point scan puts ~2.5 busy warps on a scheduler instead of 10
-//            and the per-point scalar work (transform, voxel index, bounds) is issued once per 4 points;
-//   search   what the previous iteration learnt stays with the group: the 27 table lookups (lane g keeps neighbours g,
-//            g + 8, g + 16, g + 24; valid while the transformed point stays in its voxel: the map does not change during a
+//   groups   GLANES = 16 lanes per source point, two points per warp; points are dealt round-robin over the blocks of the
+//            grid (ONE block of GWARPS = 20 warps = 640 threads per SM, 40 points per block and round), so a 5,000-point
+//            scan is served in one round by 148 blocks and the per-point scalar work (transform, voxel index, bounds)
+//            is issued once per 2 points;
+//   search   what the previous iteration learnt stays with the group: the 27 table lookups (lane g keeps neighbours g and
+//            g + 16; valid while the transformed point stays in its voxel: the map does not change during a
 //            registration) and the previous nearest neighbour, whose distance to the new position bounds the search: a
 //            neighbour voxel is read only if its distance lower bound does not exceed it (exact, ties included).  From the
 //            second iteration on a search is usually one sweep over the point's own voxel, served by L1;
 //   A9       every group linearises its own correspondence at once -- no block barrier, no serial section: the six
 //            entries of Sigma_r + R Sigma_s R^T one per lane, M = S^-1, M d and the weight in every lane, and the 29
 //            terms of (H, b, chi2, n) as ONE uniform expression  coef (u[a] u[b] - u[c] u[d])  over a small vector u
-//            = (M, M d, p, 0, 1, e2, X) in shared memory with a constant index table (four terms per lane), so the
-//            lanes do not diverge;
-//   reduce   lane-wise across the 4 groups of a warp (shuffles), across the warps of the block (shared memory), then
+//            = (M, M d, p, 0, 1, e2, X) in shared memory with a constant index table (TERM_SLOTS = 3 term columns per
+//            lane: entries g, g + 16 < 24, then 24 + g), so the lanes do not diverge;
+//   reduce   lane-wise across the 2 groups of a warp (shuffles), across the warps of the block (shared memory), then
 //            block -> group of 16 blocks -> grid as TAGGED rows: every value travels as two 8-byte words {value half,
 //            tag} (tag = launch sequence and iteration), so a consumer just polls the rows it needs -- no fence, no
 //            ticket atomics -- and sums them in a fixed order (deterministic, no floating-point atomics);
@@ -673,7 +674,7 @@ __global__ void __launch_bounds__(GTHREADS, GICP_BLOCKS_PER_SM) gicp_kernel(cons
             if (gl < 8) acc[TERM_SLOTS - 1] += term(enc[TERM_SLOTS - 1], false);
             __syncwarp(gmask);                                      // u is rewritten by the group's next point
         }
-        // ---- A10: lane-wise over the warp's 4 groups, over the block's warps, then block row -> group of 16 blocks -> grid
+        // ---- A10: lane-wise over the warp's 32 / GLANES groups, over the block's warps, then block row -> group of 16 blocks -> grid
         // as tagged words; every level summed in a fixed order
 #pragma unroll
         for (int q = 0; q < TERM_SLOTS; ++q) {
