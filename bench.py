@@ -464,8 +464,8 @@ def _leg_c3(out, far, scenes, torch):
     # ---- C3: racing sequence, 200 frames at 10 Hz, three forward LiDARs, 250 km/h (6.94 m per frame), insert + prune 200 m
     # per frame.  The initial guess is the prior of the paper's loop: far_ekf_* driven by a synthetic 100 Hz
     # IMU and corrected by the registered poses and Eq. 7 velocities, exactly the loop tests/test_gpu_full_size.py compares
-    # with the oracle frame by frame.  (LiDAR-only constant-velocity dead reckoning leaves the basin of the registration in
-    # this corridor after ~25 frames on the oracle as on the GPU: DESIGN.md section 7.)
+    # with the oracle frame by frame.  (The literal constant-velocity guess is also well-posed here once the predicted rotation is kept
+    # orthonormal: tests/test_oracle_c3.py; the EKF prior is used because it is the paper's loop.)
     track = scenes.RaceTrack(seed=2)
     rng = np.random.default_rng(2)
     n_frames, v, cap, vel, dt, s0, G0 = int(os.environ.get("FAR_BENCH_C3_FRAMES", "200")), 1.0, 20, 69.4, 0.01, 300.0, 9.80665

@@ -86,3 +86,11 @@ def twist_matrix(delta):
 
 def rot_angle(R):
     return float(np.arccos(np.clip(0.5 * (np.trace(R) - 1.0), -1.0, 1.0)))
+
+
+def rot_sin(R):
+    """sin of the rotation angle of R from its antisymmetric part.  For the tiny angles parity is about (1e-5 rad and below)
+    this is the well-conditioned measure: arccos of the trace (rot_angle) turns a deviation eps of the trace -- e.g. a
+    non-orthonormality of 1e-10 that both chains of a sequence share -- into an angle of sqrt(2 eps)."""
+    w = np.array([R[2, 1] - R[1, 2], R[0, 2] - R[2, 0], R[1, 0] - R[0, 1]])
+    return float(0.5 * np.linalg.norm(w))

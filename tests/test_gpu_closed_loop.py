@@ -4,8 +4,9 @@ undistort -> voxelise -> Sigma_s -> GICP -> ASMD map update -> prune) returns th
 which arrive at the EKF two cycles late and are applied with delay compensation and up-sampling (Eq. 11).
 
 Synthetic stand-in for the racing data: the C3 race track at 250 km/h through the end of the straight
-and into the R = 500 m arc.  LiDAR-only constant-velocity dead reckoning diverges along-track in this corridor within
-~40 frames (no along-track structure); with the IMU-driven EKF the loop must stay on the track.
+and into the R = 500 m arc.  The corridor has little along-track structure; with the IMU-driven EKF the loop
+must stay on the track.  (An earlier version of this text said the constant-velocity guess diverges here: that was the
+unprojected pose composition, see tests/test_oracle_c3.py.)
 """
 import math
 

@@ -6,9 +6,9 @@ C2: the bench step itself (far.Frontend with bench.py's parameters, one whole fr
 C3: the whole 200-frame racing sequence (3 x 60k rays at 250 km/h, per-frame insert and 200 m prune) through
     far_frontend_process_host, every frame against the oracle on the same initial guess: the prior of the paper's loop
     (the EKF, driven by a synthetic IMU and corrected by the registered poses).  The literal
-    constant-velocity guess of BASELINE.json is LiDAR-only dead reckoning; in this corridor it leaves the basin of the
-    registration after ~25 frames ON BOTH SIDES (measured: DESIGN.md section 7), so it is parity-tested on the 14 frames at
-    the straight-to-arc transition where it is still well-posed.
+    constant-velocity guess of BASELINE.json is parity-tested on 14 frames at the straight-to-arc transition and on
+    frames 2-41 of the bench leg's sequence (tests/test_oracle_c3.py: it is well-posed once the predicted rotation is
+    kept orthonormal; the divergence reported in rounds 1-2 came from the unprojected composition).
 C4: 10 M points in 100 batches of 100k, whole map compared bit for bit, then the radius prune.
 C5: 20 M-point map, 1 M queries, ids and d2 bit-exact for every query at all four voxel sizes, plus brute force
     over ALL stored points on a sample (independent of the oracle's map structure).
@@ -21,7 +21,7 @@ import torch
 
 import far_scenes as scenes
 import oracle
-from helpers import np_nn_bruteforce, rot_angle
+from helpers import np_nn_bruteforce, rot_angle, rot_sin
 
 pytestmark = pytest.mark.gpu
 
@@ -43,12 +43,27 @@ def _cov_close(g, o, tol=1e-4):
     assert rel.max() < tol, rel.max()
 
 
-# Stored coordinates after an insert at a REGISTERED pose: the two sides' poses agree to ~1e-10 m (different summation
-# orders of the same FP64 terms, amplified by the chain of frames), and a coordinate is that pose applied to the point,
-# rounded to fp32 once.  Where the 1e-10 straddles a rounding boundary the stored values differ by one fp32 ulp -- 6.1e-5 m
-# at the 1 km coordinates of the race track -- so the bar is two ulps there, far inside north_star's pose tolerance
-# (1e-4 m + 1e-5 rad x 200 m range).  At a GIVEN pose the same insert is bit-exact (tests/test_gpu_map.py).
-XYZ_TOL_1KM = 1.3e-4
+# Stored coordinates after an insert at a REGISTERED pose.  A stored coordinate is the pose applied to the point in FP64,
+# rounded to fp32 once.  The two sides' poses agree to ~1e-10 ... 1e-8 m (different summation orders of the same FP64 terms,
+# amplified by the chain of frames), which moves the FP64 value by at most  |dt| + sin(angle) x range  -- the POSE SLACK, taken
+# from the very poses the test compares, frame by frame -- and the rounding then adds at most one fp32 ulp of the value
+# (neighbouring fp32 numbers where the slack straddles a rounding boundary).  So the bar is one ulp of the value plus the
+# measured pose slack, not a number of metres picked for the scene.  (At a GIVEN pose the same insert is bit-exact:
+# tests/test_gpu_map.py.)
+MAX_RANGE_M = 200.0
+
+
+def _pose_slack(g, o):
+    return float(np.linalg.norm(g["t"] - o["t"])) + rot_sin(g["R"].T @ o["R"]) * MAX_RANGE_M
+
+
+def _xyz_within_one_ulp_plus(g, o, slack):
+    assert slack < 1e-6, slack                                   # the poses themselves are far inside north_star's 1e-4 m
+    g, o = np.ascontiguousarray(g), np.ascontiguousarray(o)
+    d = np.abs(g.astype(np.float64) - o.astype(np.float64))
+    ulp = np.spacing(np.maximum(np.abs(g), np.abs(o))).astype(np.float64)
+    worst = (d - ulp).max()
+    assert worst <= slack, (float(worst), slack, float((d > 0).mean()))
 
 
 def _result(d_res):
@@ -113,18 +128,24 @@ def test_c2_full_frame_as_benched():
     eo1, eg1 = mo.export(with_cov=True), fe.map.export(with_cov=True)
     assert np.array_equal(eg1["keys"], eo1["keys"]) and np.array_equal(eg1["counts"], eo1["counts"])
     assert np.array_equal(eg1["ids"], eo1["ids"])
-    assert np.abs(eg1["xyz"] - eo1["xyz"]).max() < 3.1e-5        # two fp32 ulps at the scene's 150 m (see XYZ_TOL_1KM)
+    _xyz_within_one_ulp_plus(eg1["xyz"], eo1["xyz"], _pose_slack(g, o))
     assert np.array_equal(eg1["cov_valid"], eo1["cov_valid"])
     fe.close()
 
 
-def test_c3_racing_frames_chain_matches_oracle_frame_by_frame():
-    n_frames, v, cap, prune_r, max_range = 14, 1.0, 20, 200.0, 200.0
+@pytest.mark.parametrize("s0,n_frames", [(990.0, 14), (300.0, 42)])
+def test_c3_racing_frames_chain_matches_oracle_frame_by_frame(s0, n_frames):
+    """The literal constant-velocity guess of BASELINE.json configs[2], T_pred = T_{t-1} (T_{t-2}^-1 T_{t-1}) with the rotation
+    projected back onto SO(3) (tests/test_oracle_c3.py shows why: without the projection the composition loses orthonormality
+    geometrically and the sequence diverges after ~30 frames -- the "drift" rounds 1-2 attributed to the method).
+    s0 = 990: the end of the straight and the entry of the R = 500 m arc, iteration counts from 2 to 30.
+    s0 = 300: the start of the bench leg's sequence, frames 2-41.
+    Same status, iterations, inliers and pose on every frame, same map at the end."""
+    v, cap, prune_r, max_range = 1.0, 20, 200.0, 200.0
     track = scenes.RaceTrack(seed=2)
     rng = np.random.default_rng(2)
     step = 69.4 * 0.1                      # 250 km/h at 10 Hz
-    # the end of the straight and the entry of the R = 500 m arc: iteration counts vary from 2 to 30 here
-    frames = [scenes.c3_racing_frame(track, 990.0 + step * f, rng) for f in range(n_frames)]
+    frames = [scenes.c3_racing_frame(track, s0 + step * f, rng) for f in range(n_frames)]
     n_max = max(len(s) for s, _ in frames)
     fe = far.Frontend(v, cap, 1 << 19, n_max, ds_voxel=v, prune_radius=prune_r, max_iters=30)
     mo = oracle.Map(v, cap)
@@ -137,10 +158,14 @@ def test_c3_racing_frames_chain_matches_oracle_frame_by_frame():
         poses_o.append(T)
         poses_g.append(T)
 
-    def predict(P):   # T_pred = T_{t-1} (T_{t-2}^-1 T_{t-1})
-        return scenes.pose_compose(P[-1], scenes.pose_compose(scenes.pose_inverse(P[-2]), P[-1]))
+    def predict(P):   # T_pred = T_{t-1} (T_{t-2}^-1 T_{t-1}), projected back onto SO(3): the product of three matrices with a
+        # transpose for the inverse multiplies any deviation from orthonormality from frame to frame (1e-11 in the
+        # bootstrap poses had grown to 2e-8 by frame 22 of the long run), and a predicted pose is a rigid transform
+        R, t = scenes.pose_compose(P[-1], scenes.pose_compose(scenes.pose_inverse(P[-2]), P[-1]))
+        U, _, Vt = np.linalg.svd(R)
+        return U @ Vt, t
 
-    iters = []
+    iters, slack = [], 0.0
     for f in range(2, n_frames):
         scan, T_gt = frames[f]
         pred_o, pred_g = predict(poses_o), predict(poses_g)
@@ -154,7 +179,11 @@ def test_c3_racing_frames_chain_matches_oracle_frame_by_frame():
         g = fe.process_host(scan, pred_g, th_g.sigma())
         assert g["status"] == o["status"] == 0, f
         assert g["n_inliers"] == o["n_inliers"] and g["iters"] == o["iters"] and g["converged"] == o["converged"], f
-        assert np.linalg.norm(g["t"] - o["t"]) < 1e-4 and rot_angle(g["R"].T @ o["R"]) < 1e-5, f
+        # sin of the angle from the antisymmetric part (helpers.rot_sin): well-conditioned at 1e-5 rad and below
+        assert np.linalg.norm(g["t"] - o["t"]) < 1e-4 and rot_sin(g["R"].T @ o["R"]) < 1e-5, f
+        for R in (g["R"], o["R"]):
+            assert np.abs(R.T @ R - np.eye(3)).max() < 1e-9, f
+        slack = max(slack, _pose_slack(g, o))
         th_o.update(pred_o, (o["R"], o["t"]))
         th_g.update(pred_g, (g["R"], g["t"]))
         assert abs(th_o.sigma() - th_g.sigma()) < 1e-6
@@ -162,17 +191,22 @@ def test_c3_racing_frames_chain_matches_oracle_frame_by_frame():
         poses_g.append((g["R"], g["t"]))
         assert mo.size() == fe.map.size(), f
         iters.append(o["iters"])
-    assert min(iters) < 10 and max(iters) > 10          # both quick and long registrations were exercised
+    assert min(iters) < 10 and max(iters) > (10 if s0 == 990.0 else 7)     # both quick and long registrations were exercised
     eo, eg = mo.export(with_cov=True), fe.map.export(with_cov=True)
     assert np.array_equal(eg["keys"], eo["keys"]) and np.array_equal(eg["ids"], eo["ids"])
-    assert np.abs(eg["xyz"] - eo["xyz"]).max() < XYZ_TOL_1KM
+    _xyz_within_one_ulp_plus(eg["xyz"], eo["xyz"], slack)
     assert np.array_equal(eg["cov_valid"], eo["cov_valid"])
     # the corridor is degenerate along-track (expect it, report it, do not tune it away):
     # only lateral / vertical / heading errors are bounded
     R, t = poses_g[-1]
     Rg, tg = frames[-1][1]
-    lateral = (Rg.T @ (t - tg))[1:]
-    assert np.abs(lateral).max() < 0.1 and rot_angle(R.T @ Rg) < math.radians(0.5)
+    err = Rg.T @ (t - tg)
+    assert rot_angle(R.T @ Rg) < math.radians(0.5)
+    if s0 == 990.0:
+        assert np.abs(err[1:]).max() < 0.1
+    else:   # well-posed on the straight, as on the oracle (test_oracle_c3.py); height is held by the road surface only and
+        # wanders by a few decimetres over 40 frames on both sides alike
+        assert abs(err[0]) < 0.2 and abs(err[1]) < 0.1 and abs(err[2]) < 0.5 and th_g.sigma() < 0.3
     fe.close()
 
 
@@ -209,7 +243,7 @@ def test_c3_racing_sequence_200_frames_ekf_prior_matches_oracle_every_frame():
         ekf.predict(np.r_[0.0, vel * w, G0] + irng.normal(0, 0.05, 3), np.r_[0.0, 0.0, w] + irng.normal(0, 0.002, 3))
         cycle += 1
 
-    iters, err_g, err_o, dmax = [], [], [], 0.0
+    iters, err_g, err_o, dmax, slack = [], [], [], 0.0, 0.0
     for f in range(2, n_frames):
         scan, T_gt = frames[f]
         while cycle < 10 * f:
@@ -227,6 +261,7 @@ def test_c3_racing_sequence_200_frames_ekf_prior_matches_oracle_every_frame():
         assert g["n_inliers"] == o["n_inliers"] and g["iters"] == o["iters"] and g["converged"] == o["converged"], f
         assert np.linalg.norm(g["t"] - o["t"]) < 1e-4 and rot_angle(g["R"].T @ o["R"]) < 1e-5, f
         dmax = max(dmax, float(np.linalg.norm(g["t"] - o["t"])))
+        slack = max(slack, _pose_slack(g, o))
         th_g.update(pred, (g["R"], g["t"])); th_o.update(pred, (o["R"], o["t"]))
         assert abs(th_g.sigma() - th_o.sigma()) < 1e-6
         assert mo.size() == fe.map.size(), f
@@ -240,7 +275,7 @@ def test_c3_racing_sequence_200_frames_ekf_prior_matches_oracle_every_frame():
     eo, eg = mo.export(with_cov=True), fe.map.export(with_cov=True)
     assert np.array_equal(eg["keys"], eo["keys"]) and np.array_equal(eg["counts"], eo["counts"])
     assert np.array_equal(eg["ids"], eo["ids"])
-    assert np.abs(eg["xyz"] - eo["xyz"]).max() < XYZ_TOL_1KM
+    _xyz_within_one_ulp_plus(eg["xyz"], eo["xyz"], slack)
     assert np.array_equal(eg["cov_valid"], eo["cov_valid"])
     st = fe.map.stats()
     assert st["full"] == 0 and st["n_rehash"] > 0 and st["n_dead_keys"] < 64 + st["n_voxels"] // 4    # 2^16-bucket map, 198 prunes
